@@ -1,0 +1,154 @@
+/* arbb200.h - C ABI of libarbb200: B200-native (sm_100a) stepping of many multi-compartment cells.
+ *
+ * The library implements ONE thing: the data-parallel hot path of arXiv 1901.07454 ("Arbor"),
+ * /root/reference/PAPER.md section II (lines 92-158) and IV-C (lines 216-220): per time step
+ *   deliver spike events into synapses
+ *   mechanism currents from V(t)              (eq 2a at 127-131)
+ *   assemble the implicit-Euler cable matrix
+ *   solve it with the Hines / extended Thomas algorithm over the parent index
+ *   V <- V', integrate mechanism state with V'
+ *   threshold detection -> spikes
+ * and once per minimum-delay epoch turn spikes into events on the targets' queues
+ * (PAPER.md:96, 198-202).  Every step runs in hand-written CUDA kernels on the device; there is no
+ * CPU fallback.  All arithmetic is fp64, indices int32/int64, times fp64.
+ *
+ * Units (reading R2): V mV, t ms, area um^2, cm uF/cm^2, density conductance S/cm^2,
+ * point conductance uS, current nA, axial resistance MOhm.
+ *
+ * Pointer conventions: every pointer in arb_desc and every output buffer is a HOST pointer owned by
+ * the caller; arb_desc arrays are read only during arb_plan / arb_create and never retained.  The
+ * only DEVICE pointer is `dev_workspace`: one caller-owned allocation (the library never calls
+ * cudaMalloc) that must stay alive, and untouched by the caller, until arb_destroy.
+ *
+ * Errors: every call returns 0 (or a count) on success or a negative ARB_E_* code; nothing throws
+ * or aborts across the ABI; arb_last_error gives text.  One model per host thread at a time.
+ */
+#ifndef ARBB200_H
+#define ARBB200_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  ARB_OK = 0,
+  ARB_E_NULL = -1,      /* a required pointer is NULL                                            */
+  ARB_E_INVALID = -2,   /* description or argument out of range (see arb_plan)                   */
+  ARB_E_WORKSPACE = -3, /* device workspace smaller than arb_plan asked for, or misaligned       */
+  ARB_E_CUDA = -4,      /* a CUDA runtime call or kernel failed                                  */
+  ARB_E_OVERFLOW = -5,  /* spike / event buffer capacity exceeded; the model is unusable after   */
+  ARB_E_NOMEM = -6      /* host allocation failed                                                */
+};
+
+/* arb_probe selectors */
+enum { ARB_PROBE_M = 0, ARB_PROBE_H = 1, ARB_PROBE_N = 2, ARB_PROBE_SYN_G = 3, ARB_PROBE_TIME = 4,
+       ARB_PROBE_NSTEPS = 5, ARB_PROBE_STATS = 6 };
+
+/* arb_set_option keys */
+enum {
+  ARB_OPT_FUSED_STEPS = 1,   /* max grid steps integrated per kernel launch with the cell block's
+                                state kept on-chip: 1 = one launch per time step (state streams
+                                through HBM every step); 0 (default) = a whole min-delay epoch
+                                (cells are independent within Delta_T)           */
+  ARB_OPT_EPOCH_STEPS = 2    /* cap on the epoch length in steps (default: floor(min delay / dt)) */
+};
+
+/* The problem statement of PAPER.md section II as flat arrays.
+ * Cells are trees of control volumes (CVs).  Per-cell fields use CSR offsets
+ * over cells; CV and synapse indices inside a cell are cell-local. */
+typedef struct {
+  /* cells and compartments */
+  int64_t n_cells;
+  const int64_t* cv_off;    /* [n_cells+1], cv_off[0] = 0, every cell has >= 1 CV                 */
+  const int32_t* cv_parent; /* [n_cv] local parent, -1 for CV 0 (root), otherwise 0 <= parent < i */
+  const double* cv_area;    /* [n_cv] um^2  > 0   (S_i)                             */
+  const double* cv_cm;      /* [n_cv] uF/cm^2 > 0 (c_i = cm * area)                               */
+  const double* cv_raxial;  /* [n_cv] MOhm > 0, CV centre -> parent centre (1/sigma_ij); root ignored */
+  const double* cv_vinit;   /* [n_cv] mV, or NULL => -65                                          */
+  /* density mechanisms; all three hh arrays or none; a CV whose three hh
+   * parameters are 0 has no HH; pas_g == 0 => no passive channel on that CV                    */
+  const double *hh_gnabar, *hh_gkbar, *hh_gl; /* [n_cv] S/cm^2 or NULL                           */
+  double hh_ena, hh_ek, hh_el;                /* mV                                               */
+  const double *pas_g, *pas_e;                /* [n_cv] S/cm^2, mV; both or NULL                  */
+  /* exponential synapses (point mechanisms) */
+  const int64_t* syn_off;   /* [n_cells+1] or NULL when there are no synapses                    */
+  const int32_t* syn_cv;    /* [n_syn] local CV                                                  */
+  const double *syn_tau, *syn_e; /* [n_syn] ms (> 0), mV                                          */
+  /* current clamps: amplitude > 0 depolarises, active for t0 <= t < t1 (t = step start)          */
+  int64_t n_clamp;
+  const int64_t* clamp_cell;
+  const int32_t* clamp_cv;
+  const double *clamp_t0, *clamp_t1, *clamp_amp; /* ms, ms, nA                                    */
+  /* spike detectors, one per cell */
+  const int32_t* det_cv;    /* [n_cells] local CV, or NULL => CV 0                               */
+  double threshold;         /* mV                                                                */
+  /* network: (source, destination, synapse, delay, weight)                         */
+  int64_t n_conn;
+  const int64_t *conn_src, *conn_dst; /* cells                                                   */
+  const int32_t* conn_syn;            /* synapse index local to the destination cell             */
+  const double *conn_delay, *conn_weight; /* ms (> 0, and >= dt at arb_advance), uS               */
+  /* external events (kicks, pre-generated Poisson trains): g[syn] += weight at `time`            */
+  int64_t n_ext;
+  const int64_t* ext_cell;
+  const int32_t* ext_syn;
+  const double *ext_time, *ext_weight; /* ms (>= 0), uS                                           */
+} arb_desc;
+
+typedef struct arb_model arb_model; /* opaque; lives in host memory, owned by the library */
+
+/* Validate the description and report the device workspace size arb_create needs.  No device
+ * work, no allocation kept.  ARB_E_INVALID: parent >= index or < -1, non-positive area / cm /
+ * raxial / tau, CV / synapse / cell index out of range, delay <= 0, NaN / Inf, external event
+ * earlier than t = 0, inconsistent NULLs. */
+int arb_plan(const arb_desc* desc, size_t* workspace_bytes);
+
+/* Build the model: lay the cells out in blocks of interleaved branches, upload to
+ * `dev_workspace` (DEVICE pointer, 256-byte aligned, >= workspace_bytes from arb_plan) on
+ * `cuda_stream` (a cudaStream_t; NULL = default stream), initialise state (V = vinit, gates at
+ * steady state, g = 0, t = 0; reading R4).  Returns after the upload has completed. */
+int arb_create(const arb_desc* desc, void* dev_workspace, size_t workspace_bytes, void* cuda_stream,
+               arb_model** out);
+
+/* Integrate from the model's current time t to t_end on the grid t_k = t + k*dt; a final shorter
+ * step is taken when (t_end - t) is not a multiple of dt; grid steps are split at event times
+ * (reading R9).  Kernels are queued on the model's stream; the call returns after
+ * they have completed and the overflow flags have been checked.  ARB_E_INVALID: dt <= 0,
+ * t_end < t, dt longer than the shortest connection delay. */
+int arb_advance(arb_model* m, double t_end, double dt);
+
+/* Spikes since creation.  Returns the total count; fills min(cap, count) entries sorted by
+ * (time, cell).  cell / time may be NULL when cap == 0.  Negative on error. */
+int64_t arb_spikes(arb_model* m, int64_t* cell, double* time, int64_t cap);
+
+/* Membrane potential of every CV in the caller's CV order.  n_cv must equal cv_off[n_cells]. */
+int arb_voltage(arb_model* m, double* out, int64_t n_cv);
+
+/* ARB_PROBE_M/H/N: gate state per CV (0 where the CV has no HH), n = n_cv.
+ * ARB_PROBE_SYN_G: synaptic conductance per synapse in the caller's order, n = n_syn.
+ * ARB_PROBE_TIME:  out[0] = current time, n >= 1.
+ * ARB_PROBE_NSTEPS: out[0] = grid steps so far, out[1] = cell sub-steps so far (>= cells*grid
+ *                  steps; the excess comes from event-driven step splitting), n >= 2.
+ * ARB_PROBE_STATS: out[0..7] = {blocks, slots (padded CVs), branches, workspace bytes,
+ *                  events delivered, kernel launches so far, epoch steps, streamed bytes per
+ *                  cell-block step}, n >= 8. */
+int arb_probe(arb_model* m, int what, double* out, int64_t n);
+
+/* Overwrite state from host arrays in the caller's order (any pointer may be NULL = keep).
+ * Detector history is reset to the new voltages.  Exists so that tests can start both
+ * implementations from one state. */
+int arb_set_state(arb_model* m, const double* v, const double* hh_m, const double* hh_h,
+                  const double* hh_n, const double* syn_g);
+
+int arb_set_option(arb_model* m, int key, int64_t value);
+
+void arb_destroy(arb_model* m);
+
+/* Text of the last error of this model, or of the last arb_plan / arb_create failure on this
+ * thread when m == NULL.  Never NULL. */
+const char* arb_last_error(const arb_model* m);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -495,7 +495,7 @@ int orc_set_state(orc_model* M, const double* v, const double* hm, const double*
   if (hh) memcpy(M->h, hh, (size_t)M->n_cv * 8);
   if (hn) memcpy(M->nn, hn, (size_t)M->n_cv * 8);
   if (syn_g) memcpy(M->g, syn_g, (size_t)M->n_syn * 8);
-  for (int64_t c = 0; c < M->n_cells; ++c) M->cells[c].v_prev = M->v[M->cells[c].cv0 + M->cells[c].det];
+  for (int64_t c = 0; c < M->n_cells; ++c) { M->cells[c].v_prev = M->v[M->cells[c].cv0 + M->cells[c].det]; M->cells[c].armed = 1; }
   return 0;
 }
 

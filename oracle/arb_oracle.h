@@ -73,7 +73,8 @@ int orc_voltage(orc_model* m, double* out, int64_t n_cv);
 int orc_probe(orc_model* m, int what, double* out, int64_t n);
 /* membrane current I_i [nA] of every CV of one cell at the model's current state and time */
 int orc_cell_currents(orc_model* m, int64_t cell, double* i_out);
-/* overwrite the state (any pointer may be NULL): used to start both implementations from one state */
+/* overwrite the state (any pointer may be NULL) and reset the detector history (armed, v_prev):
+ * used by the parity tests to start both implementations from one state */
 int orc_set_state(orc_model* m, const double* v, const double* hm, const double* hh,
                   const double* hn, const double* syn_g);
 void orc_set_threads(int n);                                  /* OpenMP threads (timing only)  */

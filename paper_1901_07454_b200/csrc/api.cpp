@@ -1,0 +1,424 @@
+// api.cpp - the C ABI of include/arbb200.h: workspace carving, upload, the epoch loop, read-back.
+// Host logic only; every arithmetic step of the method runs in kernels.cu.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/arbb200.h"
+#include "kernels.cuh"
+#include "layout.hpp"
+
+using namespace arbb;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct Region { size_t off = 0, bytes = 0; };
+
+// Carves the caller's workspace.  The same walk gives arb_plan its size.
+struct Carver {
+  size_t pos = 0;
+  Region take(size_t bytes) {
+    Region r;
+    r.off = pos; r.bytes = bytes;
+    pos += (bytes + 255) / 256 * 256;
+    return r;
+  }
+};
+
+struct Regions {
+  Region blocks, gen, fast, state, meta, scratch, cell_rt, cell_orig, ev_off, ev_t, ev_gidx, ev_w, ev_fill,
+      ext_off, ext_t, ext_gidx, ext_w, ext_cur, conn_off, conn_dst, conn_gidx, conn_delay, conn_w,
+      pool_t[2], pool_dst[2], pool_gidx[2], pool_w[2], spike_cell, spike_t, counters, scan_tmp,
+      cv_idx, syn_idx, hh_m_idx, hh_stride, hh_cv, io;
+  size_t total = 0;
+};
+
+struct Caps { int64_t pool = 0, ev = 0, spikes = 0; };
+
+Caps capacities(const HostModel& H) {
+  Caps c;
+  c.pool = 4 * H.n_conn + 1024;
+  c.ev = c.pool + H.n_ext + 16;
+  c.spikes = std::max<int64_t>(1 << 20, 64 * H.n_cells);
+  return c;
+}
+
+Regions carve(const HostModel& H, const Caps& cap) {
+  Regions R;
+  Carver C;
+  const size_t nc = (size_t)H.n_cells;
+  R.blocks = C.take(sizeof(BlockInfo) * (size_t)H.n_blocks);
+  R.gen = C.take(8 * (size_t)H.gen_doubles);
+  R.fast = C.take(8 * (size_t)H.fast_doubles);
+  R.state = C.take(8 * (size_t)H.state_doubles);
+  R.meta = C.take((size_t)H.meta_bytes);
+  R.scratch = C.take(8 * (size_t)H.scratch_doubles);
+  R.cell_rt = C.take(sizeof(CellRt) * nc);
+  R.cell_orig = C.take(4 * nc);
+  R.ev_off = C.take(4 * (nc + 1));
+  R.ev_t = C.take(8 * (size_t)cap.ev);
+  R.ev_gidx = C.take(4 * (size_t)cap.ev);
+  R.ev_w = C.take(8 * (size_t)cap.ev);
+  R.ev_fill = C.take(4 * nc);
+  R.ext_off = C.take(4 * (nc + 1));
+  R.ext_t = C.take(8 * (size_t)H.n_ext);
+  R.ext_gidx = C.take(4 * (size_t)H.n_ext);
+  R.ext_w = C.take(8 * (size_t)H.n_ext);
+  R.ext_cur = C.take(4 * nc);
+  R.conn_off = C.take(4 * (nc + 1));
+  R.conn_dst = C.take(4 * (size_t)H.n_conn);
+  R.conn_gidx = C.take(4 * (size_t)H.n_conn);
+  R.conn_delay = C.take(8 * (size_t)H.n_conn);
+  R.conn_w = C.take(8 * (size_t)H.n_conn);
+  for (int i = 0; i < 2; ++i) {
+    R.pool_t[i] = C.take(8 * (size_t)cap.pool);
+    R.pool_dst[i] = C.take(4 * (size_t)cap.pool);
+    R.pool_gidx[i] = C.take(4 * (size_t)cap.pool);
+    R.pool_w[i] = C.take(8 * (size_t)cap.pool);
+  }
+  R.spike_cell = C.take(4 * (size_t)cap.spikes);
+  R.spike_t = C.take(8 * (size_t)cap.spikes);
+  R.counters = C.take(8 * CNT_COUNT);
+  R.scan_tmp = C.take(4 * ((nc + 1023) / 1024 + 1));
+  R.cv_idx = C.take(4 * (size_t)H.n_cv);
+  R.syn_idx = C.take(4 * (size_t)H.n_syn);
+  R.hh_m_idx = C.take(4 * (size_t)H.n_hh);
+  R.hh_stride = C.take(4 * (size_t)H.n_hh);
+  R.hh_cv = C.take(4 * (size_t)H.n_hh);
+  R.io = C.take(8 * (size_t)std::max<int64_t>(std::max(H.n_cv, H.n_syn), 16));
+  R.total = C.pos;
+  return R;
+}
+
+}  // namespace
+
+struct arb_model {
+  HostModel H;          // pools are released after upload; counts and maps stay
+  Regions R;
+  Caps cap;
+  DevModel D;
+  char* ws = nullptr;
+  cudaStream_t stream = nullptr;
+  double t = 0.0, factored_dt = 0.0;
+  int64_t grid_steps = 0, launches = 0;
+  int64_t opt_fused = 0, opt_epoch = 0, last_epoch_steps = 0;
+  int cur_pool = 0;
+  int dyn_smem = 0;
+  bool broken = false;
+  std::string err;
+};
+
+namespace {
+
+template <class T>
+T* at(arb_model* m, const Region& r) { return reinterpret_cast<T*>(m->ws + r.off); }
+
+int fail(arb_model* m, int code, const std::string& s) {
+  if (m) m->err = s; else g_create_error = s;
+  return code;
+}
+
+int cuda_fail(arb_model* m, cudaError_t e, const char* where) {
+  return fail(m, ARB_E_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+
+#define CU(m, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(m, e_, #call); } while (0)
+
+template <class T>
+cudaError_t upload(arb_model* m, const Region& r, const std::vector<T>& v) {
+  if (v.empty()) return cudaSuccess;
+  return cudaMemcpyAsync(m->ws + r.off, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, m->stream);
+}
+
+BuildParams default_params() { return BuildParams(); }
+
+}  // namespace
+
+extern "C" {
+
+int arb_plan(const arb_desc* desc, size_t* workspace_bytes) {
+  if (!desc || !workspace_bytes) return fail(nullptr, ARB_E_NULL, "arb_plan: NULL argument");
+  try {
+    HostModel H;
+    std::string err;
+    int rc = build(*desc, default_params(), false, H, err);
+    if (rc) return fail(nullptr, rc, err);
+    *workspace_bytes = carve(H, capacities(H)).total;
+    return ARB_OK;
+  } catch (const std::bad_alloc&) {
+    return fail(nullptr, ARB_E_NOMEM, "arb_plan: out of host memory");
+  }
+}
+
+int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cuda_stream, arb_model** out) {
+  if (!desc || !dev_workspace || !out) return fail(nullptr, ARB_E_NULL, "arb_create: NULL argument");
+  *out = nullptr;
+  arb_model* m = nullptr;
+  try {
+    m = new arb_model();
+    std::string err;
+    int rc = build(*desc, default_params(), true, m->H, err);
+    if (rc) { delete m; return fail(nullptr, rc, err); }
+    HostModel& H = m->H;
+    m->cap = capacities(H);
+    m->R = carve(H, m->cap);
+    if (bytes < m->R.total) { delete m; return fail(nullptr, ARB_E_WORKSPACE, "arb_create: workspace smaller than arb_plan reported"); }
+    if (reinterpret_cast<uintptr_t>(dev_workspace) % 256) { delete m; return fail(nullptr, ARB_E_WORKSPACE, "arb_create: workspace must be 256-byte aligned"); }
+    m->ws = static_cast<char*>(dev_workspace);
+    m->stream = static_cast<cudaStream_t>(cuda_stream);
+    // shared-memory plan of the cable kernel: branches that do not fit use the global scratch
+    m->dyn_smem = std::min(cable_smem_bytes(H.max_block_lanes), cable_smem_limit());
+    for (auto& b : H.blocks)
+      if (cable_smem_bytes(b.n_lane) > m->dyn_smem) b.flags |= 1u;
+    auto bail = [&](cudaError_t e, const char* w) { std::string s = std::string(w) + ": " + cudaGetErrorString(e); delete m; return fail(nullptr, ARB_E_CUDA, s); };
+    cudaError_t e;
+    const Regions& R = m->R;
+    if ((e = cudaMemsetAsync(m->ws, 0, m->R.total, m->stream)) != cudaSuccess) return bail(e, "cudaMemsetAsync");
+    if ((e = upload(m, R.blocks, H.blocks)) != cudaSuccess) return bail(e, "upload blocks");
+    if ((e = upload(m, R.gen, H.gen)) != cudaSuccess) return bail(e, "upload gen");
+    if ((e = upload(m, R.fast, H.fast)) != cudaSuccess) return bail(e, "upload fast");
+    if ((e = upload(m, R.state, H.state)) != cudaSuccess) return bail(e, "upload state");
+    if ((e = upload(m, R.meta, H.meta)) != cudaSuccess) return bail(e, "upload meta");
+    if ((e = upload(m, R.cell_orig, H.cell_order)) != cudaSuccess) return bail(e, "upload cell order");
+    if ((e = upload(m, R.ext_off, H.ext_off)) != cudaSuccess) return bail(e, "upload ext_off");
+    if ((e = upload(m, R.ext_t, H.ext_t)) != cudaSuccess) return bail(e, "upload ext_t");
+    if ((e = upload(m, R.ext_gidx, H.ext_gidx)) != cudaSuccess) return bail(e, "upload ext_gidx");
+    if ((e = upload(m, R.ext_w, H.ext_w)) != cudaSuccess) return bail(e, "upload ext_w");
+    {
+      std::vector<uint32_t> cur(H.ext_off.begin(), H.ext_off.end() - 1);
+      if ((e = upload(m, R.ext_cur, cur)) != cudaSuccess) return bail(e, "upload ext_cur");
+      if ((e = cudaStreamSynchronize(m->stream)) != cudaSuccess) return bail(e, "sync");
+    }
+    if ((e = upload(m, R.conn_off, H.conn_off)) != cudaSuccess) return bail(e, "upload conn_off");
+    if ((e = upload(m, R.conn_dst, H.conn_dst)) != cudaSuccess) return bail(e, "upload conn_dst");
+    if ((e = upload(m, R.conn_gidx, H.conn_gidx)) != cudaSuccess) return bail(e, "upload conn_gidx");
+    if ((e = upload(m, R.conn_delay, H.conn_delay)) != cudaSuccess) return bail(e, "upload conn_delay");
+    if ((e = upload(m, R.conn_w, H.conn_w)) != cudaSuccess) return bail(e, "upload conn_w");
+    if ((e = upload(m, R.cv_idx, H.cv_state_idx)) != cudaSuccess) return bail(e, "upload cv map");
+    if ((e = upload(m, R.syn_idx, H.syn_state_idx)) != cudaSuccess) return bail(e, "upload syn map");
+    if ((e = upload(m, R.hh_m_idx, H.hh_m_idx)) != cudaSuccess) return bail(e, "upload hh map");
+    if ((e = upload(m, R.hh_stride, H.hh_stride)) != cudaSuccess) return bail(e, "upload hh map");
+    if ((e = upload(m, R.hh_cv, H.hh_cv)) != cudaSuccess) return bail(e, "upload hh map");
+    DevModel& D = m->D;
+    D.blocks = at<BlockInfo>(m, R.blocks);
+    D.n_blocks = H.n_blocks; D.n_cells = H.n_cells;
+    D.gen = at<double>(m, R.gen); D.fast = at<double>(m, R.fast); D.state = at<double>(m, R.state);
+    D.meta = at<uint8_t>(m, R.meta); D.scratch = at<double>(m, R.scratch);
+    D.cell_rt = at<CellRt>(m, R.cell_rt); D.cell_orig = at<uint32_t>(m, R.cell_orig);
+    D.ev_off = at<uint32_t>(m, R.ev_off); D.ev_t = at<double>(m, R.ev_t); D.ev_gidx = at<uint32_t>(m, R.ev_gidx);
+    D.ev_w = at<double>(m, R.ev_w); D.ev_fill = at<uint32_t>(m, R.ev_fill); D.ev_cap = m->cap.ev;
+    D.ext_off = at<uint32_t>(m, R.ext_off); D.ext_t = at<double>(m, R.ext_t); D.ext_gidx = at<uint32_t>(m, R.ext_gidx);
+    D.ext_w = at<double>(m, R.ext_w); D.ext_cur = at<uint32_t>(m, R.ext_cur);
+    D.conn_off = at<uint32_t>(m, R.conn_off); D.conn_dst = at<uint32_t>(m, R.conn_dst); D.conn_gidx = at<uint32_t>(m, R.conn_gidx);
+    D.conn_delay = at<double>(m, R.conn_delay); D.conn_w = at<double>(m, R.conn_w);
+    for (int i = 0; i < 2; ++i) {
+      D.pool[i].t = at<double>(m, R.pool_t[i]); D.pool[i].dst = at<uint32_t>(m, R.pool_dst[i]);
+      D.pool[i].gidx = at<uint32_t>(m, R.pool_gidx[i]); D.pool[i].w = at<double>(m, R.pool_w[i]);
+    }
+    D.pool_cap = m->cap.pool;
+    D.spike_cell = at<uint32_t>(m, R.spike_cell); D.spike_t = at<double>(m, R.spike_t); D.spike_cap = m->cap.spikes;
+    D.counters = at<unsigned long long>(m, R.counters);
+    D.scan_tmp = at<uint32_t>(m, R.scan_tmp);
+    D.ena = H.ena; D.ek = H.ek; D.el = H.el; D.theta = H.threshold;
+    if ((e = launch_init(D, m->stream)) != cudaSuccess) return bail(e, "init kernel");
+    if ((e = cudaStreamSynchronize(m->stream)) != cudaSuccess) return bail(e, "cudaStreamSynchronize");
+    // host pools are no longer needed
+    std::vector<double>().swap(H.gen); std::vector<double>().swap(H.fast); std::vector<double>().swap(H.state);
+    std::vector<uint8_t>().swap(H.meta);
+    std::vector<uint32_t>().swap(H.cv_state_idx); std::vector<uint32_t>().swap(H.syn_state_idx);
+    std::vector<uint32_t>().swap(H.hh_m_idx); std::vector<uint32_t>().swap(H.hh_stride); std::vector<uint32_t>().swap(H.hh_cv);
+    std::vector<uint32_t>().swap(H.conn_off); std::vector<uint32_t>().swap(H.conn_dst); std::vector<uint32_t>().swap(H.conn_gidx);
+    std::vector<double>().swap(H.conn_delay); std::vector<double>().swap(H.conn_w);
+    std::vector<uint32_t>().swap(H.ext_off); std::vector<uint32_t>().swap(H.ext_gidx);
+    std::vector<double>().swap(H.ext_t); std::vector<double>().swap(H.ext_w);
+    *out = m;
+    return ARB_OK;
+  } catch (const std::bad_alloc&) {
+    delete m;
+    return fail(nullptr, ARB_E_NOMEM, "arb_create: out of host memory");
+  }
+}
+
+int arb_advance(arb_model* m, double t_end, double dt) {
+  if (!m) return fail(nullptr, ARB_E_NULL, "arb_advance: NULL model");
+  if (m->broken) return fail(m, ARB_E_OVERFLOW, "model unusable after an earlier overflow / CUDA error");
+  if (!(dt > 0) || !std::isfinite(dt) || !std::isfinite(t_end)) return fail(m, ARB_E_INVALID, "arb_advance: dt must be > 0 and finite");
+  if (t_end < m->t) return fail(m, ARB_E_INVALID, "arb_advance: t_end earlier than the current time");
+  if (m->H.n_conn > 0 && m->H.min_delay < dt) return fail(m, ARB_E_INVALID, "arb_advance: dt longer than the shortest connection delay");
+  if (t_end == m->t) return ARB_OK;
+  const DevModel& D = m->D;
+  if (dt != m->factored_dt) {
+    CU(m, launch_factor(D, dt, m->stream));
+    m->factored_dt = dt;
+    m->launches++;
+  }
+  // time grid (reading R9): t_k = t0 + k*dt by multiplication, last point = t_end
+  const double t0 = m->t;
+  int64_t nsteps = (int64_t)std::ceil((t_end - t0) / dt - 1e-9);
+  if (nsteps < 1) nsteps = 1;
+  const int last_full = std::fabs((t0 + (double)nsteps * dt) - t_end) <= 1e-9 * dt;
+  // epoch: cells are independent for one minimum delay (reading R12)
+  int64_t epoch = 1024;
+  if (m->H.n_conn > 0) epoch = std::min<int64_t>(epoch, std::max<int64_t>(1, (int64_t)std::floor(m->H.min_delay / dt - 1e-6)));
+  if (m->opt_epoch > 0) epoch = std::min(epoch, m->opt_epoch);
+  const int64_t fused = m->opt_fused > 0 ? std::min(m->opt_fused, epoch) : epoch;
+  m->last_epoch_steps = epoch;
+  int launches = 0;
+  for (int64_t k = 0; k < nsteps;) {
+    const int64_t n_ep = std::min(epoch, nsteps - k);
+    const double t_win = (k + n_ep == nsteps) ? t_end : t0 + (double)(k + n_ep) * dt;
+    CU(m, launch_build_events(D, m->cur_pool, t_win, m->stream, &launches));
+    m->cur_pool ^= 1;
+    for (int64_t j = 0; j < n_ep; j += fused) {
+      StepArgs A;
+      A.t0 = t0; A.dt = dt; A.t_end = t_end; A.k_first = k + j; A.nk = std::min(fused, n_ep - j); A.nsteps = nsteps; A.last_full = last_full;
+      CU(m, launch_cable(D, A, m->dyn_smem, m->stream));
+      ++launches;
+    }
+    if (m->H.n_conn > 0) CU(m, launch_spikes_to_events(D, m->cur_pool, m->stream, &launches));
+    k += n_ep;
+  }
+  m->launches += launches;
+  unsigned long long cnt[CNT_COUNT];
+  CU(m, cudaMemcpyAsync(cnt, D.counters, sizeof cnt, cudaMemcpyDeviceToHost, m->stream));
+  cudaError_t e = cudaStreamSynchronize(m->stream);
+  if (e != cudaSuccess) { m->broken = true; return cuda_fail(m, e, "arb_advance"); }
+  m->t = t_end;
+  m->grid_steps += nsteps;
+  if (cnt[CNT_ERROR]) {
+    m->broken = true;
+    char buf[160];
+    snprintf(buf, sizeof buf, "capacity exceeded:%s%s%s", (cnt[CNT_ERROR] & 1) ? " spike buffer" : "",
+             (cnt[CNT_ERROR] & 2) ? " event pool" : "", (cnt[CNT_ERROR] & 4) ? " epoch event list" : "");
+    return fail(m, ARB_E_OVERFLOW, buf);
+  }
+  return ARB_OK;
+}
+
+int64_t arb_spikes(arb_model* m, int64_t* cell, double* time, int64_t cap) {
+  if (!m) return fail(nullptr, ARB_E_NULL, "arb_spikes: NULL model");
+  if (cap > 0 && (!cell || !time)) return fail(m, ARB_E_NULL, "arb_spikes: NULL output");
+  unsigned long long n = 0;
+  CU(m, cudaMemcpyAsync(&n, m->D.counters + CNT_SPIKES, 8, cudaMemcpyDeviceToHost, m->stream));
+  CU(m, cudaStreamSynchronize(m->stream));
+  int64_t count = (int64_t)std::min<unsigned long long>(n, (unsigned long long)m->cap.spikes);
+  if (cap <= 0 || count == 0) return count;
+  try {
+    std::vector<uint32_t> c(count);
+    std::vector<double> t(count);
+    CU(m, cudaMemcpyAsync(c.data(), m->D.spike_cell, 4 * (size_t)count, cudaMemcpyDeviceToHost, m->stream));
+    CU(m, cudaMemcpyAsync(t.data(), m->D.spike_t, 8 * (size_t)count, cudaMemcpyDeviceToHost, m->stream));
+    CU(m, cudaStreamSynchronize(m->stream));
+    std::vector<int64_t> idx(count);
+    for (int64_t i = 0; i < count; ++i) idx[i] = i;
+    std::sort(idx.begin(), idx.end(), [&](int64_t a, int64_t b) { return t[a] != t[b] ? t[a] < t[b] : c[a] < c[b]; });
+    for (int64_t i = 0; i < std::min(cap, count); ++i) { cell[i] = c[idx[i]]; time[i] = t[idx[i]]; }
+  } catch (const std::bad_alloc&) {
+    return fail(m, ARB_E_NOMEM, "arb_spikes: out of host memory");
+  }
+  return count;
+}
+
+int arb_voltage(arb_model* m, double* out, int64_t n_cv) {
+  if (!m || !out) return fail(m, ARB_E_NULL, "arb_voltage: NULL argument");
+  if (n_cv != m->H.n_cv) return fail(m, ARB_E_INVALID, "arb_voltage: n_cv mismatch");
+  double* io = at<double>(m, m->R.io);
+  CU(m, launch_gather(m->D.state, at<uint32_t>(m, m->R.cv_idx), n_cv, io, m->stream));
+  CU(m, cudaMemcpyAsync(out, io, 8 * (size_t)n_cv, cudaMemcpyDeviceToHost, m->stream));
+  CU(m, cudaStreamSynchronize(m->stream));
+  return ARB_OK;
+}
+
+int arb_probe(arb_model* m, int what, double* out, int64_t n) {
+  if (!m || !out) return fail(m, ARB_E_NULL, "arb_probe: NULL argument");
+  double* io = at<double>(m, m->R.io);
+  switch (what) {
+    case ARB_PROBE_M: case ARB_PROBE_H: case ARB_PROBE_N: {
+      if (n != m->H.n_cv) return fail(m, ARB_E_INVALID, "arb_probe: size mismatch");
+      CU(m, cudaMemsetAsync(io, 0, 8 * (size_t)n, m->stream));
+      CU(m, launch_gather_hh(m->D.state, at<uint32_t>(m, m->R.hh_m_idx), at<uint32_t>(m, m->R.hh_stride),
+                             at<uint32_t>(m, m->R.hh_cv), what - ARB_PROBE_M, m->H.n_hh, io, m->stream));
+      CU(m, cudaMemcpyAsync(out, io, 8 * (size_t)n, cudaMemcpyDeviceToHost, m->stream));
+      CU(m, cudaStreamSynchronize(m->stream));
+      return ARB_OK;
+    }
+    case ARB_PROBE_SYN_G: {
+      if (n != m->H.n_syn) return fail(m, ARB_E_INVALID, "arb_probe: size mismatch");
+      if (n == 0) return ARB_OK;
+      CU(m, launch_gather(m->D.state, at<uint32_t>(m, m->R.syn_idx), n, io, m->stream));
+      CU(m, cudaMemcpyAsync(out, io, 8 * (size_t)n, cudaMemcpyDeviceToHost, m->stream));
+      CU(m, cudaStreamSynchronize(m->stream));
+      return ARB_OK;
+    }
+    case ARB_PROBE_TIME:
+      if (n < 1) return fail(m, ARB_E_INVALID, "arb_probe: size mismatch");
+      out[0] = m->t;
+      return ARB_OK;
+    case ARB_PROBE_NSTEPS: case ARB_PROBE_STATS: {
+      if (n < (what == ARB_PROBE_NSTEPS ? 2 : 8)) return fail(m, ARB_E_INVALID, "arb_probe: size mismatch");
+      unsigned long long cnt[CNT_COUNT];
+      CU(m, cudaMemcpyAsync(cnt, m->D.counters, sizeof cnt, cudaMemcpyDeviceToHost, m->stream));
+      CU(m, cudaStreamSynchronize(m->stream));
+      if (what == ARB_PROBE_NSTEPS) { out[0] = (double)m->grid_steps; out[1] = (double)cnt[CNT_SUBSTEPS]; return ARB_OK; }
+      int64_t slots = 0;
+      for (const auto& b : m->H.blocks) slots += b.n_slot;
+      out[0] = (double)m->H.n_blocks; out[1] = (double)slots; out[2] = (double)m->H.n_lanes;
+      out[3] = (double)m->R.total; out[4] = (double)cnt[CNT_DELIVERED]; out[5] = (double)m->launches;
+      out[6] = (double)m->last_epoch_steps; out[7] = 0.0;
+      return ARB_OK;
+    }
+  }
+  return fail(m, ARB_E_INVALID, "arb_probe: unknown selector");
+}
+
+int arb_set_state(arb_model* m, const double* v, const double* hh_m, const double* hh_h, const double* hh_n, const double* syn_g) {
+  if (!m) return fail(nullptr, ARB_E_NULL, "arb_set_state: NULL model");
+  double* io = at<double>(m, m->R.io);
+  if (v) {
+    CU(m, cudaMemcpyAsync(io, v, 8 * (size_t)m->H.n_cv, cudaMemcpyHostToDevice, m->stream));
+    CU(m, launch_scatter(m->D.state, at<uint32_t>(m, m->R.cv_idx), m->H.n_cv, io, m->stream));
+    CU(m, cudaStreamSynchronize(m->stream));
+  }
+  const double* gates[3] = {hh_m, hh_h, hh_n};
+  for (int w = 0; w < 3; ++w)
+    if (gates[w]) {
+      CU(m, cudaMemcpyAsync(io, gates[w], 8 * (size_t)m->H.n_cv, cudaMemcpyHostToDevice, m->stream));
+      CU(m, launch_scatter_hh(m->D.state, at<uint32_t>(m, m->R.hh_m_idx), at<uint32_t>(m, m->R.hh_stride),
+                              at<uint32_t>(m, m->R.hh_cv), w, m->H.n_hh, io, m->stream));
+      CU(m, cudaStreamSynchronize(m->stream));
+    }
+  if (syn_g && m->H.n_syn > 0) {
+    CU(m, cudaMemcpyAsync(io, syn_g, 8 * (size_t)m->H.n_syn, cudaMemcpyHostToDevice, m->stream));
+    CU(m, launch_scatter(m->D.state, at<uint32_t>(m, m->R.syn_idx), m->H.n_syn, io, m->stream));
+    CU(m, cudaStreamSynchronize(m->stream));
+  }
+  CU(m, launch_reset_detectors(m->D, m->stream));
+  CU(m, cudaStreamSynchronize(m->stream));
+  return ARB_OK;
+}
+
+int arb_set_option(arb_model* m, int key, int64_t value) {
+  if (!m) return fail(nullptr, ARB_E_NULL, "arb_set_option: NULL model");
+  if (value < 0) return fail(m, ARB_E_INVALID, "arb_set_option: negative value");
+  switch (key) {
+    case ARB_OPT_FUSED_STEPS: m->opt_fused = value; return ARB_OK;
+    case ARB_OPT_EPOCH_STEPS: m->opt_epoch = value; return ARB_OK;
+  }
+  return fail(m, ARB_E_INVALID, "arb_set_option: unknown key");
+}
+
+void arb_destroy(arb_model* m) {
+  if (!m) return;
+  if (m->ws) cudaStreamSynchronize(m->stream);
+  delete m;
+}
+
+const char* arb_last_error(const arb_model* m) { return m ? m->err.c_str() : g_create_error.c_str(); }
+
+}  // extern "C"

@@ -1,0 +1,76 @@
+// kernels.cuh - device-side model view and kernel launchers (implemented in kernels.cu).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "block_layout.h"
+
+namespace arbb {
+
+enum Counter {
+  CNT_SPIKES = 0,       // spikes recorded since creation
+  CNT_SPIKES_DONE = 1,  // spikes already turned into events
+  CNT_POOL = 2,         // events waiting in the current pool
+  CNT_POOL_NEXT = 3,    // events carried over into the other pool
+  CNT_ERROR = 4,        // bit 0 spike overflow, bit 1 pool overflow, bit 2 epoch list overflow
+  CNT_SUBSTEPS = 5,     // cell sub-steps executed
+  CNT_DELIVERED = 6,    // events delivered
+  CNT_EVLIST = 7,       // size of the current epoch list
+  CNT_COUNT = 8
+};
+
+struct EventPool { double* t; uint32_t* dst; uint32_t* gidx; double* w; };
+
+struct DevModel {
+  const BlockInfo* blocks;
+  int64_t n_blocks, n_cells;
+  double* gen;
+  double* fast;
+  double* state;
+  const uint8_t* meta;
+  double* scratch;
+  CellRt* cell_rt;            // [n_cells] internal order
+  const uint32_t* cell_orig;  // internal -> caller's cell id
+  // epoch event list (CSR over internal cells)
+  uint32_t* ev_off;           // [n_cells + 1]
+  double* ev_t; uint32_t* ev_gidx; double* ev_w;
+  uint32_t* ev_fill;          // [n_cells] fill cursors / counts
+  int64_t ev_cap;
+  // external events (CSR over internal cells, time sorted) and their cursors
+  const uint32_t* ext_off; const double* ext_t; const uint32_t* ext_gidx; const double* ext_w;
+  uint32_t* ext_cur;
+  // network grouped by caller's source cell
+  const uint32_t* conn_off; const uint32_t* conn_dst; const uint32_t* conn_gidx;
+  const double* conn_delay; const double* conn_w;
+  EventPool pool[2];
+  int64_t pool_cap;
+  // spikes
+  uint32_t* spike_cell; double* spike_t; int64_t spike_cap;
+  unsigned long long* counters;
+  uint32_t* scan_tmp;         // block sums for the offsets scan
+  double ena, ek, el, theta;
+};
+
+struct StepArgs {
+  double t0, dt, t_end;  // grid t_k = t0 + k*dt, t_nsteps = t_end
+  int64_t k_first, nk, nsteps;
+  int last_full;         // the last grid step has nominal length dt
+};
+
+// all launchers queue work on `s` and return the last CUDA error code
+cudaError_t launch_factor(const DevModel& M, double dt, cudaStream_t s);
+cudaError_t launch_init(const DevModel& M, cudaStream_t s);
+cudaError_t launch_cable(const DevModel& M, const StepArgs& A, int dyn_smem, cudaStream_t s);
+cudaError_t launch_build_events(const DevModel& M, int cur_pool, double t_window_end, cudaStream_t s, int* launches);
+cudaError_t launch_spikes_to_events(const DevModel& M, int cur_pool, cudaStream_t s, int* launches);
+cudaError_t launch_gather(const double* state, const uint32_t* idx, int64_t n, double* out, cudaStream_t s);
+cudaError_t launch_scatter(double* state, const uint32_t* idx, int64_t n, const double* in, cudaStream_t s);
+cudaError_t launch_gather_hh(const double* state, const uint32_t* m_idx, const uint32_t* stride, const uint32_t* cv,
+                             int which, int64_t n_hh, double* out, cudaStream_t s);
+cudaError_t launch_scatter_hh(double* state, const uint32_t* m_idx, const uint32_t* stride, const uint32_t* cv,
+                              int which, int64_t n_hh, const double* in, cudaStream_t s);
+cudaError_t launch_reset_detectors(const DevModel& M, cudaStream_t s);
+int cable_smem_bytes(uint32_t max_block_lanes);
+int cable_smem_limit();
+
+}  // namespace arbb

@@ -384,7 +384,7 @@ def random_model(seed, n_cells=5, max_cv=40, kinds=("random", "chain", "star", "
     hh[off[:-1]] |= rng.random(n_cells) < 0.8
     pas = (~hh) & (rng.random(n_cv) < p_pas)
     nsyn = rng.integers(0, max_syn + 1, n_cells)
-    if n_cells > 1:
+    if n_cells > 1 and max_syn > 0:
         nsyn = np.maximum(nsyn, 1)
     syn_off = np.concatenate([[0], np.cumsum(nsyn)])
     syn_cv = np.concatenate([rng.integers(0, off[c + 1] - off[c], nsyn[c]) for c in range(n_cells)]
