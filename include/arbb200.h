@@ -43,7 +43,7 @@ enum {
 
 /* arb_probe selectors */
 enum { ARB_PROBE_M = 0, ARB_PROBE_H = 1, ARB_PROBE_N = 2, ARB_PROBE_SYN_G = 3, ARB_PROBE_TIME = 4,
-       ARB_PROBE_NSTEPS = 5, ARB_PROBE_STATS = 6 };
+       ARB_PROBE_NSTEPS = 5, ARB_PROBE_STATS = 6, ARB_PROBE_TIMING = 7 };
 
 /* arb_set_option keys */
 enum {
@@ -51,7 +51,10 @@ enum {
                                 state kept on-chip: 1 = one launch per time step (state streams
                                 through HBM every step); 0 (default) = a whole min-delay epoch
                                 (cells are independent within Delta_T)           */
-  ARB_OPT_EPOCH_STEPS = 2    /* cap on the epoch length in steps (default: floor(min delay / dt)) */
+  ARB_OPT_EPOCH_STEPS = 2,   /* cap on the epoch length in steps (default: floor(min delay / dt)) */
+  ARB_OPT_TIMING = 3         /* 1: bracket the cable-step launches and the epoch-boundary kernels of
+                                every epoch with CUDA events on the model's stream (read them with
+                                ARB_PROBE_TIMING); setting the option clears the accumulated times  */
 };
 
 /* The problem statement of PAPER.md section II as flat arrays.
@@ -131,7 +134,10 @@ int arb_voltage(arb_model* m, double* out, int64_t n_cv);
  *                  steps; the excess comes from event-driven step splitting), n >= 2.
  * ARB_PROBE_STATS: out[0..7] = {blocks, slots (padded CVs), branches, workspace bytes,
  *                  events delivered, kernel launches so far, epoch steps, streamed bytes per
- *                  cell-block step}, n >= 8. */
+ *                  cell-block step}, n >= 8.
+ * ARB_PROBE_TIMING: out[0..3] = {ms spent in cable-step kernels, cable-step launches timed,
+ *                  ms spent in epoch-boundary (spike -> event) kernels, their launches}, measured
+ *                  with CUDA events while ARB_OPT_TIMING is on, n >= 4. */
 int arb_probe(arb_model* m, int what, double* out, int64_t n);
 
 /* Overwrite state from host arrays in the caller's order (any pointer may be NULL = keep).

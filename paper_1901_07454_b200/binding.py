@@ -12,8 +12,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libarbb200.so")
 
 ARB_OK, ARB_E_NULL, ARB_E_INVALID, ARB_E_WORKSPACE, ARB_E_CUDA, ARB_E_OVERFLOW, ARB_E_NOMEM = 0, -1, -2, -3, -4, -5, -6
-ARB_PROBE_M, ARB_PROBE_H, ARB_PROBE_N, ARB_PROBE_SYN_G, ARB_PROBE_TIME, ARB_PROBE_NSTEPS, ARB_PROBE_STATS = range(7)
-ARB_OPT_FUSED_STEPS, ARB_OPT_EPOCH_STEPS = 1, 2
+ARB_PROBE_M, ARB_PROBE_H, ARB_PROBE_N, ARB_PROBE_SYN_G, ARB_PROBE_TIME, ARB_PROBE_NSTEPS, ARB_PROBE_STATS, ARB_PROBE_TIMING = range(8)
+ARB_OPT_FUSED_STEPS, ARB_OPT_EPOCH_STEPS, ARB_OPT_TIMING = 1, 2, 3
 
 EXPORTS = ("arb_plan", "arb_create", "arb_advance", "arb_spikes", "arb_voltage", "arb_probe",
            "arb_set_state", "arb_set_option", "arb_destroy", "arb_last_error")
@@ -140,7 +140,8 @@ class Model:
         return out
 
     def probe(self, what):
-        n = {ARB_PROBE_SYN_G: self.n_syn, ARB_PROBE_TIME: 1, ARB_PROBE_NSTEPS: 2, ARB_PROBE_STATS: 8}.get(what, self.n_cv)
+        n = {ARB_PROBE_SYN_G: self.n_syn, ARB_PROBE_TIME: 1, ARB_PROBE_NSTEPS: 2, ARB_PROBE_STATS: 8,
+             ARB_PROBE_TIMING: 4}.get(what, self.n_cv)
         out = np.empty(n)
         self._check(lib().arb_probe(self._h, what, _ptr(out), n))
         return out
@@ -158,6 +159,10 @@ class Model:
         s = self.probe(ARB_PROBE_STATS)
         return dict(blocks=int(s[0]), slots=int(s[1]), branches=int(s[2]), workspace_bytes=int(s[3]),
                     events_delivered=int(s[4]), launches=int(s[5]), epoch_steps=int(s[6]))
+
+    def timing(self):
+        t = self.probe(ARB_PROBE_TIMING)
+        return dict(cable_ms=float(t[0]), cable_launches=int(t[1]), event_ms=float(t[2]), event_launches=int(t[3]))
 
     def spikes(self):
         n = self._check(lib().arb_spikes(self._h, None, None, 0))

@@ -107,7 +107,10 @@ struct arb_model {
   cudaStream_t stream = nullptr;
   double t = 0.0, factored_dt = 0.0;
   int64_t grid_steps = 0, launches = 0;
-  int64_t opt_fused = 0, opt_epoch = 0, last_epoch_steps = 0;
+  int64_t opt_fused = 0, opt_epoch = 0, opt_timing = 0, last_epoch_steps = 0;
+  std::vector<cudaEvent_t> tev;          // timing events, reused (ARB_OPT_TIMING)
+  double cable_ms = 0, event_ms = 0;
+  int64_t cable_timed = 0, event_timed = 0;
   int cur_pool = 0;
   int dyn_smem = 0;
   bool broken = false;
@@ -270,18 +273,40 @@ int arb_advance(arb_model* m, double t_end, double dt) {
   const int64_t fused = m->opt_fused > 0 ? std::min(m->opt_fused, epoch) : epoch;
   m->last_epoch_steps = epoch;
   int launches = 0;
+  // optional device timing (ARB_OPT_TIMING): four events per epoch on the model's stream
+  size_t n_tev = 0;
+  std::vector<int> tev_cable, tev_event;   // launches between events (1,2) and (0,1)+(2,3)
+  auto stamp = [&]() -> cudaError_t {
+    if (!m->opt_timing) return cudaSuccess;
+    if (n_tev == m->tev.size()) {
+      cudaEvent_t ev;
+      cudaError_t ce = cudaEventCreate(&ev);
+      if (ce != cudaSuccess) return ce;
+      m->tev.push_back(ev);
+    }
+    return cudaEventRecord(m->tev[n_tev++], m->stream);
+  };
   for (int64_t k = 0; k < nsteps;) {
     const int64_t n_ep = std::min(epoch, nsteps - k);
     const double t_win = (k + n_ep == nsteps) ? t_end : t0 + (double)(k + n_ep) * dt;
+    int l0 = launches;
+    CU(m, stamp());
     CU(m, launch_build_events(D, m->cur_pool, t_win, m->stream, &launches));
     m->cur_pool ^= 1;
+    CU(m, stamp());
+    int l1 = launches;
     for (int64_t j = 0; j < n_ep; j += fused) {
       StepArgs A;
       A.t0 = t0; A.dt = dt; A.t_end = t_end; A.k_first = k + j; A.nk = std::min(fused, n_ep - j); A.nsteps = nsteps; A.last_full = last_full;
       CU(m, launch_cable(D, A, m->dyn_smem, m->stream));
       ++launches;
     }
+    CU(m, stamp());
+    int l2 = launches;
     if (m->H.n_conn > 0) CU(m, launch_spikes_to_events(D, m->cur_pool, m->stream, &launches));
+    CU(m, stamp());
+    tev_cable.push_back(l2 - l1);
+    tev_event.push_back((l1 - l0) + (launches - l2));
     k += n_ep;
   }
   m->launches += launches;
@@ -289,6 +314,14 @@ int arb_advance(arb_model* m, double t_end, double dt) {
   CU(m, cudaMemcpyAsync(cnt, D.counters, sizeof cnt, cudaMemcpyDeviceToHost, m->stream));
   cudaError_t e = cudaStreamSynchronize(m->stream);
   if (e != cudaSuccess) { m->broken = true; return cuda_fail(m, e, "arb_advance"); }
+  for (size_t i = 0; i + 3 < n_tev; i += 4) {
+    float a = 0, b = 0, c = 0;
+    cudaEventElapsedTime(&a, m->tev[i], m->tev[i + 1]);
+    cudaEventElapsedTime(&b, m->tev[i + 1], m->tev[i + 2]);
+    cudaEventElapsedTime(&c, m->tev[i + 2], m->tev[i + 3]);
+    m->cable_ms += b; m->event_ms += a + c;
+    m->cable_timed += tev_cable[i / 4]; m->event_timed += tev_event[i / 4];
+  }
   m->t = t_end;
   m->grid_steps += nsteps;
   if (cnt[CNT_ERROR]) {
@@ -360,6 +393,10 @@ int arb_probe(arb_model* m, int what, double* out, int64_t n) {
       if (n < 1) return fail(m, ARB_E_INVALID, "arb_probe: size mismatch");
       out[0] = m->t;
       return ARB_OK;
+    case ARB_PROBE_TIMING:
+      if (n < 4) return fail(m, ARB_E_INVALID, "arb_probe: size mismatch");
+      out[0] = m->cable_ms; out[1] = (double)m->cable_timed; out[2] = m->event_ms; out[3] = (double)m->event_timed;
+      return ARB_OK;
     case ARB_PROBE_NSTEPS: case ARB_PROBE_STATS: {
       if (n < (what == ARB_PROBE_NSTEPS ? 2 : 8)) return fail(m, ARB_E_INVALID, "arb_probe: size mismatch");
       unsigned long long cnt[CNT_COUNT];
@@ -409,6 +446,10 @@ int arb_set_option(arb_model* m, int key, int64_t value) {
   switch (key) {
     case ARB_OPT_FUSED_STEPS: m->opt_fused = value; return ARB_OK;
     case ARB_OPT_EPOCH_STEPS: m->opt_epoch = value; return ARB_OK;
+    case ARB_OPT_TIMING:
+      m->opt_timing = value;
+      m->cable_ms = m->event_ms = 0; m->cable_timed = m->event_timed = 0;
+      return ARB_OK;
   }
   return fail(m, ARB_E_INVALID, "arb_set_option: unknown key");
 }
@@ -416,6 +457,7 @@ int arb_set_option(arb_model* m, int key, int64_t value) {
 void arb_destroy(arb_model* m) {
   if (!m) return;
   if (m->ws) cudaStreamSynchronize(m->stream);
+  for (cudaEvent_t ev : m->tev) cudaEventDestroy(ev);
   delete m;
 }
 

@@ -176,8 +176,9 @@ def _binary_tree(nb):
     return np.array([-1] + [(b - 1) // 2 for b in range(1, nb)], np.int64)
 
 
-def _homogeneous(cfg, n_cells, nb, n, n_syn, t_end):
-    """Cells of configs 1-3: full binary tree of nb branches with n CVs each, HH soma, passive dendrites."""
+def _homogeneous(cfg, n_cells, nb, n, n_syn, t_end, first_cell=0):
+    """Cells of configs 1-3: full binary tree of nb branches with n CVs each, HH soma, passive dendrites.
+    `first_cell` shifts the per-cell seeds: cell c draws from stream [seed, first_cell + c]."""
     seed = BASE_SEED + cfg
     ncv = 1 + nb * n
     L = np.empty((n_cells, nb))
@@ -185,7 +186,7 @@ def _homogeneous(cfg, n_cells, nb, n, n_syn, t_end):
     syn_cv = np.empty((n_cells, n_syn), np.int32)
     rngs = []
     for c in range(n_cells):
-        rng = np.random.default_rng([seed, c])
+        rng = np.random.default_rng([seed, first_cell + c])
         L[c] = rng.uniform(100.0, 300.0, nb)
         D[c] = rng.uniform(0.5, 2.0, nb)
         syn_cv[c] = rng.integers(0, ncv, n_syn)
@@ -290,10 +291,11 @@ def config2(n_cells=10000, t_end=1000.0):
     return finalize(m)
 
 
-def config3(n_cells=100000, t_end=200.0, driven=True):
+def config3(n_cells=100000, t_end=200.0, driven=True, first_cell=0):
     """configs[3]: depth-6 trees (63 branches x 8 CVs), 50 expsyn, 50 incoming connections.
-    BASELINE.json names no drive; `driven` adds 200 Hz/cell Poisson input."""
-    m, rngs = _homogeneous(3, n_cells, 63, 8, 50, t_end)
+    BASELINE.json names no drive; `driven` adds 200 Hz/cell Poisson input.
+    `first_cell` selects another closed network of the same population (bench.py: one per rank)."""
+    m, rngs = _homogeneous(3, n_cells, 63, 8, 50, t_end, first_cell)
     _random_network(m, rngs, 50, 0.002, 200.0 if driven else 0.0, 0, 50, 0.002, t_end)
     m["name"] = "C3 large %d%s" % (n_cells, "" if driven else " undriven")
     return finalize(m)
