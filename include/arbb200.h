@@ -52,9 +52,18 @@ enum {
                                 through HBM every step); 0 (default) = a whole min-delay epoch
                                 (cells are independent within Delta_T)           */
   ARB_OPT_EPOCH_STEPS = 2,   /* cap on the epoch length in steps (default: floor(min delay / dt)) */
+  ARB_OPT_STAGES = 4,        /* shared-memory stages per warp of the cable kernel: 0 (default) = 2 when
+                                every launch streams the state once, 1 when launches are fused     */
   ARB_OPT_TIMING = 3         /* 1: bracket the cable-step launches and the epoch-boundary kernels of
                                 every epoch with CUDA events on the model's stream (read them with
                                 ARB_PROBE_TIMING); setting the option clears the accumulated times  */
+};
+
+/* arb_configure keys (process-wide defaults read by later arb_plan / arb_create calls) */
+enum {
+  ARB_CFG_UNIT_BYTES = 1     /* bytes of streamed records (coefficients + state) one warp's shared-memory
+                                stage may hold; cells are packed into units up to this size, larger
+                                cells are integrated by a whole CTA.  0 = built-in default (22528)  */
 };
 
 /* The problem statement of PAPER.md section II as flat arrays.
@@ -106,7 +115,7 @@ typedef struct arb_model arb_model; /* opaque; lives in host memory, owned by th
  * earlier than t = 0, inconsistent NULLs. */
 int arb_plan(const arb_desc* desc, size_t* workspace_bytes);
 
-/* Build the model: lay the cells out in blocks of interleaved branches, upload to
+/* Build the model: lay the cells out in units of interleaved branches, upload to
  * `dev_workspace` (DEVICE pointer, 256-byte aligned, >= workspace_bytes from arb_plan) on
  * `cuda_stream` (a cudaStream_t; NULL = default stream), initialise state (V = vinit, gates at
  * steady state, g = 0, t = 0; reading R4).  Returns after the upload has completed. */
@@ -132,9 +141,10 @@ int arb_voltage(arb_model* m, double* out, int64_t n_cv);
  * ARB_PROBE_TIME:  out[0] = current time, n >= 1.
  * ARB_PROBE_NSTEPS: out[0] = grid steps so far, out[1] = cell sub-steps so far (>= cells*grid
  *                  steps; the excess comes from event-driven step splitting), n >= 2.
- * ARB_PROBE_STATS: out[0..7] = {blocks, slots (padded CVs), branches, workspace bytes,
- *                  events delivered, kernel launches so far, epoch steps, streamed bytes per
- *                  cell-block step}, n >= 8.
+ * ARB_PROBE_STATS: out[0..7] = {units, slots (CVs incl. padding), branches, workspace bytes,
+ *                  events delivered, kernel launches so far, epoch steps, bytes of the records one
+ *                  grid step reads (all units)}, n >= 8; when n >= 12 also {warp units, warps per
+ *                  CTA and shared-memory bytes per warp of the last launch, distinct tree records}.
  * ARB_PROBE_TIMING: out[0..3] = {ms spent in cable-step kernels, cable-step launches timed,
  *                  ms spent in epoch-boundary (spike -> event) kernels, their launches}, measured
  *                  with CUDA events while ARB_OPT_TIMING is on, n >= 4. */
@@ -147,6 +157,9 @@ int arb_set_state(arb_model* m, const double* v, const double* hh_m, const doubl
                   const double* hh_n, const double* syn_g);
 
 int arb_set_option(arb_model* m, int key, int64_t value);
+
+/* Process-wide build defaults (ARB_CFG_*); affects models planned / created afterwards. */
+int arb_configure(int key, int64_t value);
 
 void arb_destroy(arb_model* m);
 

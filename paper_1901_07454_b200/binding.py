@@ -13,10 +13,11 @@ LIB_PATH = os.path.join(_HERE, "libarbb200.so")
 
 ARB_OK, ARB_E_NULL, ARB_E_INVALID, ARB_E_WORKSPACE, ARB_E_CUDA, ARB_E_OVERFLOW, ARB_E_NOMEM = 0, -1, -2, -3, -4, -5, -6
 ARB_PROBE_M, ARB_PROBE_H, ARB_PROBE_N, ARB_PROBE_SYN_G, ARB_PROBE_TIME, ARB_PROBE_NSTEPS, ARB_PROBE_STATS, ARB_PROBE_TIMING = range(8)
-ARB_OPT_FUSED_STEPS, ARB_OPT_EPOCH_STEPS, ARB_OPT_TIMING = 1, 2, 3
+ARB_OPT_FUSED_STEPS, ARB_OPT_EPOCH_STEPS, ARB_OPT_TIMING, ARB_OPT_STAGES = 1, 2, 3, 4
+ARB_CFG_UNIT_BYTES = 1
 
 EXPORTS = ("arb_plan", "arb_create", "arb_advance", "arb_spikes", "arb_voltage", "arb_probe",
-           "arb_set_state", "arb_set_option", "arb_destroy", "arb_last_error")
+           "arb_set_state", "arb_set_option", "arb_configure", "arb_destroy", "arb_last_error")
 
 
 class ArbError(RuntimeError):
@@ -64,6 +65,7 @@ def lib():
         L.arb_probe.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int64]
         L.arb_set_state.argtypes = [C.c_void_p] * 6
         L.arb_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
+        L.arb_configure.argtypes = [C.c_int, C.c_int64]
         L.arb_destroy.argtypes = [C.c_void_p]
         L.arb_destroy.restype = None
         L.arb_last_error.restype = C.c_char_p
@@ -88,6 +90,12 @@ def make_desc(m):
         else:
             setattr(d, name, v)
     return d
+
+
+def configure(key, value):
+    rc = lib().arb_configure(int(key), int(value))
+    if rc:
+        raise ArbError(rc, lib().arb_last_error(None).decode())
 
 
 def arb_plan(m):
@@ -140,7 +148,7 @@ class Model:
         return out
 
     def probe(self, what):
-        n = {ARB_PROBE_SYN_G: self.n_syn, ARB_PROBE_TIME: 1, ARB_PROBE_NSTEPS: 2, ARB_PROBE_STATS: 8,
+        n = {ARB_PROBE_SYN_G: self.n_syn, ARB_PROBE_TIME: 1, ARB_PROBE_NSTEPS: 2, ARB_PROBE_STATS: 12,
              ARB_PROBE_TIMING: 4}.get(what, self.n_cv)
         out = np.empty(n)
         self._check(lib().arb_probe(self._h, what, _ptr(out), n))
@@ -157,8 +165,10 @@ class Model:
 
     def stats(self):
         s = self.probe(ARB_PROBE_STATS)
-        return dict(blocks=int(s[0]), slots=int(s[1]), branches=int(s[2]), workspace_bytes=int(s[3]),
-                    events_delivered=int(s[4]), launches=int(s[5]), epoch_steps=int(s[6]))
+        return dict(units=int(s[0]), slots=int(s[1]), branches=int(s[2]), workspace_bytes=int(s[3]),
+                    events_delivered=int(s[4]), launches=int(s[5]), epoch_steps=int(s[6]),
+                    streamed_bytes_per_step=int(s[7]), warp_units=int(s[8]), warps_per_cta=int(s[9]),
+                    smem_per_warp=int(s[10]), topo_records=int(s[11]))
 
     def timing(self):
         t = self.probe(ARB_PROBE_TIMING)

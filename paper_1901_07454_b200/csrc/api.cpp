@@ -32,7 +32,7 @@ struct Carver {
 };
 
 struct Regions {
-  Region blocks, gen, fast, state, meta, scratch, cell_rt, cell_orig, ev_off, ev_t, ev_gidx, ev_w, ev_fill,
+  Region units, gen, fast, state, topo, scratch, warp_scratch, factor_dcontrib, cell_rt_idx, cell_orig, ev_off, ev_t, ev_gidx, ev_w, ev_fill,
       ext_off, ext_t, ext_gidx, ext_w, ext_cur, conn_off, conn_dst, conn_gidx, conn_delay, conn_w,
       pool_t[2], pool_dst[2], pool_gidx[2], pool_w[2], spike_cell, spike_t, counters, scan_tmp,
       cv_idx, syn_idx, hh_m_idx, hh_stride, hh_cv, io;
@@ -49,17 +49,35 @@ Caps capacities(const HostModel& H) {
   return c;
 }
 
+int64_t warp_scratch_stride(const HostModel& H) { return 2 * (int64_t)H.slot_cap + align_up(H.lane_cap, 2); }
+
+// Shared-memory plan of the warp kernel for n_stage stages per warp; warps == 0: does not fit.
+WarpSmemPlan make_plan(const HostModel& H, uint32_t n_stage) {
+  WarpSmemPlan P;
+  P.fast_cap = H.fast_cap; P.state_cap = H.state_cap; P.stage_bytes = H.fast_cap + H.state_cap;
+  P.n_stage = n_stage;
+  P.slot_cap = H.slot_cap; P.lane_cap = H.lane_cap; P.spec_cap = H.spec_cap; P.cell_cap = std::max(H.cell_cap, 1u);
+  P.topo_cap = align_up(H.topo_cap, 16);
+  const ScratchOff so = scratch_offsets(P.topo_cap, P.lane_cap, P.spec_cap, P.cell_cap, n_stage);
+  P.scratch_off = n_stage * P.stage_bytes;
+  P.warp_bytes = align_up(P.scratch_off + so.total, 128);
+  P.warps = std::min<uint32_t>((uint32_t)cable_max_warps(), (uint32_t)cable_smem_limit() / P.warp_bytes);
+  return P;
+}
+
 Regions carve(const HostModel& H, const Caps& cap) {
   Regions R;
   Carver C;
   const size_t nc = (size_t)H.n_cells;
-  R.blocks = C.take(sizeof(BlockInfo) * (size_t)H.n_blocks);
+  R.units = C.take(sizeof(UnitDesc) * (size_t)H.n_units);
   R.gen = C.take(8 * (size_t)H.gen_doubles);
-  R.fast = C.take(8 * (size_t)H.fast_doubles);
+  R.fast = C.take((size_t)H.fast_bytes);
   R.state = C.take(8 * (size_t)H.state_doubles);
-  R.meta = C.take((size_t)H.meta_bytes);
+  R.topo = C.take((size_t)H.topo_bytes);
   R.scratch = C.take(8 * (size_t)H.scratch_doubles);
-  R.cell_rt = C.take(sizeof(CellRt) * nc);
+  R.warp_scratch = C.take(H.n_warp_units > 0 ? 8 * (size_t)(kMaxWarps * warp_scratch_stride(H)) : 0);
+  R.factor_dcontrib = C.take(8 * (size_t)H.n_lanes);
+  R.cell_rt_idx = C.take(4 * nc);
   R.cell_orig = C.take(4 * nc);
   R.ev_off = C.take(4 * (nc + 1));
   R.ev_t = C.take(8 * (size_t)cap.ev);
@@ -112,7 +130,8 @@ struct arb_model {
   double cable_ms = 0, event_ms = 0;
   int64_t cable_timed = 0, event_timed = 0;
   int cur_pool = 0;
-  int dyn_smem = 0;
+  int sm_count = 148;
+  int64_t opt_stages = 0;
   bool broken = false;
   std::string err;
 };
@@ -139,7 +158,13 @@ cudaError_t upload(arb_model* m, const Region& r, const std::vector<T>& v) {
   return cudaMemcpyAsync(m->ws + r.off, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, m->stream);
 }
 
-BuildParams default_params() { return BuildParams(); }
+int64_t g_unit_bytes = 0;   // arb_configure(ARB_CFG_UNIT_BYTES)
+
+BuildParams default_params() {
+  BuildParams P;
+  if (g_unit_bytes > 0) P.unit_bytes = (uint32_t)g_unit_bytes;
+  return P;
+}
 
 }  // namespace
 
@@ -175,20 +200,22 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     if (reinterpret_cast<uintptr_t>(dev_workspace) % 256) { delete m; return fail(nullptr, ARB_E_WORKSPACE, "arb_create: workspace must be 256-byte aligned"); }
     m->ws = static_cast<char*>(dev_workspace);
     m->stream = static_cast<cudaStream_t>(cuda_stream);
-    // shared-memory plan of the cable kernel: branches that do not fit use the global scratch
-    m->dyn_smem = std::min(cable_smem_bytes(H.max_block_lanes), cable_smem_limit());
-    for (auto& b : H.blocks)
-      if (cable_smem_bytes(b.n_lane) > m->dyn_smem) b.flags |= 1u;
+    if (H.n_warp_units > 0 && make_plan(H, 1).warps == 0) { delete m; return fail(nullptr, ARB_E_INVALID, "arb_create: a warp unit does not fit in shared memory"); }
+    {
+      int dev = 0, sms = 0;
+      if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) m->sm_count = sms;
+    }
     auto bail = [&](cudaError_t e, const char* w) { std::string s = std::string(w) + ": " + cudaGetErrorString(e); delete m; return fail(nullptr, ARB_E_CUDA, s); };
     cudaError_t e;
     const Regions& R = m->R;
     if ((e = cudaMemsetAsync(m->ws, 0, m->R.total, m->stream)) != cudaSuccess) return bail(e, "cudaMemsetAsync");
-    if ((e = upload(m, R.blocks, H.blocks)) != cudaSuccess) return bail(e, "upload blocks");
+    if ((e = upload(m, R.units, H.descs)) != cudaSuccess) return bail(e, "upload units");
     if ((e = upload(m, R.gen, H.gen)) != cudaSuccess) return bail(e, "upload gen");
     if ((e = upload(m, R.fast, H.fast)) != cudaSuccess) return bail(e, "upload fast");
     if ((e = upload(m, R.state, H.state)) != cudaSuccess) return bail(e, "upload state");
-    if ((e = upload(m, R.meta, H.meta)) != cudaSuccess) return bail(e, "upload meta");
+    if ((e = upload(m, R.topo, H.topo)) != cudaSuccess) return bail(e, "upload topo");
     if ((e = upload(m, R.cell_orig, H.cell_order)) != cudaSuccess) return bail(e, "upload cell order");
+    if ((e = upload(m, R.cell_rt_idx, H.cell_rt_idx)) != cudaSuccess) return bail(e, "upload cell runtime map");
     if ((e = upload(m, R.ext_off, H.ext_off)) != cudaSuccess) return bail(e, "upload ext_off");
     if ((e = upload(m, R.ext_t, H.ext_t)) != cudaSuccess) return bail(e, "upload ext_t");
     if ((e = upload(m, R.ext_gidx, H.ext_gidx)) != cudaSuccess) return bail(e, "upload ext_gidx");
@@ -209,11 +236,14 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     if ((e = upload(m, R.hh_stride, H.hh_stride)) != cudaSuccess) return bail(e, "upload hh map");
     if ((e = upload(m, R.hh_cv, H.hh_cv)) != cudaSuccess) return bail(e, "upload hh map");
     DevModel& D = m->D;
-    D.blocks = at<BlockInfo>(m, R.blocks);
-    D.n_blocks = H.n_blocks; D.n_cells = H.n_cells;
-    D.gen = at<double>(m, R.gen); D.fast = at<double>(m, R.fast); D.state = at<double>(m, R.state);
-    D.meta = at<uint8_t>(m, R.meta); D.scratch = at<double>(m, R.scratch);
-    D.cell_rt = at<CellRt>(m, R.cell_rt); D.cell_orig = at<uint32_t>(m, R.cell_orig);
+    std::memset(&D, 0, sizeof D);
+    D.units = at<UnitDesc>(m, R.units);
+    D.n_units = H.n_units; D.n_warp_units = H.n_warp_units; D.n_cells = H.n_cells;
+    D.gen = at<double>(m, R.gen); D.fast = at<uint8_t>(m, R.fast); D.state = at<double>(m, R.state);
+    D.topo = at<uint8_t>(m, R.topo); D.scratch = at<double>(m, R.scratch);
+    D.warp_scratch = at<double>(m, R.warp_scratch); D.warp_scratch_stride = warp_scratch_stride(H);
+    D.factor_dcontrib = at<double>(m, R.factor_dcontrib);
+    D.cell_orig = at<uint32_t>(m, R.cell_orig); D.cell_rt_idx = at<uint32_t>(m, R.cell_rt_idx);
     D.ev_off = at<uint32_t>(m, R.ev_off); D.ev_t = at<double>(m, R.ev_t); D.ev_gidx = at<uint32_t>(m, R.ev_gidx);
     D.ev_w = at<double>(m, R.ev_w); D.ev_fill = at<uint32_t>(m, R.ev_fill); D.ev_cap = m->cap.ev;
     D.ext_off = at<uint32_t>(m, R.ext_off); D.ext_t = at<double>(m, R.ext_t); D.ext_gidx = at<uint32_t>(m, R.ext_gidx);
@@ -224,6 +254,8 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
       D.pool[i].t = at<double>(m, R.pool_t[i]); D.pool[i].dst = at<uint32_t>(m, R.pool_dst[i]);
       D.pool[i].gidx = at<uint32_t>(m, R.pool_gidx[i]); D.pool[i].w = at<double>(m, R.pool_w[i]);
     }
+    D.syn_uniform = H.syn_uniform ? 1 : 0; D.syn_e_u = H.syn_e_u; D.syn_tau_u = H.syn_tau_u; D.syn_decay_u = 1.0;
+    D.plan = make_plan(H, 1);
     D.pool_cap = m->cap.pool;
     D.spike_cell = at<uint32_t>(m, R.spike_cell); D.spike_t = at<double>(m, R.spike_t); D.spike_cap = m->cap.spikes;
     D.counters = at<unsigned long long>(m, R.counters);
@@ -232,8 +264,8 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     if ((e = launch_init(D, m->stream)) != cudaSuccess) return bail(e, "init kernel");
     if ((e = cudaStreamSynchronize(m->stream)) != cudaSuccess) return bail(e, "cudaStreamSynchronize");
     // host pools are no longer needed
-    std::vector<double>().swap(H.gen); std::vector<double>().swap(H.fast); std::vector<double>().swap(H.state);
-    std::vector<uint8_t>().swap(H.meta);
+    std::vector<double>().swap(H.gen); std::vector<uint8_t>().swap(H.fast); std::vector<double>().swap(H.state);
+    std::vector<uint8_t>().swap(H.topo); std::vector<UnitDesc>().swap(H.descs); std::vector<uint32_t>().swap(H.cell_rt_idx);
     std::vector<uint32_t>().swap(H.cv_state_idx); std::vector<uint32_t>().swap(H.syn_state_idx);
     std::vector<uint32_t>().swap(H.hh_m_idx); std::vector<uint32_t>().swap(H.hh_stride); std::vector<uint32_t>().swap(H.hh_cv);
     std::vector<uint32_t>().swap(H.conn_off); std::vector<uint32_t>().swap(H.conn_dst); std::vector<uint32_t>().swap(H.conn_gidx);
@@ -255,8 +287,9 @@ int arb_advance(arb_model* m, double t_end, double dt) {
   if (t_end < m->t) return fail(m, ARB_E_INVALID, "arb_advance: t_end earlier than the current time");
   if (m->H.n_conn > 0 && m->H.min_delay < dt) return fail(m, ARB_E_INVALID, "arb_advance: dt longer than the shortest connection delay");
   if (t_end == m->t) return ARB_OK;
-  const DevModel& D = m->D;
+  DevModel& D = m->D;
   if (dt != m->factored_dt) {
+    D.syn_decay_u = D.syn_uniform ? std::exp(-dt / D.syn_tau_u) : 1.0;
     CU(m, launch_factor(D, dt, m->stream));
     m->factored_dt = dt;
     m->launches++;
@@ -272,6 +305,18 @@ int arb_advance(arb_model* m, double t_end, double dt) {
   if (m->opt_epoch > 0) epoch = std::min(epoch, m->opt_epoch);
   const int64_t fused = m->opt_fused > 0 ? std::min(m->opt_fused, epoch) : epoch;
   m->last_epoch_steps = epoch;
+  // shared-memory plan: two stages per warp (load the next unit while this one is integrated) when
+  // every launch streams the state once, one stage (more resident warps) when launches are fused
+  int grid = 1;
+  if (m->H.n_warp_units > 0) {
+    uint32_t n_stage = m->opt_stages > 0 ? (uint32_t)std::min<int64_t>(m->opt_stages, 2) : (fused > 1 ? 1u : 2u);
+    WarpSmemPlan P = make_plan(m->H, n_stage);
+    if (P.warps == 0) P = make_plan(m->H, 1);
+    const int64_t per_sm = (m->H.n_warp_units + m->sm_count - 1) / m->sm_count;
+    P.warps = (uint32_t)std::max<int64_t>(1, std::min<int64_t>(P.warps, per_sm));
+    grid = (int)std::min<int64_t>(m->sm_count, (m->H.n_warp_units + P.warps - 1) / P.warps);
+    D.plan = P;
+  }
   int launches = 0;
   // optional device timing (ARB_OPT_TIMING): four events per epoch on the model's stream
   size_t n_tev = 0;
@@ -298,8 +343,7 @@ int arb_advance(arb_model* m, double t_end, double dt) {
     for (int64_t j = 0; j < n_ep; j += fused) {
       StepArgs A;
       A.t0 = t0; A.dt = dt; A.t_end = t_end; A.k_first = k + j; A.nk = std::min(fused, n_ep - j); A.nsteps = nsteps; A.last_full = last_full;
-      CU(m, launch_cable(D, A, m->dyn_smem, m->stream));
-      ++launches;
+      CU(m, launch_cable(D, A, grid, m->stream, &launches));
     }
     CU(m, stamp());
     int l2 = launches;
@@ -403,11 +447,15 @@ int arb_probe(arb_model* m, int what, double* out, int64_t n) {
       CU(m, cudaMemcpyAsync(cnt, m->D.counters, sizeof cnt, cudaMemcpyDeviceToHost, m->stream));
       CU(m, cudaStreamSynchronize(m->stream));
       if (what == ARB_PROBE_NSTEPS) { out[0] = (double)m->grid_steps; out[1] = (double)cnt[CNT_SUBSTEPS]; return ARB_OK; }
-      int64_t slots = 0;
-      for (const auto& b : m->H.blocks) slots += b.n_slot;
-      out[0] = (double)m->H.n_blocks; out[1] = (double)slots; out[2] = (double)m->H.n_lanes;
+      int64_t slots = 0, streamed = 0;
+      for (const auto& u : m->H.units) { slots += u.n_slot; streamed += u.fast_bytes + u.state_bytes; }
+      out[0] = (double)m->H.n_units; out[1] = (double)slots; out[2] = (double)m->H.n_lanes;
       out[3] = (double)m->R.total; out[4] = (double)cnt[CNT_DELIVERED]; out[5] = (double)m->launches;
-      out[6] = (double)m->last_epoch_steps; out[7] = 0.0;
+      out[6] = (double)m->last_epoch_steps; out[7] = (double)streamed;
+      if (n >= 12) {
+        out[8] = (double)m->H.n_warp_units; out[9] = (double)m->D.plan.warps; out[10] = (double)m->D.plan.warp_bytes;
+        out[11] = (double)m->H.topo_records;
+      }
       return ARB_OK;
     }
   }
@@ -446,12 +494,24 @@ int arb_set_option(arb_model* m, int key, int64_t value) {
   switch (key) {
     case ARB_OPT_FUSED_STEPS: m->opt_fused = value; return ARB_OK;
     case ARB_OPT_EPOCH_STEPS: m->opt_epoch = value; return ARB_OK;
+    case ARB_OPT_STAGES: m->opt_stages = value; return ARB_OK;
     case ARB_OPT_TIMING:
       m->opt_timing = value;
       m->cable_ms = m->event_ms = 0; m->cable_timed = m->event_timed = 0;
       return ARB_OK;
   }
   return fail(m, ARB_E_INVALID, "arb_set_option: unknown key");
+}
+
+int arb_configure(int key, int64_t value) {
+  if (value < 0) return fail(nullptr, ARB_E_INVALID, "arb_configure: negative value");
+  switch (key) {
+    case ARB_CFG_UNIT_BYTES:
+      if (value != 0 && (value < 1024 || value > 112 * 1024)) return fail(nullptr, ARB_E_INVALID, "arb_configure: unit bytes out of range");
+      g_unit_bytes = value;
+      return ARB_OK;
+  }
+  return fail(nullptr, ARB_E_INVALID, "arb_configure: unknown key");
 }
 
 void arb_destroy(arb_model* m) {

@@ -1,25 +1,34 @@
 // kernels.cu - hand-written fp64 CUDA kernels for sm_100a: the whole hot path of arbb200.
 //
-//   cable_kernel        per grid step (or per fused run of steps) and per cell block:
+//   cable_warp_kernel   the cable step for "warp units" (unit_layout.h).  A persistent grid; every
+//                       warp is its own software pipeline: one lane issues bulk-async copies (TMA,
+//                       cp.async.bulk + mbarrier) that bring the next unit's fast and state records
+//                       into the warp's second shared-memory stage while all 32 lanes integrate the
+//                       current unit out of the first.  Per grid step (or fused run of steps):
 //                       event delivery -> mechanism currents (eq 2a)
-//                       -> rhs of the implicit Euler system -> branched Thomas /
-//                       Hines sweeps over levels of interleaved branches -> V <- V'
-//                       -> gate / synapse state update with V' -> threshold test
-//
-//   factor_kernel       once per dt: eliminates the (constant, reading R1) matrix of every cell
-//   build_events / spikes_to_events   once per min-delay epoch
+//                       -> rhs of the implicit Euler system -> branched Thomas / Hines
+//                       sweeps over tasks of interleaved branches -> V <- V' -> gate /
+//                       synapse state update with V' -> threshold test.
+//                       No block-level barrier anywhere: only __syncwarp between tree levels.
+//   cable_block_kernel  the same step for cells too large for a warp's stage: one CTA per unit,
+//                       working straight out of global memory (L1/L2), __syncthreads between levels.
+//   factor_kernel       once per dt: eliminates the (constant, reading R1) matrix of every unit
+//   ev_* / spikes_to_events   once per min-delay epoch
 //
 // No tensor cores: nothing here is a dense contraction.  The path is bound by HBM traffic when
-// state streams every step and by fp64 issue / dependent-chain latency when a block stays on chip.
+// state streams every step and by fp64 dependent-chain latency when a unit stays on chip.
 #include "kernels.cuh"
+
+#include <math_constants.h>
 
 namespace arbb {
 
 namespace {
 
-constexpr int kThreads = 256;
-constexpr int kWarps = kThreads / 32;
-constexpr int kMaxCells = 64;   // == BuildParams::max_cells
+constexpr int kBlockThreads = 256;              // cable_block_kernel, factor_kernel, init_kernel
+constexpr int kBlockWarps = kBlockThreads / 32;
+constexpr int kMaxWarpsPerCta = 8;              // cable_warp_kernel
+constexpr unsigned kFull = 0xffffffffu;
 
 // ------------------------------------------------------------------------------------------
 // HH rate functions (reading R5): textbook Hodgkin-Huxley 1952, 6.3 C, rest at -65 mV.
@@ -38,340 +47,695 @@ __device__ __forceinline__ Rates hh_rates(double v) {
   return r;
 }
 
-// Pointers of one block, resolved once per CTA.
-struct View {
-  const Task* tasks; const uint32_t* level_begin;
-  const uint32_t* br_pslot; const uint32_t* br_cbeg; const uint16_t* br_len; const uint16_t* br_cell;
-  const uint16_t* br_ccnt; const uint32_t* child; const uint32_t* cell_det;
-  const uint32_t* hh_slot; const uint16_t* hh_cell; const uint16_t* syn_cell;
-  const uint32_t* sp_slot; const int32_t* sp_hh; const uint32_t* sp_syn_beg; const uint32_t* sp_cl_beg;
-  const uint16_t* sp_syn_cnt; const uint16_t* sp_cl_cnt; const uint16_t* sp_cell;
-  // gen
-  const double *C, *S, *sig, *G, *bg;
-  // fast
-  double *f, *invd, *a, *b;
-  const double *hh_gna, *hh_gk, *hh_gl, *syn_e, *syn_tau, *cl_t0, *cl_t1, *cl_amp;
-  double* syn_decay;
-  // state
-  double *V, *m, *h, *n, *g;
-  // scratch (global): factors of a non-nominal step, extra currents
-  double *fgen, *invdgen;
+// ------------------------------------------------------------------------------------------
+// bulk-async copy (TMA) and mbarrier primitives
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
+               "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  const uint32_t addr = smem_u32(bar);
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(addr), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+
+// ------------------------------------------------------------------------------------------
+// scopes: a unit is integrated either by one warp or by one CTA
+// ------------------------------------------------------------------------------------------
+template <bool kWarp> struct Scope;
+template <> struct Scope<true> {
+  static constexpr int size = 32, warps = 1;
+  static __device__ __forceinline__ int tid() { return threadIdx.x & 31; }
+  static __device__ __forceinline__ int warp() { return 0; }
+  static __device__ __forceinline__ void sync() { __syncwarp(); }
+  static __device__ __forceinline__ bool any(bool p) { return __any_sync(kFull, p) != 0; }
+};
+template <> struct Scope<false> {
+  static constexpr int size = kBlockThreads, warps = kBlockWarps;
+  static __device__ __forceinline__ int tid() { return threadIdx.x; }
+  static __device__ __forceinline__ int warp() { return threadIdx.x >> 5; }
+  static __device__ __forceinline__ void sync() { __syncthreads(); }
+  static __device__ __forceinline__ bool any(bool p) { return __syncthreads_or(p) != 0; }
 };
 
-__device__ __forceinline__ View make_view(const DevModel& M, const BlockInfo& bi) {
-  View v;
-  const uint8_t* meta = M.meta + bi.meta_base;
-  MetaOff mo = meta_offsets(bi);
-  v.tasks = (const Task*)(meta + mo.tasks);
-  v.level_begin = (const uint32_t*)(meta + mo.level_begin);
-  v.br_pslot = (const uint32_t*)(meta + mo.br_pslot);
-  v.br_cbeg = (const uint32_t*)(meta + mo.br_cbeg);
-  v.br_len = (const uint16_t*)(meta + mo.br_len);
-  v.br_cell = (const uint16_t*)(meta + mo.br_cell);
-  v.br_ccnt = (const uint16_t*)(meta + mo.br_ccnt);
-  v.child = (const uint32_t*)(meta + mo.child);
-  v.cell_det = (const uint32_t*)(meta + mo.cell_det);
-  v.hh_slot = (const uint32_t*)(meta + mo.hh_slot);
-  v.hh_cell = (const uint16_t*)(meta + mo.hh_cell);
-  v.syn_cell = (const uint16_t*)(meta + mo.syn_cell);
-  v.sp_slot = (const uint32_t*)(meta + mo.sp_slot);
-  v.sp_hh = (const int32_t*)(meta + mo.sp_hh);
-  v.sp_syn_beg = (const uint32_t*)(meta + mo.sp_syn_beg);
-  v.sp_cl_beg = (const uint32_t*)(meta + mo.sp_cl_beg);
-  v.sp_syn_cnt = (const uint16_t*)(meta + mo.sp_syn_cnt);
-  v.sp_cl_cnt = (const uint16_t*)(meta + mo.sp_cl_cnt);
-  v.sp_cell = (const uint16_t*)(meta + mo.sp_cell);
-  GenOff go = gen_offsets(bi);
-  const double* gen = M.gen + bi.gen_base;
-  v.C = gen + go.C; v.S = gen + go.S; v.sig = gen + go.sig; v.G = gen + go.G; v.bg = gen + go.b;
-  FastOff fo = fast_offsets(bi);
-  double* fast = M.fast + bi.fast_base;
-  v.f = fast + fo.f; v.invd = fast + fo.invd; v.a = fast + fo.a; v.b = fast + fo.b;
-  v.hh_gna = fast + fo.hh_gna; v.hh_gk = fast + fo.hh_gk; v.hh_gl = fast + fo.hh_gl;
-  v.syn_e = fast + fo.syn_e; v.syn_decay = fast + fo.syn_decay; v.syn_tau = fast + fo.syn_tau;
-  v.cl_t0 = fast + fo.cl_t0; v.cl_t1 = fast + fo.cl_t1; v.cl_amp = fast + fo.cl_amp;
-  StateOff so = state_offsets(bi);
-  double* st = M.state + bi.state_base;
-  v.V = st + so.v; v.m = st + so.m; v.h = st + so.h; v.n = st + so.n; v.g = st + so.g;
-  double* sc = M.scratch + bi.scratch_base;
-  v.fgen = sc; v.invdgen = sc + bi.n_slot;
-  return v;
+// Pointers of one unit.  "Working" pointers address shared memory in the warp kernel and global
+// memory in the block kernel; g* pointers always address the unit's state record in global memory.
+struct UnitView {
+  uint32_t n_slot, n_lane, n_task, n_level, n_cell, n_hh, n_syn, n_clamp;
+  const double *f, *invd, *a, *b, *hh_gna, *hh_gk, *hh_gl, *syn_e, *syn_decay, *cl_t0, *cl_t1, *cl_amp;
+  const uint32_t *hh_slot, *syn_slot, *cl_slot;
+  const uint16_t *hh_cell, *syn_cell, *cl_cell;
+  double *V, *m, *h, *n, *g, *rt;
+  double *gV, *gm, *gh, *gn, *gg, *grt;
+  uint32_t g_gidx0;                 // state-pool index of g[0]
+  const Task* tasks; const LaneRec* lanes; const uint32_t *level_begin, *child, *cell_det;
+  const double *C, *S, *sig, *G, *bg, *syn_tau;
+  double *contrib, *dcontrib, *xI, *fgen, *invdgen;
+  int64_t cell_base;
+};
+
+__device__ __forceinline__ void make_view(UnitView& U, const DevModel& M, const UnitHeader& H, uint8_t* fastw, double* statew,
+                                          const uint8_t* topow) {
+  U.n_slot = H.n_slot; U.n_lane = H.n_lane; U.n_task = H.n_task; U.n_level = H.n_level;
+  U.n_cell = H.n_cell; U.n_hh = H.n_hh; U.n_syn = H.n_syn; U.n_clamp = H.n_clamp;
+  const FastOff fo = fast_offsets(H.n_slot, H.n_hh, H.n_syn, H.n_clamp, H.n_cell, M.syn_uniform != 0);
+  U.f = (const double*)(fastw + fo.f); U.invd = (const double*)(fastw + fo.invd);
+  U.a = (const double*)(fastw + fo.a); U.b = (const double*)(fastw + fo.b);
+  U.hh_gna = (const double*)(fastw + fo.hh_gna); U.hh_gk = (const double*)(fastw + fo.hh_gk); U.hh_gl = (const double*)(fastw + fo.hh_gl);
+  U.syn_e = (const double*)(fastw + fo.syn_e); U.syn_decay = (const double*)(fastw + fo.syn_decay);
+  U.cl_t0 = (const double*)(fastw + fo.cl_t0); U.cl_t1 = (const double*)(fastw + fo.cl_t1); U.cl_amp = (const double*)(fastw + fo.cl_amp);
+  U.hh_slot = (const uint32_t*)(fastw + fo.hh_slot); U.syn_slot = (const uint32_t*)(fastw + fo.syn_slot); U.cl_slot = (const uint32_t*)(fastw + fo.cl_slot);
+  U.hh_cell = (const uint16_t*)(fastw + fo.hh_cell); U.syn_cell = (const uint16_t*)(fastw + fo.syn_cell); U.cl_cell = (const uint16_t*)(fastw + fo.cl_cell);
+  const StateOff so = state_offsets(H.n_slot, H.n_hh, H.n_syn, H.n_cell);
+  U.V = statew + so.v; U.m = statew + so.m; U.h = statew + so.h; U.n = statew + so.n; U.g = statew + so.g; U.rt = statew + so.rt;
+  double* gs = M.state + H.state_base;
+  U.gV = gs + so.v; U.gm = gs + so.m; U.gh = gs + so.h; U.gn = gs + so.n; U.gg = gs + so.g; U.grt = gs + so.rt;
+  U.g_gidx0 = (uint32_t)(H.state_base + so.g);
+  const TopoOff to = topo_offsets(H.n_task, H.n_level, H.n_lane, H.n_child, H.n_cell);
+  U.tasks = (const Task*)(topow + to.tasks); U.lanes = (const LaneRec*)(topow + to.lanes);
+  U.level_begin = (const uint32_t*)(topow + to.level_begin); U.child = (const uint32_t*)(topow + to.child);
+  U.cell_det = (const uint32_t*)(topow + to.cell_det);
+  const GenOff go = gen_offsets(H.n_slot, H.n_syn);
+  const double* gen = M.gen + H.gen_base;
+  U.C = gen + go.C; U.S = gen + go.S; U.sig = gen + go.sig; U.G = gen + go.G; U.bg = gen + go.b; U.syn_tau = gen + go.syn_tau;
+  U.cell_base = H.cell_base;
+}
+
+// per-cell runtime of the (sub-)step in progress, in shared memory
+struct CellS {
+  double *tcur, *tnext, *delta, *vprev;
+  uint32_t *evcur, *evend, *armed, *mode, *wb, *dirty;
+};
+__device__ __forceinline__ CellS carve_cells(uint8_t* p, uint32_t cap) {
+  CellS c;
+  c.tcur = (double*)p; c.tnext = c.tcur + cap; c.delta = c.tnext + cap; c.vprev = c.delta + cap;
+  c.evcur = (uint32_t*)(c.vprev + cap); c.evend = c.evcur + cap; c.armed = c.evend + cap;
+  c.mode = c.armed + cap; c.wb = c.mode + cap; c.dirty = c.wb + cap;
+  return c;
+}
+
+struct TaskCtx { Task T; LaneRec R; };
+__device__ __forceinline__ TaskCtx load_ctx(const UnitView& U, uint32_t ti, int lane) {
+  TaskCtx c;
+  c.T = U.tasks[ti];
+  c.R = U.lanes[c.T.lane_off + ((uint32_t)lane < c.T.nlanes ? lane : 0)];
+  return c;
 }
 
 // ------------------------------------------------------------------------------------------
-// Backward (leaves -> root) elimination of the diagonal for one step length, used by the
-// factorisation and by non-nominal (split) steps.  For a branch (lane) with CVs k = 0..len-1:
+// Elimination of the diagonal for one step length (factorisation, and event-split sub-steps).
+// For a branch (lane) with CVs k = 0..len-1:
 //   d_k = C_k/delta + S_k - sum_children sigma_c^2 / d_c ;  f_k = -sigma_k / d_k = u_k / d_k
-// Returns through fout/invdout; dcontrib[tl] = f_0 * u_0 is what the parent's terminal CV loses.
+// fout/invdout receive f and 1/d; dcontrib[branch] = f_0 * u_0 is what the parent's last CV loses.
+// Every lane of the warp must call it (ragged rows are counted with ballots); `on` selects the
+// lanes that take part.
 // ------------------------------------------------------------------------------------------
-__device__ __forceinline__ void eliminate_branch(const View& W, const Task& T, uint32_t lane, uint32_t tl,
-                                                 double delta, double* fout, double* invdout,
-                                                 double* dcontrib) {
-  const uint32_t len = W.br_len[tl];
-  const uint32_t base = T.slot_off + lane;
-  uint32_t s = base + (len - 1) * T.width;
-  double d = W.C[s] / delta + W.S[s];
-  const uint32_t cb = W.br_cbeg[tl], cc = W.br_ccnt[tl];
-  for (uint32_t j = 0; j < cc; ++j) d -= dcontrib[W.child[cb + j]];
-  for (uint32_t k = len - 1;; --k) {
-    double invd = 1.0 / d;
-    double sg = W.sig[s];
-    double f = -sg * invd;
-    fout[s] = f;
-    invdout[s] = invd;
-    if (k == 0) { dcontrib[tl] = -f * sg; break; }     // f*u with u = -sigma
-    s -= T.width;
-    d = W.C[s] / delta + W.S[s] + f * sg;                // d_p -= f*u
+__device__ __forceinline__ void eliminate_task(const UnitView& U, const TaskCtx& X, int lane, bool on, double delta,
+                                               double* fout, double* invdout, double* dcontrib) {
+  const Task& T = X.T;
+  const bool in = (uint32_t)lane < T.nlanes;
+  const uint32_t len = in ? X.R.len : 0u;
+  const uint32_t maxlen = T.maxlen_full & 0x7FFFu;
+  const bool full = (T.maxlen_full & kTaskFull) != 0;
+  const uint32_t tl = T.lane_off + lane;
+  uint32_t row = T.slot_off + T.nslots;
+  double fp = 0.0, sgp = 0.0;
+  for (int k = (int)maxlen - 1; k >= 0; --k) {
+    const bool act = (uint32_t)k < len;
+    const uint32_t cnt = full ? T.nlanes : (uint32_t)__popc(__ballot_sync(kFull, act));
+    row -= cnt;
+    if (act && on) {
+      const uint32_t s = row + lane;
+      double d = U.C[s] / delta + U.S[s];
+      if ((uint32_t)k == len - 1) {
+        for (uint32_t j = 0; j < X.R.ccnt; ++j) d -= dcontrib[U.child[X.R.cbeg + j]];
+      } else {
+        d = fma(fp, sgp, d);                 // d_p -= f*u with u = -sigma
+      }
+      const double invd = 1.0 / d;
+      const double sg = U.sig[s];
+      const double fk = -sg * invd;
+      fout[s] = fk;
+      invdout[s] = invd;
+      fp = fk; sgp = sg;
+      if (k == 0) dcontrib[tl] = -fk * sg;   // f*u
+    }
   }
 }
 
-__global__ void __launch_bounds__(kThreads) factor_kernel(DevModel M, double dt) {
-  __shared__ BlockInfo bi;
-  if (threadIdx.x == 0) bi = M.blocks[blockIdx.x];
-  __syncthreads();
-  View W = make_view(M, bi);
-  double* dcontrib = M.scratch + bi.scratch_base + 2 * (int64_t)bi.n_slot;   // global scratch
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  for (int lvl = (int)bi.n_level - 1; lvl >= 0; --lvl) {
-    for (uint32_t ti = W.level_begin[lvl] + warp; ti < W.level_begin[lvl + 1]; ti += kWarps) {
-      Task T = W.tasks[ti];
-      if ((uint32_t)lane < T.nlanes) eliminate_branch(W, T, lane, T.lane_off + lane, dt, W.f, W.invd, dcontrib);
+// ------------------------------------------------------------------------------------------
+// Backward (leaves -> root) sweep of one task on the rhs held in U.V:
+//   rhs_{k-1} -= f_k rhs_k along the branch, the parent's last CV loses contrib[child] = f_0 rhs_0;
+// every CV is left holding rhs_k / d_k, which is what the forward sweep needs.
+// kGen: cells of the unit may be inactive (mode 0) or on an event-split sub-step (mode 2).
+// ------------------------------------------------------------------------------------------
+template <bool kGen>
+__device__ __forceinline__ void backward_task(const UnitView& U, const CellS& cs, const TaskCtx& X, int lane) {
+  const Task& T = X.T;
+  const bool in = (uint32_t)lane < T.nlanes;
+  const uint32_t len = in ? X.R.len : 0u;
+  const uint32_t maxlen = T.maxlen_full & 0x7FFFu;
+  const bool full = (T.maxlen_full & kTaskFull) != 0;
+  const uint32_t tl = T.lane_off + lane;
+  uint32_t md = in ? 1u : 0u;
+  if (kGen) {
+    double delta = 0.0;
+    if (in) { md = cs.mode[X.R.cell]; delta = cs.delta[X.R.cell]; }
+    if (__any_sync(kFull, md == 2u)) eliminate_task(U, X, lane, md == 2u, delta, U.fgen, U.invdgen, U.dcontrib);
+  }
+  if (!kGen && full) {
+    // every row is full and every lane takes a nominal step: rows are prefetched four at a time so
+    // that only the dependent fma chain is exposed
+    if (!in) return;
+    const uint32_t w = T.nlanes;
+    uint32_t s = T.slot_off + T.nslots - w + lane;
+    double r = U.V[s];
+    for (uint32_t j = 0; j < X.R.ccnt; ++j) r -= U.contrib[U.child[X.R.cbeg + j]];
+    double fc = U.f[s], ic = U.invd[s];
+    uint32_t k = maxlen - 1;
+    while (k >= 4) {
+      const uint32_t s1 = s - w, s2 = s1 - w, s3 = s2 - w, s4 = s3 - w;
+      const double r1 = U.V[s1], r2 = U.V[s2], r3 = U.V[s3], r4 = U.V[s4];
+      const double f1 = U.f[s1], f2 = U.f[s2], f3 = U.f[s3], f4 = U.f[s4];
+      const double i1 = U.invd[s1], i2 = U.invd[s2], i3 = U.invd[s3], i4 = U.invd[s4];
+      U.V[s] = r * ic;   r = fma(-fc, r, r1);
+      U.V[s1] = r * i1;  r = fma(-f1, r, r2);
+      U.V[s2] = r * i2;  r = fma(-f2, r, r3);
+      U.V[s3] = r * i3;  r = fma(-f3, r, r4);
+      fc = f4; ic = i4; s = s4; k -= 4;
     }
+    while (k >= 1) {
+      const uint32_t s1 = s - w;
+      const double r1 = U.V[s1], f1 = U.f[s1], i1 = U.invd[s1];
+      U.V[s] = r * ic;   r = fma(-fc, r, r1);
+      fc = f1; ic = i1; s = s1; --k;
+    }
+    U.V[s] = r * ic;
+    U.contrib[tl] = fc * r;
+    return;
+  }
+  uint32_t row = T.slot_off + T.nslots;
+  double r = 0.0, fp = 0.0;
+  for (int k = (int)maxlen - 1; k >= 0; --k) {
+    const bool act = (uint32_t)k < len;
+    const uint32_t cnt = full ? T.nlanes : (uint32_t)__popc(__ballot_sync(kFull, act));
+    row -= cnt;
+    if (act && md) {
+      const uint32_t s = row + lane;
+      double rk = U.V[s];
+      if ((uint32_t)k == len - 1) {
+        for (uint32_t j = 0; j < X.R.ccnt; ++j) rk -= U.contrib[U.child[X.R.cbeg + j]];
+      } else {
+        rk = fma(-fp, r, rk);
+      }
+      double fk, ik;
+      if (kGen && md == 2u) { fk = U.fgen[s]; ik = U.invdgen[s]; }
+      else { fk = U.f[s]; ik = U.invd[s]; }
+      U.V[s] = rk * ik;
+      r = rk; fp = fk;
+      if (k == 0) U.contrib[tl] = fk * rk;
+    }
+  }
+}
+
+// Forward (root -> leaves) substitution of one task: V'_k = rhs_k/d_k - f_k V'_{k-1}; V <- V'.
+// kStore: also store V' to the unit's state record in global memory when the cell's step ends.
+template <bool kGen, bool kStore>
+__device__ __forceinline__ void forward_task(const UnitView& U, const CellS& cs, const TaskCtx& X, int lane) {
+  const Task& T = X.T;
+  const bool in = (uint32_t)lane < T.nlanes;
+  const uint32_t len = in ? X.R.len : 0u;
+  const uint32_t maxlen = T.maxlen_full & 0x7FFFu;
+  const bool full = (T.maxlen_full & kTaskFull) != 0;
+  uint32_t md = in ? 1u : 0u;
+  bool wb = false;
+  if (kGen) {
+    if (in) { md = cs.mode[X.R.cell]; wb = kStore && cs.wb[X.R.cell] != 0u; }
+  } else {
+    wb = kStore && cs.wb[0] != 0u;
+  }
+  double vp = 0.0;
+  if (in && md && X.R.pslot != kNoSlot) vp = U.V[X.R.pslot];
+  if (!kGen && full) {
+    if (!in) return;
+    const uint32_t w = T.nlanes;
+    uint32_t s = T.slot_off + lane;
+    uint32_t k = maxlen;
+    while (k >= 4) {
+      const uint32_t s1 = s + w, s2 = s1 + w, s3 = s2 + w;
+      const double f0 = U.f[s], f1 = U.f[s1], f2 = U.f[s2], f3 = U.f[s3];
+      const double q0 = U.V[s], q1 = U.V[s1], q2 = U.V[s2], q3 = U.V[s3];
+      const double v0 = fma(-f0, vp, q0), v1 = fma(-f1, v0, q1), v2 = fma(-f2, v1, q2), v3 = fma(-f3, v2, q3);
+      U.V[s] = v0; U.V[s1] = v1; U.V[s2] = v2; U.V[s3] = v3;
+      if (wb) { U.gV[s] = v0; U.gV[s1] = v1; U.gV[s2] = v2; U.gV[s3] = v3; }
+      vp = v3; s = s3 + w; k -= 4;
+    }
+    while (k >= 1) {
+      vp = fma(-U.f[s], vp, U.V[s]);
+      U.V[s] = vp;
+      if (wb) U.gV[s] = vp;
+      s += w; --k;
+    }
+    return;
+  }
+  uint32_t row = T.slot_off;
+  for (uint32_t k = 0; k < maxlen; ++k) {
+    const bool act = k < len;
+    const uint32_t cnt = full ? T.nlanes : (uint32_t)__popc(__ballot_sync(kFull, act));
+    if (act && md) {
+      const uint32_t s = row + lane;
+      const double fk = (kGen && md == 2u) ? U.fgen[s] : U.f[s];
+      vp = fma(-fk, vp, U.V[s]);
+      U.V[s] = vp;
+      if (wb) U.gV[s] = vp;
+    }
+    row += cnt;
+  }
+}
+
+// rhs_i = (C_i/delta - G_i) V_i + G_i e_i in place of V, one task (general path only)
+__device__ __forceinline__ void rhs_task(const UnitView& U, const CellS& cs, const TaskCtx& X, int lane) {
+  const Task& T = X.T;
+  const bool in = (uint32_t)lane < T.nlanes;
+  const uint32_t len = in ? X.R.len : 0u;
+  const uint32_t maxlen = T.maxlen_full & 0x7FFFu;
+  const bool full = (T.maxlen_full & kTaskFull) != 0;
+  uint32_t md = 0;
+  double delta = 0.0;
+  if (in) { md = cs.mode[X.R.cell]; delta = cs.delta[X.R.cell]; }
+  uint32_t row = T.slot_off;
+  for (uint32_t k = 0; k < maxlen; ++k) {
+    const bool act = k < len;
+    const uint32_t cnt = full ? T.nlanes : (uint32_t)__popc(__ballot_sync(kFull, act));
+    if (act && md) {
+      const uint32_t s = row + lane;
+      if (md == 1u) U.V[s] = fma(U.a[s], U.V[s], U.b[s]);
+      else U.V[s] = fma(U.C[s] / delta - U.G[s], U.V[s], U.bg[s]);
+    }
+    row += cnt;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// One (sub-)step of every active cell of a unit, phases B..F of the step (phase A, event delivery
+// and the choice of the sub-step, is in run_unit).
+// ------------------------------------------------------------------------------------------
+template <bool kWarp, bool kGen>
+__device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, const CellS& cs, double dt) {
+  using S = Scope<kWarp>;
+  const int tid = S::tid(), lane = threadIdx.x & 31;
+  const bool multi = U.n_cell > 1;
+  const uint32_t n_hh = U.n_hh, n_syn = U.n_syn, n_cl = U.n_clamp;
+
+  // ---- B: currents of HH, synapses and clamps from V(t); the passive current is
+  // folded into a, b.  Items on one CV form a run; the first lane of a run sums it in index order.
+  for (uint32_t i = tid; i < n_hh; i += S::size) {
+    if (kGen && !cs.mode[multi ? U.hh_cell[i] : 0]) continue;
+    const double v = U.V[U.hh_slot[i]];
+    const double m = U.m[i], h = U.h[i], n = U.n[i];
+    U.xI[i] = U.hh_gna[i] * m * m * m * h * (v - M.ena) + U.hh_gk[i] * n * n * n * n * (v - M.ek) + U.hh_gl[i] * (v - M.el);
+  }
+  for (uint32_t i = tid; i < n_syn; i += S::size) {
+    const uint32_t slot = U.syn_slot[i];
+    if (i > 0 && U.syn_slot[i - 1] == slot) continue;
+    if (kGen && !cs.mode[multi ? U.syn_cell[i] : 0]) continue;
+    const double v = U.V[slot];
+    double I = 0.0;
+    uint32_t j = i;
+    do {
+      I += U.g[j] * (v - (M.syn_uniform ? M.syn_e_u : U.syn_e[j]));
+      ++j;
+    } while (j < n_syn && U.syn_slot[j] == slot);
+    U.xI[n_hh + i] = I;
+  }
+  for (uint32_t i = tid; i < n_cl; i += S::size) {
+    const uint32_t slot = U.cl_slot[i];
+    if (i > 0 && U.cl_slot[i - 1] == slot) continue;
+    const uint32_t c = multi ? U.cl_cell[i] : 0;
+    if (kGen && !cs.mode[c]) continue;
+    const double t = cs.tcur[c];
+    double I = 0.0;
+    uint32_t j = i;
+    do {
+      if (U.cl_t0[j] <= t && t < U.cl_t1[j]) I -= U.cl_amp[j];
+      ++j;
+    } while (j < n_cl && U.cl_slot[j] == slot);
+    U.xI[n_hh + n_syn + i] = I;
+  }
+  S::sync();
+
+  // ---- C: rhs_i = (C_i/delta - G_i) V_i + G_i e_i - I_i, in place of V
+  if (!kGen) {
+    const uint32_t n = U.n_slot;
+#pragma unroll 4
+    for (uint32_t s = tid; s < n; s += S::size) U.V[s] = fma(U.a[s], U.V[s], U.b[s]);
+  } else {
+    for (uint32_t ti = S::warp(); ti < U.n_task; ti += S::warps) rhs_task(U, cs, load_ctx(U, ti, lane), lane);
+  }
+  S::sync();
+  if (n_hh) {
+    for (uint32_t i = tid; i < n_hh; i += S::size) {
+      if (kGen && !cs.mode[multi ? U.hh_cell[i] : 0]) continue;
+      U.V[U.hh_slot[i]] -= U.xI[i];
+    }
+    S::sync();
+  }
+  if (n_syn) {
+    for (uint32_t i = tid; i < n_syn; i += S::size) {
+      const uint32_t slot = U.syn_slot[i];
+      if (i > 0 && U.syn_slot[i - 1] == slot) continue;
+      if (kGen && !cs.mode[multi ? U.syn_cell[i] : 0]) continue;
+      U.V[slot] -= U.xI[n_hh + i];
+    }
+    S::sync();
+  }
+  if (n_cl) {
+    for (uint32_t i = tid; i < n_cl; i += S::size) {
+      const uint32_t slot = U.cl_slot[i];
+      if (i > 0 && U.cl_slot[i - 1] == slot) continue;
+      if (kGen && !cs.mode[multi ? U.cl_cell[i] : 0]) continue;
+      U.V[slot] -= U.xI[n_hh + n_syn + i];
+    }
+    S::sync();
+  }
+
+  // ---- D: backward sweep, deepest level first; E: forward substitution, root first; V <- V'
+  if (kWarp) {
+    // one warp owns the unit: tasks are ordered by level, the next task's records are fetched
+    // while the current one is swept
+    TaskCtx cur = load_ctx(U, U.n_task - 1, lane);
+    for (int ti = (int)U.n_task - 1; ti >= 0; --ti) {
+      TaskCtx nxt = cur;
+      if (ti > 0) nxt = load_ctx(U, ti - 1, lane);
+      backward_task<kGen>(U, cs, cur, lane);
+      cur = nxt;
+      __syncwarp();
+    }
+    for (uint32_t ti = 0; ti < U.n_task; ++ti) {        // cur == task 0 here
+      TaskCtx nxt = cur;
+      if (ti + 1 < U.n_task) nxt = load_ctx(U, ti + 1, lane);
+      forward_task<kGen, true>(U, cs, cur, lane);
+      cur = nxt;
+      __syncwarp();
+    }
+  } else {
+    const int warp = S::warp();
+    for (int lvl = (int)U.n_level - 1; lvl >= 0; --lvl) {
+      for (uint32_t ti = U.level_begin[lvl] + warp; ti < U.level_begin[lvl + 1]; ti += S::warps)
+        backward_task<kGen>(U, cs, load_ctx(U, ti, lane), lane);
+      __syncthreads();
+    }
+    for (uint32_t lvl = 0; lvl < U.n_level; ++lvl) {
+      for (uint32_t ti = U.level_begin[lvl] + warp; ti < U.level_begin[lvl + 1]; ti += S::warps)
+        forward_task<kGen, false>(U, cs, load_ctx(U, ti, lane), lane);
+      __syncthreads();
+    }
+  }
+
+  // ---- F: state update with V', threshold test
+  for (uint32_t i = tid; i < n_hh; i += S::size) {
+    const uint32_t c = (kGen && multi) ? U.hh_cell[i] : 0;
+    if (kGen && !cs.mode[c]) continue;
+    const double delta = kGen ? cs.delta[c] : dt;
+    const Rates r = hh_rates(U.V[U.hh_slot[i]]);
+    double inf = r.am / (r.am + r.bm);
+    const double m = inf + (U.m[i] - inf) * exp(-delta * (r.am + r.bm));
+    inf = r.ah / (r.ah + r.bh);
+    const double h = inf + (U.h[i] - inf) * exp(-delta * (r.ah + r.bh));
+    inf = r.an / (r.an + r.bn);
+    const double n = inf + (U.n[i] - inf) * exp(-delta * (r.an + r.bn));
+    U.m[i] = m; U.h[i] = h; U.n[i] = n;
+    if (kWarp && cs.wb[c]) { U.gm[i] = m; U.gh[i] = h; U.gn[i] = n; }
+  }
+  for (uint32_t i = tid; i < n_syn; i += S::size) {
+    const uint32_t c = (kGen && multi) ? U.syn_cell[i] : 0;
+    const uint32_t md = kGen ? cs.mode[c] : 1u;
+    if (!md) continue;
+    double decay;
+    if (md == 1u) decay = M.syn_uniform ? M.syn_decay_u : U.syn_decay[i];
+    else decay = exp(-cs.delta[c] / (M.syn_uniform ? M.syn_tau_u : U.syn_tau[i]));
+    const double g = U.g[i] * decay;
+    U.g[i] = g;
+    if (kWarp && cs.wb[c]) U.gg[i] = g;
+  }
+  if ((uint32_t)tid < U.n_cell && (!kGen || cs.mode[tid])) {
+    const double vd = U.V[U.cell_det[tid]], vp = cs.vprev[tid];
+    if (cs.armed[tid] && vp < M.theta && M.theta <= vd) {
+      const double ts = cs.tcur[tid] + cs.delta[tid] * (M.theta - vp) / (vd - vp);
+      const unsigned long long pos = atomicAdd(&M.counters[CNT_SPIKES], 1ull);
+      if ((int64_t)pos < M.spike_cap) { M.spike_cell[pos] = M.cell_orig[U.cell_base + tid]; M.spike_t[pos] = ts; }
+      else atomicOr(&M.counters[CNT_ERROR], 1ull);
+      cs.armed[tid] = 0; cs.dirty[tid] = 1;
+    }
+    if (vd < M.theta && !cs.armed[tid]) { cs.armed[tid] = 1; cs.dirty[tid] = 1; }
+    cs.tcur[tid] = cs.tnext[tid];
+  }
+  S::sync();
+}
+
+// ------------------------------------------------------------------------------------------
+// A.nk grid steps of one unit.  Phase A: deliver the events due now and choose each cell's
+// sub-step (reading R9), then the step itself.
+// ------------------------------------------------------------------------------------------
+template <bool kWarp>
+__device__ __forceinline__ void run_unit(const DevModel& M, const StepArgs& A, const UnitView& U, const CellS& cs,
+                                         unsigned& n_sub, unsigned& n_del) {
+  using S = Scope<kWarp>;
+  const int tid = S::tid();
+  const uint32_t n_cell = U.n_cell;
+  if ((uint32_t)tid < n_cell) {
+    const unsigned long long pk = (unsigned long long)__double_as_longlong(U.rt[kRtDoubles * tid + 1]);
+    cs.evcur[tid] = (uint32_t)pk; cs.evend[tid] = (uint32_t)(pk >> 32);
+    cs.armed[tid] = U.rt[kRtDoubles * tid + 2] != 0.0 ? 1u : 0u;
+    cs.dirty[tid] = 0;
+  }
+  for (int64_t k = A.k_first; k < A.k_first + A.nk; ++k) {
+    const double ta = (k == 0) ? A.t0 : __dadd_rn(A.t0, __dmul_rn((double)k, A.dt));
+    const double tb = (k + 1 == A.nsteps) ? A.t_end : __dadd_rn(A.t0, __dmul_rn((double)(k + 1), A.dt));
+    const bool nominal = (k + 1 < A.nsteps) || A.last_full;
+    const bool last = (k + 1 == A.k_first + A.nk);
+    if ((uint32_t)tid < n_cell) cs.tcur[tid] = ta;
+    S::sync();
+    for (;;) {
+      bool active = false, plain = true;
+      if ((uint32_t)tid < n_cell) {
+        const double t = cs.tcur[tid];
+        uint32_t md = 0;
+        if (t < tb) {
+          double tn = U.rt[kRtDoubles * tid];
+          if (tn <= t) {
+            uint32_t cur = cs.evcur[tid];
+            const uint32_t end = cs.evend[tid];
+            while (cur < end && M.ev_t[cur] <= t) { U.g[M.ev_gidx[cur] - U.g_gidx0] += M.ev_w[cur]; ++cur; ++n_del; }
+            tn = cur < end ? M.ev_t[cur] : CUDART_INF;
+            cs.evcur[tid] = cur; U.rt[kRtDoubles * tid] = tn; cs.dirty[tid] = 1;
+          }
+          const double next = tn < tb ? tn : tb;
+          const bool fast = nominal && t == ta && next == tb;
+          cs.delta[tid] = fast ? A.dt : next - t;
+          md = fast ? 1u : 2u;
+          cs.tnext[tid] = next;
+          cs.vprev[tid] = U.V[U.cell_det[tid]];
+          cs.wb[tid] = (last && next == tb) ? 1u : 0u;
+          active = true;
+          ++n_sub;
+        }
+        cs.mode[tid] = md;
+        plain = md == 1u;
+      }
+      if (!S::any(active)) break;
+      const bool general = S::any(!plain);
+      S::sync();
+      if (general) substep<kWarp, true>(M, U, cs, A.dt);
+      else substep<kWarp, false>(M, U, cs, A.dt);
+    }
+  }
+  if ((uint32_t)tid < n_cell && cs.dirty[tid]) {
+    double* rt = U.grt + kRtDoubles * tid;
+    const unsigned long long pk = ((unsigned long long)cs.evend[tid] << 32) | cs.evcur[tid];
+    rt[0] = U.rt[kRtDoubles * tid];
+    rt[1] = __longlong_as_double((long long)pk);
+    rt[2] = cs.armed[tid] ? 1.0 : 0.0;
+    if (kWarp) { U.rt[kRtDoubles * tid + 1] = rt[1]; U.rt[kRtDoubles * tid + 2] = rt[2]; }
+  }
+}
+
+__device__ __forceinline__ void flush_stats(const DevModel& M, unsigned n_sub, unsigned n_del) {
+  for (int o = 16; o; o >>= 1) { n_sub += __shfl_xor_sync(kFull, n_sub, o); n_del += __shfl_xor_sync(kFull, n_del, o); }
+  if ((threadIdx.x & 31) == 0) {
+    if (n_sub) atomicAdd(&M.counters[CNT_SUBSTEPS], (unsigned long long)n_sub);
+    if (n_del) atomicAdd(&M.counters[CNT_DELIVERED], (unsigned long long)n_del);
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// The cable step for warp units.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kMaxWarpsPerCta * 32, 1) cable_warp_kernel(DevModel M, StepArgs A) {
+  extern __shared__ __align__(128) uint8_t smem[];
+  const WarpSmemPlan P = M.plan;
+  const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t gw = blockIdx.x * (int64_t)P.warps + w;
+  const int64_t NW = gridDim.x * (int64_t)P.warps;
+  const int64_t n_units = M.n_warp_units;
+  if (gw >= n_units) return;                       // no block-level barrier is ever used
+  uint8_t* region = smem + (size_t)w * P.warp_bytes;
+  uint8_t* scr = region + P.scratch_off;
+  const ScratchOff so = scratch_offsets(P.topo_cap, P.lane_cap, P.spec_cap, P.cell_cap, P.n_stage);
+  uint64_t* mbar = (uint64_t*)(scr + so.mbar);
+  uint8_t* topow = scr + so.topo;
+  const CellS cs = carve_cells(scr + so.cell, P.cell_cap);
+  const uint32_t n_stage = P.n_stage;
+
+  auto issue = [&](const UnitDesc& d, uint32_t st) {
+    uint8_t* dst = region + (size_t)st * P.stage_bytes;
+    mbar_expect_tx(&mbar[st], d.fast_bytes + d.state_bytes);
+    bulk_g2s(dst, M.fast + d.fast_off, d.fast_bytes, &mbar[st]);
+    bulk_g2s(dst + P.fast_cap, M.state + d.state_base, d.state_bytes, &mbar[st]);
+  };
+  if (lane == 0) {
+    for (uint32_t s = 0; s < n_stage; ++s) mbar_init(&mbar[s], 1);
+    fence_mbar_init();
+    fence_proxy_async();
+    for (uint32_t s = 0; s < n_stage; ++s) {
+      const int64_t u = gw + (int64_t)s * NW;
+      if (u < n_units) issue(M.units[u], s);
+    }
+  }
+  __syncwarp();
+
+  int64_t cached_topo = -1;
+  unsigned n_sub = 0, n_del = 0;
+  uint32_t it = 0;
+  for (int64_t u = gw; u < n_units; u += NW, ++it) {
+    const uint32_t st = it % n_stage, parity = (it / n_stage) & 1u;
+    const int64_t un = u + (int64_t)n_stage * NW;
+    UnitDesc dn;
+    dn.fast_off = 0; dn.state_base = 0; dn.fast_bytes = 0; dn.state_bytes = 0;
+    if (lane == 0 && un < n_units) dn = M.units[un];        // in flight while this unit is integrated
+    mbar_wait(&mbar[st], parity);
+    uint8_t* fastw = region + (size_t)st * P.stage_bytes;
+    const UnitHeader H = *(const UnitHeader*)fastw;
+    if (H.topo_off != cached_topo) {
+      // tree structure differs from the previous unit's: fetch its record (L2-resident when shared)
+      const uint32_t bytes = topo_offsets(H.n_task, H.n_level, H.n_lane, H.n_child, H.n_cell).total;
+      const uint4* src = (const uint4*)(M.topo + H.topo_off);
+      uint4* dst = (uint4*)topow;
+      __syncwarp();
+      for (uint32_t i = lane; i < bytes / 16; i += 32) dst[i] = src[i];
+      __syncwarp();
+      cached_topo = H.topo_off;
+    }
+    UnitView U;
+    make_view(U, M, H, fastw, (double*)(fastw + P.fast_cap), topow);
+    U.contrib = (double*)(scr + so.contrib);
+    U.xI = (double*)(scr + so.xI);
+    double* ws = M.warp_scratch + gw * M.warp_scratch_stride;     // event-split sub-steps only
+    U.fgen = ws; U.invdgen = ws + P.slot_cap; U.dcontrib = ws + 2 * (size_t)P.slot_cap;
+    run_unit<true>(M, A, U, cs, n_sub, n_del);
+    fence_proxy_async();          // this warp's accesses to the stage come before the next bulk copy into it
+    __syncwarp();
+    if (lane == 0 && un < n_units) issue(dn, st);
+  }
+  flush_stats(M, n_sub, n_del);
+}
+
+// ------------------------------------------------------------------------------------------
+// The cable step for block units: one CTA per unit, working copy = the records in global memory.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void block_view(UnitView& U, const DevModel& M, const UnitHeader& H, const UnitDesc& d) {
+  make_view(U, M, H, M.fast + d.fast_off, M.state + d.state_base, M.topo + H.topo_off);
+  double* sc = M.scratch + H.scratch_base;
+  const uint32_t nl = align_up(H.n_lane, 2), ns = align_up(H.n_hh + H.n_syn + H.n_clamp, 2);
+  U.contrib = sc; U.dcontrib = sc + nl; U.xI = sc + 2 * (size_t)nl;
+  U.fgen = U.xI + ns; U.invdgen = U.fgen + H.n_slot;
+}
+
+__global__ void __launch_bounds__(kBlockThreads) cable_block_kernel(DevModel M, StepArgs A) {
+  __shared__ UnitHeader H;
+  __shared__ __align__(16) uint8_t cell_mem[kCellScratchBytes * kBlockUnitMaxCells];
+  const UnitDesc d = M.units[M.n_warp_units + blockIdx.x];
+  if (threadIdx.x < sizeof(UnitHeader) / 4) ((uint32_t*)&H)[threadIdx.x] = ((const uint32_t*)(M.fast + d.fast_off))[threadIdx.x];
+  __syncthreads();
+  UnitView U;
+  block_view(U, M, H, d);
+  const CellS cs = carve_cells(cell_mem, kBlockUnitMaxCells);
+  unsigned n_sub = 0, n_del = 0;
+  run_unit<false>(M, A, U, cs, n_sub, n_del);
+  flush_stats(M, n_sub, n_del);
+}
+
+// ------------------------------------------------------------------------------------------
+// Once per dt: f, 1/d, a, b (and per-synapse decay factors) of every unit.  One CTA per unit.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kBlockThreads) factor_kernel(DevModel M, double dt) {
+  __shared__ UnitHeader H;
+  const UnitDesc d = M.units[blockIdx.x];
+  if (threadIdx.x < sizeof(UnitHeader) / 4) ((uint32_t*)&H)[threadIdx.x] = ((const uint32_t*)(M.fast + d.fast_off))[threadIdx.x];
+  __syncthreads();
+  UnitView U;
+  make_view(U, M, H, M.fast + d.fast_off, M.state + d.state_base, M.topo + H.topo_off);
+  const int64_t lane_base = (int64_t)(((uint64_t)H.pad[1] << 32) | H.pad[0]);
+  double* dcontrib = M.factor_dcontrib + lane_base;
+  double* f = const_cast<double*>(U.f);
+  double* invd = const_cast<double*>(U.invd);
+  double* a = const_cast<double*>(U.a);
+  double* b = const_cast<double*>(U.b);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  for (int lvl = (int)U.n_level - 1; lvl >= 0; --lvl) {
+    for (uint32_t ti = U.level_begin[lvl] + warp; ti < U.level_begin[lvl + 1]; ti += kBlockWarps)
+      eliminate_task(U, load_ctx(U, ti, lane), lane, true, dt, f, invd, dcontrib);
     __syncthreads();
   }
-  for (uint32_t ti = warp; ti < bi.n_task; ti += kWarps) {
-    Task T = W.tasks[ti];
-    if ((uint32_t)lane < T.nlanes) {
-      uint32_t len = W.br_len[T.lane_off + lane];
-      for (uint32_t k = 0; k < len; ++k) {
-        uint32_t s = T.slot_off + lane + k * T.width;
-        W.a[s] = W.C[s] / dt - W.G[s];
-        W.b[s] = W.bg[s];
-      }
-    }
+  for (uint32_t s = threadIdx.x; s < U.n_slot; s += kBlockThreads) {
+    a[s] = U.C[s] / dt - U.G[s];
+    b[s] = U.bg[s];
   }
-  for (uint32_t i = threadIdx.x; i < bi.n_syn; i += kThreads) W.syn_decay[i] = exp(-dt / W.syn_tau[i]);
+  if (!M.syn_uniform) {
+    double* decay = const_cast<double*>(U.syn_decay);
+    for (uint32_t i = threadIdx.x; i < U.n_syn; i += kBlockThreads) decay[i] = exp(-dt / U.syn_tau[i]);
+  }
 }
 
-// R4: gates start at their steady state for the initial voltage; detectors armed.
-__global__ void __launch_bounds__(kThreads) init_kernel(DevModel M) {
-  __shared__ BlockInfo bi;
-  if (threadIdx.x == 0) bi = M.blocks[blockIdx.x];
+// R4: gates start at their steady state for the initial voltage.
+__global__ void __launch_bounds__(kBlockThreads) init_kernel(DevModel M) {
+  __shared__ UnitHeader H;
+  const UnitDesc d = M.units[blockIdx.x];
+  if (threadIdx.x < sizeof(UnitHeader) / 4) ((uint32_t*)&H)[threadIdx.x] = ((const uint32_t*)(M.fast + d.fast_off))[threadIdx.x];
   __syncthreads();
-  View W = make_view(M, bi);
-  for (uint32_t i = threadIdx.x; i < bi.n_hh; i += kThreads) {
-    Rates r = hh_rates(W.V[W.hh_slot[i]]);
-    W.m[i] = r.am / (r.am + r.bm);
-    W.h[i] = r.ah / (r.ah + r.bh);
-    W.n[i] = r.an / (r.an + r.bn);
-  }
-  for (uint32_t i = threadIdx.x; i < bi.n_cell; i += kThreads) {
-    CellRt rt; rt.ev_cur = 0; rt.ev_end = 0; rt.armed = 1; rt.pad = 0;
-    M.cell_rt[bi.cell_base + i] = rt;
+  UnitView U;
+  make_view(U, M, H, M.fast + d.fast_off, M.state + d.state_base, M.topo + H.topo_off);
+  for (uint32_t i = threadIdx.x; i < U.n_hh; i += kBlockThreads) {
+    const Rates r = hh_rates(U.V[U.hh_slot[i]]);
+    U.m[i] = r.am / (r.am + r.bm);
+    U.h[i] = r.ah / (r.ah + r.bh);
+    U.n[i] = r.an / (r.an + r.bn);
   }
 }
 
 __global__ void reset_detectors_kernel(DevModel M) {
   int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-  if (c < M.n_cells) M.cell_rt[c].armed = 1;
-}
-
-// ------------------------------------------------------------------------------------------
-// The cable step.  One CTA per cell block; A.nk consecutive grid steps per launch.
-// ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kThreads) cable_kernel(DevModel M, StepArgs A) {
-  extern __shared__ double dyn_smem[];
-  __shared__ BlockInfo bi;
-  __shared__ double s_tcur[kMaxCells], s_tnext[kMaxCells], s_delta[kMaxCells], s_vprev[kMaxCells];
-  __shared__ uint32_t s_evcur[kMaxCells], s_evend[kMaxCells], s_armed[kMaxCells];
-  __shared__ uint8_t s_mode[kMaxCells];
-  __shared__ unsigned int s_substeps, s_delivered;
-  if (threadIdx.x == 0) { bi = M.blocks[blockIdx.x]; s_substeps = 0; s_delivered = 0; }
-  __syncthreads();
-  const View W = make_view(M, bi);
-  const uint32_t lanes_pad = align_up(bi.n_lane, 16);
-  double* contrib;
-  double* dcontrib;
-  if (bi.flags & 1u) {   // too many branches for shared memory: use the block's global scratch
-    contrib = M.scratch + bi.scratch_base + 2 * (int64_t)bi.n_slot;
-    dcontrib = contrib + lanes_pad;
-  } else {
-    contrib = dyn_smem;
-    dcontrib = dyn_smem + lanes_pad;
-  }
-  double* const extra = W.fgen;   // extra currents live here between phases B and B2
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const uint32_t n_cell = bi.n_cell;
-  if ((uint32_t)tid < n_cell) {
-    CellRt rt = M.cell_rt[bi.cell_base + tid];
-    s_evcur[tid] = rt.ev_cur; s_evend[tid] = rt.ev_end; s_armed[tid] = rt.armed;
-  }
-
-  for (int64_t k = A.k_first; k < A.k_first + A.nk; ++k) {
-    const double ta = (k == 0) ? A.t0 : __dadd_rn(A.t0, __dmul_rn((double)k, A.dt));
-    const double tb = (k + 1 == A.nsteps) ? A.t_end : __dadd_rn(A.t0, __dmul_rn((double)(k + 1), A.dt));
-    const bool nominal = (k + 1 < A.nsteps) || A.last_full;
-    if ((uint32_t)tid < n_cell) s_tcur[tid] = ta;
-    __syncthreads();
-    for (;;) {
-      // ---- phase A: deliver events due now, choose the sub-step (reading R9)
-      int active = 0;
-      if ((uint32_t)tid < n_cell) {
-        const double t = s_tcur[tid];
-        if (t < tb) {
-          uint32_t cur = s_evcur[tid];
-          const uint32_t end = s_evend[tid];
-          uint32_t ndel = 0;
-          while (cur < end && M.ev_t[cur] <= t) { M.state[M.ev_gidx[cur]] += M.ev_w[cur]; ++cur; ++ndel; }
-          s_evcur[tid] = cur;
-          double next = tb;
-          if (cur < end) { double te = M.ev_t[cur]; if (te < tb) next = te; }
-          const bool fast = nominal && t == ta && next == tb;
-          s_delta[tid] = fast ? A.dt : next - t;
-          s_mode[tid] = fast ? 1 : 2;
-          s_tnext[tid] = next;
-          s_vprev[tid] = W.V[W.cell_det[tid]];
-          active = 1;
-          atomicAdd(&s_substeps, 1u);
-          if (ndel) atomicAdd(&s_delivered, ndel);
-        } else {
-          s_mode[tid] = 0;
-        }
-      }
-      if (!__syncthreads_or(active)) break;
-
-      // ---- phase B: currents of HH, synapses and clamps from V(t)
-      for (uint32_t sp = tid; sp < bi.n_sp; sp += kThreads) {
-        const uint32_t c = W.sp_cell[sp];
-        if (!s_mode[c]) continue;
-        const double v = W.V[W.sp_slot[sp]];
-        double I = 0.0;
-        const int32_t hi = W.sp_hh[sp];
-        if (hi >= 0) {
-          const double m = W.m[hi], h = W.h[hi], n = W.n[hi];
-          I += W.hh_gna[hi] * m * m * m * h * (v - M.ena) + W.hh_gk[hi] * n * n * n * n * (v - M.ek) +
-               W.hh_gl[hi] * (v - M.el);
-        }
-        const uint32_t sb = W.sp_syn_beg[sp], sc = W.sp_syn_cnt[sp];
-        for (uint32_t j = 0; j < sc; ++j) I += W.g[sb + j] * (v - W.syn_e[sb + j]);
-        const uint32_t cb = W.sp_cl_beg[sp], cc = W.sp_cl_cnt[sp];
-        const double t = s_tcur[c];
-        for (uint32_t j = 0; j < cc; ++j)
-          if (W.cl_t0[cb + j] <= t && t < W.cl_t1[cb + j]) I -= W.cl_amp[cb + j];
-        extra[sp] = I;
-      }
-      __syncthreads();
-      // ---- phase C: rhs_i = (C_i/delta - G_i) V_i + G_i e_i, in place of V
-      for (uint32_t ti = warp; ti < bi.n_task; ti += kWarps) {
-        const Task T = W.tasks[ti];
-        if ((uint32_t)lane >= T.nlanes) continue;
-        const uint32_t tl = T.lane_off + lane;
-        const uint32_t c = W.br_cell[tl];
-        const uint32_t md = s_mode[c];
-        if (!md) continue;
-        const uint32_t len = W.br_len[tl];
-        uint32_t s = T.slot_off + lane;
-        if (md == 1) {
-          for (uint32_t q = 0; q < len; ++q, s += T.width) W.V[s] = fma(W.a[s], W.V[s], W.b[s]);
-        } else {
-          const double delta = s_delta[c];
-          for (uint32_t q = 0; q < len; ++q, s += T.width) W.V[s] = fma(W.C[s] / delta - W.G[s], W.V[s], W.bg[s]);
-        }
-      }
-      __syncthreads();
-      for (uint32_t sp = tid; sp < bi.n_sp; sp += kThreads)
-        if (s_mode[W.sp_cell[sp]]) W.V[W.sp_slot[sp]] -= extra[sp];
-      __syncthreads();
-      // ---- phase D: backward sweep, deepest level first
-      for (int lvl = (int)bi.n_level - 1; lvl >= 0; --lvl) {
-        for (uint32_t ti = W.level_begin[lvl] + warp; ti < W.level_begin[lvl + 1]; ti += kWarps) {
-          const Task T = W.tasks[ti];
-          if ((uint32_t)lane >= T.nlanes) continue;
-          const uint32_t tl = T.lane_off + lane;
-          const uint32_t c = W.br_cell[tl];
-          const uint32_t md = s_mode[c];
-          if (!md) continue;
-          const uint32_t len = W.br_len[tl];
-          const double* fp = W.f;
-          if (md == 2) { eliminate_branch(W, T, lane, tl, s_delta[c], W.fgen, W.invdgen, dcontrib); fp = W.fgen; }
-          uint32_t s = T.slot_off + lane + (len - 1) * T.width;
-          double r = W.V[s];
-          const uint32_t cb = W.br_cbeg[tl], cc = W.br_ccnt[tl];
-          for (uint32_t j = 0; j < cc; ++j) r -= contrib[W.child[cb + j]];
-          W.V[s] = r;
-          for (uint32_t q = len - 1; q > 0; --q) {
-            const double fq = fp[s];
-            s -= T.width;
-            r = fma(-fq, r, W.V[s]);
-            W.V[s] = r;
-          }
-          contrib[tl] = fp[s] * r;
-        }
-        __syncthreads();
-      }
-      // ---- phase E: forward substitution, root level first; V <- V'
-      for (uint32_t lvl = 0; lvl < bi.n_level; ++lvl) {
-        for (uint32_t ti = W.level_begin[lvl] + warp; ti < W.level_begin[lvl + 1]; ti += kWarps) {
-          const Task T = W.tasks[ti];
-          if ((uint32_t)lane >= T.nlanes) continue;
-          const uint32_t tl = T.lane_off + lane;
-          const uint32_t md = s_mode[W.br_cell[tl]];
-          if (!md) continue;
-          const uint32_t len = W.br_len[tl];
-          const double* fp = md == 1 ? W.f : W.fgen;
-          const double* ip = md == 1 ? W.invd : W.invdgen;
-          const uint32_t ps = W.br_pslot[tl];
-          double vp = ps == kNoSlot ? 0.0 : W.V[ps];
-          uint32_t s = T.slot_off + lane;
-          for (uint32_t q = 0; q < len; ++q, s += T.width) {
-            vp = fma(-fp[s], vp, W.V[s] * ip[s]);
-            W.V[s] = vp;
-          }
-        }
-        __syncthreads();
-      }
-      // ---- phase F: state update with V', threshold test
-      for (uint32_t i = tid; i < bi.n_hh; i += kThreads) {
-        const uint32_t c = W.hh_cell[i];
-        if (!s_mode[c]) continue;
-        const double delta = s_delta[c];
-        const Rates r = hh_rates(W.V[W.hh_slot[i]]);
-        double inf = r.am / (r.am + r.bm);
-        W.m[i] = inf + (W.m[i] - inf) * exp(-delta * (r.am + r.bm));
-        inf = r.ah / (r.ah + r.bh);
-        W.h[i] = inf + (W.h[i] - inf) * exp(-delta * (r.ah + r.bh));
-        inf = r.an / (r.an + r.bn);
-        W.n[i] = inf + (W.n[i] - inf) * exp(-delta * (r.an + r.bn));
-      }
-      for (uint32_t i = tid; i < bi.n_syn; i += kThreads) {
-        const uint32_t c = W.syn_cell[i];
-        const uint32_t md = s_mode[c];
-        if (!md) continue;
-        W.g[i] = W.g[i] * (md == 1 ? W.syn_decay[i] : exp(-s_delta[c] / W.syn_tau[i]));
-      }
-      if ((uint32_t)tid < n_cell && s_mode[tid]) {
-        const double vd = W.V[W.cell_det[tid]], vp = s_vprev[tid];
-        if (s_armed[tid] && vp < M.theta && M.theta <= vd) {
-          const double ts = s_tcur[tid] + s_delta[tid] * (M.theta - vp) / (vd - vp);
-          const unsigned long long pos = atomicAdd(&M.counters[CNT_SPIKES], 1ull);
-          if ((int64_t)pos < M.spike_cap) { M.spike_cell[pos] = M.cell_orig[bi.cell_base + tid]; M.spike_t[pos] = ts; }
-          else atomicOr(&M.counters[CNT_ERROR], 1ull);
-          s_armed[tid] = 0;
-        }
-        if (vd < M.theta) s_armed[tid] = 1;
-        s_tcur[tid] = s_tnext[tid];
-      }
-      __syncthreads();
-    }
-  }
-  if ((uint32_t)tid < n_cell) {
-    CellRt rt; rt.ev_cur = s_evcur[tid]; rt.ev_end = s_evend[tid]; rt.armed = s_armed[tid]; rt.pad = 0;
-    M.cell_rt[bi.cell_base + tid] = rt;
-  }
-  if (tid == 0) {
-    atomicAdd(&M.counters[CNT_SUBSTEPS], (unsigned long long)s_substeps);
-    if (s_delivered) atomicAdd(&M.counters[CNT_DELIVERED], (unsigned long long)s_delivered);
-  }
+  if (c < M.n_cells) M.state[M.cell_rt_idx[c] + 2] = 1.0;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -467,9 +831,8 @@ __global__ void ev_place_kernel(DevModel M, double t_win) {
   }
   const uint32_t total = M.ev_fill[c];
   M.ev_fill[c] = q;
-  CellRt rt = M.cell_rt[c];
-  rt.ev_cur = off; rt.ev_end = ok ? off + total : off;
-  M.cell_rt[c] = rt;
+  const unsigned long long pk = ((unsigned long long)(ok ? off + total : off) << 32) | off;
+  M.state[M.cell_rt_idx[c] + 1] = __longlong_as_double((long long)pk);
 }
 
 __global__ void ev_scatter_pool_kernel(DevModel M, int cur, double t_win) {
@@ -487,11 +850,14 @@ __global__ void ev_scatter_pool_kernel(DevModel M, int cur, double t_win) {
   }
 }
 
-// per cell: order by (time, synapse, weight) - lists are a handful of events long
+// per cell: order by (time, synapse, weight) - lists are a handful of events long - and publish the
+// time of the first one
 __global__ void ev_sort_kernel(DevModel M) {
   int64_t c = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (c >= M.n_cells) return;
-  const uint32_t b = M.cell_rt[c].ev_cur, e = M.cell_rt[c].ev_end;
+  double* rt = M.state + M.cell_rt_idx[c];
+  const unsigned long long pk = (unsigned long long)__double_as_longlong(rt[1]);
+  const uint32_t b = (uint32_t)pk, e = (uint32_t)(pk >> 32);
   for (uint32_t i = b + 1; i < e; ++i) {
     const double t = M.ev_t[i], w = M.ev_w[i];
     const uint32_t g = M.ev_gidx[i];
@@ -506,6 +872,7 @@ __global__ void ev_sort_kernel(DevModel M) {
     }
     M.ev_t[j] = t; M.ev_gidx[j] = g; M.ev_w[j] = w;
   }
+  rt[0] = b < e ? M.ev_t[b] : CUDART_INF;
 }
 
 __global__ void pool_swap_kernel(DevModel M) {
@@ -539,16 +906,16 @@ inline unsigned grid_for(int64_t n, int block) { return (unsigned)((n + block - 
 
 }  // namespace
 
-int cable_smem_bytes(uint32_t max_block_lanes) { return (int)(2 * align_up(max_block_lanes, 16) * sizeof(double)); }
-int cable_smem_limit() { return 160 * 1024; }
+int cable_smem_limit() { return 227 * 1024; }
+int cable_max_warps() { return kMaxWarpsPerCta; }
 
 cudaError_t launch_factor(const DevModel& M, double dt, cudaStream_t s) {
-  factor_kernel<<<(unsigned)M.n_blocks, kThreads, 0, s>>>(M, dt);
+  factor_kernel<<<(unsigned)M.n_units, kBlockThreads, 0, s>>>(M, dt);
   return cudaGetLastError();
 }
 
 cudaError_t launch_init(const DevModel& M, cudaStream_t s) {
-  init_kernel<<<(unsigned)M.n_blocks, kThreads, 0, s>>>(M);
+  init_kernel<<<(unsigned)M.n_units, kBlockThreads, 0, s>>>(M);
   return cudaGetLastError();
 }
 
@@ -557,14 +924,22 @@ cudaError_t launch_reset_detectors(const DevModel& M, cudaStream_t s) {
   return cudaGetLastError();
 }
 
-cudaError_t launch_cable(const DevModel& M, const StepArgs& A, int dyn_smem, cudaStream_t s) {
-  static int configured = -1;
-  if (dyn_smem > 48 * 1024 && configured < dyn_smem) {
-    cudaError_t e = cudaFuncSetAttribute(cable_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, dyn_smem);
-    if (e != cudaSuccess) return e;
-    configured = dyn_smem;
+cudaError_t launch_cable(const DevModel& M, const StepArgs& A, int grid, cudaStream_t s, int* launches) {
+  if (M.n_warp_units > 0) {
+    const int smem = (int)(M.plan.warps * M.plan.warp_bytes);
+    static int configured = -1;
+    if (smem > 48 * 1024 && configured < smem) {
+      cudaError_t e = cudaFuncSetAttribute(cable_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+      if (e != cudaSuccess) return e;
+      configured = smem;
+    }
+    cable_warp_kernel<<<(unsigned)grid, (unsigned)(M.plan.warps * 32), smem, s>>>(M, A);
+    if (launches) ++*launches;
   }
-  cable_kernel<<<(unsigned)M.n_blocks, kThreads, dyn_smem, s>>>(M, A);
+  if (M.n_units > M.n_warp_units) {
+    cable_block_kernel<<<(unsigned)(M.n_units - M.n_warp_units), kBlockThreads, 0, s>>>(M, A);
+    if (launches) ++*launches;
+  }
   return cudaGetLastError();
 }
 

@@ -3,7 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#include "block_layout.h"
+#include "unit_layout.h"
 
 namespace arbb {
 
@@ -22,15 +22,18 @@ enum Counter {
 struct EventPool { double* t; uint32_t* dst; uint32_t* gidx; double* w; };
 
 struct DevModel {
-  const BlockInfo* blocks;
-  int64_t n_blocks, n_cells;
-  double* gen;
-  double* fast;
+  const UnitDesc* units;      // warp units first, then block units
+  int64_t n_units, n_warp_units, n_cells;
+  uint8_t* fast;
   double* state;
-  const uint8_t* meta;
-  double* scratch;
-  CellRt* cell_rt;            // [n_cells] internal order
+  const double* gen;
+  const uint8_t* topo;
+  double* scratch;            // block units: contrib | dcontrib | xI | fgen | invdgen at header.scratch_base
+  double* warp_scratch;       // warp kernel: per resident warp fgen | invdgen | dcontrib
+  int64_t warp_scratch_stride;
+  double* factor_dcontrib;    // [total branches], used by factor_kernel only
   const uint32_t* cell_orig;  // internal -> caller's cell id
+  const uint32_t* cell_rt_idx;// internal cell -> state index of its runtime triple
   // epoch event list (CSR over internal cells)
   uint32_t* ev_off;           // [n_cells + 1]
   double* ev_t; uint32_t* ev_gidx; double* ev_w;
@@ -48,7 +51,11 @@ struct DevModel {
   uint32_t* spike_cell; double* spike_t; int64_t spike_cap;
   unsigned long long* counters;
   uint32_t* scan_tmp;         // block sums for the offsets scan
+  // synapse parameters when every synapse of the model has the same tau and e
+  int syn_uniform;
+  double syn_e_u, syn_tau_u, syn_decay_u;
   double ena, ek, el, theta;
+  WarpSmemPlan plan;
 };
 
 struct StepArgs {
@@ -60,7 +67,8 @@ struct StepArgs {
 // all launchers queue work on `s` and return the last CUDA error code
 cudaError_t launch_factor(const DevModel& M, double dt, cudaStream_t s);
 cudaError_t launch_init(const DevModel& M, cudaStream_t s);
-cudaError_t launch_cable(const DevModel& M, const StepArgs& A, int dyn_smem, cudaStream_t s);
+// the cable step: a persistent grid of `grid` CTAs of plan.warps warps for the warp units, one CTA per block unit
+cudaError_t launch_cable(const DevModel& M, const StepArgs& A, int grid, cudaStream_t s, int* launches);
 cudaError_t launch_build_events(const DevModel& M, int cur_pool, double t_window_end, cudaStream_t s, int* launches);
 cudaError_t launch_spikes_to_events(const DevModel& M, int cur_pool, cudaStream_t s, int* launches);
 cudaError_t launch_gather(const double* state, const uint32_t* idx, int64_t n, double* out, cudaStream_t s);
@@ -70,7 +78,7 @@ cudaError_t launch_gather_hh(const double* state, const uint32_t* m_idx, const u
 cudaError_t launch_scatter_hh(double* state, const uint32_t* m_idx, const uint32_t* stride, const uint32_t* cv,
                               int which, int64_t n_hh, const double* in, cudaStream_t s);
 cudaError_t launch_reset_detectors(const DevModel& M, cudaStream_t s);
-int cable_smem_bytes(uint32_t max_block_lanes);
-int cable_smem_limit();
+int cable_smem_limit();       // bytes of dynamic shared memory a CTA of the warp kernel may use
+int cable_max_warps();        // warps per CTA the warp kernel is compiled for
 
 }  // namespace arbb

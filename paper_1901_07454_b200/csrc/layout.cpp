@@ -7,6 +7,7 @@
 #include <cstring>
 #include <limits>
 #include <thread>
+#include <unordered_map>
 
 namespace arbb {
 
@@ -45,6 +46,12 @@ struct Lane {          // one branch of one cell of the block
 struct CellScratch {
   uint32_t lane_begin = 0, n_br = 0;  // lanes of this cell are [lane_begin, lane_begin + n_br) before sorting
 };
+
+uint64_t fnv1a(const uint8_t* p, size_t n) {
+  uint64_t h = 1469598103934665603ull;
+  for (size_t i = 0; i < n; ++i) { h ^= p[i]; h *= 1099511628211ull; }
+  return h;
+}
 
 }  // namespace
 
@@ -122,8 +129,8 @@ int validate(const arb_desc& d, std::string& err) {
 
 namespace {
 
-// Everything about one block.  Called twice: counts only (plan), then with the pools to fill.
-struct BlockBuilder {
+// Everything about one unit.  Called twice: counts + topo record (plan), then with the pools to fill.
+struct UnitBuilder {
   const arb_desc& d;
   const BuildParams& P;
   const HostModel& H;
@@ -132,8 +139,17 @@ struct BlockBuilder {
 
   std::vector<Lane> lanes;
   std::vector<uint32_t> cvs;               // CV lists of all lanes
-  std::vector<uint32_t> nchild, br_of;
+  std::vector<uint32_t> nchild, br_of, blen;
   std::vector<CellScratch> cells;
+  // layout of the unit
+  std::vector<uint32_t> order, tl_of, task_of, row_begin, rowoff;
+  std::vector<Task> tasks;
+  std::vector<uint32_t> level_begin;
+  bool bad = false;                        // a count does not fit its field
+
+  bool has_hh(int64_t gi) const {
+    return d.hh_gnabar && (d.hh_gnabar[gi] != 0.0 || d.hh_gkbar[gi] != 0.0 || d.hh_gl[gi] != 0.0);
+  }
 
   void decompose(int64_t cell_begin, uint32_t n_cell) {
     lanes.clear(); cvs.clear(); cells.assign(n_cell, CellScratch());
@@ -144,14 +160,13 @@ struct BlockBuilder {
       const int32_t* par = d.cv_parent + a;
       nchild.assign(n, 0);
       br_of.assign(n, 0);
+      blen.clear();
       for (uint32_t i = 1; i < n; ++i) nchild[par[i]]++;
       cells[lc].lane_begin = (uint32_t)lanes.size();
       // pass 1: branch id of every CV (parent < index, so one forward sweep suffices)
-      const std::vector<uint32_t>& nch = nchild;
       uint32_t nb = 0;
-      std::vector<uint32_t> blen;
       for (uint32_t i = 0; i < n; ++i) {
-        bool fresh = (i == 0) || nch[par[i]] != 1 || blen[br_of[par[i]]] >= P.max_branch_len;
+        bool fresh = (i == 0) || nchild[par[i]] != 1 || blen[br_of[par[i]]] >= P.max_branch_len;
         if (fresh) {
           Lane L;
           L.lc = lc; L.br = nb; L.len = 0; L.first_cv = i;
@@ -185,17 +200,10 @@ struct BlockBuilder {
     }
   }
 
-  // Builds block `b`.  When pools are given (fill), writes them; always returns the counts.
-  BlockInfo run(int64_t cell_begin, uint32_t n_cell, const BlockInfo* placed, HostModel* out, int64_t hh_global) {
-    decompose(cell_begin, n_cell);
-    BlockInfo bi;
-    std::memset(&bi, 0, sizeof bi);
-    if (placed) bi = *placed;
-    bi.cell_base = cell_begin;
-    bi.n_cell = n_cell;
+  // tasks and ragged rows (unit_layout.h)
+  uint32_t make_tasks() {
     const uint32_t n_lane = (uint32_t)lanes.size();
-    // order of lanes inside the block: level, then longest first (sliced-ELL style padding)
-    std::vector<uint32_t> order(n_lane);
+    order.resize(n_lane);
     for (uint32_t i = 0; i < n_lane; ++i) order[i] = i;
     std::stable_sort(order.begin(), order.end(), [&](uint32_t x, uint32_t y) {
       const Lane &A = lanes[x], &B = lanes[y];
@@ -203,11 +211,11 @@ struct BlockBuilder {
       if (A.len != B.len) return A.len > B.len;
       return x < y;
     });
-    std::vector<uint32_t> tl_of(n_lane);   // unsorted lane -> block-local lane index
+    tl_of.resize(n_lane);
     for (uint32_t t = 0; t < n_lane; ++t) tl_of[order[t]] = t;
-    std::vector<Task> tasks;
-    std::vector<uint32_t> level_begin;
-    uint32_t slot = 0, n_level = 0;
+    tasks.clear(); level_begin.clear(); row_begin.clear(); rowoff.clear();
+    task_of.resize(n_lane);
+    uint32_t slot = 0;
     for (uint32_t t = 0; t < n_lane;) {
       uint32_t lvl = lanes[order[t]].level;
       while (level_begin.size() <= lvl) level_begin.push_back((uint32_t)tasks.size());
@@ -215,102 +223,144 @@ struct BlockBuilder {
       while (e < n_lane && e - t < 32 && lanes[order[e]].level == lvl) ++e;
       Task T;
       T.slot_off = slot; T.lane_off = t; T.nlanes = (uint16_t)(e - t);
-      T.width = (uint16_t)align_up(e - t, 4);
-      T.maxlen = (uint16_t)lanes[order[t]].len; T.level = (uint16_t)lvl;
-      slot += (uint32_t)T.maxlen * T.width;
+      const uint32_t maxlen = lanes[order[t]].len;
+      T.maxlen_full = (uint16_t)(maxlen | (lanes[order[e - 1]].len == maxlen ? kTaskFull : 0));
+      row_begin.push_back((uint32_t)rowoff.size());
+      uint32_t acc = 0;
+      for (uint32_t k = 0; k < maxlen; ++k) {
+        rowoff.push_back(acc);
+        uint32_t cnt = 0;
+        for (uint32_t l = t; l < e; ++l) cnt += lanes[order[l]].len > k;
+        acc += cnt;
+      }
+      T.nslots = acc;
+      for (uint32_t l = t; l < e; ++l) task_of[l] = (uint32_t)tasks.size();
+      slot += acc;
       tasks.push_back(T);
-      n_level = lvl + 1;
       t = e;
     }
     level_begin.push_back((uint32_t)tasks.size());
-    bi.n_slot = align_up(slot, 16);
-    bi.n_lane = n_lane;
-    bi.n_task = (uint32_t)tasks.size();
-    bi.n_level = n_level;
-    // counts of mechanisms
-    uint32_t n_hh = 0, n_syn = 0, n_clamp = 0, n_sp = 0, n_child = 0;
+    return slot;
+  }
+
+  uint32_t slot_of(uint32_t tl, uint32_t k) const {
+    const uint32_t ti = task_of[tl];
+    return tasks[ti].slot_off + rowoff[row_begin[ti] + k] + (tl - tasks[ti].lane_off);
+  }
+
+  UnitCounts run(int64_t cell_begin, uint32_t n_cell, std::vector<uint8_t>* topo_out, const UnitCounts* placed, HostModel* out) {
+    decompose(cell_begin, n_cell);
+    UnitCounts uc;
+    if (placed) uc = *placed;
+    uc.cell_base = cell_begin;
+    uc.n_cell = n_cell;
+    const uint32_t n_lane = (uint32_t)lanes.size();
+    uc.n_cv = make_tasks();
+    uc.n_slot = align_up(uc.n_cv, 2);
+    uc.n_lane = n_lane;
+    uc.n_task = (uint32_t)tasks.size();
+    uc.n_level = (uint32_t)level_begin.size() - 1;
+    uint32_t n_hh = 0, n_syn = 0, n_clamp = 0, n_child = 0;
     for (uint32_t i = 0; i < n_lane; ++i) n_child += lanes[i].parent_br >= 0 ? 1 : 0;
     for (uint32_t lc = 0; lc < n_cell; ++lc) {
       int64_t orig = H.cell_order[cell_begin + lc];
       int64_t a = d.cv_off[orig];
       uint32_t n = (uint32_t)(d.cv_off[orig + 1] - a);
-      std::vector<uint8_t> flag(n, 0);
-      if (d.hh_gnabar)
-        for (uint32_t i = 0; i < n; ++i)
-          if (d.hh_gnabar[a + i] != 0.0 || d.hh_gkbar[a + i] != 0.0 || d.hh_gl[a + i] != 0.0) { flag[i] = 1; ++n_hh; }
-      if (d.syn_off) {
-        for (int64_t s = d.syn_off[orig]; s < d.syn_off[orig + 1]; ++s) flag[d.syn_cv[s]] = 1;
-        n_syn += (uint32_t)(d.syn_off[orig + 1] - d.syn_off[orig]);
-      }
-      for (int64_t q = clamp_off[orig]; q < clamp_off[orig + 1]; ++q) flag[d.clamp_cv[clamp_idx[q]]] = 1;
+      for (uint32_t i = 0; i < n; ++i) n_hh += has_hh(a + i);
+      if (d.syn_off) n_syn += (uint32_t)(d.syn_off[orig + 1] - d.syn_off[orig]);
       n_clamp += (uint32_t)(clamp_off[orig + 1] - clamp_off[orig]);
-      for (uint32_t i = 0; i < n; ++i) n_sp += flag[i];
     }
-    bi.n_hh = n_hh; bi.n_syn = n_syn; bi.n_clamp = n_clamp; bi.n_sp = n_sp; bi.n_child = n_child;
-    MetaOff mo = meta_offsets(bi);
-    bi.meta_bytes = mo.total;
-    if (!out) return bi;
+    uc.n_hh = n_hh; uc.n_syn = n_syn; uc.n_clamp = n_clamp; uc.n_child = n_child;
+    const FastOff fo = fast_offsets(uc.n_slot, n_hh, n_syn, n_clamp, n_cell, H.syn_uniform);
+    const StateOff so = state_offsets(uc.n_slot, n_hh, n_syn, n_cell);
+    uc.fast_bytes = fo.total;
+    uc.state_bytes = 8 * so.total;
 
-    // ------------------------------------------------------------------ fill
-    FastOff fo = fast_offsets(bi);
-    StateOff so = state_offsets(bi);
-    GenOff go = gen_offsets(bi);
-    double* gen = out->gen.data() + bi.gen_base;
-    double* fast = out->fast.data() + bi.fast_base;
-    double* st = out->state.data() + bi.state_base;
-    uint8_t* meta = out->meta.data() + bi.meta_base;
-    std::memcpy(meta + mo.tasks, tasks.data(), tasks.size() * sizeof(Task));
-    std::memcpy(meta + mo.level_begin, level_begin.data(), level_begin.size() * 4);
-    uint32_t* br_pslot = (uint32_t*)(meta + mo.br_pslot);
-    uint32_t* br_cbeg = (uint32_t*)(meta + mo.br_cbeg);
-    uint16_t* br_len = (uint16_t*)(meta + mo.br_len);
-    uint16_t* br_cell = (uint16_t*)(meta + mo.br_cell);
-    uint16_t* br_ccnt = (uint16_t*)(meta + mo.br_ccnt);
-    uint32_t* child = (uint32_t*)(meta + mo.child);
-    uint32_t* cell_det = (uint32_t*)(meta + mo.cell_det);
-    uint32_t* hh_slot = (uint32_t*)(meta + mo.hh_slot);
-    uint16_t* hh_cell = (uint16_t*)(meta + mo.hh_cell);
-    uint16_t* syn_cell = (uint16_t*)(meta + mo.syn_cell);
-    uint32_t* sp_slot = (uint32_t*)(meta + mo.sp_slot);
-    int32_t* sp_hh = (int32_t*)(meta + mo.sp_hh);
-    uint32_t* sp_syn_beg = (uint32_t*)(meta + mo.sp_syn_beg);
-    uint32_t* sp_cl_beg = (uint32_t*)(meta + mo.sp_cl_beg);
-    uint16_t* sp_syn_cnt = (uint16_t*)(meta + mo.sp_syn_cnt);
-    uint16_t* sp_cl_cnt = (uint16_t*)(meta + mo.sp_cl_cnt);
-    uint16_t* sp_cell = (uint16_t*)(meta + mo.sp_cell);
-
-    // slot of lane t, position k
-    std::vector<uint32_t> task_of(n_lane);
-    for (uint32_t ti = 0; ti < tasks.size(); ++ti)
-      for (uint32_t l = 0; l < tasks[ti].nlanes; ++l) task_of[tasks[ti].lane_off + l] = ti;
-    auto slot_of = [&](uint32_t tl, uint32_t k) {
-      const Task& T = tasks[task_of[tl]];
-      return T.slot_off + k * (uint32_t)T.width + (tl - T.lane_off);
-    };
-    // children lists: for each parent lane, its child lanes in DESCENDING first-CV order (the
-    // order in which a leaves->root elimination meets them)
+    // children lists: for each parent lane, its child lanes in DESCENDING first-CV order (the order
+    // in which a leaves->root elimination meets them)
     std::vector<std::vector<uint32_t>> kids(n_lane);
     for (uint32_t i = 0; i < n_lane; ++i)
       if (lanes[i].parent_br >= 0) kids[cells[lanes[i].lc].lane_begin + lanes[i].parent_br].push_back(i);
-    uint32_t cpos = 0;
-    for (uint32_t i = 0; i < n_lane; ++i) {
-      uint32_t tl = tl_of[i];
-      const Lane& L = lanes[i];
-      br_len[tl] = (uint16_t)L.len;
-      br_cell[tl] = (uint16_t)L.lc;
-      if (L.parent_br >= 0) {
-        uint32_t pi = cells[L.lc].lane_begin + L.parent_br;
-        br_pslot[tl] = slot_of(tl_of[pi], lanes[pi].len - 1);
-      } else {
-        br_pslot[tl] = kNoSlot;
+
+    if (topo_out) {
+      const TopoOff to = topo_offsets(uc.n_task, uc.n_level, n_lane, n_child, n_cell);
+      topo_out->assign(to.total, 0);
+      uint8_t* tp = topo_out->data();
+      std::memcpy(tp + to.tasks, tasks.data(), tasks.size() * sizeof(Task));
+      std::memcpy(tp + to.level_begin, level_begin.data(), level_begin.size() * 4);
+      LaneRec* lrec = (LaneRec*)(tp + to.lanes);
+      uint32_t* child = (uint32_t*)(tp + to.child);
+      uint32_t* cell_det = (uint32_t*)(tp + to.cell_det);
+      uint32_t cpos = 0;
+      for (uint32_t tl = 0; tl < n_lane; ++tl) {       // in unit-local branch order
+        const uint32_t i = order[tl];
+        const Lane& L = lanes[i];
+        LaneRec& R = lrec[tl];
+        R.len = (uint16_t)L.len;
+        R.cell = (uint16_t)L.lc;
+        R.pad = 0;
+        if (L.parent_br >= 0) {
+          uint32_t pi = cells[L.lc].lane_begin + L.parent_br;
+          R.pslot = slot_of(tl_of[pi], lanes[pi].len - 1);
+        } else {
+          R.pslot = kNoSlot;
+        }
+        std::sort(kids[i].begin(), kids[i].end(), [&](uint32_t x, uint32_t y) { return lanes[x].first_cv > lanes[y].first_cv; });
+        R.cbeg = cpos;
+        if (kids[i].size() > 65535) bad = true;
+        R.ccnt = (uint16_t)std::min<size_t>(kids[i].size(), 65535);
+        for (uint32_t k : kids[i]) child[cpos++] = tl_of[k];
       }
-      std::sort(kids[i].begin(), kids[i].end(), [&](uint32_t x, uint32_t y) { return lanes[x].first_cv > lanes[y].first_cv; });
-      br_cbeg[tl] = cpos;
-      br_ccnt[tl] = (uint16_t)kids[i].size();
-      for (uint32_t k : kids[i]) child[cpos++] = tl_of[k];
+      for (uint32_t lc = 0; lc < n_cell; ++lc) {
+        int64_t orig = H.cell_order[cell_begin + lc];
+        uint32_t det = d.det_cv ? (uint32_t)d.det_cv[orig] : 0u;
+        // slot of the detector CV: find its branch
+        const uint32_t lb = cells[lc].lane_begin;
+        uint32_t found = kNoSlot;
+        for (uint32_t b2 = 0; b2 < cells[lc].n_br && found == kNoSlot; ++b2) {
+          const Lane& L = lanes[lb + b2];
+          if (det < L.first_cv) continue;
+          for (uint32_t k = 0; k < L.len; ++k)
+            if (cvs[L.cv_begin + k] == det) { found = slot_of(tl_of[lb + b2], k); break; }
+        }
+        cell_det[lc] = found;
+      }
     }
-    // per CV: slot, constants, initial state
-    uint32_t hh_pos = 0, syn_pos = 0, cl_pos = 0, sp_pos = 0;
+    if (!out) return uc;
+
+    // ------------------------------------------------------------------ fill
+    const GenOff go = gen_offsets(uc.n_slot, n_syn);
+    uint8_t* fast = out->fast.data() + uc.fast_off;
+    double* st = out->state.data() + uc.state_base;
+    double* gen = out->gen.data() + uc.gen_base;
+    UnitHeader hd;
+    std::memset(&hd, 0, sizeof hd);
+    hd.n_slot = uc.n_slot; hd.n_lane = n_lane; hd.n_task = uc.n_task; hd.n_level = uc.n_level;
+    hd.n_cell = n_cell; hd.n_hh = n_hh; hd.n_syn = n_syn; hd.n_clamp = n_clamp;
+    hd.n_child = n_child; hd.flags = uc.flags; hd.fast_bytes = uc.fast_bytes; hd.state_bytes = uc.state_bytes;
+    hd.topo_off = uc.topo_off; hd.gen_base = uc.gen_base; hd.state_base = uc.state_base;
+    hd.cell_base = uc.cell_base; hd.scratch_base = uc.scratch_base;
+    hd.pad[0] = (uint32_t)(uc.lane_base & 0xFFFFFFFFu); hd.pad[1] = (uint32_t)((uint64_t)uc.lane_base >> 32);
+    std::memcpy(fast, &hd, sizeof hd);
+    double* hh_gna = (double*)(fast + fo.hh_gna);
+    double* hh_gk = (double*)(fast + fo.hh_gk);
+    double* hh_gl = (double*)(fast + fo.hh_gl);
+    double* syn_e = (double*)(fast + fo.syn_e);
+    double* cl_t0 = (double*)(fast + fo.cl_t0);
+    double* cl_t1 = (double*)(fast + fo.cl_t1);
+    double* cl_amp = (double*)(fast + fo.cl_amp);
+    uint32_t* hh_slot = (uint32_t*)(fast + fo.hh_slot);
+    uint32_t* syn_slot = (uint32_t*)(fast + fo.syn_slot);
+    uint32_t* cl_slot = (uint32_t*)(fast + fo.cl_slot);
+    uint16_t* hh_cell = (uint16_t*)(fast + fo.hh_cell);
+    uint16_t* syn_cell = (uint16_t*)(fast + fo.syn_cell);
+    uint16_t* cl_cell = (uint16_t*)(fast + fo.cl_cell);
+    const bool multi = n_cell > 1;
+
+    struct Item { uint32_t slot, lc; int64_t id; };
+    std::vector<Item> syn_items, cl_items;
+    syn_items.reserve(n_syn); cl_items.reserve(n_clamp);
+    uint32_t hh_pos = 0;
     for (uint32_t lc = 0; lc < n_cell; ++lc) {
       int64_t orig = H.cell_order[cell_begin + lc];
       int64_t a = d.cv_off[orig];
@@ -335,53 +385,52 @@ struct BlockBuilder {
         gen[go.G + s] = G;
         gen[go.b + s] = d.pas_g ? G * d.pas_e[a + i] : 0.0;           // nA
         st[so.v + s] = d.cv_vinit ? d.cv_vinit[a + i] : -65.0;
-        out->cv_state_idx[a + i] = (uint32_t)(bi.state_base + so.v + s);
-      }
-      cell_det[lc] = cv_slot[d.det_cv ? d.det_cv[orig] : 0];
-      // mechanisms, grouped per CV in ascending CV order; synapses and clamps ascending inside a CV
-      std::vector<std::vector<int64_t>> syn_on(n), cl_on(n);
-      if (d.syn_off)
-        for (int64_t s = d.syn_off[orig]; s < d.syn_off[orig + 1]; ++s) syn_on[d.syn_cv[s]].push_back(s);
-      for (int64_t q = clamp_off[orig]; q < clamp_off[orig + 1]; ++q) cl_on[d.clamp_cv[clamp_idx[q]]].push_back(clamp_idx[q]);
-      for (uint32_t i = 0; i < n; ++i) {
-        bool hh = d.hh_gnabar && (d.hh_gnabar[a + i] != 0.0 || d.hh_gkbar[a + i] != 0.0 || d.hh_gl[a + i] != 0.0);
-        if (!hh && syn_on[i].empty() && cl_on[i].empty()) continue;
-        sp_slot[sp_pos] = cv_slot[i];
-        sp_cell[sp_pos] = (uint16_t)lc;
-        sp_hh[sp_pos] = hh ? (int32_t)hh_pos : -1;
-        if (hh) {
-          double sc = d.cv_area[a + i] * 1e-2;
-          fast[fo.hh_gna + hh_pos] = d.hh_gnabar[a + i] * sc;
-          fast[fo.hh_gk + hh_pos] = d.hh_gkbar[a + i] * sc;
-          fast[fo.hh_gl + hh_pos] = d.hh_gl[a + i] * sc;
-          hh_slot[hh_pos] = cv_slot[i];
-          hh_cell[hh_pos] = (uint16_t)lc;
-          out->hh_m_idx[hh_global + hh_pos] = (uint32_t)(bi.state_base + so.m + hh_pos);
-          out->hh_stride[hh_global + hh_pos] = so.h - so.m;
-          out->hh_cv[hh_global + hh_pos] = (uint32_t)(a + i);
+        out->cv_state_idx[a + i] = (uint32_t)(uc.state_base + so.v + s);
+        if (has_hh(a + i)) {
+          double sc = area * 1e-2;
+          hh_gna[hh_pos] = d.hh_gnabar[a + i] * sc;
+          hh_gk[hh_pos] = d.hh_gkbar[a + i] * sc;
+          hh_gl[hh_pos] = d.hh_gl[a + i] * sc;
+          hh_slot[hh_pos] = s;
+          if (multi) hh_cell[hh_pos] = (uint16_t)lc;
+          out->hh_m_idx[uc.hh_base + hh_pos] = (uint32_t)(uc.state_base + so.m + hh_pos);
+          out->hh_stride[uc.hh_base + hh_pos] = so.h - so.m;
+          out->hh_cv[uc.hh_base + hh_pos] = (uint32_t)(a + i);
           ++hh_pos;
         }
-        sp_syn_beg[sp_pos] = syn_pos;
-        sp_syn_cnt[sp_pos] = (uint16_t)std::min<size_t>(syn_on[i].size(), 65535);
-        for (int64_t s : syn_on[i]) {
-          fast[fo.syn_e + syn_pos] = d.syn_e[s];
-          fast[fo.syn_tau + syn_pos] = d.syn_tau[s];
-          syn_cell[syn_pos] = (uint16_t)lc;
-          out->syn_state_idx[s] = (uint32_t)(bi.state_base + so.g + syn_pos);
-          ++syn_pos;
-        }
-        sp_cl_beg[sp_pos] = cl_pos;
-        sp_cl_cnt[sp_pos] = (uint16_t)std::min<size_t>(cl_on[i].size(), 65535);
-        for (int64_t k : cl_on[i]) {
-          fast[fo.cl_t0 + cl_pos] = d.clamp_t0[k];
-          fast[fo.cl_t1 + cl_pos] = d.clamp_t1[k];
-          fast[fo.cl_amp + cl_pos] = d.clamp_amp[k];
-          ++cl_pos;
-        }
-        ++sp_pos;
       }
+      if (d.syn_off)
+        for (int64_t s = d.syn_off[orig]; s < d.syn_off[orig + 1]; ++s) syn_items.push_back({cv_slot[d.syn_cv[s]], lc, s});
+      for (int64_t q = clamp_off[orig]; q < clamp_off[orig + 1]; ++q) cl_items.push_back({cv_slot[d.clamp_cv[clamp_idx[q]]], lc, clamp_idx[q]});
+      // runtime triple: no event pending, empty segment, detector armed (reading R10)
+      double* rt = st + so.rt + kRtDoubles * lc;
+      rt[0] = std::numeric_limits<double>::infinity();
+      rt[1] = 0.0;
+      rt[2] = 1.0;
+      out->cell_rt_idx[cell_begin + lc] = (uint32_t)(uc.state_base + so.rt + kRtDoubles * lc);
     }
-    return bi;
+    // point mechanisms sorted by (slot, caller's index): the items on one CV form a run that one
+    // lane sums in ascending index order
+    auto by_slot = [](const Item& x, const Item& y) { return x.slot != y.slot ? x.slot < y.slot : x.id < y.id; };
+    std::sort(syn_items.begin(), syn_items.end(), by_slot);
+    std::sort(cl_items.begin(), cl_items.end(), by_slot);
+    for (uint32_t p = 0; p < syn_items.size(); ++p) {
+      const Item& it = syn_items[p];
+      syn_slot[p] = it.slot;
+      if (multi) syn_cell[p] = (uint16_t)it.lc;
+      if (!H.syn_uniform) syn_e[p] = d.syn_e[it.id];
+      gen[go.syn_tau + p] = d.syn_tau[it.id];
+      out->syn_state_idx[it.id] = (uint32_t)(uc.state_base + so.g + p);
+    }
+    for (uint32_t p = 0; p < cl_items.size(); ++p) {
+      const Item& it = cl_items[p];
+      cl_slot[p] = it.slot;
+      if (multi) cl_cell[p] = (uint16_t)it.lc;
+      cl_t0[p] = d.clamp_t0[it.id];
+      cl_t1[p] = d.clamp_t1[it.id];
+      cl_amp[p] = d.clamp_amp[it.id];
+    }
+    return uc;
   }
 };
 
@@ -397,33 +446,12 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
   H.n_clamp = d.n_clamp; H.n_conn = d.n_conn; H.n_ext = d.n_ext;
   H.ena = d.hh_ena; H.ek = d.hh_ek; H.el = d.hh_el; H.threshold = d.threshold;
   const int64_t nc = d.n_cells;
-  // synapses / clamps on one CV are counted in 16 bits
-  // internal cell order: identity for homogeneous networks, else big cells first (load balance)
-  H.cell_order.resize(nc);
-  for (int64_t c = 0; c < nc; ++c) H.cell_order[c] = (uint32_t)c;
-  bool homogeneous = true;
-  int64_t n0 = d.cv_off[1] - d.cv_off[0];
-  for (int64_t c = 1; c < nc && homogeneous; ++c) homogeneous = (d.cv_off[c + 1] - d.cv_off[c]) == n0;
-  if (!homogeneous)
-    std::stable_sort(H.cell_order.begin(), H.cell_order.end(), [&](uint32_t x, uint32_t y) {
-      return d.cv_off[x + 1] - d.cv_off[x] > d.cv_off[y + 1] - d.cv_off[y];
-    });
-  H.cell_internal.resize(nc);
-  for (int64_t i = 0; i < nc; ++i) H.cell_internal[H.cell_order[i]] = (uint32_t)i;
-  // partition into blocks
-  std::vector<int64_t> blk_begin;
-  {
-    int64_t cvs = 0; uint32_t cells = 0;
-    for (int64_t i = 0; i < nc; ++i) {
-      int64_t n = d.cv_off[H.cell_order[i] + 1] - d.cv_off[H.cell_order[i]];
-      if (cells == 0 || cvs + n > P.target_slots || cells >= P.max_cells) { blk_begin.push_back(i); cvs = 0; cells = 0; }
-      cvs += n; ++cells;
-    }
-    blk_begin.push_back(nc);
+  // uniform synapse parameters (true for every BASELINE config): no per-synapse e / decay arrays
+  H.syn_uniform = H.n_syn > 0;
+  if (H.n_syn > 0) {
+    H.syn_tau_u = d.syn_tau[0]; H.syn_e_u = d.syn_e[0];
+    for (int64_t s = 1; s < H.n_syn && H.syn_uniform; ++s) H.syn_uniform = d.syn_tau[s] == H.syn_tau_u && d.syn_e[s] == H.syn_e_u;
   }
-  H.n_blocks = (int64_t)blk_begin.size() - 1;
-  H.blocks.resize(H.n_blocks);
-  H.cell_block.resize(nc);
   // clamps grouped by cell
   std::vector<int64_t> clamp_off(nc + 1, 0), clamp_idx(d.n_clamp);
   for (int64_t k = 0; k < d.n_clamp; ++k) clamp_off[d.clamp_cell[k] + 1]++;
@@ -432,29 +460,114 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     std::vector<int64_t> cur(clamp_off.begin(), clamp_off.end() - 1);
     for (int64_t k = 0; k < d.n_clamp; ++k) clamp_idx[cur[d.clamp_cell[k]]++] = k;
   }
-  // pass 1: counts
+  // bytes a cell needs as a unit of its own (HH instances counted exactly)
+  std::vector<uint32_t> cell_hh(nc, 0);
+  if (d.hh_gnabar)
+    parallel_for(nc, [&](int64_t c) {
+      uint32_t n = 0;
+      for (int64_t i = d.cv_off[c]; i < d.cv_off[c + 1]; ++i) n += d.hh_gnabar[i] != 0.0 || d.hh_gkbar[i] != 0.0 || d.hh_gl[i] != 0.0;
+      cell_hh[c] = n;
+    });
+  auto unit_bytes = [&](uint64_t n_cv, uint64_t n_hh, uint64_t n_syn, uint64_t n_clamp, uint64_t n_cell) -> uint64_t {
+    if (n_cv > 0x3FFFFFFFull || n_syn > 0x3FFFFFFFull || n_clamp > 0x3FFFFFFFull) return ~0ull;
+    const uint32_t ns = align_up((uint32_t)n_cv, 2);
+    return (uint64_t)fast_offsets(ns, (uint32_t)n_hh, (uint32_t)n_syn, (uint32_t)n_clamp, (uint32_t)n_cell, H.syn_uniform).total +
+           8ull * state_offsets(ns, (uint32_t)n_hh, (uint32_t)n_syn, (uint32_t)n_cell).total;
+  };
+  auto cell_counts = [&](int64_t c, uint64_t& n_cv, uint64_t& n_syn, uint64_t& n_cl) {
+    n_cv = (uint64_t)(d.cv_off[c + 1] - d.cv_off[c]);
+    n_syn = d.syn_off ? (uint64_t)(d.syn_off[c + 1] - d.syn_off[c]) : 0;
+    n_cl = (uint64_t)(clamp_off[c + 1] - clamp_off[c]);
+  };
+  // internal cell order: warp-class cells (big first when sizes differ), then block-class cells
+  std::vector<uint32_t> warp_cells, block_cells;
+  bool homogeneous = true;
+  for (int64_t c = 0; c < nc; ++c) {
+    uint64_t n_cv, n_syn, n_cl;
+    cell_counts(c, n_cv, n_syn, n_cl);
+    if (unit_bytes(n_cv, cell_hh[c], n_syn, n_cl, 1) <= P.unit_bytes) warp_cells.push_back((uint32_t)c);
+    else block_cells.push_back((uint32_t)c);
+    homogeneous = homogeneous && (d.cv_off[c + 1] - d.cv_off[c]) == (d.cv_off[1] - d.cv_off[0]);
+  }
+  auto bigger = [&](uint32_t x, uint32_t y) { return d.cv_off[x + 1] - d.cv_off[x] > d.cv_off[y + 1] - d.cv_off[y]; };
+  if (!homogeneous) {
+    std::stable_sort(warp_cells.begin(), warp_cells.end(), bigger);
+    std::stable_sort(block_cells.begin(), block_cells.end(), bigger);
+  }
+  H.cell_order = warp_cells;
+  H.cell_order.insert(H.cell_order.end(), block_cells.begin(), block_cells.end());
+  H.cell_internal.resize(nc);
+  for (int64_t i = 0; i < nc; ++i) H.cell_internal[H.cell_order[i]] = (uint32_t)i;
+  // partition into units
+  std::vector<int64_t> unit_begin;
+  {
+    uint64_t cv = 0, hh = 0, syn = 0, cl = 0, cells = 0;
+    for (int64_t i = 0; i < (int64_t)warp_cells.size(); ++i) {
+      uint64_t n_cv, n_syn, n_cl;
+      cell_counts(warp_cells[i], n_cv, n_syn, n_cl);
+      const uint64_t n_hh = cell_hh[warp_cells[i]];
+      if (cells == 0 || cells >= kWarpUnitMaxCells || unit_bytes(cv + n_cv + 1, hh + n_hh, syn + n_syn, cl + n_cl, cells + 1) > P.unit_bytes) {
+        unit_begin.push_back(i); cv = hh = syn = cl = cells = 0;
+      }
+      cv += n_cv; hh += n_hh; syn += n_syn; cl += n_cl; ++cells;
+    }
+    H.n_warp_units = (int64_t)unit_begin.size();
+    for (int64_t i = 0; i < (int64_t)block_cells.size(); ++i) unit_begin.push_back((int64_t)warp_cells.size() + i);
+    unit_begin.push_back(nc);
+  }
+  H.n_units = (int64_t)unit_begin.size() - 1;
+  H.units.resize(H.n_units);
+  // pass 1: counts and topo records
+  std::vector<std::vector<uint8_t>> topo(H.n_units);
   std::atomic<int> too_many(0);
-  parallel_for(H.n_blocks, [&](int64_t b) {
-    BlockBuilder B{d, P, H, clamp_off, clamp_idx, {}, {}, {}, {}, {}};
-    H.blocks[b] = B.run(blk_begin[b], (uint32_t)(blk_begin[b + 1] - blk_begin[b]), nullptr, nullptr, 0);
-    for (int64_t i = blk_begin[b]; i < blk_begin[b + 1]; ++i) H.cell_block[i] = (uint32_t)b;
-    if (H.blocks[b].n_level > 60000 || H.blocks[b].n_slot > 0x7FFFFFFFu) too_many.store(1);
+  parallel_for(H.n_units, [&](int64_t u) {
+    UnitBuilder B{d, P, H, clamp_off, clamp_idx, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, false};
+    H.units[u] = B.run(unit_begin[u], (uint32_t)(unit_begin[u + 1] - unit_begin[u]), &topo[u], nullptr, nullptr);
+    if (u >= H.n_warp_units) H.units[u].flags |= UNIT_BLOCK;
+    if (H.units[u].n_level > 60000 || H.units[u].n_slot > 0x3FFFFFFFu) too_many.store(1);
+    if (B.bad) too_many.store(1);
   });
-  if (too_many.load()) { err = "a cell is too deep or too large for the block layout"; return ARB_E_INVALID; }
-  // placement
-  std::vector<uint32_t> hh_first(H.n_blocks);
-  for (int64_t b = 0; b < H.n_blocks; ++b) {
-    BlockInfo& bi = H.blocks[b];
-    bi.gen_base = H.gen_doubles;     H.gen_doubles += gen_offsets(bi).total;
-    bi.fast_base = H.fast_doubles;   H.fast_doubles += fast_offsets(bi).total;
-    bi.state_base = H.state_doubles; H.state_doubles += state_offsets(bi).total;
-    bi.meta_base = H.meta_bytes;     H.meta_bytes += align_up(bi.meta_bytes, 128);
-    bi.scratch_base = H.scratch_doubles; H.scratch_doubles += 2 * (int64_t)bi.n_slot + 2 * align_up(bi.n_lane, 16);
-    hh_first[b] = (uint32_t)H.n_hh;  H.n_hh += bi.n_hh;
-    H.n_lanes += bi.n_lane;
-    H.max_block_slots = std::max(H.max_block_slots, bi.n_slot);
-    H.max_block_lanes = std::max(H.max_block_lanes, bi.n_lane);
-    H.max_block_cells = std::max(H.max_block_cells, bi.n_cell);
+  if (too_many.load()) { err = "a cell is too deep or too large for the unit layout"; return ARB_E_INVALID; }
+  // placement; tree structures are deduplicated by content
+  std::unordered_map<uint64_t, std::vector<int64_t>> seen;   // hash -> units that own a stored record
+  std::vector<int64_t> topo_owner(H.n_units, -1);
+  for (int64_t u = 0; u < H.n_units; ++u) {
+    UnitCounts& uc = H.units[u];
+    uc.fast_off = H.fast_bytes;     H.fast_bytes += align_up(uc.fast_bytes, 128);
+    uc.state_base = H.state_doubles; H.state_doubles += align_up(uc.state_bytes, 128) / 8;
+    uc.gen_base = H.gen_doubles;    H.gen_doubles += gen_offsets(uc.n_slot, uc.n_syn).total;
+    uc.lane_base = H.n_lanes;       H.n_lanes += uc.n_lane;
+    uc.hh_base = H.n_hh;            H.n_hh += uc.n_hh;
+    const uint64_t h = fnv1a(topo[u].data(), topo[u].size());
+    auto& bucket = seen[h];
+    int64_t owner = -1;
+    for (int64_t v : bucket)
+      if (topo[v].size() == topo[u].size() && std::memcmp(topo[v].data(), topo[u].data(), topo[u].size()) == 0) { owner = v; break; }
+    if (owner < 0) {
+      bucket.push_back(u);
+      uc.topo_off = H.topo_bytes;
+      H.topo_bytes += (int64_t)align_up((uint32_t)topo[u].size(), 128);
+      H.topo_records++;
+      topo_owner[u] = u;
+    } else {
+      uc.topo_off = H.units[owner].topo_off;
+      std::vector<uint8_t>().swap(topo[u]);
+    }
+    const uint32_t n_spec = uc.n_hh + uc.n_syn + uc.n_clamp;
+    if (uc.flags & UNIT_BLOCK) {
+      // contrib | dcontrib | xI | fgen | invdgen
+      uc.scratch_base = H.scratch_doubles;
+      H.scratch_doubles += 2 * (int64_t)align_up(uc.n_lane, 2) + align_up(n_spec, 2) + 2 * (int64_t)uc.n_slot;
+      H.block_lane_cap = std::max(H.block_lane_cap, uc.n_lane);
+    } else {
+      H.fast_cap = std::max(H.fast_cap, align_up(uc.fast_bytes, 128));
+      H.state_cap = std::max(H.state_cap, align_up(uc.state_bytes, 128));
+      H.lane_cap = std::max(H.lane_cap, uc.n_lane);
+      H.spec_cap = std::max(H.spec_cap, n_spec);
+      H.cell_cap = std::max(H.cell_cap, uc.n_cell);
+      H.topo_cap = std::max(H.topo_cap, (uint32_t)topo_offsets(uc.n_task, uc.n_level, uc.n_lane, uc.n_child, uc.n_cell).total);
+      H.slot_cap = std::max(H.slot_cap, uc.n_slot);
+    }
   }
   if (H.state_doubles >= (int64_t)0xFFFFFFF0u) { err = "state pool exceeds 2^32 doubles"; return ARB_E_INVALID; }
   // delays
@@ -464,17 +577,27 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
   if (!fill) return ARB_OK;
 
   // pass 2: fill
-  H.gen.assign(H.gen_doubles, 0.0);
-  H.fast.assign(H.fast_doubles, 0.0);
+  H.fast.assign(H.fast_bytes, 0);
   H.state.assign(H.state_doubles, 0.0);
-  H.meta.assign(H.meta_bytes, 0);
+  H.gen.assign(H.gen_doubles, 0.0);
+  H.topo.assign(H.topo_bytes, 0);
+  H.descs.resize(H.n_units);
+  H.cell_rt_idx.resize(nc);
   H.cv_state_idx.resize(H.n_cv);
   H.syn_state_idx.resize(H.n_syn);
   H.hh_m_idx.resize(H.n_hh); H.hh_stride.resize(H.n_hh); H.hh_cv.resize(H.n_hh);
-  parallel_for(H.n_blocks, [&](int64_t b) {
-    BlockBuilder B{d, P, H, clamp_off, clamp_idx, {}, {}, {}, {}, {}};
-    BlockInfo placed = H.blocks[b];
-    B.run(blk_begin[b], (uint32_t)(blk_begin[b + 1] - blk_begin[b]), &placed, &H, hh_first[b]);
+  for (int64_t u = 0; u < H.n_units; ++u) {
+    if (topo_owner[u] == u) std::memcpy(H.topo.data() + H.units[u].topo_off, topo[u].data(), topo[u].size());
+    UnitDesc& ud = H.descs[u];
+    ud.fast_off = H.units[u].fast_off; ud.state_base = H.units[u].state_base;
+    ud.fast_bytes = H.units[u].fast_bytes; ud.state_bytes = H.units[u].state_bytes;
+    ud.pad[0] = ud.pad[1] = 0;
+  }
+  std::vector<std::vector<uint8_t>>().swap(topo);
+  parallel_for(H.n_units, [&](int64_t u) {
+    UnitBuilder B{d, P, H, clamp_off, clamp_idx, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, false};
+    UnitCounts placed = H.units[u];
+    B.run(unit_begin[u], (uint32_t)(unit_begin[u + 1] - unit_begin[u]), nullptr, &placed, &H);
   });
   // connections grouped by caller's source cell, ascending k inside a group
   H.conn_off.assign(nc + 1, 0);

@@ -1,35 +1,51 @@
-// layout.hpp - host-side model builder: validation, branch decomposition, cell blocks.
-// Pure C++ (no CUDA): turns the caller's arb_desc into the pools described in block_layout.h.
+// layout.hpp - host-side model builder: validation, branch decomposition, cell units.
+// Pure C++ (no CUDA): turns the caller's arb_desc into the pools described in unit_layout.h.
 #pragma once
 #include <cstdint>
 #include <string>
 #include <vector>
 
 #include "../../include/arbb200.h"
-#include "block_layout.h"
+#include "unit_layout.h"
 
 namespace arbb {
 
 struct BuildParams {
-  uint32_t target_slots = 2304;   // close a block once it holds this many CVs (on-chip budget)
-  uint32_t max_cells = 64;        // cells per block
+  uint32_t unit_bytes = 22528;    // fast + state bytes a warp unit may hold (one shared-memory stage)
   uint32_t max_branch_len = 1024; // longer unbranched chains are cut into pieces
+};
+
+constexpr int64_t kMaxWarps = 2048;   // upper bound of resident warps of the warp kernel (scratch sizing)
+
+struct UnitCounts {                   // everything the offset functions need
+  uint32_t n_slot = 0, n_cv = 0, n_lane = 0, n_task = 0, n_level = 0, n_cell = 0, n_hh = 0, n_syn = 0,
+           n_clamp = 0, n_child = 0;
+  uint32_t flags = 0;
+  int64_t cell_base = 0, lane_base = 0, hh_base = 0;
+  int64_t fast_off = 0, state_base = 0, gen_base = 0, topo_off = 0, scratch_base = -1;
+  uint32_t fast_bytes = 0, state_bytes = 0;
 };
 
 struct HostModel {
   int64_t n_cells = 0, n_cv = 0, n_syn = 0, n_clamp = 0, n_conn = 0, n_ext = 0, n_hh = 0;
-  int64_t n_blocks = 0, n_lanes = 0;
-  int64_t gen_doubles = 0, fast_doubles = 0, state_doubles = 0, meta_bytes = 0, scratch_doubles = 0;
-  uint32_t max_block_slots = 0, max_block_lanes = 0, max_block_cells = 0;
+  int64_t n_units = 0, n_warp_units = 0, n_lanes = 0;
+  int64_t fast_bytes = 0, state_doubles = 0, gen_doubles = 0, topo_bytes = 0, scratch_doubles = 0;
+  int64_t topo_records = 0;           // distinct tree structures
+  // caps over warp units (shared-memory plan) and over block units
+  uint32_t fast_cap = 0, state_cap = 0, lane_cap = 0, spec_cap = 0, cell_cap = 0, slot_cap = 0, topo_cap = 0;
+  uint32_t block_lane_cap = 0;
+  bool syn_uniform = false;
+  double syn_tau_u = 0, syn_e_u = 0;
   double min_delay = 0, max_delay = 0;
   double ena = 0, ek = 0, el = 0, threshold = 0;
-  std::vector<BlockInfo> blocks;
+  std::vector<UnitCounts> units;
   std::vector<uint32_t> cell_order;     // internal -> caller's cell id
   std::vector<uint32_t> cell_internal;  // caller's cell id -> internal
-  std::vector<uint32_t> cell_block;     // internal -> block
   // ---- filled only by build(..., fill = true) ----
-  std::vector<double> gen, fast, state;
-  std::vector<uint8_t> meta;
+  std::vector<uint8_t> fast, topo;
+  std::vector<double> state, gen;
+  std::vector<UnitDesc> descs;
+  std::vector<uint32_t> cell_rt_idx;    // internal cell -> index of its runtime triple in the state pool
   std::vector<uint32_t> cv_state_idx;   // caller's CV -> index of its V in the state pool
   std::vector<uint32_t> syn_state_idx;  // caller's synapse -> index of its g in the state pool
   std::vector<uint32_t> hh_m_idx, hh_stride, hh_cv;  // per HH instance: index of m, distance to h, caller's CV
