@@ -61,9 +61,13 @@ enum {
 
 /* arb_configure keys (process-wide defaults read by later arb_plan / arb_create calls) */
 enum {
-  ARB_CFG_UNIT_BYTES = 1     /* bytes of streamed records (coefficients + state) one warp's shared-memory
+  ARB_CFG_UNIT_BYTES = 1,    /* bytes of streamed records (coefficients + state) one warp's shared-memory
                                 stage may hold; cells are packed into units up to this size, larger
                                 cells are integrated by a whole CTA.  0 = built-in default (22528)  */
+  ARB_CFG_GROUP_MIN_CELLS = 2 /* cells with identical trees are laid out cell-interleaved in groups
+                                (lane = cell) when their topology class has at least this many cells;
+                                smaller classes are laid out as units (lane = branch).  0 = built-in
+                                default (4); 1 = every cell in groups; >= 2^31 = no groups          */
 };
 
 /* The problem statement of PAPER.md section II as flat arrays.

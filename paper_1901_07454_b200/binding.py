@@ -15,6 +15,7 @@ ARB_OK, ARB_E_NULL, ARB_E_INVALID, ARB_E_WORKSPACE, ARB_E_CUDA, ARB_E_OVERFLOW, 
 ARB_PROBE_M, ARB_PROBE_H, ARB_PROBE_N, ARB_PROBE_SYN_G, ARB_PROBE_TIME, ARB_PROBE_NSTEPS, ARB_PROBE_STATS, ARB_PROBE_TIMING = range(8)
 ARB_OPT_FUSED_STEPS, ARB_OPT_EPOCH_STEPS, ARB_OPT_TIMING, ARB_OPT_STAGES = 1, 2, 3, 4
 ARB_CFG_UNIT_BYTES = 1
+ARB_CFG_GROUP_MIN_CELLS = 2
 
 EXPORTS = ("arb_plan", "arb_create", "arb_advance", "arb_spikes", "arb_voltage", "arb_probe",
            "arb_set_state", "arb_set_option", "arb_configure", "arb_destroy", "arb_last_error")

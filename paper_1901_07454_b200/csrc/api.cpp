@@ -32,7 +32,7 @@ struct Carver {
 };
 
 struct Regions {
-  Region units, gen, fast, state, topo, scratch, warp_scratch, factor_dcontrib, cell_rt_idx, cell_orig, ev_off, ev_t, ev_gidx, ev_w, ev_fill,
+  Region units, gdescs, gscratch, gen, fast, state, topo, scratch, warp_scratch, factor_dcontrib, cell_rt_idx, cell_orig, ev_off, ev_t, ev_gidx, ev_w, ev_fill,
       ext_off, ext_t, ext_gidx, ext_w, ext_cur, conn_off, conn_dst, conn_gidx, conn_delay, conn_w,
       pool_t[2], pool_dst[2], pool_gidx[2], pool_w[2], spike_cell, spike_t, counters, scan_tmp,
       cv_idx, syn_idx, hh_m_idx, hh_stride, hh_cv, io;
@@ -48,6 +48,10 @@ Caps capacities(const HostModel& H) {
   c.spikes = std::max<int64_t>(1 << 20, 64 * H.n_cells);
   return c;
 }
+
+// group kernel: per resident CTA fgen | invdgen for event-split sub-steps
+int64_t gscratch_stride(const HostModel& H) { return 2 * (int64_t)H.g_slot_cap * kG; }
+int64_t gscratch_ctas(const HostModel& H) { return std::min<int64_t>(H.n_groups, kMaxGroupCtas); }
 
 int64_t warp_scratch_stride(const HostModel& H) { return 2 * (int64_t)H.slot_cap + align_up(H.lane_cap, 2); }
 
@@ -70,6 +74,8 @@ Regions carve(const HostModel& H, const Caps& cap) {
   Carver C;
   const size_t nc = (size_t)H.n_cells;
   R.units = C.take(sizeof(UnitDesc) * (size_t)H.n_units);
+  R.gdescs = C.take(sizeof(GroupDesc) * (size_t)H.n_groups);
+  R.gscratch = C.take(8 * (size_t)(gscratch_ctas(H) * gscratch_stride(H)));
   R.gen = C.take(8 * (size_t)H.gen_doubles);
   R.fast = C.take((size_t)H.fast_bytes);
   R.state = C.take(8 * (size_t)H.state_doubles);
@@ -131,6 +137,7 @@ struct arb_model {
   int64_t cable_timed = 0, event_timed = 0;
   int cur_pool = 0;
   int sm_count = 148;
+  int group_grid = 0;
   int64_t opt_stages = 0;
   bool broken = false;
   std::string err;
@@ -159,10 +166,12 @@ cudaError_t upload(arb_model* m, const Region& r, const std::vector<T>& v) {
 }
 
 int64_t g_unit_bytes = 0;   // arb_configure(ARB_CFG_UNIT_BYTES)
+int64_t g_group_min = 0;    // arb_configure(ARB_CFG_GROUP_MIN_CELLS)
 
 BuildParams default_params() {
   BuildParams P;
   if (g_unit_bytes > 0) P.unit_bytes = (uint32_t)g_unit_bytes;
+  if (g_group_min > 0) P.group_min_cells = g_group_min >= 0x7FFFFFFF ? 0u : (uint32_t)g_group_min;
   return P;
 }
 
@@ -200,6 +209,7 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     if (reinterpret_cast<uintptr_t>(dev_workspace) % 256) { delete m; return fail(nullptr, ARB_E_WORKSPACE, "arb_create: workspace must be 256-byte aligned"); }
     m->ws = static_cast<char*>(dev_workspace);
     m->stream = static_cast<cudaStream_t>(cuda_stream);
+    if (H.n_groups > 0 && group_ctas_per_sm(group_smem_plan(H.g_slot_cap, H.g_buf_rows).bytes) == 0) { delete m; return fail(nullptr, ARB_E_INVALID, "arb_create: a cell group does not fit in shared memory"); }
     if (H.n_warp_units > 0 && make_plan(H, 1).warps == 0) { delete m; return fail(nullptr, ARB_E_INVALID, "arb_create: a warp unit does not fit in shared memory"); }
     {
       int dev = 0, sms = 0;
@@ -210,6 +220,7 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     const Regions& R = m->R;
     if ((e = cudaMemsetAsync(m->ws, 0, m->R.total, m->stream)) != cudaSuccess) return bail(e, "cudaMemsetAsync");
     if ((e = upload(m, R.units, H.descs)) != cudaSuccess) return bail(e, "upload units");
+    if ((e = upload(m, R.gdescs, H.gdescs)) != cudaSuccess) return bail(e, "upload groups");
     if ((e = upload(m, R.gen, H.gen)) != cudaSuccess) return bail(e, "upload gen");
     if ((e = upload(m, R.fast, H.fast)) != cudaSuccess) return bail(e, "upload fast");
     if ((e = upload(m, R.state, H.state)) != cudaSuccess) return bail(e, "upload state");
@@ -256,16 +267,22 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     }
     D.syn_uniform = H.syn_uniform ? 1 : 0; D.syn_e_u = H.syn_e_u; D.syn_tau_u = H.syn_tau_u; D.syn_decay_u = 1.0;
     D.plan = make_plan(H, 1);
+    D.groups = at<GroupDesc>(m, R.gdescs); D.n_groups = H.n_groups;
+    D.gscratch = at<double>(m, R.gscratch); D.gscratch_stride = gscratch_stride(H);
+    D.gplan = group_smem_plan(H.g_slot_cap, H.g_buf_rows);
+    if (H.n_groups > 0)
+      m->group_grid = (int)std::min<int64_t>(gscratch_ctas(H), (int64_t)m->sm_count * group_ctas_per_sm(D.gplan.bytes));
     D.pool_cap = m->cap.pool;
     D.spike_cell = at<uint32_t>(m, R.spike_cell); D.spike_t = at<double>(m, R.spike_t); D.spike_cap = m->cap.spikes;
     D.counters = at<unsigned long long>(m, R.counters);
     D.scan_tmp = at<uint32_t>(m, R.scan_tmp);
     D.ena = H.ena; D.ek = H.ek; D.el = H.el; D.theta = H.threshold;
     if ((e = launch_init(D, m->stream)) != cudaSuccess) return bail(e, "init kernel");
+    if ((e = launch_group_init(D, m->stream)) != cudaSuccess) return bail(e, "group init kernel");
     if ((e = cudaStreamSynchronize(m->stream)) != cudaSuccess) return bail(e, "cudaStreamSynchronize");
     // host pools are no longer needed
     std::vector<double>().swap(H.gen); std::vector<uint8_t>().swap(H.fast); std::vector<double>().swap(H.state);
-    std::vector<uint8_t>().swap(H.topo); std::vector<UnitDesc>().swap(H.descs); std::vector<uint32_t>().swap(H.cell_rt_idx);
+    std::vector<uint8_t>().swap(H.topo); std::vector<UnitDesc>().swap(H.descs); std::vector<GroupDesc>().swap(H.gdescs); std::vector<uint32_t>().swap(H.cell_rt_idx);
     std::vector<uint32_t>().swap(H.cv_state_idx); std::vector<uint32_t>().swap(H.syn_state_idx);
     std::vector<uint32_t>().swap(H.hh_m_idx); std::vector<uint32_t>().swap(H.hh_stride); std::vector<uint32_t>().swap(H.hh_cv);
     std::vector<uint32_t>().swap(H.conn_off); std::vector<uint32_t>().swap(H.conn_dst); std::vector<uint32_t>().swap(H.conn_gidx);
@@ -291,6 +308,7 @@ int arb_advance(arb_model* m, double t_end, double dt) {
   if (dt != m->factored_dt) {
     D.syn_decay_u = D.syn_uniform ? std::exp(-dt / D.syn_tau_u) : 1.0;
     CU(m, launch_factor(D, dt, m->stream));
+    CU(m, launch_group_factor(D, dt, m->H.g_seg_cap, m->stream));
     m->factored_dt = dt;
     m->launches++;
   }
@@ -343,6 +361,7 @@ int arb_advance(arb_model* m, double t_end, double dt) {
     for (int64_t j = 0; j < n_ep; j += fused) {
       StepArgs A;
       A.t0 = t0; A.dt = dt; A.t_end = t_end; A.k_first = k + j; A.nk = std::min(fused, n_ep - j); A.nsteps = nsteps; A.last_full = last_full;
+      CU(m, launch_group_cable(D, A, m->group_grid, m->stream, &launches));
       CU(m, launch_cable(D, A, grid, m->stream, &launches));
     }
     CU(m, stamp());
@@ -509,6 +528,9 @@ int arb_configure(int key, int64_t value) {
     case ARB_CFG_UNIT_BYTES:
       if (value != 0 && (value < 1024 || value > 112 * 1024)) return fail(nullptr, ARB_E_INVALID, "arb_configure: unit bytes out of range");
       g_unit_bytes = value;
+      return ARB_OK;
+    case ARB_CFG_GROUP_MIN_CELLS:
+      g_group_min = value;
       return ARB_OK;
   }
   return fail(nullptr, ARB_E_INVALID, "arb_configure: unknown key");

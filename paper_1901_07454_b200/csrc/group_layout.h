@@ -1,0 +1,134 @@
+// group_layout.h - the in-HBM layout of a "cell group", shared by the host builder and the kernels.
+//
+// Cells with identical trees (same parent array) form a topology CLASS.  A class is cut into
+// GROUPS of kG cells; a group is stored CELL-INTERLEAVED: row s of an array holds the value of
+// control volume `slot s` for the kG cells of the group (kG * 8 contiguous bytes), and the rows of
+// one array are contiguous, so that kG consecutive lanes (one "lane group", lane = cell) read
+// consecutive addresses while they walk the tree.  (The paper's GPU solver interleaves whole cell
+// matrices with one thread per cell; here several lane groups and several warps walk
+// different subtrees of the same cells at the same time.)
+//
+//   segment   a maximal unbranched chain of control volumes; its slots are consecutive
+//             (slot0 = proximal end).  One lane group eliminates a segment serially, carrying the
+//             recurrence in a register.
+//   chunk     a connected set of segments that one lane group eliminates one after the other
+//   stage     chunks that do not depend on each other; the CTA's lane groups run them
+//             concurrently, __syncthreads separates stages.  Backward (leaves -> root) runs stages
+//             0..n_stage-1, forward (root -> leaves) runs them in reverse, segments reversed.
+//
+// Per class there is one ClassRecord in the topo pool (read through L1, never staged).
+// Per group there are three records:
+//   const (fast pool, bytes)   f | invd | a | b | hh gna, gk, gl | syn e, decay (non-uniform only) |
+//                              clamp t0, t1, amp | hh_slot | syn_slot | cl_slot | det_slot
+//   state (state pool, doubles) V | m | h | n | g | per-cell runtime triples [cell][3]
+//   gen   (gen pool, doubles)   C | S | sigma | G | bg | syn_tau   (dt-independent; factorisation
+//                              and event-split sub-steps only)
+// Rows of per-instance arrays (HH, synapses, clamps): row j = the j-th instance of every cell in
+// ascending (slot, caller's index) order; cells with fewer instances are padded with slot kNoSlot16.
+#pragma once
+#include <stdint.h>
+
+#include "unit_layout.h"
+
+namespace arbb {
+
+#ifndef ARBB_G
+#define ARBB_G 8
+#endif
+#ifndef ARBB_GROUP_WARPS
+#define ARBB_GROUP_WARPS 4
+#endif
+constexpr int kG = ARBB_G;                    // cells per group = lanes per lane group (8, 16 or 32)
+constexpr int kLaneGroups = 32 / kG;          // lane groups per warp
+constexpr int kGroupWarps = ARBB_GROUP_WARPS; // warps per CTA of the group kernel
+constexpr int kGroupThreads = kGroupWarps * 32;
+constexpr int kGroupSlots = kGroupWarps * kLaneGroups;   // chunks a stage can run concurrently
+constexpr uint16_t kNoSlot16 = 0xFFFFu;
+constexpr uint32_t kGroupMaxCv = 65000;       // slots are stored as uint16
+
+struct SegRec {          // 16 bytes, one broadcast load per lane group
+  uint32_t slot0;        // slot of the proximal control volume
+  uint32_t pslot;        // slot of the parent control volume of slot0, or kNoSlot
+  uint16_t len;          // control volumes in the segment
+  uint16_t ccnt;         // child segments hanging off its last control volume
+  uint32_t cbeg;         // first entry of its child list
+};
+
+struct ClassRecord {     // header of a class record; arrays follow at the byte offsets below
+  uint32_t n_cv, n_seg, n_stage, n_child;
+  uint32_t off_segs;     // SegRec[n_seg]
+  uint32_t off_order;    // uint16[n_seg]: segments in backward processing order, grouped by (stage, slot)
+  uint32_t off_sched;    // uint16[n_stage * kGroupSlots + 1]: begin of each (stage, slot) range in order[]
+  uint32_t off_child;    // uint16[n_child]: child segments
+  uint32_t bytes;
+  uint32_t pad[7];
+};
+static_assert(sizeof(ClassRecord) == 64, "ClassRecord must be 64 bytes");
+
+struct GroupDesc {       // 64 bytes
+  int64_t const_off;     // byte offset into the fast pool (128-byte aligned)
+  int64_t state_base;    // double index into the state pool (16-double aligned)
+  int64_t gen_base;      // double index into the gen pool
+  int64_t class_off;     // byte offset of the ClassRecord in the topo pool
+  int64_t cell_base;     // internal index of the group's first cell
+  uint32_t n_cv, n_cell, n_hh_rows, n_syn_rows, n_cl_rows, n_seg;
+};
+static_assert(sizeof(GroupDesc) == 64, "GroupDesc must be 64 bytes");
+
+// Byte offsets inside a group's const record (every section 128-byte aligned).
+struct GConstOff {
+  uint32_t f, invd, a, b, hh_gna, hh_gk, hh_gl, syn_e, syn_decay, cl_t0, cl_t1, cl_amp,
+      hh_slot, syn_slot, cl_slot, det_slot, total;
+};
+ARBB_HD GConstOff gconst_offsets(uint32_t n_cv, uint32_t n_hh, uint32_t n_syn, uint32_t n_cl, bool syn_uniform) {
+  GConstOff o;
+  uint32_t p = 0;
+  auto sec = [&](uint32_t bytes) { uint32_t at = p; p = align_up(p + bytes, 128); return at; };
+  const uint32_t row = 8 * kG, row16 = 2 * kG;
+  o.f = sec(row * n_cv); o.invd = sec(row * n_cv); o.a = sec(row * n_cv); o.b = sec(row * n_cv);
+  o.hh_gna = sec(row * n_hh); o.hh_gk = sec(row * n_hh); o.hh_gl = sec(row * n_hh);
+  o.syn_e = sec(syn_uniform ? 0 : row * n_syn); o.syn_decay = sec(syn_uniform ? 0 : row * n_syn);
+  o.cl_t0 = sec(row * n_cl); o.cl_t1 = sec(row * n_cl); o.cl_amp = sec(row * n_cl);
+  o.hh_slot = sec(row16 * n_hh); o.syn_slot = sec(row16 * n_syn); o.cl_slot = sec(row16 * n_cl);
+  o.det_slot = sec(row16);
+  o.total = p;
+  return o;
+}
+
+// Double offsets inside a group's state record (every section 16-double aligned).
+struct GStateOff { uint32_t v, m, h, n, g, rt, total; };
+ARBB_HD GStateOff gstate_offsets(uint32_t n_cv, uint32_t n_hh, uint32_t n_syn) {
+  GStateOff o;
+  uint32_t p = 0;
+  auto sec = [&](uint32_t n) { uint32_t at = p; p = align_up(p + n, 16); return at; };
+  o.v = sec(kG * n_cv); o.m = sec(kG * n_hh); o.h = sec(kG * n_hh); o.n = sec(kG * n_hh);
+  o.g = sec(kG * n_syn); o.rt = sec(kRtDoubles * kG);
+  o.total = p;
+  return o;
+}
+
+// Double offsets inside a group's gen record.
+struct GGenOff { uint32_t C, S, sig, G, b, syn_tau, total; };
+ARBB_HD GGenOff ggen_offsets(uint32_t n_cv, uint32_t n_syn) {
+  GGenOff o;
+  const uint32_t n = kG * n_cv;
+  o.C = 0; o.S = n; o.sig = 2 * n; o.G = 3 * n; o.b = 4 * n; o.syn_tau = 5 * n;
+  o.total = align_up(5 * n + kG * n_syn, 16);
+  return o;
+}
+
+// Shared memory of one CTA of the group kernel: V of the group | buf (xI, then contrib) | cells.
+// slot_cap = largest n_cv of any group, buf_rows = largest max(n_seg, n_hh + n_syn + n_cl rows).
+struct GroupSmemPlan { uint32_t slot_cap, buf_rows, off_buf, off_cell, off_mbar, bytes; };
+ARBB_HD GroupSmemPlan group_smem_plan(uint32_t slot_cap, uint32_t buf_rows) {
+  GroupSmemPlan P;
+  P.slot_cap = slot_cap; P.buf_rows = buf_rows;
+  uint32_t p = align_up(8 * kG * slot_cap, 128);
+  P.off_buf = p;  p = align_up(p + 8 * kG * buf_rows, 128);
+  P.off_cell = p; p = align_up(p + kCellScratchBytes * kG, 128);
+  P.off_mbar = p; p += 16;
+  P.bytes = align_up(p, 128);
+  return P;
+}
+
+}  // namespace arbb

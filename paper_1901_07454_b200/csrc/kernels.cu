@@ -18,8 +18,7 @@
 // No tensor cores: nothing here is a dense contraction.  The path is bound by HBM traffic when
 // state streams every step and by fp64 dependent-chain latency when a unit stays on chip.
 #include "kernels.cuh"
-
-#include <math_constants.h>
+#include "device_common.cuh"
 
 namespace arbb {
 
@@ -28,56 +27,6 @@ namespace {
 constexpr int kBlockThreads = 256;              // cable_block_kernel, factor_kernel, init_kernel
 constexpr int kBlockWarps = kBlockThreads / 32;
 constexpr int kMaxWarpsPerCta = 8;              // cable_warp_kernel
-constexpr unsigned kFull = 0xffffffffu;
-
-// ------------------------------------------------------------------------------------------
-// HH rate functions (reading R5): textbook Hodgkin-Huxley 1952, 6.3 C, rest at -65 mV.
-// ------------------------------------------------------------------------------------------
-__device__ __forceinline__ double exprelr(double x) { return x == 0.0 ? 1.0 : x / expm1(x); }
-
-struct Rates { double am, bm, ah, bh, an, bn; };
-__device__ __forceinline__ Rates hh_rates(double v) {
-  Rates r;
-  r.am = exprelr(-(v + 40.0) / 10.0);
-  r.bm = 4.0 * exp(-(v + 65.0) / 18.0);
-  r.ah = 0.07 * exp(-(v + 65.0) / 20.0);
-  r.bh = 1.0 / (1.0 + exp(-(v + 35.0) / 10.0));
-  r.an = 0.1 * exprelr(-(v + 55.0) / 10.0);
-  r.bn = 0.125 * exp(-(v + 65.0) / 80.0);
-  return r;
-}
-
-// ------------------------------------------------------------------------------------------
-// bulk-async copy (TMA) and mbarrier primitives
-// ------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst_smem)),
-               "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
-               : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  const uint32_t addr = smem_u32(bar);
-  uint32_t ok;
-  do {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(ok)
-        : "r"(addr), "r"(parity)
-        : "memory");
-  } while (!ok);
-}
 
 // ------------------------------------------------------------------------------------------
 // scopes: a unit is integrated either by one warp or by one CTA
@@ -139,19 +88,6 @@ __device__ __forceinline__ void make_view(UnitView& U, const DevModel& M, const 
   const double* gen = M.gen + H.gen_base;
   U.C = gen + go.C; U.S = gen + go.S; U.sig = gen + go.sig; U.G = gen + go.G; U.bg = gen + go.b; U.syn_tau = gen + go.syn_tau;
   U.cell_base = H.cell_base;
-}
-
-// per-cell runtime of the (sub-)step in progress, in shared memory
-struct CellS {
-  double *tcur, *tnext, *delta, *vprev;
-  uint32_t *evcur, *evend, *armed, *mode, *wb, *dirty;
-};
-__device__ __forceinline__ CellS carve_cells(uint8_t* p, uint32_t cap) {
-  CellS c;
-  c.tcur = (double*)p; c.tnext = c.tcur + cap; c.delta = c.tnext + cap; c.vprev = c.delta + cap;
-  c.evcur = (uint32_t*)(c.vprev + cap); c.evend = c.evcur + cap; c.armed = c.evend + cap;
-  c.mode = c.armed + cap; c.wb = c.mode + cap; c.dirty = c.wb + cap;
-  return c;
 }
 
 struct TaskCtx { Task T; LaneRec R; };
@@ -910,11 +846,13 @@ int cable_smem_limit() { return 227 * 1024; }
 int cable_max_warps() { return kMaxWarpsPerCta; }
 
 cudaError_t launch_factor(const DevModel& M, double dt, cudaStream_t s) {
+  if (M.n_units == 0) return cudaSuccess;
   factor_kernel<<<(unsigned)M.n_units, kBlockThreads, 0, s>>>(M, dt);
   return cudaGetLastError();
 }
 
 cudaError_t launch_init(const DevModel& M, cudaStream_t s) {
+  if (M.n_units == 0) return cudaSuccess;
   init_kernel<<<(unsigned)M.n_units, kBlockThreads, 0, s>>>(M);
   return cudaGetLastError();
 }

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "group_layout.h"
 #include "unit_layout.h"
 
 namespace arbb {
@@ -56,6 +57,12 @@ struct DevModel {
   double syn_e_u, syn_tau_u, syn_decay_u;
   double ena, ek, el, theta;
   WarpSmemPlan plan;
+  // cell groups (group_layout.h); cells of groups come first in the internal cell order
+  const GroupDesc* groups;
+  int64_t n_groups;
+  double* gscratch;           // group kernel: per CTA fgen | invdgen (event-split sub-steps only)
+  int64_t gscratch_stride;
+  GroupSmemPlan gplan;
 };
 
 struct StepArgs {
@@ -78,6 +85,11 @@ cudaError_t launch_gather_hh(const double* state, const uint32_t* m_idx, const u
 cudaError_t launch_scatter_hh(double* state, const uint32_t* m_idx, const uint32_t* stride, const uint32_t* cv,
                               int which, int64_t n_hh, const double* in, cudaStream_t s);
 cudaError_t launch_reset_detectors(const DevModel& M, cudaStream_t s);
+// cell groups (group_kernel.cu)
+cudaError_t launch_group_factor(const DevModel& M, double dt, uint32_t seg_cap, cudaStream_t s);
+cudaError_t launch_group_init(const DevModel& M, cudaStream_t s);
+cudaError_t launch_group_cable(const DevModel& M, const StepArgs& A, int grid, cudaStream_t s, int* launches);
+int group_ctas_per_sm(uint32_t smem_bytes);   // resident CTAs of the group kernel per SM (0: does not fit)
 int cable_smem_limit();       // bytes of dynamic shared memory a CTA of the warp kernel may use
 int cable_max_warps();        // warps per CTA the warp kernel is compiled for
 

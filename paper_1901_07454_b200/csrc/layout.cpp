@@ -436,6 +436,142 @@ struct UnitBuilder {
 
 }  // namespace
 
+
+namespace {
+
+// ---------------------------------------------------------------------------------------------
+// Cell groups (group_layout.h)
+// ---------------------------------------------------------------------------------------------
+struct ClassInfo {
+  uint32_t n_cv = 0, n_seg = 0;
+  std::vector<uint32_t> cv_slot;       // control volume -> slot
+  std::vector<uint8_t> record;         // ClassRecord + arrays
+  int64_t topo_off = 0;
+  std::vector<uint32_t> cells;         // caller's cell ids, ascending
+  bool grouped = false;
+};
+
+constexpr uint32_t kMinChunk = 16;     // control volumes below which a stage is not split further
+constexpr uint32_t kMaxSegLen = 4096;
+
+// Segments, stages of independent chunks, slot numbering and the serialised record of one tree.
+void build_class(const int32_t* par, uint32_t n, ClassInfo& K) {
+  K.n_cv = n;
+  std::vector<uint32_t> nchild(n, 0), seg_of(n, 0);
+  for (uint32_t i = 1; i < n; ++i) nchild[par[i]]++;
+  struct Seg { uint32_t first, len; int32_t parent; std::vector<uint32_t> kids; };
+  std::vector<Seg> segs;
+  for (uint32_t i = 0; i < n; ++i) {
+    const bool fresh = i == 0 || nchild[par[i]] != 1 || segs[seg_of[par[i]]].len >= kMaxSegLen ||
+                       i != segs[seg_of[par[i]]].first + segs[seg_of[par[i]]].len;
+    if (fresh) {
+      Seg sg;
+      sg.first = i; sg.len = 0; sg.parent = i == 0 ? -1 : (int32_t)seg_of[par[i]];
+      seg_of[i] = (uint32_t)segs.size();
+      segs.push_back(sg);
+    } else {
+      seg_of[i] = seg_of[par[i]];
+    }
+    segs[seg_of[i]].len++;
+  }
+  // a chain that is not numbered consecutively is cut, so CV k of a segment is always first + k, and
+  // children hang off the last control volume of their parent segment
+  const uint32_t ns = (uint32_t)segs.size();
+  K.n_seg = ns;
+  for (uint32_t s2 = 1; s2 < ns; ++s2) segs[segs[s2].parent].kids.push_back(s2);
+  // stages: repeatedly peel the maximal subtrees that fit the per-slot share of what is left
+  std::vector<uint8_t> left(ns, 1);
+  std::vector<uint64_t> w(ns, 0);
+  std::vector<std::vector<std::vector<uint32_t>>> stages;   // [stage][slot] -> segments in backward order
+  uint32_t n_left = ns;
+  while (n_left > 0) {
+    for (uint32_t s2 = ns; s2-- > 0;) {
+      if (!left[s2]) continue;
+      w[s2] = segs[s2].len;
+      for (uint32_t k : segs[s2].kids) if (left[k]) w[s2] += w[k];
+    }
+    const uint64_t total = w[0];
+    const uint64_t cap = std::max<uint64_t>((total + kGroupSlots - 1) / kGroupSlots, kMinChunk);
+    std::vector<uint32_t> roots;
+    for (uint32_t s2 = 0; s2 < ns; ++s2)
+      if (left[s2] && w[s2] <= cap && (segs[s2].parent < 0 || w[segs[s2].parent] > cap)) roots.push_back(s2);
+    if (roots.empty())
+      for (uint32_t s2 = 0; s2 < ns; ++s2) {
+        if (!left[s2]) continue;
+        bool leaf = true;
+        for (uint32_t k : segs[s2].kids) leaf = leaf && !left[k];
+        if (leaf) roots.push_back(s2);
+      }
+    std::stable_sort(roots.begin(), roots.end(), [&](uint32_t x, uint32_t y) { return w[x] > w[y]; });
+    std::vector<std::vector<uint32_t>> slots(kGroupSlots);
+    std::vector<uint64_t> load(kGroupSlots, 0);
+    for (uint32_t r : roots) {
+      uint32_t best = 0;
+      for (uint32_t h = 1; h < (uint32_t)kGroupSlots; ++h) if (load[h] < load[best]) best = h;
+      load[best] += w[r];
+      // the remaining subtree of r, children before parents (descending segment id)
+      std::vector<uint32_t> sub{r};
+      for (size_t q = 0; q < sub.size(); ++q)
+        for (uint32_t k : segs[sub[q]].kids) if (left[k]) sub.push_back(k);
+      std::sort(sub.begin(), sub.end(), [](uint32_t x, uint32_t y) { return x > y; });
+      slots[best].insert(slots[best].end(), sub.begin(), sub.end());
+    }
+    for (auto& v : slots) for (uint32_t s2 : v) { left[s2] = 0; --n_left; }
+    stages.push_back(std::move(slots));
+  }
+  // slots: ascending addresses along the forward sweep
+  std::vector<uint32_t> slot0(ns, 0);
+  uint32_t next = 0;
+  for (size_t st = stages.size(); st-- > 0;)
+    for (uint32_t h = 0; h < (uint32_t)kGroupSlots; ++h)
+      for (size_t q = stages[st][h].size(); q-- > 0;) {
+        const uint32_t s2 = stages[st][h][q];
+        slot0[s2] = next;
+        next += segs[s2].len;
+      }
+  K.cv_slot.resize(n);
+  for (uint32_t i = 0; i < n; ++i) K.cv_slot[i] = slot0[seg_of[i]] + (i - segs[seg_of[i]].first);
+  // record
+  uint32_t n_child = ns - 1;
+  ClassRecord R;
+  std::memset(&R, 0, sizeof R);
+  R.n_cv = n; R.n_seg = ns; R.n_stage = (uint32_t)stages.size(); R.n_child = n_child;
+  uint32_t p = sizeof(ClassRecord);
+  auto sec = [&](uint32_t bytes) { uint32_t at = p; p = align_up(p + bytes, 16); return at; };
+  R.off_segs = sec(ns * (uint32_t)sizeof(SegRec));
+  R.off_order = sec(ns * 2);
+  R.off_sched = sec(((uint32_t)stages.size() * kGroupSlots + 1) * 2);
+  R.off_child = sec(n_child * 2);
+  R.bytes = align_up(p, 128);
+  K.record.assign(R.bytes, 0);
+  std::memcpy(K.record.data(), &R, sizeof R);
+  SegRec* sr = (SegRec*)(K.record.data() + R.off_segs);
+  uint16_t* order = (uint16_t*)(K.record.data() + R.off_order);
+  uint16_t* sched = (uint16_t*)(K.record.data() + R.off_sched);
+  uint16_t* child = (uint16_t*)(K.record.data() + R.off_child);
+  uint32_t cpos = 0;
+  for (uint32_t s2 = 0; s2 < ns; ++s2) {
+    sr[s2].slot0 = slot0[s2];
+    sr[s2].pslot = segs[s2].parent < 0 ? kNoSlot : K.cv_slot[par[segs[s2].first]];
+    sr[s2].len = (uint16_t)segs[s2].len;
+    sr[s2].ccnt = (uint16_t)segs[s2].kids.size();
+    sr[s2].cbeg = cpos;
+    // children in descending order: the order in which a leaves -> root elimination meets them
+    for (size_t q = segs[s2].kids.size(); q-- > 0;) child[cpos++] = (uint16_t)segs[s2].kids[q];
+  }
+  uint32_t opos = 0, spos = 0;
+  for (size_t st = 0; st < stages.size(); ++st)
+    for (uint32_t h = 0; h < (uint32_t)kGroupSlots; ++h) {
+      sched[spos++] = (uint16_t)opos;
+      for (uint32_t s2 : stages[st][h]) order[opos++] = (uint16_t)s2;
+    }
+  sched[spos] = (uint16_t)opos;
+}
+
+struct GroupCounts { uint32_t cls = 0, n_cell = 0, n_hh_rows = 0, n_syn_rows = 0, n_cl_rows = 0; int64_t cell_begin = 0, hh_base = 0; };
+
+}  // namespace
+
 int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std::string& err) {
   int rc = validate(d, err);
   if (rc) return rc;
@@ -479,10 +615,59 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     n_syn = d.syn_off ? (uint64_t)(d.syn_off[c + 1] - d.syn_off[c]) : 0;
     n_cl = (uint64_t)(clamp_off[c + 1] - clamp_off[c]);
   };
-  // internal cell order: warp-class cells (big first when sizes differ), then block-class cells
+  // ---- topology classes -> cell groups (group_layout.h)
+  std::vector<ClassInfo> classes;
+  std::vector<int32_t> cell_class(nc, -1);
+  std::vector<GroupCounts> groups;
+  std::vector<uint32_t> group_cells;
+  if (P.group_min_cells > 0) {
+    std::vector<uint64_t> hash(nc);
+    parallel_for(nc, [&](int64_t c) {
+      hash[c] = fnv1a((const uint8_t*)(d.cv_parent + d.cv_off[c]), 4 * (size_t)(d.cv_off[c + 1] - d.cv_off[c]));
+    });
+    std::unordered_map<uint64_t, std::vector<int32_t>> by_hash;
+    for (int64_t c = 0; c < nc; ++c) {
+      const uint32_t n = (uint32_t)(d.cv_off[c + 1] - d.cv_off[c]);
+      if (n > std::min(P.group_max_cv, kGroupMaxCv)) continue;
+      auto& bucket = by_hash[hash[c]];
+      int32_t cls = -1;
+      for (int32_t k : bucket) {
+        const uint32_t rep = classes[k].cells[0];
+        if (classes[k].n_cv == n && std::memcmp(d.cv_parent + d.cv_off[rep], d.cv_parent + d.cv_off[c], 4 * (size_t)n) == 0) { cls = k; break; }
+      }
+      if (cls < 0) {
+        cls = (int32_t)classes.size();
+        classes.emplace_back();
+        classes[cls].n_cv = n;
+        bucket.push_back(cls);
+      }
+      classes[cls].cells.push_back((uint32_t)c);
+    }
+    for (size_t k = 0; k < classes.size(); ++k) {
+      ClassInfo& K = classes[k];
+      K.grouped = K.cells.size() >= P.group_min_cells;
+      if (!K.grouped) continue;
+      for (size_t i = 0; i < K.cells.size(); i += kG) {
+        GroupCounts G;
+        G.cls = (uint32_t)k;
+        G.n_cell = (uint32_t)std::min<size_t>(kG, K.cells.size() - i);
+        G.cell_begin = (int64_t)group_cells.size();
+        for (uint32_t j = 0; j < G.n_cell; ++j) { group_cells.push_back(K.cells[i + j]); cell_class[K.cells[i + j]] = (int32_t)k; }
+        groups.push_back(G);
+      }
+    }
+    parallel_for((int64_t)classes.size(), [&](int64_t k) {
+      if (classes[k].grouped) build_class(d.cv_parent + d.cv_off[classes[k].cells[0]], classes[k].n_cv, classes[k]);
+    });
+  }
+  const int64_t ngc = (int64_t)group_cells.size();
+  H.n_groups = (int64_t)groups.size();
+  H.n_group_cells = ngc;
+  // internal cell order: group cells, warp-class cells (big first when sizes differ), block-class cells
   std::vector<uint32_t> warp_cells, block_cells;
   bool homogeneous = true;
   for (int64_t c = 0; c < nc; ++c) {
+    if (cell_class[c] >= 0) continue;
     uint64_t n_cv, n_syn, n_cl;
     cell_counts(c, n_cv, n_syn, n_cl);
     if (unit_bytes(n_cv, cell_hh[c], n_syn, n_cl, 1) <= P.unit_bytes) warp_cells.push_back((uint32_t)c);
@@ -494,7 +679,8 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     std::stable_sort(warp_cells.begin(), warp_cells.end(), bigger);
     std::stable_sort(block_cells.begin(), block_cells.end(), bigger);
   }
-  H.cell_order = warp_cells;
+  H.cell_order = group_cells;
+  H.cell_order.insert(H.cell_order.end(), warp_cells.begin(), warp_cells.end());
   H.cell_order.insert(H.cell_order.end(), block_cells.begin(), block_cells.end());
   H.cell_internal.resize(nc);
   for (int64_t i = 0; i < nc; ++i) H.cell_internal[H.cell_order[i]] = (uint32_t)i;
@@ -507,12 +693,12 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
       cell_counts(warp_cells[i], n_cv, n_syn, n_cl);
       const uint64_t n_hh = cell_hh[warp_cells[i]];
       if (cells == 0 || cells >= kWarpUnitMaxCells || unit_bytes(cv + n_cv + 1, hh + n_hh, syn + n_syn, cl + n_cl, cells + 1) > P.unit_bytes) {
-        unit_begin.push_back(i); cv = hh = syn = cl = cells = 0;
+        unit_begin.push_back(ngc + i); cv = hh = syn = cl = cells = 0;
       }
       cv += n_cv; hh += n_hh; syn += n_syn; cl += n_cl; ++cells;
     }
     H.n_warp_units = (int64_t)unit_begin.size();
-    for (int64_t i = 0; i < (int64_t)block_cells.size(); ++i) unit_begin.push_back((int64_t)warp_cells.size() + i);
+    for (int64_t i = 0; i < (int64_t)block_cells.size(); ++i) unit_begin.push_back(ngc + (int64_t)warp_cells.size() + i);
     unit_begin.push_back(nc);
   }
   H.n_units = (int64_t)unit_begin.size() - 1;
@@ -528,6 +714,39 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     if (B.bad) too_many.store(1);
   });
   if (too_many.load()) { err = "a cell is too deep or too large for the unit layout"; return ARB_E_INVALID; }
+  // groups: row counts, then placement (groups first in every pool)
+  parallel_for(H.n_groups, [&](int64_t g) {
+    GroupCounts& G = groups[g];
+    for (uint32_t lc = 0; lc < G.n_cell; ++lc) {
+      const uint32_t c = group_cells[G.cell_begin + lc];
+      G.n_hh_rows = std::max(G.n_hh_rows, cell_hh[c]);
+      if (d.syn_off) G.n_syn_rows = std::max(G.n_syn_rows, (uint32_t)(d.syn_off[c + 1] - d.syn_off[c]));
+      G.n_cl_rows = std::max(G.n_cl_rows, (uint32_t)(clamp_off[c + 1] - clamp_off[c]));
+    }
+  });
+  for (auto& K : classes)
+    if (K.grouped) {
+      K.topo_off = H.topo_bytes;
+      H.topo_bytes += (int64_t)K.record.size();
+      H.n_classes++;
+      H.g_seg_cap = std::max(H.g_seg_cap, K.n_seg);
+    }
+  H.gdescs.resize(H.n_groups);
+  for (int64_t g = 0; g < H.n_groups; ++g) {
+    GroupCounts& G = groups[g];
+    const ClassInfo& K = classes[G.cls];
+    GroupDesc& D = H.gdescs[g];
+    D.n_cv = K.n_cv; D.n_cell = G.n_cell; D.n_hh_rows = G.n_hh_rows; D.n_syn_rows = G.n_syn_rows; D.n_cl_rows = G.n_cl_rows; D.n_seg = K.n_seg;
+    D.class_off = K.topo_off;
+    D.cell_base = G.cell_begin;
+    D.const_off = H.fast_bytes;   H.fast_bytes += gconst_offsets(K.n_cv, G.n_hh_rows, G.n_syn_rows, G.n_cl_rows, H.syn_uniform).total;
+    D.state_base = H.state_doubles; H.state_doubles += gstate_offsets(K.n_cv, G.n_hh_rows, G.n_syn_rows).total;
+    D.gen_base = H.gen_doubles;   H.gen_doubles += ggen_offsets(K.n_cv, G.n_syn_rows).total;
+    G.hh_base = H.n_hh;
+    for (uint32_t lc = 0; lc < G.n_cell; ++lc) H.n_hh += cell_hh[group_cells[G.cell_begin + lc]];
+    H.g_slot_cap = std::max(H.g_slot_cap, K.n_cv);
+    H.g_buf_rows = std::max(H.g_buf_rows, std::max(K.n_seg, G.n_hh_rows + G.n_syn_rows + G.n_cl_rows));
+  }
   // placement; tree structures are deduplicated by content
   std::unordered_map<uint64_t, std::vector<int64_t>> seen;   // hash -> units that own a stored record
   std::vector<int64_t> topo_owner(H.n_units, -1);
@@ -586,6 +805,105 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
   H.cv_state_idx.resize(H.n_cv);
   H.syn_state_idx.resize(H.n_syn);
   H.hh_m_idx.resize(H.n_hh); H.hh_stride.resize(H.n_hh); H.hh_cv.resize(H.n_hh);
+  for (const auto& K : classes)
+    if (K.grouped) std::memcpy(H.topo.data() + K.topo_off, K.record.data(), K.record.size());
+  parallel_for(H.n_groups, [&](int64_t g) {
+    const GroupCounts& G = groups[g];
+    const ClassInfo& K = classes[G.cls];
+    const GroupDesc& D = H.gdescs[g];
+    const uint32_t n = K.n_cv;
+    const GConstOff co = gconst_offsets(n, G.n_hh_rows, G.n_syn_rows, G.n_cl_rows, H.syn_uniform);
+    const GStateOff so = gstate_offsets(n, G.n_hh_rows, G.n_syn_rows);
+    const GGenOff go = ggen_offsets(n, G.n_syn_rows);
+    uint8_t* cb = H.fast.data() + D.const_off;
+    double* st = H.state.data() + D.state_base;
+    double* gen = H.gen.data() + D.gen_base;
+    double* f = (double*)(cb + co.f); double* invd = (double*)(cb + co.invd);
+    double* a = (double*)(cb + co.a); double* b = (double*)(cb + co.b);
+    double* hh_gna = (double*)(cb + co.hh_gna); double* hh_gk = (double*)(cb + co.hh_gk); double* hh_gl = (double*)(cb + co.hh_gl);
+    double* syn_e = (double*)(cb + co.syn_e);
+    double* cl_t0 = (double*)(cb + co.cl_t0); double* cl_t1 = (double*)(cb + co.cl_t1); double* cl_amp = (double*)(cb + co.cl_amp);
+    uint16_t* hh_slot = (uint16_t*)(cb + co.hh_slot); uint16_t* syn_slot = (uint16_t*)(cb + co.syn_slot);
+    uint16_t* cl_slot = (uint16_t*)(cb + co.cl_slot); uint16_t* det_slot = (uint16_t*)(cb + co.det_slot);
+    for (uint32_t e = 0; e < kG * G.n_hh_rows; ++e) hh_slot[e] = kNoSlot16;
+    for (uint32_t e = 0; e < kG * G.n_syn_rows; ++e) syn_slot[e] = kNoSlot16;
+    for (uint32_t e = 0; e < kG * G.n_cl_rows; ++e) cl_slot[e] = kNoSlot16;
+    int64_t hh_pos = G.hh_base;
+    struct Item { uint32_t slot; int64_t id; };
+    std::vector<Item> items;
+    auto by_slot = [](const Item& x, const Item& y) { return x.slot != y.slot ? x.slot < y.slot : x.id < y.id; };
+    for (uint32_t lc = 0; lc < (uint32_t)kG; ++lc) {
+      double* rt = st + so.rt + kRtDoubles * lc;
+      rt[0] = std::numeric_limits<double>::infinity();
+      rt[1] = 0.0;
+      if (lc >= G.n_cell) {
+        // padding lane: an isolated, inert "cell" (V stays where it is, no instances, detector unarmed)
+        for (uint32_t s2 = 0; s2 < n; ++s2) {
+          const uint32_t e = s2 * kG + lc;
+          gen[go.C + e] = 1.0; st[so.v + e] = -65.0; invd[e] = 1.0; a[e] = 1.0;
+        }
+        det_slot[lc] = 0;
+        rt[2] = 0.0;
+        continue;
+      }
+      const int64_t orig = group_cells[G.cell_begin + lc];
+      const int64_t a0 = d.cv_off[orig];
+      const int32_t* par = d.cv_parent + a0;
+      std::vector<double> S(n, 0.0);
+      for (uint32_t i = 1; i < n; ++i) S[i] = 1.0 / d.cv_raxial[a0 + i];
+      for (uint32_t i = 1; i < n; ++i) S[par[i]] += 1.0 / d.cv_raxial[a0 + i];   // ascending child order
+      items.clear();
+      for (uint32_t i = 0; i < n; ++i) {
+        const uint32_t e = K.cv_slot[i] * kG + lc;
+        const double area = d.cv_area[a0 + i];
+        gen[go.C + e] = d.cv_cm[a0 + i] * area * 1e-5;                 // nF
+        gen[go.S + e] = S[i];                                          // uS
+        gen[go.sig + e] = i ? 1.0 / d.cv_raxial[a0 + i] : 0.0;         // uS
+        const double Gp = d.pas_g ? d.pas_g[a0 + i] * area * 1e-2 : 0.0;  // uS
+        gen[go.G + e] = Gp;
+        gen[go.b + e] = d.pas_g ? Gp * d.pas_e[a0 + i] : 0.0;          // nA
+        st[so.v + e] = d.cv_vinit ? d.cv_vinit[a0 + i] : -65.0;
+        H.cv_state_idx[a0 + i] = (uint32_t)(D.state_base + so.v + e);
+        if (d.hh_gnabar && (d.hh_gnabar[a0 + i] != 0.0 || d.hh_gkbar[a0 + i] != 0.0 || d.hh_gl[a0 + i] != 0.0)) items.push_back({K.cv_slot[i], (int64_t)i});
+      }
+      std::sort(items.begin(), items.end(), by_slot);
+      for (uint32_t j = 0; j < items.size(); ++j) {
+        const uint32_t e = j * kG + lc;
+        const int64_t gi = a0 + items[j].id;
+        const double sc = d.cv_area[gi] * 1e-2;
+        hh_gna[e] = d.hh_gnabar[gi] * sc; hh_gk[e] = d.hh_gkbar[gi] * sc; hh_gl[e] = d.hh_gl[gi] * sc;
+        hh_slot[e] = (uint16_t)items[j].slot;
+        H.hh_m_idx[hh_pos] = (uint32_t)(D.state_base + so.m + e);
+        H.hh_stride[hh_pos] = so.h - so.m;
+        H.hh_cv[hh_pos] = (uint32_t)gi;
+        ++hh_pos;
+      }
+      items.clear();
+      if (d.syn_off)
+        for (int64_t q = d.syn_off[orig]; q < d.syn_off[orig + 1]; ++q) items.push_back({K.cv_slot[d.syn_cv[q]], q});
+      std::sort(items.begin(), items.end(), by_slot);
+      for (uint32_t j = 0; j < items.size(); ++j) {
+        const uint32_t e = j * kG + lc;
+        syn_slot[e] = (uint16_t)items[j].slot;
+        if (!H.syn_uniform) syn_e[e] = d.syn_e[items[j].id];
+        gen[go.syn_tau + e] = d.syn_tau[items[j].id];
+        H.syn_state_idx[items[j].id] = (uint32_t)(D.state_base + so.g + e);
+      }
+      items.clear();
+      for (int64_t q = clamp_off[orig]; q < clamp_off[orig + 1]; ++q) items.push_back({K.cv_slot[d.clamp_cv[clamp_idx[q]]], clamp_idx[q]});
+      std::sort(items.begin(), items.end(), by_slot);
+      for (uint32_t j = 0; j < items.size(); ++j) {
+        const uint32_t e = j * kG + lc;
+        cl_slot[e] = (uint16_t)items[j].slot;
+        cl_t0[e] = d.clamp_t0[items[j].id]; cl_t1[e] = d.clamp_t1[items[j].id]; cl_amp[e] = d.clamp_amp[items[j].id];
+      }
+      det_slot[lc] = (uint16_t)K.cv_slot[d.det_cv ? d.det_cv[orig] : 0];
+      rt[2] = 1.0;                                                     // detector armed (reading R10)
+      H.cell_rt_idx[G.cell_begin + lc] = (uint32_t)(D.state_base + so.rt + kRtDoubles * lc);
+    }
+    // padding rows of syn_tau must stay finite for exp(-delta / tau)
+    for (uint32_t e = 0; e < kG * G.n_syn_rows; ++e) if (syn_slot[e] == kNoSlot16) gen[go.syn_tau + e] = 1.0;
+  });
   for (int64_t u = 0; u < H.n_units; ++u) {
     if (topo_owner[u] == u) std::memcpy(H.topo.data() + H.units[u].topo_off, topo[u].data(), topo[u].size());
     UnitDesc& ud = H.descs[u];

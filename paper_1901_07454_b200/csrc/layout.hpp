@@ -6,6 +6,7 @@
 #include <vector>
 
 #include "../../include/arbb200.h"
+#include "group_layout.h"
 #include "unit_layout.h"
 
 namespace arbb {
@@ -13,7 +14,12 @@ namespace arbb {
 struct BuildParams {
   uint32_t unit_bytes = 22528;    // fast + state bytes a warp unit may hold (one shared-memory stage)
   uint32_t max_branch_len = 1024; // longer unbranched chains are cut into pieces
+  uint32_t group_min_cells = 4;   // a topology class with fewer cells is laid out as units; 0 = no groups
+  uint32_t group_max_cv = 1536;   // cells with more control volumes are laid out as units (V of a
+                                  // group must fit in shared memory: 8 * kG bytes per control volume)
 };
+
+constexpr int64_t kMaxGroupCtas = 148 * 16;   // upper bound of resident CTAs of the group kernel (scratch sizing)
 
 constexpr int64_t kMaxWarps = 2048;   // upper bound of resident warps of the warp kernel (scratch sizing)
 
@@ -38,6 +44,10 @@ struct HostModel {
   double syn_tau_u = 0, syn_e_u = 0;
   double min_delay = 0, max_delay = 0;
   double ena = 0, ek = 0, el = 0, threshold = 0;
+  // cell groups: cells [0, n_group_cells) of the internal order
+  int64_t n_groups = 0, n_group_cells = 0, n_classes = 0;
+  uint32_t g_slot_cap = 0, g_buf_rows = 0, g_seg_cap = 0;
+  std::vector<GroupDesc> gdescs;
   std::vector<UnitCounts> units;
   std::vector<uint32_t> cell_order;     // internal -> caller's cell id
   std::vector<uint32_t> cell_internal;  // caller's cell id -> internal

@@ -28,6 +28,15 @@ def B():
     return binding
 
 
+@pytest.fixture(params=["default", "groups", "units"], autouse=True)
+def layout(request, B):
+    """Every test runs under three layouts: the default (cells of a topology class of >= 4 cells in
+    cell-interleaved groups, the rest in branch-interleaved units), every cell in groups, no groups."""
+    B.configure(B.ARB_CFG_GROUP_MIN_CELLS, {"default": 0, "groups": 1, "units": 2 ** 31}[request.param])
+    yield request.param
+    B.configure(B.ARB_CFG_GROUP_MIN_CELLS, 0)
+
+
 def rel(a, b):
     return float(np.max(np.abs(a - b) / np.maximum(np.abs(b), 1.0))) if len(a) else 0.0
 
@@ -295,10 +304,12 @@ def test_spike_buffer_cap_and_order(B, orc):
 # ---------------------------------------------------------------------------------------------
 # full-size configuration, sampled cells
 # ---------------------------------------------------------------------------------------------
-def test_full_size_large_config_sampled_cells(B, orc):
+def test_full_size_large_config_sampled_cells(B, orc, layout):
     """configs[3] at its full 100,000 cells, in the launch configuration bench.py times.  Until the
     first network event can arrive (one minimum delay, 5 ms = 200 steps) every cell depends only on
     its own external events, so the oracle can integrate a sample of cells on its own."""
+    if layout != "default":
+        pytest.skip("full size runs once, in the layout bench.py times")
     m = W.config3()
     g = B.Model(m)
     g.advance(5.0, DT)
