@@ -54,6 +54,8 @@ enum {
   ARB_OPT_EPOCH_STEPS = 2,   /* cap on the epoch length in steps (default: floor(min delay / dt)) */
   ARB_OPT_STAGES = 4,        /* shared-memory stages per warp of the cable kernel: 0 (default) = 2 when
                                 every launch streams the state once, 1 when launches are fused     */
+  ARB_OPT_L2_PREFETCH = 5,   /* cell-group kernel: 1 (default) = ask the TMA unit to pull the next group's
+                                records into L2 while the current group is integrated; 0 = off      */
   ARB_OPT_TIMING = 3         /* 1: bracket the cable-step launches and the epoch-boundary kernels of
                                 every epoch with CUDA events on the model's stream (read them with
                                 ARB_PROBE_TIMING); setting the option clears the accumulated times  */

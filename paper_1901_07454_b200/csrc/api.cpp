@@ -50,7 +50,7 @@ Caps capacities(const HostModel& H) {
 }
 
 // group kernel: per resident CTA fgen | invdgen for event-split sub-steps
-int64_t gscratch_stride(const HostModel& H) { return 2 * (int64_t)H.g_slot_cap * kG; }
+int64_t gscratch_stride(const HostModel& H) { return 2 * (int64_t)H.gcaps.slot_cap * kG; }
 int64_t gscratch_ctas(const HostModel& H) { return std::min<int64_t>(H.n_groups, kMaxGroupCtas); }
 
 int64_t warp_scratch_stride(const HostModel& H) { return 2 * (int64_t)H.slot_cap + align_up(H.lane_cap, 2); }
@@ -209,7 +209,8 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     if (reinterpret_cast<uintptr_t>(dev_workspace) % 256) { delete m; return fail(nullptr, ARB_E_WORKSPACE, "arb_create: workspace must be 256-byte aligned"); }
     m->ws = static_cast<char*>(dev_workspace);
     m->stream = static_cast<cudaStream_t>(cuda_stream);
-    if (H.n_groups > 0 && group_ctas_per_sm(group_smem_plan(H.g_slot_cap, H.g_buf_rows).bytes) == 0) { delete m; return fail(nullptr, ARB_E_INVALID, "arb_create: a cell group does not fit in shared memory"); }
+    int group_ctas = 0;
+    if (H.n_groups > 0 && (group_ctas = group_ctas_per_sm(group_smem_plan(H.gcaps).bytes)) == 0) { delete m; return fail(nullptr, ARB_E_INVALID, "arb_create: a cell group does not fit in shared memory"); }
     if (H.n_warp_units > 0 && make_plan(H, 1).warps == 0) { delete m; return fail(nullptr, ARB_E_INVALID, "arb_create: a warp unit does not fit in shared memory"); }
     {
       int dev = 0, sms = 0;
@@ -269,9 +270,10 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     D.plan = make_plan(H, 1);
     D.groups = at<GroupDesc>(m, R.gdescs); D.n_groups = H.n_groups;
     D.gscratch = at<double>(m, R.gscratch); D.gscratch_stride = gscratch_stride(H);
-    D.gplan = group_smem_plan(H.g_slot_cap, H.g_buf_rows);
+    D.gplan = group_smem_plan(H.gcaps);
+    D.l2_prefetch = 1;
     if (H.n_groups > 0)
-      m->group_grid = (int)std::min<int64_t>(gscratch_ctas(H), (int64_t)m->sm_count * group_ctas_per_sm(D.gplan.bytes));
+      m->group_grid = (int)std::min<int64_t>(gscratch_ctas(H), (int64_t)m->sm_count * group_ctas);
     D.pool_cap = m->cap.pool;
     D.spike_cell = at<uint32_t>(m, R.spike_cell); D.spike_t = at<double>(m, R.spike_t); D.spike_cap = m->cap.spikes;
     D.counters = at<unsigned long long>(m, R.counters);
@@ -514,6 +516,7 @@ int arb_set_option(arb_model* m, int key, int64_t value) {
     case ARB_OPT_FUSED_STEPS: m->opt_fused = value; return ARB_OK;
     case ARB_OPT_EPOCH_STEPS: m->opt_epoch = value; return ARB_OK;
     case ARB_OPT_STAGES: m->opt_stages = value; return ARB_OK;
+    case ARB_OPT_L2_PREFETCH: m->D.l2_prefetch = value != 0; return ARB_OK;
     case ARB_OPT_TIMING:
       m->opt_timing = value;
       m->cable_ms = m->event_ms = 0; m->cable_timed = m->event_timed = 0;

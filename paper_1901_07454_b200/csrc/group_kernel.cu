@@ -1,23 +1,29 @@
 // group_kernel.cu - the cable step for cell groups (group_layout.h): cells of one topology class,
 // stored cell-interleaved, lane = cell.
 //
-//   cable_group_kernel   persistent grid, one CTA integrates one group at a time.  The group's
-//                        voltages arrive in shared memory by one bulk-async copy (TMA,
-//                        cp.async.bulk + mbarrier) and leave by one bulk store; the coefficient
-//                        rows (a, b, f, 1/d) stream from HBM / L2 straight into registers with
-//                        coalesced loads, eight rows in flight per lane group; the next group's
-//                        records are pulled into L2 by a TMA prefetch while this one is integrated.
+//   cable_group_kernel   persistent grid, one CTA integrates one group at a time, several CTAs per SM.
+//                        Everything a group-step touches more than once lives in shared memory and
+//                        arrives there by bulk-async copies (TMA, cp.async.bulk + one mbarrier): the
+//                        state record (V, synaptic g, per-cell runtime, gates), the solver factors f
+//                        and 1/d, and the tail of the const record (instance tables).  The rhs
+//                        coefficients a, b are used once and stream from L2 (pulled there ahead of
+//                        time by a TMA L2 prefetch) into registers.  V, g and the runtime leave by one
+//                        bulk store.  The class record (segments, stages) is kept in shared memory.
 //                        Per grid step (or fused run of steps): event delivery ->
 //                        mechanism currents (eq 2a) -> rhs of the implicit Euler system
 //                         -> Hines / branched Thomas sweeps: the class
 //                        schedule cuts the tree into stages of independent chunks, the CTA's lane
 //                        groups eliminate the chunks of a stage concurrently -> V <- V' -> gate and
 //                        synapse state update with V' -> threshold test.
+//                        The gate update (fp64 exp and divide chains) of a group's last step is
+//                        carried in registers and overlaps the next group's copies.
 //   group_factor_kernel  once per dt: eliminates the constant matrix (reading R1) of every group
 //   group_init_kernel    gates at their steady state for the initial voltage (reading R4)
 //
 // HBM-bound by design: 48 B per control volume and step (V in + out, a, b, f, 1/d) against ~6 fp64
 // instructions.  No tensor cores: nothing here is a dense contraction.
+#include <cstdio>
+
 #include "device_common.cuh"
 #include "group_layout.h"
 #include "kernels.cuh"
@@ -27,49 +33,78 @@ namespace arbb {
 namespace {
 
 constexpr int kT = kGroupThreads;
-constexpr int kRows = 8;                  // rows a lane group keeps in flight in a sweep
+constexpr int kRows = 4;                  // rows of a segment a lane group loads ahead of the recurrence
 
+// -DARBB_PROFILE: one CTA prints clock64() at the phase boundaries of a few group-steps (development aid)
+#ifdef ARBB_PROFILE
+#define TICK(i) do { if (prof) prof[i] = clock64(); } while (0)
+#else
+#define TICK(i) do { } while (0)
+#endif
+
+// Pointers of one group.  "s" pointers address the CTA's shared memory, "g" pointers global memory.
+// Rarely used arrays (clamps, non-uniform synapse parameters, the dt-independent "gen" arrays of
+// event-split sub-steps) are derived on demand, which keeps the kernel's register count down.
 struct GView {
   uint32_t n_cv, n_cell, n_hh, n_syn, n_cl;          // rows
-  const double *f, *invd, *a, *b, *hh_gna, *hh_gk, *hh_gl, *syn_e, *syn_decay, *cl_t0, *cl_t1, *cl_amp;
-  const uint16_t *hh_slot, *syn_slot, *cl_slot, *det_slot;
-  double *gV, *gm, *gh, *gn, *gg, *grt;
-  const double *C, *S, *sig, *G, *bg, *syn_tau;
-  const SegRec* segs;
+  uint32_t n_stage, n_block;
+  uint32_t hh_cs, hh_ss;                             // doubles between gna|gk|gl and between m|h|n
+  int syn_uniform;
+  const uint8_t* tail;                               // const record from hh_gna on
+  const double* gen;                                 // global: gen record
+  const double *a, *b;                               // global
+  const double* hh_gna;
+  const uint16_t *hh_slot, *syn_slot, *det_slot;
+  double *sm, *sg, *srt;                             // gates m (h, n follow), g, runtime: working copy
+  double* gm;                                        // global: gates m (h, n follow)
+  const SegRec* segs;                                // class record
   const uint16_t *order, *sched, *child;
-  uint32_t n_stage, n_seg;
   int64_t cell_base;
+
+  __device__ __forceinline__ GConstOff co() const { return gconst_offsets(n_cv, n_hh, n_syn, n_cl, syn_uniform != 0); }
+  __device__ __forceinline__ const uint8_t* tl(uint32_t off) const { return tail + (off - co().hh_gna); }
+  __device__ __forceinline__ const double* syn_e() const { return (const double*)tl(co().syn_e); }
+  __device__ __forceinline__ const double* syn_decay() const { return (const double*)tl(co().syn_decay); }
+  __device__ __forceinline__ const double* cl_t0() const { return (const double*)tl(co().cl_t0); }
+  __device__ __forceinline__ const double* cl_t1() const { return (const double*)tl(co().cl_t1); }
+  __device__ __forceinline__ const double* cl_amp() const { return (const double*)tl(co().cl_amp); }
+  __device__ __forceinline__ const uint16_t* cl_slot() const { return (const uint16_t*)tl(co().cl_slot); }
+  __device__ __forceinline__ const double* C() const { return gen + ggen_offsets(n_cv, n_syn).C; }
+  __device__ __forceinline__ const double* S() const { return gen + ggen_offsets(n_cv, n_syn).S; }
+  __device__ __forceinline__ const double* sig() const { return gen + ggen_offsets(n_cv, n_syn).sig; }
+  __device__ __forceinline__ const double* G() const { return gen + ggen_offsets(n_cv, n_syn).G; }
+  __device__ __forceinline__ const double* bg() const { return gen + ggen_offsets(n_cv, n_syn).b; }
+  __device__ __forceinline__ const double* syn_tau() const { return gen + ggen_offsets(n_cv, n_syn).syn_tau; }
 };
 
-__device__ __forceinline__ void make_gview(GView& U, const DevModel& M, const GroupDesc& D) {
+// `state`, `tail`, `cls`: where the group's state record, const-record tail and class record are
+// (shared memory in the cable kernel, global memory in the factor / init kernels).
+__device__ __forceinline__ void make_gview(GView& U, const DevModel& M, const GroupDesc& D, double* state, const uint8_t* tail,
+                                           const uint8_t* cls) {
   U.n_cv = D.n_cv; U.n_cell = D.n_cell; U.n_hh = D.n_hh_rows; U.n_syn = D.n_syn_rows; U.n_cl = D.n_cl_rows;
+  U.syn_uniform = M.syn_uniform;
   const GConstOff co = gconst_offsets(D.n_cv, D.n_hh_rows, D.n_syn_rows, D.n_cl_rows, M.syn_uniform != 0);
   const uint8_t* cb = M.fast + D.const_off;
-  U.f = (const double*)(cb + co.f); U.invd = (const double*)(cb + co.invd);
+  U.tail = tail;
   U.a = (const double*)(cb + co.a); U.b = (const double*)(cb + co.b);
-  U.hh_gna = (const double*)(cb + co.hh_gna); U.hh_gk = (const double*)(cb + co.hh_gk); U.hh_gl = (const double*)(cb + co.hh_gl);
-  U.syn_e = (const double*)(cb + co.syn_e); U.syn_decay = (const double*)(cb + co.syn_decay);
-  U.cl_t0 = (const double*)(cb + co.cl_t0); U.cl_t1 = (const double*)(cb + co.cl_t1); U.cl_amp = (const double*)(cb + co.cl_amp);
-  U.hh_slot = (const uint16_t*)(cb + co.hh_slot); U.syn_slot = (const uint16_t*)(cb + co.syn_slot);
-  U.cl_slot = (const uint16_t*)(cb + co.cl_slot); U.det_slot = (const uint16_t*)(cb + co.det_slot);
+  U.hh_gna = (const double*)tail; U.hh_cs = (co.hh_gk - co.hh_gna) / 8;
+  U.hh_slot = (const uint16_t*)(tail + (co.hh_slot - co.hh_gna)); U.syn_slot = (const uint16_t*)(tail + (co.syn_slot - co.hh_gna));
+  U.det_slot = (const uint16_t*)(tail + (co.det_slot - co.hh_gna));
   const GStateOff so = gstate_offsets(D.n_cv, D.n_hh_rows, D.n_syn_rows);
-  double* gs = M.state + D.state_base;
-  U.gV = gs + so.v; U.gm = gs + so.m; U.gh = gs + so.h; U.gn = gs + so.n; U.gg = gs + so.g; U.grt = gs + so.rt;
-  const GGenOff go = ggen_offsets(D.n_cv, D.n_syn_rows);
-  const double* gen = M.gen + D.gen_base;
-  U.C = gen + go.C; U.S = gen + go.S; U.sig = gen + go.sig; U.G = gen + go.G; U.bg = gen + go.b; U.syn_tau = gen + go.syn_tau;
-  const uint8_t* cp = M.topo + D.class_off;
-  const ClassRecord* R = (const ClassRecord*)cp;
-  U.n_stage = R->n_stage; U.n_seg = R->n_seg;
-  U.segs = (const SegRec*)(cp + R->off_segs);
-  U.order = (const uint16_t*)(cp + R->off_order);
-  U.sched = (const uint16_t*)(cp + R->off_sched);
-  U.child = (const uint16_t*)(cp + R->off_child);
+  U.sm = state + so.m; U.hh_ss = so.h - so.m; U.sg = state + so.g; U.srt = state + so.rt;
+  U.gm = M.state + D.state_base + so.m;
+  U.gen = M.gen + D.gen_base;
+  const ClassRecord* R = (const ClassRecord*)cls;
+  U.n_stage = R->n_stage; U.n_block = R->n_block;
+  U.segs = (const SegRec*)(cls + R->off_segs);
+  U.order = (const uint16_t*)(cls + R->off_order);
+  U.sched = (const uint16_t*)(cls + R->off_sched);
+  U.child = (const uint16_t*)(cls + R->off_child);
   U.cell_base = D.cell_base;
 }
 
 __device__ __forceinline__ SegRec load_seg(const SegRec* p) {
-  const uint4 q = __ldg((const uint4*)p);
+  const uint4 q = *(const uint4*)p;
   SegRec s;
   s.slot0 = q.x; s.pslot = q.y; s.len = (uint16_t)(q.z & 0xFFFFu); s.ccnt = (uint16_t)(q.z >> 16); s.cbeg = q.w;
   return s;
@@ -82,19 +117,20 @@ __device__ __forceinline__ SegRec load_seg(const SegRec* p) {
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ void eliminate_seg(const GView& U, const SegRec& sg, uint32_t seg_idx, int c, double delta,
                                               double* fout, double* invdout, double* dcon) {
+  const double *C = U.C(), *S = U.S(), *sig = U.sig();
   uint32_t s = (sg.slot0 + sg.len - 1) * kG + c;
-  double d = U.C[s] / delta + U.S[s];
+  double d = C[s] / delta + S[s];
   for (uint32_t j = 0; j < sg.ccnt; ++j) d -= dcon[(uint32_t)U.child[sg.cbeg + j] * kG + c];
   double fk = 0.0, sk = 0.0;
   for (uint32_t k = sg.len; k-- > 0;) {
     const double invd = 1.0 / d;
-    sk = U.sig[s];
+    sk = sig[s];
     fk = -sk * invd;
     fout[s] = fk;
     invdout[s] = invd;
     if (k > 0) {
       s -= kG;
-      d = fma(fk, sk, U.C[s] / delta + U.S[s]);      // d_p -= f*u with u = -sigma
+      d = fma(fk, sk, C[s] / delta + S[s]);          // d_p -= f*u with u = -sigma
     }
   }
   dcon[seg_idx * kG + c] = -fk * sk;
@@ -104,6 +140,7 @@ __device__ __forceinline__ void eliminate_seg(const GView& U, const SegRec& sg, 
 // Backward (leaves -> root) sweep of one segment on the rhs held in Vs:
 //   rhs_{k-1} -= f_k rhs_k along the segment; the parent control volume loses con[segment] = f_0 rhs_0;
 // every control volume is left holding rhs_k / d_k, which is what the forward sweep needs.
+// F, I: the factors f and 1/d (shared memory; the cell's own re-elimination on event-split sub-steps).
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ void backward_seg(const GView& U, const SegRec& sg, uint32_t seg_idx, int c,
                                              const double* __restrict__ F, const double* __restrict__ I,
@@ -155,19 +192,109 @@ __device__ __forceinline__ void forward_seg(const SegRec& sg, int c, const doubl
   }
 }
 
+__device__ __forceinline__ void backward_stage(const GView& U, uint32_t st, int h, int c, bool on, const double* F,
+                                               const double* I, double* Vs, double* con) {
+  const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
+  if (on)
+    for (uint32_t q = beg; q < end; ++q) {
+      const uint32_t si = U.order[q];
+      backward_seg(U, load_seg(U.segs + si), si, c, F, I, Vs, con);
+    }
+}
+__device__ __forceinline__ void forward_stage(const GView& U, uint32_t st, int h, int c, bool on, const double* F, double* Vs) {
+  const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
+  if (on)
+    for (uint32_t q = end; q-- > beg;) forward_seg(load_seg(U.segs + U.order[q]), c, F, Vs);
+}
+
+// Both sweeps.  Stages [0, n_block) hold chunks on lane groups of several warps: block barriers.
+// Stages [n_block, n_stage) only use the lane groups of warp 0: it runs them back to back, backward
+// and then forward, with warp barriers only.
+__device__ __forceinline__ void sweeps(const GView& U, int h, int c, bool on, const double* F, const double* I,
+                                       double* Vs, double* con, long long* prof) {
+  const uint32_t n_stage = U.n_stage, n_block = U.n_block;
+  for (uint32_t st = 0; st < n_block; ++st) {
+    backward_stage(U, st, h, c, on, F, I, Vs, con);
+    __syncthreads();
+  }
+  TICK(8);
+  if (threadIdx.x < 32) {
+    for (uint32_t st = n_block; st < n_stage; ++st) {
+      backward_stage(U, st, h, c, on, F, I, Vs, con);
+      __syncwarp();
+    }
+    for (uint32_t st = n_stage; st-- > n_block;) {
+      forward_stage(U, st, h, c, on, F, Vs);
+      __syncwarp();
+    }
+  }
+  TICK(9);
+  for (uint32_t st = n_block; st-- > 0;) {
+    __syncthreads();
+    forward_stage(U, st, h, c, on, F, Vs);
+  }
+  TICK(10);
+}
+
+// ------------------------------------------------------------------------------------------
+// HH gate update x <- x_inf(V') + (x - x_inf) exp(-delta (alpha + beta)) (reading R5),
+// deferred: phase F only captures (V', delta, m, h, n) in registers; the exp / divide chains run
+// later, off the critical path of the CTA.
+// ------------------------------------------------------------------------------------------
+constexpr int kHHDefer = 1;       // HH instances per thread that can be deferred
+
+struct HHDefer {
+  double v[kHHDefer], delta[kHHDefer], m[kHHDefer], h[kHHDefer], n[kHHDefer];
+  uint32_t e[kHHDefer];           // kNoSlot: empty
+};
+__device__ __forceinline__ void clear(HHDefer& d) {
+#pragma unroll
+  for (int i = 0; i < kHHDefer; ++i) d.e[i] = kNoSlot;
+}
+
+__device__ __forceinline__ void hh_gates(double v, double delta, double& m, double& h, double& n) {
+  const Rates r = hh_rates(v);
+  double inf = r.am / (r.am + r.bm);
+  m = inf + (m - inf) * exp(-delta * (r.am + r.bm));
+  inf = r.ah / (r.ah + r.bh);
+  h = inf + (h - inf) * exp(-delta * (r.ah + r.bh));
+  inf = r.an / (r.an + r.bn);
+  n = inf + (n - inf) * exp(-delta * (r.an + r.bn));
+}
+
+// run the deferred updates; results go to dst0 and (when not null) dst1: m at [e], h and n at +ss, +2 ss
+__device__ __forceinline__ void run_deferred(HHDefer& dh, double* dst0, double* dst1, uint32_t ss) {
+#pragma unroll
+  for (int i = 0; i < kHHDefer; ++i)
+    if (dh.e[i] != kNoSlot) {
+      double m = dh.m[i], h = dh.h[i], n = dh.n[i];
+      hh_gates(dh.v[i], dh.delta[i], m, h, n);
+      double* p = dst0 + dh.e[i];
+      p[0] = m; p[ss] = h; p[2 * ss] = n;
+      if (dst1) { p = dst1 + dh.e[i]; p[0] = m; p[ss] = h; p[2 * ss] = n; }
+      dh.e[i] = kNoSlot;
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // One (sub-)step of every active cell of the group (phases B..F; phase A, event delivery and the
-// choice of the sub-step, is in the kernel body).  md / delta are this thread's cell's.
+// choice of the sub-step, is in the kernel body).  Point-mechanism instances are dealt to threads
+// from the END of the CTA (thread kT-1 first) so that they do not land on warp 0, which owns the
+// serial parts (phase A, the narrow stages).  The HH gate updates come back deferred in `dh`.
 // ------------------------------------------------------------------------------------------
-__device__ __forceinline__ void group_substep(const DevModel& M, const GView& U, double* Vs, double* buf, const CellS& cs,
-                                              double* fgen, double* invdgen, bool any_gen, uint32_t md, double delta) {
+template <bool kGen>
+__device__ __forceinline__ void group_substep(const DevModel& M, const GView& U, double* Vs, const double* Fs, const double* Is,
+                                              double* buf, const CellS& cs, double* fgen, double* invdgen, double dt, HHDefer& dh,
+                                              long long* prof) {
   const int tid = threadIdx.x, c = tid % kG, h = tid / kG;
+  const int rtid = kT - 1 - tid, rc = rtid % kG;      // reversed dealing of instances; cell of those
   const uint32_t nE_cv = U.n_cv * kG, nE_hh = U.n_hh * kG, nE_syn = U.n_syn * kG, nE_cl = U.n_cl * kG;
-  const uint32_t n_stage = U.n_stage;
+  const uint32_t md = kGen ? cs.mode[c] : 1u, rmd = kGen ? cs.mode[rc] : 1u;
+  const double delta = kGen ? cs.delta[c] : dt, rdelta = kGen ? cs.delta[rc] : dt;
 
   // ---- event-split sub-steps: this cell's matrix is re-eliminated for its own delta (reading R9)
-  if (any_gen) {
-    for (uint32_t st = 0; st < n_stage; ++st) {
+  if (kGen) {
+    for (uint32_t st = 0; st < U.n_stage; ++st) {
       const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
       if (md == 2u)
         for (uint32_t q = beg; q < end; ++q) {
@@ -181,123 +308,132 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
   // ---- B: currents of HH, synapses and clamps from V(t); the passive current is
   // folded into a, b.  Items of one cell on one CV form a run; its first item sums it in index order.
   double* xI = buf;
-  for (uint32_t e = tid; e < nE_hh; e += kT) {
+  for (uint32_t e = rtid; e < nE_hh; e += kT) {
     const uint32_t slot = U.hh_slot[e];
-    if (slot == kNoSlot16 || !md) continue;
-    const double v = Vs[slot * kG + c];
-    const double m = U.gm[e], hh = U.gh[e], n = U.gn[e];
-    xI[e] = U.hh_gna[e] * m * m * m * hh * (v - M.ena) + U.hh_gk[e] * n * n * n * n * (v - M.ek) + U.hh_gl[e] * (v - M.el);
+    if (slot == kNoSlot16 || !rmd) continue;
+    const double v = Vs[slot * kG + rc];
+    const double m = U.sm[e], hh = U.sm[e + U.hh_ss], n = U.sm[e + 2 * U.hh_ss];
+    xI[e] = U.hh_gna[e] * m * m * m * hh * (v - M.ena) + U.hh_gna[e + U.hh_cs] * n * n * n * n * (v - M.ek) +
+            U.hh_gna[e + 2 * U.hh_cs] * (v - M.el);
   }
-  for (uint32_t e = tid; e < nE_syn; e += kT) {
+  for (uint32_t e = rtid; e < nE_syn; e += kT) {
     const uint32_t slot = U.syn_slot[e];
-    if (slot == kNoSlot16 || !md) continue;
+    if (slot == kNoSlot16 || !rmd) continue;
     if (e >= (uint32_t)kG && U.syn_slot[e - kG] == slot) continue;
-    const double v = Vs[slot * kG + c];
+    const double v = Vs[slot * kG + rc];
     double I = 0.0;
     uint32_t j = e;
     do {
-      I += U.gg[j] * (v - (M.syn_uniform ? M.syn_e_u : U.syn_e[j]));
+      I += U.sg[j] * (v - (M.syn_uniform ? M.syn_e_u : U.syn_e()[j]));
       j += kG;
     } while (j < nE_syn && U.syn_slot[j] == slot);
     xI[nE_hh + e] = I;
   }
+  TICK(3);
   if (nE_cl) {
-    const double t = cs.tcur[c];
-    for (uint32_t e = tid; e < nE_cl; e += kT) {
-      const uint32_t slot = U.cl_slot[e];
-      if (slot == kNoSlot16 || !md) continue;
-      if (e >= (uint32_t)kG && U.cl_slot[e - kG] == slot) continue;
+    const double t = cs.tcur[rc];
+    const uint16_t* cl_slot = U.cl_slot();
+    const double *cl_t0 = U.cl_t0(), *cl_t1 = U.cl_t1(), *cl_amp = U.cl_amp();
+    for (uint32_t e = rtid; e < nE_cl; e += kT) {
+      const uint32_t slot = cl_slot[e];
+      if (slot == kNoSlot16 || !rmd) continue;
+      if (e >= (uint32_t)kG && cl_slot[e - kG] == slot) continue;
       double I = 0.0;
       uint32_t j = e;
       do {
-        if (U.cl_t0[j] <= t && t < U.cl_t1[j]) I -= U.cl_amp[j];
+        if (cl_t0[j] <= t && t < cl_t1[j]) I -= cl_amp[j];
         j += kG;
-      } while (j < nE_cl && U.cl_slot[j] == slot);
+      } while (j < nE_cl && cl_slot[j] == slot);
       xI[nE_hh + nE_syn + e] = I;
     }
   }
   __syncthreads();
+  TICK(4);
 
   // ---- C: rhs_i = (C_i/delta - G_i) V_i + G_i e_i - I_i, in place of V
   if (md == 1u) {
-    uint32_t e = tid;
-    for (; e + 3 * kT < nE_cv; e += 4 * kT) {
-      const double a0 = U.a[e], a1 = U.a[e + kT], a2 = U.a[e + 2 * kT], a3 = U.a[e + 3 * kT];
-      const double b0 = U.b[e], b1 = U.b[e + kT], b2 = U.b[e + 2 * kT], b3 = U.b[e + 3 * kT];
-      Vs[e] = fma(a0, Vs[e], b0); Vs[e + kT] = fma(a1, Vs[e + kT], b1);
-      Vs[e + 2 * kT] = fma(a2, Vs[e + 2 * kT], b2); Vs[e + 3 * kT] = fma(a3, Vs[e + 3 * kT], b3);
+    for (uint32_t e = tid; e < nE_cv; e += 8 * kT) {
+      double ar[8], br[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j)
+        if (e + j * kT < nE_cv) { ar[j] = U.a[e + j * kT]; br[j] = U.b[e + j * kT]; }
+#pragma unroll
+      for (int j = 0; j < 8; ++j)
+        if (e + j * kT < nE_cv) Vs[e + j * kT] = fma(ar[j], Vs[e + j * kT], br[j]);
     }
-    for (; e < nE_cv; e += kT) Vs[e] = fma(U.a[e], Vs[e], U.b[e]);
-  } else if (md == 2u) {
-    for (uint32_t e = tid; e < nE_cv; e += kT) Vs[e] = fma(U.C[e] / delta - U.G[e], Vs[e], U.bg[e]);
+  } else if (kGen && md == 2u) {
+    const double *C = U.C(), *G = U.G(), *bg = U.bg();
+    for (uint32_t e = tid; e < nE_cv; e += kT) Vs[e] = fma(C[e] / delta - G[e], Vs[e], bg[e]);
   }
+  TICK(5);
   __syncthreads();
+  TICK(6);
   if (nE_hh) {
-    for (uint32_t e = tid; e < nE_hh; e += kT) {
+    for (uint32_t e = rtid; e < nE_hh; e += kT) {
       const uint32_t slot = U.hh_slot[e];
-      if (slot == kNoSlot16 || !md) continue;
-      Vs[slot * kG + c] -= xI[e];
+      if (slot == kNoSlot16 || !rmd) continue;
+      Vs[slot * kG + rc] -= xI[e];
     }
     __syncthreads();
   }
   if (nE_syn) {
-    for (uint32_t e = tid; e < nE_syn; e += kT) {
+    for (uint32_t e = rtid; e < nE_syn; e += kT) {
       const uint32_t slot = U.syn_slot[e];
-      if (slot == kNoSlot16 || !md) continue;
+      if (slot == kNoSlot16 || !rmd) continue;
       if (e >= (uint32_t)kG && U.syn_slot[e - kG] == slot) continue;
-      Vs[slot * kG + c] -= xI[nE_hh + e];
+      Vs[slot * kG + rc] -= xI[nE_hh + e];
     }
     __syncthreads();
   }
   if (nE_cl) {
-    for (uint32_t e = tid; e < nE_cl; e += kT) {
-      const uint32_t slot = U.cl_slot[e];
-      if (slot == kNoSlot16 || !md) continue;
-      if (e >= (uint32_t)kG && U.cl_slot[e - kG] == slot) continue;
-      Vs[slot * kG + c] -= xI[nE_hh + nE_syn + e];
+    const uint16_t* cl_slot = U.cl_slot();
+    for (uint32_t e = rtid; e < nE_cl; e += kT) {
+      const uint32_t slot = cl_slot[e];
+      if (slot == kNoSlot16 || !rmd) continue;
+      if (e >= (uint32_t)kG && cl_slot[e - kG] == slot) continue;
+      Vs[slot * kG + rc] -= xI[nE_hh + nE_syn + e];
     }
     __syncthreads();
   }
 
+  TICK(7);
   // ---- D: backward sweep, stage by stage; E: forward substitution, stages reversed; V <- V'
-  const double* F = md == 2u ? fgen : U.f;
-  const double* I = md == 2u ? invdgen : U.invd;
-  double* con = buf;                    // xI is dead
-  for (uint32_t st = 0; st < n_stage; ++st) {
-    const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
-    if (md)
-      for (uint32_t q = beg; q < end; ++q) {
-        const uint32_t si = U.order[q];
-        backward_seg(U, load_seg(U.segs + si), si, c, F, I, Vs, con);
-      }
-    __syncthreads();
-  }
-  for (uint32_t st = n_stage; st-- > 0;) {
-    const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
-    if (md)
-      for (uint32_t q = end; q-- > beg;) forward_seg(load_seg(U.segs + U.order[q]), c, F, Vs);
-    __syncthreads();
-  }
+  if (kGen) sweeps(U, h, c, md != 0u, md == 2u ? fgen : Fs, md == 2u ? invdgen : Is, Vs, buf, prof);
+  else sweeps(U, h, c, true, Fs, Is, Vs, buf, prof);   // buf: xI is dead, it now holds the contributions
+  __syncthreads();
+  TICK(11);
 
   // ---- F: state update with V', threshold test
-  for (uint32_t e = tid; e < nE_hh; e += kT) {
-    const uint32_t slot = U.hh_slot[e];
-    if (slot == kNoSlot16 || !md) continue;
-    const Rates r = hh_rates(Vs[slot * kG + c]);
-    double inf = r.am / (r.am + r.bm);
-    U.gm[e] = inf + (U.gm[e] - inf) * exp(-delta * (r.am + r.bm));
-    inf = r.ah / (r.ah + r.bh);
-    U.gh[e] = inf + (U.gh[e] - inf) * exp(-delta * (r.ah + r.bh));
-    inf = r.an / (r.an + r.bn);
-    U.gn[e] = inf + (U.gn[e] - inf) * exp(-delta * (r.an + r.bn));
+  {
+    uint32_t e = rtid;
+#pragma unroll
+    for (int i = 0; i < kHHDefer; ++i, e += kT) {
+      dh.e[i] = kNoSlot;
+      if (e < nE_hh) {
+        const uint32_t slot = U.hh_slot[e];
+        if (slot != kNoSlot16 && rmd) {
+          dh.v[i] = Vs[slot * kG + rc]; dh.delta[i] = rdelta; dh.e[i] = e;
+          dh.m[i] = U.sm[e]; dh.h[i] = U.sm[e + U.hh_ss]; dh.n[i] = U.sm[e + 2 * U.hh_ss];
+        }
+      }
+    }
+    for (; e < nE_hh; e += kT) {          // more instances than can be deferred: update in place
+      const uint32_t slot = U.hh_slot[e];
+      if (slot == kNoSlot16 || !rmd) continue;
+      double m = U.sm[e], hh = U.sm[e + U.hh_ss], n = U.sm[e + 2 * U.hh_ss];
+      hh_gates(Vs[slot * kG + rc], rdelta, m, hh, n);
+      U.sm[e] = m; U.sm[e + U.hh_ss] = hh; U.sm[e + 2 * U.hh_ss] = n;
+      U.gm[e] = m; U.gm[e + U.hh_ss] = hh; U.gm[e + 2 * U.hh_ss] = n;
+    }
   }
-  if (md) {
-    for (uint32_t e = tid; e < nE_syn; e += kT) {
+  if (rmd) {
+    double decay_u = M.syn_decay_u;
+    if (kGen && rmd == 2u && M.syn_uniform) decay_u = exp(-rdelta / M.syn_tau_u);
+    for (uint32_t e = rtid; e < nE_syn; e += kT) {
       if (U.syn_slot[e] == kNoSlot16) continue;
-      double decay;
-      if (md == 1u) decay = M.syn_uniform ? M.syn_decay_u : U.syn_decay[e];
-      else decay = exp(-delta / (M.syn_uniform ? M.syn_tau_u : U.syn_tau[e]));
-      U.gg[e] *= decay;
+      double decay = decay_u;
+      if (!M.syn_uniform) decay = (!kGen || rmd == 1u) ? U.syn_decay()[e] : exp(-rdelta / U.syn_tau()[e]);
+      U.sg[e] *= decay;
     }
   }
   if (tid < kG && md) {
@@ -308,62 +444,96 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
         const unsigned long long pos = atomicAdd(&M.counters[CNT_SPIKES], 1ull);
         if ((int64_t)pos < M.spike_cap) { M.spike_cell[pos] = M.cell_orig[U.cell_base + tid]; M.spike_t[pos] = ts; }
         else atomicOr(&M.counters[CNT_ERROR], 1ull);
-        cs.armed[tid] = 0; cs.dirty[tid] = 1;
+        cs.armed[tid] = 0;
       }
-      if (vd < M.theta && !cs.armed[tid]) { cs.armed[tid] = 1; cs.dirty[tid] = 1; }
+      if (vd < M.theta && !cs.armed[tid]) cs.armed[tid] = 1;
     }
     cs.tcur[tid] = cs.tnext[tid];
   }
-  __syncthreads();
+  TICK(12);
 }
 
 // ------------------------------------------------------------------------------------------
 // The cable step for cell groups.
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kGroupThreads) cable_group_kernel(DevModel M, StepArgs A) {
+__global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kernel(DevModel M, StepArgs A) {
   extern __shared__ __align__(128) uint8_t smem[];
-  __shared__ double rt0[kG];             // time of each cell's next undelivered event
+  __shared__ GroupDesc sD[2];            // this group's and the next group's descriptors
   __shared__ uint32_t flags[2];
   const GroupSmemPlan P = M.gplan;
-  double* Vs = (double*)smem;
+  double* Ss = (double*)smem;            // state record; V first
+  double* Vs = Ss;
+  const double* Fs = (const double*)(smem + P.off_f);
+  const double* Is = (const double*)(smem + P.off_i);
+  const uint8_t* tail = smem + P.off_tail;
+  uint8_t* cls = smem + P.off_class;
   double* buf = (double*)(smem + P.off_buf);
   const CellS cs = carve_cells(smem + P.off_cell, kG);
   uint64_t* mbar = (uint64_t*)(smem + P.off_mbar);
-  const int tid = threadIdx.x, c = tid % kG;
+  const int tid = threadIdx.x;
   double* fgen = M.gscratch + (int64_t)blockIdx.x * M.gscratch_stride;
   double* invdgen = fgen + (size_t)P.slot_cap * kG;
   if (tid == 0) { mbar_init(mbar, 1); fence_mbar_init(); }
+  if (tid < 16 && blockIdx.x < M.n_groups) ((uint32_t*)&sD[0])[tid] = ((const uint32_t*)&M.groups[blockIdx.x])[tid];
   __syncthreads();
   unsigned n_sub = 0, n_del = 0;
   uint32_t it = 0;
+  int64_t cached_class = -1;
+  HHDefer dh;
+  clear(dh);
+  double* dh_gm = nullptr;               // where the carried gate update of the previous group goes
+  uint32_t dh_ss = 0;
+#ifdef ARBB_PROFILE
+  long long prof_buf[16];
+#endif
+  long long* prof = nullptr;
   for (int64_t g = blockIdx.x; g < M.n_groups; g += gridDim.x, ++it) {
-    const GroupDesc D = M.groups[g];
-    GView U;
-    make_gview(U, M, D);
+#ifdef ARBB_PROFILE
+    prof = (blockIdx.x == 7 && tid == 0 && it >= 2 && it < 6 && A.k_first == 150) ? prof_buf : nullptr;
+    if (prof) for (int i = 0; i < 16; ++i) prof[i] = 0;
+#endif
+    TICK(0);
+    const GroupDesc& D = sD[it & 1u];
+    const GConstOff co = gconst_offsets(D.n_cv, D.n_hh_rows, D.n_syn_rows, D.n_cl_rows, M.syn_uniform != 0);
+    const GStateOff so = gstate_offsets(D.n_cv, D.n_hh_rows, D.n_syn_rows);
     const uint32_t vbytes = D.n_cv * kG * 8u;
+    const int64_t gn = g + gridDim.x;
     if (tid == 0) {
+      // state record, f, 1/d and the const tail of the group -> shared memory (one barrier)
+      const uint8_t* cb = M.fast + D.const_off;
+      const uint32_t tbytes = co.total - co.hh_gna;
       fence_proxy_async();
-      mbar_expect_tx(mbar, vbytes);
-      bulk_g2s(Vs, U.gV, vbytes, mbar);
-      const int64_t gn = g + gridDim.x;
-      if (gn < M.n_groups) {             // next group's records -> L2 while this one is integrated
-        const GroupDesc Dn = M.groups[gn];
-        const uint32_t nb = Dn.n_cv * kG * 8u;
-        const GConstOff con = gconst_offsets(Dn.n_cv, Dn.n_hh_rows, Dn.n_syn_rows, Dn.n_cl_rows, M.syn_uniform != 0);
-        bulk_prefetch_l2(M.fast + Dn.const_off, con.hh_gna);
-        bulk_prefetch_l2(M.state + Dn.state_base, nb);
-      }
+      mbar_expect_tx(mbar, 8u * so.total + 2u * vbytes + tbytes);
+      bulk_g2s(Ss, M.state + D.state_base, 8u * so.total, mbar);
+      bulk_g2s((void*)Fs, cb + co.f, vbytes, mbar);
+      bulk_g2s((void*)Is, cb + co.invd, vbytes, mbar);
+      bulk_g2s((void*)tail, cb + co.hh_gna, tbytes, mbar);
+      if (M.l2_prefetch) bulk_prefetch_l2(cb + co.a, co.hh_gna - co.a);     // a, b of this group -> L2
+    } else if (tid >= 32 && tid < 48 && gn < M.n_groups) {
+      ((uint32_t*)&sD[(it + 1) & 1u])[tid - 32] = ((const uint32_t*)&M.groups[gn])[tid - 32];
     }
-    if (tid < kG) {
-      const double* rt = U.grt + kRtDoubles * tid;
-      const unsigned long long pk = (unsigned long long)__double_as_longlong(rt[1]);
-      rt0[tid] = rt[0];
-      cs.evcur[tid] = (uint32_t)pk; cs.evend[tid] = (uint32_t)(pk >> 32);
-      cs.armed[tid] = rt[2] != 0.0 ? 1u : 0u;
-      cs.dirty[tid] = 0;
+    if (D.class_off != cached_class) {   // tree structure differs from the previous group's
+      const ClassRecord* R = (const ClassRecord*)(M.topo + D.class_off);
+      const uint32_t n16 = R->bytes / 16;
+      const uint4* src = (const uint4*)R;
+      for (uint32_t i = tid; i < n16; i += kT) ((uint4*)cls)[i] = src[i];
+      cached_class = D.class_off;
+      __syncthreads();
     }
+    GView U;
+    make_gview(U, M, D, Ss, tail, cls);
+    // the previous group's last gate update: registers -> global m, h, n, while the copies are in flight
+    run_deferred(dh, dh_gm, nullptr, dh_ss);
+    dh_gm = U.gm; dh_ss = U.hh_ss;
+    TICK(1);
     mbar_wait(mbar, it & 1u);
+    if (tid < kG) {
+      const unsigned long long pk = (unsigned long long)__double_as_longlong(U.srt[kRtDoubles * tid + 1]);
+      cs.evcur[tid] = (uint32_t)pk; cs.evend[tid] = (uint32_t)(pk >> 32);
+      cs.armed[tid] = U.srt[kRtDoubles * tid + 2] != 0.0 ? 1u : 0u;
+    }
     __syncthreads();
+    TICK(2);
 
     for (int64_t k = A.k_first; k < A.k_first + A.nk; ++k) {
       const double ta = (k == 0) ? A.t0 : __dadd_rn(A.t0, __dmul_rn((double)k, A.dt));
@@ -378,13 +548,13 @@ __global__ void __launch_bounds__(kGroupThreads) cable_group_kernel(DevModel M, 
             const double t = cs.tcur[tid];
             uint32_t md = 0;
             if (t < tb) {
-              double tn = rt0[tid];
+              double tn = U.srt[kRtDoubles * tid];
               if (tn <= t) {
                 uint32_t cur = cs.evcur[tid];
                 const uint32_t end = cs.evend[tid];
-                while (cur < end && M.ev_t[cur] <= t) { M.state[M.ev_gidx[cur]] += M.ev_w[cur]; ++cur; ++n_del; }
+                while (cur < end && M.ev_t[cur] <= t) { Ss[M.ev_gidx[cur] - (uint32_t)D.state_base] += M.ev_w[cur]; ++cur; ++n_del; }
                 tn = cur < end ? M.ev_t[cur] : CUDART_INF;
-                cs.evcur[tid] = cur; rt0[tid] = tn; cs.dirty[tid] = 1;
+                cs.evcur[tid] = cur; U.srt[kRtDoubles * tid] = tn;
               }
               const double next = tn < tb ? tn : tb;
               const bool fast = nominal && t == ta && next == tb;
@@ -396,35 +566,54 @@ __global__ void __launch_bounds__(kGroupThreads) cable_group_kernel(DevModel M, 
               if ((uint32_t)tid < U.n_cell) ++n_sub;
             }
             cs.mode[tid] = md;
-            gen = md == 2u;
+            gen = md != 1u;
           }
           const unsigned ba = __ballot_sync(kFull, active), bg = __ballot_sync(kFull, gen);
           if (tid == 0) { flags[0] = ba; flags[1] = bg; }
         }
         __syncthreads();                  // also orders the delivered g += w before phase B
         if (!flags[0]) break;
-        const bool any_gen = flags[1] != 0;
-        const uint32_t md = cs.mode[c];
-        const double delta = cs.delta[c];
-        group_substep(M, U, Vs, buf, cs, fgen, invdgen, any_gen, md, delta);
+        // another (sub-)step follows: the gates of the previous one are needed now (working copy and global)
+        run_deferred(dh, U.sm, U.gm, U.hh_ss);
+        if (flags[1]) group_substep<true>(M, U, Vs, Fs, Is, buf, cs, fgen, invdgen, A.dt, dh, prof);
+        else group_substep<false>(M, U, Vs, Fs, Is, buf, cs, fgen, invdgen, A.dt, dh, prof);
+        __syncthreads();
       }
       __syncthreads();                    // flags are rewritten by the next grid step
     }
 
-    // ---- V' -> HBM (one bulk store), per-cell runtime
+    // ---- V', g, per-cell runtime -> HBM (one bulk store); the gates follow from registers
+    TICK(13);
+    if (tid < kG) {
+      const unsigned long long pk = ((unsigned long long)cs.evend[tid] << 32) | cs.evcur[tid];
+      U.srt[kRtDoubles * tid + 1] = __longlong_as_double((long long)pk);
+      U.srt[kRtDoubles * tid + 2] = cs.armed[tid] ? 1.0 : 0.0;
+    }
     fence_proxy_async();
     __syncthreads();
-    if (tid == 0) { bulk_s2g(U.gV, Vs, vbytes); bulk_commit(); }
-    if (tid < kG && cs.dirty[tid]) {
-      double* rt = U.grt + kRtDoubles * tid;
-      const unsigned long long pk = ((unsigned long long)cs.evend[tid] << 32) | cs.evcur[tid];
-      rt[0] = rt0[tid];
-      rt[1] = __longlong_as_double((long long)pk);
-      rt[2] = cs.armed[tid] ? 1.0 : 0.0;
+    if (tid == 0) {
+      bulk_s2g(M.state + D.state_base, Ss, 8u * so.m);
+      bulk_commit();
+      if (M.l2_prefetch && gn < M.n_groups) {   // next group's records -> L2
+        const GroupDesc& Dn = sD[(it + 1) & 1u];
+        const GConstOff con = gconst_offsets(Dn.n_cv, Dn.n_hh_rows, Dn.n_syn_rows, Dn.n_cl_rows, M.syn_uniform != 0);
+        bulk_prefetch_l2(M.fast + Dn.const_off, con.a);
+        bulk_prefetch_l2(M.fast + Dn.const_off + con.hh_gna, con.total - con.hh_gna);
+        bulk_prefetch_l2(M.state + Dn.state_base, 8u * gstate_offsets(Dn.n_cv, Dn.n_hh_rows, Dn.n_syn_rows).total);
+      }
+      bulk_wait_read0();
     }
-    if (tid == 0) bulk_wait_read0();
-    __syncthreads();                      // Vs may be overwritten by the next group's copy
+    __syncthreads();                      // shared memory may be overwritten by the next group's copies
+    TICK(14);
+#ifdef ARBB_PROFILE
+    if (prof) {
+      printf("grp %lld:", (long long)g);
+      for (int i = 1; i < 15; ++i) printf(" %d:%lld", i, prof[i] ? prof[i] - prof[0] : -1ll);
+      printf("\n");
+    }
+#endif
   }
+  run_deferred(dh, dh_gm, nullptr, dh_ss);
   if (tid < 32) {
     for (int o = 16; o; o >>= 1) { n_sub += __shfl_xor_sync(kFull, n_sub, o); n_del += __shfl_xor_sync(kFull, n_del, o); }
     if (tid == 0) {
@@ -442,11 +631,13 @@ __global__ void __launch_bounds__(kGroupThreads) group_factor_kernel(DevModel M,
   extern __shared__ __align__(128) uint8_t smem[];
   double* dcon = (double*)smem;
   const GroupDesc D = M.groups[blockIdx.x];
+  const GConstOff co = gconst_offsets(D.n_cv, D.n_hh_rows, D.n_syn_rows, D.n_cl_rows, M.syn_uniform != 0);
+  uint8_t* cb = M.fast + D.const_off;
   GView U;
-  make_gview(U, M, D);
+  make_gview(U, M, D, M.state + D.state_base, cb + co.hh_gna, M.topo + D.class_off);
   const int tid = threadIdx.x, c = tid % kG, h = tid / kG;
-  double* f = const_cast<double*>(U.f);
-  double* invd = const_cast<double*>(U.invd);
+  double* f = (double*)(cb + co.f);
+  double* invd = (double*)(cb + co.invd);
   for (uint32_t st = 0; st < U.n_stage; ++st) {
     const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
     for (uint32_t q = beg; q < end; ++q) {
@@ -455,40 +646,49 @@ __global__ void __launch_bounds__(kGroupThreads) group_factor_kernel(DevModel M,
     }
     __syncthreads();
   }
-  double* a = const_cast<double*>(U.a);
-  double* b = const_cast<double*>(U.b);
+  double* a = (double*)(cb + co.a);
+  double* b = (double*)(cb + co.b);
+  const double *C = U.C(), *G = U.G(), *bg = U.bg();
   for (uint32_t e = tid; e < U.n_cv * kG; e += kT) {
-    a[e] = U.C[e] / dt - U.G[e];
-    b[e] = U.bg[e];
+    a[e] = C[e] / dt - G[e];
+    b[e] = bg[e];
   }
   if (!M.syn_uniform) {
-    double* decay = const_cast<double*>(U.syn_decay);
-    for (uint32_t e = tid; e < U.n_syn * kG; e += kT) decay[e] = exp(-dt / U.syn_tau[e]);
+    double* decay = (double*)(cb + co.syn_decay);
+    const double* tau = U.syn_tau();
+    for (uint32_t e = tid; e < U.n_syn * kG; e += kT) decay[e] = exp(-dt / tau[e]);
   }
 }
 
 // R4: gates start at their steady state for the initial voltage.
 __global__ void __launch_bounds__(kGroupThreads) group_init_kernel(DevModel M) {
   const GroupDesc D = M.groups[blockIdx.x];
+  const GConstOff co = gconst_offsets(D.n_cv, D.n_hh_rows, D.n_syn_rows, D.n_cl_rows, M.syn_uniform != 0);
+  double* st = M.state + D.state_base;
   GView U;
-  make_gview(U, M, D);
+  make_gview(U, M, D, st, M.fast + D.const_off + co.hh_gna, M.topo + D.class_off);
   const int c = threadIdx.x % kG;
   for (uint32_t e = threadIdx.x; e < U.n_hh * kG; e += kT) {
     const uint32_t slot = U.hh_slot[e];
     if (slot == kNoSlot16) continue;
-    const Rates r = hh_rates(U.gV[slot * kG + c]);
+    const Rates r = hh_rates(st[slot * kG + c]);
     U.gm[e] = r.am / (r.am + r.bm);
-    U.gh[e] = r.ah / (r.ah + r.bh);
-    U.gn[e] = r.an / (r.an + r.bn);
+    U.gm[e + U.hh_ss] = r.ah / (r.ah + r.bh);
+    U.gm[e + 2 * U.hh_ss] = r.an / (r.an + r.bn);
   }
 }
 
 }  // namespace
 
+// Resident CTAs of the group kernel per SM for `smem_bytes` of dynamic shared memory (asks the
+// runtime; also opts the kernel into that much shared memory).  0: does not fit / no device.
 int group_ctas_per_sm(uint32_t smem_bytes) {
-  const int by_smem = (int)((228u * 1024u) / (smem_bytes + 1024u + 64u));
-  const int by_threads = 2048 / kGroupThreads;
-  return by_smem < 1 ? 0 : (by_smem < by_threads ? by_smem : by_threads);
+  if (smem_bytes + 1024u > 227u * 1024u) return 0;
+  if (cudaFuncSetAttribute(cable_group_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes) != cudaSuccess) return 0;
+  cudaFuncSetAttribute(cable_group_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  int n = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, cable_group_kernel, kGroupThreads, smem_bytes) != cudaSuccess) return 0;
+  return n;
 }
 
 cudaError_t launch_group_factor(const DevModel& M, double dt, uint32_t seg_cap, cudaStream_t s) {
@@ -505,13 +705,7 @@ cudaError_t launch_group_init(const DevModel& M, cudaStream_t s) {
 
 cudaError_t launch_group_cable(const DevModel& M, const StepArgs& A, int grid, cudaStream_t s, int* launches) {
   if (M.n_groups == 0) return cudaSuccess;
-  const int smem = (int)M.gplan.bytes;
-  static int configured = -1;
-  if (smem > 48 * 1024 && configured < smem) {
-    cudaError_t e = cudaFuncSetAttribute(cable_group_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    configured = smem;
-  }
+  const int smem = (int)M.gplan.bytes;          // group_ctas_per_sm() has opted the kernel in
   cable_group_kernel<<<(unsigned)grid, kGroupThreads, smem, s>>>(M, A);
   if (launches) ++*launches;
   return cudaGetLastError();

@@ -33,15 +33,19 @@
 namespace arbb {
 
 #ifndef ARBB_G
-#define ARBB_G 8
+#define ARBB_G 4
 #endif
 #ifndef ARBB_GROUP_WARPS
 #define ARBB_GROUP_WARPS 4
+#endif
+#ifndef ARBB_GROUP_MIN_CTAS
+#define ARBB_GROUP_MIN_CTAS 4
 #endif
 constexpr int kG = ARBB_G;                    // cells per group = lanes per lane group (8, 16 or 32)
 constexpr int kLaneGroups = 32 / kG;          // lane groups per warp
 constexpr int kGroupWarps = ARBB_GROUP_WARPS; // warps per CTA of the group kernel
 constexpr int kGroupThreads = kGroupWarps * 32;
+constexpr int kGroupMinCtas = ARBB_GROUP_MIN_CTAS;      // resident CTAs per SM the kernel is compiled for
 constexpr int kGroupSlots = kGroupWarps * kLaneGroups;   // chunks a stage can run concurrently
 constexpr uint16_t kNoSlot16 = 0xFFFFu;
 constexpr uint32_t kGroupMaxCv = 65000;       // slots are stored as uint16
@@ -61,7 +65,9 @@ struct ClassRecord {     // header of a class record; arrays follow at the byte 
   uint32_t off_sched;    // uint16[n_stage * kGroupSlots + 1]: begin of each (stage, slot) range in order[]
   uint32_t off_child;    // uint16[n_child]: child segments
   uint32_t bytes;
-  uint32_t pad[7];
+  uint32_t n_block;      // stages [0, n_block) use lane groups of several warps (block barriers between
+                         // them); stages [n_block, n_stage) only use the lane groups of warp 0
+  uint32_t pad[6];
 };
 static_assert(sizeof(ClassRecord) == 64, "ClassRecord must be 64 bytes");
 
@@ -95,14 +101,15 @@ ARBB_HD GConstOff gconst_offsets(uint32_t n_cv, uint32_t n_hh, uint32_t n_syn, u
   return o;
 }
 
-// Double offsets inside a group's state record (every section 16-double aligned).
-struct GStateOff { uint32_t v, m, h, n, g, rt, total; };
+// Double offsets inside a group's state record (every section 16-double aligned).  V | g | rt are
+// what a launch writes back with one bulk store; the gates m | h | n are written by their own threads.
+struct GStateOff { uint32_t v, g, rt, m, h, n, total; };
 ARBB_HD GStateOff gstate_offsets(uint32_t n_cv, uint32_t n_hh, uint32_t n_syn) {
   GStateOff o;
   uint32_t p = 0;
   auto sec = [&](uint32_t n) { uint32_t at = p; p = align_up(p + n, 16); return at; };
-  o.v = sec(kG * n_cv); o.m = sec(kG * n_hh); o.h = sec(kG * n_hh); o.n = sec(kG * n_hh);
-  o.g = sec(kG * n_syn); o.rt = sec(kRtDoubles * kG);
+  o.v = sec(kG * n_cv); o.g = sec(kG * n_syn); o.rt = sec(kRtDoubles * kG);
+  o.m = sec(kG * n_hh); o.h = sec(kG * n_hh); o.n = sec(kG * n_hh);
   o.total = p;
   return o;
 }
@@ -117,16 +124,23 @@ ARBB_HD GGenOff ggen_offsets(uint32_t n_cv, uint32_t n_syn) {
   return o;
 }
 
-// Shared memory of one CTA of the group kernel: V of the group | buf (xI, then contrib) | cells.
-// slot_cap = largest n_cv of any group, buf_rows = largest max(n_seg, n_hh + n_syn + n_cl rows).
-struct GroupSmemPlan { uint32_t slot_cap, buf_rows, off_buf, off_cell, off_mbar, bytes; };
-ARBB_HD GroupSmemPlan group_smem_plan(uint32_t slot_cap, uint32_t buf_rows) {
+// Shared memory of one CTA of the group kernel:
+//   state record (V | g | rt | m | h | n) | f | 1/d | tail of the const record (hh conductances ...
+//   det_slot) | class record | buf (xI, then contrib) | per-cell scratch | mbarrier
+// Caps are maxima over all groups / classes of the model.
+struct GroupCaps { uint32_t slot_cap, state_bytes, tail_bytes, class_bytes, buf_rows; };
+struct GroupSmemPlan { uint32_t slot_cap, off_f, off_i, off_tail, off_class, off_buf, off_cell, off_mbar, bytes; };
+ARBB_HD GroupSmemPlan group_smem_plan(const GroupCaps& c) {
   GroupSmemPlan P;
-  P.slot_cap = slot_cap; P.buf_rows = buf_rows;
-  uint32_t p = align_up(8 * kG * slot_cap, 128);
-  P.off_buf = p;  p = align_up(p + 8 * kG * buf_rows, 128);
-  P.off_cell = p; p = align_up(p + kCellScratchBytes * kG, 128);
-  P.off_mbar = p; p += 16;
+  P.slot_cap = c.slot_cap;
+  uint32_t p = align_up(c.state_bytes, 128);
+  P.off_f = p;     p = align_up(p + 8 * kG * c.slot_cap, 128);
+  P.off_i = p;     p = align_up(p + 8 * kG * c.slot_cap, 128);
+  P.off_tail = p;  p = align_up(p + c.tail_bytes, 128);
+  P.off_class = p; p = align_up(p + c.class_bytes, 128);
+  P.off_buf = p;   p = align_up(p + 8 * kG * c.buf_rows, 128);
+  P.off_cell = p;  p = align_up(p + kCellScratchBytes * kG, 128);
+  P.off_mbar = p;  p += 16;
   P.bytes = align_up(p, 128);
   return P;
 }

@@ -63,6 +63,7 @@ struct DevModel {
   double* gscratch;           // group kernel: per CTA fgen | invdgen (event-split sub-steps only)
   int64_t gscratch_stride;
   GroupSmemPlan gplan;
+  int l2_prefetch;            // group kernel: TMA-prefetch the next group's records into L2
 };
 
 struct StepArgs {

@@ -543,6 +543,13 @@ void build_class(const int32_t* par, uint32_t n, ClassInfo& K) {
   R.off_sched = sec(((uint32_t)stages.size() * kGroupSlots + 1) * 2);
   R.off_child = sec(n_child * 2);
   R.bytes = align_up(p, 128);
+  R.n_block = (uint32_t)stages.size();
+  while (R.n_block > 0) {
+    bool narrow = true;
+    for (uint32_t h = kLaneGroups; h < (uint32_t)kGroupSlots; ++h) narrow = narrow && stages[R.n_block - 1][h].empty();
+    if (!narrow) break;
+    --R.n_block;
+  }
   K.record.assign(R.bytes, 0);
   std::memcpy(K.record.data(), &R, sizeof R);
   SegRec* sr = (SegRec*)(K.record.data() + R.off_segs);
@@ -730,6 +737,7 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
       H.topo_bytes += (int64_t)K.record.size();
       H.n_classes++;
       H.g_seg_cap = std::max(H.g_seg_cap, K.n_seg);
+      H.gcaps.class_bytes = std::max(H.gcaps.class_bytes, (uint32_t)K.record.size());
     }
   H.gdescs.resize(H.n_groups);
   for (int64_t g = 0; g < H.n_groups; ++g) {
@@ -739,13 +747,17 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     D.n_cv = K.n_cv; D.n_cell = G.n_cell; D.n_hh_rows = G.n_hh_rows; D.n_syn_rows = G.n_syn_rows; D.n_cl_rows = G.n_cl_rows; D.n_seg = K.n_seg;
     D.class_off = K.topo_off;
     D.cell_base = G.cell_begin;
-    D.const_off = H.fast_bytes;   H.fast_bytes += gconst_offsets(K.n_cv, G.n_hh_rows, G.n_syn_rows, G.n_cl_rows, H.syn_uniform).total;
-    D.state_base = H.state_doubles; H.state_doubles += gstate_offsets(K.n_cv, G.n_hh_rows, G.n_syn_rows).total;
+    const GConstOff co = gconst_offsets(K.n_cv, G.n_hh_rows, G.n_syn_rows, G.n_cl_rows, H.syn_uniform);
+    const GStateOff so = gstate_offsets(K.n_cv, G.n_hh_rows, G.n_syn_rows);
+    D.const_off = H.fast_bytes;   H.fast_bytes += co.total;
+    D.state_base = H.state_doubles; H.state_doubles += so.total;
+    H.gcaps.state_bytes = std::max(H.gcaps.state_bytes, 8 * so.total);
+    H.gcaps.tail_bytes = std::max(H.gcaps.tail_bytes, co.total - co.hh_gna);
     D.gen_base = H.gen_doubles;   H.gen_doubles += ggen_offsets(K.n_cv, G.n_syn_rows).total;
     G.hh_base = H.n_hh;
     for (uint32_t lc = 0; lc < G.n_cell; ++lc) H.n_hh += cell_hh[group_cells[G.cell_begin + lc]];
-    H.g_slot_cap = std::max(H.g_slot_cap, K.n_cv);
-    H.g_buf_rows = std::max(H.g_buf_rows, std::max(K.n_seg, G.n_hh_rows + G.n_syn_rows + G.n_cl_rows));
+    H.gcaps.slot_cap = std::max(H.gcaps.slot_cap, K.n_cv);
+    H.gcaps.buf_rows = std::max(H.gcaps.buf_rows, std::max(K.n_seg, G.n_hh_rows + G.n_syn_rows + G.n_cl_rows));
   }
   // placement; tree structures are deduplicated by content
   std::unordered_map<uint64_t, std::vector<int64_t>> seen;   // hash -> units that own a stored record

@@ -46,7 +46,8 @@ struct HostModel {
   double ena = 0, ek = 0, el = 0, threshold = 0;
   // cell groups: cells [0, n_group_cells) of the internal order
   int64_t n_groups = 0, n_group_cells = 0, n_classes = 0;
-  uint32_t g_slot_cap = 0, g_buf_rows = 0, g_seg_cap = 0;
+  GroupCaps gcaps = {0, 0, 0, 0, 0};
+  uint32_t g_seg_cap = 0;
   std::vector<GroupDesc> gdescs;
   std::vector<UnitCounts> units;
   std::vector<uint32_t> cell_order;     // internal -> caller's cell id
