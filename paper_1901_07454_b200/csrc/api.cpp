@@ -50,7 +50,7 @@ Caps capacities(const HostModel& H) {
 }
 
 // group kernel: per resident CTA fgen | invdgen for event-split sub-steps
-int64_t gscratch_stride(const HostModel& H) { return 2 * (int64_t)H.gcaps.slot_cap * kG; }
+int64_t gscratch_stride(const HostModel& H) { return 2 * (int64_t)gcv_elems(H.gcaps.slot_cap); }
 int64_t gscratch_ctas(const HostModel& H) { return std::min<int64_t>(H.n_groups, kMaxGroupCtas); }
 
 int64_t warp_scratch_stride(const HostModel& H) { return 2 * (int64_t)H.slot_cap + align_up(H.lane_cap, 2); }

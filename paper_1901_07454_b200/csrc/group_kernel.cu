@@ -32,8 +32,15 @@ namespace arbb {
 
 namespace {
 
+#ifndef ARBB_SUBSTEP_INLINE
+#define ARBB_SUBSTEP_INLINE __forceinline__
+#endif
+#ifndef ARBB_CVREGS
+#define ARBB_CVREGS 8
+#endif
 constexpr int kT = kGroupThreads;
 constexpr int kRows = 4;                  // rows of a segment a lane group loads ahead of the recurrence
+constexpr int kCvRegs = ARBB_CVREGS;               // rhs coefficient pairs (a, b) a thread keeps in flight in phase C
 
 // -DARBB_PROFILE: one CTA prints clock64() at the phase boundaries of a few group-steps (development aid)
 #ifdef ARBB_PROFILE
@@ -118,7 +125,7 @@ __device__ __forceinline__ SegRec load_seg(const SegRec* p) {
 __device__ __forceinline__ void eliminate_seg(const GView& U, const SegRec& sg, uint32_t seg_idx, int c, double delta,
                                               double* fout, double* invdout, double* dcon) {
   const double *C = U.C(), *S = U.S(), *sig = U.sig();
-  uint32_t s = (sg.slot0 + sg.len - 1) * kG + c;
+  uint32_t lin = (sg.slot0 + sg.len - 1) * kG + c, s = gswz(lin);
   double d = C[s] / delta + S[s];
   for (uint32_t j = 0; j < sg.ccnt; ++j) d -= dcon[(uint32_t)U.child[sg.cbeg + j] * kG + c];
   double fk = 0.0, sk = 0.0;
@@ -129,7 +136,7 @@ __device__ __forceinline__ void eliminate_seg(const GView& U, const SegRec& sg, 
     fout[s] = fk;
     invdout[s] = invd;
     if (k > 0) {
-      s -= kG;
+      lin -= kG; s = gswz(lin);
       d = fma(fk, sk, C[s] / delta + S[s]);          // d_p -= f*u with u = -sigma
     }
   }
@@ -149,46 +156,64 @@ __device__ __forceinline__ void backward_seg(const GView& U, const SegRec& sg, u
   double fp = 0.0, rp = 0.0;
   int left = sg.len;
   bool first = true;
-  while (left > 0) {
+  while (left >= kRows) {                 // whole blocks: no predication
     double fr[kRows], ir[kRows], vr[kRows];
+    uint32_t p[kRows];
 #pragma unroll
-    for (int j = 0; j < kRows; ++j)
-      if (j < left) { fr[j] = F[s - j * kG]; ir[j] = I[s - j * kG]; vr[j] = Vs[s - j * kG]; }
+    for (int j = 0; j < kRows; ++j) { p[j] = gswz(s - j * kG); fr[j] = F[p[j]]; ir[j] = I[p[j]]; vr[j] = Vs[p[j]]; }
     if (first) {
+#pragma unroll 1
       for (uint32_t j = 0; j < sg.ccnt; ++j) vr[0] -= con[(uint32_t)U.child[sg.cbeg + j] * kG + c];
       first = false;
     }
 #pragma unroll
-    for (int j = 0; j < kRows; ++j)
-      if (j < left) {
-        const double r = fma(-fp, rp, vr[j]);
-        Vs[s - j * kG] = r * ir[j];
-        fp = fr[j]; rp = r;
-      }
+    for (int j = 0; j < kRows; ++j) {
+      const double r = fma(-fp, rp, vr[j]);
+      Vs[p[j]] = r * ir[j];
+      fp = fr[j]; rp = r;
+    }
     s -= kRows * kG;
     left -= kRows;
+  }
+#pragma unroll 1
+  for (; left > 0; --left, s -= kG) {
+    const uint32_t p = gswz(s);
+    double v = Vs[p];
+    if (first) {
+#pragma unroll 1
+      for (uint32_t j = 0; j < sg.ccnt; ++j) v -= con[(uint32_t)U.child[sg.cbeg + j] * kG + c];
+      first = false;
+    }
+    const double r = fma(-fp, rp, v);
+    Vs[p] = r * I[p];
+    fp = F[p]; rp = r;
   }
   con[seg_idx * kG + c] = fp * rp;
 }
 
 // Forward (root -> leaves) substitution of one segment: V'_k = rhs_k/d_k - f_k V'_{k-1}; V <- V'.
 __device__ __forceinline__ void forward_seg(const SegRec& sg, int c, const double* __restrict__ F, double* Vs) {
-  double vp = sg.pslot != kNoSlot ? Vs[sg.pslot * kG + c] : 0.0;
+  double vp = sg.pslot != kNoSlot ? Vs[gpos(sg.pslot, c)] : 0.0;
   uint32_t s = sg.slot0 * kG + c;
   int left = sg.len;
-  while (left > 0) {
+  while (left >= kRows) {
     double fr[kRows], vr[kRows];
+    uint32_t p[kRows];
 #pragma unroll
-    for (int j = 0; j < kRows; ++j)
-      if (j < left) { fr[j] = F[s + j * kG]; vr[j] = Vs[s + j * kG]; }
+    for (int j = 0; j < kRows; ++j) { p[j] = gswz(s + j * kG); fr[j] = F[p[j]]; vr[j] = Vs[p[j]]; }
 #pragma unroll
-    for (int j = 0; j < kRows; ++j)
-      if (j < left) {
-        vp = fma(-fr[j], vp, vr[j]);
-        Vs[s + j * kG] = vp;
-      }
+    for (int j = 0; j < kRows; ++j) {
+      vp = fma(-fr[j], vp, vr[j]);
+      Vs[p[j]] = vp;
+    }
     s += kRows * kG;
     left -= kRows;
+  }
+#pragma unroll 1
+  for (; left > 0; --left, s += kG) {
+    const uint32_t p = gswz(s);
+    vp = fma(-F[p], vp, Vs[p]);
+    Vs[p] = vp;
   }
 }
 
@@ -252,7 +277,8 @@ __device__ __forceinline__ void clear(HHDefer& d) {
   for (int i = 0; i < kHHDefer; ++i) d.e[i] = kNoSlot;
 }
 
-__device__ __forceinline__ void hh_gates(double v, double delta, double& m, double& h, double& n) {
+// not inlined: the exp / expm1 / divide chains are ~1,000 instructions and there are several call sites
+__device__ __noinline__ void hh_gates(double v, double delta, double& m, double& h, double& n) {
   const Rates r = hh_rates(v);
   double inf = r.am / (r.am + r.bm);
   m = inf + (m - inf) * exp(-delta * (r.am + r.bm));
@@ -283,12 +309,12 @@ __device__ __forceinline__ void run_deferred(HHDefer& dh, double* dst0, double* 
 // serial parts (phase A, the narrow stages).  The HH gate updates come back deferred in `dh`.
 // ------------------------------------------------------------------------------------------
 template <bool kGen>
-__device__ __forceinline__ void group_substep(const DevModel& M, const GView& U, double* Vs, const double* Fs, const double* Is,
+__device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView& U, double* Vs, const double* Fs, const double* Is,
                                               double* buf, const CellS& cs, double* fgen, double* invdgen, double dt, HHDefer& dh,
                                               long long* prof) {
   const int tid = threadIdx.x, c = tid % kG, h = tid / kG;
   const int rtid = kT - 1 - tid, rc = rtid % kG;      // reversed dealing of instances; cell of those
-  const uint32_t nE_cv = U.n_cv * kG, nE_hh = U.n_hh * kG, nE_syn = U.n_syn * kG, nE_cl = U.n_cl * kG;
+  const uint32_t nE_cv = gcv_elems(U.n_cv), nE_hh = U.n_hh * kG, nE_syn = U.n_syn * kG, nE_cl = U.n_cl * kG;
   const uint32_t md = kGen ? cs.mode[c] : 1u, rmd = kGen ? cs.mode[rc] : 1u;
   const double delta = kGen ? cs.delta[c] : dt, rdelta = kGen ? cs.delta[rc] : dt;
 
@@ -308,19 +334,21 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
   // ---- B: currents of HH, synapses and clamps from V(t); the passive current is
   // folded into a, b.  Items of one cell on one CV form a run; its first item sums it in index order.
   double* xI = buf;
+#pragma unroll 1
   for (uint32_t e = rtid; e < nE_hh; e += kT) {
     const uint32_t slot = U.hh_slot[e];
     if (slot == kNoSlot16 || !rmd) continue;
-    const double v = Vs[slot * kG + rc];
+    const double v = Vs[gpos(slot, rc)];
     const double m = U.sm[e], hh = U.sm[e + U.hh_ss], n = U.sm[e + 2 * U.hh_ss];
     xI[e] = U.hh_gna[e] * m * m * m * hh * (v - M.ena) + U.hh_gna[e + U.hh_cs] * n * n * n * n * (v - M.ek) +
             U.hh_gna[e + 2 * U.hh_cs] * (v - M.el);
   }
+#pragma unroll 1
   for (uint32_t e = rtid; e < nE_syn; e += kT) {
     const uint32_t slot = U.syn_slot[e];
     if (slot == kNoSlot16 || !rmd) continue;
     if (e >= (uint32_t)kG && U.syn_slot[e - kG] == slot) continue;
-    const double v = Vs[slot * kG + rc];
+    const double v = Vs[gpos(slot, rc)];
     double I = 0.0;
     uint32_t j = e;
     do {
@@ -350,38 +378,48 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
   __syncthreads();
   TICK(4);
 
-  // ---- C: rhs_i = (C_i/delta - G_i) V_i + G_i e_i - I_i, in place of V
-  if (md == 1u) {
-    for (uint32_t e = tid; e < nE_cv; e += 8 * kT) {
-      double ar[8], br[8];
+  // ---- C: rhs_i = (C_i/delta - G_i) V_i + G_i e_i - I_i, in place of V; positions, not
+  // (slot, cell) pairs: every per-CV array of the group uses the same positions
+  if (!kGen) {
+    double ar[kCvRegs], br[kCvRegs];      // one round trip to L2 for the whole group when it fits
 #pragma unroll
-      for (int j = 0; j < 8; ++j)
-        if (e + j * kT < nE_cv) { ar[j] = U.a[e + j * kT]; br[j] = U.b[e + j * kT]; }
-#pragma unroll
-      for (int j = 0; j < 8; ++j)
-        if (e + j * kT < nE_cv) Vs[e + j * kT] = fma(ar[j], Vs[e + j * kT], br[j]);
+    for (int j = 0; j < kCvRegs; ++j) {
+      const uint32_t p = tid + j * kT;
+      if (p < nE_cv) { ar[j] = U.a[p]; br[j] = U.b[p]; }
     }
-  } else if (kGen && md == 2u) {
+#pragma unroll
+    for (int j = 0; j < kCvRegs; ++j) {
+      const uint32_t p = tid + j * kT;
+      if (p < nE_cv) Vs[p] = fma(ar[j], Vs[p], br[j]);
+    }
+    for (uint32_t p = tid + kCvRegs * kT; p < nE_cv; p += kT) Vs[p] = fma(U.a[p], Vs[p], U.b[p]);
+  } else {
     const double *C = U.C(), *G = U.G(), *bg = U.bg();
-    for (uint32_t e = tid; e < nE_cv; e += kT) Vs[e] = fma(C[e] / delta - G[e], Vs[e], bg[e]);
+    for (uint32_t p = tid; p < nE_cv; p += kT) {
+      const uint32_t cell = gswz(p) % kG, m = cs.mode[cell];
+      if (m == 1u) Vs[p] = fma(U.a[p], Vs[p], U.b[p]);
+      else if (m == 2u) Vs[p] = fma(C[p] / cs.delta[cell] - G[p], Vs[p], bg[p]);
+    }
   }
   TICK(5);
   __syncthreads();
   TICK(6);
   if (nE_hh) {
-    for (uint32_t e = rtid; e < nE_hh; e += kT) {
+  #pragma unroll 1
+  for (uint32_t e = rtid; e < nE_hh; e += kT) {
       const uint32_t slot = U.hh_slot[e];
       if (slot == kNoSlot16 || !rmd) continue;
-      Vs[slot * kG + rc] -= xI[e];
+      Vs[gpos(slot, rc)] -= xI[e];
     }
     __syncthreads();
   }
   if (nE_syn) {
-    for (uint32_t e = rtid; e < nE_syn; e += kT) {
+  #pragma unroll 1
+  for (uint32_t e = rtid; e < nE_syn; e += kT) {
       const uint32_t slot = U.syn_slot[e];
       if (slot == kNoSlot16 || !rmd) continue;
       if (e >= (uint32_t)kG && U.syn_slot[e - kG] == slot) continue;
-      Vs[slot * kG + rc] -= xI[nE_hh + e];
+      Vs[gpos(slot, rc)] -= xI[nE_hh + e];
     }
     __syncthreads();
   }
@@ -391,7 +429,7 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
       const uint32_t slot = cl_slot[e];
       if (slot == kNoSlot16 || !rmd) continue;
       if (e >= (uint32_t)kG && cl_slot[e - kG] == slot) continue;
-      Vs[slot * kG + rc] -= xI[nE_hh + nE_syn + e];
+      Vs[gpos(slot, rc)] -= xI[nE_hh + nE_syn + e];
     }
     __syncthreads();
   }
@@ -412,7 +450,7 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
       if (e < nE_hh) {
         const uint32_t slot = U.hh_slot[e];
         if (slot != kNoSlot16 && rmd) {
-          dh.v[i] = Vs[slot * kG + rc]; dh.delta[i] = rdelta; dh.e[i] = e;
+          dh.v[i] = Vs[gpos(slot, rc)]; dh.delta[i] = rdelta; dh.e[i] = e;
           dh.m[i] = U.sm[e]; dh.h[i] = U.sm[e + U.hh_ss]; dh.n[i] = U.sm[e + 2 * U.hh_ss];
         }
       }
@@ -421,7 +459,7 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
       const uint32_t slot = U.hh_slot[e];
       if (slot == kNoSlot16 || !rmd) continue;
       double m = U.sm[e], hh = U.sm[e + U.hh_ss], n = U.sm[e + 2 * U.hh_ss];
-      hh_gates(Vs[slot * kG + rc], rdelta, m, hh, n);
+      hh_gates(Vs[gpos(slot, rc)], rdelta, m, hh, n);
       U.sm[e] = m; U.sm[e + U.hh_ss] = hh; U.sm[e + 2 * U.hh_ss] = n;
       U.gm[e] = m; U.gm[e + U.hh_ss] = hh; U.gm[e + 2 * U.hh_ss] = n;
     }
@@ -429,7 +467,8 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
   if (rmd) {
     double decay_u = M.syn_decay_u;
     if (kGen && rmd == 2u && M.syn_uniform) decay_u = exp(-rdelta / M.syn_tau_u);
-    for (uint32_t e = rtid; e < nE_syn; e += kT) {
+  #pragma unroll 1
+  for (uint32_t e = rtid; e < nE_syn; e += kT) {
       if (U.syn_slot[e] == kNoSlot16) continue;
       double decay = decay_u;
       if (!M.syn_uniform) decay = (!kGen || rmd == 1u) ? U.syn_decay()[e] : exp(-rdelta / U.syn_tau()[e]);
@@ -437,7 +476,7 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
     }
   }
   if (tid < kG && md) {
-    const double vd = Vs[(uint32_t)U.det_slot[tid] * kG + tid], vp = cs.vprev[tid];
+    const double vd = Vs[gpos(U.det_slot[tid], tid)], vp = cs.vprev[tid];
     if ((uint32_t)tid < U.n_cell) {
       if (cs.armed[tid] && vp < M.theta && M.theta <= vd) {
         const double ts = cs.tcur[tid] + cs.delta[tid] * (M.theta - vp) / (vd - vp);
@@ -472,7 +511,7 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
   uint64_t* mbar = (uint64_t*)(smem + P.off_mbar);
   const int tid = threadIdx.x;
   double* fgen = M.gscratch + (int64_t)blockIdx.x * M.gscratch_stride;
-  double* invdgen = fgen + (size_t)P.slot_cap * kG;
+  double* invdgen = fgen + (size_t)gcv_elems(P.slot_cap);
   if (tid == 0) { mbar_init(mbar, 1); fence_mbar_init(); }
   if (tid < 16 && blockIdx.x < M.n_groups) ((uint32_t*)&sD[0])[tid] = ((const uint32_t*)&M.groups[blockIdx.x])[tid];
   __syncthreads();
@@ -496,7 +535,7 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
     const GroupDesc& D = sD[it & 1u];
     const GConstOff co = gconst_offsets(D.n_cv, D.n_hh_rows, D.n_syn_rows, D.n_cl_rows, M.syn_uniform != 0);
     const GStateOff so = gstate_offsets(D.n_cv, D.n_hh_rows, D.n_syn_rows);
-    const uint32_t vbytes = D.n_cv * kG * 8u;
+    const uint32_t vbytes = 8u * gcv_elems(D.n_cv);
     const int64_t gn = g + gridDim.x;
     if (tid == 0) {
       // state record, f, 1/d and the const tail of the group -> shared memory (one barrier)
@@ -561,7 +600,7 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
               cs.delta[tid] = fast ? A.dt : next - t;
               md = fast ? 1u : 2u;
               cs.tnext[tid] = next;
-              cs.vprev[tid] = Vs[(uint32_t)U.det_slot[tid] * kG + tid];
+              cs.vprev[tid] = Vs[gpos(U.det_slot[tid], tid)];
               active = true;
               if ((uint32_t)tid < U.n_cell) ++n_sub;
             }
@@ -649,7 +688,7 @@ __global__ void __launch_bounds__(kGroupThreads) group_factor_kernel(DevModel M,
   double* a = (double*)(cb + co.a);
   double* b = (double*)(cb + co.b);
   const double *C = U.C(), *G = U.G(), *bg = U.bg();
-  for (uint32_t e = tid; e < U.n_cv * kG; e += kT) {
+  for (uint32_t e = tid; e < gcv_elems(U.n_cv); e += kT) {
     a[e] = C[e] / dt - G[e];
     b[e] = bg[e];
   }
@@ -671,7 +710,7 @@ __global__ void __launch_bounds__(kGroupThreads) group_init_kernel(DevModel M) {
   for (uint32_t e = threadIdx.x; e < U.n_hh * kG; e += kT) {
     const uint32_t slot = U.hh_slot[e];
     if (slot == kNoSlot16) continue;
-    const Rates r = hh_rates(st[slot * kG + c]);
+    const Rates r = hh_rates(st[gpos(slot, c)]);
     U.gm[e] = r.am / (r.am + r.bm);
     U.gm[e + U.hh_ss] = r.ah / (r.ah + r.bh);
     U.gm[e + 2 * U.hh_ss] = r.an / (r.an + r.bn);

@@ -50,6 +50,17 @@ constexpr int kGroupSlots = kGroupWarps * kLaneGroups;   // chunks a stage can r
 constexpr uint16_t kNoSlot16 = 0xFFFFu;
 constexpr uint32_t kGroupMaxCv = 65000;       // slots are stored as uint16
 
+// Position of element (slot, cell) inside a per-control-volume array of a group: the linear index
+// slot * kG + cell with the 16-byte chunk index inside each 128-byte line XORed with the line index
+// (the TMA "128B swizzle" pattern, applied to the HBM layout itself so that linear bulk copies keep
+// it).  Lane groups that walk rows 8 apart then fall on different shared-memory banks.  An involution;
+// all per-CV arrays of a group (V, f, 1/d, a, b, C, S, sigma, G, bg) use the same positions, so
+// element-wise loops may run over raw positions.
+ARBB_HD uint32_t gswz(uint32_t e) { return e ^ (((e >> 4) & 7u) << 1); }
+ARBB_HD uint32_t gpos(uint32_t slot, uint32_t cell) { return gswz(slot * (uint32_t)kG + cell); }
+// positions of a per-CV array: whole 128-byte lines (the swizzle permutes inside a line)
+ARBB_HD uint32_t gcv_elems(uint32_t n_cv) { return align_up(n_cv * (uint32_t)kG, 16); }
+
 struct SegRec {          // 16 bytes, one broadcast load per lane group
   uint32_t slot0;        // slot of the proximal control volume
   uint32_t pslot;        // slot of the parent control volume of slot0, or kNoSlot
@@ -91,7 +102,8 @@ ARBB_HD GConstOff gconst_offsets(uint32_t n_cv, uint32_t n_hh, uint32_t n_syn, u
   uint32_t p = 0;
   auto sec = [&](uint32_t bytes) { uint32_t at = p; p = align_up(p + bytes, 128); return at; };
   const uint32_t row = 8 * kG, row16 = 2 * kG;
-  o.f = sec(row * n_cv); o.invd = sec(row * n_cv); o.a = sec(row * n_cv); o.b = sec(row * n_cv);
+  const uint32_t cvb = 8 * gcv_elems(n_cv);
+  o.f = sec(cvb); o.invd = sec(cvb); o.a = sec(cvb); o.b = sec(cvb);
   o.hh_gna = sec(row * n_hh); o.hh_gk = sec(row * n_hh); o.hh_gl = sec(row * n_hh);
   o.syn_e = sec(syn_uniform ? 0 : row * n_syn); o.syn_decay = sec(syn_uniform ? 0 : row * n_syn);
   o.cl_t0 = sec(row * n_cl); o.cl_t1 = sec(row * n_cl); o.cl_amp = sec(row * n_cl);
@@ -108,7 +120,7 @@ ARBB_HD GStateOff gstate_offsets(uint32_t n_cv, uint32_t n_hh, uint32_t n_syn) {
   GStateOff o;
   uint32_t p = 0;
   auto sec = [&](uint32_t n) { uint32_t at = p; p = align_up(p + n, 16); return at; };
-  o.v = sec(kG * n_cv); o.g = sec(kG * n_syn); o.rt = sec(kRtDoubles * kG);
+  o.v = sec(gcv_elems(n_cv)); o.g = sec(kG * n_syn); o.rt = sec(kRtDoubles * kG);
   o.m = sec(kG * n_hh); o.h = sec(kG * n_hh); o.n = sec(kG * n_hh);
   o.total = p;
   return o;
@@ -118,7 +130,7 @@ ARBB_HD GStateOff gstate_offsets(uint32_t n_cv, uint32_t n_hh, uint32_t n_syn) {
 struct GGenOff { uint32_t C, S, sig, G, b, syn_tau, total; };
 ARBB_HD GGenOff ggen_offsets(uint32_t n_cv, uint32_t n_syn) {
   GGenOff o;
-  const uint32_t n = kG * n_cv;
+  const uint32_t n = gcv_elems(n_cv);
   o.C = 0; o.S = n; o.sig = 2 * n; o.G = 3 * n; o.b = 4 * n; o.syn_tau = 5 * n;
   o.total = align_up(5 * n + kG * n_syn, 16);
   return o;
@@ -134,8 +146,8 @@ ARBB_HD GroupSmemPlan group_smem_plan(const GroupCaps& c) {
   GroupSmemPlan P;
   P.slot_cap = c.slot_cap;
   uint32_t p = align_up(c.state_bytes, 128);
-  P.off_f = p;     p = align_up(p + 8 * kG * c.slot_cap, 128);
-  P.off_i = p;     p = align_up(p + 8 * kG * c.slot_cap, 128);
+  P.off_f = p;     p = align_up(p + 8 * gcv_elems(c.slot_cap), 128);
+  P.off_i = p;     p = align_up(p + 8 * gcv_elems(c.slot_cap), 128);
   P.off_tail = p;  p = align_up(p + c.tail_bytes, 128);
   P.off_class = p; p = align_up(p + c.class_bytes, 128);
   P.off_buf = p;   p = align_up(p + 8 * kG * c.buf_rows, 128);

@@ -851,7 +851,7 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
       if (lc >= G.n_cell) {
         // padding lane: an isolated, inert "cell" (V stays where it is, no instances, detector unarmed)
         for (uint32_t s2 = 0; s2 < n; ++s2) {
-          const uint32_t e = s2 * kG + lc;
+          const uint32_t e = gpos(s2, lc);
           gen[go.C + e] = 1.0; st[so.v + e] = -65.0; invd[e] = 1.0; a[e] = 1.0;
         }
         det_slot[lc] = 0;
@@ -866,7 +866,7 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
       for (uint32_t i = 1; i < n; ++i) S[par[i]] += 1.0 / d.cv_raxial[a0 + i];   // ascending child order
       items.clear();
       for (uint32_t i = 0; i < n; ++i) {
-        const uint32_t e = K.cv_slot[i] * kG + lc;
+        const uint32_t e = gpos(K.cv_slot[i], lc);
         const double area = d.cv_area[a0 + i];
         gen[go.C + e] = d.cv_cm[a0 + i] * area * 1e-5;                 // nF
         gen[go.S + e] = S[i];                                          // uS
