@@ -138,6 +138,7 @@ struct arb_model {
   int cur_pool = 0;
   int sm_count = 148;
   int group_grid = 0;
+  int64_t group_launches = 0;
   int64_t opt_stages = 0;
   bool broken = false;
   std::string err;
@@ -279,6 +280,11 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     D.counters = at<unsigned long long>(m, R.counters);
     D.scan_tmp = at<uint32_t>(m, R.scan_tmp);
     D.ena = H.ena; D.ek = H.ek; D.el = H.el; D.theta = H.threshold;
+    {
+      const unsigned long long g0[2] = {(unsigned long long)m->group_grid, (unsigned long long)m->group_grid};
+      if ((e = cudaMemcpyAsync(D.counters + CNT_GROUP0, g0, sizeof g0, cudaMemcpyHostToDevice, m->stream)) != cudaSuccess) return bail(e, "upload counters");
+      if ((e = cudaStreamSynchronize(m->stream)) != cudaSuccess) return bail(e, "cudaStreamSynchronize");
+    }
     if ((e = launch_init(D, m->stream)) != cudaSuccess) return bail(e, "init kernel");
     if ((e = launch_group_init(D, m->stream)) != cudaSuccess) return bail(e, "group init kernel");
     if ((e = cudaStreamSynchronize(m->stream)) != cudaSuccess) return bail(e, "cudaStreamSynchronize");
@@ -363,6 +369,7 @@ int arb_advance(arb_model* m, double t_end, double dt) {
     for (int64_t j = 0; j < n_ep; j += fused) {
       StepArgs A;
       A.t0 = t0; A.dt = dt; A.t_end = t_end; A.k_first = k + j; A.nk = std::min(fused, n_ep - j); A.nsteps = nsteps; A.last_full = last_full;
+      A.parity = (int)(m->group_launches++ & 1);
       CU(m, launch_group_cable(D, A, m->group_grid, m->stream, &launches));
       CU(m, launch_cable(D, A, grid, m->stream, &launches));
     }

@@ -524,11 +524,23 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
   uint32_t dh_ss = 0;
 #ifdef ARBB_PROFILE
   long long prof_buf[16];
+  unsigned long long gt0;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt0));
+  const long long ck0 = clock64();
 #endif
   long long* prof = nullptr;
-  for (int64_t g = blockIdx.x; g < M.n_groups; g += gridDim.x, ++it) {
+  // Groups are claimed dynamically (group-steps differ in length: event-split sub-steps, memory
+  // placement): the first one is blockIdx.x, further ones come from this launch's work counter, which
+  // the previous launch has reset to gridDim.x; this launch resets the other one.
+  __shared__ int64_t sG[2];
+  if (tid == 0) {
+    sG[0] = blockIdx.x;
+    if (blockIdx.x == 0) M.counters[CNT_GROUP0 + (A.parity ^ 1)] = gridDim.x;
+  }
+  __syncthreads();
+  for (int64_t g = sG[0]; g < M.n_groups; g = sG[(++it) & 1u]) {
 #ifdef ARBB_PROFILE
-    prof = (blockIdx.x == 7 && tid == 0 && it >= 2 && it < 6 && A.k_first == 150) ? prof_buf : nullptr;
+    prof = (blockIdx.x == 7 && tid == 0 && (it == 2 || it == 3 || it == 20 || it == 21 || it == 38 || it == 39) && A.k_first == 150) ? prof_buf : nullptr;
     if (prof) for (int i = 0; i < 16; ++i) prof[i] = 0;
 #endif
     TICK(0);
@@ -536,7 +548,6 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
     const GConstOff co = gconst_offsets(D.n_cv, D.n_hh_rows, D.n_syn_rows, D.n_cl_rows, M.syn_uniform != 0);
     const GStateOff so = gstate_offsets(D.n_cv, D.n_hh_rows, D.n_syn_rows);
     const uint32_t vbytes = 8u * gcv_elems(D.n_cv);
-    const int64_t gn = g + gridDim.x;
     if (tid == 0) {
       // state record, f, 1/d and the const tail of the group -> shared memory (one barrier)
       const uint8_t* cb = M.fast + D.const_off;
@@ -548,8 +559,12 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
       bulk_g2s((void*)Is, cb + co.invd, vbytes, mbar);
       bulk_g2s((void*)tail, cb + co.hh_gna, tbytes, mbar);
       if (M.l2_prefetch) bulk_prefetch_l2(cb + co.a, co.hh_gna - co.a);     // a, b of this group -> L2
-    } else if (tid >= 32 && tid < 48 && gn < M.n_groups) {
-      ((uint32_t*)&sD[(it + 1) & 1u])[tid - 32] = ((const uint32_t*)&M.groups[gn])[tid - 32];
+    } else if (tid >= 32 && tid < 64) {     // warp 1 claims the next group and fetches its descriptor
+      unsigned long long gn = 0;
+      if (tid == 32) gn = atomicAdd(&M.counters[CNT_GROUP0 + A.parity], 1ull);
+      gn = __shfl_sync(kFull, gn, 0);
+      if (tid == 32) sG[(it + 1) & 1u] = (int64_t)gn;
+      if (tid < 48 && (int64_t)gn < M.n_groups) ((uint32_t*)&sD[(it + 1) & 1u])[tid - 32] = ((const uint32_t*)&M.groups[gn])[tid - 32];
     }
     if (D.class_off != cached_class) {   // tree structure differs from the previous group's
       const ClassRecord* R = (const ClassRecord*)(M.topo + D.class_off);
@@ -633,7 +648,7 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
     if (tid == 0) {
       bulk_s2g(M.state + D.state_base, Ss, 8u * so.m);
       bulk_commit();
-      if (M.l2_prefetch && gn < M.n_groups) {   // next group's records -> L2
+      if (M.l2_prefetch && sG[(it + 1) & 1u] < M.n_groups) {   // next group's records -> L2
         const GroupDesc& Dn = sD[(it + 1) & 1u];
         const GConstOff con = gconst_offsets(Dn.n_cv, Dn.n_hh_rows, Dn.n_syn_rows, Dn.n_cl_rows, M.syn_uniform != 0);
         bulk_prefetch_l2(M.fast + Dn.const_off, con.a);
@@ -653,6 +668,13 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
 #endif
   }
   run_deferred(dh, dh_gm, nullptr, dh_ss);
+#ifdef ARBB_PROFILE
+  if (tid == 0 && A.k_first == 150 && (blockIdx.x % 97 == 0 || blockIdx.x == gridDim.x - 1)) {
+    unsigned long long gt1;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt1));
+    printf("cta %d: start %llu ns, dur %llu ns, %lld cycles, %u groups\n", (int)blockIdx.x, gt0 % 100000000ull, gt1 - gt0, clock64() - ck0, it);
+  }
+#endif
   if (tid < 32) {
     for (int o = 16; o; o >>= 1) { n_sub += __shfl_xor_sync(kFull, n_sub, o); n_del += __shfl_xor_sync(kFull, n_del, o); }
     if (tid == 0) {

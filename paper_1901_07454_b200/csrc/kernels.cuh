@@ -17,7 +17,9 @@ enum Counter {
   CNT_SUBSTEPS = 5,     // cell sub-steps executed
   CNT_DELIVERED = 6,    // events delivered
   CNT_EVLIST = 7,       // size of the current epoch list
-  CNT_COUNT = 8
+  CNT_GROUP0 = 8,       // group kernel: next unclaimed group of even / odd launches (dynamic
+  CNT_GROUP1 = 9,       //   distribution of groups over the persistent CTAs)
+  CNT_COUNT = 10
 };
 
 struct EventPool { double* t; uint32_t* dst; uint32_t* gidx; double* w; };
@@ -70,6 +72,7 @@ struct StepArgs {
   double t0, dt, t_end;  // grid t_k = t0 + k*dt, t_nsteps = t_end
   int64_t k_first, nk, nsteps;
   int last_full;         // the last grid step has nominal length dt
+  int parity;            // launch counter & 1 (group kernel: which work counter this launch claims from)
 };
 
 // all launchers queue work on `s` and return the last CUDA error code
