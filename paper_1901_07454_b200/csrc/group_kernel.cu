@@ -39,7 +39,13 @@ namespace {
 #define ARBB_CVREGS 8
 #endif
 constexpr int kT = kGroupThreads;
-constexpr int kRows = 4;                  // rows of a segment a lane group loads ahead of the recurrence
+#ifndef ARBB_ROWS
+#define ARBB_ROWS 4
+#endif
+#ifndef ARBB_CV_EARLY
+#define ARBB_CV_EARLY 0
+#endif
+constexpr int kRows = ARBB_ROWS;                  // rows of a segment a lane group loads ahead of the recurrence
 constexpr int kCvRegs = ARBB_CVREGS;               // rhs coefficient pairs (a, b) a thread keeps in flight in phase C
 
 // -DARBB_PROFILE: one CTA prints clock64() at the phase boundaries of a few group-steps (development aid)
@@ -331,6 +337,19 @@ __device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView
     }
   }
 
+  TICK(17);
+#if ARBB_CV_EARLY
+  // the first rhs coefficients of phase C are requested now (L2, pulled there by the TMA prefetch) so
+  // that their latency hides behind phase B
+  double ar[kCvRegs], br[kCvRegs];
+  if (!kGen) {
+#pragma unroll
+    for (int j = 0; j < kCvRegs; ++j) {
+      const uint32_t p = tid + j * kT;
+      if (p < nE_cv) { ar[j] = U.a[p]; br[j] = U.b[p]; }
+    }
+  }
+#endif
   // ---- B: currents of HH, synapses and clamps from V(t); the passive current is
   // folded into a, b.  Items of one cell on one CV form a run; its first item sums it in index order.
   double* xI = buf;
@@ -343,6 +362,7 @@ __device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView
     xI[e] = U.hh_gna[e] * m * m * m * hh * (v - M.ena) + U.hh_gna[e + U.hh_cs] * n * n * n * n * (v - M.ek) +
             U.hh_gna[e + 2 * U.hh_cs] * (v - M.el);
   }
+  TICK(18);
 #pragma unroll 1
   for (uint32_t e = rtid; e < nE_syn; e += kT) {
     const uint32_t slot = U.syn_slot[e];
@@ -381,12 +401,14 @@ __device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView
   // ---- C: rhs_i = (C_i/delta - G_i) V_i + G_i e_i - I_i, in place of V; positions, not
   // (slot, cell) pairs: every per-CV array of the group uses the same positions
   if (!kGen) {
-    double ar[kCvRegs], br[kCvRegs];      // one round trip to L2 for the whole group when it fits
+#if !ARBB_CV_EARLY
+    double ar[kCvRegs], br[kCvRegs];
 #pragma unroll
     for (int j = 0; j < kCvRegs; ++j) {
       const uint32_t p = tid + j * kT;
       if (p < nE_cv) { ar[j] = U.a[p]; br[j] = U.b[p]; }
     }
+#endif
 #pragma unroll
     for (int j = 0; j < kCvRegs; ++j) {
       const uint32_t p = tid + j * kT;
@@ -523,7 +545,7 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
   double* dh_gm = nullptr;               // where the carried gate update of the previous group goes
   uint32_t dh_ss = 0;
 #ifdef ARBB_PROFILE
-  long long prof_buf[16];
+  long long prof_buf[24];
   unsigned long long gt0;
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt0));
   const long long ck0 = clock64();
@@ -540,8 +562,8 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
   __syncthreads();
   for (int64_t g = sG[0]; g < M.n_groups; g = sG[(++it) & 1u]) {
 #ifdef ARBB_PROFILE
-    prof = (blockIdx.x == 7 && tid == 0 && (it == 2 || it == 3 || it == 20 || it == 21 || it == 38 || it == 39) && A.k_first == 150) ? prof_buf : nullptr;
-    if (prof) for (int i = 0; i < 16; ++i) prof[i] = 0;
+    prof = (blockIdx.x == 291 && tid == 0 && (it == 10 || it == 11 || it == 12) && A.k_first == 150) ? prof_buf : nullptr;
+    if (prof) for (int i = 0; i < 24; ++i) prof[i] = 0;
 #endif
     TICK(0);
     const GroupDesc& D = sD[it & 1u];
@@ -625,7 +647,9 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
           const unsigned ba = __ballot_sync(kFull, active), bg = __ballot_sync(kFull, gen);
           if (tid == 0) { flags[0] = ba; flags[1] = bg; }
         }
+        TICK(15);
         __syncthreads();                  // also orders the delivered g += w before phase B
+        TICK(16);
         if (!flags[0]) break;
         // another (sub-)step follows: the gates of the previous one are needed now (working copy and global)
         run_deferred(dh, U.sm, U.gm, U.hh_ss);
@@ -662,7 +686,7 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
 #ifdef ARBB_PROFILE
     if (prof) {
       printf("grp %lld:", (long long)g);
-      for (int i = 1; i < 15; ++i) printf(" %d:%lld", i, prof[i] ? prof[i] - prof[0] : -1ll);
+      for (int i = 1; i < 24; ++i) printf(" %d:%lld", i, prof[i] ? prof[i] - prof[0] : -1ll);
       printf("\n");
     }
 #endif
