@@ -56,6 +56,7 @@ enum {
                                 every launch streams the state once, 1 when launches are fused     */
   ARB_OPT_L2_PREFETCH = 5,   /* cell-group kernel: 1 (default) = ask the TMA unit to pull the next group's
                                 records into L2 while the current group is integrated; 0 = off      */
+  ARB_OPT_GROUP_CTAS = 6,    /* cell-group kernel: cap on the CTAs of a launch (0 = as many as are resident) */
   ARB_OPT_TIMING = 3         /* 1: bracket the cable-step launches and the epoch-boundary kernels of
                                 every epoch with CUDA events on the model's stream (read them with
                                 ARB_PROBE_TIMING); setting the option clears the accumulated times  */
@@ -121,7 +122,8 @@ typedef struct arb_model arb_model; /* opaque; lives in host memory, owned by th
  * earlier than t = 0, inconsistent NULLs. */
 int arb_plan(const arb_desc* desc, size_t* workspace_bytes);
 
-/* Build the model: lay the cells out in units of interleaved branches, upload to
+/* Build the model: lay the cells out (cell-interleaved groups for cells that share a tree, units of
+ * interleaved branches for the rest), upload to
  * `dev_workspace` (DEVICE pointer, 256-byte aligned, >= workspace_bytes from arb_plan) on
  * `cuda_stream` (a cudaStream_t; NULL = default stream), initialise state (V = vinit, gates at
  * steady state, g = 0, t = 0; reading R4).  Returns after the upload has completed. */
@@ -149,8 +151,10 @@ int arb_voltage(arb_model* m, double* out, int64_t n_cv);
  *                  steps; the excess comes from event-driven step splitting), n >= 2.
  * ARB_PROBE_STATS: out[0..7] = {units, slots (CVs incl. padding), branches, workspace bytes,
  *                  events delivered, kernel launches so far, epoch steps, bytes of the records one
- *                  grid step reads (all units)}, n >= 8; when n >= 12 also {warp units, warps per
- *                  CTA and shared-memory bytes per warp of the last launch, distinct tree records}.
+ *                  grid step moves (all units and groups)}, n >= 8; when n >= 12 also {warp units,
+ *                  warps per CTA and shared-memory bytes per warp of the last launch, distinct tree
+ *                  records}; when n >= 16 also {cell groups, topology classes in groups, CTAs of a
+ *                  cell-group launch, shared-memory bytes per CTA of the cell-group kernel}.
  * ARB_PROBE_TIMING: out[0..3] = {ms spent in cable-step kernels, cable-step launches timed,
  *                  ms spent in epoch-boundary (spike -> event) kernels, their launches}, measured
  *                  with CUDA events while ARB_OPT_TIMING is on, n >= 4. */

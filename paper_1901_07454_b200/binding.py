@@ -13,7 +13,7 @@ LIB_PATH = os.environ.get("ARBB200_LIB") or os.path.join(_HERE, "libarbb200.so")
 
 ARB_OK, ARB_E_NULL, ARB_E_INVALID, ARB_E_WORKSPACE, ARB_E_CUDA, ARB_E_OVERFLOW, ARB_E_NOMEM = 0, -1, -2, -3, -4, -5, -6
 ARB_PROBE_M, ARB_PROBE_H, ARB_PROBE_N, ARB_PROBE_SYN_G, ARB_PROBE_TIME, ARB_PROBE_NSTEPS, ARB_PROBE_STATS, ARB_PROBE_TIMING = range(8)
-ARB_OPT_FUSED_STEPS, ARB_OPT_EPOCH_STEPS, ARB_OPT_TIMING, ARB_OPT_STAGES, ARB_OPT_L2_PREFETCH = 1, 2, 3, 4, 5
+ARB_OPT_FUSED_STEPS, ARB_OPT_EPOCH_STEPS, ARB_OPT_TIMING, ARB_OPT_STAGES, ARB_OPT_L2_PREFETCH, ARB_OPT_GROUP_CTAS = 1, 2, 3, 4, 5, 6
 ARB_CFG_UNIT_BYTES = 1
 ARB_CFG_GROUP_MIN_CELLS = 2
 
@@ -149,7 +149,7 @@ class Model:
         return out
 
     def probe(self, what):
-        n = {ARB_PROBE_SYN_G: self.n_syn, ARB_PROBE_TIME: 1, ARB_PROBE_NSTEPS: 2, ARB_PROBE_STATS: 12,
+        n = {ARB_PROBE_SYN_G: self.n_syn, ARB_PROBE_TIME: 1, ARB_PROBE_NSTEPS: 2, ARB_PROBE_STATS: 16,
              ARB_PROBE_TIMING: 4}.get(what, self.n_cv)
         out = np.empty(n)
         self._check(lib().arb_probe(self._h, what, _ptr(out), n))
@@ -169,7 +169,8 @@ class Model:
         return dict(units=int(s[0]), slots=int(s[1]), branches=int(s[2]), workspace_bytes=int(s[3]),
                     events_delivered=int(s[4]), launches=int(s[5]), epoch_steps=int(s[6]),
                     streamed_bytes_per_step=int(s[7]), warp_units=int(s[8]), warps_per_cta=int(s[9]),
-                    smem_per_warp=int(s[10]), topo_records=int(s[11]))
+                    smem_per_warp=int(s[10]), topo_records=int(s[11]), groups=int(s[12]), classes=int(s[13]),
+                    group_ctas=int(s[14]), group_smem=int(s[15]))
 
     def timing(self):
         t = self.probe(ARB_PROBE_TIMING)

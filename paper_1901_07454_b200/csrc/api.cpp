@@ -49,8 +49,9 @@ Caps capacities(const HostModel& H) {
   return c;
 }
 
-// group kernel: per resident CTA fgen | invdgen for event-split sub-steps
-int64_t gscratch_stride(const HostModel& H) { return 2 * (int64_t)gcv_elems(H.gcaps.slot_cap); }
+// group kernel: no global scratch any more (event-split sub-steps overwrite their column of the
+// shared-memory factors); the region is kept at zero size
+int64_t gscratch_stride(const HostModel&) { return 0; }
 int64_t gscratch_ctas(const HostModel& H) { return std::min<int64_t>(H.n_groups, kMaxGroupCtas); }
 
 int64_t warp_scratch_stride(const HostModel& H) { return 2 * (int64_t)H.slot_cap + align_up(H.lane_cap, 2); }
@@ -137,8 +138,9 @@ struct arb_model {
   int64_t cable_timed = 0, event_timed = 0;
   int cur_pool = 0;
   int sm_count = 148;
-  int group_grid = 0;
-  int64_t group_launches = 0;
+  int group_grid = 0, last_ggrid = 0;
+  int64_t group_launches = 0, opt_group_ctas = 0;
+  int64_t group_slots = 0, group_streamed = 0;   // statistics: CV slots incl. padding, bytes one grid step streams
   int64_t opt_stages = 0;
   bool broken = false;
   std::string err;
@@ -270,6 +272,11 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     D.syn_uniform = H.syn_uniform ? 1 : 0; D.syn_e_u = H.syn_e_u; D.syn_tau_u = H.syn_tau_u; D.syn_decay_u = 1.0;
     D.plan = make_plan(H, 1);
     D.groups = at<GroupDesc>(m, R.gdescs); D.n_groups = H.n_groups;
+    for (const GroupDesc& g : H.gdescs) {
+      const GConstOff co = gconst_offsets(g.n_cv, g.n_hh_rows, g.n_syn_rows, g.n_cl_rows, H.syn_uniform);
+      m->group_slots += (int64_t)g.n_cv * kG;
+      m->group_streamed += co.total + 8 * (int64_t)gstate_offsets(g.n_cv, g.n_hh_rows, g.n_syn_rows).total + 8 * (int64_t)gcv_elems(g.n_cv);
+    }
     D.gscratch = at<double>(m, R.gscratch); D.gscratch_stride = gscratch_stride(H);
     D.gplan = group_smem_plan(H.gcaps);
     D.l2_prefetch = 1;
@@ -284,6 +291,7 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
       const unsigned long long g0[2] = {(unsigned long long)m->group_grid, (unsigned long long)m->group_grid};
       if ((e = cudaMemcpyAsync(D.counters + CNT_GROUP0, g0, sizeof g0, cudaMemcpyHostToDevice, m->stream)) != cudaSuccess) return bail(e, "upload counters");
       if ((e = cudaStreamSynchronize(m->stream)) != cudaSuccess) return bail(e, "cudaStreamSynchronize");
+      m->last_ggrid = m->group_grid;
     }
     if ((e = launch_init(D, m->stream)) != cudaSuccess) return bail(e, "init kernel");
     if ((e = launch_group_init(D, m->stream)) != cudaSuccess) return bail(e, "group init kernel");
@@ -343,6 +351,14 @@ int arb_advance(arb_model* m, double t_end, double dt) {
     grid = (int)std::min<int64_t>(m->sm_count, (m->H.n_warp_units + P.warps - 1) / P.warps);
     D.plan = P;
   }
+  // a changed CTA count invalidates the work counters (they are reset to gridDim.x by the previous launch)
+  const int ggrid = m->opt_group_ctas > 0 ? (int)std::min<int64_t>(m->opt_group_ctas, m->group_grid) : m->group_grid;
+  if (ggrid != m->last_ggrid && m->H.n_groups > 0) {
+    const unsigned long long g0[2] = {(unsigned long long)ggrid, (unsigned long long)ggrid};
+    CU(m, cudaMemcpyAsync(D.counters + CNT_GROUP0, g0, sizeof g0, cudaMemcpyHostToDevice, m->stream));
+    CU(m, cudaStreamSynchronize(m->stream));
+    m->last_ggrid = ggrid;
+  }
   int launches = 0;
   // optional device timing (ARB_OPT_TIMING): four events per epoch on the model's stream
   size_t n_tev = 0;
@@ -370,7 +386,7 @@ int arb_advance(arb_model* m, double t_end, double dt) {
       StepArgs A;
       A.t0 = t0; A.dt = dt; A.t_end = t_end; A.k_first = k + j; A.nk = std::min(fused, n_ep - j); A.nsteps = nsteps; A.last_full = last_full;
       A.parity = (int)(m->group_launches++ & 1);
-      CU(m, launch_group_cable(D, A, m->group_grid, m->stream, &launches));
+      CU(m, launch_group_cable(D, A, ggrid, m->stream, &launches));
       CU(m, launch_cable(D, A, grid, m->stream, &launches));
     }
     CU(m, stamp());
@@ -477,12 +493,17 @@ int arb_probe(arb_model* m, int what, double* out, int64_t n) {
       if (what == ARB_PROBE_NSTEPS) { out[0] = (double)m->grid_steps; out[1] = (double)cnt[CNT_SUBSTEPS]; return ARB_OK; }
       int64_t slots = 0, streamed = 0;
       for (const auto& u : m->H.units) { slots += u.n_slot; streamed += u.fast_bytes + u.state_bytes; }
+      slots += m->group_slots; streamed += m->group_streamed;
       out[0] = (double)m->H.n_units; out[1] = (double)slots; out[2] = (double)m->H.n_lanes;
       out[3] = (double)m->R.total; out[4] = (double)cnt[CNT_DELIVERED]; out[5] = (double)m->launches;
       out[6] = (double)m->last_epoch_steps; out[7] = (double)streamed;
       if (n >= 12) {
         out[8] = (double)m->H.n_warp_units; out[9] = (double)m->D.plan.warps; out[10] = (double)m->D.plan.warp_bytes;
         out[11] = (double)m->H.topo_records;
+      }
+      if (n >= 16) {
+        out[12] = (double)m->H.n_groups; out[13] = (double)m->H.n_classes; out[14] = (double)m->group_grid;
+        out[15] = (double)m->D.gplan.bytes;
       }
       return ARB_OK;
     }
@@ -524,6 +545,7 @@ int arb_set_option(arb_model* m, int key, int64_t value) {
     case ARB_OPT_EPOCH_STEPS: m->opt_epoch = value; return ARB_OK;
     case ARB_OPT_STAGES: m->opt_stages = value; return ARB_OK;
     case ARB_OPT_L2_PREFETCH: m->D.l2_prefetch = value != 0; return ARB_OK;
+    case ARB_OPT_GROUP_CTAS: m->opt_group_ctas = value; return ARB_OK;
     case ARB_OPT_TIMING:
       m->opt_timing = value;
       m->cable_ms = m->event_ms = 0; m->cable_timed = m->event_timed = 0;

@@ -131,20 +131,31 @@ __device__ __forceinline__ SegRec load_seg(const SegRec* p) {
 __device__ __forceinline__ void eliminate_seg(const GView& U, const SegRec& sg, uint32_t seg_idx, int c, double delta,
                                               double* fout, double* invdout, double* dcon) {
   const double *C = U.C(), *S = U.S(), *sig = U.sig();
-  uint32_t lin = (sg.slot0 + sg.len - 1) * kG + c, s = gswz(lin);
-  double d = C[s] / delta + S[s];
-  for (uint32_t j = 0; j < sg.ccnt; ++j) d -= dcon[(uint32_t)U.child[sg.cbeg + j] * kG + c];
+  constexpr int kB = 8;                   // rows whose C, S, sigma are requested together (global memory)
+  uint32_t lin = (sg.slot0 + sg.len - 1) * kG + c;
+  double carry = 0.0;                     // f_{k+1} * sigma_{k+1}: what row k loses to its child in the segment
+  for (uint32_t j = 0; j < sg.ccnt; ++j) carry -= dcon[(uint32_t)U.child[sg.cbeg + j] * kG + c];
   double fk = 0.0, sk = 0.0;
-  for (uint32_t k = sg.len; k-- > 0;) {
-    const double invd = 1.0 / d;
-    sk = sig[s];
-    fk = -sk * invd;
-    fout[s] = fk;
-    invdout[s] = invd;
-    if (k > 0) {
-      lin -= kG; s = gswz(lin);
-      d = fma(fk, sk, C[s] / delta + S[s]);          // d_p -= f*u with u = -sigma
-    }
+  int left = sg.len;
+  while (left > 0) {
+    double cr[kB], sr[kB], gr[kB];
+    uint32_t p[kB];
+#pragma unroll
+    for (int j = 0; j < kB; ++j)
+      if (j < left) { p[j] = gswz(lin - j * kG); cr[j] = C[p[j]]; sr[j] = S[p[j]]; gr[j] = sig[p[j]]; }
+#pragma unroll
+    for (int j = 0; j < kB; ++j)
+      if (j < left) {
+        const double d = (cr[j] / delta + sr[j]) + carry;
+        const double invd = 1.0 / d;
+        sk = gr[j];
+        fk = -sk * invd;
+        fout[p[j]] = fk;
+        invdout[p[j]] = invd;
+        carry = fk * sk;                  // d_p -= f*u with u = -sigma
+      }
+    lin -= kB * kG;
+    left -= kB;
   }
   dcon[seg_idx * kG + c] = -fk * sk;
 }
@@ -316,7 +327,7 @@ __device__ __forceinline__ void run_deferred(HHDefer& dh, double* dst0, double* 
 // ------------------------------------------------------------------------------------------
 template <bool kGen>
 __device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView& U, double* Vs, const double* Fs, const double* Is,
-                                              double* buf, const CellS& cs, double* fgen, double* invdgen, double dt, HHDefer& dh,
+                                              double* buf, const CellS& cs, double dt, HHDefer& dh,
                                               long long* prof) {
   const int tid = threadIdx.x, c = tid % kG, h = tid / kG;
   const int rtid = kT - 1 - tid, rc = rtid % kG;      // reversed dealing of instances; cell of those
@@ -324,14 +335,15 @@ __device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView
   const uint32_t md = kGen ? cs.mode[c] : 1u, rmd = kGen ? cs.mode[rc] : 1u;
   const double delta = kGen ? cs.delta[c] : dt, rdelta = kGen ? cs.delta[rc] : dt;
 
-  // ---- event-split sub-steps: this cell's matrix is re-eliminated for its own delta (reading R9)
+  // ---- event-split sub-steps: this cell's matrix is re-eliminated for its own delta (reading R9); its
+  // column of the shared-memory factors is overwritten (the caller reloads them before they are needed again)
   if (kGen) {
     for (uint32_t st = 0; st < U.n_stage; ++st) {
       const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
       if (md == 2u)
         for (uint32_t q = beg; q < end; ++q) {
           const uint32_t si = U.order[q];
-          eliminate_seg(U, load_seg(U.segs + si), si, c, delta, fgen, invdgen, buf);
+          eliminate_seg(U, load_seg(U.segs + si), si, c, delta, const_cast<double*>(Fs), const_cast<double*>(Is), buf);
         }
       __syncthreads();
     }
@@ -458,8 +470,7 @@ __device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView
 
   TICK(7);
   // ---- D: backward sweep, stage by stage; E: forward substitution, stages reversed; V <- V'
-  if (kGen) sweeps(U, h, c, md != 0u, md == 2u ? fgen : Fs, md == 2u ? invdgen : Is, Vs, buf, prof);
-  else sweeps(U, h, c, true, Fs, Is, Vs, buf, prof);   // buf: xI is dead, it now holds the contributions
+  sweeps(U, h, c, kGen ? md != 0u : true, Fs, Is, Vs, buf, prof);   // buf: xI is dead, it now holds the contributions
   __syncthreads();
   TICK(11);
 
@@ -520,7 +531,7 @@ __device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView
 __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kernel(DevModel M, StepArgs A) {
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ GroupDesc sD[2];            // this group's and the next group's descriptors
-  __shared__ uint32_t flags[2];
+  __shared__ uint32_t flags[3];
   const GroupSmemPlan P = M.gplan;
   double* Ss = (double*)smem;            // state record; V first
   double* Vs = Ss;
@@ -532,13 +543,12 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
   const CellS cs = carve_cells(smem + P.off_cell, kG);
   uint64_t* mbar = (uint64_t*)(smem + P.off_mbar);
   const int tid = threadIdx.x;
-  double* fgen = M.gscratch + (int64_t)blockIdx.x * M.gscratch_stride;
-  double* invdgen = fgen + (size_t)gcv_elems(P.slot_cap);
-  if (tid == 0) { mbar_init(mbar, 1); fence_mbar_init(); }
+  if (tid == 0) { mbar_init(mbar, 1); mbar_init(mbar + 1, 1); fence_mbar_init(); }
   if (tid < 16 && blockIdx.x < M.n_groups) ((uint32_t*)&sD[0])[tid] = ((const uint32_t*)&M.groups[blockIdx.x])[tid];
   __syncthreads();
   unsigned n_sub = 0, n_del = 0;
-  uint32_t it = 0;
+  uint32_t it = 0, par2 = 0;
+  bool fi_dirty = false;                 // f, 1/d in shared memory differ from the group's record
   int64_t cached_class = -1;
   HHDefer dh;
   clear(dh);
@@ -562,7 +572,7 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
   __syncthreads();
   for (int64_t g = sG[0]; g < M.n_groups; g = sG[(++it) & 1u]) {
 #ifdef ARBB_PROFILE
-    prof = (blockIdx.x == 291 && tid == 0 && (it == 10 || it == 11 || it == 12) && A.k_first == 150) ? prof_buf : nullptr;
+    prof = (blockIdx.x == 7 && tid == 0 && it >= 1 && it <= 3 && A.k_first == 150) ? prof_buf : nullptr;
     if (prof) for (int i = 0; i < 24; ++i) prof[i] = 0;
 #endif
     TICK(0);
@@ -596,6 +606,7 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
       cached_class = D.class_off;
       __syncthreads();
     }
+    fi_dirty = false;                    // fresh copies are on their way
     GView U;
     make_gview(U, M, D, Ss, tail, cls);
     // the previous group's last gate update: registers -> global m, h, n, while the copies are in flight
@@ -619,7 +630,7 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
       for (;;) {
         // ---- A: deliver the events due now, choose each cell's (sub-)step (R9)
         if (tid < 32) {
-          bool active = false, gen = false;
+          bool active = false, gen = false, split = false;
           if (tid < kG) {
             const double t = cs.tcur[tid];
             uint32_t md = 0;
@@ -642,10 +653,10 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
               if ((uint32_t)tid < U.n_cell) ++n_sub;
             }
             cs.mode[tid] = md;
-            gen = md != 1u;
+            gen = md != 1u; split = md == 2u;
           }
-          const unsigned ba = __ballot_sync(kFull, active), bg = __ballot_sync(kFull, gen);
-          if (tid == 0) { flags[0] = ba; flags[1] = bg; }
+          const unsigned ba = __ballot_sync(kFull, active), bg = __ballot_sync(kFull, gen), bs = __ballot_sync(kFull, split);
+          if (tid == 0) { flags[0] = ba; flags[1] = bg; flags[2] = bs; }
         }
         TICK(15);
         __syncthreads();                  // also orders the delivered g += w before phase B
@@ -653,8 +664,24 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
         if (!flags[0]) break;
         // another (sub-)step follows: the gates of the previous one are needed now (working copy and global)
         run_deferred(dh, U.sm, U.gm, U.hh_ss);
-        if (flags[1]) group_substep<true>(M, U, Vs, Fs, Is, buf, cs, fgen, invdgen, A.dt, dh, prof);
-        else group_substep<false>(M, U, Vs, Fs, Is, buf, cs, fgen, invdgen, A.dt, dh, prof);
+        if (fi_dirty) {                   // an event-split sub-step has overwritten columns of f, 1/d: reload
+          if (tid == 0) {
+            const uint8_t* cb = M.fast + D.const_off;
+            fence_proxy_async();
+            mbar_expect_tx(mbar + 1, 2u * vbytes);
+            bulk_g2s((void*)Fs, cb + co.f, vbytes, mbar + 1);
+            bulk_g2s((void*)Is, cb + co.invd, vbytes, mbar + 1);
+          }
+          mbar_wait(mbar + 1, par2);
+          par2 ^= 1u;
+          fi_dirty = false;
+        }
+        if (flags[1]) {
+          group_substep<true>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, prof);
+          fi_dirty = flags[2] != 0;
+        } else {
+          group_substep<false>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, prof);
+        }
         __syncthreads();
       }
       __syncthreads();                    // flags are rewritten by the next grid step
@@ -693,10 +720,10 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
   }
   run_deferred(dh, dh_gm, nullptr, dh_ss);
 #ifdef ARBB_PROFILE
-  if (tid == 0 && A.k_first == 150 && (blockIdx.x % 97 == 0 || blockIdx.x == gridDim.x - 1)) {
+  if (tid == 0 && A.k_first >= 150 && A.k_first < 156 && (blockIdx.x == 0 || blockIdx.x == gridDim.x - 1)) {
     unsigned long long gt1;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt1));
-    printf("cta %d: start %llu ns, dur %llu ns, %lld cycles, %u groups\n", (int)blockIdx.x, gt0 % 100000000ull, gt1 - gt0, clock64() - ck0, it);
+    printf("k %d cta %d: start %llu end %llu ns, %u groups\n", (int)A.k_first, (int)blockIdx.x, gt0 % 100000000ull, gt1 % 100000000ull, it);
   }
 #endif
   if (tid < 32) {

@@ -326,7 +326,10 @@ def test_full_size_large_config_sampled_cells(B, orc, layout):
     # properties that hold at any size
     assert np.all(np.isfinite(v)) and v.min() > -90 and v.max() < 60
     steps = g.probe(B.ARB_PROBE_NSTEPS)
-    delivered = g.stats()["events_delivered"]
+    st = g.stats()
+    # every cell of configs[3] has the same tree: one class, all cells in cell-interleaved groups
+    assert st["classes"] == 1 and st["units"] == 0 and st["groups"] * 4 >= m["n_cells"] and st["group_ctas"] >= 148
+    delivered = st["events_delivered"]
     assert steps[0] == 200 and delivered == int(np.sum(m["ext_time"] < 5.0))
     assert steps[1] >= 200 * m["n_cells"]
     g.close()
