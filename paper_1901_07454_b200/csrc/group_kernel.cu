@@ -160,6 +160,28 @@ __device__ __forceinline__ void eliminate_seg(const GView& U, const SegRec& sg, 
   dcon[seg_idx * kG + c] = -fk * sk;
 }
 
+// The same elimination for an event-split sub-step, out of shared memory: the caller has put
+// C_k/delta + S_k into I and sigma_k into F (this cell's column); they are replaced by 1/d_k and f_k.
+__device__ __forceinline__ void eliminate_seg_smem(const GView& U, const SegRec& sg, uint32_t seg_idx, int c,
+                                                   double* F, double* I, double* dcon) {
+  uint32_t lin = (sg.slot0 + sg.len - 1) * kG + c;
+  double carry = 0.0;
+  for (uint32_t j = 0; j < sg.ccnt; ++j) carry -= dcon[(uint32_t)U.child[sg.cbeg + j] * kG + c];
+  double fk = 0.0, sk = 0.0;
+#pragma unroll 2
+  for (int left = sg.len; left > 0; --left, lin -= kG) {
+    const uint32_t p = gswz(lin);
+    const double d = I[p] + carry;
+    const double invd = 1.0 / d;
+    sk = F[p];
+    fk = -sk * invd;
+    F[p] = fk;
+    I[p] = invd;
+    carry = fk * sk;                      // d_p -= f*u with u = -sigma
+  }
+  dcon[seg_idx * kG + c] = -fk * sk;
+}
+
 // ------------------------------------------------------------------------------------------
 // Backward (leaves -> root) sweep of one segment on the rhs held in Vs:
 //   rhs_{k-1} -= f_k rhs_k along the segment; the parent control volume loses con[segment] = f_0 rhs_0;
@@ -338,12 +360,23 @@ __device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView
   // ---- event-split sub-steps: this cell's matrix is re-eliminated for its own delta (reading R9); its
   // column of the shared-memory factors is overwritten (the caller reloads them before they are needed again)
   if (kGen) {
+    double* F = const_cast<double*>(Fs);
+    double* I = const_cast<double*>(Is);
+    {                                     // one round trip to global memory for all rows of the split cells
+      const double *C = U.C(), *S = U.S(), *sig = U.sig();
+#pragma unroll 4
+      for (uint32_t p = tid; p < nE_cv; p += kT) {
+        const uint32_t cell = gswz(p) % kG;
+        if (cs.mode[cell] == 2u) { I[p] = C[p] / cs.delta[cell] + S[p]; F[p] = sig[p]; }
+      }
+    }
+    __syncthreads();
     for (uint32_t st = 0; st < U.n_stage; ++st) {
       const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
       if (md == 2u)
         for (uint32_t q = beg; q < end; ++q) {
           const uint32_t si = U.order[q];
-          eliminate_seg(U, load_seg(U.segs + si), si, c, delta, const_cast<double*>(Fs), const_cast<double*>(Is), buf);
+          eliminate_seg_smem(U, load_seg(U.segs + si), si, c, F, I, buf);
         }
       __syncthreads();
     }
@@ -559,6 +592,8 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
   unsigned long long gt0;
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt0));
   const long long ck0 = clock64();
+  int prof_ngen = 0;
+  unsigned long long prof_gen_ns = 0;
 #endif
   long long* prof = nullptr;
   // Groups are claimed dynamically (group-steps differ in length: event-split sub-steps, memory
@@ -677,7 +712,15 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
           fi_dirty = false;
         }
         if (flags[1]) {
+#ifdef ARBB_PROFILE
+          unsigned long long ga, gb;
+          asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ga));
+#endif
           group_substep<true>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, prof);
+#ifdef ARBB_PROFILE
+          asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gb));
+          ++prof_ngen; prof_gen_ns += gb - ga;
+#endif
           fi_dirty = flags[2] != 0;
         } else {
           group_substep<false>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, prof);
@@ -720,10 +763,10 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
   }
   run_deferred(dh, dh_gm, nullptr, dh_ss);
 #ifdef ARBB_PROFILE
-  if (tid == 0 && A.k_first >= 150 && A.k_first < 156 && (blockIdx.x == 0 || blockIdx.x == gridDim.x - 1)) {
-    unsigned long long gt1;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt1));
-    printf("k %d cta %d: start %llu end %llu ns, %u groups\n", (int)A.k_first, (int)blockIdx.x, gt0 % 100000000ull, gt1 % 100000000ull, it);
+  unsigned long long gt1;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt1));
+  if (tid == 0 && A.k_first >= 150 && A.k_first < 153 && (gt1 - gt0 > 110000 || blockIdx.x == 0)) {
+    printf("k %d cta %d: dur %llu ns, %u groups, %d general passes, gen ns %llu\n", (int)A.k_first, (int)blockIdx.x, gt1 - gt0, it, prof_ngen, prof_gen_ns);
   }
 #endif
   if (tid < 32) {
