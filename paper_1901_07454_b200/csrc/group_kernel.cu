@@ -364,10 +364,11 @@ __device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView
     double* I = const_cast<double*>(Is);
     {                                     // one round trip to global memory for all rows of the split cells
       const double *C = U.C(), *S = U.S(), *sig = U.sig();
+      const uint32_t pcell = gswz((uint32_t)tid) % kG;       // the cell of all positions tid + j * kT
+      if (cs.mode[pcell] == 2u) {
+        const double pdelta = cs.delta[pcell];
 #pragma unroll 4
-      for (uint32_t p = tid; p < nE_cv; p += kT) {
-        const uint32_t cell = gswz(p) % kG;
-        if (cs.mode[cell] == 2u) { I[p] = C[p] / cs.delta[cell] + S[p]; F[p] = sig[p]; }
+        for (uint32_t p = tid; p < nE_cv; p += kT) { I[p] = C[p] / pdelta + S[p]; F[p] = sig[p]; }
       }
     }
     __syncthreads();
@@ -461,11 +462,18 @@ __device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView
     }
     for (uint32_t p = tid + kCvRegs * kT; p < nE_cv; p += kT) Vs[p] = fma(U.a[p], Vs[p], U.b[p]);
   } else {
-    const double *C = U.C(), *G = U.G(), *bg = U.bg();
-    for (uint32_t p = tid; p < nE_cv; p += kT) {
-      const uint32_t cell = gswz(p) % kG, m = cs.mode[cell];
-      if (m == 1u) Vs[p] = fma(U.a[p], Vs[p], U.b[p]);
-      else if (m == 2u) Vs[p] = fma(C[p] / cs.delta[cell] - G[p], Vs[p], bg[p]);
+    // every position p = tid + j * kT a thread visits belongs to the same cell: kT is a multiple of
+    // 128 positions, the period of the swizzle
+    static_assert(kT % 128 == 0, "element-wise loops assume one cell per thread");
+    const uint32_t pcell = gswz((uint32_t)tid) % kG, pmd = cs.mode[pcell];
+    if (pmd == 1u) {
+#pragma unroll 4
+      for (uint32_t p = tid; p < nE_cv; p += kT) Vs[p] = fma(U.a[p], Vs[p], U.b[p]);
+    } else if (pmd == 2u) {
+      const double *C = U.C(), *G = U.G(), *bg = U.bg();
+      const double pdelta = cs.delta[pcell];
+#pragma unroll 4
+      for (uint32_t p = tid; p < nE_cv; p += kT) Vs[p] = fma(C[p] / pdelta - G[p], Vs[p], bg[p]);
     }
   }
   TICK(5);
