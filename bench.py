@@ -314,8 +314,34 @@ def run_ours(args):
            "h2d_bytes_per_step": 8 * (n_cv + m["n_syn"]), "d2h_bytes_per_step": 8 * n_cv + d2h_spikes,
            "what": "arb_set_state(V, g from pinned host) + arb_advance(one epoch) + arb_voltage + arb_spikes to host; wall clock"}
 
+    g.close()
+    del g
+    torch.cuda.empty_cache()
+
+    # ---- configs[3] exactly as BASELINE.json words it (no external drive: the network stays silent);
+    # the headline above adds the Poisson drive of SURVEY.md 8(d) C3(i), which costs event-split sub-steps
+    as_written = None
+    if not args.no_as_written:
+        mu = W.config3(n_cells=args.cells, first_cell=rank * args.cells, driven=False)
+        gu = B.Model(mu, device="cuda:%d" % local)
+        gu.set_option(B.ARB_OPT_FUSED_STEPS, fused_steps[args.mode])
+        tu = 0.0
+        _, tu = timed_epochs(torch, gu, tu, 2, sync_all)
+        gu.set_option(B.ARB_OPT_TIMING, 1)
+        n_u = max(2, args.steps // 2)
+        ums, tu = timed_epochs(torch, gu, tu, n_u, sync_all)
+        utim = gu.timing()
+        ums_all, uunits_all = reduce_over_ranks(ums, mu["n_cv"] * STEPS_PER_EPOCH * n_u, world, dev)
+        spl = STEPS_PER_EPOCH if args.mode == "fused" else 1
+        u_launch_ms = utim["cable_ms"] / max(1, utim["cable_launches"])
+        u_ach = algorithmic_bytes_per_grid_step(mu) * spl / (u_launch_ms * 1e-3) / 1e9
+        as_written = {"workload": "configs[3] as written (undriven, no events)", "value": uunits_all / (ums_all * 1e-3),
+                      "unit": UNIT, "steps": n_u, "ms_per_step": ums_all / n_u, "avg_launch_ms": u_launch_ms,
+                      "achieved_gbs": u_ach, "roofline_frac": u_ach / measured_peak_hbm()[0]}
+        gu.close()
+        del gu
+
     if rank != 0:
-        g.close()
         return
 
     # ---- roofline of the dominant kernel (cable_group_kernel: every cell of C3 is in a cell group), measured
@@ -356,8 +382,9 @@ def run_ours(args):
             "substep_overhead": float((sub1[1] - sub0[1]) / (m["n_cells"] * (sub1[0] - sub0[0])) - 1.0)}
     if other_res:
         line["fused_epoch" if other == "fused" else "stream"] = other_res
+    if as_written:
+        line["as_written"] = as_written
     print(json.dumps(line), flush=True)
-    g.close()
     if world > 1:
         torch.distributed.destroy_process_group()
 
@@ -387,6 +414,7 @@ def main():
     ap.add_argument("--ref-cells", type=int, default=2000, help="cells in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other", action="store_true", help="skip the other launch granularity")
+    ap.add_argument("--no-as-written", action="store_true", help="skip the undriven (as worded in BASELINE.json) variant")
     ap.add_argument("--selftest-dist", action="store_true", help=argparse.SUPPRESS)
     args = ap.parse_args()
     if args.selftest_dist:
