@@ -16,11 +16,11 @@
 //             concurrently, __syncthreads separates stages.  Backward (leaves -> root) runs stages
 //             0..n_stage-1, forward (root -> leaves) runs them in reverse, segments reversed.
 //
-// Per class there is one ClassRecord in the topo pool (read through L1, never staged).
+// Per class there is one ClassRecord in the topo pool (the kernel keeps the current one in shared memory).
 // Per group there are three records:
 //   const (fast pool, bytes)   f | invd | a | b | hh gna, gk, gl | syn e, decay (non-uniform only) |
 //                              clamp t0, t1, amp | hh_slot | syn_slot | cl_slot | det_slot
-//   state (state pool, doubles) V | m | h | n | g | per-cell runtime triples [cell][3]
+//   state (state pool, doubles) V | g | per-cell runtime triples [cell][3] | m | h | n
 //   gen   (gen pool, doubles)   C | S | sigma | G | bg | syn_tau   (dt-independent; factorisation
 //                              and event-split sub-steps only)
 // Rows of per-instance arrays (HH, synapses, clamps): row j = the j-th instance of every cell in
@@ -41,7 +41,7 @@ namespace arbb {
 #ifndef ARBB_GROUP_MIN_CTAS
 #define ARBB_GROUP_MIN_CTAS 4
 #endif
-constexpr int kG = ARBB_G;                    // cells per group = lanes per lane group (8, 16 or 32)
+constexpr int kG = ARBB_G;                    // cells per group = lanes per lane group (4, 8, 16 or 32)
 constexpr int kLaneGroups = 32 / kG;          // lane groups per warp
 constexpr int kGroupWarps = ARBB_GROUP_WARPS; // warps per CTA of the group kernel
 constexpr int kGroupThreads = kGroupWarps * 32;
