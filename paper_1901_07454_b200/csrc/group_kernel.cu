@@ -160,26 +160,30 @@ __device__ __forceinline__ void eliminate_seg(const GView& U, const SegRec& sg, 
   dcon[seg_idx * kG + c] = -fk * sk;
 }
 
-// The same elimination for an event-split sub-step, out of shared memory: the caller has put
-// C_k/delta + S_k into I and sigma_k into F (this cell's column); they are replaced by 1/d_k and f_k.
-__device__ __forceinline__ void eliminate_seg_smem(const GView& U, const SegRec& sg, uint32_t seg_idx, int c,
-                                                   double* F, double* I, double* dcon) {
+// Re-elimination for an event-split sub-step of length delta = dt / r, out of shared memory and
+// without the dt-independent arrays: F, I hold this cell's NOMINAL f_k, 1/d_k and are replaced by the
+// ones for delta.  With sigma_k = -f_k d_k and q_c = sigma_c (1 + f_c) for the children c of k,
+//     C_k/dt = d_k - sigma_k - sum_c q_c      and      d'_k = r C_k/dt + sigma_k + sum_c q'_c,
+// so   d'_k = r (d_k - sigma_k) + sigma_k + sum_c z_c   with   z_c = q'_c - r q_c ,
+// which only needs one number per child (carried along a segment, zcon[] across segments).
+__device__ __forceinline__ void eliminate_seg_smem(const GView& U, const SegRec& sg, uint32_t seg_idx, int c, double r,
+                                                   double* F, double* I, double* zcon) {
   uint32_t lin = (sg.slot0 + sg.len - 1) * kG + c;
-  double carry = 0.0;
-  for (uint32_t j = 0; j < sg.ccnt; ++j) carry -= dcon[(uint32_t)U.child[sg.cbeg + j] * kG + c];
-  double fk = 0.0, sk = 0.0;
+  double z = 0.0;
+  for (uint32_t j = 0; j < sg.ccnt; ++j) z += zcon[(uint32_t)U.child[sg.cbeg + j] * kG + c];
 #pragma unroll 2
   for (int left = sg.len; left > 0; --left, lin -= kG) {
     const uint32_t p = gswz(lin);
-    const double d = I[p] + carry;
-    const double invd = 1.0 / d;
-    sk = F[p];
-    fk = -sk * invd;
-    F[p] = fk;
+    const double f0 = F[p], d0 = 1.0 / I[p];
+    const double sk = -f0 * d0;
+    const double d1 = fma(r, d0 - sk, sk) + z;
+    const double invd = 1.0 / d1;
+    const double f1 = -sk * invd;
+    F[p] = f1;
     I[p] = invd;
-    carry = fk * sk;                      // d_p -= f*u with u = -sigma
+    z = sk * ((1.0 + f1) - r * (1.0 + f0));
   }
-  dcon[seg_idx * kG + c] = -fk * sk;
+  zcon[seg_idx * kG + c] = z;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -362,22 +366,12 @@ __device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView
   if (kGen) {
     double* F = const_cast<double*>(Fs);
     double* I = const_cast<double*>(Is);
-    {                                     // one round trip to global memory for all rows of the split cells
-      const double *C = U.C(), *S = U.S(), *sig = U.sig();
-      const uint32_t pcell = gswz((uint32_t)tid) % kG;       // the cell of all positions tid + j * kT
-      if (cs.mode[pcell] == 2u) {
-        const double pdelta = cs.delta[pcell];
-#pragma unroll 4
-        for (uint32_t p = tid; p < nE_cv; p += kT) { I[p] = C[p] / pdelta + S[p]; F[p] = sig[p]; }
-      }
-    }
-    __syncthreads();
     for (uint32_t st = 0; st < U.n_stage; ++st) {
       const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
       if (md == 2u)
         for (uint32_t q = beg; q < end; ++q) {
           const uint32_t si = U.order[q];
-          eliminate_seg_smem(U, load_seg(U.segs + si), si, c, F, I, buf);
+          eliminate_seg_smem(U, load_seg(U.segs + si), si, c, dt / cs.delta[c], F, I, buf);
         }
       __syncthreads();
     }
@@ -466,14 +460,17 @@ __device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView
     // 128 positions, the period of the swizzle
     static_assert(kT % 128 == 0, "element-wise loops assume one cell per thread");
     const uint32_t pcell = gswz((uint32_t)tid) % kG, pmd = cs.mode[pcell];
+    double* __restrict__ Vr = Vs;                            // no aliasing: the loads may run ahead of the stores
     if (pmd == 1u) {
+      const double* __restrict__ ar = U.a; const double* __restrict__ br = U.b;
 #pragma unroll 4
-      for (uint32_t p = tid; p < nE_cv; p += kT) Vs[p] = fma(U.a[p], Vs[p], U.b[p]);
+      for (uint32_t p = tid; p < nE_cv; p += kT) Vr[p] = fma(ar[p], Vr[p], br[p]);
     } else if (pmd == 2u) {
-      const double *C = U.C(), *G = U.G(), *bg = U.bg();
-      const double pdelta = cs.delta[pcell];
+      // (C/delta - G) V + G e  with  C/delta - G = a + (r - 1) C/dt  and  G e = b
+      const double* __restrict__ ar = U.a; const double* __restrict__ br = U.b; const double* __restrict__ C = U.C();
+      const double rm1 = dt / cs.delta[pcell] - 1.0;
 #pragma unroll 4
-      for (uint32_t p = tid; p < nE_cv; p += kT) Vs[p] = fma(C[p] / pdelta - G[p], Vs[p], bg[p]);
+      for (uint32_t p = tid; p < nE_cv; p += kT) Vr[p] = fma(fma(rm1, C[p] / dt, ar[p]), Vr[p], br[p]);
     }
   }
   TICK(5);
@@ -690,6 +687,7 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
               const bool fast = nominal && t == ta && next == tb;
               cs.delta[tid] = fast ? A.dt : next - t;
               md = fast ? 1u : 2u;
+              if (!fast && M.l2_prefetch) bulk_prefetch_l2(U.C(), 8u * gcv_elems(U.n_cv));   // C for the general rhs
               cs.tnext[tid] = next;
               cs.vprev[tid] = Vs[gpos(U.det_slot[tid], tid)];
               active = true;
