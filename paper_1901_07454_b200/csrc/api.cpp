@@ -32,7 +32,7 @@ struct Carver {
 };
 
 struct Regions {
-  Region units, gdescs, gscratch, gen, fast, state, topo, scratch, warp_scratch, factor_dcontrib, cell_rt_idx, cell_orig, ev_off, ev_t, ev_gidx, ev_w, ev_fill,
+  Region units, gdescs, gen, fast, state, topo, scratch, warp_scratch, factor_dcontrib, cell_rt_idx, cell_orig, ev_off, ev_t, ev_gidx, ev_w, ev_fill,
       ext_off, ext_t, ext_gidx, ext_w, ext_cur, conn_off, conn_dst, conn_gidx, conn_delay, conn_w,
       pool_t[2], pool_dst[2], pool_gidx[2], pool_w[2], spike_cell, spike_t, counters, scan_tmp,
       cv_idx, syn_idx, hh_m_idx, hh_stride, hh_cv, io;
@@ -49,10 +49,8 @@ Caps capacities(const HostModel& H) {
   return c;
 }
 
-// group kernel: no global scratch any more (event-split sub-steps overwrite their column of the
-// shared-memory factors); the region is kept at zero size
-int64_t gscratch_stride(const HostModel&) { return 0; }
-int64_t gscratch_ctas(const HostModel& H) { return std::min<int64_t>(H.n_groups, kMaxGroupCtas); }
+// upper bound of the CTAs of a cell-group launch
+int64_t group_cta_cap(const HostModel& H) { return std::min<int64_t>(H.n_groups, kMaxGroupCtas); }
 
 int64_t warp_scratch_stride(const HostModel& H) { return 2 * (int64_t)H.slot_cap + align_up(H.lane_cap, 2); }
 
@@ -76,7 +74,6 @@ Regions carve(const HostModel& H, const Caps& cap) {
   const size_t nc = (size_t)H.n_cells;
   R.units = C.take(sizeof(UnitDesc) * (size_t)H.n_units);
   R.gdescs = C.take(sizeof(GroupDesc) * (size_t)H.n_groups);
-  R.gscratch = C.take(8 * (size_t)(gscratch_ctas(H) * gscratch_stride(H)));
   R.gen = C.take(8 * (size_t)H.gen_doubles);
   R.fast = C.take((size_t)H.fast_bytes);
   R.state = C.take(8 * (size_t)H.state_doubles);
@@ -277,11 +274,10 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
       m->group_slots += (int64_t)g.n_cv * kG;
       m->group_streamed += co.total + 8 * (int64_t)gstate_offsets(g.n_cv, g.n_hh_rows, g.n_syn_rows).total + 8 * (int64_t)gcv_elems(g.n_cv);
     }
-    D.gscratch = at<double>(m, R.gscratch); D.gscratch_stride = gscratch_stride(H);
     D.gplan = group_smem_plan(H.gcaps);
     D.l2_prefetch = 1;
     if (H.n_groups > 0)
-      m->group_grid = (int)std::min<int64_t>(gscratch_ctas(H), (int64_t)m->sm_count * group_ctas);
+      m->group_grid = (int)std::min<int64_t>(group_cta_cap(H), (int64_t)m->sm_count * group_ctas);
     D.pool_cap = m->cap.pool;
     D.spike_cell = at<uint32_t>(m, R.spike_cell); D.spike_t = at<double>(m, R.spike_t); D.spike_cap = m->cap.spikes;
     D.counters = at<unsigned long long>(m, R.counters);

@@ -32,18 +32,12 @@ namespace arbb {
 
 namespace {
 
-#ifndef ARBB_SUBSTEP_INLINE
-#define ARBB_SUBSTEP_INLINE __forceinline__
-#endif
 #ifndef ARBB_CVREGS
 #define ARBB_CVREGS 8
 #endif
 constexpr int kT = kGroupThreads;
 #ifndef ARBB_ROWS
 #define ARBB_ROWS 4
-#endif
-#ifndef ARBB_CV_EARLY
-#define ARBB_CV_EARLY 0
 #endif
 constexpr int kRows = ARBB_ROWS;                  // rows of a segment a lane group loads ahead of the recurrence
 constexpr int kCvRegs = ARBB_CVREGS;               // rhs coefficient pairs (a, b) a thread keeps in flight in phase C
@@ -352,8 +346,8 @@ __device__ __forceinline__ void run_deferred(HHDefer& dh, double* dst0, double* 
 // serial parts (phase A, the narrow stages).  The HH gate updates come back deferred in `dh`.
 // ------------------------------------------------------------------------------------------
 template <bool kGen>
-__device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView& U, double* Vs, const double* Fs, const double* Is,
-                                              double* buf, const CellS& cs, double dt, HHDefer& dh,
+__device__ __forceinline__ void group_substep(const DevModel& M, const GView& U, double* Vs, const double* Fs, const double* Is,
+                                              double* buf, const CellS& cs, double dt, HHDefer& dh, double vprev, double tstart,
                                               long long* prof) {
   const int tid = threadIdx.x, c = tid % kG, h = tid / kG;
   const int rtid = kT - 1 - tid, rc = rtid % kG;      // reversed dealing of instances; cell of those
@@ -378,18 +372,6 @@ __device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView
   }
 
   TICK(17);
-#if ARBB_CV_EARLY
-  // the first rhs coefficients of phase C are requested now (L2, pulled there by the TMA prefetch) so
-  // that their latency hides behind phase B
-  double ar[kCvRegs], br[kCvRegs];
-  if (!kGen) {
-#pragma unroll
-    for (int j = 0; j < kCvRegs; ++j) {
-      const uint32_t p = tid + j * kT;
-      if (p < nE_cv) { ar[j] = U.a[p]; br[j] = U.b[p]; }
-    }
-  }
-#endif
   // ---- B: currents of HH, synapses and clamps from V(t); the passive current is
   // folded into a, b.  Items of one cell on one CV form a run; its first item sums it in index order.
   double* xI = buf;
@@ -419,7 +401,7 @@ __device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView
   }
   TICK(3);
   if (nE_cl) {
-    const double t = cs.tcur[rc];
+    const double t = kGen ? cs.tcur[rc] : tstart;
     const uint16_t* cl_slot = U.cl_slot();
     const double *cl_t0 = U.cl_t0(), *cl_t1 = U.cl_t1(), *cl_amp = U.cl_amp();
     for (uint32_t e = rtid; e < nE_cl; e += kT) {
@@ -441,14 +423,12 @@ __device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView
   // ---- C: rhs_i = (C_i/delta - G_i) V_i + G_i e_i - I_i, in place of V; positions, not
   // (slot, cell) pairs: every per-CV array of the group uses the same positions
   if (!kGen) {
-#if !ARBB_CV_EARLY
     double ar[kCvRegs], br[kCvRegs];
 #pragma unroll
     for (int j = 0; j < kCvRegs; ++j) {
       const uint32_t p = tid + j * kT;
       if (p < nE_cv) { ar[j] = U.a[p]; br[j] = U.b[p]; }
     }
-#endif
 #pragma unroll
     for (int j = 0; j < kCvRegs; ++j) {
       const uint32_t p = tid + j * kT;
@@ -547,10 +527,10 @@ __device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView
     }
   }
   if (tid < kG && md) {
-    const double vd = Vs[gpos(U.det_slot[tid], tid)], vp = cs.vprev[tid];
+    const double vd = Vs[gpos(U.det_slot[tid], tid)], vp = kGen ? cs.vprev[tid] : vprev;
     if ((uint32_t)tid < U.n_cell) {
-      if (cs.armed[tid] && vp < M.theta && M.theta <= vd) {
-        const double ts = cs.tcur[tid] + cs.delta[tid] * (M.theta - vp) / (vd - vp);
+      if (vp < M.theta && M.theta <= vd && cs.armed[tid]) {
+        const double ts = (kGen ? cs.tcur[tid] : tstart) + (kGen ? cs.delta[tid] : dt) * (M.theta - vp) / (vd - vp);
         const unsigned long long pos = atomicAdd(&M.counters[CNT_SPIKES], 1ull);
         if ((int64_t)pos < M.spike_cap) { M.spike_cell[pos] = M.cell_orig[U.cell_base + tid]; M.spike_t[pos] = ts; }
         else atomicOr(&M.counters[CNT_ERROR], 1ull);
@@ -558,7 +538,7 @@ __device__ ARBB_SUBSTEP_INLINE void group_substep(const DevModel& M, const GView
       }
       if (vd < M.theta && !cs.armed[tid]) cs.armed[tid] = 1;
     }
-    cs.tcur[tid] = cs.tnext[tid];
+    if (kGen) cs.tcur[tid] = cs.tnext[tid];
   }
   TICK(12);
 }
@@ -666,6 +646,39 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
       const double ta = (k == 0) ? A.t0 : __dadd_rn(A.t0, __dmul_rn((double)k, A.dt));
       const double tb = (k + 1 == A.nsteps) ? A.t_end : __dadd_rn(A.t0, __dmul_rn((double)(k + 1), A.dt));
       const bool nominal = (k + 1 < A.nsteps) || A.last_full;
+      // fast check: no cell has an event before the end of this nominal step -> one nominal step of the
+      // whole group, with the cells' runtime in registers (the common case; reading R9 otherwise)
+      double vprev = 0.0;
+      if (tid < 32) {
+        bool fast = true;
+        if (tid < kG) {
+          fast = nominal && !(U.srt[kRtDoubles * tid] < tb);
+          vprev = Vs[gpos(U.det_slot[tid], tid)];
+        }
+        const int all_fast = __all_sync(kFull, fast);
+        if (tid == 0) flags[0] = (uint32_t)all_fast;
+      }
+      __syncthreads();
+      if (flags[0]) {
+        if ((uint32_t)tid < U.n_cell) ++n_sub;
+        run_deferred(dh, U.sm, U.gm, U.hh_ss);
+        if (fi_dirty) {                   // an event-split sub-step has overwritten columns of f, 1/d: reload
+          if (tid == 0) {
+            const uint8_t* cb = M.fast + D.const_off;
+            fence_proxy_async();
+            mbar_expect_tx(mbar + 1, 2u * vbytes);
+            bulk_g2s((void*)Fs, cb + co.f, vbytes, mbar + 1);
+            bulk_g2s((void*)Is, cb + co.invd, vbytes, mbar + 1);
+          }
+          mbar_wait(mbar + 1, par2);
+          par2 ^= 1u;
+          fi_dirty = false;
+        }
+        group_substep<false>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, vprev, ta, prof);
+        __syncthreads();                  // flags are rewritten by the next grid step
+        continue;
+      }
+      __syncthreads();                    // everyone has read flags[0]
       if (tid < kG) cs.tcur[tid] = ta;
       for (;;) {
         // ---- A: deliver the events due now, choose each cell's (sub-)step (R9)
@@ -717,19 +730,17 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
           par2 ^= 1u;
           fi_dirty = false;
         }
-        if (flags[1]) {
+        {                                 // (all cells nominal only after events delivered exactly at the step start)
 #ifdef ARBB_PROFILE
           unsigned long long ga, gb;
           asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ga));
 #endif
-          group_substep<true>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, prof);
+          group_substep<true>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, 0.0, 0.0, prof);
 #ifdef ARBB_PROFILE
           asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gb));
           ++prof_ngen; prof_gen_ns += gb - ga;
 #endif
           fi_dirty = flags[2] != 0;
-        } else {
-          group_substep<false>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, prof);
         }
         __syncthreads();
       }

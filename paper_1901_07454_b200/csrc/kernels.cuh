@@ -62,8 +62,6 @@ struct DevModel {
   // cell groups (group_layout.h); cells of groups come first in the internal cell order
   const GroupDesc* groups;
   int64_t n_groups;
-  double* gscratch;           // group kernel: per CTA fgen | invdgen (event-split sub-steps only)
-  int64_t gscratch_stride;
   GroupSmemPlan gplan;
   int l2_prefetch;            // group kernel: TMA-prefetch the next group's records into L2
 };
