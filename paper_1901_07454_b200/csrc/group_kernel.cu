@@ -32,15 +32,18 @@ namespace arbb {
 
 namespace {
 
-#ifndef ARBB_CVREGS
-#define ARBB_CVREGS 8
+#ifndef ARBB_CUNROLL
+#define ARBB_CUNROLL 4
+#endif
+#ifndef ARBB_CRESTRICT
+#define ARBB_CRESTRICT 0
 #endif
 constexpr int kT = kGroupThreads;
+constexpr int kCUnroll = ARBB_CUNROLL;    // unrolling of the rhs loop (phase C)
 #ifndef ARBB_ROWS
-#define ARBB_ROWS 4
+#define ARBB_ROWS 8
 #endif
 constexpr int kRows = ARBB_ROWS;                  // rows of a segment a lane group loads ahead of the recurrence
-constexpr int kCvRegs = ARBB_CVREGS;               // rhs coefficient pairs (a, b) a thread keeps in flight in phase C
 
 // -DARBB_PROFILE: one CTA prints clock64() at the phase boundaries of a few group-steps (development aid)
 #ifdef ARBB_PROFILE
@@ -423,18 +426,13 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
   // ---- C: rhs_i = (C_i/delta - G_i) V_i + G_i e_i - I_i, in place of V; positions, not
   // (slot, cell) pairs: every per-CV array of the group uses the same positions
   if (!kGen) {
-    double ar[kCvRegs], br[kCvRegs];
-#pragma unroll
-    for (int j = 0; j < kCvRegs; ++j) {
-      const uint32_t p = tid + j * kT;
-      if (p < nE_cv) { ar[j] = U.a[p]; br[j] = U.b[p]; }
-    }
-#pragma unroll
-    for (int j = 0; j < kCvRegs; ++j) {
-      const uint32_t p = tid + j * kT;
-      if (p < nE_cv) Vs[p] = fma(ar[j], Vs[p], br[j]);
-    }
-    for (uint32_t p = tid + kCvRegs * kT; p < nE_cv; p += kT) Vs[p] = fma(U.a[p], Vs[p], U.b[p]);
+#if ARBB_CRESTRICT
+    const double* __restrict__ ag = U.a; const double* __restrict__ bgl = U.b; double* __restrict__ Vr = Vs;
+#else
+    const double* ag = U.a; const double* bgl = U.b; double* Vr = Vs;
+#endif
+#pragma unroll kCUnroll
+    for (uint32_t p = tid; p < nE_cv; p += kT) Vr[p] = fma(ag[p], Vr[p], bgl[p]);
   } else {
     // every position p = tid + j * kT a thread visits belongs to the same cell: kT is a multiple of
     // 128 positions, the period of the swizzle
