@@ -57,7 +57,7 @@ constexpr int kRows = ARBB_ROWS;                  // rows of a segment a lane gr
 // event-split sub-steps) are derived on demand, which keeps the kernel's register count down.
 struct GView {
   uint32_t n_cv, n_cell, n_hh, n_syn, n_cl;          // rows
-  uint32_t n_stage, n_block;
+  uint32_t n_stage, n_block, flags;
   uint32_t hh_cs, hh_ss;                             // doubles between gna|gk|gl and between m|h|n
   int syn_uniform;
   const uint8_t* tail;                               // const record from hh_gna on
@@ -92,6 +92,7 @@ struct GView {
 __device__ __forceinline__ void make_gview(GView& U, const DevModel& M, const GroupDesc& D, double* state, const uint8_t* tail,
                                            const uint8_t* cls) {
   U.n_cv = D.n_cv; U.n_cell = D.n_cell; U.n_hh = D.n_hh_rows; U.n_syn = D.n_syn_rows; U.n_cl = D.n_cl_rows;
+  U.flags = D.flags;
   U.syn_uniform = M.syn_uniform;
   const GConstOff co = gconst_offsets(D.n_cv, D.n_hh_rows, D.n_syn_rows, D.n_cl_rows, M.syn_uniform != 0);
   const uint8_t* cb = M.fast + D.const_off;
@@ -454,6 +455,9 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
   TICK(5);
   __syncthreads();
   TICK(6);
+  // HH, synapse and clamp currents of a cell may meet on a control volume: barriers in between, unless
+  // the host found that they never do in this group
+  const bool disjoint = (U.flags & GROUP_POINT_DISJOINT) != 0;
   if (nE_hh) {
   #pragma unroll 1
   for (uint32_t e = rtid; e < nE_hh; e += kT) {
@@ -461,7 +465,7 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
       if (slot == kNoSlot16 || !rmd) continue;
       Vs[gpos(slot, rc)] -= xI[e];
     }
-    __syncthreads();
+    if (!disjoint) __syncthreads();
   }
   if (nE_syn) {
   #pragma unroll 1
@@ -471,7 +475,7 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
       if (e >= (uint32_t)kG && U.syn_slot[e - kG] == slot) continue;
       Vs[gpos(slot, rc)] -= xI[nE_hh + e];
     }
-    __syncthreads();
+    if (!disjoint) __syncthreads();
   }
   if (nE_cl) {
     const uint16_t* cl_slot = U.cl_slot();
@@ -481,8 +485,9 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
       if (e >= (uint32_t)kG && cl_slot[e - kG] == slot) continue;
       Vs[gpos(slot, rc)] -= xI[nE_hh + nE_syn + e];
     }
-    __syncthreads();
+    if (!disjoint) __syncthreads();
   }
+  if (disjoint && (nE_hh | nE_syn | nE_cl)) __syncthreads();
 
   TICK(7);
   // ---- D: backward sweep, stage by stage; E: forward substitution, stages reversed; V <- V'

@@ -88,7 +88,12 @@ struct GroupDesc {       // 64 bytes
   int64_t gen_base;      // double index into the gen pool
   int64_t class_off;     // byte offset of the ClassRecord in the topo pool
   int64_t cell_base;     // internal index of the group's first cell
-  uint32_t n_cv, n_cell, n_hh_rows, n_syn_rows, n_cl_rows, n_seg;
+  uint32_t n_cv, n_cell, n_hh_rows, n_syn_rows, n_cl_rows;
+  uint32_t flags;        // GROUP_*
+};
+enum : uint32_t {
+  GROUP_POINT_DISJOINT = 1u   // no two kinds of point mechanism (HH, synapse, clamp) of a cell share a control
+                              // volume: their currents can be subtracted without barriers in between
 };
 static_assert(sizeof(GroupDesc) == 64, "GroupDesc must be 64 bytes");
 

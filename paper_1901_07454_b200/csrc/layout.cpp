@@ -575,7 +575,7 @@ void build_class(const int32_t* par, uint32_t n, ClassInfo& K) {
   sched[spos] = (uint16_t)opos;
 }
 
-struct GroupCounts { uint32_t cls = 0, n_cell = 0, n_hh_rows = 0, n_syn_rows = 0, n_cl_rows = 0; int64_t cell_begin = 0, hh_base = 0; };
+struct GroupCounts { uint32_t cls = 0, n_cell = 0, n_hh_rows = 0, n_syn_rows = 0, n_cl_rows = 0; int64_t cell_begin = 0, hh_base = 0; bool disjoint = false; };
 
 }  // namespace
 
@@ -724,8 +724,21 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
   // groups: row counts, then placement (groups first in every pool)
   parallel_for(H.n_groups, [&](int64_t g) {
     GroupCounts& G = groups[g];
+    G.disjoint = true;
+    std::vector<uint8_t> kind;
     for (uint32_t lc = 0; lc < G.n_cell; ++lc) {
       const uint32_t c = group_cells[G.cell_begin + lc];
+      {                                   // does any control volume of the cell carry two kinds of point mechanism?
+        const int64_t a0 = d.cv_off[c];
+        kind.assign((size_t)(d.cv_off[c + 1] - a0), 0);
+        if (d.hh_gnabar)
+          for (size_t i = 0; i < kind.size(); ++i)
+            if (d.hh_gnabar[a0 + i] != 0.0 || d.hh_gkbar[a0 + i] != 0.0 || d.hh_gl[a0 + i] != 0.0) kind[i] |= 1;
+        if (d.syn_off)
+          for (int64_t q = d.syn_off[c]; q < d.syn_off[c + 1]; ++q) kind[d.syn_cv[q]] |= 2;
+        for (int64_t q = clamp_off[c]; q < clamp_off[c + 1]; ++q) kind[d.clamp_cv[clamp_idx[q]]] |= 4;
+        for (uint8_t k : kind) if (k & (k - 1)) G.disjoint = false;
+      }
       G.n_hh_rows = std::max(G.n_hh_rows, cell_hh[c]);
       if (d.syn_off) G.n_syn_rows = std::max(G.n_syn_rows, (uint32_t)(d.syn_off[c + 1] - d.syn_off[c]));
       G.n_cl_rows = std::max(G.n_cl_rows, (uint32_t)(clamp_off[c + 1] - clamp_off[c]));
@@ -744,7 +757,7 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     GroupCounts& G = groups[g];
     const ClassInfo& K = classes[G.cls];
     GroupDesc& D = H.gdescs[g];
-    D.n_cv = K.n_cv; D.n_cell = G.n_cell; D.n_hh_rows = G.n_hh_rows; D.n_syn_rows = G.n_syn_rows; D.n_cl_rows = G.n_cl_rows; D.n_seg = K.n_seg;
+    D.n_cv = K.n_cv; D.n_cell = G.n_cell; D.n_hh_rows = G.n_hh_rows; D.n_syn_rows = G.n_syn_rows; D.n_cl_rows = G.n_cl_rows; D.flags = G.disjoint ? GROUP_POINT_DISJOINT : 0u;
     D.class_off = K.topo_off;
     D.cell_base = G.cell_begin;
     const GConstOff co = gconst_offsets(K.n_cv, G.n_hh_rows, G.n_syn_rows, G.n_cl_rows, H.syn_uniform);
