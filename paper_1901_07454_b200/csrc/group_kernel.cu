@@ -352,28 +352,12 @@ __device__ __forceinline__ void run_deferred(HHDefer& dh, double* dst0, double* 
 template <bool kGen>
 __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U, double* Vs, const double* Fs, const double* Is,
                                               double* buf, const CellS& cs, double dt, HHDefer& dh, double vprev, double tstart,
-                                              long long* prof) {
+                                              const uint8_t* fg, uint32_t vbytes, uint64_t* mbarB, uint32_t& parB, long long* prof) {
   const int tid = threadIdx.x, c = tid % kG, h = tid / kG;
   const int rtid = kT - 1 - tid, rc = rtid % kG;      // reversed dealing of instances; cell of those
   const uint32_t nE_cv = gcv_elems(U.n_cv), nE_hh = U.n_hh * kG, nE_syn = U.n_syn * kG, nE_cl = U.n_cl * kG;
   const uint32_t md = kGen ? cs.mode[c] : 1u, rmd = kGen ? cs.mode[rc] : 1u;
   const double delta = kGen ? cs.delta[c] : dt, rdelta = kGen ? cs.delta[rc] : dt;
-
-  // ---- event-split sub-steps: this cell's matrix is re-eliminated for its own delta (reading R9); its
-  // column of the shared-memory factors is overwritten (the caller reloads them before they are needed again)
-  if (kGen) {
-    double* F = const_cast<double*>(Fs);
-    double* I = const_cast<double*>(Is);
-    for (uint32_t st = 0; st < U.n_stage; ++st) {
-      const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
-      if (md == 2u)
-        for (uint32_t q = beg; q < end; ++q) {
-          const uint32_t si = U.order[q];
-          eliminate_seg_smem(U, load_seg(U.segs + si), si, c, dt / cs.delta[c], F, I, buf);
-        }
-      __syncthreads();
-    }
-  }
 
   TICK(17);
   // ---- B: currents of HH, synapses and clamps from V(t); the passive current is
@@ -426,14 +410,10 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
 
   // ---- C: rhs_i = (C_i/delta - G_i) V_i + G_i e_i - I_i, in place of V; positions, not
   // (slot, cell) pairs: every per-CV array of the group uses the same positions
+  // (a, b sit in the two coefficient buffers, Fs and Is, until the rhs is formed)
   if (!kGen) {
-#if ARBB_CRESTRICT
-    const double* __restrict__ ag = U.a; const double* __restrict__ bgl = U.b; double* __restrict__ Vr = Vs;
-#else
-    const double* ag = U.a; const double* bgl = U.b; double* Vr = Vs;
-#endif
 #pragma unroll kCUnroll
-    for (uint32_t p = tid; p < nE_cv; p += kT) Vr[p] = fma(ag[p], Vr[p], bgl[p]);
+    for (uint32_t p = tid; p < nE_cv; p += kT) Vs[p] = fma(Fs[p], Vs[p], Is[p]);
   } else {
     // every position p = tid + j * kT a thread visits belongs to the same cell: kT is a multiple of
     // 128 positions, the period of the swizzle
@@ -441,12 +421,12 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
     const uint32_t pcell = gswz((uint32_t)tid) % kG, pmd = cs.mode[pcell];
     double* __restrict__ Vr = Vs;                            // no aliasing: the loads may run ahead of the stores
     if (pmd == 1u) {
-      const double* __restrict__ ar = U.a; const double* __restrict__ br = U.b;
+      const double* __restrict__ ar = Fs; const double* __restrict__ br = Is;
 #pragma unroll 4
       for (uint32_t p = tid; p < nE_cv; p += kT) Vr[p] = fma(ar[p], Vr[p], br[p]);
     } else if (pmd == 2u) {
       // (C/delta - G) V + G e  with  C/delta - G = a + (r - 1) C/dt  and  G e = b
-      const double* __restrict__ ar = U.a; const double* __restrict__ br = U.b; const double* __restrict__ C = U.C();
+      const double* __restrict__ ar = Fs; const double* __restrict__ br = Is; const double* __restrict__ C = U.C();
       const double rm1 = dt / cs.delta[pcell] - 1.0;
 #pragma unroll 4
       for (uint32_t p = tid; p < nE_cv; p += kT) Vr[p] = fma(fma(rm1, C[p] / dt, ar[p]), Vr[p], br[p]);
@@ -455,6 +435,14 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
   TICK(5);
   __syncthreads();
   TICK(6);
+  // a, b are dead: the same two buffers now receive the solver factors f, 1/d (L2, prefetched) while
+  // the point currents are subtracted
+  if (tid == 0) {
+    fence_proxy_async();
+    mbar_expect_tx(mbarB, 2u * vbytes);
+    bulk_g2s((void*)Fs, fg, vbytes, mbarB);
+    bulk_g2s((void*)Is, fg + vbytes, vbytes, mbarB);
+  }
   // HH, synapse and clamp currents of a cell may meet on a control volume: barriers in between, unless
   // the host found that they never do in this group
   const bool disjoint = (U.flags & GROUP_POINT_DISJOINT) != 0;
@@ -490,6 +478,24 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
   if (disjoint && (nE_hh | nE_syn | nE_cl)) __syncthreads();
 
   TICK(7);
+  mbar_wait(mbarB, parB);
+  parB ^= 1u;
+  // ---- event-split sub-steps: this cell's matrix is re-eliminated for its own delta (reading R9); its
+  // column of the shared-memory factors is overwritten (every (sub-)step copies them afresh)
+  if (kGen) {
+    double* F = const_cast<double*>(Fs);
+    double* I = const_cast<double*>(Is);
+    for (uint32_t st = 0; st < U.n_stage; ++st) {
+      const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
+      if (md == 2u)
+        for (uint32_t q = beg; q < end; ++q) {
+          const uint32_t si = U.order[q];
+          eliminate_seg_smem(U, load_seg(U.segs + si), si, c, dt / cs.delta[c], F, I, buf);
+        }
+      __syncthreads();
+    }
+  }
+
   // ---- D: backward sweep, stage by stage; E: forward substitution, stages reversed; V <- V'
   sweeps(U, h, c, kGen ? md != 0u : true, Fs, Is, Vs, buf, prof);   // buf: xI is dead, it now holds the contributions
   __syncthreads();
@@ -569,7 +575,7 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
   __syncthreads();
   unsigned n_sub = 0, n_del = 0;
   uint32_t it = 0, par2 = 0;
-  bool fi_dirty = false;                 // f, 1/d in shared memory differ from the group's record
+  bool ab_ready = false;                 // the coefficient buffers hold a, b (else f, 1/d of the last (sub-)step)
   int64_t cached_class = -1;
   HHDefer dh;
   clear(dh);
@@ -603,17 +609,29 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
     const GConstOff co = gconst_offsets(D.n_cv, D.n_hh_rows, D.n_syn_rows, D.n_cl_rows, M.syn_uniform != 0);
     const GStateOff so = gstate_offsets(D.n_cv, D.n_hh_rows, D.n_syn_rows);
     const uint32_t vbytes = 8u * gcv_elems(D.n_cv);
+    // a further (sub-)step of the same residency: a, b back into the coefficient buffers (L2)
+    auto reload_ab = [&]() {
+      if (tid == 0) {
+        const uint8_t* cb = M.fast + D.const_off;
+        fence_proxy_async();
+        mbar_expect_tx(mbar + 1, 2u * vbytes);
+        bulk_g2s((void*)Fs, cb + co.a, vbytes, mbar + 1);
+        bulk_g2s((void*)Is, cb + co.b, vbytes, mbar + 1);
+      }
+      mbar_wait(mbar + 1, par2);
+      par2 ^= 1u;
+    };
     if (tid == 0) {
-      // state record, f, 1/d and the const tail of the group -> shared memory (one barrier)
+      // state record, a, b and the const tail of the group -> shared memory (one barrier)
       const uint8_t* cb = M.fast + D.const_off;
       const uint32_t tbytes = co.total - co.hh_gna;
       fence_proxy_async();
       mbar_expect_tx(mbar, 8u * so.total + 2u * vbytes + tbytes);
       bulk_g2s(Ss, M.state + D.state_base, 8u * so.total, mbar);
-      bulk_g2s((void*)Fs, cb + co.f, vbytes, mbar);
-      bulk_g2s((void*)Is, cb + co.invd, vbytes, mbar);
+      bulk_g2s((void*)Fs, cb + co.a, vbytes, mbar);           // a, b first: the two coefficient buffers hold
+      bulk_g2s((void*)Is, cb + co.b, vbytes, mbar);           // them until the rhs is formed, then f, 1/d
       bulk_g2s((void*)tail, cb + co.hh_gna, tbytes, mbar);
-      if (M.l2_prefetch) bulk_prefetch_l2(cb + co.a, co.hh_gna - co.a);     // a, b of this group -> L2
+      if (M.l2_prefetch) bulk_prefetch_l2(cb + co.f, co.a - co.f);          // f, 1/d of this group -> L2
     } else if (tid >= 32 && tid < 64) {     // warp 1 claims the next group and fetches its descriptor
       unsigned long long gn = 0;
       if (tid == 32) gn = atomicAdd(&M.counters[CNT_GROUP0 + A.parity], 1ull);
@@ -629,7 +647,7 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
       cached_class = D.class_off;
       __syncthreads();
     }
-    fi_dirty = false;                    // fresh copies are on their way
+    ab_ready = true;                     // a, b are on their way into the coefficient buffers
     GView U;
     make_gview(U, M, D, Ss, tail, cls);
     // the previous group's last gate update: registers -> global m, h, n, while the copies are in flight
@@ -665,19 +683,9 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
       if (flags[0]) {
         if ((uint32_t)tid < U.n_cell) ++n_sub;
         run_deferred(dh, U.sm, U.gm, U.hh_ss);
-        if (fi_dirty) {                   // an event-split sub-step has overwritten columns of f, 1/d: reload
-          if (tid == 0) {
-            const uint8_t* cb = M.fast + D.const_off;
-            fence_proxy_async();
-            mbar_expect_tx(mbar + 1, 2u * vbytes);
-            bulk_g2s((void*)Fs, cb + co.f, vbytes, mbar + 1);
-            bulk_g2s((void*)Is, cb + co.invd, vbytes, mbar + 1);
-          }
-          mbar_wait(mbar + 1, par2);
-          par2 ^= 1u;
-          fi_dirty = false;
-        }
-        group_substep<false>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, vprev, ta, prof);
+        if (!ab_ready) reload_ab();
+        ab_ready = false;
+        group_substep<false>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, vprev, ta, M.fast + D.const_off + co.f, vbytes, mbar + 1, par2, prof);
         __syncthreads();                  // flags are rewritten by the next grid step
         continue;
       }
@@ -721,29 +729,18 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
         if (!flags[0]) break;
         // another (sub-)step follows: the gates of the previous one are needed now (working copy and global)
         run_deferred(dh, U.sm, U.gm, U.hh_ss);
-        if (fi_dirty) {                   // an event-split sub-step has overwritten columns of f, 1/d: reload
-          if (tid == 0) {
-            const uint8_t* cb = M.fast + D.const_off;
-            fence_proxy_async();
-            mbar_expect_tx(mbar + 1, 2u * vbytes);
-            bulk_g2s((void*)Fs, cb + co.f, vbytes, mbar + 1);
-            bulk_g2s((void*)Is, cb + co.invd, vbytes, mbar + 1);
-          }
-          mbar_wait(mbar + 1, par2);
-          par2 ^= 1u;
-          fi_dirty = false;
-        }
+        if (!ab_ready) reload_ab();
+        ab_ready = false;
         {                                 // (all cells nominal only after events delivered exactly at the step start)
 #ifdef ARBB_PROFILE
           unsigned long long ga, gb;
           asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ga));
 #endif
-          group_substep<true>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, 0.0, 0.0, prof);
+          group_substep<true>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, 0.0, 0.0, M.fast + D.const_off + co.f, vbytes, mbar + 1, par2, prof);
 #ifdef ARBB_PROFILE
           asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gb));
           ++prof_ngen; prof_gen_ns += gb - ga;
 #endif
-          fi_dirty = flags[2] != 0;
         }
         __syncthreads();
       }
@@ -765,8 +762,7 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
       if (M.l2_prefetch && sG[(it + 1) & 1u] < M.n_groups) {   // next group's records -> L2
         const GroupDesc& Dn = sD[(it + 1) & 1u];
         const GConstOff con = gconst_offsets(Dn.n_cv, Dn.n_hh_rows, Dn.n_syn_rows, Dn.n_cl_rows, M.syn_uniform != 0);
-        bulk_prefetch_l2(M.fast + Dn.const_off, con.a);
-        bulk_prefetch_l2(M.fast + Dn.const_off + con.hh_gna, con.total - con.hh_gna);
+        bulk_prefetch_l2(M.fast + Dn.const_off + con.a, con.total - con.a);      // a, b and the tables
         bulk_prefetch_l2(M.state + Dn.state_base, 8u * gstate_offsets(Dn.n_cv, Dn.n_hh_rows, Dn.n_syn_rows).total);
       }
       bulk_wait_read0();
