@@ -1,14 +1,15 @@
 // group_kernel.cu - the cable step for cell groups (group_layout.h): cells of one topology class,
 // stored cell-interleaved, lane = cell.
 //
-//   cable_group_kernel   persistent grid, one CTA integrates one group at a time, several CTAs per SM.
-//                        Everything a group-step touches more than once lives in shared memory and
-//                        arrives there by bulk-async copies (TMA, cp.async.bulk + one mbarrier): the
-//                        state record (V, synaptic g, per-cell runtime, gates), the solver factors f
-//                        and 1/d, and the tail of the const record (instance tables).  The rhs
-//                        coefficients a, b are used once and stream from L2 (pulled there ahead of
-//                        time by a TMA L2 prefetch) into registers.  V, g and the runtime leave by one
-//                        bulk store.  The class record (segments, stages) is kept in shared memory.
+//   cable_group_kernel   persistent grid, one CTA integrates one group at a time, several CTAs per SM;
+//                        groups are claimed from a work counter.  Everything a group-step touches lives
+//                        in shared memory and arrives there by bulk-async copies (TMA, cp.async.bulk +
+//                        mbarrier): the state record (V, synaptic g, per-cell runtime, gates), the tail
+//                        of the const record (instance tables) and, in two coefficient buffers, first the
+//                        rhs coefficients a, b and then - once the rhs is formed - the solver factors f,
+//                        1/d (second pair of copies, from L2, where a TMA prefetch has put them).  V, g
+//                        and the runtime leave by one bulk store.  The class record (segments, stages)
+//                        is kept in shared memory.  The nominal step has no global loads.
 //                        Per grid step (or fused run of steps): event delivery ->
 //                        mechanism currents (eq 2a) -> rhs of the implicit Euler system
 //                         -> Hines / branched Thomas sweeps: the class
@@ -34,9 +35,6 @@ namespace {
 
 #ifndef ARBB_CUNROLL
 #define ARBB_CUNROLL 4
-#endif
-#ifndef ARBB_CRESTRICT
-#define ARBB_CRESTRICT 0
 #endif
 constexpr int kT = kGroupThreads;
 constexpr int kCUnroll = ARBB_CUNROLL;    // unrolling of the rhs loop (phase C)

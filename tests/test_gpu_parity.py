@@ -242,6 +242,38 @@ def test_wide_star_and_deep_comb(B, orc):
     lockstep(B, orc, _simple(np.array(par, np.int32), clamp_cell=[0], clamp_cv=[3], clamp_t0=[0.0], clamp_t1=[9.0], clamp_amp=[0.2]), 40)
 
 
+def test_two_topology_classes_with_partial_groups(B, orc):
+    """Two tree shapes, 6 and 7 cells each: every class has a full cell group and a partly filled one
+    (padding lanes), the cells differ in geometry, synapses sit on shared and on branch-point CVs, and
+    a clamp shares the soma with the HH mechanism (the point currents meet on one control volume)."""
+    rng = np.random.default_rng(77)
+    par_a = np.array([-1, 0, 1, 2, 2, 4, 3, 6, 6, 5], np.int32)             # two forks
+    par_b = np.array([-1, 0, 0, 0, 1, 4, 5, 2, 7, 3, 9, 10], np.int32)       # three-way fork at the soma
+    cells = [par_a] * 6 + [par_b] * 7
+    off = np.concatenate([[0], np.cumsum([len(p_) for p_ in cells])])
+    n_cv, n_cells = int(off[-1]), len(cells)
+    hh = np.zeros(n_cv)
+    hh[off[:-1]] = 1
+    hh[off[:-1] + 4] = 1                                                     # a second HH CV per cell
+    n_syn = 6
+    syn_cv = np.concatenate([np.array([0, 0, 2, 4, 4, len(p_) - 1], np.int32) for p_ in cells])
+    m = dict(n_cells=n_cells, cv_off=off, cv_parent=np.concatenate(cells),
+             cv_area=rng.uniform(60.0, 200.0, n_cv), cv_cm=np.full(n_cv, 1.0), cv_raxial=rng.uniform(2.0, 8.0, n_cv),
+             hh_gnabar=hh * W.GNABAR, hh_gkbar=hh * W.GKBAR, hh_gl=hh * W.GL,
+             pas_g=np.where(hh > 0, 0.0, 2e-4), pas_e=np.full(n_cv, -65.0),
+             syn_off=np.arange(n_cells + 1) * n_syn, syn_cv=syn_cv, syn_tau=np.full(n_cells * n_syn, 2.0),
+             syn_e=np.zeros(n_cells * n_syn),
+             clamp_cell=[0, 7, 12], clamp_cv=[0, 0, 4], clamp_t0=[0.5, 1.0, 0.0], clamp_t1=[6.0, 7.0, 9.0],
+             clamp_amp=[0.3, 0.25, 0.2],
+             ext_cell=rng.integers(0, n_cells, 60), ext_syn=rng.integers(0, n_syn, 60),
+             ext_time=np.round(rng.uniform(0.0, 9.0, 60), 2) + rng.choice([0.0, 0.0031], 60),
+             ext_weight=rng.uniform(0.001, 0.02, 60),
+             conn_src=np.arange(n_cells), conn_dst=(np.arange(n_cells) + 1) % n_cells,
+             conn_syn=np.zeros(n_cells, np.int32), conn_delay=np.full(n_cells, 1.0), conn_weight=np.full(n_cells, 0.02),
+             t_end=10.0)
+    lockstep(B, orc, W.finalize(m), 400)
+
+
 def test_no_synapses_no_network(B, orc):
     m = W.random_model(11, n_cells=4, max_syn=0, n_conn=0, n_ext=0, t_end=5.0)
     assert m["n_syn"] == 0
