@@ -853,7 +853,11 @@ __global__ void __launch_bounds__(kGroupThreads) group_init_kernel(DevModel M) {
 // runtime; also opts the kernel into that much shared memory).  0: does not fit / no device.
 int group_ctas_per_sm(uint32_t smem_bytes) {
   if (smem_bytes + 1024u > 227u * 1024u) return 0;
-  if (cudaFuncSetAttribute(cable_group_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes) != cudaSuccess) return 0;
+  static uint32_t opted_in = 0;           // the attribute is per kernel, not per model: never lower it
+  if (smem_bytes > opted_in) {
+    if (cudaFuncSetAttribute(cable_group_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes) != cudaSuccess) return 0;
+    opted_in = smem_bytes;
+  }
   cudaFuncSetAttribute(cable_group_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
   int n = 0;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, cable_group_kernel, kGroupThreads, smem_bytes) != cudaSuccess) return 0;

@@ -274,6 +274,23 @@ def test_two_topology_classes_with_partial_groups(B, orc):
     lockstep(B, orc, W.finalize(m), 400)
 
 
+def test_two_models_alive_at_once(B, orc):
+    """Two models with different shared-memory footprints, created one after the other and advanced
+    alternately in both launch granularities: nothing in the library is per-process state."""
+    ma = W.config3(n_cells=40, t_end=12.0)
+    ma["ext_weight"] = ma["ext_weight"] * 4
+    mb = W.config1(n_cells=12, t_end=12.0)
+    ga, gb = B.Model(ma), B.Model(mb)
+    ga.set_option(B.ARB_OPT_FUSED_STEPS, 1)
+    oa, ob = orc.Oracle(ma), orc.Oracle(mb)
+    for t in (3.0, 6.5, 12.0):
+        ga.advance(t, DT), gb.advance(t, DT)
+        oa.advance(t, DT), ob.advance(t, DT)
+    assert rel(ga.voltage(), oa.voltage()) < 1e-6 and rel(gb.voltage(), ob.voltage()) < 1e-6
+    check_spikes(ga, oa, 40), check_spikes(gb, ob, 12)
+    ga.close(), gb.close()
+
+
 def test_no_synapses_no_network(B, orc):
     m = W.random_model(11, n_cells=4, max_syn=0, n_conn=0, n_ext=0, t_end=5.0)
     assert m["n_syn"] == 0
