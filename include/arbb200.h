@@ -56,6 +56,9 @@ enum {
                                 every launch streams the state once, 1 when launches are fused     */
   ARB_OPT_L2_PREFETCH = 5,   /* cell-group kernel: 1 (default) = ask the TMA unit to pull the next group's
                                 records into L2 while the current group is integrated; 0 = off      */
+  ARB_OPT_HOT_FIRST = 7,     /* cell-group kernel, one launch per grid step: 1 (default) = groups with an event in
+                                the coming step are integrated first (their event-split steps take longer and
+                                would otherwise end up at the tail of the launch); 0 = index order          */
   ARB_OPT_GROUP_CTAS = 6,    /* cell-group kernel: cap on the CTAs of a launch (0 = as many as are resident) */
   ARB_OPT_TIMING = 3         /* 1: bracket the cable-step launches and the epoch-boundary kernels of
                                 every epoch with CUDA events on the model's stream (read them with

@@ -32,7 +32,7 @@ struct Carver {
 };
 
 struct Regions {
-  Region units, gdescs, gen, fast, state, topo, scratch, warp_scratch, factor_dcontrib, cell_rt_idx, cell_orig, ev_off, ev_t, ev_gidx, ev_w, ev_fill,
+  Region units, gdescs, ghot, ghotflag, gen, fast, state, topo, scratch, warp_scratch, factor_dcontrib, cell_rt_idx, cell_orig, ev_off, ev_t, ev_gidx, ev_w, ev_fill,
       ext_off, ext_t, ext_gidx, ext_w, ext_cur, conn_off, conn_dst, conn_gidx, conn_delay, conn_w,
       pool_t[2], pool_dst[2], pool_gidx[2], pool_w[2], spike_cell, spike_t, counters, scan_tmp,
       cv_idx, syn_idx, hh_m_idx, hh_stride, hh_cv, io;
@@ -74,6 +74,8 @@ Regions carve(const HostModel& H, const Caps& cap) {
   const size_t nc = (size_t)H.n_cells;
   R.units = C.take(sizeof(UnitDesc) * (size_t)H.n_units);
   R.gdescs = C.take(sizeof(GroupDesc) * (size_t)H.n_groups);
+  R.ghot = C.take(4 * 3 * (size_t)H.n_groups);
+  R.ghotflag = C.take(4 * (size_t)H.n_groups);
   R.gen = C.take(8 * (size_t)H.gen_doubles);
   R.fast = C.take((size_t)H.fast_bytes);
   R.state = C.take(8 * (size_t)H.state_doubles);
@@ -136,7 +138,8 @@ struct arb_model {
   int cur_pool = 0;
   int sm_count = 148;
   int group_grid = 0, last_ggrid = 0;
-  int64_t group_launches = 0, opt_group_ctas = 0;
+  int64_t group_launches = 0, opt_group_ctas = 0, opt_hot = 1;
+  bool prev_marked_hot = false;
   int64_t group_slots = 0, group_streamed = 0;   // statistics: CV slots incl. padding, bytes one grid step streams
   int64_t opt_stages = 0;
   bool broken = false;
@@ -276,6 +279,7 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     }
     D.gplan = group_smem_plan(H.gcaps);
     D.l2_prefetch = 1;
+    D.ghot = at<uint32_t>(m, R.ghot); D.ghotflag = at<uint32_t>(m, R.ghotflag);   // zeroed with the workspace
     if (H.n_groups > 0)
       m->group_grid = (int)std::min<int64_t>(group_cta_cap(H), (int64_t)m->sm_count * group_ctas);
     D.pool_cap = m->cap.pool;
@@ -381,7 +385,11 @@ int arb_advance(arb_model* m, double t_end, double dt) {
     for (int64_t j = 0; j < n_ep; j += fused) {
       StepArgs A;
       A.t0 = t0; A.dt = dt; A.t_end = t_end; A.k_first = k + j; A.nk = std::min(fused, n_ep - j); A.nsteps = nsteps; A.last_full = last_full;
-      A.parity = (int)(m->group_launches++ & 1);
+      A.parity = (int)(m->group_launches & 1);
+      A.launch_id = (uint32_t)m->group_launches++;
+      A.mark_hot = (A.nk == 1 && m->opt_hot) ? 1 : 0;
+      A.hot_valid = m->prev_marked_hot ? 1 : 0;
+      m->prev_marked_hot = A.mark_hot != 0;
       CU(m, launch_group_cable(D, A, ggrid, m->stream, &launches));
       CU(m, launch_cable(D, A, grid, m->stream, &launches));
     }
@@ -542,6 +550,7 @@ int arb_set_option(arb_model* m, int key, int64_t value) {
     case ARB_OPT_STAGES: m->opt_stages = value; return ARB_OK;
     case ARB_OPT_L2_PREFETCH: m->D.l2_prefetch = value != 0; return ARB_OK;
     case ARB_OPT_GROUP_CTAS: m->opt_group_ctas = value; return ARB_OK;
+    case ARB_OPT_HOT_FIRST: m->opt_hot = value != 0; m->prev_marked_hot = false; return ARB_OK;
     case ARB_OPT_TIMING:
       m->opt_timing = value;
       m->cable_ms = m->event_ms = 0; m->cable_timed = m->event_timed = 0;

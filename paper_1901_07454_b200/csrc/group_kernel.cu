@@ -550,6 +550,17 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
   TICK(12);
 }
 
+// Work item -> group.  Items [0, n_hot) are the groups of this launch's hot list (an event falls into
+// the coming grid step: their event-split steps take longer, so they go first); items n_hot + g are
+// the groups in index order, minus the hot ones.  Returns n_groups past the end, -1 for "skip".
+__device__ __forceinline__ int64_t map_item(const DevModel& M, const StepArgs& A, uint32_t n_hot, unsigned long long i) {
+  if (i < n_hot) return (int64_t)M.ghot[(size_t)(A.launch_id % 3u) * (size_t)M.n_groups + i];
+  const int64_t g = (int64_t)(i - n_hot);
+  if (g >= M.n_groups) return M.n_groups;
+  if (n_hot != 0 && M.ghotflag[g] == A.launch_id) return -1;
+  return g;
+}
+
 // ------------------------------------------------------------------------------------------
 // The cable step for cell groups.
 // ------------------------------------------------------------------------------------------
@@ -569,7 +580,24 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
   uint64_t* mbar = (uint64_t*)(smem + P.off_mbar);
   const int tid = threadIdx.x;
   if (tid == 0) { mbar_init(mbar, 1); mbar_init(mbar + 1, 1); fence_mbar_init(); }
-  if (tid < 16 && blockIdx.x < M.n_groups) ((uint32_t*)&sD[0])[tid] = ((const uint32_t*)&M.groups[blockIdx.x])[tid];
+  __shared__ int64_t sG[2];
+  __shared__ uint32_t sNHot;
+  if (tid == 0) {
+    // Groups are claimed dynamically (group-steps differ in length): item blockIdx.x first, further
+    // items from this launch's work counter, which the previous launch has reset to gridDim.x; this
+    // launch resets the other one and clears the hot list after the next
+    const uint32_t n_hot = A.hot_valid ? (uint32_t)M.counters[CNT_HOT0 + A.launch_id % 3u] : 0u;
+    sNHot = n_hot;
+    if (blockIdx.x == 0) {
+      M.counters[CNT_GROUP0 + (A.parity ^ 1)] = gridDim.x;
+      M.counters[CNT_HOT0 + (A.launch_id + 2u) % 3u] = 0ull;
+    }
+    int64_t g0 = map_item(M, A, n_hot, blockIdx.x);
+    while (g0 < 0) g0 = map_item(M, A, n_hot, atomicAdd(&M.counters[CNT_GROUP0 + A.parity], 1ull));
+    sG[0] = g0;
+  }
+  __syncthreads();
+  if (tid < 16 && sG[0] < M.n_groups) ((uint32_t*)&sD[0])[tid] = ((const uint32_t*)&M.groups[sG[0]])[tid];
   __syncthreads();
   unsigned n_sub = 0, n_del = 0;
   uint32_t it = 0, par2 = 0;
@@ -588,15 +616,6 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
   unsigned long long prof_gen_ns = 0;
 #endif
   long long* prof = nullptr;
-  // Groups are claimed dynamically (group-steps differ in length: event-split sub-steps, memory
-  // placement): the first one is blockIdx.x, further ones come from this launch's work counter, which
-  // the previous launch has reset to gridDim.x; this launch resets the other one.
-  __shared__ int64_t sG[2];
-  if (tid == 0) {
-    sG[0] = blockIdx.x;
-    if (blockIdx.x == 0) M.counters[CNT_GROUP0 + (A.parity ^ 1)] = gridDim.x;
-  }
-  __syncthreads();
   for (int64_t g = sG[0]; g < M.n_groups; g = sG[(++it) & 1u]) {
 #ifdef ARBB_PROFILE
     prof = (blockIdx.x == 7 && tid == 0 && it >= 1 && it <= 3 && A.k_first == 150) ? prof_buf : nullptr;
@@ -631,11 +650,13 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
       bulk_g2s((void*)tail, cb + co.hh_gna, tbytes, mbar);
       if (M.l2_prefetch) bulk_prefetch_l2(cb + co.f, co.a - co.f);          // f, 1/d of this group -> L2
     } else if (tid >= 32 && tid < 64) {     // warp 1 claims the next group and fetches its descriptor
-      unsigned long long gn = 0;
-      if (tid == 32) gn = atomicAdd(&M.counters[CNT_GROUP0 + A.parity], 1ull);
+      long long gn = 0;
+      if (tid == 32) {
+        do gn = map_item(M, A, sNHot, atomicAdd(&M.counters[CNT_GROUP0 + A.parity], 1ull)); while (gn < 0);
+        sG[(it + 1) & 1u] = gn;
+      }
       gn = __shfl_sync(kFull, gn, 0);
-      if (tid == 32) sG[(it + 1) & 1u] = (int64_t)gn;
-      if (tid < 48 && (int64_t)gn < M.n_groups) ((uint32_t*)&sD[(it + 1) & 1u])[tid - 32] = ((const uint32_t*)&M.groups[gn])[tid - 32];
+      if (tid < 48 && gn < M.n_groups) ((uint32_t*)&sD[(it + 1) & 1u])[tid - 32] = ((const uint32_t*)&M.groups[gn])[tid - 32];
     }
     if (D.class_off != cached_class) {   // tree structure differs from the previous group's
       const ClassRecord* R = (const ClassRecord*)(M.topo + D.class_off);
@@ -751,6 +772,16 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
       const unsigned long long pk = ((unsigned long long)cs.evend[tid] << 32) | cs.evcur[tid];
       U.srt[kRtDoubles * tid + 1] = __longlong_as_double((long long)pk);
       U.srt[kRtDoubles * tid + 2] = cs.armed[tid] ? 1.0 : 0.0;
+    }
+    if (A.mark_hot && tid < 32) {         // does an event of this group fall into the next grid step?
+      const double t_hot = A.t0 + (double)(A.k_first + A.nk + 1) * A.dt;
+      const bool hot = (uint32_t)tid < U.n_cell && U.srt[kRtDoubles * (tid < kG ? tid : 0)] < t_hot;
+      if (__any_sync(kFull, hot) && tid == 0) {
+        const uint32_t nxt = A.launch_id + 1u;
+        const unsigned long long pos = atomicAdd(&M.counters[CNT_HOT0 + nxt % 3u], 1ull);
+        M.ghot[(size_t)(nxt % 3u) * (size_t)M.n_groups + pos] = (uint32_t)g;
+        M.ghotflag[g] = nxt;
+      }
     }
     fence_proxy_async();
     __syncthreads();

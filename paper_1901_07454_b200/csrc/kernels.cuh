@@ -19,7 +19,10 @@ enum Counter {
   CNT_EVLIST = 7,       // size of the current epoch list
   CNT_GROUP0 = 8,       // group kernel: next unclaimed group of even / odd launches (dynamic
   CNT_GROUP1 = 9,       //   distribution of groups over the persistent CTAs)
-  CNT_COUNT = 10
+  CNT_HOT0 = 10,        // group kernel: lengths of the three rotating "hot" lists (groups with an event in
+  CNT_HOT1 = 11,        //   the next grid step, which are integrated first so that their longer
+  CNT_HOT2 = 12,        //   event-split steps do not end up at the tail of the launch)
+  CNT_COUNT = 13
 };
 
 struct EventPool { double* t; uint32_t* dst; uint32_t* gidx; double* w; };
@@ -64,6 +67,8 @@ struct DevModel {
   int64_t n_groups;
   GroupSmemPlan gplan;
   int l2_prefetch;            // group kernel: TMA-prefetch the next group's records into L2
+  uint32_t* ghot;             // group kernel: three lists of n_groups entries (see CNT_HOT0)
+  uint32_t* ghotflag;         // [n_groups] launch_id of the launch whose hot list holds the group
 };
 
 struct StepArgs {
@@ -71,6 +76,9 @@ struct StepArgs {
   int64_t k_first, nk, nsteps;
   int last_full;         // the last grid step has nominal length dt
   int parity;            // launch counter & 1 (group kernel: which work counter this launch claims from)
+  uint32_t launch_id;    // group kernel: running number of the launch
+  int hot_valid;         // the hot list of this launch was written by the launch before it
+  int mark_hot;          // write the hot list of the next launch
 };
 
 // all launchers queue work on `s` and return the last CUDA error code

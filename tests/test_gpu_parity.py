@@ -187,6 +187,31 @@ def test_large_config_cut_spikes(B, orc):
     g.close()
 
 
+def test_stream_mode_hot_groups_first(B, orc):
+    """One launch per grid step (state through HBM every step).  Groups with an event in the coming
+    step are integrated first (ARB_OPT_HOT_FIRST); the order in which groups are integrated must not
+    change a bit, and the run must match the oracle."""
+    m = W.config3(n_cells=200, t_end=30.0)
+    m["conn_weight"] = m["conn_weight"] * 4
+    m["ext_weight"] = m["ext_weight"] * 4
+    o = orc.Oracle(m, threads=4)
+    o.advance(30.0, m["dt"])
+    res = []
+    for hot in (1, 0):
+        g = B.Model(m)
+        g.set_option(B.ARB_OPT_FUSED_STEPS, 1)
+        g.set_option(B.ARB_OPT_HOT_FIRST, hot)
+        for t in (7.5, 30.0):
+            g.advance(t, m["dt"])
+        assert check_spikes(g, o, 200) > 20
+        assert rel(g.voltage(), o.voltage()) < 1e-6
+        assert tuple(g.probe(B.ARB_PROBE_NSTEPS)) == tuple(o.probe(orc.PROBE_NSTEPS))
+        res.append(state_of(g) + g.spikes())
+        g.close()
+    for a, b in zip(*res):
+        assert np.array_equal(a, b)
+
+
 def test_heterogeneous_cut_spikes(B, orc):
     m = W.config4(n_cells=120, t_end=60.0)
     g, o = run_both(B, orc, m, 60.0)
