@@ -75,7 +75,7 @@ Regions carve(const HostModel& H, const Caps& cap) {
   R.units = C.take(sizeof(UnitDesc) * (size_t)H.n_units);
   R.gdescs = C.take(sizeof(GroupDesc) * (size_t)H.n_groups);
   R.ghot = C.take(4 * 3 * (size_t)H.n_groups);
-  R.ghotflag = C.take(4 * (size_t)H.n_groups);
+  R.ghotflag = C.take(4 * 2 * (size_t)H.n_groups);
   R.gen = C.take(8 * (size_t)H.gen_doubles);
   R.fast = C.take((size_t)H.fast_bytes);
   R.state = C.take(8 * (size_t)H.state_doubles);

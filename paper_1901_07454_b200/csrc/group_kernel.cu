@@ -557,7 +557,7 @@ __device__ __forceinline__ int64_t map_item(const DevModel& M, const StepArgs& A
   if (i < n_hot) return (int64_t)M.ghot[(size_t)(A.launch_id % 3u) * (size_t)M.n_groups + i];
   const int64_t g = (int64_t)(i - n_hot);
   if (g >= M.n_groups) return M.n_groups;
-  if (n_hot != 0 && M.ghotflag[g] == A.launch_id) return -1;
+  if (n_hot != 0 && M.ghotflag[(size_t)(A.launch_id & 1u) * (size_t)M.n_groups + g] == A.launch_id) return -1;
   return g;
 }
 
@@ -780,7 +780,7 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
         const uint32_t nxt = A.launch_id + 1u;
         const unsigned long long pos = atomicAdd(&M.counters[CNT_HOT0 + nxt % 3u], 1ull);
         M.ghot[(size_t)(nxt % 3u) * (size_t)M.n_groups + pos] = (uint32_t)g;
-        M.ghotflag[g] = nxt;
+        M.ghotflag[(size_t)(nxt & 1u) * (size_t)M.n_groups + g] = nxt;   // (this launch may still look at the other half)
       }
     }
     fence_proxy_async();

@@ -68,7 +68,7 @@ struct DevModel {
   GroupSmemPlan gplan;
   int l2_prefetch;            // group kernel: TMA-prefetch the next group's records into L2
   uint32_t* ghot;             // group kernel: three lists of n_groups entries (see CNT_HOT0)
-  uint32_t* ghotflag;         // [n_groups] launch_id of the launch whose hot list holds the group
+  uint32_t* ghotflag;         // [2][n_groups], half launch_id & 1: launch_id of the launch whose hot list holds the group
 };
 
 struct StepArgs {
