@@ -653,6 +653,25 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     for (size_t k = 0; k < classes.size(); ++k) {
       ClassInfo& K = classes[k];
       K.grouped = K.cells.size() >= P.group_min_cells;
+      if (K.grouped) {
+        // a group's state record (V, synaptic g, gates), two coefficient buffers and instance tables
+        // must fit in shared memory - twice per SM at least; cells with very many point mechanisms
+        // (the paper's 10,000-synapse ring cell) are laid out as units instead
+        uint32_t mx_hh = 0, mx_syn = 0, mx_cl = 0;
+        for (uint32_t c : K.cells) {
+          mx_hh = std::max(mx_hh, cell_hh[c]);
+          if (d.syn_off) mx_syn = std::max(mx_syn, (uint32_t)std::min<int64_t>(d.syn_off[c + 1] - d.syn_off[c], 1 << 24));
+          mx_cl = std::max(mx_cl, (uint32_t)std::min<int64_t>(clamp_off[c + 1] - clamp_off[c], 1 << 24));
+        }
+        const GConstOff co = gconst_offsets(K.n_cv, mx_hh, mx_syn, mx_cl, H.syn_uniform);
+        GroupCaps caps;
+        caps.slot_cap = K.n_cv;
+        caps.state_bytes = 8 * gstate_offsets(K.n_cv, mx_hh, mx_syn).total;
+        caps.tail_bytes = co.total - co.hh_gna;
+        caps.class_bytes = 64 + 40 * K.n_cv;               // upper bound: one segment per control volume
+        caps.buf_rows = std::max(K.n_cv, mx_hh + mx_syn + mx_cl);
+        if (group_smem_plan(caps).bytes > P.group_max_smem) K.grouped = false;
+      }
       if (!K.grouped) continue;
       for (size_t i = 0; i < K.cells.size(); i += kG) {
         GroupCounts G;

@@ -345,6 +345,44 @@ def config4(n_cells=50000, t_end=200.0):
     return finalize(m)
 
 
+def paper_ring(n_cells=1024, n_syn=10000, t_end=200.0, weight=0.05, kick_weight=0.1):
+    """The paper's own single-node benchmark cell: random
+    morphologies of ~130 control volumes (here: a binary tree of 7 branches with U{12..24} CVs each),
+    HH soma, passive dendrites, `n_syn` exponential synapses per cell at random control volumes of
+    which ONE is wired: cell i -> cell i+1 (synapse 0, delay 5 ms); cell 0 is kicked at t = 1 ms.
+    Synapse-dominated: ~10,000 synapse instances against ~130 control volumes per cell."""
+    seed = BASE_SEED + 5
+    bp = _binary_tree(7)
+    parents, areas, raxs, syns, offs = [], [], [], [], [0]
+    for c in range(n_cells):
+        rng = np.random.default_rng([seed, c])
+        ncvb = rng.integers(12, 25, 7)
+        L = rng.uniform(100.0, 300.0, 7)
+        D = rng.uniform(0.5, 2.0, 7)
+        parent, area, rax, _ = cell_cvs(bp, ncvb, L, D)
+        n = len(parent)
+        s = rng.integers(0, n, n_syn).astype(np.int32)
+        s[0] = 0                                            # the wired synapse sits on the soma
+        parents.append(parent), areas.append(area), raxs.append(rax), syns.append(s)
+        offs.append(offs[-1] + n)
+    n_cv = offs[-1]
+    soma = np.asarray(offs[:-1], np.int64)
+    hh = np.zeros(n_cv)
+    hh[soma] = 1.0
+    m = dict(n_cells=n_cells, cv_off=offs, cv_parent=np.concatenate(parents), cv_area=np.concatenate(areas),
+             cv_cm=np.full(n_cv, CM), cv_raxial=np.concatenate(raxs),
+             hh_gnabar=hh * GNABAR, hh_gkbar=hh * GKBAR, hh_gl=hh * GL,
+             pas_g=np.where(hh > 0, 0.0, G_PAS), pas_e=np.full(n_cv, E_PAS),
+             syn_off=np.arange(n_cells + 1, dtype=np.int64) * n_syn, syn_cv=np.concatenate(syns),
+             syn_tau=np.full(n_cells * n_syn, SYN_TAU), syn_e=np.full(n_cells * n_syn, SYN_E),
+             conn_src=np.arange(n_cells), conn_dst=(np.arange(n_cells) + 1) % n_cells,
+             conn_syn=np.zeros(n_cells, np.int32), conn_delay=np.full(n_cells, 5.0),
+             conn_weight=np.full(n_cells, weight),
+             ext_cell=[0], ext_syn=[0], ext_time=[1.0], ext_weight=[kick_weight],
+             t_end=t_end, name="paper ring %d x %d synapses" % (n_cells, n_syn))
+    return finalize(m)
+
+
 def config(k, **kw):
     return (config0, config1, config2, config3, config4)[k](**kw)
 

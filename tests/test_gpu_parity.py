@@ -212,6 +212,25 @@ def test_stream_mode_hot_groups_first(B, orc):
         assert np.array_equal(a, b)
 
 
+def test_paper_ring_cell_many_synapses(B, orc):
+    """SURVEY.md 8(f) NEXT-1, first cut: the paper's ring cell (~130 CVs, 10,000 exponential synapses
+    each, one of them wired).  Functional parity only: such cells run on the block-unit
+    kernel; a kernel designed for the synapse-dominated case is the next step."""
+    m = W.paper_ring(n_cells=6, n_syn=10000, t_end=30.0)
+    # a few hundred extra events so that more than one synapse per cell carries conductance
+    rng = np.random.default_rng(5)
+    m["ext_cell"] = np.concatenate([m["ext_cell"], rng.integers(0, 6, 300)])
+    m["ext_syn"] = np.concatenate([m["ext_syn"], rng.integers(0, 10000, 300).astype(np.int32)])
+    m["ext_time"] = np.concatenate([m["ext_time"], rng.uniform(0.0, 25.0, 300)])
+    m["ext_weight"] = np.concatenate([m["ext_weight"], rng.uniform(0.0005, 0.004, 300)])
+    m = W.finalize(m)
+    g, o = run_both(B, orc, m, 30.0)
+    assert check_spikes(g, o, 6) >= 4
+    assert rel(g.voltage(), o.voltage()) < 1e-6
+    assert rel_pure(g.syn_g(), o.syn_g()) < 1e-9
+    g.close()
+
+
 def test_heterogeneous_cut_spikes(B, orc):
     m = W.config4(n_cells=120, t_end=60.0)
     g, o = run_both(B, orc, m, 60.0)
