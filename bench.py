@@ -174,10 +174,10 @@ def oracle_sample(n_cells_sample, first_cell=0):
     return W.take_cells(m, np.arange(n_cells_sample))
 
 
-def time_oracle(sample_cells, steps, warmup):
+def time_oracle(sample_cells, steps, warmup, threads=None):
     from oracle import orc
     orc.build()
-    cores = os.cpu_count() or 1
+    cores = threads or os.cpu_count() or 1
     sub = oracle_sample(sample_cells)
     o = orc.Oracle(sub, threads=cores)
     t = 0.0
@@ -193,7 +193,8 @@ def time_oracle(sample_cells, steps, warmup):
     per_step = float(np.mean(times))
     return dict(value=sub["n_cv"] * STEPS_PER_EPOCH / per_step, ms_per_step=per_step * 1e3, cores=cores,
                 sample="first %d cells of C3 (%d CVs, connections dropped, external events kept), "
-                       "%d epochs of 200 steps, OpenMP over cells" % (sample_cells, sub["n_cv"], steps))
+                       "%d epochs of 200 steps, %s" % (sample_cells, sub["n_cv"], steps,
+                                                       "OpenMP over cells" if cores > 1 else "one thread"))
 
 
 def run_reference(args):
@@ -260,7 +261,8 @@ def run_ours(args):
     t_now = 0.0
     _, t_now = timed_epochs(torch, g, t_now, args.warmup, sync_all)
     g.set_option(B.ARB_OPT_TIMING, 1)
-    l0 = g.stats()["launches"]
+    st0 = g.stats()
+    l0 = st0["launches"]
     sub0 = g.probe(B.ARB_PROBE_NSTEPS)
     spikes0 = int(B.lib().arb_spikes(g._h, None, None, 0))
     sampler = ClockSampler(local)
@@ -270,7 +272,9 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else None
     tim = g.timing()
     g.set_option(B.ARB_OPT_TIMING, 0)
-    launches = g.stats()["launches"] - l0
+    st1 = g.stats()
+    launches = st1["launches"] - l0
+    n_events = st1["events_delivered"] - st0["events_delivered"]
     sub1 = g.probe(B.ARB_PROBE_NSTEPS)
     n_spikes = int(B.lib().arb_spikes(g._h, None, None, 0)) - spikes0
     ms_all, units_all = reduce_over_ranks(ms, units_per_step * args.steps, world, dev)
@@ -357,6 +361,18 @@ def run_ours(args):
                 "avg_launch_ms": avg_launch_ms, "launches_timed": tim["cable_launches"],
                 "kernel_share_of_step": tim["cable_ms"] / ms if ms > 0 else None,
                 "epoch_boundary_ms_per_step": tim["event_ms"] / args.steps}
+    # secondary (arithmetic) bound: DP instructions of a launch (committed ncu count) over the
+    # fp64 rate measured live by the library's DFMA kernel
+    try:
+        dfma_rate, _ = B.arb_fp64_peak(torch.cuda.current_stream().cuda_stream)
+        dp_inst = committed_traffic("cable_group_kernel:%s:dp_inst" % args.mode)
+        roofline["fp64"] = {"peak_dfma_per_s": dfma_rate, "peak_source": "arb_fp64_peak (live DFMA microbenchmark)",
+                            "dp_inst_per_launch": dp_inst,
+                            "fp64_ms": (dp_inst / dfma_rate * 1e3) if dp_inst else None,
+                            "hbm_ms": alg / (peak * 1e9) * 1e3,
+                            "note": "roofline time = max(hbm_ms, fp64_ms): HBM-bound"}
+    except Exception as e:  # the figure is context; the HBM roofline above is the claim
+        roofline["fp64"] = {"error": str(e)}
     if args.mode == "fused":
         roofline["note"] = ("fused launches keep state on chip for 200 steps; algorithmic bytes are the level-A "
                             "per-step figure x 200, so frac > 1 means HBM traffic was avoided, not that work was skipped")
@@ -365,6 +381,8 @@ def run_ours(args):
     if not args.no_cpu_baseline:
         r = time_oracle(args.ref_cells, 2, 1)
         cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
+        r1 = time_oracle(max(1, args.ref_cells // 10), 1, 1, threads=1)   # SURVEY.md 8(d) oracle timing (i)
+        cpu["single_thread"] = {"value": r1["value"], "unit": UNIT, "cores": 1, "sample": r1["sample"]}
 
     line = {"metric": METRIC, "value": units_all / (ms_all * 1e-3), "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_all / args.steps,
@@ -379,6 +397,7 @@ def run_ours(args):
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roofline, "cpu_baseline": cpu,
             "spikes": n_spikes, "spikes_per_s": n_spikes / (ms * 1e-3),
+            "events_delivered": int(n_events), "events_per_s": n_events / (ms * 1e-3),
             "substep_overhead": float((sub1[1] - sub0[1]) / (m["n_cells"] * (sub1[0] - sub0[0])) - 1.0)}
     if other_res:
         line["fused_epoch" if other == "fused" else "stream"] = other_res

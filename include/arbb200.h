@@ -174,6 +174,13 @@ int arb_set_option(arb_model* m, int key, int64_t value);
 /* Process-wide build defaults (ARB_CFG_*); affects models planned / created afterwards. */
 int arb_configure(int key, int64_t value);
 
+/* Measures the fp64 fused-multiply-add rate of the current device (independent DFMA chains in
+ * registers, no memory traffic; kernel timed with CUDA events on `cuda_stream`, NULL = default
+ * stream): the peak of the arithmetic bound of the roofline ("Roofline time per
+ * step = max(bytes/BW, DP-instr/peak)").  *dfma_per_s receives DFMA instructions (thread level) per
+ * second, *ms (may be NULL) the duration of the timed launch.  Needs no model. */
+int arb_fp64_peak(void* cuda_stream, double* dfma_per_s, double* ms);
+
 void arb_destroy(arb_model* m);
 
 /* Text of the last error of this model, or of the last arb_plan / arb_create failure on this

@@ -67,6 +67,7 @@ def lib():
         L.arb_set_state.argtypes = [C.c_void_p] * 6
         L.arb_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
         L.arb_configure.argtypes = [C.c_int, C.c_int64]
+        L.arb_fp64_peak.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.arb_destroy.argtypes = [C.c_void_p]
         L.arb_destroy.restype = None
         L.arb_last_error.restype = C.c_char_p
@@ -97,6 +98,15 @@ def configure(key, value):
     rc = lib().arb_configure(int(key), int(value))
     if rc:
         raise ArbError(rc, lib().arb_last_error(None).decode())
+
+
+def arb_fp64_peak(stream=None):
+    """(DFMA per second, ms of the timed launch) of the current CUDA device; `stream` = a cudaStream_t handle."""
+    r, ms = C.c_double(0.0), C.c_double(0.0)
+    rc = lib().arb_fp64_peak(C.c_void_p(stream or 0), C.byref(r), C.byref(ms))
+    if rc:
+        raise ArbError(rc, "arb_fp64_peak failed")
+    return r.value, ms.value
 
 
 def arb_plan(m):

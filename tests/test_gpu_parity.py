@@ -437,3 +437,11 @@ def test_full_size_large_config_sampled_cells(B, orc, layout):
         assert np.array_equal(a, b)
     g2.close()
     g.close()
+
+
+def test_fp64_peak_measurement(B):
+    """arb_fp64_peak: the DFMA rate of the device lies between a tenth of and the nominal fp64 peak
+    (148 SMs x 64 DFMA/clk x < 2.2 GHz = 2.1e13, B200_PROFILING.md unit counts)."""
+    import torch
+    rate, ms = B.arb_fp64_peak(torch.cuda.current_stream().cuda_stream)
+    assert 2e12 < rate < 2.2e13 and ms > 0
