@@ -26,6 +26,7 @@ namespace {
 
 constexpr int kBlockThreads = 256;              // cable_block_kernel, factor_kernel, init_kernel
 constexpr int kBlockWarps = kBlockThreads / 32;
+constexpr uint32_t kSynKeyReduceMin = 1024;     // block units with at least this many synapses reduce currents by key
 constexpr int kMaxWarpsPerCta = 8;              // cable_warp_kernel
 
 // ------------------------------------------------------------------------------------------
@@ -311,6 +312,42 @@ __device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, co
     const double m = U.m[i], h = U.h[i], n = U.n[i];
     U.xI[i] = U.hh_gna[i] * m * m * m * h * (v - M.ena) + U.hh_gk[i] * n * n * n * n * (v - M.ek) + U.hh_gl[i] * (v - M.el);
   }
+  if (!kWarp && n_syn >= kSynKeyReduceMin) {
+    // Many synapses per control volume (the paper's ring cell): a run head summing its
+    // run alone would leave the other lanes idle.  Each warp takes 32 consecutive synapses (coalesced),
+    // reduces them by key = control volume with shuffles (the "key reduction" of PAPER.md:218; runs are
+    // contiguous), and the first lane of every key inside the chunk stores a partial sum; in phase C the run
+    // heads add the partials of the chunks their run extends into, in index order (no atomics).
+    constexpr int kCh = 4;               // chunks per warp and trip: independent loads in flight
+    for (uint32_t base = (uint32_t)S::warp() * 32u * kCh; base < n_syn; base += (uint32_t)S::warps * 32u * kCh) {
+      uint32_t slot[kCh];
+      double term[kCh];
+#pragma unroll
+      for (int q = 0; q < kCh; ++q) {
+        const uint32_t i = base + q * 32u + lane;
+        slot[q] = i < n_syn ? U.syn_slot[i] : 0xFFFFFFFFu;
+      }
+#pragma unroll
+      for (int q = 0; q < kCh; ++q) {
+        const uint32_t i = base + q * 32u + lane;
+        term[q] = 0.0;
+        if (i < n_syn && !(kGen && !cs.mode[multi ? U.syn_cell[i] : 0]))
+          term[q] = U.g[i] * (U.V[slot[q]] - (M.syn_uniform ? M.syn_e_u : U.syn_e[i]));
+      }
+#pragma unroll
+      for (int q = 0; q < kCh; ++q) {
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const double t = __shfl_down_sync(kFull, term[q], o);
+          const uint32_t k = __shfl_down_sync(kFull, slot[q], o);
+          if (lane + o < 32 && k == slot[q]) term[q] += t;
+        }
+        const uint32_t prev = __shfl_up_sync(kFull, slot[q], 1);
+        const uint32_t i = base + q * 32u + lane;
+        if (i < n_syn && (lane == 0 || prev != slot[q])) U.xI[n_hh + i] = term[q];
+      }
+    }
+  } else
   for (uint32_t i = tid; i < n_syn; i += S::size) {
     const uint32_t slot = U.syn_slot[i];
     if (i > 0 && U.syn_slot[i - 1] == slot) continue;
@@ -361,7 +398,10 @@ __device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, co
       const uint32_t slot = U.syn_slot[i];
       if (i > 0 && U.syn_slot[i - 1] == slot) continue;
       if (kGen && !cs.mode[multi ? U.syn_cell[i] : 0]) continue;
-      U.V[slot] -= U.xI[n_hh + i];
+      double I = U.xI[n_hh + i];
+      if (!kWarp && n_syn >= kSynKeyReduceMin)      // partial sums of the chunks the run extends into, in index order
+        for (uint32_t j = (i & ~31u) + 32u; j < n_syn && U.syn_slot[j] == slot; j += 32u) I += U.xI[n_hh + j];
+      U.V[slot] -= I;
     }
     S::sync();
   }
@@ -423,6 +463,11 @@ __device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, co
     U.m[i] = m; U.h[i] = h; U.n[i] = n;
     if (kWarp && cs.wb[c]) { U.gm[i] = m; U.gh[i] = h; U.gn[i] = n; }
   }
+  if (!kGen && !kWarp && M.syn_uniform) {
+    const double decay = M.syn_decay_u;
+#pragma unroll 4
+    for (uint32_t i = tid; i < n_syn; i += S::size) U.g[i] *= decay;
+  } else
   for (uint32_t i = tid; i < n_syn; i += S::size) {
     const uint32_t c = (kGen && multi) ? U.syn_cell[i] : 0;
     const uint32_t md = kGen ? cs.mode[c] : 1u;
@@ -607,7 +652,10 @@ __device__ __forceinline__ void block_view(UnitView& U, const DevModel& M, const
   U.fgen = U.xI + ns; U.invdgen = U.fgen + H.n_slot;
 }
 
-__global__ void __launch_bounds__(kBlockThreads) cable_block_kernel(DevModel M, StepArgs A) {
+#ifndef ARBB_BLOCK_MIN_CTAS
+#define ARBB_BLOCK_MIN_CTAS 8   // latency-bound out of L2: full occupancy beats registers (measured 1..8)
+#endif
+__global__ void __launch_bounds__(kBlockThreads, ARBB_BLOCK_MIN_CTAS) cable_block_kernel(DevModel M, StepArgs A) {
   __shared__ UnitHeader H;
   __shared__ __align__(16) uint8_t cell_mem[kCellScratchBytes * kBlockUnitMaxCells];
   const UnitDesc d = M.units[M.n_warp_units + blockIdx.x];
