@@ -69,7 +69,7 @@ enum {
 enum {
   ARB_CFG_UNIT_BYTES = 1,    /* bytes of streamed records (coefficients + state) one warp's shared-memory
                                 stage may hold; cells are packed into units up to this size, larger
-                                cells are integrated by a whole CTA.  0 = built-in default (22528)  */
+                                cells are integrated by a whole CTA.  0 = built-in default (4096)   */
   ARB_CFG_GROUP_MIN_CELLS = 2 /* cells with identical trees are laid out cell-interleaved in groups
                                 (lane = cell) when their topology class has at least this many cells;
                                 smaller classes are laid out as units (lane = branch).  0 = built-in

@@ -24,7 +24,10 @@ namespace arbb {
 
 namespace {
 
-constexpr int kBlockThreads = 256;              // cable_block_kernel, factor_kernel, init_kernel
+#ifndef ARBB_BLOCK_THREADS
+#define ARBB_BLOCK_THREADS 128
+#endif
+constexpr int kBlockThreads = ARBB_BLOCK_THREADS;              // cable_block_kernel, factor_kernel, init_kernel
 constexpr int kBlockWarps = kBlockThreads / 32;
 constexpr uint32_t kSynKeyReduceMin = 1024;     // block units with at least this many synapses reduce currents by key
 constexpr int kMaxWarpsPerCta = 8;              // cable_warp_kernel
@@ -653,7 +656,7 @@ __device__ __forceinline__ void block_view(UnitView& U, const DevModel& M, const
 }
 
 #ifndef ARBB_BLOCK_MIN_CTAS
-#define ARBB_BLOCK_MIN_CTAS 8   // latency-bound out of L2: full occupancy beats registers (measured 1..8)
+#define ARBB_BLOCK_MIN_CTAS 16   // latency-bound out of L2: full occupancy beats registers (measured 1..16 x 64..256 threads)
 #endif
 __global__ void __launch_bounds__(kBlockThreads, ARBB_BLOCK_MIN_CTAS) cable_block_kernel(DevModel M, StepArgs A) {
   __shared__ UnitHeader H;

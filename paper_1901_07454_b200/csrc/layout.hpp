@@ -12,7 +12,7 @@
 namespace arbb {
 
 struct BuildParams {
-  uint32_t unit_bytes = 22528;    // fast + state bytes a warp unit may hold (one shared-memory stage)
+  uint32_t unit_bytes = 4096;     // fast + state bytes a warp unit may hold (one shared-memory stage); measured on C4
   uint32_t max_branch_len = 1024; // longer unbranched chains are cut into pieces
   uint32_t group_min_cells = 4;   // a topology class with fewer cells is laid out as units; 0 = no groups
   uint32_t group_max_smem = 112 * 1024;  // shared memory a cell group may need (two CTAs per SM at least)
