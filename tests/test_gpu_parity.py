@@ -231,6 +231,26 @@ def test_paper_ring_cell_many_synapses(B, orc):
     g.close()
 
 
+def test_many_synapses_key_reduction_every_step(B, orc):
+    """Cells with thousands of synapses whose tau and e differ from synapse to synapse: the block-unit
+    kernel sums the currents of a control volume by a warp key reduction instead of in
+    index order, so this is the per-step parity case for that path, with events on and off the grid
+    (event-split sub-steps take its general variant)."""
+    m = W.paper_ring(n_cells=3, n_syn=3000, t_end=10.0)
+    rng = np.random.default_rng(7)
+    m["syn_tau"] = rng.uniform(1.0, 4.0, m["n_syn"])
+    m["syn_e"] = rng.uniform(-20.0, 10.0, m["n_syn"])
+    n_ev = 2000
+    m["ext_cell"] = np.concatenate([m["ext_cell"], rng.integers(0, 3, n_ev)])
+    m["ext_syn"] = np.concatenate([m["ext_syn"], rng.integers(0, 3000, n_ev).astype(np.int32)])
+    t_ev = rng.uniform(0.0, 5.0, n_ev)
+    t_ev[::3] = np.round(t_ev[::3] / DT) * DT          # a third of them on grid points
+    m["ext_time"] = np.concatenate([m["ext_time"], t_ev])
+    m["ext_weight"] = np.concatenate([m["ext_weight"], rng.uniform(0.0001, 0.001, n_ev)])
+    m = W.finalize(m)
+    lockstep(B, orc, m, 200)
+
+
 def test_heterogeneous_cut_spikes(B, orc):
     m = W.config4(n_cells=120, t_end=60.0)
     g, o = run_both(B, orc, m, 60.0)
