@@ -64,6 +64,7 @@ struct UnitView {
   const Task* tasks; const LaneRec* lanes; const uint32_t *level_begin, *child, *cell_det;
   const double *C, *S, *sig, *G, *bg, *syn_tau;
   double *contrib, *dcontrib, *xI, *fgen, *invdgen;
+  uint32_t* heads;              // block units: heads[0] = runs in the synapse list, heads[1..] = their first synapse
   int64_t cell_base;
 };
 
@@ -334,8 +335,12 @@ __device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, co
       for (int q = 0; q < kCh; ++q) {
         const uint32_t i = base + q * 32u + lane;
         term[q] = 0.0;
-        if (i < n_syn && !(kGen && !cs.mode[multi ? U.syn_cell[i] : 0]))
-          term[q] = U.g[i] * (U.V[slot[q]] - (M.syn_uniform ? M.syn_e_u : U.syn_e[i]));
+        if (i < n_syn && !(kGen && !cs.mode[multi ? U.syn_cell[i] : 0])) {
+          const double gi = U.g[i];
+          term[q] = gi * (U.V[slot[q]] - (M.syn_uniform ? M.syn_e_u : U.syn_e[i]));
+          // nominal step: the decay over dt does not depend on V', so g is updated while it is here
+          if (!kGen) U.g[i] = gi * (M.syn_uniform ? M.syn_decay_u : U.syn_decay[i]);
+        }
       }
 #pragma unroll
       for (int q = 0; q < kCh; ++q) {
@@ -396,15 +401,25 @@ __device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, co
     }
     S::sync();
   }
-  if (n_syn) {
+  if (!kWarp && n_syn >= kSynKeyReduceMin) {
+    // run heads (listed once per dt by factor_kernel) add the partial sums of the chunks their run
+    // extends into, in index order
+    const uint32_t nh = U.heads[0];
+    for (uint32_t h = tid; h < nh; h += S::size) {
+      const uint32_t i = U.heads[1 + h];
+      const uint32_t slot = U.syn_slot[i];
+      if (kGen && !cs.mode[multi ? U.syn_cell[i] : 0]) continue;
+      double I = U.xI[n_hh + i];
+      for (uint32_t j = (i & ~31u) + 32u; j < n_syn && U.syn_slot[j] == slot; j += 32u) I += U.xI[n_hh + j];
+      U.V[slot] -= I;
+    }
+    S::sync();
+  } else if (n_syn) {
     for (uint32_t i = tid; i < n_syn; i += S::size) {
       const uint32_t slot = U.syn_slot[i];
       if (i > 0 && U.syn_slot[i - 1] == slot) continue;
       if (kGen && !cs.mode[multi ? U.syn_cell[i] : 0]) continue;
-      double I = U.xI[n_hh + i];
-      if (!kWarp && n_syn >= kSynKeyReduceMin)      // partial sums of the chunks the run extends into, in index order
-        for (uint32_t j = (i & ~31u) + 32u; j < n_syn && U.syn_slot[j] == slot; j += 32u) I += U.xI[n_hh + j];
-      U.V[slot] -= I;
+      U.V[slot] -= U.xI[n_hh + i];
     }
     S::sync();
   }
@@ -466,10 +481,8 @@ __device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, co
     U.m[i] = m; U.h[i] = h; U.n[i] = n;
     if (kWarp && cs.wb[c]) { U.gm[i] = m; U.gh[i] = h; U.gn[i] = n; }
   }
-  if (!kGen && !kWarp && M.syn_uniform) {
-    const double decay = M.syn_decay_u;
-#pragma unroll 4
-    for (uint32_t i = tid; i < n_syn; i += S::size) U.g[i] *= decay;
+  if (!kGen && !kWarp && n_syn >= kSynKeyReduceMin) {
+    // done in phase B
   } else
   for (uint32_t i = tid; i < n_syn; i += S::size) {
     const uint32_t c = (kGen && multi) ? U.syn_cell[i] : 0;
@@ -653,6 +666,7 @@ __device__ __forceinline__ void block_view(UnitView& U, const DevModel& M, const
   const uint32_t nl = align_up(H.n_lane, 2), ns = align_up(H.n_hh + H.n_syn + H.n_clamp, 2);
   U.contrib = sc; U.dcontrib = sc + nl; U.xI = sc + 2 * (size_t)nl;
   U.fgen = U.xI + ns; U.invdgen = U.fgen + H.n_slot;
+  U.heads = (uint32_t*)(U.invdgen + H.n_slot);
 }
 
 #ifndef ARBB_BLOCK_MIN_CTAS
@@ -701,6 +715,17 @@ __global__ void __launch_bounds__(kBlockThreads) factor_kernel(DevModel M, doubl
   if (!M.syn_uniform) {
     double* decay = const_cast<double*>(U.syn_decay);
     for (uint32_t i = threadIdx.x; i < U.n_syn; i += kBlockThreads) decay[i] = exp(-dt / U.syn_tau[i]);
+  }
+  if (blockIdx.x >= M.n_warp_units && U.n_syn >= kSynKeyReduceMin) {   // run heads of the synapse list (order irrelevant)
+    __shared__ uint32_t n_heads;
+    uint32_t* heads = (uint32_t*)(M.scratch + H.scratch_base + 2 * (size_t)align_up(H.n_lane, 2) +
+                                  align_up(H.n_hh + H.n_syn + H.n_clamp, 2) + 2 * (size_t)H.n_slot);
+    if (threadIdx.x == 0) n_heads = 0;
+    __syncthreads();
+    for (uint32_t i = threadIdx.x; i < U.n_syn; i += kBlockThreads)
+      if (i == 0 || U.syn_slot[i - 1] != U.syn_slot[i]) heads[1 + atomicAdd(&n_heads, 1u)] = i;
+    __syncthreads();
+    if (threadIdx.x == 0) heads[0] = n_heads;
   }
 }
 

@@ -818,9 +818,10 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     }
     const uint32_t n_spec = uc.n_hh + uc.n_syn + uc.n_clamp;
     if (uc.flags & UNIT_BLOCK) {
-      // contrib | dcontrib | xI | fgen | invdgen
+      // contrib | dcontrib | xI | fgen | invdgen | run heads of the synapse list (uint32 count, then indices)
       uc.scratch_base = H.scratch_doubles;
-      H.scratch_doubles += 2 * (int64_t)align_up(uc.n_lane, 2) + align_up(n_spec, 2) + 2 * (int64_t)uc.n_slot;
+      H.scratch_doubles += 2 * (int64_t)align_up(uc.n_lane, 2) + align_up(n_spec, 2) + 2 * (int64_t)uc.n_slot +
+                           align_up(uc.n_slot / 2 + 2, 2);
       H.block_lane_cap = std::max(H.block_lane_cap, uc.n_lane);
     } else {
       H.fast_cap = std::max(H.fast_cap, align_up(uc.fast_bytes, 128));
