@@ -322,7 +322,10 @@ __device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, co
     // reduces them by key = control volume with shuffles (the "key reduction" of PAPER.md:218; runs are
     // contiguous), and the first lane of every key inside the chunk stores a partial sum; in phase C the run
     // heads add the partials of the chunks their run extends into, in index order (no atomics).
-    constexpr int kCh = 4;               // chunks per warp and trip: independent loads in flight
+#ifndef ARBB_KCH
+#define ARBB_KCH 2
+#endif
+    constexpr int kCh = ARBB_KCH;        // chunks per warp and trip: independent loads in flight
     for (uint32_t base = (uint32_t)S::warp() * 32u * kCh; base < n_syn; base += (uint32_t)S::warps * 32u * kCh) {
       uint32_t slot[kCh];
       double term[kCh];
