@@ -16,6 +16,12 @@
  *   synapse / event path .............. closed-form decay and split-step exactness (P8), step
  *                                      splitting continuity (P12), hand-computed network timings
  *                                      and the ring invariant (P11), ordering invariance (P10)
+ *   synapse current I = g (V - e) ..... one-step closed form with e != 0, two synapses on one CV,
+ *                                      conductance-weighted steady state (P13)
+ *   "state integrated with V'" ........ hand-computed gates after one step with V' - V > 3 mV (P14)
+ *   clamp window t0 <= t < t1 ......... hand-computed recurrence, exactly steps 5 and 6 see it (P15)
+ * tests/test_oracle_mutations.py mutates a copy of this file line by line and checks that the pins
+ * above turn red for every mutation in its list.
  * Parity unpinned (inputs / constants only, identical on both sides): HH reversal potentials and
  * temperature (R5), V_init (R4), the cell-centred generator (R3), drive and kick weights.
  *
@@ -106,6 +112,7 @@ typedef struct {
   int64_t* clamps; int64_t n_clamps;
   int32_t det; double v_prev; int armed;
   double new_spikes[8]; int n_new;   /* spikes of the grid step in progress */
+  int spike_overflow;                /* a ninth spike in one grid step: orc_advance reports it, nothing is dropped silently */
   int64_t substeps;
 } cell_t;
 
@@ -222,6 +229,7 @@ static void cell_step(orc_model* M, cell_t* c, double t, double delta) {
   double vd = v[c->det];
   if (c->armed && c->v_prev < M->theta && M->theta <= vd) {
     if (c->n_new < 8) c->new_spikes[c->n_new++] = t + delta * (M->theta - c->v_prev) / (vd - c->v_prev);
+    else c->spike_overflow = 1;
     c->armed = 0;
   }
   if (vd < M->theta) c->armed = 1;
@@ -414,6 +422,8 @@ int orc_advance(orc_model* M, double t_end, double dt) {
       M->cells[c].n_new = 0;
       cell_interval(M, &M->cells[c], ta, tb, dt, nominal);
     }
+    for (int64_t c = 0; c < M->n_cells; ++c)
+      if (M->cells[c].spike_overflow) FAIL(-6, "cell %lld fired more than 8 spikes in one grid step", (long long)c);
     for (int64_t c = 0; c < M->n_cells; ++c) {
       cell_t* ce = &M->cells[c];
       for (int j = 0; j < ce->n_new; ++j) {

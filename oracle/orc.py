@@ -14,6 +14,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = [os.path.join(_HERE, "arb_oracle.c"), os.path.join(_HERE, "arb_oracle.h")]
 _LIB = os.path.join(_HERE, "liborc.so")
+# tests/test_oracle_mutations.py points this at deliberately broken builds to show that the pins catch them
+_LIB_OVERRIDE = os.environ.get("ORC_MUTANT_LIB")
 CFLAGS = ["-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC", "-shared", "-std=c11",
           "-Wall"]
 
@@ -53,7 +55,7 @@ _lib = None
 def lib():
     global _lib
     if _lib is None:
-        L = C.CDLL(build())
+        L = C.CDLL(_LIB_OVERRIDE or build())
         L.orc_exprelr.restype = C.c_double
         L.orc_exprelr.argtypes = [C.c_double]
         L.orc_hh_rates.argtypes = [C.c_double, C.c_void_p]

@@ -531,3 +531,128 @@ def test_validation_errors(orc):
     o.advance(1.0, DT)
     with pytest.raises(orc.OracleError):
         o.advance(0.5, DT)
+
+
+# ---------------------------------------------------------------------------------------------
+# P13 synapse current I = g (V - e): magnitude and reversal potential   (eq 2a, R7)
+# Mutations this pin kills (tests/test_oracle_mutations.py): `I += 0.5*g*(V-e)`, `I += g*(V+e)`.
+# ---------------------------------------------------------------------------------------------
+def _one_cv_syns(es, taus, area=400.0, g_pas=1e-4, e_pas=-65.0, vinit=-60.0):
+    n = len(es)
+    m = dict(n_cells=1, cv_off=[0, 1], cv_parent=[-1], cv_area=[area], cv_cm=[1.0], cv_raxial=[1.0],
+             cv_vinit=[vinit], pas_g=[g_pas], pas_e=[e_pas], syn_off=[0, n], syn_cv=[0] * n,
+             syn_tau=taus, syn_e=es, t_end=10.0)
+    return W.finalize(m)
+
+
+def test_p13_synapse_current_magnitude_and_reversal(orc):
+    area, g_pas, e_pas, v0 = 400.0, 1e-4, -65.0, -60.0
+    C, G = 1.0 * area * 1e-5, g_pas * area * 1e-2
+    # one synapse held at a known conductance, reversal potential != 0: one step of eq 2a / PAPER.md:154
+    for g, e in ((0.003, -20.0), (0.0007, 15.0), (0.002, -80.0)):
+        o = orc.Oracle(_one_cv_syns([e], [2.0], vinit=v0))
+        o.set_state(syn_g=[g])
+        o.advance(DT, DT)
+        ref = ((C / DT) * v0 - G * (v0 - e_pas) - g * (v0 - e)) / (C / DT)
+        assert o.voltage()[0] == pytest.approx(ref, rel=1e-13)
+        assert (o.voltage()[0] > v0 - DT / C * G * (v0 - e_pas)) == (e > v0)     # pulls towards e
+    # two synapses with different reversal potentials on the same CV add up
+    (g1, e1), (g2, e2) = (0.0021, -10.0), (0.0013, -75.0)
+    o = orc.Oracle(_one_cv_syns([e1, e2], [2.0, 3.0], vinit=v0))
+    o.set_state(syn_g=[g1, g2])
+    o.advance(DT, DT)
+    ref = ((C / DT) * v0 - G * (v0 - e_pas) - g1 * (v0 - e1) - g2 * (v0 - e2)) / (C / DT)
+    assert o.voltage()[0] == pytest.approx(ref, rel=1e-13)
+    # constant conductance (tau -> infinity): the steady state is the conductance-weighted mean
+    g, e = 0.0025, -30.0
+    o = orc.Oracle(_one_cv_syns([e], [1e15], vinit=v0))
+    o.set_state(syn_g=[g])
+    o.advance(40.0, DT)                                   # tau_m = C/(G+g) ~ 1.4 ms
+    assert o.voltage()[0] == pytest.approx((G * e_pas + g * e) / (G + g), abs=1e-10)
+    assert o.syn_g()[0] == pytest.approx(g, rel=1e-10)
+
+
+# ---------------------------------------------------------------------------------------------
+# P14 "the state variables are integrated with the updated voltage values"
+# Mutation this pin kills: gate rates evaluated at V(t) instead of V'.
+# ---------------------------------------------------------------------------------------------
+def test_p14_gates_are_integrated_with_the_updated_voltage(orc):
+    def rates(v):           # textbook form (as in P9), independent of the oracle
+        return (0.1 * (v + 40) / (1 - np.exp(-(v + 40) / 10)), 4 * np.exp(-(v + 65) / 18),
+                0.07 * np.exp(-(v + 65) / 20), 1 / (1 + np.exp(-(v + 35) / 10)),
+                0.01 * (v + 55) / (1 - np.exp(-(v + 55) / 10)), 0.125 * np.exp(-(v + 65) / 80))
+
+    def gates_after(v, x, delta):
+        r = rates(v)
+        out = []
+        for k in range(3):
+            a, b = r[2 * k], r[2 * k + 1]
+            inf = a / (a + b)
+            out.append(inf + (x[k] - inf) * np.exp(-delta * (a + b)))
+        return np.array(out)
+
+    area, amp, v0 = 500.0, 2.0, -52.0                     # large clamp: V' - V is several mV
+    x0 = np.array([0.31, 0.42, 0.47])
+    o = orc.Oracle(_single_hh(v0, amp, 0.0, 1e9))
+    o.set_state(m=[x0[0]], h=[x0[1]], n=[x0[2]])
+    o.advance(DT, DT)
+    C = 1.0 * area * 1e-5
+    dens = W.GNABAR * x0[0] ** 3 * x0[1] * (v0 - W.ENA) + W.GKBAR * x0[2] ** 4 * (v0 - W.EK) + W.GL * (v0 - W.EL)
+    v1 = v0 + DT / C * (amp - dens * area * 1e-2)         # single CV: eq at PAPER.md:154 has no axial term
+    assert v1 - v0 > 3.0
+    assert o.voltage()[0] == pytest.approx(v1, rel=1e-13)
+    got = np.array([g[0] for g in o.gates()])
+    with_new, with_old = gates_after(v1, x0, DT), gates_after(v0, x0, DT)
+    assert np.max(np.abs(with_new - with_old)) > 1e-6     # the pin has teeth
+    assert np.max(np.abs(got - with_new)) <= 1e-13
+    assert np.max(np.abs(got - with_old)) > 1e-6
+
+
+# ---------------------------------------------------------------------------------------------
+# P15 clamp window t0 <= t < t1, t = step start                             (R8; eq 2a's injected current)
+# Mutation this pin kills: `t0 < t && t <= t1`.
+# ---------------------------------------------------------------------------------------------
+def test_p15_clamp_window_is_half_open_at_the_step_start(orc):
+    area, g_pas, e_pas, amp = 300.0, 2e-4, -65.0, 0.05
+    C, G = 1.0 * area * 1e-5, g_pas * area * 1e-2
+    m = W.finalize(dict(n_cells=1, cv_off=[0, 1], cv_parent=[-1], cv_area=[area], cv_cm=[1.0], cv_raxial=[1.0],
+                        pas_g=[g_pas], pas_e=[e_pas], clamp_cell=[0], clamp_cv=[0], clamp_t0=[5 * DT],
+                        clamp_t1=[7 * DT], clamp_amp=[amp], t_end=1.0))
+    o = orc.Oracle(m)
+    v, seen = e_pas, []
+    for k in range(10):                                   # step k starts at t = k * dt
+        on = 5 <= k < 7
+        v = v - DT / C * (G * (v - e_pas) - (amp if on else 0.0))
+        o.advance((k + 1) * DT, DT)
+        assert o.voltage()[0] == pytest.approx(v, rel=1e-14), k
+        seen.append(o.voltage()[0])
+    assert seen[4] == e_pas and seen[5] > e_pas           # exactly steps 5 and 6 see the current
+    assert seen[6] - seen[5] > 0.5 * (seen[5] - seen[4]) and seen[7] < seen[6]
+
+
+def test_ninth_spike_in_one_grid_step_is_an_error_not_a_drop(orc):
+    """The oracle keeps at most 8 spikes of a cell per grid step; a ninth must be reported."""
+    dt, nsub = 0.05, 24
+    area, cm = 400.0, 1.0
+    C = cm * area * 1e-5
+    delta = dt / nsub
+    g_pas = 0.9 * C / delta / (area * 1e-2)                # leak wipes 90% of (V - E) per sub-step
+    w = 0.4 * C / delta / 65.0                              # a sub-step with g = w lifts V by ~0.4 mV
+    t = 2 * dt + (np.arange(nsub - 1) + 1) * delta
+    wt = np.where(np.arange(nsub - 1) % 2 == 0, w, -w)
+    m = W.finalize(dict(n_cells=1, cv_off=[0, 1], cv_parent=[-1], cv_area=[area], cv_cm=[cm], cv_raxial=[1.0],
+                        pas_g=[g_pas], pas_e=[-65.0], syn_off=[0, 1], syn_cv=[0], syn_tau=[1e9], syn_e=[0.0],
+                        ext_cell=np.zeros(nsub - 1, np.int64), ext_syn=np.zeros(nsub - 1, np.int32), ext_time=t,
+                        ext_weight=wt, threshold=-64.9, dt=dt, t_end=1.0))
+    o = orc.Oracle(m)
+    o.advance(2 * dt, dt)
+    assert len(o.spikes()[1]) == 0
+    with pytest.raises(orc.OracleError, match="more than 8 spikes"):
+        o.advance(3 * dt, dt)
+    # eight or fewer are kept: the same input cut after 8 upward crossings
+    m2 = dict(m)
+    keep = 2 * 8 - 1
+    m2.update(ext_cell=m["ext_cell"][:keep], ext_syn=m["ext_syn"][:keep], ext_time=t[:keep], ext_weight=wt[:keep])
+    o = orc.Oracle(W.finalize(m2))
+    o.advance(3 * dt, dt)
+    assert len(o.spikes()[1]) == 8
