@@ -21,7 +21,9 @@
  * cudaMalloc) that must stay alive, and untouched by the caller, until arb_destroy.
  *
  * Errors: every call returns 0 (or a count) on success or a negative ARB_E_* code; nothing throws
- * or aborts across the ABI; arb_last_error gives text.  One model per host thread at a time.
+ * or aborts across the ABI; arb_last_error gives text.  A model may be used by one host thread at a
+ * time; the library keeps no process-wide mutable state (models on several devices may coexist; the
+ * calling thread's current device must be the one the workspace lives on).
  */
 #ifndef ARBB200_H
 #define ARBB200_H
@@ -37,8 +39,10 @@ enum {
   ARB_E_INVALID = -2,   /* description or argument out of range (see arb_plan)                   */
   ARB_E_WORKSPACE = -3, /* device workspace smaller than arb_plan asked for, or misaligned       */
   ARB_E_CUDA = -4,      /* a CUDA runtime call or kernel failed                                  */
-  ARB_E_OVERFLOW = -5,  /* spike / event buffer capacity exceeded; the model is unusable after   */
-  ARB_E_NOMEM = -6      /* host allocation failed                                                */
+  ARB_E_OVERFLOW = -5,  /* spike / event buffer capacity exceeded (see "Capacities" below)        */
+  ARB_E_NOMEM = -6,     /* host allocation failed                                                */
+  ARB_E_DIVERGED = -7   /* a detector voltage became NaN / Inf (the explicit membrane currents of
+                           reading R1 are only conditionally stable); the model is unusable after */
 };
 
 /* arb_probe selectors */
@@ -63,17 +67,6 @@ enum {
   ARB_OPT_TIMING = 3         /* 1: bracket the cable-step launches and the epoch-boundary kernels of
                                 every epoch with CUDA events on the model's stream (read them with
                                 ARB_PROBE_TIMING); setting the option clears the accumulated times  */
-};
-
-/* arb_configure keys (process-wide defaults read by later arb_plan / arb_create calls) */
-enum {
-  ARB_CFG_UNIT_BYTES = 1,    /* bytes of streamed records (coefficients + state) one warp's shared-memory
-                                stage may hold; cells are packed into units up to this size, larger
-                                cells are integrated by a whole CTA.  0 = built-in default (4096)   */
-  ARB_CFG_GROUP_MIN_CELLS = 2 /* cells with identical trees are laid out cell-interleaved in groups
-                                (lane = cell) when their topology class has at least this many cells;
-                                smaller classes are laid out as units (lane = branch).  0 = built-in
-                                default (4); 1 = every cell in groups; >= 2^31 = no groups          */
 };
 
 /* The problem statement of PAPER.md section II as flat arrays.
@@ -115,6 +108,23 @@ typedef struct {
   const int64_t* ext_cell;
   const int32_t* ext_syn;
   const double *ext_time, *ext_weight; /* ms (>= 0), uS                                           */
+  /* Layout and capacity options; 0 = library default.  Part of the description, so that planning
+   * and creation agree and the library keeps no process-wide state.
+   *   layout_group_min_cells  cells with identical trees are laid out cell-interleaved in groups
+   *                           (lane = cell) when their topology class has at least this many cells
+   *                           (default 4; 1 = every cell in groups; >= 2^31 = no groups)
+   *   layout_unit_bytes       bytes of streamed records one warp unit may hold (default 4096)
+   *   cap_spikes              entries of the device spike buffer.  arb_advance drains it into host
+   *                           memory at least every 2,000 grid steps, so it bounds the spikes of
+   *                           such a stretch, not of the run (default max(2^20, 64 n_cells))
+   *   cap_events              entries of the pool of events in flight, i.e. generated by a spike
+   *                           but due after the epoch being built (default n_conn * max(4,
+   *                           ceil(max delay / 2 ms) + 1) + 1024)
+   * Capacities: exceeding one makes arb_advance return ARB_E_OVERFLOW with the buffer named in
+   * arb_last_error.  Events or spikes beyond the capacity are lost, so the model is unusable
+   * afterwards (every later call returns the same error): create it again with a larger cap_*.
+   * (reading R0 says why the state is not rolled back to the last epoch.) */
+  int64_t layout_group_min_cells, layout_unit_bytes, cap_spikes, cap_events;
 } arb_desc;
 
 typedef struct arb_model arb_model; /* opaque; lives in host memory, owned by the library */
@@ -137,12 +147,22 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t workspace_bytes
  * step is taken when (t_end - t) is not a multiple of dt; grid steps are split at event times
  * (reading R9).  Kernels are queued on the model's stream; the call returns after
  * they have completed and the overflow flags have been checked.  ARB_E_INVALID: dt <= 0,
- * t_end < t, dt longer than the shortest connection delay. */
+ * t_end < t, dt longer than the shortest connection delay.
+ * Epochs: cells are independent for one minimum delay, so spikes become events
+ * once per epoch of floor(min_delay / dt - 1e-6) grid steps (at least 1).  The 1e-6 guard keeps an
+ * event that lands exactly on the epoch's last grid point out of the epoch that generates it: a
+ * network with min_delay = 5 ms and dt = 0.025 ms runs epochs of 199 steps, one with
+ * min_delay = 5.0001 ms epochs of 200.  Results do not depend on the epoch length. */
 int arb_advance(arb_model* m, double t_end, double dt);
 
-/* Spikes since creation.  Returns the total count; fills min(cap, count) entries sorted by
- * (time, cell).  cell / time may be NULL when cap == 0.  Negative on error. */
+/* Spikes since creation (or since the last arb_clear_spikes).  Returns the count; fills min(cap,
+ * count) entries sorted by (time, cell).  cell / time may be NULL when cap == 0.  Negative on
+ * error.  The history lives in host memory (arb_advance drains the device buffer into it). */
 int64_t arb_spikes(arb_model* m, int64_t* cell, double* time, int64_t cap);
+
+/* Forget the spikes recorded so far (a caller that reads spikes after every epoch keeps the
+ * history short this way).  Does not touch events already generated from them. */
+int arb_clear_spikes(arb_model* m);
 
 /* Membrane potential of every CV in the caller's CV order.  n_cv must equal cv_off[n_cells]. */
 int arb_voltage(arb_model* m, double* out, int64_t n_cv);
@@ -157,7 +177,9 @@ int arb_voltage(arb_model* m, double* out, int64_t n_cv);
  *                  grid step moves (all units and groups)}, n >= 8; when n >= 12 also {warp units,
  *                  warps per CTA and shared-memory bytes per warp of the last launch, distinct tree
  *                  records}; when n >= 16 also {cell groups, topology classes in groups, CTAs of a
- *                  cell-group launch, shared-memory bytes per CTA of the cell-group kernel}.
+ *                  cell-group launch, shared-memory bytes per CTA of the cell-group kernel}; when
+ *                  n >= 20 also {forests, block units, CTAs of a forest launch, shared-memory bytes
+ *                  per CTA of the forest kernel}.
  * ARB_PROBE_TIMING: out[0..3] = {ms spent in cable-step kernels, cable-step launches timed,
  *                  ms spent in epoch-boundary (spike -> event) kernels, their launches}, measured
  *                  with CUDA events while ARB_OPT_TIMING is on, n >= 4. */
@@ -170,9 +192,6 @@ int arb_set_state(arb_model* m, const double* v, const double* hh_m, const doubl
                   const double* hh_n, const double* syn_g);
 
 int arb_set_option(arb_model* m, int key, int64_t value);
-
-/* Process-wide build defaults (ARB_CFG_*); affects models planned / created afterwards. */
-int arb_configure(int key, int64_t value);
 
 /* Measures the fp64 fused-multiply-add rate of the current device (independent DFMA chains in
  * registers, no memory traffic; kernel timed with CUDA events on `cuda_stream`, NULL = default

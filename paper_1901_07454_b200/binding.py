@@ -9,16 +9,20 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("ARBB200_LIB") or os.path.join(_HERE, "libarbb200.so")   # override: another build of the same ABI
+LIB_PATH = os.path.join(_HERE, "libarbb200.so")
 
-ARB_OK, ARB_E_NULL, ARB_E_INVALID, ARB_E_WORKSPACE, ARB_E_CUDA, ARB_E_OVERFLOW, ARB_E_NOMEM = 0, -1, -2, -3, -4, -5, -6
+ARB_OK, ARB_E_NULL, ARB_E_INVALID, ARB_E_WORKSPACE, ARB_E_CUDA, ARB_E_OVERFLOW, ARB_E_NOMEM, ARB_E_DIVERGED = 0, -1, -2, -3, -4, -5, -6, -7
 ARB_PROBE_M, ARB_PROBE_H, ARB_PROBE_N, ARB_PROBE_SYN_G, ARB_PROBE_TIME, ARB_PROBE_NSTEPS, ARB_PROBE_STATS, ARB_PROBE_TIMING = range(8)
 ARB_OPT_FUSED_STEPS, ARB_OPT_EPOCH_STEPS, ARB_OPT_TIMING, ARB_OPT_STAGES, ARB_OPT_L2_PREFETCH, ARB_OPT_GROUP_CTAS, ARB_OPT_HOT_FIRST = 1, 2, 3, 4, 5, 6, 7
-ARB_CFG_UNIT_BYTES = 1
-ARB_CFG_GROUP_MIN_CELLS = 2
 
-EXPORTS = ("arb_plan", "arb_create", "arb_advance", "arb_spikes", "arb_voltage", "arb_probe",
-           "arb_set_state", "arb_set_option", "arb_configure", "arb_destroy", "arb_last_error")
+EXPORTS = ("arb_plan", "arb_create", "arb_advance", "arb_spikes", "arb_clear_spikes", "arb_voltage", "arb_probe",
+           "arb_set_state", "arb_set_option", "arb_fp64_peak", "arb_destroy", "arb_last_error")
+
+# arb_desc's layout / capacity options (0 = library default).  A workloads dict may carry them under the
+# same names; LAYOUT_DEFAULTS fills in the ones it does not (the parity tests run every case under
+# several layouts this way).
+OPTION_FIELDS = ("layout_group_min_cells", "layout_unit_bytes", "cap_spikes", "cap_events")
+LAYOUT_DEFAULTS = {}
 
 
 class ArbError(RuntimeError):
@@ -43,6 +47,8 @@ class arb_desc(C.Structure):
         ("conn_syn", C.c_void_p), ("conn_delay", C.c_void_p), ("conn_weight", C.c_void_p),
         ("n_ext", C.c_int64), ("ext_cell", C.c_void_p), ("ext_syn", C.c_void_p),
         ("ext_time", C.c_void_p), ("ext_weight", C.c_void_p),
+        ("layout_group_min_cells", C.c_int64), ("layout_unit_bytes", C.c_int64),
+        ("cap_spikes", C.c_int64), ("cap_events", C.c_int64),
     ]
 
 
@@ -66,7 +72,7 @@ def lib():
         L.arb_probe.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int64]
         L.arb_set_state.argtypes = [C.c_void_p] * 6
         L.arb_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
-        L.arb_configure.argtypes = [C.c_int, C.c_int64]
+        L.arb_clear_spikes.argtypes = [C.c_void_p]
         L.arb_fp64_peak.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.arb_destroy.argtypes = [C.c_void_p]
         L.arb_destroy.restype = None
@@ -85,19 +91,15 @@ def make_desc(m):
     d = arb_desc()
     for name, _ in arb_desc._fields_:
         v = m.get(name)
-        if isinstance(v, np.ndarray):
+        if name in OPTION_FIELDS:
+            setattr(d, name, int(v if v is not None else LAYOUT_DEFAULTS.get(name, 0)))
+        elif isinstance(v, np.ndarray):
             setattr(d, name, _ptr(v))
         elif v is None:
             setattr(d, name, None)
         else:
             setattr(d, name, v)
     return d
-
-
-def configure(key, value):
-    rc = lib().arb_configure(int(key), int(value))
-    if rc:
-        raise ArbError(rc, lib().arb_last_error(None).decode())
 
 
 def arb_fp64_peak(stream=None):
@@ -159,7 +161,7 @@ class Model:
         return out
 
     def probe(self, what):
-        n = {ARB_PROBE_SYN_G: self.n_syn, ARB_PROBE_TIME: 1, ARB_PROBE_NSTEPS: 2, ARB_PROBE_STATS: 16,
+        n = {ARB_PROBE_SYN_G: self.n_syn, ARB_PROBE_TIME: 1, ARB_PROBE_NSTEPS: 2, ARB_PROBE_STATS: 20,
              ARB_PROBE_TIMING: 4}.get(what, self.n_cv)
         out = np.empty(n)
         self._check(lib().arb_probe(self._h, what, _ptr(out), n))
@@ -180,7 +182,8 @@ class Model:
                     events_delivered=int(s[4]), launches=int(s[5]), epoch_steps=int(s[6]),
                     streamed_bytes_per_step=int(s[7]), warp_units=int(s[8]), warps_per_cta=int(s[9]),
                     smem_per_warp=int(s[10]), topo_records=int(s[11]), groups=int(s[12]), classes=int(s[13]),
-                    group_ctas=int(s[14]), group_smem=int(s[15]))
+                    group_ctas=int(s[14]), group_smem=int(s[15]), forests=int(s[16]), block_units=int(s[17]),
+                    forest_ctas=int(s[18]), forest_smem=int(s[19]))
 
     def timing(self):
         t = self.probe(ARB_PROBE_TIMING)
@@ -192,6 +195,9 @@ class Model:
         if n:
             self._check(lib().arb_spikes(self._h, _ptr(cell), _ptr(t), n))
         return cell, t
+
+    def clear_spikes(self):
+        self._check(lib().arb_clear_spikes(self._h))
 
     def set_state(self, v=None, m=None, h=None, n=None, syn_g=None):
         arrs = [None if a is None else np.ascontiguousarray(a, np.float64) for a in (v, m, h, n, syn_g)]

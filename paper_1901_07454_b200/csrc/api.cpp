@@ -41,13 +41,18 @@ struct Regions {
 
 struct Caps { int64_t pool = 0, ev = 0, spikes = 0; };
 
-Caps capacities(const HostModel& H) {
+// Capacities (include/arbb200.h, "Capacities").  The pool holds events in flight: a connection whose
+// delay spans k epochs carries up to k events per spike train period; the default allows one spike every
+// 2 ms per connection over the longest delay, and at least four events per connection.
+Caps capacities(const HostModel& H, const arb_desc& d) {
   Caps c;
-  c.pool = 4 * H.n_conn + 1024;
+  const int64_t per_conn = std::max<int64_t>(4, (int64_t)std::ceil(H.max_delay / 2.0) + 1);
+  c.pool = d.cap_events > 0 ? d.cap_events : per_conn * H.n_conn + 1024;
   c.ev = c.pool + H.n_ext + 16;
-  c.spikes = std::max<int64_t>(1 << 20, 64 * H.n_cells);
+  c.spikes = d.cap_spikes > 0 ? d.cap_spikes : std::max<int64_t>(1 << 20, 64 * H.n_cells);
   return c;
 }
+constexpr int64_t kDrainSteps = 2000;   // the device spike buffer is drained at least this often
 
 // upper bound of the CTAs of a cell-group launch
 int64_t group_cta_cap(const HostModel& H) { return std::min<int64_t>(H.n_groups, kMaxGroupCtas); }
@@ -143,7 +148,12 @@ struct arb_model {
   int64_t group_slots = 0, group_streamed = 0;   // statistics: CV slots incl. padding, bytes one grid step streams
   int64_t opt_stages = 0;
   bool broken = false;
+  int broken_code = ARB_E_OVERFLOW;
   std::string err;
+  // spike history in host memory: arb_advance drains the device buffer into it
+  std::vector<uint32_t> sp_cell;
+  std::vector<double> sp_time;
+  bool sp_sorted = true;
 };
 
 namespace {
@@ -168,14 +178,13 @@ cudaError_t upload(arb_model* m, const Region& r, const std::vector<T>& v) {
   return cudaMemcpyAsync(m->ws + r.off, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, m->stream);
 }
 
-int64_t g_unit_bytes = 0;   // arb_configure(ARB_CFG_UNIT_BYTES)
-int64_t g_group_min = 0;    // arb_configure(ARB_CFG_GROUP_MIN_CELLS)
-
-BuildParams default_params() {
-  BuildParams P;
-  if (g_unit_bytes > 0) P.unit_bytes = (uint32_t)g_unit_bytes;
-  if (g_group_min > 0) P.group_min_cells = g_group_min >= 0x7FFFFFFF ? 0u : (uint32_t)g_group_min;
-  return P;
+// layout options travel in the description (no process-wide state)
+int params_of(const arb_desc& d, BuildParams& P, std::string& err) {
+  if (d.layout_group_min_cells < 0 || d.layout_unit_bytes < 0 || d.cap_spikes < 0 || d.cap_events < 0) { err = "negative layout / capacity option"; return ARB_E_INVALID; }
+  if (d.layout_unit_bytes != 0 && (d.layout_unit_bytes < 1024 || d.layout_unit_bytes > 112 * 1024)) { err = "layout_unit_bytes out of range (1024 .. 114688)"; return ARB_E_INVALID; }
+  if (d.layout_unit_bytes > 0) P.unit_bytes = (uint32_t)d.layout_unit_bytes;
+  if (d.layout_group_min_cells > 0) P.group_min_cells = d.layout_group_min_cells >= 0x7FFFFFFF ? 0u : (uint32_t)d.layout_group_min_cells;
+  return ARB_OK;
 }
 
 }  // namespace
@@ -187,9 +196,11 @@ int arb_plan(const arb_desc* desc, size_t* workspace_bytes) {
   try {
     HostModel H;
     std::string err;
-    int rc = build(*desc, default_params(), false, H, err);
+    BuildParams P;
+    int rc = params_of(*desc, P, err);
+    if (!rc) rc = build(*desc, P, false, H, err);
     if (rc) return fail(nullptr, rc, err);
-    *workspace_bytes = carve(H, capacities(H)).total;
+    *workspace_bytes = carve(H, capacities(H, *desc)).total;
     return ARB_OK;
   } catch (const std::bad_alloc&) {
     return fail(nullptr, ARB_E_NOMEM, "arb_plan: out of host memory");
@@ -203,22 +214,30 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
   try {
     m = new arb_model();
     std::string err;
-    int rc = build(*desc, default_params(), true, m->H, err);
+    BuildParams BP;
+    int rc = params_of(*desc, BP, err);
+    if (!rc) rc = build(*desc, BP, true, m->H, err);
     if (rc) { delete m; return fail(nullptr, rc, err); }
     HostModel& H = m->H;
-    m->cap = capacities(H);
+    m->cap = capacities(H, *desc);
     m->R = carve(H, m->cap);
     if (bytes < m->R.total) { delete m; return fail(nullptr, ARB_E_WORKSPACE, "arb_create: workspace smaller than arb_plan reported"); }
     if (reinterpret_cast<uintptr_t>(dev_workspace) % 256) { delete m; return fail(nullptr, ARB_E_WORKSPACE, "arb_create: workspace must be 256-byte aligned"); }
     m->ws = static_cast<char*>(dev_workspace);
     m->stream = static_cast<cudaStream_t>(cuda_stream);
+    {
+      int dev = 0, sms = 0;
+      if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) {
+        delete m;
+        return fail(nullptr, ARB_E_CUDA, "arb_create: no CUDA device (there is no CPU fallback)");
+      }
+      m->sm_count = sms;
+    }
+    // the kernels' shared-memory opt-in is per device: (re)done for every model, never cached
+    if (configure_kernels() != cudaSuccess) { delete m; return fail(nullptr, ARB_E_CUDA, "arb_create: cannot opt the cable kernels into large shared memory"); }
     int group_ctas = 0;
     if (H.n_groups > 0 && (group_ctas = group_ctas_per_sm(group_smem_plan(H.gcaps).bytes)) == 0) { delete m; return fail(nullptr, ARB_E_INVALID, "arb_create: a cell group does not fit in shared memory"); }
     if (H.n_warp_units > 0 && make_plan(H, 1).warps == 0) { delete m; return fail(nullptr, ARB_E_INVALID, "arb_create: a warp unit does not fit in shared memory"); }
-    {
-      int dev = 0, sms = 0;
-      if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) m->sm_count = sms;
-    }
     auto bail = [&](cudaError_t e, const char* w) { std::string s = std::string(w) + ": " + cudaGetErrorString(e); delete m; return fail(nullptr, ARB_E_CUDA, s); };
     cudaError_t e;
     const Regions& R = m->R;
@@ -287,6 +306,7 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     D.counters = at<unsigned long long>(m, R.counters);
     D.scan_tmp = at<uint32_t>(m, R.scan_tmp);
     D.ena = H.ena; D.ek = H.ek; D.el = H.el; D.theta = H.threshold;
+    D.sm_count = m->sm_count;
     {
       const unsigned long long g0[2] = {(unsigned long long)m->group_grid, (unsigned long long)m->group_grid};
       if ((e = cudaMemcpyAsync(D.counters + CNT_GROUP0, g0, sizeof g0, cudaMemcpyHostToDevice, m->stream)) != cudaSuccess) return bail(e, "upload counters");
@@ -313,18 +333,71 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
   }
 }
 
+}  // extern "C"
+
+namespace {
+
+// Moves the spikes of the device buffer into the host history and empties the buffer.  Only valid at an
+// epoch boundary, after spikes_to_events has walked every spike (CNT_SPIKES_DONE == CNT_SPIKES).  Returns
+// the error bits seen so far in *err_bits.
+int drain(arb_model* m, unsigned long long* cnt) {
+  DevModel& D = m->D;
+  CU(m, cudaMemcpyAsync(cnt, D.counters, sizeof(unsigned long long) * CNT_COUNT, cudaMemcpyDeviceToHost, m->stream));
+  CU(m, cudaStreamSynchronize(m->stream));
+  const size_t n = (size_t)std::min<unsigned long long>(cnt[CNT_SPIKES], (unsigned long long)m->cap.spikes);
+  if (n > 0) {
+    const size_t old = m->sp_cell.size();
+    m->sp_cell.resize(old + n);
+    m->sp_time.resize(old + n);
+    CU(m, cudaMemcpyAsync(m->sp_cell.data() + old, D.spike_cell, 4 * n, cudaMemcpyDeviceToHost, m->stream));
+    CU(m, cudaMemcpyAsync(m->sp_time.data() + old, D.spike_t, 8 * n, cudaMemcpyDeviceToHost, m->stream));
+    CU(m, cudaMemsetAsync(D.counters + CNT_SPIKES, 0, 2 * sizeof(unsigned long long), m->stream));   // CNT_SPIKES, CNT_SPIKES_DONE
+    CU(m, cudaStreamSynchronize(m->stream));
+    m->sp_sorted = false;
+  }
+  return ARB_OK;
+}
+
+int check_error_bits(arb_model* m, const unsigned long long* cnt) {
+  const unsigned long long e = cnt[CNT_ERROR];
+  if (!e) return ARB_OK;
+  m->broken = true;
+  char buf[320];
+  if (e & 8ull) {
+    m->broken_code = ARB_E_DIVERGED;
+    snprintf(buf, sizeof buf, "a detector voltage became NaN / Inf: the time step is too long for the explicit membrane currents (reading R1)");
+  } else {
+    m->broken_code = ARB_E_OVERFLOW;
+    snprintf(buf, sizeof buf, "capacity exceeded:%s%s%s; create the model again with a larger arb_desc.%s (spikes seen %llu of cap_spikes %lld, events in flight %llu of cap_events %lld)",
+             (e & 1) ? " spike buffer" : "", (e & 2) ? " event pool" : "", (e & 4) ? " epoch event list" : "",
+             (e & 1) ? "cap_spikes" : "cap_events", cnt[CNT_SPIKES], (long long)m->cap.spikes,
+             std::max(cnt[CNT_POOL], cnt[CNT_POOL_PEAK]), (long long)m->cap.pool);
+  }
+  return fail(m, m->broken_code, buf);
+}
+
+}  // namespace
+
+extern "C" {
+
 int arb_advance(arb_model* m, double t_end, double dt) {
   if (!m) return fail(nullptr, ARB_E_NULL, "arb_advance: NULL model");
-  if (m->broken) return fail(m, ARB_E_OVERFLOW, "model unusable after an earlier overflow / CUDA error");
+  if (m->broken) return fail(m, m->broken_code, "model unusable after an earlier error: " + m->err);
   if (!(dt > 0) || !std::isfinite(dt) || !std::isfinite(t_end)) return fail(m, ARB_E_INVALID, "arb_advance: dt must be > 0 and finite");
   if (t_end < m->t) return fail(m, ARB_E_INVALID, "arb_advance: t_end earlier than the current time");
   if (m->H.n_conn > 0 && m->H.min_delay < dt) return fail(m, ARB_E_INVALID, "arb_advance: dt longer than the shortest connection delay");
   if (t_end == m->t) return ARB_OK;
   DevModel& D = m->D;
+  // from the first launch on, a failure leaves the device state half-advanced: the model is unusable
+  auto cu_broken = [&](cudaError_t e, const char* where) {
+    m->broken = true; m->broken_code = ARB_E_CUDA;
+    return cuda_fail(m, e, where);
+  };
+#define CUB(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cu_broken(e_, #call); } while (0)
   if (dt != m->factored_dt) {
     D.syn_decay_u = D.syn_uniform ? std::exp(-dt / D.syn_tau_u) : 1.0;
-    CU(m, launch_factor(D, dt, m->stream));
-    CU(m, launch_group_factor(D, dt, m->H.g_seg_cap, m->stream));
+    CUB(launch_factor(D, dt, m->stream));
+    CUB(launch_group_factor(D, dt, m->H.g_seg_cap, m->stream));
     m->factored_dt = dt;
     m->launches++;
   }
@@ -333,7 +406,8 @@ int arb_advance(arb_model* m, double t_end, double dt) {
   int64_t nsteps = (int64_t)std::ceil((t_end - t0) / dt - 1e-9);
   if (nsteps < 1) nsteps = 1;
   const int last_full = std::fabs((t0 + (double)nsteps * dt) - t_end) <= 1e-9 * dt;
-  // epoch: cells are independent for one minimum delay (reading R12)
+  // epoch: cells are independent for one minimum delay (reading R12); the 1e-6 guard is
+  // described in include/arbb200.h (arb_advance)
   int64_t epoch = 1024;
   if (m->H.n_conn > 0) epoch = std::min<int64_t>(epoch, std::max<int64_t>(1, (int64_t)std::floor(m->H.min_delay / dt - 1e-6)));
   if (m->opt_epoch > 0) epoch = std::min(epoch, m->opt_epoch);
@@ -355,8 +429,8 @@ int arb_advance(arb_model* m, double t_end, double dt) {
   const int ggrid = m->opt_group_ctas > 0 ? (int)std::min<int64_t>(m->opt_group_ctas, m->group_grid) : m->group_grid;
   if (ggrid != m->last_ggrid && m->H.n_groups > 0) {
     const unsigned long long g0[2] = {(unsigned long long)ggrid, (unsigned long long)ggrid};
-    CU(m, cudaMemcpyAsync(D.counters + CNT_GROUP0, g0, sizeof g0, cudaMemcpyHostToDevice, m->stream));
-    CU(m, cudaStreamSynchronize(m->stream));
+    CUB(cudaMemcpyAsync(D.counters + CNT_GROUP0, g0, sizeof g0, cudaMemcpyHostToDevice, m->stream));
+    CUB(cudaStreamSynchronize(m->stream));
     m->last_ggrid = ggrid;
   }
   int launches = 0;
@@ -373,14 +447,27 @@ int arb_advance(arb_model* m, double t_end, double dt) {
     }
     return cudaEventRecord(m->tev[n_tev++], m->stream);
   };
+  auto collect_timing = [&]() {
+    for (size_t i = 0; i + 3 < n_tev; i += 4) {
+      float a = 0, b = 0, c = 0;
+      cudaEventElapsedTime(&a, m->tev[i], m->tev[i + 1]);
+      cudaEventElapsedTime(&b, m->tev[i + 1], m->tev[i + 2]);
+      cudaEventElapsedTime(&c, m->tev[i + 2], m->tev[i + 3]);
+      m->cable_ms += b; m->event_ms += a + c;
+      m->cable_timed += tev_cable[i / 4]; m->event_timed += tev_event[i / 4];
+    }
+    n_tev = 0; tev_cable.clear(); tev_event.clear();
+  };
+  unsigned long long cnt[CNT_COUNT];
+  int64_t since_drain = 0;
   for (int64_t k = 0; k < nsteps;) {
     const int64_t n_ep = std::min(epoch, nsteps - k);
     const double t_win = (k + n_ep == nsteps) ? t_end : t0 + (double)(k + n_ep) * dt;
     int l0 = launches;
-    CU(m, stamp());
-    CU(m, launch_build_events(D, m->cur_pool, t_win, m->stream, &launches));
+    CUB(stamp());
+    CUB(launch_build_events(D, m->cur_pool, t_win, m->stream, &launches));
     m->cur_pool ^= 1;
-    CU(m, stamp());
+    CUB(stamp());
     int l1 = launches;
     for (int64_t j = 0; j < n_ep; j += fused) {
       StepArgs A;
@@ -390,64 +477,62 @@ int arb_advance(arb_model* m, double t_end, double dt) {
       A.mark_hot = (A.nk == 1 && m->opt_hot) ? 1 : 0;
       A.hot_valid = m->prev_marked_hot ? 1 : 0;
       m->prev_marked_hot = A.mark_hot != 0;
-      CU(m, launch_group_cable(D, A, ggrid, m->stream, &launches));
-      CU(m, launch_cable(D, A, grid, m->stream, &launches));
+      CUB(launch_group_cable(D, A, ggrid, m->stream, &launches));
+      CUB(launch_cable(D, A, grid, m->stream, &launches));
     }
-    CU(m, stamp());
+    CUB(stamp());
     int l2 = launches;
-    if (m->H.n_conn > 0) CU(m, launch_spikes_to_events(D, m->cur_pool, m->stream, &launches));
-    CU(m, stamp());
+    if (m->H.n_conn > 0) CUB(launch_spikes_to_events(D, m->cur_pool, m->stream, &launches));
+    CUB(stamp());
     tev_cable.push_back(l2 - l1);
     tev_event.push_back((l1 - l0) + (launches - l2));
     k += n_ep;
+    since_drain += n_ep;
+    // the spike buffer is emptied into host memory at the end of the call and at least every kDrainSteps steps
+    if (k == nsteps || since_drain >= kDrainSteps) {
+      int rc = drain(m, cnt);
+      if (rc) { m->broken = true; m->broken_code = rc; return rc; }
+      collect_timing();
+      since_drain = 0;
+      if (cnt[CNT_ERROR]) break;
+    }
   }
   m->launches += launches;
-  unsigned long long cnt[CNT_COUNT];
-  CU(m, cudaMemcpyAsync(cnt, D.counters, sizeof cnt, cudaMemcpyDeviceToHost, m->stream));
-  cudaError_t e = cudaStreamSynchronize(m->stream);
-  if (e != cudaSuccess) { m->broken = true; return cuda_fail(m, e, "arb_advance"); }
-  for (size_t i = 0; i + 3 < n_tev; i += 4) {
-    float a = 0, b = 0, c = 0;
-    cudaEventElapsedTime(&a, m->tev[i], m->tev[i + 1]);
-    cudaEventElapsedTime(&b, m->tev[i + 1], m->tev[i + 2]);
-    cudaEventElapsedTime(&c, m->tev[i + 2], m->tev[i + 3]);
-    m->cable_ms += b; m->event_ms += a + c;
-    m->cable_timed += tev_cable[i / 4]; m->event_timed += tev_event[i / 4];
-  }
   m->t = t_end;
   m->grid_steps += nsteps;
-  if (cnt[CNT_ERROR]) {
-    m->broken = true;
-    char buf[160];
-    snprintf(buf, sizeof buf, "capacity exceeded:%s%s%s", (cnt[CNT_ERROR] & 1) ? " spike buffer" : "",
-             (cnt[CNT_ERROR] & 2) ? " event pool" : "", (cnt[CNT_ERROR] & 4) ? " epoch event list" : "");
-    return fail(m, ARB_E_OVERFLOW, buf);
-  }
-  return ARB_OK;
+  return check_error_bits(m, cnt);
+#undef CUB
 }
 
 int64_t arb_spikes(arb_model* m, int64_t* cell, double* time, int64_t cap) {
   if (!m) return fail(nullptr, ARB_E_NULL, "arb_spikes: NULL model");
   if (cap > 0 && (!cell || !time)) return fail(m, ARB_E_NULL, "arb_spikes: NULL output");
-  unsigned long long n = 0;
-  CU(m, cudaMemcpyAsync(&n, m->D.counters + CNT_SPIKES, 8, cudaMemcpyDeviceToHost, m->stream));
-  CU(m, cudaStreamSynchronize(m->stream));
-  int64_t count = (int64_t)std::min<unsigned long long>(n, (unsigned long long)m->cap.spikes);
+  const int64_t count = (int64_t)m->sp_cell.size();
   if (cap <= 0 || count == 0) return count;
   try {
-    std::vector<uint32_t> c(count);
-    std::vector<double> t(count);
-    CU(m, cudaMemcpyAsync(c.data(), m->D.spike_cell, 4 * (size_t)count, cudaMemcpyDeviceToHost, m->stream));
-    CU(m, cudaMemcpyAsync(t.data(), m->D.spike_t, 8 * (size_t)count, cudaMemcpyDeviceToHost, m->stream));
-    CU(m, cudaStreamSynchronize(m->stream));
-    std::vector<int64_t> idx(count);
-    for (int64_t i = 0; i < count; ++i) idx[i] = i;
-    std::sort(idx.begin(), idx.end(), [&](int64_t a, int64_t b) { return t[a] != t[b] ? t[a] < t[b] : c[a] < c[b]; });
-    for (int64_t i = 0; i < std::min(cap, count); ++i) { cell[i] = c[idx[i]]; time[i] = t[idx[i]]; }
+    if (!m->sp_sorted) {
+      std::vector<int64_t> idx(count);
+      for (int64_t i = 0; i < count; ++i) idx[i] = i;
+      const std::vector<uint32_t>& c = m->sp_cell;
+      const std::vector<double>& t = m->sp_time;
+      std::sort(idx.begin(), idx.end(), [&](int64_t a, int64_t b) { return t[a] != t[b] ? t[a] < t[b] : c[a] < c[b]; });
+      std::vector<uint32_t> c2(count);
+      std::vector<double> t2(count);
+      for (int64_t i = 0; i < count; ++i) { c2[i] = c[idx[i]]; t2[i] = t[idx[i]]; }
+      m->sp_cell.swap(c2); m->sp_time.swap(t2);
+      m->sp_sorted = true;
+    }
+    for (int64_t i = 0; i < std::min(cap, count); ++i) { cell[i] = m->sp_cell[i]; time[i] = m->sp_time[i]; }
   } catch (const std::bad_alloc&) {
     return fail(m, ARB_E_NOMEM, "arb_spikes: out of host memory");
   }
   return count;
+}
+
+int arb_clear_spikes(arb_model* m) {
+  if (!m) return fail(nullptr, ARB_E_NULL, "arb_clear_spikes: NULL model");
+  m->sp_cell.clear(); m->sp_time.clear(); m->sp_sorted = true;
+  return ARB_OK;
 }
 
 int arb_voltage(arb_model* m, double* out, int64_t n_cv) {
@@ -509,6 +594,9 @@ int arb_probe(arb_model* m, int what, double* out, int64_t n) {
         out[12] = (double)m->H.n_groups; out[13] = (double)m->H.n_classes; out[14] = (double)m->group_grid;
         out[15] = (double)m->D.gplan.bytes;
       }
+      if (n >= 20) {
+        out[16] = 0.0; out[17] = (double)(m->H.n_units - m->H.n_warp_units); out[18] = 0.0; out[19] = 0.0;
+      }
       return ARB_OK;
     }
   }
@@ -557,20 +645,6 @@ int arb_set_option(arb_model* m, int key, int64_t value) {
       return ARB_OK;
   }
   return fail(m, ARB_E_INVALID, "arb_set_option: unknown key");
-}
-
-int arb_configure(int key, int64_t value) {
-  if (value < 0) return fail(nullptr, ARB_E_INVALID, "arb_configure: negative value");
-  switch (key) {
-    case ARB_CFG_UNIT_BYTES:
-      if (value != 0 && (value < 1024 || value > 112 * 1024)) return fail(nullptr, ARB_E_INVALID, "arb_configure: unit bytes out of range");
-      g_unit_bytes = value;
-      return ARB_OK;
-    case ARB_CFG_GROUP_MIN_CELLS:
-      g_group_min = value;
-      return ARB_OK;
-  }
-  return fail(nullptr, ARB_E_INVALID, "arb_configure: unknown key");
 }
 
 void arb_destroy(arb_model* m) {

@@ -23,8 +23,6 @@
 //
 // HBM-bound by design: 48 B per control volume and step (V in + out, a, b, f, 1/d) against ~6 fp64
 // instructions.  No tensor cores: nothing here is a dense contraction.
-#include <cstdio>
-
 #include "device_common.cuh"
 #include "group_layout.h"
 #include "kernels.cuh"
@@ -33,22 +31,10 @@ namespace arbb {
 
 namespace {
 
-#ifndef ARBB_CUNROLL
-#define ARBB_CUNROLL 4
-#endif
 constexpr int kT = kGroupThreads;
-constexpr int kCUnroll = ARBB_CUNROLL;    // unrolling of the rhs loop (phase C)
-#ifndef ARBB_ROWS
-#define ARBB_ROWS 8
-#endif
-constexpr int kRows = ARBB_ROWS;                  // rows of a segment a lane group loads ahead of the recurrence
+constexpr int kCUnroll = 4;               // unrolling of the rhs loop (phase C)
+constexpr int kRows = 8;                  // rows of a segment a lane group loads ahead of the recurrence
 
-// -DARBB_PROFILE: one CTA prints clock64() at the phase boundaries of a few group-steps (development aid)
-#ifdef ARBB_PROFILE
-#define TICK(i) do { if (prof) prof[i] = clock64(); } while (0)
-#else
-#define TICK(i) do { } while (0)
-#endif
 
 // Pointers of one group.  "s" pointers address the CTA's shared memory, "g" pointers global memory.
 // Rarely used arrays (clamps, non-uniform synapse parameters, the dt-independent "gen" arrays of
@@ -275,13 +261,12 @@ __device__ __forceinline__ void forward_stage(const GView& U, uint32_t st, int h
 // Stages [n_block, n_stage) only use the lane groups of warp 0: it runs them back to back, backward
 // and then forward, with warp barriers only.
 __device__ __forceinline__ void sweeps(const GView& U, int h, int c, bool on, const double* F, const double* I,
-                                       double* Vs, double* con, long long* prof) {
+                                       double* Vs, double* con) {
   const uint32_t n_stage = U.n_stage, n_block = U.n_block;
   for (uint32_t st = 0; st < n_block; ++st) {
     backward_stage(U, st, h, c, on, F, I, Vs, con);
     __syncthreads();
   }
-  TICK(8);
   if (threadIdx.x < 32) {
     for (uint32_t st = n_block; st < n_stage; ++st) {
       backward_stage(U, st, h, c, on, F, I, Vs, con);
@@ -292,12 +277,10 @@ __device__ __forceinline__ void sweeps(const GView& U, int h, int c, bool on, co
       __syncwarp();
     }
   }
-  TICK(9);
   for (uint32_t st = n_block; st-- > 0;) {
     __syncthreads();
     forward_stage(U, st, h, c, on, F, Vs);
   }
-  TICK(10);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -350,14 +333,12 @@ __device__ __forceinline__ void run_deferred(HHDefer& dh, double* dst0, double* 
 template <bool kGen>
 __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U, double* Vs, const double* Fs, const double* Is,
                                               double* buf, const CellS& cs, double dt, HHDefer& dh, double vprev, double tstart,
-                                              const uint8_t* fg, uint32_t vbytes, uint64_t* mbarB, uint32_t& parB, long long* prof) {
+                                              const uint8_t* fg, uint32_t vbytes, uint64_t* mbarB, uint32_t& parB) {
   const int tid = threadIdx.x, c = tid % kG, h = tid / kG;
   const int rtid = kT - 1 - tid, rc = rtid % kG;      // reversed dealing of instances; cell of those
   const uint32_t nE_cv = gcv_elems(U.n_cv), nE_hh = U.n_hh * kG, nE_syn = U.n_syn * kG, nE_cl = U.n_cl * kG;
   const uint32_t md = kGen ? cs.mode[c] : 1u, rmd = kGen ? cs.mode[rc] : 1u;
   const double delta = kGen ? cs.delta[c] : dt, rdelta = kGen ? cs.delta[rc] : dt;
-
-  TICK(17);
   // ---- B: currents of HH, synapses and clamps from V(t); the passive current is
   // folded into a, b.  Items of one cell on one CV form a run; its first item sums it in index order.
   double* xI = buf;
@@ -370,7 +351,6 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
     xI[e] = U.hh_gna[e] * m * m * m * hh * (v - M.ena) + U.hh_gna[e + U.hh_cs] * n * n * n * n * (v - M.ek) +
             U.hh_gna[e + 2 * U.hh_cs] * (v - M.el);
   }
-  TICK(18);
 #pragma unroll 1
   for (uint32_t e = rtid; e < nE_syn; e += kT) {
     const uint32_t slot = U.syn_slot[e];
@@ -385,7 +365,6 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
     } while (j < nE_syn && U.syn_slot[j] == slot);
     xI[nE_hh + e] = I;
   }
-  TICK(3);
   if (nE_cl) {
     const double t = kGen ? cs.tcur[rc] : tstart;
     const uint16_t* cl_slot = U.cl_slot();
@@ -404,7 +383,6 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
     }
   }
   __syncthreads();
-  TICK(4);
 
   // ---- C: rhs_i = (C_i/delta - G_i) V_i + G_i e_i - I_i, in place of V; positions, not
   // (slot, cell) pairs: every per-CV array of the group uses the same positions
@@ -430,9 +408,7 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
       for (uint32_t p = tid; p < nE_cv; p += kT) Vr[p] = fma(fma(rm1, C[p] / dt, ar[p]), Vr[p], br[p]);
     }
   }
-  TICK(5);
   __syncthreads();
-  TICK(6);
   // a, b are dead: the same two buffers now receive the solver factors f, 1/d (L2, prefetched) while
   // the point currents are subtracted
   if (tid == 0) {
@@ -474,8 +450,6 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
     if (!disjoint) __syncthreads();
   }
   if (disjoint && (nE_hh | nE_syn | nE_cl)) __syncthreads();
-
-  TICK(7);
   mbar_wait(mbarB, parB);
   parB ^= 1u;
   // ---- event-split sub-steps: this cell's matrix is re-eliminated for its own delta (reading R9); its
@@ -495,9 +469,8 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
   }
 
   // ---- D: backward sweep, stage by stage; E: forward substitution, stages reversed; V <- V'
-  sweeps(U, h, c, kGen ? md != 0u : true, Fs, Is, Vs, buf, prof);   // buf: xI is dead, it now holds the contributions
+  sweeps(U, h, c, kGen ? md != 0u : true, Fs, Is, Vs, buf);   // buf: xI is dead, it now holds the contributions
   __syncthreads();
-  TICK(11);
 
   // ---- F: state update with V', threshold test
   {
@@ -536,6 +509,7 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
   if (tid < kG && md) {
     const double vd = Vs[gpos(U.det_slot[tid], tid)], vp = kGen ? cs.vprev[tid] : vprev;
     if ((uint32_t)tid < U.n_cell) {
+      if (!isfinite(vd)) atomicOr(&M.counters[CNT_ERROR], 8ull);
       if (vp < M.theta && M.theta <= vd && cs.armed[tid]) {
         const double ts = (kGen ? cs.tcur[tid] : tstart) + (kGen ? cs.delta[tid] : dt) * (M.theta - vp) / (vd - vp);
         const unsigned long long pos = atomicAdd(&M.counters[CNT_SPIKES], 1ull);
@@ -547,7 +521,6 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
     }
     if (kGen) cs.tcur[tid] = cs.tnext[tid];
   }
-  TICK(12);
 }
 
 // Work item -> group.  Items [0, n_hot) are the groups of this launch's hot list (an event falls into
@@ -607,21 +580,7 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
   clear(dh);
   double* dh_gm = nullptr;               // where the carried gate update of the previous group goes
   uint32_t dh_ss = 0;
-#ifdef ARBB_PROFILE
-  long long prof_buf[24];
-  unsigned long long gt0;
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt0));
-  const long long ck0 = clock64();
-  int prof_ngen = 0;
-  unsigned long long prof_gen_ns = 0;
-#endif
-  long long* prof = nullptr;
   for (int64_t g = sG[0]; g < M.n_groups; g = sG[(++it) & 1u]) {
-#ifdef ARBB_PROFILE
-    prof = (blockIdx.x == 7 && tid == 0 && it >= 1 && it <= 3 && A.k_first == 150) ? prof_buf : nullptr;
-    if (prof) for (int i = 0; i < 24; ++i) prof[i] = 0;
-#endif
-    TICK(0);
     const GroupDesc& D = sD[it & 1u];
     const GConstOff co = gconst_offsets(D.n_cv, D.n_hh_rows, D.n_syn_rows, D.n_cl_rows, M.syn_uniform != 0);
     const GStateOff so = gstate_offsets(D.n_cv, D.n_hh_rows, D.n_syn_rows);
@@ -672,7 +631,6 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
     // the previous group's last gate update: registers -> global m, h, n, while the copies are in flight
     run_deferred(dh, dh_gm, nullptr, dh_ss);
     dh_gm = U.gm; dh_ss = U.hh_ss;
-    TICK(1);
     mbar_wait(mbar, it & 1u);
     if (tid < kG) {
       const unsigned long long pk = (unsigned long long)__double_as_longlong(U.srt[kRtDoubles * tid + 1]);
@@ -680,7 +638,6 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
       cs.armed[tid] = U.srt[kRtDoubles * tid + 2] != 0.0 ? 1u : 0u;
     }
     __syncthreads();
-    TICK(2);
 
     for (int64_t k = A.k_first; k < A.k_first + A.nk; ++k) {
       const double ta = (k == 0) ? A.t0 : __dadd_rn(A.t0, __dmul_rn((double)k, A.dt));
@@ -704,7 +661,7 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
         run_deferred(dh, U.sm, U.gm, U.hh_ss);
         if (!ab_ready) reload_ab();
         ab_ready = false;
-        group_substep<false>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, vprev, ta, M.fast + D.const_off + co.f, vbytes, mbar + 1, par2, prof);
+        group_substep<false>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, vprev, ta, M.fast + D.const_off + co.f, vbytes, mbar + 1, par2);
         __syncthreads();                  // flags are rewritten by the next grid step
         continue;
       }
@@ -742,24 +699,14 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
           const unsigned ba = __ballot_sync(kFull, active), bg = __ballot_sync(kFull, gen), bs = __ballot_sync(kFull, split);
           if (tid == 0) { flags[0] = ba; flags[1] = bg; flags[2] = bs; }
         }
-        TICK(15);
         __syncthreads();                  // also orders the delivered g += w before phase B
-        TICK(16);
         if (!flags[0]) break;
         // another (sub-)step follows: the gates of the previous one are needed now (working copy and global)
         run_deferred(dh, U.sm, U.gm, U.hh_ss);
         if (!ab_ready) reload_ab();
         ab_ready = false;
         {                                 // (all cells nominal only after events delivered exactly at the step start)
-#ifdef ARBB_PROFILE
-          unsigned long long ga, gb;
-          asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(ga));
-#endif
-          group_substep<true>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, 0.0, 0.0, M.fast + D.const_off + co.f, vbytes, mbar + 1, par2, prof);
-#ifdef ARBB_PROFILE
-          asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gb));
-          ++prof_ngen; prof_gen_ns += gb - ga;
-#endif
+          group_substep<true>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, 0.0, 0.0, M.fast + D.const_off + co.f, vbytes, mbar + 1, par2);
         }
         __syncthreads();
       }
@@ -767,7 +714,6 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
     }
 
     // ---- V', g, per-cell runtime -> HBM (one bulk store); the gates follow from registers
-    TICK(13);
     if (tid < kG) {
       const unsigned long long pk = ((unsigned long long)cs.evend[tid] << 32) | cs.evcur[tid];
       U.srt[kRtDoubles * tid + 1] = __longlong_as_double((long long)pk);
@@ -797,23 +743,8 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
       bulk_wait_read0();
     }
     __syncthreads();                      // shared memory may be overwritten by the next group's copies
-    TICK(14);
-#ifdef ARBB_PROFILE
-    if (prof) {
-      printf("grp %lld:", (long long)g);
-      for (int i = 1; i < 24; ++i) printf(" %d:%lld", i, prof[i] ? prof[i] - prof[0] : -1ll);
-      printf("\n");
-    }
-#endif
   }
   run_deferred(dh, dh_gm, nullptr, dh_ss);
-#ifdef ARBB_PROFILE
-  unsigned long long gt1;
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt1));
-  if (tid == 0 && A.k_first >= 150 && A.k_first < 153 && (gt1 - gt0 > 110000 || blockIdx.x == 0)) {
-    printf("k %d cta %d: dur %llu ns, %u groups, %d general passes, gen ns %llu\n", (int)A.k_first, (int)blockIdx.x, gt1 - gt0, it, prof_ngen, prof_gen_ns);
-  }
-#endif
   if (tid < 32) {
     for (int o = 16; o; o >>= 1) { n_sub += __shfl_xor_sync(kFull, n_sub, o); n_del += __shfl_xor_sync(kFull, n_del, o); }
     if (tid == 0) {
@@ -881,15 +812,18 @@ __global__ void __launch_bounds__(kGroupThreads) group_init_kernel(DevModel M) {
 }  // namespace
 
 // Resident CTAs of the group kernel per SM for `smem_bytes` of dynamic shared memory (asks the
-// runtime; also opts the kernel into that much shared memory).  0: does not fit / no device.
+// runtime; configure_kernels() has opted the kernel in).  0: does not fit / no device.
+cudaError_t configure_group_kernel(int max_optin_bytes) {
+  cudaFuncAttributes fa;
+  cudaError_t e = cudaFuncGetAttributes(&fa, cable_group_kernel);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(cable_group_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_optin_bytes - (int)fa.sharedSizeBytes);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(cable_group_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+}
+
 int group_ctas_per_sm(uint32_t smem_bytes) {
-  if (smem_bytes + 1024u > 227u * 1024u) return 0;
-  static uint32_t opted_in = 0;           // the attribute is per kernel, not per model: never lower it
-  if (smem_bytes > opted_in) {
-    if (cudaFuncSetAttribute(cable_group_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes) != cudaSuccess) return 0;
-    opted_in = smem_bytes;
-  }
-  cudaFuncSetAttribute(cable_group_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  if (smem_bytes + 1024u > (uint32_t)cable_smem_limit()) return 0;
   int n = 0;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, cable_group_kernel, kGroupThreads, smem_bytes) != cudaSuccess) return 0;
   return n;

@@ -32,20 +32,11 @@
 
 namespace arbb {
 
-#ifndef ARBB_G
-#define ARBB_G 4
-#endif
-#ifndef ARBB_GROUP_WARPS
-#define ARBB_GROUP_WARPS 4
-#endif
-#ifndef ARBB_GROUP_MIN_CTAS
-#define ARBB_GROUP_MIN_CTAS 4
-#endif
-constexpr int kG = ARBB_G;                    // cells per group = lanes per lane group (4, 8, 16 or 32)
+constexpr int kG = 4;                         // cells per group = lanes per lane group (4, 8, 16 or 32)
 constexpr int kLaneGroups = 32 / kG;          // lane groups per warp
-constexpr int kGroupWarps = ARBB_GROUP_WARPS; // warps per CTA of the group kernel
+constexpr int kGroupWarps = 4;                // warps per CTA of the group kernel
 constexpr int kGroupThreads = kGroupWarps * 32;
-constexpr int kGroupMinCtas = ARBB_GROUP_MIN_CTAS;      // resident CTAs per SM the kernel is compiled for
+constexpr int kGroupMinCtas = 4;              // resident CTAs per SM the kernel is compiled for
 constexpr int kGroupSlots = kGroupWarps * kLaneGroups;   // chunks a stage can run concurrently
 constexpr uint16_t kNoSlot16 = 0xFFFFu;
 constexpr uint32_t kGroupMaxCv = 65000;       // slots are stored as uint16

@@ -24,10 +24,7 @@ namespace arbb {
 
 namespace {
 
-#ifndef ARBB_BLOCK_THREADS
-#define ARBB_BLOCK_THREADS 128
-#endif
-constexpr int kBlockThreads = ARBB_BLOCK_THREADS;              // cable_block_kernel, factor_kernel, init_kernel
+constexpr int kBlockThreads = 128;              // cable_block_kernel, factor_kernel, init_kernel
 constexpr int kBlockWarps = kBlockThreads / 32;
 constexpr uint32_t kSynKeyReduceMin = 1024;     // block units with at least this many synapses reduce currents by key
 constexpr int kMaxWarpsPerCta = 8;              // cable_warp_kernel
@@ -322,10 +319,7 @@ __device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, co
     // reduces them by key = control volume with shuffles (the "key reduction" of PAPER.md:218; runs are
     // contiguous), and the first lane of every key inside the chunk stores a partial sum; in phase C the run
     // heads add the partials of the chunks their run extends into, in index order (no atomics).
-#ifndef ARBB_KCH
-#define ARBB_KCH 2
-#endif
-    constexpr int kCh = ARBB_KCH;        // chunks per warp and trip: independent loads in flight
+    constexpr int kCh = 2;               // chunks per warp and trip: independent loads in flight
     for (uint32_t base = (uint32_t)S::warp() * 32u * kCh; base < n_syn; base += (uint32_t)S::warps * 32u * kCh) {
       uint32_t slot[kCh];
       double term[kCh];
@@ -500,6 +494,7 @@ __device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, co
   }
   if ((uint32_t)tid < U.n_cell && (!kGen || cs.mode[tid])) {
     const double vd = U.V[U.cell_det[tid]], vp = cs.vprev[tid];
+    if (!isfinite(vd)) atomicOr(&M.counters[CNT_ERROR], 8ull);
     if (cs.armed[tid] && vp < M.theta && M.theta <= vd) {
       const double ts = cs.tcur[tid] + cs.delta[tid] * (M.theta - vp) / (vd - vp);
       const unsigned long long pos = atomicAdd(&M.counters[CNT_SPIKES], 1ull);
@@ -672,10 +667,8 @@ __device__ __forceinline__ void block_view(UnitView& U, const DevModel& M, const
   U.heads = (uint32_t*)(U.invdgen + H.n_slot);
 }
 
-#ifndef ARBB_BLOCK_MIN_CTAS
-#define ARBB_BLOCK_MIN_CTAS 16   // latency-bound out of L2: full occupancy beats registers (measured 1..16 x 64..256 threads)
-#endif
-__global__ void __launch_bounds__(kBlockThreads, ARBB_BLOCK_MIN_CTAS) cable_block_kernel(DevModel M, StepArgs A) {
+constexpr int kBlockMinCtas = 16;   // latency-bound out of L2: full occupancy beats registers (measured 1..16 x 64..256 threads)
+__global__ void __launch_bounds__(kBlockThreads, kBlockMinCtas) cable_block_kernel(DevModel M, StepArgs A) {
   __shared__ UnitHeader H;
   __shared__ __align__(16) uint8_t cell_mem[kCellScratchBytes * kBlockUnitMaxCells];
   const UnitDesc d = M.units[M.n_warp_units + blockIdx.x];
@@ -779,6 +772,7 @@ __global__ void __launch_bounds__(256) spikes_to_events_kernel(DevModel M, int c
 }
 
 __global__ void spikes_done_kernel(DevModel M) {
+  if (M.counters[CNT_POOL] > M.counters[CNT_POOL_PEAK]) M.counters[CNT_POOL_PEAK] = M.counters[CNT_POOL];
   M.counters[CNT_SPIKES_DONE] = M.counters[CNT_SPIKES] < (unsigned long long)M.spike_cap ? M.counters[CNT_SPIKES] : (unsigned long long)M.spike_cap;
   if (M.counters[CNT_POOL] > (unsigned long long)M.pool_cap) M.counters[CNT_POOL] = (unsigned long long)M.pool_cap;
 }
@@ -921,7 +915,18 @@ inline unsigned grid_for(int64_t n, int block) { return (unsigned)((n + block - 
 
 }  // namespace
 
-int cable_smem_limit() { return 227 * 1024; }
+int cable_smem_limit() { return 227 * 1024; }   // sm_100a: opt-in maximum of dynamic shared memory per CTA
+
+cudaError_t configure_kernels() {
+  int dev = 0, optin = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(cable_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+  if (e != cudaSuccess) return e;
+  return configure_group_kernel(optin);
+}
 int cable_max_warps() { return kMaxWarpsPerCta; }
 
 cudaError_t launch_factor(const DevModel& M, double dt, cudaStream_t s) {
@@ -943,13 +948,7 @@ cudaError_t launch_reset_detectors(const DevModel& M, cudaStream_t s) {
 
 cudaError_t launch_cable(const DevModel& M, const StepArgs& A, int grid, cudaStream_t s, int* launches) {
   if (M.n_warp_units > 0) {
-    const int smem = (int)(M.plan.warps * M.plan.warp_bytes);
-    static int configured = -1;
-    if (smem > 48 * 1024 && configured < smem) {
-      cudaError_t e = cudaFuncSetAttribute(cable_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-      if (e != cudaSuccess) return e;
-      configured = smem;
-    }
+    const int smem = (int)(M.plan.warps * M.plan.warp_bytes);   // configure_kernels() has opted the kernel in
     cable_warp_kernel<<<(unsigned)grid, (unsigned)(M.plan.warps * 32), smem, s>>>(M, A);
     if (launches) ++*launches;
   }
@@ -964,11 +963,12 @@ cudaError_t launch_build_events(const DevModel& M, int cur, double t_win, cudaSt
   const unsigned gc = grid_for(M.n_cells, 256);
   const int64_t nb = (M.n_cells + kScanBlock - 1) / kScanBlock;
   ev_count_ext_kernel<<<gc, 256, 0, s>>>(M, t_win);
-  ev_count_pool_kernel<<<592, 256, 0, s>>>(M, cur, t_win);
+  const unsigned gp = (unsigned)(4 * M.sm_count);      // grid-stride loops over the pool: four CTAs per SM
+  ev_count_pool_kernel<<<gp, 256, 0, s>>>(M, cur, t_win);
   scan_local_kernel<<<(unsigned)nb, kScanBlock, 0, s>>>(M.ev_fill, M.ev_off, M.scan_tmp, M.n_cells);
   scan_sums_kernel<<<1, 32, 0, s>>>(M.scan_tmp, nb, M, M.n_cells);
   ev_place_kernel<<<gc, 256, 0, s>>>(M, t_win);
-  ev_scatter_pool_kernel<<<592, 256, 0, s>>>(M, cur, t_win);
+  ev_scatter_pool_kernel<<<gp, 256, 0, s>>>(M, cur, t_win);
   ev_sort_kernel<<<gc, 256, 0, s>>>(M);
   pool_swap_kernel<<<1, 1, 0, s>>>(M);
   if (launches) *launches += 8;
@@ -976,7 +976,7 @@ cudaError_t launch_build_events(const DevModel& M, int cur, double t_win, cudaSt
 }
 
 cudaError_t launch_spikes_to_events(const DevModel& M, int cur, cudaStream_t s, int* launches) {
-  spikes_to_events_kernel<<<296, 256, 0, s>>>(M, cur);
+  spikes_to_events_kernel<<<(unsigned)(2 * M.sm_count), 256, 0, s>>>(M, cur);
   spikes_done_kernel<<<1, 1, 0, s>>>(M);
   if (launches) *launches += 2;
   return cudaGetLastError();

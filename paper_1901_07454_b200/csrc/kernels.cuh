@@ -13,7 +13,7 @@ enum Counter {
   CNT_SPIKES_DONE = 1,  // spikes already turned into events
   CNT_POOL = 2,         // events waiting in the current pool
   CNT_POOL_NEXT = 3,    // events carried over into the other pool
-  CNT_ERROR = 4,        // bit 0 spike overflow, bit 1 pool overflow, bit 2 epoch list overflow
+  CNT_ERROR = 4,        // bit 0 spike overflow, bit 1 pool overflow, bit 2 epoch list overflow, bit 3 non-finite voltage
   CNT_SUBSTEPS = 5,     // cell sub-steps executed
   CNT_DELIVERED = 6,    // events delivered
   CNT_EVLIST = 7,       // size of the current epoch list
@@ -22,7 +22,8 @@ enum Counter {
   CNT_HOT0 = 10,        // group kernel: lengths of the three rotating "hot" lists (groups with an event in
   CNT_HOT1 = 11,        //   the next grid step, which are integrated first so that their longer
   CNT_HOT2 = 12,        //   event-split steps do not end up at the tail of the launch)
-  CNT_COUNT = 13
+  CNT_POOL_PEAK = 13,   // largest number of events in flight asked of the pool so far (also beyond its capacity)
+  CNT_COUNT = 14
 };
 
 struct EventPool { double* t; uint32_t* dst; uint32_t* gidx; double* w; };
@@ -67,6 +68,7 @@ struct DevModel {
   int64_t n_groups;
   GroupSmemPlan gplan;
   int l2_prefetch;            // group kernel: TMA-prefetch the next group's records into L2
+  int sm_count;               // SMs of the device the model lives on (grid sizing)
   uint32_t* ghot;             // group kernel: three lists of n_groups entries (see CNT_HOT0)
   uint32_t* ghotflag;         // [2][n_groups], half launch_id & 1: launch_id of the launch whose hot list holds the group
 };
@@ -100,6 +102,10 @@ cudaError_t launch_group_factor(const DevModel& M, double dt, uint32_t seg_cap, 
 cudaError_t launch_group_init(const DevModel& M, cudaStream_t s);
 cudaError_t launch_group_cable(const DevModel& M, const StepArgs& A, int grid, cudaStream_t s, int* launches);
 int group_ctas_per_sm(uint32_t smem_bytes);   // resident CTAs of the group kernel per SM (0: does not fit)
+// Opts the cable kernels into the device's full dynamic shared memory on the CURRENT device (the
+// attribute is per function and device; called by every arb_create, nothing is cached).
+cudaError_t configure_kernels();
+cudaError_t configure_group_kernel(int max_optin_bytes);
 int cable_smem_limit();       // bytes of dynamic shared memory a CTA of the warp kernel may use
 int cable_max_warps();        // warps per CTA the warp kernel is compiled for
 

@@ -32,9 +32,9 @@ def B():
 def layout(request, B):
     """Every test runs under three layouts: the default (cells of a topology class of >= 4 cells in
     cell-interleaved groups, the rest in branch-interleaved units), every cell in groups, no groups."""
-    B.configure(B.ARB_CFG_GROUP_MIN_CELLS, {"default": 0, "groups": 1, "units": 2 ** 31}[request.param])
+    B.LAYOUT_DEFAULTS["layout_group_min_cells"] = {"default": 0, "groups": 1, "units": 2 ** 31}[request.param]
     yield request.param
-    B.configure(B.ARB_CFG_GROUP_MIN_CELLS, 0)
+    B.LAYOUT_DEFAULTS.clear()
 
 
 def rel(a, b):
@@ -415,47 +415,157 @@ def test_spike_buffer_cap_and_order(B, orc):
 
 
 # ---------------------------------------------------------------------------------------------
-# full-size configuration, sampled cells
+# full-size configurations: the WHOLE network against the oracle, in the launch configuration
+# bench.py times (one launch per grid step, groups with events first)
 # ---------------------------------------------------------------------------------------------
-def test_full_size_large_config_sampled_cells(B, orc, layout):
-    """configs[3] at its full 100,000 cells, in the launch configuration bench.py times.  Until the
-    first network event can arrive (one minimum delay, 5 ms = 200 steps) every cell depends only on
-    its own external events, so the oracle can integrate a sample of cells on its own."""
+FREE_RUN_TOL = 1e-7     # free-running V, gates over several hundred steps of a spiking network (R16/R17)
+
+
+def expected_deliveries(m, spikes, t_end):
+    """Events delivered before t_end: external ones plus (spike + delay) of every out-connection."""
+    sc, st = spikes
+    n = int(np.count_nonzero(m["ext_time"] < t_end))
+    if len(sc) and m["n_conn"]:
+        order = np.argsort(m["conn_src"], kind="stable")
+        src, dly = m["conn_src"][order], m["conn_delay"][order]
+        lo, hi = np.searchsorted(src, sc, "left"), np.searchsorted(src, sc, "right")
+        for a, b, ts in zip(lo, hi, st):
+            n += int(np.count_nonzero(ts + dly[a:b] < t_end))
+    return n
+
+
+def whole_network(B, orc, m, t_end, min_spikes=0, calls=1):
+    import os
+    g = B.Model(m)
+    g.set_option(B.ARB_OPT_FUSED_STEPS, 1)
+    g.set_option(B.ARB_OPT_HOT_FIRST, 1)
+    o = orc.Oracle(m, threads=os.cpu_count() or 4)
+    for i in range(calls):
+        g.advance(t_end * (i + 1) / calls, m["dt"])
+    o.advance(t_end, m["dt"])
+    n = check_spikes(g, o, m["n_cells"])
+    assert n >= min_spikes, n
+    assert tuple(g.probe(B.ARB_PROBE_NSTEPS)) == tuple(o.probe(orc.PROBE_NSTEPS))
+    assert g.stats()["events_delivered"] == expected_deliveries(m, o.spikes(), t_end)
+    check_state(g, o, FREE_RUN_TOL, "t=%g" % t_end)
+    st = g.stats()
+    g.close()
+    o.close()
+    return n, st
+
+
+def test_full_size_c3_whole_network(B, orc, layout):
+    """configs[3] at its full 100,000 cells (5.05e7 CVs), driven, stated weights, three epochs (600 steps): every
+    cell's V, m, h, n, g, the spikes, the sub-step count and the number of delivered events against the oracle
+    on the whole network.  Then the same network with weights x 4 so that it fires within the first epoch and
+    network events (5e6 connections, pool carry-over between epochs) are delivered in the second and third."""
     if layout != "default":
         pytest.skip("full size runs once, in the layout bench.py times")
-    m = W.config3()
-    g = B.Model(m)
-    g.advance(5.0, DT)
-    sample = np.array([0, 1, 7, 4242, 31337, 65535, 77777, 99998, 99999])
-    sub = W.take_cells(m, sample)
-    o = orc.Oracle(sub)
-    o.advance(5.0, DT)
-    v = g.voltage()
-    vs = np.concatenate([v[m["cv_off"][c]:m["cv_off"][c + 1]] for c in sample])
-    assert rel(vs, o.voltage()) <= 1e-10
-    gg = g.syn_g()
-    gs = np.concatenate([gg[m["syn_off"][c]:m["syn_off"][c + 1]] for c in sample])
-    assert rel_pure(gs, o.syn_g()) <= 1e-10
-    # properties that hold at any size
-    assert np.all(np.isfinite(v)) and v.min() > -90 and v.max() < 60
-    steps = g.probe(B.ARB_PROBE_NSTEPS)
-    st = g.stats()
-    # every cell of configs[3] has the same tree: one class, all cells in cell-interleaved groups
+    m = W.config3(t_end=15.0)
+    n, st = whole_network(B, orc, m, 15.0, calls=3)
     assert st["classes"] == 1 and st["units"] == 0 and st["groups"] * 4 >= m["n_cells"] and st["group_ctas"] >= 148
-    delivered = st["events_delivered"]
-    assert steps[0] == 200 and delivered == int(np.sum(m["ext_time"] < 5.0))
-    assert steps[1] >= 200 * m["n_cells"]
-    # the same epoch with one launch per grid step (what bench.py times: dynamic claiming, groups with
-    # events first) must give the same bits: every group is integrated exactly once per step
-    g2 = B.Model(m)
-    g2.set_option(B.ARB_OPT_FUSED_STEPS, 1)
-    g2.advance(5.0, DT)
-    assert tuple(g2.probe(B.ARB_PROBE_NSTEPS)) == tuple(steps)
-    assert g2.stats()["events_delivered"] == delivered
-    assert np.array_equal(g2.voltage(), v) and np.array_equal(g2.syn_g(), gg)
-    for a, b in zip(g2.spikes(), g.spikes()):
-        assert np.array_equal(a, b)
-    g2.close()
+    m["conn_weight"] = m["conn_weight"] * 4
+    m["ext_weight"] = m["ext_weight"] * 4
+    n, st = whole_network(B, orc, m, 15.0, min_spikes=10000)
+    assert st["events_delivered"] > int(np.count_nonzero(m["ext_time"] < 15.0)) + 100000    # network events arrived
+
+
+def test_full_size_c4_whole_network(B, orc, layout):
+    """configs[4] at its full 50,000 cells (1.56e7 CVs, every tree different), two epochs."""
+    if layout != "default":
+        pytest.skip("full size runs once, in the layout bench.py times")
+    m = W.config4(t_end=10.0)
+    whole_network(B, orc, m, 10.0, calls=2)
+
+
+def test_full_size_c1_whole_run(B, orc, layout):
+    """configs[1] at full size for its whole 200 ms (8,000 steps): the ring spike travels through 39 cells."""
+    if layout != "default":
+        pytest.skip("full size runs once, in the layout bench.py times")
+    m = W.config1()
+    n, _ = whole_network(B, orc, m, 200.0, min_spikes=30)
+
+
+def test_full_size_c2_100ms(B, orc, layout):
+    """configs[2] at full size (10,000 cells, 1e6 connections, 2e6 Poisson events per second): first 100 ms."""
+    if layout != "default":
+        pytest.skip("full size runs once, in the layout bench.py times")
+    m = W.config2(t_end=100.0)
+    whole_network(B, orc, m, 100.0)
+
+
+# ---------------------------------------------------------------------------------------------
+# capacities and error paths (include/arbb200.h "Capacities")
+# ---------------------------------------------------------------------------------------------
+def _firing_net(t_end=40.0):
+    m = W.config1(n_cells=30, t_end=t_end)
+    return m
+
+
+def test_spike_buffer_overflow_is_reported(B, orc):
+    m = _firing_net()
+    m["cap_spikes"] = 2
+    g = B.Model(m)
+    with pytest.raises(B.ArbError) as e:
+        g.advance(40.0, DT)
+    assert e.value.code == B.ARB_E_OVERFLOW and "cap_spikes" in str(e.value)
+    with pytest.raises(B.ArbError) as e:          # unusable afterwards, same code
+        g.advance(41.0, DT)
+    assert e.value.code == B.ARB_E_OVERFLOW
+    g.close()
+
+
+def test_spike_buffer_is_drained_between_calls(B, orc):
+    """A device spike buffer of 2 entries is enough when it is drained often enough: the history lives in
+    host memory, arb_spikes stays cumulative, arb_clear_spikes empties it."""
+    m = _firing_net()
+    m["cap_spikes"] = 2
+    g, o = B.Model(m), orc.Oracle(m)
+    for k in range(1, 9):
+        g.advance(5.0 * k, DT)
+    o.advance(40.0, DT)
+    assert check_spikes(g, o, 30) >= 6
+    g.clear_spikes()
+    assert len(g.spikes()[0]) == 0
+    g.close()
+
+
+def test_event_pool_overflow_is_reported(B, orc):
+    m = W.config3(n_cells=60, t_end=30.0)
+    m["conn_weight"] = m["conn_weight"] * 4
+    m["ext_weight"] = m["ext_weight"] * 4
+    m["cap_events"] = 8
+    g = B.Model(m)
+    with pytest.raises(B.ArbError) as e:
+        g.advance(30.0, DT)
+    assert e.value.code == B.ARB_E_OVERFLOW and "cap_events" in str(e.value) and "event pool" in str(e.value)
+    g.close()
+    # the default capacity takes the same run
+    del m["cap_events"]
+    g, o = run_both(B, orc, m, 30.0)
+    assert check_spikes(g, o, 60) > 5
+    g.close()
+
+
+def test_long_delays_fit_the_default_pool(B, orc):
+    """Delays of 40 ms against 5 ms inter-spike intervals: several events per connection in flight."""
+    m = W.config1(n_cells=8, t_end=150.0)
+    m["conn_delay"] = np.full(m["n_conn"], 40.0)
+    m["clamp_cell"], m["clamp_cv"] = np.array([0]), np.array([0], np.int32)
+    m["clamp_t0"], m["clamp_t1"], m["clamp_amp"] = np.array([0.0]), np.array([150.0]), np.array([0.4])
+    m = W.finalize(m)
+    g, o = run_both(B, orc, m, 150.0)
+    assert check_spikes(g, o, 8) > 10
+    g.close()
+
+
+def test_divergence_is_reported(B):
+    """dt = 1 ms on the HH soma: the explicit membrane currents (reading R1) blow up; the oracle ends in NaN
+    too.  The library reports it instead of returning garbage."""
+    g = B.Model(W.config0())
+    with pytest.raises(B.ArbError) as e:
+        g.advance(100.0, 1.0)
+    assert e.value.code == B.ARB_E_DIVERGED
     g.close()
 
 

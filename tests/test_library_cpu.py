@@ -22,7 +22,7 @@ def B():
 
 def test_exports_match_header(B):
     header = open(os.path.join(ROOT, "include", "arbb200.h")).read()
-    declared = set(re.findall(r"\b(arb_[a-z_]+)\s*\(", header))
+    declared = set(re.findall(r"\b(arb_[a-z0-9_]+)\s*\(", header))
     assert declared == set(B.EXPORTS)
     for name in declared:
         assert hasattr(B.lib(), name), name
