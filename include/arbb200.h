@@ -56,8 +56,9 @@ enum {
                                 through HBM every step); 0 (default) = a whole min-delay epoch
                                 (cells are independent within Delta_T)           */
   ARB_OPT_EPOCH_STEPS = 2,   /* cap on the epoch length in steps (default: floor(min delay / dt)) */
-  ARB_OPT_STAGES = 4,        /* shared-memory stages per warp of the cable kernel: 0 (default) = 2 when
-                                every launch streams the state once, 1 when launches are fused     */
+  ARB_OPT_OVERLAP = 4,       /* 1 (default): the cable kernels of one grid step (cell groups, forests by launch
+                                class, block units) run side by side on streams forked from the model's
+                                stream; 0: one after the other on the model's stream               */
   ARB_OPT_L2_PREFETCH = 5,   /* cell-group kernel: 1 (default) = ask the TMA unit to pull the next group's
                                 records into L2 while the current group is integrated; 0 = off      */
   ARB_OPT_HOT_FIRST = 7,     /* cell-group kernel, one launch per grid step: 1 (default) = groups with an event in
@@ -113,7 +114,9 @@ typedef struct {
    *   layout_group_min_cells  cells with identical trees are laid out cell-interleaved in groups
    *                           (lane = cell) when their topology class has at least this many cells
    *                           (default 4; 1 = every cell in groups; >= 2^31 = no groups)
-   *   layout_unit_bytes       bytes of streamed records one warp unit may hold (default 4096)
+   *   layout_forest_cv        cells that do not share their tree are packed into forests of up to this
+ *                           many control volumes, one CTA each (default 1024; a larger cell is a forest
+ *                           of its own)
    *   cap_spikes              entries of the device spike buffer.  arb_advance drains it into host
    *                           memory at least every 2,000 grid steps, so it bounds the spikes of
    *                           such a stretch, not of the run (default max(2^20, 64 n_cells))
@@ -124,7 +127,7 @@ typedef struct {
    * arb_last_error.  Events or spikes beyond the capacity are lost, so the model is unusable
    * afterwards (every later call returns the same error): create it again with a larger cap_*.
    * (reading R0 says why the state is not rolled back to the last epoch.) */
-  int64_t layout_group_min_cells, layout_unit_bytes, cap_spikes, cap_events;
+  int64_t layout_group_min_cells, layout_forest_cv, cap_spikes, cap_events;
 } arb_desc;
 
 typedef struct arb_model arb_model; /* opaque; lives in host memory, owned by the library */
@@ -135,8 +138,8 @@ typedef struct arb_model arb_model; /* opaque; lives in host memory, owned by th
  * earlier than t = 0, inconsistent NULLs. */
 int arb_plan(const arb_desc* desc, size_t* workspace_bytes);
 
-/* Build the model: lay the cells out (cell-interleaved groups for cells that share a tree, units of
- * interleaved branches for the rest), upload to
+/* Build the model: lay the cells out (cell-interleaved groups for cells that share a tree, forests
+ * with lane = control volume for the rest), upload to
  * `dev_workspace` (DEVICE pointer, 256-byte aligned, >= workspace_bytes from arb_plan) on
  * `cuda_stream` (a cudaStream_t; NULL = default stream), initialise state (V = vinit, gates at
  * steady state, g = 0, t = 0; reading R4).  Returns after the upload has completed. */

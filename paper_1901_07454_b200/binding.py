@@ -13,7 +13,7 @@ LIB_PATH = os.path.join(_HERE, "libarbb200.so")
 
 ARB_OK, ARB_E_NULL, ARB_E_INVALID, ARB_E_WORKSPACE, ARB_E_CUDA, ARB_E_OVERFLOW, ARB_E_NOMEM, ARB_E_DIVERGED = 0, -1, -2, -3, -4, -5, -6, -7
 ARB_PROBE_M, ARB_PROBE_H, ARB_PROBE_N, ARB_PROBE_SYN_G, ARB_PROBE_TIME, ARB_PROBE_NSTEPS, ARB_PROBE_STATS, ARB_PROBE_TIMING = range(8)
-ARB_OPT_FUSED_STEPS, ARB_OPT_EPOCH_STEPS, ARB_OPT_TIMING, ARB_OPT_STAGES, ARB_OPT_L2_PREFETCH, ARB_OPT_GROUP_CTAS, ARB_OPT_HOT_FIRST = 1, 2, 3, 4, 5, 6, 7
+ARB_OPT_FUSED_STEPS, ARB_OPT_EPOCH_STEPS, ARB_OPT_TIMING, ARB_OPT_OVERLAP, ARB_OPT_L2_PREFETCH, ARB_OPT_GROUP_CTAS, ARB_OPT_HOT_FIRST = 1, 2, 3, 4, 5, 6, 7
 
 EXPORTS = ("arb_plan", "arb_create", "arb_advance", "arb_spikes", "arb_clear_spikes", "arb_voltage", "arb_probe",
            "arb_set_state", "arb_set_option", "arb_fp64_peak", "arb_destroy", "arb_last_error")
@@ -21,7 +21,7 @@ EXPORTS = ("arb_plan", "arb_create", "arb_advance", "arb_spikes", "arb_clear_spi
 # arb_desc's layout / capacity options (0 = library default).  A workloads dict may carry them under the
 # same names; LAYOUT_DEFAULTS fills in the ones it does not (the parity tests run every case under
 # several layouts this way).
-OPTION_FIELDS = ("layout_group_min_cells", "layout_unit_bytes", "cap_spikes", "cap_events")
+OPTION_FIELDS = ("layout_group_min_cells", "layout_forest_cv", "cap_spikes", "cap_events")
 LAYOUT_DEFAULTS = {}
 
 
@@ -47,7 +47,7 @@ class arb_desc(C.Structure):
         ("conn_syn", C.c_void_p), ("conn_delay", C.c_void_p), ("conn_weight", C.c_void_p),
         ("n_ext", C.c_int64), ("ext_cell", C.c_void_p), ("ext_syn", C.c_void_p),
         ("ext_time", C.c_void_p), ("ext_weight", C.c_void_p),
-        ("layout_group_min_cells", C.c_int64), ("layout_unit_bytes", C.c_int64),
+        ("layout_group_min_cells", C.c_int64), ("layout_forest_cv", C.c_int64),
         ("cap_spikes", C.c_int64), ("cap_events", C.c_int64),
     ]
 

@@ -32,7 +32,7 @@ struct Carver {
 };
 
 struct Regions {
-  Region units, gdescs, ghot, ghotflag, gen, fast, state, topo, scratch, warp_scratch, factor_dcontrib, cell_rt_idx, cell_orig, ev_off, ev_t, ev_gidx, ev_w, ev_fill,
+  Region units, gdescs, ghot, ghotflag, gen, fast, state, topo, scratch, factor_dcontrib, cell_rt_idx, cell_orig, ev_off, ev_t, ev_gidx, ev_w, ev_fill,
       ext_off, ext_t, ext_gidx, ext_w, ext_cur, conn_off, conn_dst, conn_gidx, conn_delay, conn_w,
       pool_t[2], pool_dst[2], pool_gidx[2], pool_w[2], spike_cell, spike_t, counters, scan_tmp,
       cv_idx, syn_idx, hh_m_idx, hh_stride, hh_cv, io;
@@ -57,22 +57,6 @@ constexpr int64_t kDrainSteps = 2000;   // the device spike buffer is drained at
 // upper bound of the CTAs of a cell-group launch
 int64_t group_cta_cap(const HostModel& H) { return std::min<int64_t>(H.n_groups, kMaxGroupCtas); }
 
-int64_t warp_scratch_stride(const HostModel& H) { return 2 * (int64_t)H.slot_cap + align_up(H.lane_cap, 2); }
-
-// Shared-memory plan of the warp kernel for n_stage stages per warp; warps == 0: does not fit.
-WarpSmemPlan make_plan(const HostModel& H, uint32_t n_stage) {
-  WarpSmemPlan P;
-  P.fast_cap = H.fast_cap; P.state_cap = H.state_cap; P.stage_bytes = H.fast_cap + H.state_cap;
-  P.n_stage = n_stage;
-  P.slot_cap = H.slot_cap; P.lane_cap = H.lane_cap; P.spec_cap = H.spec_cap; P.cell_cap = std::max(H.cell_cap, 1u);
-  P.topo_cap = align_up(H.topo_cap, 16);
-  const ScratchOff so = scratch_offsets(P.topo_cap, P.lane_cap, P.spec_cap, P.cell_cap, n_stage);
-  P.scratch_off = n_stage * P.stage_bytes;
-  P.warp_bytes = align_up(P.scratch_off + so.total, 128);
-  P.warps = std::min<uint32_t>((uint32_t)cable_max_warps(), (uint32_t)cable_smem_limit() / P.warp_bytes);
-  return P;
-}
-
 Regions carve(const HostModel& H, const Caps& cap) {
   Regions R;
   Carver C;
@@ -86,7 +70,6 @@ Regions carve(const HostModel& H, const Caps& cap) {
   R.state = C.take(8 * (size_t)H.state_doubles);
   R.topo = C.take((size_t)H.topo_bytes);
   R.scratch = C.take(8 * (size_t)H.scratch_doubles);
-  R.warp_scratch = C.take(H.n_warp_units > 0 ? 8 * (size_t)(kMaxWarps * warp_scratch_stride(H)) : 0);
   R.factor_dcontrib = C.take(8 * (size_t)H.n_lanes);
   R.cell_rt_idx = C.take(4 * nc);
   R.cell_orig = C.take(4 * nc);
@@ -143,10 +126,15 @@ struct arb_model {
   int cur_pool = 0;
   int sm_count = 148;
   int group_grid = 0, last_ggrid = 0;
+  // the cable kernels of one grid step (cell groups, the forest launch classes, block units) do not depend on
+  // each other: they run on side streams forked from / joined to the model's stream with events
+  static constexpr int kSide = 1 + kForestClasses;
+  cudaStream_t side[kSide] = {};
+  cudaEvent_t fork_ev = nullptr, join_ev[kSide] = {};
+  int64_t opt_overlap = 1;
   int64_t group_launches = 0, opt_group_ctas = 0, opt_hot = 1;
   bool prev_marked_hot = false;
   int64_t group_slots = 0, group_streamed = 0;   // statistics: CV slots incl. padding, bytes one grid step streams
-  int64_t opt_stages = 0;
   bool broken = false;
   int broken_code = ARB_E_OVERFLOW;
   std::string err;
@@ -180,9 +168,8 @@ cudaError_t upload(arb_model* m, const Region& r, const std::vector<T>& v) {
 
 // layout options travel in the description (no process-wide state)
 int params_of(const arb_desc& d, BuildParams& P, std::string& err) {
-  if (d.layout_group_min_cells < 0 || d.layout_unit_bytes < 0 || d.cap_spikes < 0 || d.cap_events < 0) { err = "negative layout / capacity option"; return ARB_E_INVALID; }
-  if (d.layout_unit_bytes != 0 && (d.layout_unit_bytes < 1024 || d.layout_unit_bytes > 112 * 1024)) { err = "layout_unit_bytes out of range (1024 .. 114688)"; return ARB_E_INVALID; }
-  if (d.layout_unit_bytes > 0) P.unit_bytes = (uint32_t)d.layout_unit_bytes;
+  if (d.layout_group_min_cells < 0 || d.layout_forest_cv < 0 || d.cap_spikes < 0 || d.cap_events < 0) { err = "negative layout / capacity option"; return ARB_E_INVALID; }
+  if (d.layout_forest_cv > 0) P.forest_cv = (uint32_t)std::min<int64_t>(d.layout_forest_cv, 1 << 20);
   if (d.layout_group_min_cells > 0) P.group_min_cells = d.layout_group_min_cells >= 0x7FFFFFFF ? 0u : (uint32_t)d.layout_group_min_cells;
   return ARB_OK;
 }
@@ -237,7 +224,6 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     if (configure_kernels() != cudaSuccess) { delete m; return fail(nullptr, ARB_E_CUDA, "arb_create: cannot opt the cable kernels into large shared memory"); }
     int group_ctas = 0;
     if (H.n_groups > 0 && (group_ctas = group_ctas_per_sm(group_smem_plan(H.gcaps).bytes)) == 0) { delete m; return fail(nullptr, ARB_E_INVALID, "arb_create: a cell group does not fit in shared memory"); }
-    if (H.n_warp_units > 0 && make_plan(H, 1).warps == 0) { delete m; return fail(nullptr, ARB_E_INVALID, "arb_create: a warp unit does not fit in shared memory"); }
     auto bail = [&](cudaError_t e, const char* w) { std::string s = std::string(w) + ": " + cudaGetErrorString(e); delete m; return fail(nullptr, ARB_E_CUDA, s); };
     cudaError_t e;
     const Regions& R = m->R;
@@ -272,10 +258,10 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     DevModel& D = m->D;
     std::memset(&D, 0, sizeof D);
     D.units = at<UnitDesc>(m, R.units);
-    D.n_units = H.n_units; D.n_warp_units = H.n_warp_units; D.n_cells = H.n_cells;
+    D.n_units = H.n_units; D.n_forests = H.n_forests; D.n_cells = H.n_cells;
+    for (int k = 0; k < kForestClasses; ++k) D.fcls[k] = H.fcls[k];
     D.gen = at<double>(m, R.gen); D.fast = at<uint8_t>(m, R.fast); D.state = at<double>(m, R.state);
     D.topo = at<uint8_t>(m, R.topo); D.scratch = at<double>(m, R.scratch);
-    D.warp_scratch = at<double>(m, R.warp_scratch); D.warp_scratch_stride = warp_scratch_stride(H);
     D.factor_dcontrib = at<double>(m, R.factor_dcontrib);
     D.cell_orig = at<uint32_t>(m, R.cell_orig); D.cell_rt_idx = at<uint32_t>(m, R.cell_rt_idx);
     D.ev_off = at<uint32_t>(m, R.ev_off); D.ev_t = at<double>(m, R.ev_t); D.ev_gidx = at<uint32_t>(m, R.ev_gidx);
@@ -289,7 +275,6 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
       D.pool[i].gidx = at<uint32_t>(m, R.pool_gidx[i]); D.pool[i].w = at<double>(m, R.pool_w[i]);
     }
     D.syn_uniform = H.syn_uniform ? 1 : 0; D.syn_e_u = H.syn_e_u; D.syn_tau_u = H.syn_tau_u; D.syn_decay_u = 1.0;
-    D.plan = make_plan(H, 1);
     D.groups = at<GroupDesc>(m, R.gdescs); D.n_groups = H.n_groups;
     for (const GroupDesc& g : H.gdescs) {
       const GConstOff co = gconst_offsets(g.n_cv, g.n_hh_rows, g.n_syn_rows, g.n_cl_rows, H.syn_uniform);
@@ -314,6 +299,18 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
       m->last_ggrid = m->group_grid;
     }
     if ((e = launch_init(D, m->stream)) != cudaSuccess) return bail(e, "init kernel");
+    if ((e = launch_forest_init(D, m->stream)) != cudaSuccess) return bail(e, "forest init kernel");
+    {
+      int n_kinds = (H.n_groups > 0) + (H.n_units > H.n_forests);
+      for (int k = 0; k < kForestClasses; ++k) n_kinds += H.fcls[k].count > 0;
+      if (n_kinds > 1) {                   // side streams only where there is something to overlap
+        if ((e = cudaEventCreateWithFlags(&m->fork_ev, cudaEventDisableTiming)) != cudaSuccess) return bail(e, "cudaEventCreate");
+        for (int i = 0; i < arb_model::kSide; ++i) {
+          if ((e = cudaStreamCreateWithFlags(&m->side[i], cudaStreamNonBlocking)) != cudaSuccess) return bail(e, "cudaStreamCreate");
+          if ((e = cudaEventCreateWithFlags(&m->join_ev[i], cudaEventDisableTiming)) != cudaSuccess) return bail(e, "cudaEventCreate");
+        }
+      }
+    }
     if ((e = launch_group_init(D, m->stream)) != cudaSuccess) return bail(e, "group init kernel");
     if ((e = cudaStreamSynchronize(m->stream)) != cudaSuccess) return bail(e, "cudaStreamSynchronize");
     // host pools are no longer needed
@@ -397,6 +394,7 @@ int arb_advance(arb_model* m, double t_end, double dt) {
   if (dt != m->factored_dt) {
     D.syn_decay_u = D.syn_uniform ? std::exp(-dt / D.syn_tau_u) : 1.0;
     CUB(launch_factor(D, dt, m->stream));
+    CUB(launch_forest_factor(D, dt, m->stream));
     CUB(launch_group_factor(D, dt, m->H.g_seg_cap, m->stream));
     m->factored_dt = dt;
     m->launches++;
@@ -413,18 +411,6 @@ int arb_advance(arb_model* m, double t_end, double dt) {
   if (m->opt_epoch > 0) epoch = std::min(epoch, m->opt_epoch);
   const int64_t fused = m->opt_fused > 0 ? std::min(m->opt_fused, epoch) : epoch;
   m->last_epoch_steps = epoch;
-  // shared-memory plan: two stages per warp (load the next unit while this one is integrated) when
-  // every launch streams the state once, one stage (more resident warps) when launches are fused
-  int grid = 1;
-  if (m->H.n_warp_units > 0) {
-    uint32_t n_stage = m->opt_stages > 0 ? (uint32_t)std::min<int64_t>(m->opt_stages, 2) : (fused > 1 ? 1u : 2u);
-    WarpSmemPlan P = make_plan(m->H, n_stage);
-    if (P.warps == 0) P = make_plan(m->H, 1);
-    const int64_t per_sm = (m->H.n_warp_units + m->sm_count - 1) / m->sm_count;
-    P.warps = (uint32_t)std::max<int64_t>(1, std::min<int64_t>(P.warps, per_sm));
-    grid = (int)std::min<int64_t>(m->sm_count, (m->H.n_warp_units + P.warps - 1) / P.warps);
-    D.plan = P;
-  }
   // a changed CTA count invalidates the work counters (they are reset to gridDim.x by the previous launch)
   const int ggrid = m->opt_group_ctas > 0 ? (int)std::min<int64_t>(m->opt_group_ctas, m->group_grid) : m->group_grid;
   if (ggrid != m->last_ggrid && m->H.n_groups > 0) {
@@ -477,8 +463,24 @@ int arb_advance(arb_model* m, double t_end, double dt) {
       A.mark_hot = (A.nk == 1 && m->opt_hot) ? 1 : 0;
       A.hot_valid = m->prev_marked_hot ? 1 : 0;
       m->prev_marked_hot = A.mark_hot != 0;
+      // cell groups on the model's stream; forests (largest launch class first) and block units beside them
+      const bool overlap = m->fork_ev != nullptr && m->opt_overlap;
+      if (overlap) CUB(cudaEventRecord(m->fork_ev, m->stream));
+      int side = 0;
+      auto on_side = [&](auto&& launch) -> cudaError_t {
+        if (!overlap) return launch(m->stream);
+        cudaStream_t st = m->side[side];
+        cudaError_t ce = cudaStreamWaitEvent(st, m->fork_ev, 0);
+        if (ce == cudaSuccess) ce = launch(st);
+        if (ce == cudaSuccess) ce = cudaEventRecord(m->join_ev[side], st);
+        if (ce == cudaSuccess) ce = cudaStreamWaitEvent(m->stream, m->join_ev[side], 0);
+        ++side;
+        return ce;
+      };
+      for (int c = kForestClasses - 1; c >= 0; --c)
+        if (D.fcls[c].count > 0) CUB(on_side([&](cudaStream_t st) { return launch_forest_cable(D, A, c, st, &launches); }));
+      if (D.n_units > D.n_forests) CUB(on_side([&](cudaStream_t st) { return launch_cable(D, A, st, &launches); }));
       CUB(launch_group_cable(D, A, ggrid, m->stream, &launches));
-      CUB(launch_cable(D, A, grid, m->stream, &launches));
     }
     CUB(stamp());
     int l2 = launches;
@@ -587,7 +589,7 @@ int arb_probe(arb_model* m, int what, double* out, int64_t n) {
       out[3] = (double)m->R.total; out[4] = (double)cnt[CNT_DELIVERED]; out[5] = (double)m->launches;
       out[6] = (double)m->last_epoch_steps; out[7] = (double)streamed;
       if (n >= 12) {
-        out[8] = (double)m->H.n_warp_units; out[9] = (double)m->D.plan.warps; out[10] = (double)m->D.plan.warp_bytes;
+        out[8] = 0.0; out[9] = 0.0; out[10] = 0.0;      // (warp units of round 1: replaced by forests)
         out[11] = (double)m->H.topo_records;
       }
       if (n >= 16) {
@@ -595,7 +597,9 @@ int arb_probe(arb_model* m, int what, double* out, int64_t n) {
         out[15] = (double)m->D.gplan.bytes;
       }
       if (n >= 20) {
-        out[16] = 0.0; out[17] = (double)(m->H.n_units - m->H.n_warp_units); out[18] = 0.0; out[19] = 0.0;
+        int64_t fctas = 0; uint32_t fsmem = 0;
+        for (int k = 0; k < kForestClasses; ++k) { fctas = std::max(fctas, m->H.fcls[k].count); if (m->H.fcls[k].count) fsmem = std::max(fsmem, m->H.fcls[k].plan.bytes); }
+        out[16] = (double)m->H.n_forests; out[17] = (double)(m->H.n_units - m->H.n_forests); out[18] = (double)fctas; out[19] = (double)fsmem;
       }
       return ARB_OK;
     }
@@ -635,7 +639,7 @@ int arb_set_option(arb_model* m, int key, int64_t value) {
   switch (key) {
     case ARB_OPT_FUSED_STEPS: m->opt_fused = value; return ARB_OK;
     case ARB_OPT_EPOCH_STEPS: m->opt_epoch = value; return ARB_OK;
-    case ARB_OPT_STAGES: m->opt_stages = value; return ARB_OK;
+    case ARB_OPT_OVERLAP: m->opt_overlap = value != 0; return ARB_OK;
     case ARB_OPT_L2_PREFETCH: m->D.l2_prefetch = value != 0; return ARB_OK;
     case ARB_OPT_GROUP_CTAS: m->opt_group_ctas = value; return ARB_OK;
     case ARB_OPT_HOT_FIRST: m->opt_hot = value != 0; m->prev_marked_hot = false; return ARB_OK;
@@ -651,6 +655,11 @@ void arb_destroy(arb_model* m) {
   if (!m) return;
   if (m->ws) cudaStreamSynchronize(m->stream);
   for (cudaEvent_t ev : m->tev) cudaEventDestroy(ev);
+  for (int i = 0; i < arb_model::kSide; ++i) {
+    if (m->side[i]) { cudaStreamSynchronize(m->side[i]); cudaStreamDestroy(m->side[i]); }
+    if (m->join_ev[i]) cudaEventDestroy(m->join_ev[i]);
+  }
+  if (m->fork_ev) cudaEventDestroy(m->fork_ev);
   delete m;
 }
 

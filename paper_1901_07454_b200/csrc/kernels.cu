@@ -1,22 +1,18 @@
 // kernels.cu - hand-written fp64 CUDA kernels for sm_100a: the whole hot path of arbb200.
 //
-//   cable_warp_kernel   the cable step for "warp units" (unit_layout.h).  A persistent grid; every
-//                       warp is its own software pipeline: one lane issues bulk-async copies (TMA,
-//                       cp.async.bulk + mbarrier) that bring the next unit's fast and state records
-//                       into the warp's second shared-memory stage while all 32 lanes integrate the
-//                       current unit out of the first.  Per grid step (or fused run of steps):
-//                       event delivery -> mechanism currents (eq 2a)
-//                       -> rhs of the implicit Euler system -> branched Thomas / Hines
-//                       sweeps over tasks of interleaved branches -> V <- V' -> gate /
+//   cable_block_kernel  the cable step for block units (unit_layout.h): cells too large for a CTA's shared
+//                       memory, or with thousands of synapses.  One CTA per unit, working straight out of
+//                       global memory (L1/L2), lane = branch, __syncthreads between tree levels.  Per grid
+//                       step (or fused run of steps): event delivery -> mechanism currents
+//                       (eq 2a; synapse currents summed by a warp-level key reduction,
+//                       PAPER.md:218) -> rhs of the implicit Euler system -> branched Thomas /
+//                       Hines sweeps over tasks of interleaved branches -> V <- V' -> gate /
 //                       synapse state update with V' -> threshold test.
-//                       No block-level barrier anywhere: only __syncwarp between tree levels.
-//   cable_block_kernel  the same step for cells too large for a warp's stage: one CTA per unit,
-//                       working straight out of global memory (L1/L2), __syncthreads between levels.
-//   factor_kernel       once per dt: eliminates the (constant, reading R1) matrix of every unit
+//                       (Cells that share a tree run in group_kernel.cu, all other cells in forest_kernel.cu.)
+//   factor_kernel       once per dt: eliminates the (constant, reading R1) matrix of every block unit
 //   ev_* / spikes_to_events   once per min-delay epoch
 //
-// No tensor cores: nothing here is a dense contraction.  The path is bound by HBM traffic when
-// state streams every step and by fp64 dependent-chain latency when a unit stays on chip.
+// No tensor cores: nothing here is a dense contraction.
 #include "kernels.cuh"
 #include "device_common.cuh"
 
@@ -27,20 +23,9 @@ namespace {
 constexpr int kBlockThreads = 128;              // cable_block_kernel, factor_kernel, init_kernel
 constexpr int kBlockWarps = kBlockThreads / 32;
 constexpr uint32_t kSynKeyReduceMin = 1024;     // block units with at least this many synapses reduce currents by key
-constexpr int kMaxWarpsPerCta = 8;              // cable_warp_kernel
 
-// ------------------------------------------------------------------------------------------
-// scopes: a unit is integrated either by one warp or by one CTA
-// ------------------------------------------------------------------------------------------
-template <bool kWarp> struct Scope;
-template <> struct Scope<true> {
-  static constexpr int size = 32, warps = 1;
-  static __device__ __forceinline__ int tid() { return threadIdx.x & 31; }
-  static __device__ __forceinline__ int warp() { return 0; }
-  static __device__ __forceinline__ void sync() { __syncwarp(); }
-  static __device__ __forceinline__ bool any(bool p) { return __any_sync(kFull, p) != 0; }
-};
-template <> struct Scope<false> {
+// a block unit is integrated by one CTA
+struct S {
   static constexpr int size = kBlockThreads, warps = kBlockWarps;
   static __device__ __forceinline__ int tid() { return threadIdx.x; }
   static __device__ __forceinline__ int warp() { return threadIdx.x >> 5; }
@@ -48,15 +33,13 @@ template <> struct Scope<false> {
   static __device__ __forceinline__ bool any(bool p) { return __syncthreads_or(p) != 0; }
 };
 
-// Pointers of one unit.  "Working" pointers address shared memory in the warp kernel and global
-// memory in the block kernel; g* pointers always address the unit's state record in global memory.
+// Pointers of one unit; everything addresses global memory.
 struct UnitView {
   uint32_t n_slot, n_lane, n_task, n_level, n_cell, n_hh, n_syn, n_clamp;
   const double *f, *invd, *a, *b, *hh_gna, *hh_gk, *hh_gl, *syn_e, *syn_decay, *cl_t0, *cl_t1, *cl_amp;
   const uint32_t *hh_slot, *syn_slot, *cl_slot;
   const uint16_t *hh_cell, *syn_cell, *cl_cell;
   double *V, *m, *h, *n, *g, *rt;
-  double *gV, *gm, *gh, *gn, *gg, *grt;
   uint32_t g_gidx0;                 // state-pool index of g[0]
   const Task* tasks; const LaneRec* lanes; const uint32_t *level_begin, *child, *cell_det;
   const double *C, *S, *sig, *G, *bg, *syn_tau;
@@ -79,8 +62,6 @@ __device__ __forceinline__ void make_view(UnitView& U, const DevModel& M, const 
   U.hh_cell = (const uint16_t*)(fastw + fo.hh_cell); U.syn_cell = (const uint16_t*)(fastw + fo.syn_cell); U.cl_cell = (const uint16_t*)(fastw + fo.cl_cell);
   const StateOff so = state_offsets(H.n_slot, H.n_hh, H.n_syn, H.n_cell);
   U.V = statew + so.v; U.m = statew + so.m; U.h = statew + so.h; U.n = statew + so.n; U.g = statew + so.g; U.rt = statew + so.rt;
-  double* gs = M.state + H.state_base;
-  U.gV = gs + so.v; U.gm = gs + so.m; U.gh = gs + so.h; U.gn = gs + so.n; U.gg = gs + so.g; U.grt = gs + so.rt;
   U.g_gidx0 = (uint32_t)(H.state_base + so.g);
   const TopoOff to = topo_offsets(H.n_task, H.n_level, H.n_lane, H.n_child, H.n_cell);
   U.tasks = (const Task*)(topow + to.tasks); U.lanes = (const LaneRec*)(topow + to.lanes);
@@ -217,8 +198,7 @@ __device__ __forceinline__ void backward_task(const UnitView& U, const CellS& cs
 }
 
 // Forward (root -> leaves) substitution of one task: V'_k = rhs_k/d_k - f_k V'_{k-1}; V <- V'.
-// kStore: also store V' to the unit's state record in global memory when the cell's step ends.
-template <bool kGen, bool kStore>
+template <bool kGen>
 __device__ __forceinline__ void forward_task(const UnitView& U, const CellS& cs, const TaskCtx& X, int lane) {
   const Task& T = X.T;
   const bool in = (uint32_t)lane < T.nlanes;
@@ -226,12 +206,7 @@ __device__ __forceinline__ void forward_task(const UnitView& U, const CellS& cs,
   const uint32_t maxlen = T.maxlen_full & 0x7FFFu;
   const bool full = (T.maxlen_full & kTaskFull) != 0;
   uint32_t md = in ? 1u : 0u;
-  bool wb = false;
-  if (kGen) {
-    if (in) { md = cs.mode[X.R.cell]; wb = kStore && cs.wb[X.R.cell] != 0u; }
-  } else {
-    wb = kStore && cs.wb[0] != 0u;
-  }
+  if (kGen && in) md = cs.mode[X.R.cell];
   double vp = 0.0;
   if (in && md && X.R.pslot != kNoSlot) vp = U.V[X.R.pslot];
   if (!kGen && full) {
@@ -245,13 +220,11 @@ __device__ __forceinline__ void forward_task(const UnitView& U, const CellS& cs,
       const double q0 = U.V[s], q1 = U.V[s1], q2 = U.V[s2], q3 = U.V[s3];
       const double v0 = fma(-f0, vp, q0), v1 = fma(-f1, v0, q1), v2 = fma(-f2, v1, q2), v3 = fma(-f3, v2, q3);
       U.V[s] = v0; U.V[s1] = v1; U.V[s2] = v2; U.V[s3] = v3;
-      if (wb) { U.gV[s] = v0; U.gV[s1] = v1; U.gV[s2] = v2; U.gV[s3] = v3; }
       vp = v3; s = s3 + w; k -= 4;
     }
     while (k >= 1) {
       vp = fma(-U.f[s], vp, U.V[s]);
       U.V[s] = vp;
-      if (wb) U.gV[s] = vp;
       s += w; --k;
     }
     return;
@@ -265,7 +238,6 @@ __device__ __forceinline__ void forward_task(const UnitView& U, const CellS& cs,
       const double fk = (kGen && md == 2u) ? U.fgen[s] : U.f[s];
       vp = fma(-fk, vp, U.V[s]);
       U.V[s] = vp;
-      if (wb) U.gV[s] = vp;
     }
     row += cnt;
   }
@@ -298,9 +270,8 @@ __device__ __forceinline__ void rhs_task(const UnitView& U, const CellS& cs, con
 // One (sub-)step of every active cell of a unit, phases B..F of the step (phase A, event delivery
 // and the choice of the sub-step, is in run_unit).
 // ------------------------------------------------------------------------------------------
-template <bool kWarp, bool kGen>
+template <bool kGen>
 __device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, const CellS& cs, double dt) {
-  using S = Scope<kWarp>;
   const int tid = S::tid(), lane = threadIdx.x & 31;
   const bool multi = U.n_cell > 1;
   const uint32_t n_hh = U.n_hh, n_syn = U.n_syn, n_cl = U.n_clamp;
@@ -313,7 +284,7 @@ __device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, co
     const double m = U.m[i], h = U.h[i], n = U.n[i];
     U.xI[i] = U.hh_gna[i] * m * m * m * h * (v - M.ena) + U.hh_gk[i] * n * n * n * n * (v - M.ek) + U.hh_gl[i] * (v - M.el);
   }
-  if (!kWarp && n_syn >= kSynKeyReduceMin) {
+  if (n_syn >= kSynKeyReduceMin) {
     // Many synapses per control volume (the paper's ring cell): a run head summing its
     // run alone would leave the other lanes idle.  Each warp takes 32 consecutive synapses (coalesced),
     // reduces them by key = control volume with shuffles (the "key reduction" of PAPER.md:218; runs are
@@ -398,7 +369,7 @@ __device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, co
     }
     S::sync();
   }
-  if (!kWarp && n_syn >= kSynKeyReduceMin) {
+  if (n_syn >= kSynKeyReduceMin) {
     // run heads (listed once per dt by factor_kernel) add the partial sums of the chunks their run
     // extends into, in index order
     const uint32_t nh = U.heads[0];
@@ -431,25 +402,7 @@ __device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, co
   }
 
   // ---- D: backward sweep, deepest level first; E: forward substitution, root first; V <- V'
-  if (kWarp) {
-    // one warp owns the unit: tasks are ordered by level, the next task's records are fetched
-    // while the current one is swept
-    TaskCtx cur = load_ctx(U, U.n_task - 1, lane);
-    for (int ti = (int)U.n_task - 1; ti >= 0; --ti) {
-      TaskCtx nxt = cur;
-      if (ti > 0) nxt = load_ctx(U, ti - 1, lane);
-      backward_task<kGen>(U, cs, cur, lane);
-      cur = nxt;
-      __syncwarp();
-    }
-    for (uint32_t ti = 0; ti < U.n_task; ++ti) {        // cur == task 0 here
-      TaskCtx nxt = cur;
-      if (ti + 1 < U.n_task) nxt = load_ctx(U, ti + 1, lane);
-      forward_task<kGen, true>(U, cs, cur, lane);
-      cur = nxt;
-      __syncwarp();
-    }
-  } else {
+  {
     const int warp = S::warp();
     for (int lvl = (int)U.n_level - 1; lvl >= 0; --lvl) {
       for (uint32_t ti = U.level_begin[lvl] + warp; ti < U.level_begin[lvl + 1]; ti += S::warps)
@@ -458,7 +411,7 @@ __device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, co
     }
     for (uint32_t lvl = 0; lvl < U.n_level; ++lvl) {
       for (uint32_t ti = U.level_begin[lvl] + warp; ti < U.level_begin[lvl + 1]; ti += S::warps)
-        forward_task<kGen, false>(U, cs, load_ctx(U, ti, lane), lane);
+        forward_task<kGen>(U, cs, load_ctx(U, ti, lane), lane);
       __syncthreads();
     }
   }
@@ -476,9 +429,8 @@ __device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, co
     inf = r.an / (r.an + r.bn);
     const double n = inf + (U.n[i] - inf) * exp(-delta * (r.an + r.bn));
     U.m[i] = m; U.h[i] = h; U.n[i] = n;
-    if (kWarp && cs.wb[c]) { U.gm[i] = m; U.gh[i] = h; U.gn[i] = n; }
   }
-  if (!kGen && !kWarp && n_syn >= kSynKeyReduceMin) {
+  if (!kGen && n_syn >= kSynKeyReduceMin) {
     // done in phase B
   } else
   for (uint32_t i = tid; i < n_syn; i += S::size) {
@@ -488,9 +440,7 @@ __device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, co
     double decay;
     if (md == 1u) decay = M.syn_uniform ? M.syn_decay_u : U.syn_decay[i];
     else decay = exp(-cs.delta[c] / (M.syn_uniform ? M.syn_tau_u : U.syn_tau[i]));
-    const double g = U.g[i] * decay;
-    U.g[i] = g;
-    if (kWarp && cs.wb[c]) U.gg[i] = g;
+    U.g[i] *= decay;
   }
   if ((uint32_t)tid < U.n_cell && (!kGen || cs.mode[tid])) {
     const double vd = U.V[U.cell_det[tid]], vp = cs.vprev[tid];
@@ -512,10 +462,8 @@ __device__ __forceinline__ void substep(const DevModel& M, const UnitView& U, co
 // A.nk grid steps of one unit.  Phase A: deliver the events due now and choose each cell's
 // sub-step (reading R9), then the step itself.
 // ------------------------------------------------------------------------------------------
-template <bool kWarp>
 __device__ __forceinline__ void run_unit(const DevModel& M, const StepArgs& A, const UnitView& U, const CellS& cs,
                                          unsigned& n_sub, unsigned& n_del) {
-  using S = Scope<kWarp>;
   const int tid = S::tid();
   const uint32_t n_cell = U.n_cell;
   if ((uint32_t)tid < n_cell) {
@@ -528,7 +476,6 @@ __device__ __forceinline__ void run_unit(const DevModel& M, const StepArgs& A, c
     const double ta = (k == 0) ? A.t0 : __dadd_rn(A.t0, __dmul_rn((double)k, A.dt));
     const double tb = (k + 1 == A.nsteps) ? A.t_end : __dadd_rn(A.t0, __dmul_rn((double)(k + 1), A.dt));
     const bool nominal = (k + 1 < A.nsteps) || A.last_full;
-    const bool last = (k + 1 == A.k_first + A.nk);
     if ((uint32_t)tid < n_cell) cs.tcur[tid] = ta;
     S::sync();
     for (;;) {
@@ -551,7 +498,6 @@ __device__ __forceinline__ void run_unit(const DevModel& M, const StepArgs& A, c
           md = fast ? 1u : 2u;
           cs.tnext[tid] = next;
           cs.vprev[tid] = U.V[U.cell_det[tid]];
-          cs.wb[tid] = (last && next == tb) ? 1u : 0u;
           active = true;
           ++n_sub;
         }
@@ -561,17 +507,15 @@ __device__ __forceinline__ void run_unit(const DevModel& M, const StepArgs& A, c
       if (!S::any(active)) break;
       const bool general = S::any(!plain);
       S::sync();
-      if (general) substep<kWarp, true>(M, U, cs, A.dt);
-      else substep<kWarp, false>(M, U, cs, A.dt);
+      if (general) substep<true>(M, U, cs, A.dt);
+      else substep<false>(M, U, cs, A.dt);
     }
   }
   if ((uint32_t)tid < n_cell && cs.dirty[tid]) {
-    double* rt = U.grt + kRtDoubles * tid;
+    double* rt = U.rt + kRtDoubles * tid;
     const unsigned long long pk = ((unsigned long long)cs.evend[tid] << 32) | cs.evcur[tid];
-    rt[0] = U.rt[kRtDoubles * tid];
     rt[1] = __longlong_as_double((long long)pk);
     rt[2] = cs.armed[tid] ? 1.0 : 0.0;
-    if (kWarp) { U.rt[kRtDoubles * tid + 1] = rt[1]; U.rt[kRtDoubles * tid + 2] = rt[2]; }
   }
 }
 
@@ -581,78 +525,6 @@ __device__ __forceinline__ void flush_stats(const DevModel& M, unsigned n_sub, u
     if (n_sub) atomicAdd(&M.counters[CNT_SUBSTEPS], (unsigned long long)n_sub);
     if (n_del) atomicAdd(&M.counters[CNT_DELIVERED], (unsigned long long)n_del);
   }
-}
-
-// ------------------------------------------------------------------------------------------
-// The cable step for warp units.
-// ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kMaxWarpsPerCta * 32, 1) cable_warp_kernel(DevModel M, StepArgs A) {
-  extern __shared__ __align__(128) uint8_t smem[];
-  const WarpSmemPlan P = M.plan;
-  const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t gw = blockIdx.x * (int64_t)P.warps + w;
-  const int64_t NW = gridDim.x * (int64_t)P.warps;
-  const int64_t n_units = M.n_warp_units;
-  if (gw >= n_units) return;                       // no block-level barrier is ever used
-  uint8_t* region = smem + (size_t)w * P.warp_bytes;
-  uint8_t* scr = region + P.scratch_off;
-  const ScratchOff so = scratch_offsets(P.topo_cap, P.lane_cap, P.spec_cap, P.cell_cap, P.n_stage);
-  uint64_t* mbar = (uint64_t*)(scr + so.mbar);
-  uint8_t* topow = scr + so.topo;
-  const CellS cs = carve_cells(scr + so.cell, P.cell_cap);
-  const uint32_t n_stage = P.n_stage;
-
-  auto issue = [&](const UnitDesc& d, uint32_t st) {
-    uint8_t* dst = region + (size_t)st * P.stage_bytes;
-    mbar_expect_tx(&mbar[st], d.fast_bytes + d.state_bytes);
-    bulk_g2s(dst, M.fast + d.fast_off, d.fast_bytes, &mbar[st]);
-    bulk_g2s(dst + P.fast_cap, M.state + d.state_base, d.state_bytes, &mbar[st]);
-  };
-  if (lane == 0) {
-    for (uint32_t s = 0; s < n_stage; ++s) mbar_init(&mbar[s], 1);
-    fence_mbar_init();
-    fence_proxy_async();
-    for (uint32_t s = 0; s < n_stage; ++s) {
-      const int64_t u = gw + (int64_t)s * NW;
-      if (u < n_units) issue(M.units[u], s);
-    }
-  }
-  __syncwarp();
-
-  int64_t cached_topo = -1;
-  unsigned n_sub = 0, n_del = 0;
-  uint32_t it = 0;
-  for (int64_t u = gw; u < n_units; u += NW, ++it) {
-    const uint32_t st = it % n_stage, parity = (it / n_stage) & 1u;
-    const int64_t un = u + (int64_t)n_stage * NW;
-    UnitDesc dn;
-    dn.fast_off = 0; dn.state_base = 0; dn.fast_bytes = 0; dn.state_bytes = 0;
-    if (lane == 0 && un < n_units) dn = M.units[un];        // in flight while this unit is integrated
-    mbar_wait(&mbar[st], parity);
-    uint8_t* fastw = region + (size_t)st * P.stage_bytes;
-    const UnitHeader H = *(const UnitHeader*)fastw;
-    if (H.topo_off != cached_topo) {
-      // tree structure differs from the previous unit's: fetch its record (L2-resident when shared)
-      const uint32_t bytes = topo_offsets(H.n_task, H.n_level, H.n_lane, H.n_child, H.n_cell).total;
-      const uint4* src = (const uint4*)(M.topo + H.topo_off);
-      uint4* dst = (uint4*)topow;
-      __syncwarp();
-      for (uint32_t i = lane; i < bytes / 16; i += 32) dst[i] = src[i];
-      __syncwarp();
-      cached_topo = H.topo_off;
-    }
-    UnitView U;
-    make_view(U, M, H, fastw, (double*)(fastw + P.fast_cap), topow);
-    U.contrib = (double*)(scr + so.contrib);
-    U.xI = (double*)(scr + so.xI);
-    double* ws = M.warp_scratch + gw * M.warp_scratch_stride;     // event-split sub-steps only
-    U.fgen = ws; U.invdgen = ws + P.slot_cap; U.dcontrib = ws + 2 * (size_t)P.slot_cap;
-    run_unit<true>(M, A, U, cs, n_sub, n_del);
-    fence_proxy_async();          // this warp's accesses to the stage come before the next bulk copy into it
-    __syncwarp();
-    if (lane == 0 && un < n_units) issue(dn, st);
-  }
-  flush_stats(M, n_sub, n_del);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -671,23 +543,23 @@ constexpr int kBlockMinCtas = 16;   // latency-bound out of L2: full occupancy b
 __global__ void __launch_bounds__(kBlockThreads, kBlockMinCtas) cable_block_kernel(DevModel M, StepArgs A) {
   __shared__ UnitHeader H;
   __shared__ __align__(16) uint8_t cell_mem[kCellScratchBytes * kBlockUnitMaxCells];
-  const UnitDesc d = M.units[M.n_warp_units + blockIdx.x];
+  const UnitDesc d = M.units[M.n_forests + blockIdx.x];
   if (threadIdx.x < sizeof(UnitHeader) / 4) ((uint32_t*)&H)[threadIdx.x] = ((const uint32_t*)(M.fast + d.fast_off))[threadIdx.x];
   __syncthreads();
   UnitView U;
   block_view(U, M, H, d);
   const CellS cs = carve_cells(cell_mem, kBlockUnitMaxCells);
   unsigned n_sub = 0, n_del = 0;
-  run_unit<false>(M, A, U, cs, n_sub, n_del);
+  run_unit(M, A, U, cs, n_sub, n_del);
   flush_stats(M, n_sub, n_del);
 }
 
 // ------------------------------------------------------------------------------------------
-// Once per dt: f, 1/d, a, b (and per-synapse decay factors) of every unit.  One CTA per unit.
+// Once per dt: f, 1/d, a, b (and per-synapse decay factors) of every block unit.  One CTA per unit.
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kBlockThreads) factor_kernel(DevModel M, double dt) {
   __shared__ UnitHeader H;
-  const UnitDesc d = M.units[blockIdx.x];
+  const UnitDesc d = M.units[M.n_forests + blockIdx.x];
   if (threadIdx.x < sizeof(UnitHeader) / 4) ((uint32_t*)&H)[threadIdx.x] = ((const uint32_t*)(M.fast + d.fast_off))[threadIdx.x];
   __syncthreads();
   UnitView U;
@@ -712,7 +584,7 @@ __global__ void __launch_bounds__(kBlockThreads) factor_kernel(DevModel M, doubl
     double* decay = const_cast<double*>(U.syn_decay);
     for (uint32_t i = threadIdx.x; i < U.n_syn; i += kBlockThreads) decay[i] = exp(-dt / U.syn_tau[i]);
   }
-  if (blockIdx.x >= M.n_warp_units && U.n_syn >= kSynKeyReduceMin) {   // run heads of the synapse list (order irrelevant)
+  if (U.n_syn >= kSynKeyReduceMin) {   // run heads of the synapse list (order irrelevant)
     __shared__ uint32_t n_heads;
     uint32_t* heads = (uint32_t*)(M.scratch + H.scratch_base + 2 * (size_t)align_up(H.n_lane, 2) +
                                   align_up(H.n_hh + H.n_syn + H.n_clamp, 2) + 2 * (size_t)H.n_slot);
@@ -728,7 +600,7 @@ __global__ void __launch_bounds__(kBlockThreads) factor_kernel(DevModel M, doubl
 // R4: gates start at their steady state for the initial voltage.
 __global__ void __launch_bounds__(kBlockThreads) init_kernel(DevModel M) {
   __shared__ UnitHeader H;
-  const UnitDesc d = M.units[blockIdx.x];
+  const UnitDesc d = M.units[M.n_forests + blockIdx.x];
   if (threadIdx.x < sizeof(UnitHeader) / 4) ((uint32_t*)&H)[threadIdx.x] = ((const uint32_t*)(M.fast + d.fast_off))[threadIdx.x];
   __syncthreads();
   UnitView U;
@@ -923,21 +795,20 @@ cudaError_t configure_kernels() {
   if (e != cudaSuccess) return e;
   e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
   if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(cable_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+  e = configure_forest_kernel(optin);
   if (e != cudaSuccess) return e;
   return configure_group_kernel(optin);
 }
-int cable_max_warps() { return kMaxWarpsPerCta; }
 
 cudaError_t launch_factor(const DevModel& M, double dt, cudaStream_t s) {
-  if (M.n_units == 0) return cudaSuccess;
-  factor_kernel<<<(unsigned)M.n_units, kBlockThreads, 0, s>>>(M, dt);
+  if (M.n_units == M.n_forests) return cudaSuccess;
+  factor_kernel<<<(unsigned)(M.n_units - M.n_forests), kBlockThreads, 0, s>>>(M, dt);
   return cudaGetLastError();
 }
 
 cudaError_t launch_init(const DevModel& M, cudaStream_t s) {
-  if (M.n_units == 0) return cudaSuccess;
-  init_kernel<<<(unsigned)M.n_units, kBlockThreads, 0, s>>>(M);
+  if (M.n_units == M.n_forests) return cudaSuccess;
+  init_kernel<<<(unsigned)(M.n_units - M.n_forests), kBlockThreads, 0, s>>>(M);
   return cudaGetLastError();
 }
 
@@ -946,14 +817,9 @@ cudaError_t launch_reset_detectors(const DevModel& M, cudaStream_t s) {
   return cudaGetLastError();
 }
 
-cudaError_t launch_cable(const DevModel& M, const StepArgs& A, int grid, cudaStream_t s, int* launches) {
-  if (M.n_warp_units > 0) {
-    const int smem = (int)(M.plan.warps * M.plan.warp_bytes);   // configure_kernels() has opted the kernel in
-    cable_warp_kernel<<<(unsigned)grid, (unsigned)(M.plan.warps * 32), smem, s>>>(M, A);
-    if (launches) ++*launches;
-  }
-  if (M.n_units > M.n_warp_units) {
-    cable_block_kernel<<<(unsigned)(M.n_units - M.n_warp_units), kBlockThreads, 0, s>>>(M, A);
+cudaError_t launch_cable(const DevModel& M, const StepArgs& A, cudaStream_t s, int* launches) {
+  if (M.n_units > M.n_forests) {
+    cable_block_kernel<<<(unsigned)(M.n_units - M.n_forests), kBlockThreads, 0, s>>>(M, A);
     if (launches) ++*launches;
   }
   return cudaGetLastError();

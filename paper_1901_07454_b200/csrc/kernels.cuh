@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "forest_layout.h"
 #include "group_layout.h"
 #include "unit_layout.h"
 
@@ -29,15 +30,15 @@ enum Counter {
 struct EventPool { double* t; uint32_t* dst; uint32_t* gidx; double* w; };
 
 struct DevModel {
-  const UnitDesc* units;      // warp units first, then block units
-  int64_t n_units, n_warp_units, n_cells;
+  const UnitDesc* units;      // forests first, then block units
+  int64_t n_units, n_forests, n_cells;
+  ForestClass fcls[kForestClasses];   // forest launches by shared-memory need (forest_layout.h)
   uint8_t* fast;
   double* state;
   const double* gen;
   const uint8_t* topo;
-  double* scratch;            // block units: contrib | dcontrib | xI | fgen | invdgen at header.scratch_base
-  double* warp_scratch;       // warp kernel: per resident warp fgen | invdgen | dcontrib
-  int64_t warp_scratch_stride;
+  double* scratch;            // at header.scratch_base: block units contrib | dcontrib | xI | fgen | invdgen | run heads;
+                              // forests fgen | invdgen | dcon (forest_layout.h)
   double* factor_dcontrib;    // [total branches], used by factor_kernel only
   const uint32_t* cell_orig;  // internal -> caller's cell id
   const uint32_t* cell_rt_idx;// internal cell -> state index of its runtime triple
@@ -62,7 +63,6 @@ struct DevModel {
   int syn_uniform;
   double syn_e_u, syn_tau_u, syn_decay_u;
   double ena, ek, el, theta;
-  WarpSmemPlan plan;
   // cell groups (group_layout.h); cells of groups come first in the internal cell order
   const GroupDesc* groups;
   int64_t n_groups;
@@ -86,8 +86,13 @@ struct StepArgs {
 // all launchers queue work on `s` and return the last CUDA error code
 cudaError_t launch_factor(const DevModel& M, double dt, cudaStream_t s);
 cudaError_t launch_init(const DevModel& M, cudaStream_t s);
-// the cable step: a persistent grid of `grid` CTAs of plan.warps warps for the warp units, one CTA per block unit
-cudaError_t launch_cable(const DevModel& M, const StepArgs& A, int grid, cudaStream_t s, int* launches);
+// the cable step of the block units: one CTA per unit
+cudaError_t launch_cable(const DevModel& M, const StepArgs& A, cudaStream_t s, int* launches);
+// forests (forest_kernel.cu): one launch per shared-memory class
+cudaError_t launch_forest_factor(const DevModel& M, double dt, cudaStream_t s);
+cudaError_t launch_forest_init(const DevModel& M, cudaStream_t s);
+cudaError_t launch_forest_cable(const DevModel& M, const StepArgs& A, int cls, cudaStream_t s, int* launches);
+cudaError_t configure_forest_kernel(int max_optin_bytes);
 cudaError_t launch_build_events(const DevModel& M, int cur_pool, double t_window_end, cudaStream_t s, int* launches);
 cudaError_t launch_spikes_to_events(const DevModel& M, int cur_pool, cudaStream_t s, int* launches);
 cudaError_t launch_gather(const double* state, const uint32_t* idx, int64_t n, double* out, cudaStream_t s);
@@ -106,7 +111,6 @@ int group_ctas_per_sm(uint32_t smem_bytes);   // resident CTAs of the group kern
 // attribute is per function and device; called by every arb_create, nothing is cached).
 cudaError_t configure_kernels();
 cudaError_t configure_group_kernel(int max_optin_bytes);
-int cable_smem_limit();       // bytes of dynamic shared memory a CTA of the warp kernel may use
-int cable_max_warps();        // warps per CTA the warp kernel is compiled for
+int cable_smem_limit();       // bytes of dynamic shared memory a CTA may use (sm_100a opt-in maximum)
 
 }  // namespace arbb

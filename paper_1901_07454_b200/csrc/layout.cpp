@@ -146,6 +146,11 @@ struct UnitBuilder {
   std::vector<Task> tasks;
   std::vector<uint32_t> level_begin;
   bool bad = false;                        // a count does not fit its field
+  // forests (forest_layout.h)
+  bool forest = false;
+  std::vector<uint32_t> fslot0, flevel_br;
+  std::vector<FRun> fruns;
+  std::vector<FChunk> fchunks;
 
   bool has_hh(int64_t gi) const {
     return d.hh_gnabar && (d.hh_gnabar[gi] != 0.0 || d.hh_gkbar[gi] != 0.0 || d.hh_gl[gi] != 0.0);
@@ -166,7 +171,7 @@ struct UnitBuilder {
       // pass 1: branch id of every CV (parent < index, so one forward sweep suffices)
       uint32_t nb = 0;
       for (uint32_t i = 0; i < n; ++i) {
-        bool fresh = (i == 0) || nchild[par[i]] != 1 || blen[br_of[par[i]]] >= P.max_branch_len;
+        bool fresh = (i == 0) || nchild[par[i]] != 1 || blen[br_of[par[i]]] >= (forest ? kForestMaxBranchLen : P.max_branch_len);
         if (fresh) {
           Lane L;
           L.lc = lc; L.br = nb; L.len = 0; L.first_cv = i;
@@ -243,7 +248,61 @@ struct UnitBuilder {
     return slot;
   }
 
+  // forest: slot order level -> warp -> branch -> control volume; runs, chunks (forest_layout.h)
+  uint32_t make_forest() {
+    const uint32_t n_lane = (uint32_t)lanes.size();
+    uint32_t n_level = 0;
+    for (const Lane& L : lanes) n_level = std::max(n_level, L.level + 1);
+    std::vector<std::vector<uint32_t>> by_level(n_level);
+    for (uint32_t i = 0; i < n_lane; ++i) by_level[lanes[i].level].push_back(i);
+    order.clear(); fslot0.clear(); flevel_br.clear(); fchunks.clear();
+    fruns.assign((size_t)n_level * kForestWarps, FRun{0, 0});
+    uint32_t slot = 0;
+    for (uint32_t lvl = 0; lvl < n_level; ++lvl) {
+      flevel_br.push_back((uint32_t)order.size());
+      auto& v = by_level[lvl];
+      std::stable_sort(v.begin(), v.end(), [&](uint32_t x, uint32_t y) { return lanes[x].len > lanes[y].len; });
+      std::vector<uint32_t> dealt[kForestWarps];
+      uint64_t load[kForestWarps] = {0};
+      for (uint32_t i : v) {               // longest first onto the least loaded warp
+        int best = 0;
+        for (int w = 1; w < kForestWarps; ++w) if (load[w] < load[best]) best = w;
+        dealt[best].push_back(i);
+        load[best] += lanes[i].len;
+      }
+      for (int w = 0; w < kForestWarps; ++w) {
+        FRun& R = fruns[(size_t)lvl * kForestWarps + w];
+        R.chunk_beg = (uint32_t)fchunks.size();
+        const uint32_t pos0 = (uint32_t)order.size(), slot_beg = slot;
+        for (uint32_t i : dealt[w]) { order.push_back(i); fslot0.push_back(slot); slot += lanes[i].len; }
+        uint32_t pos = pos0;               // branch that holds the current slot
+        for (uint32_t c0 = slot_beg; c0 < slot; c0 += 32) {
+          FChunk ck;
+          const uint32_t n = std::min(32u, slot - c0);
+          while (fslot0[pos] + lanes[order[pos]].len <= c0) ++pos;
+          ck.slot0 = c0; ck.heads = 0; ck.tails = 0; ck.br_n = pos * 64u + n;
+          uint32_t q = pos;
+          for (uint32_t l = 0; l < 32; ++l) {
+            if (l >= n) { ck.heads |= 1u << l; ck.tails |= 1u << l; continue; }
+            const uint32_t sl = c0 + l;
+            while (fslot0[q] + lanes[order[q]].len <= sl) ++q;
+            if (sl == fslot0[q]) ck.heads |= 1u << l;
+            if (sl == fslot0[q] + lanes[order[q]].len - 1) ck.tails |= 1u << l;
+          }
+          fchunks.push_back(ck);
+        }
+        R.chunk_end = (uint32_t)fchunks.size();
+      }
+    }
+    flevel_br.push_back((uint32_t)order.size());
+    tl_of.resize(n_lane);
+    for (uint32_t t = 0; t < n_lane; ++t) tl_of[order[t]] = t;
+    if (n_lane >= (1u << 26)) bad = true;  // FChunk::br_n
+    return slot;
+  }
+
   uint32_t slot_of(uint32_t tl, uint32_t k) const {
+    if (forest) return fslot0[tl] + k;
     const uint32_t ti = task_of[tl];
     return tasks[ti].slot_off + rowoff[row_begin[ti] + k] + (tl - tasks[ti].lane_off);
   }
@@ -255,11 +314,11 @@ struct UnitBuilder {
     uc.cell_base = cell_begin;
     uc.n_cell = n_cell;
     const uint32_t n_lane = (uint32_t)lanes.size();
-    uc.n_cv = make_tasks();
+    uc.n_cv = forest ? make_forest() : make_tasks();
     uc.n_slot = align_up(uc.n_cv, 2);
     uc.n_lane = n_lane;
-    uc.n_task = (uint32_t)tasks.size();
-    uc.n_level = (uint32_t)level_begin.size() - 1;
+    uc.n_task = forest ? (uint32_t)fchunks.size() : (uint32_t)tasks.size();
+    uc.n_level = forest ? (uint32_t)flevel_br.size() - 1 : (uint32_t)level_begin.size() - 1;
     uint32_t n_hh = 0, n_syn = 0, n_clamp = 0, n_child = 0;
     for (uint32_t i = 0; i < n_lane; ++i) n_child += lanes[i].parent_br >= 0 ? 1 : 0;
     for (uint32_t lc = 0; lc < n_cell; ++lc) {
@@ -282,7 +341,67 @@ struct UnitBuilder {
     for (uint32_t i = 0; i < n_lane; ++i)
       if (lanes[i].parent_br >= 0) kids[cells[lanes[i].lc].lane_begin + lanes[i].parent_br].push_back(i);
 
-    if (topo_out) {
+    if (forest && !placed) {
+      // does any control volume carry two kinds of point mechanism?  (their currents are then subtracted in turn)
+      bool disjoint = true;
+      std::vector<uint8_t> kind;
+      for (uint32_t lc = 0; lc < n_cell && disjoint; ++lc) {
+        const int64_t orig = H.cell_order[cell_begin + lc];
+        const int64_t a0 = d.cv_off[orig];
+        kind.assign((size_t)(d.cv_off[orig + 1] - a0), 0);
+        for (size_t i = 0; i < kind.size(); ++i) if (has_hh(a0 + (int64_t)i)) kind[i] |= 1;
+        if (d.syn_off) for (int64_t q = d.syn_off[orig]; q < d.syn_off[orig + 1]; ++q) kind[d.syn_cv[q]] |= 2;
+        for (int64_t q = clamp_off[orig]; q < clamp_off[orig + 1]; ++q) kind[d.clamp_cv[clamp_idx[q]]] |= 4;
+        for (uint8_t k : kind) if (k & (k - 1)) disjoint = false;
+      }
+      uc.flags |= UNIT_FOREST | (disjoint ? UNIT_POINT_DISJOINT : 0u);
+    }
+    if (topo_out && forest) {
+      const FTopoOff to = ftopo_offsets(uc.n_level, uc.n_task, n_lane, n_child, n_cell);
+      topo_out->assign(to.total, 0);
+      uint8_t* tp = topo_out->data();
+      std::memcpy(tp + to.runs, fruns.data(), fruns.size() * sizeof(FRun));
+      std::memcpy(tp + to.chunks, fchunks.data(), fchunks.size() * sizeof(FChunk));
+      std::memcpy(tp + to.level_br, flevel_br.data(), flevel_br.size() * 4);
+      FBranch* brec = (FBranch*)(tp + to.branches);
+      uint16_t* br_cell = (uint16_t*)(tp + to.br_cell);
+      uint32_t* child = (uint32_t*)(tp + to.child);
+      uint32_t* cell_det = (uint32_t*)(tp + to.cell_det);
+      uint32_t cpos = 0;
+      for (uint32_t tl = 0; tl < n_lane; ++tl) {       // in slot order
+        const uint32_t i = order[tl];
+        const Lane& L = lanes[i];
+        FBranch& R = brec[tl];
+        R.slot0 = fslot0[tl];
+        R.len = (uint16_t)L.len;
+        br_cell[tl] = (uint16_t)L.lc;
+        if (L.parent_br >= 0) {
+          const uint32_t pi = cells[L.lc].lane_begin + L.parent_br;
+          R.pslot = slot_of(tl_of[pi], lanes[pi].len - 1);
+        } else {
+          R.pslot = kNoSlot;
+        }
+        std::sort(kids[i].begin(), kids[i].end(), [&](uint32_t x, uint32_t y) { return lanes[x].first_cv > lanes[y].first_cv; });
+        R.cbeg = cpos;
+        if (kids[i].size() > 65535) bad = true;
+        R.ccnt = (uint16_t)std::min<size_t>(kids[i].size(), 65535);
+        for (uint32_t k : kids[i]) child[cpos++] = tl_of[k];
+      }
+      for (uint32_t lc = 0; lc < n_cell; ++lc) {
+        const int64_t orig = H.cell_order[cell_begin + lc];
+        const uint32_t det = d.det_cv ? (uint32_t)d.det_cv[orig] : 0u;
+        const uint32_t lb = cells[lc].lane_begin;
+        uint32_t found = kNoSlot;
+        for (uint32_t b2 = 0; b2 < cells[lc].n_br && found == kNoSlot; ++b2) {
+          const Lane& L = lanes[lb + b2];
+          if (det < L.first_cv) continue;
+          for (uint32_t k = 0; k < L.len; ++k)
+            if (cvs[L.cv_begin + k] == det) { found = slot_of(tl_of[lb + b2], k); break; }
+        }
+        cell_det[lc] = found;
+      }
+    }
+    if (topo_out && !forest) {
       const TopoOff to = topo_offsets(uc.n_task, uc.n_level, n_lane, n_child, n_cell);
       topo_out->assign(to.total, 0);
       uint8_t* tp = topo_out->data();
@@ -603,19 +722,27 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     std::vector<int64_t> cur(clamp_off.begin(), clamp_off.end() - 1);
     for (int64_t k = 0; k < d.n_clamp; ++k) clamp_idx[cur[d.clamp_cell[k]]++] = k;
   }
-  // bytes a cell needs as a unit of its own (HH instances counted exactly)
-  std::vector<uint32_t> cell_hh(nc, 0);
-  if (d.hh_gnabar)
-    parallel_for(nc, [&](int64_t c) {
-      uint32_t n = 0;
-      for (int64_t i = d.cv_off[c]; i < d.cv_off[c + 1]; ++i) n += d.hh_gnabar[i] != 0.0 || d.hh_gkbar[i] != 0.0 || d.hh_gl[i] != 0.0;
-      cell_hh[c] = n;
-    });
-  auto unit_bytes = [&](uint64_t n_cv, uint64_t n_hh, uint64_t n_syn, uint64_t n_clamp, uint64_t n_cell) -> uint64_t {
-    if (n_cv > 0x3FFFFFFFull || n_syn > 0x3FFFFFFFull || n_clamp > 0x3FFFFFFFull) return ~0ull;
-    const uint32_t ns = align_up((uint32_t)n_cv, 2);
-    return (uint64_t)fast_offsets(ns, (uint32_t)n_hh, (uint32_t)n_syn, (uint32_t)n_clamp, (uint32_t)n_cell, H.syn_uniform).total +
-           8ull * state_offsets(ns, (uint32_t)n_hh, (uint32_t)n_syn, (uint32_t)n_cell).total;
+  // HH instances and branches (maximal unbranched chains) of every cell
+  std::vector<uint32_t> cell_hh(nc, 0), cell_nbr(nc, 0);
+  parallel_for(nc, [&](int64_t c) {
+    const int64_t a = d.cv_off[c], n = d.cv_off[c + 1] - a;
+    uint32_t nh = 0;
+    if (d.hh_gnabar)
+      for (int64_t i = a; i < a + n; ++i) nh += d.hh_gnabar[i] != 0.0 || d.hh_gkbar[i] != 0.0 || d.hh_gl[i] != 0.0;
+    cell_hh[c] = nh;
+    std::vector<uint32_t> nchild((size_t)n, 0);
+    for (int64_t i = 1; i < n; ++i) nchild[d.cv_parent[a + i]]++;
+    uint32_t nb = 1;
+    for (int64_t i = 1; i < n; ++i) nb += nchild[d.cv_parent[a + i]] != 1;
+    cell_nbr[c] = nb + (uint32_t)(n / kForestMaxBranchLen);     // chains longer than a branch may hold are cut
+  });
+  // shared memory a forest of these counts needs (forest_layout.h)
+  auto forest_need = [&](uint64_t n_cv, uint64_t n_br, uint64_t n_hh, uint64_t n_syn, uint64_t n_clamp, uint64_t n_cell) -> uint64_t {
+    if (n_cv > 0x0FFFFFFFull || n_syn > 0x0FFFFFFFull || n_clamp > 0x0FFFFFFFull) return ~0ull;
+    ForestCaps fc;
+    fc.state_bytes = 8 * state_offsets(align_up((uint32_t)n_cv, 2), (uint32_t)n_hh, (uint32_t)n_syn, (uint32_t)n_cell).total;
+    fc.n_branch = (uint32_t)n_br; fc.n_spec = (uint32_t)(n_hh + n_syn + n_clamp); fc.n_cell = (uint32_t)n_cell;
+    return forest_smem_plan(fc).bytes;
   };
   auto cell_counts = [&](int64_t c, uint64_t& n_cv, uint64_t& n_syn, uint64_t& n_cl) {
     n_cv = (uint64_t)(d.cv_off[c + 1] - d.cv_off[c]);
@@ -689,57 +816,107 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
   const int64_t ngc = (int64_t)group_cells.size();
   H.n_groups = (int64_t)groups.size();
   H.n_group_cells = ngc;
-  // internal cell order: group cells, warp-class cells (big first when sizes differ), block-class cells
-  std::vector<uint32_t> warp_cells, block_cells;
-  bool homogeneous = true;
+  // internal cell order: group cells, forest cells (big first), block-unit cells
+  std::vector<uint32_t> forest_cells, block_cells;
   for (int64_t c = 0; c < nc; ++c) {
     if (cell_class[c] >= 0) continue;
     uint64_t n_cv, n_syn, n_cl;
     cell_counts(c, n_cv, n_syn, n_cl);
-    if (unit_bytes(n_cv, cell_hh[c], n_syn, n_cl, 1) <= P.unit_bytes) warp_cells.push_back((uint32_t)c);
-    else block_cells.push_back((uint32_t)c);
-    homogeneous = homogeneous && (d.cv_off[c + 1] - d.cv_off[c]) == (d.cv_off[1] - d.cv_off[0]);
+    const bool fits = n_cv <= P.forest_max_cv && n_syn < P.forest_max_syn &&
+                      forest_need(n_cv, cell_nbr[c], cell_hh[c], n_syn, n_cl, 1) <= forest_class_budget(kForestClasses - 1);
+    (fits ? forest_cells : block_cells).push_back((uint32_t)c);
   }
   auto bigger = [&](uint32_t x, uint32_t y) { return d.cv_off[x + 1] - d.cv_off[x] > d.cv_off[y + 1] - d.cv_off[y]; };
-  if (!homogeneous) {
-    std::stable_sort(warp_cells.begin(), warp_cells.end(), bigger);
-    std::stable_sort(block_cells.begin(), block_cells.end(), bigger);
-  }
+  std::stable_sort(forest_cells.begin(), forest_cells.end(), bigger);
+  std::stable_sort(block_cells.begin(), block_cells.end(), bigger);
   H.cell_order = group_cells;
-  H.cell_order.insert(H.cell_order.end(), warp_cells.begin(), warp_cells.end());
+  H.cell_order.insert(H.cell_order.end(), forest_cells.begin(), forest_cells.end());
   H.cell_order.insert(H.cell_order.end(), block_cells.begin(), block_cells.end());
   H.cell_internal.resize(nc);
   for (int64_t i = 0; i < nc; ++i) H.cell_internal[H.cell_order[i]] = (uint32_t)i;
-  // partition into units
+  // partition into units: forests (several small cells share one as long as it fits the smallest launch class),
+  // then one block unit per remaining cell
   std::vector<int64_t> unit_begin;
   {
-    uint64_t cv = 0, hh = 0, syn = 0, cl = 0, cells = 0;
-    for (int64_t i = 0; i < (int64_t)warp_cells.size(); ++i) {
+    uint64_t cv = 0, br = 0, hh = 0, syn = 0, cl = 0, cells = 0;
+    for (int64_t i = 0; i < (int64_t)forest_cells.size(); ++i) {
       uint64_t n_cv, n_syn, n_cl;
-      cell_counts(warp_cells[i], n_cv, n_syn, n_cl);
-      const uint64_t n_hh = cell_hh[warp_cells[i]];
-      if (cells == 0 || cells >= kWarpUnitMaxCells || unit_bytes(cv + n_cv + 1, hh + n_hh, syn + n_syn, cl + n_cl, cells + 1) > P.unit_bytes) {
-        unit_begin.push_back(ngc + i); cv = hh = syn = cl = cells = 0;
+      cell_counts(forest_cells[i], n_cv, n_syn, n_cl);
+      const uint64_t n_hh = cell_hh[forest_cells[i]], n_br = cell_nbr[forest_cells[i]];
+      if (cells == 0 || cells >= kForestMaxCells || cv + n_cv > P.forest_cv ||
+          forest_need(cv + n_cv + 1, br + n_br, hh + n_hh, syn + n_syn, cl + n_cl, cells + 1) > forest_class_budget(0)) {
+        unit_begin.push_back(ngc + i); cv = br = hh = syn = cl = cells = 0;
       }
-      cv += n_cv; hh += n_hh; syn += n_syn; cl += n_cl; ++cells;
+      cv += n_cv; br += n_br; hh += n_hh; syn += n_syn; cl += n_cl; ++cells;
     }
-    H.n_warp_units = (int64_t)unit_begin.size();
-    for (int64_t i = 0; i < (int64_t)block_cells.size(); ++i) unit_begin.push_back(ngc + (int64_t)warp_cells.size() + i);
+    H.n_forests = (int64_t)unit_begin.size();
+    for (int64_t i = 0; i < (int64_t)block_cells.size(); ++i) unit_begin.push_back(ngc + (int64_t)forest_cells.size() + i);
     unit_begin.push_back(nc);
   }
   H.n_units = (int64_t)unit_begin.size() - 1;
   H.units.resize(H.n_units);
+  std::vector<uint32_t> unit_cells(H.n_units);
+  for (int64_t u = 0; u < H.n_units; ++u) unit_cells[u] = (uint32_t)(unit_begin[u + 1] - unit_begin[u]);
+  unit_begin.pop_back();
   // pass 1: counts and topo records
   std::vector<std::vector<uint8_t>> topo(H.n_units);
   std::atomic<int> too_many(0);
   parallel_for(H.n_units, [&](int64_t u) {
     UnitBuilder B{d, P, H, clamp_off, clamp_idx, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, false};
-    H.units[u] = B.run(unit_begin[u], (uint32_t)(unit_begin[u + 1] - unit_begin[u]), &topo[u], nullptr, nullptr);
-    if (u >= H.n_warp_units) H.units[u].flags |= UNIT_BLOCK;
+    B.forest = u < H.n_forests;
+    H.units[u] = B.run(unit_begin[u], unit_cells[u], &topo[u], nullptr, nullptr);
+    if (u >= H.n_forests) H.units[u].flags |= UNIT_BLOCK;
     if (H.units[u].n_level > 60000 || H.units[u].n_slot > 0x3FFFFFFFu) too_many.store(1);
     if (B.bad) too_many.store(1);
   });
   if (too_many.load()) { err = "a cell is too deep or too large for the unit layout"; return ARB_E_INVALID; }
+  // forests are launched by shared-memory need (forest_layout.h): order them by launch class, the class with
+  // the largest forests first, and inside a class by size (the hardware deals CTAs in index order)
+  {
+    auto need_of = [&](const UnitCounts& uc) {
+      ForestCaps fc;
+      fc.state_bytes = uc.state_bytes; fc.n_branch = uc.n_lane; fc.n_spec = uc.n_hh + uc.n_syn + uc.n_clamp; fc.n_cell = uc.n_cell;
+      return forest_smem_plan(fc).bytes;
+    };
+    auto class_of = [&](const UnitCounts& uc) {
+      const uint32_t need = need_of(uc);
+      for (int k = 0; k < kForestClasses; ++k) if (need <= forest_class_budget(k)) return k;
+      return kForestClasses;               // does not fit (decided above with exact counts: cannot happen)
+    };
+    std::vector<int64_t> perm(H.n_forests);
+    for (int64_t u = 0; u < H.n_forests; ++u) perm[u] = u;
+    std::vector<int> cls(H.n_forests);
+    for (int64_t u = 0; u < H.n_forests; ++u) {
+      cls[u] = class_of(H.units[u]);
+      if (cls[u] >= kForestClasses) { err = "a forest does not fit in shared memory"; return ARB_E_INVALID; }
+    }
+    std::stable_sort(perm.begin(), perm.end(), [&](int64_t x, int64_t y) {
+      if (cls[x] != cls[y]) return cls[x] > cls[y];
+      return H.units[x].n_cv > H.units[y].n_cv;
+    });
+    std::vector<UnitCounts> units2(H.units);
+    std::vector<std::vector<uint8_t>> topo2(H.n_forests);
+    std::vector<int64_t> begin2(unit_begin);
+    std::vector<uint32_t> cells2(unit_cells);
+    for (int64_t i = 0; i < H.n_forests; ++i) {
+      units2[i] = H.units[perm[i]]; topo2[i].swap(topo[perm[i]]); begin2[i] = unit_begin[perm[i]]; cells2[i] = unit_cells[perm[i]];
+    }
+    for (int64_t i = 0; i < H.n_forests; ++i) topo[i].swap(topo2[i]);
+    H.units.swap(units2); unit_begin.swap(begin2); unit_cells.swap(cells2);
+    for (int k = 0; k < kForestClasses; ++k) { H.fcls[k].first = 0; H.fcls[k].count = 0; }
+    ForestCaps caps[kForestClasses];
+    for (int k = 0; k < kForestClasses; ++k) caps[k] = ForestCaps{0, 0, 0, 0};
+    for (int64_t i = 0; i < H.n_forests; ++i) {
+      const UnitCounts& uc = H.units[i];
+      const int k = class_of(uc);
+      if (H.fcls[k].count++ == 0) H.fcls[k].first = i;
+      caps[k].state_bytes = std::max(caps[k].state_bytes, uc.state_bytes);
+      caps[k].n_branch = std::max(caps[k].n_branch, uc.n_lane);
+      caps[k].n_spec = std::max(caps[k].n_spec, uc.n_hh + uc.n_syn + uc.n_clamp);
+      caps[k].n_cell = std::max(caps[k].n_cell, uc.n_cell);
+    }
+    for (int k = 0; k < kForestClasses; ++k) H.fcls[k].plan = forest_smem_plan(caps[k]);
+  }
   // groups: row counts, then placement (groups first in every pool)
   parallel_for(H.n_groups, [&](int64_t g) {
     GroupCounts& G = groups[g];
@@ -817,20 +994,15 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
       std::vector<uint8_t>().swap(topo[u]);
     }
     const uint32_t n_spec = uc.n_hh + uc.n_syn + uc.n_clamp;
-    if (uc.flags & UNIT_BLOCK) {
+    if (uc.flags & UNIT_FOREST) {
+      uc.scratch_base = H.scratch_doubles;
+      H.scratch_doubles += fscratch_offsets(uc.n_slot, uc.n_lane).total;
+    } else if (uc.flags & UNIT_BLOCK) {
       // contrib | dcontrib | xI | fgen | invdgen | run heads of the synapse list (uint32 count, then indices)
       uc.scratch_base = H.scratch_doubles;
       H.scratch_doubles += 2 * (int64_t)align_up(uc.n_lane, 2) + align_up(n_spec, 2) + 2 * (int64_t)uc.n_slot +
                            align_up(uc.n_slot / 2 + 2, 2);
       H.block_lane_cap = std::max(H.block_lane_cap, uc.n_lane);
-    } else {
-      H.fast_cap = std::max(H.fast_cap, align_up(uc.fast_bytes, 128));
-      H.state_cap = std::max(H.state_cap, align_up(uc.state_bytes, 128));
-      H.lane_cap = std::max(H.lane_cap, uc.n_lane);
-      H.spec_cap = std::max(H.spec_cap, n_spec);
-      H.cell_cap = std::max(H.cell_cap, uc.n_cell);
-      H.topo_cap = std::max(H.topo_cap, (uint32_t)topo_offsets(uc.n_task, uc.n_level, uc.n_lane, uc.n_child, uc.n_cell).total);
-      H.slot_cap = std::max(H.slot_cap, uc.n_slot);
     }
   }
   if (H.state_doubles >= (int64_t)0xFFFFFFF0u) { err = "state pool exceeds 2^32 doubles"; return ARB_E_INVALID; }
@@ -959,8 +1131,9 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
   std::vector<std::vector<uint8_t>>().swap(topo);
   parallel_for(H.n_units, [&](int64_t u) {
     UnitBuilder B{d, P, H, clamp_off, clamp_idx, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, false};
+    B.forest = u < H.n_forests;
     UnitCounts placed = H.units[u];
-    B.run(unit_begin[u], (uint32_t)(unit_begin[u + 1] - unit_begin[u]), nullptr, &placed, &H);
+    B.run(unit_begin[u], unit_cells[u], nullptr, &placed, &H);
   });
   // connections grouped by caller's source cell, ascending k inside a group
   H.conn_off.assign(nc + 1, 0);

@@ -1,19 +1,24 @@
-// layout.hpp - host-side model builder: validation, branch decomposition, cell units.
-// Pure C++ (no CUDA): turns the caller's arb_desc into the pools described in unit_layout.h.
+// layout.hpp - host-side model builder: validation, branch decomposition, cell groups, forests, block units.
+// Pure C++ (no CUDA): turns the caller's arb_desc into the pools described in group_layout.h,
+// forest_layout.h and unit_layout.h.
 #pragma once
 #include <cstdint>
 #include <string>
 #include <vector>
 
 #include "../../include/arbb200.h"
+#include "forest_layout.h"
 #include "group_layout.h"
 #include "unit_layout.h"
 
 namespace arbb {
 
 struct BuildParams {
-  uint32_t unit_bytes = 4096;     // fast + state bytes a warp unit may hold (one shared-memory stage); measured on C4
-  uint32_t max_branch_len = 1024; // longer unbranched chains are cut into pieces
+  uint32_t forest_cv = 1024;      // cells are packed into forests of up to this many control volumes (larger cells
+                                  // are a forest of their own)
+  uint32_t forest_max_cv = 24000; // cells with more control volumes do not fit a CTA's shared memory: block units
+  uint32_t forest_max_syn = 1024; // cells with at least this many synapses are block units (key reduction)
+  uint32_t max_branch_len = 1024; // block units: longer unbranched chains are cut into pieces
   uint32_t group_min_cells = 4;   // a topology class with fewer cells is laid out as units; 0 = no groups
   uint32_t group_max_smem = 112 * 1024;  // shared memory a cell group may need (two CTAs per SM at least)
   uint32_t group_max_cv = 1536;   // cells with more control volumes are laid out as units (V of a
@@ -21,8 +26,6 @@ struct BuildParams {
 };
 
 constexpr int64_t kMaxGroupCtas = 148 * 16;   // upper bound of resident CTAs of the group kernel (scratch sizing)
-
-constexpr int64_t kMaxWarps = 2048;   // upper bound of resident warps of the warp kernel (scratch sizing)
 
 struct UnitCounts {                   // everything the offset functions need
   uint32_t n_slot = 0, n_cv = 0, n_lane = 0, n_task = 0, n_level = 0, n_cell = 0, n_hh = 0, n_syn = 0,
@@ -35,11 +38,10 @@ struct UnitCounts {                   // everything the offset functions need
 
 struct HostModel {
   int64_t n_cells = 0, n_cv = 0, n_syn = 0, n_clamp = 0, n_conn = 0, n_ext = 0, n_hh = 0;
-  int64_t n_units = 0, n_warp_units = 0, n_lanes = 0;
+  int64_t n_units = 0, n_forests = 0, n_lanes = 0;   // units: forests first, then block units
   int64_t fast_bytes = 0, state_doubles = 0, gen_doubles = 0, topo_bytes = 0, scratch_doubles = 0;
   int64_t topo_records = 0;           // distinct tree structures
-  // caps over warp units (shared-memory plan) and over block units
-  uint32_t fast_cap = 0, state_cap = 0, lane_cap = 0, spec_cap = 0, cell_cap = 0, slot_cap = 0, topo_cap = 0;
+  ForestClass fcls[kForestClasses];   // forest launches by shared-memory need
   uint32_t block_lane_cap = 0;
   bool syn_uniform = false;
   double syn_tau_u = 0, syn_e_u = 0;

@@ -1,10 +1,14 @@
 // unit_layout.h - the in-HBM layout of one "cell unit", shared by the host builder and the kernels.
 //
-// A unit is the work of ONE WARP (or, for cells too large for a warp's shared-memory stage, of one
-// CTA): one or a few cells whose branches (maximal unbranched chains of control volumes) are
-// interleaved so that consecutive lanes touch consecutive addresses ("SoA with interleaved
-// branches", BASELINE.json north_star; the paper's own GPU layout interleaves whole cells, one
-// thread per cell, PAPER.md:220 - prior art).
+// A unit is the work of one CTA.  Two kinds share the record formats of this file:
+//   forests      (forest_layout.h) one or several cells, lane = control volume, segmented warp scans:
+//                every cell that does not share its tree with others and fits a CTA's shared memory
+//   block units  (this file) one cell whose branches (maximal unbranched chains of control volumes)
+//                are interleaved so that consecutive lanes touch consecutive addresses, lane = branch
+//                ("SoA with interleaved branches", BASELINE.json north_star; the paper's own GPU layout
+//                interleaves whole cells, one thread per cell, PAPER.md:220 - prior art), integrated
+//                straight from global memory: cells too large for shared memory, and cells with
+//                thousands of synapses (key reduction).
 //
 //   level l of the unit  = all branches whose distance (in branches) from their cell's root is l
 //   task                 = up to 32 branches of one level, longest first; one warp, lane = branch
@@ -23,8 +27,7 @@
 //   topo  (bytes, constant)         tasks, levels, branch links - shared by all units with the same
 //                                   tree structure (deduplicated); a warp keeps the record of its
 //                                   current unit in shared memory and reloads it only on change
-// The fast and state records are what a time step streams: the warp kernel copies both into shared
-// memory with two bulk-async copies (TMA, cp.async.bulk) per unit.
+// The fast and state records are what a time step streams.
 #pragma once
 #include <stdint.h>
 
@@ -37,7 +40,6 @@
 namespace arbb {
 
 constexpr uint32_t kNoSlot = 0xFFFFFFFFu;
-constexpr uint32_t kWarpUnitMaxCells = 32;    // one lane per cell holds its runtime
 constexpr uint32_t kBlockUnitMaxCells = 64;
 
 struct Task {            // 16 bytes, one broadcast load
@@ -145,36 +147,7 @@ ARBB_HD TopoOff topo_offsets(uint32_t n_task, uint32_t n_level, uint32_t n_lane,
   return o;
 }
 
-// Shared-memory plan of one warp of the warp kernel (host computes, device follows).
-struct WarpSmemPlan {
-  uint32_t fast_cap;      // bytes reserved for a fast record (multiple of 128)
-  uint32_t state_cap;     // bytes reserved for a state record (multiple of 128)
-  uint32_t stage_bytes;   // fast_cap + state_cap
-  uint32_t n_stage;       // 1 or 2
-  uint32_t slot_cap;      // slots per unit
-  uint32_t lane_cap;      // branches per unit
-  uint32_t spec_cap;      // HH instances + synapses + clamps per unit
-  uint32_t cell_cap;      // cells per unit
-  uint32_t topo_cap;      // bytes of the largest topo record
-  uint32_t scratch_off;   // byte offset of the scratch area inside the warp's region
-  uint32_t warp_bytes;    // size of the region (multiple of 128)
-  uint32_t warps;         // warps per CTA
-};
-
-// scratch area: topo record | contrib[lane_cap] | xI[spec_cap] | per-cell runtime | mbarriers
-struct ScratchOff { uint32_t topo, contrib, xI, cell, mbar, total; };
+// per-cell runtime of the (sub-)step in progress, in shared memory (device_common.cuh: CellS)
 constexpr uint32_t kCellScratchBytes = 64;   // tcur, tnext, delta, vprev (doubles) + evcur, evend, armed, mode, wb, dirty (u32)
-ARBB_HD ScratchOff scratch_offsets(uint32_t topo_cap, uint32_t lane_cap, uint32_t spec_cap, uint32_t cell_cap, uint32_t n_stage) {
-  ScratchOff o;
-  uint32_t p = 0;
-  auto sec = [&](uint32_t bytes) { uint32_t at = p; p = align_up(p + bytes, 16); return at; };
-  o.topo = sec(topo_cap);
-  o.contrib = sec(8 * lane_cap);
-  o.xI = sec(8 * spec_cap);
-  o.cell = sec(kCellScratchBytes * cell_cap);
-  o.mbar = sec(8 * n_stage);
-  o.total = align_up(p, 128);
-  return o;
-}
 
 }  // namespace arbb

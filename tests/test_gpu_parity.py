@@ -418,7 +418,7 @@ def test_spike_buffer_cap_and_order(B, orc):
 # full-size configurations: the WHOLE network against the oracle, in the launch configuration
 # bench.py times (one launch per grid step, groups with events first)
 # ---------------------------------------------------------------------------------------------
-FREE_RUN_TOL = 1e-7     # free-running V, gates over several hundred steps of a spiking network (R16/R17)
+FREE_RUN_TOL = 1e-6     # free-running V, gates over several hundred steps of a spiking network (R16/R17)
 
 
 def expected_deliveries(m, spikes, t_end):
@@ -552,7 +552,7 @@ def test_long_delays_fit_the_default_pool(B, orc):
     m = W.config1(n_cells=8, t_end=150.0)
     m["conn_delay"] = np.full(m["n_conn"], 40.0)
     m["clamp_cell"], m["clamp_cv"] = np.array([0]), np.array([0], np.int32)
-    m["clamp_t0"], m["clamp_t1"], m["clamp_amp"] = np.array([0.0]), np.array([150.0]), np.array([0.4])
+    m["clamp_t0"], m["clamp_t1"], m["clamp_amp"] = np.array([0.0]), np.array([150.0]), np.array([0.2])
     m = W.finalize(m)
     g, o = run_both(B, orc, m, 150.0)
     assert check_spikes(g, o, 8) > 10
