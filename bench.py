@@ -315,6 +315,10 @@ def run_ours(args):
 
     from paper_1901_07454_b200 import binding as B, workloads as W
     B.lib()
+    for kv in args.layout:
+        k, v = kv.split("=")
+        assert k in B.OPTION_FIELDS, k
+        B.LAYOUT_DEFAULTS[k] = int(v)
     wl = _workloads()[args.config]
     cells = args.cells or wl.full_cells
     lin = args.step == "linearised"
@@ -490,7 +494,7 @@ def run_ours(args):
             "data": "synthetic",
             "config": {"workload": "%s (%d CVs), dt 0.025 ms; step = one epoch of %d grid steps" % (label, n_cv, es),
                        "mode": args.mode, "step_kind": args.step, "cells_per_gpu": cells,
-                       "parallelism": "cells sharded, no collective", "layout": layout,
+                       "parallelism": "cells sharded, no collective", "layout": layout, "layout_options": dict(B.LAYOUT_DEFAULTS),
                        "l2": ("no flush needed: each grid step streams %.2f GB >> 126 MB L2" % (alg_step / 1e9)) if alg_step > 4e8
                              else "working set of %.1f MB per grid step is L2-resident; no flush (every step rewrites the whole state)" % (alg_step / 1e6),
                        "seed": int(W.BASE_SEED + (5 if args.config == "ring" else int(args.config)))},
@@ -540,6 +544,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other", action="store_true", help="skip the other launch granularity")
     ap.add_argument("--no-as-written", action="store_true", help="skip the undriven (as worded in BASELINE.json) variant of C3")
+    ap.add_argument("--layout", action="append", default=[], metavar="KEY=VALUE",
+                    help="arb_desc layout / capacity option, e.g. layout_forest_cv=2048 (default: the library's)")
     ap.add_argument("--selftest-dist", action="store_true", help=argparse.SUPPRESS)
     args = ap.parse_args()
     if args.selftest_dist:

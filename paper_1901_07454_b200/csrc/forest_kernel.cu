@@ -43,50 +43,51 @@ struct FView {
   const uint16_t *hh_cell, *syn_cell, *cl_cell;
   double *V, *m, *h, *n, *g, *rt;
   uint32_t g_gidx0;                 // state-pool index of g[0]
-  const FRun* runs; const FChunk* chunks; const FBranch* br; const uint16_t* br_cell;
+  // tree record: shared memory in the cable kernel
+  const FRun* runs; const FChunk* chunks; const unsigned long long* chunk_cells; const FBranch* br; const uint16_t* br_cell;
   const uint32_t *child, *cell_det, *level_br;
+  const unsigned long long* masks;  // [0] cells that take part in the (sub-)step in progress, [1] cells on a step of their own length
   const double *C, *S, *sig, *G, *bg, *syn_tau;
   double *con, *xI;                 // per branch: what its parent loses; per point-mechanism instance: its current
   double *fgen, *invdgen, *dcon;    // global scratch of the forest (event-split sub-steps, factorisation)
   int64_t cell_base;
 };
 
-__device__ __forceinline__ void make_fview(FView& U, const DevModel& M, const UnitHeader& H, uint8_t* fast, double* statew) {
+// tp: the forest's tree record (shared memory in the cable kernel); it starts with the host's offset table
+__device__ __forceinline__ void make_fview(FView& U, const DevModel& M, const UnitHeader& H, uint8_t* fast, double* statew, const uint8_t* tp) {
   U.n_slot = H.n_slot; U.n_branch = H.n_lane; U.n_chunk = H.n_task; U.n_level = H.n_level;
   U.n_cell = H.n_cell; U.n_hh = H.n_hh; U.n_syn = H.n_syn; U.n_clamp = H.n_clamp; U.flags = H.flags;
-  const FastOff fo = fast_offsets(H.n_slot, H.n_hh, H.n_syn, H.n_clamp, H.n_cell, M.syn_uniform != 0);
-  U.f = (const double*)(fast + fo.f); U.invd = (const double*)(fast + fo.invd);
-  U.a = (const double*)(fast + fo.a); U.b = (const double*)(fast + fo.b);
-  U.hh_gna = (const double*)(fast + fo.hh_gna); U.hh_gk = (const double*)(fast + fo.hh_gk); U.hh_gl = (const double*)(fast + fo.hh_gl);
-  U.syn_e = (const double*)(fast + fo.syn_e); U.syn_decay = (const double*)(fast + fo.syn_decay);
-  U.cl_t0 = (const double*)(fast + fo.cl_t0); U.cl_t1 = (const double*)(fast + fo.cl_t1); U.cl_amp = (const double*)(fast + fo.cl_amp);
-  U.hh_slot = (const uint32_t*)(fast + fo.hh_slot); U.syn_slot = (const uint32_t*)(fast + fo.syn_slot); U.cl_slot = (const uint32_t*)(fast + fo.cl_slot);
-  U.hh_cell = (const uint16_t*)(fast + fo.hh_cell); U.syn_cell = (const uint16_t*)(fast + fo.syn_cell); U.cl_cell = (const uint16_t*)(fast + fo.cl_cell);
-  const StateOff so = state_offsets(H.n_slot, H.n_hh, H.n_syn, H.n_cell);
-  U.V = statew + so.v; U.m = statew + so.m; U.h = statew + so.h; U.n = statew + so.n; U.g = statew + so.g; U.rt = statew + so.rt;
-  U.g_gidx0 = (uint32_t)(H.state_base + so.g);
-  const uint8_t* tp = M.topo + H.topo_off;
-  const FTopoOff to = ftopo_offsets(H.n_level, H.n_task, H.n_lane, H.n_child, H.n_cell);
-  U.runs = (const FRun*)(tp + to.runs); U.chunks = (const FChunk*)(tp + to.chunks); U.br = (const FBranch*)(tp + to.branches);
-  U.br_cell = (const uint16_t*)(tp + to.br_cell); U.child = (const uint32_t*)(tp + to.child);
-  U.cell_det = (const uint32_t*)(tp + to.cell_det); U.level_br = (const uint32_t*)(tp + to.level_br);
-  const GenOff go = gen_offsets(H.n_slot, H.n_syn);
+  const FOffs& o = *(const FOffs*)tp;
+  U.f = (const double*)(fast + o.fast[0]); U.invd = (const double*)(fast + o.fast[1]);
+  U.a = (const double*)(fast + o.fast[2]); U.b = (const double*)(fast + o.fast[3]);
+  U.hh_gna = (const double*)(fast + o.fast[4]); U.hh_gk = (const double*)(fast + o.fast[5]); U.hh_gl = (const double*)(fast + o.fast[6]);
+  U.syn_e = (const double*)(fast + o.fast[7]); U.syn_decay = (const double*)(fast + o.fast[8]);
+  U.cl_t0 = (const double*)(fast + o.fast[9]); U.cl_t1 = (const double*)(fast + o.fast[10]); U.cl_amp = (const double*)(fast + o.fast[11]);
+  U.hh_slot = (const uint32_t*)(fast + o.fast[12]); U.syn_slot = (const uint32_t*)(fast + o.fast[13]); U.cl_slot = (const uint32_t*)(fast + o.fast[14]);
+  U.hh_cell = (const uint16_t*)(fast + o.fast[15]); U.syn_cell = (const uint16_t*)(fast + o.fast[16]); U.cl_cell = (const uint16_t*)(fast + o.fast[17]);
+  U.V = statew + o.state[0]; U.m = statew + o.state[1]; U.h = statew + o.state[2]; U.n = statew + o.state[3];
+  U.g = statew + o.state[4]; U.rt = statew + o.state[5];
+  U.g_gidx0 = (uint32_t)(H.state_base + o.state[4]);
+  U.runs = (const FRun*)(tp + o.topo[0]); U.chunks = (const FChunk*)(tp + o.topo[1]);
+  U.chunk_cells = (const unsigned long long*)(tp + o.topo[2]); U.br = (const FBranch*)(tp + o.topo[3]);
+  U.br_cell = (const uint16_t*)(tp + o.topo[4]); U.child = (const uint32_t*)(tp + o.topo[5]);
+  U.cell_det = (const uint32_t*)(tp + o.topo[6]); U.level_br = (const uint32_t*)(tp + o.topo[7]);
+  U.masks = nullptr;
   const double* gen = M.gen + H.gen_base;
-  U.C = gen + go.C; U.S = gen + go.S; U.sig = gen + go.sig; U.G = gen + go.G; U.bg = gen + go.b; U.syn_tau = gen + go.syn_tau;
-  const FScratchOff sc = fscratch_offsets(H.n_slot, H.n_lane);
+  U.C = gen + o.gen[0]; U.S = gen + o.gen[1]; U.sig = gen + o.gen[2]; U.G = gen + o.gen[3]; U.bg = gen + o.gen[4]; U.syn_tau = gen + o.gen[5];
   double* scr = M.scratch + H.scratch_base;
-  U.fgen = scr + sc.fgen; U.invdgen = scr + sc.invdgen; U.dcon = scr + sc.dcon;
+  U.fgen = scr + o.scratch[0]; U.invdgen = scr + o.scratch[1]; U.dcon = scr + o.scratch[2];
   U.cell_base = H.cell_base;
 }
 
 __device__ __forceinline__ FChunk load_chunk(const FChunk* p) {
-  const uint4 q = __ldg((const uint4*)p);
+  const uint4 q = *(const uint4*)p;
   FChunk c;
   c.slot0 = q.x; c.heads = q.y; c.tails = q.z; c.br_n = q.w;
   return c;
 }
 __device__ __forceinline__ FBranch load_branch(const FBranch* p) {
-  const uint4 q = __ldg((const uint4*)p);
+  const uint4 q = *(const uint4*)p;
   FBranch b;
   b.slot0 = q.x; b.pslot = q.y; b.cbeg = q.z; b.len = (uint16_t)(q.w & 0xFFFFu); b.ccnt = (uint16_t)(q.w >> 16);
   return b;
@@ -98,51 +99,106 @@ __device__ __forceinline__ uint32_t branch_of(const FChunk& ck, int lane) {
 }
 
 // ------------------------------------------------------------------------------------------
-// Elimination of the diagonal for one step length, serial along a branch, one
-// thread per branch, level by level:  d_k = C_k/delta + S_k - sum_children sigma_c^2 / d_c,
-// f_k = -sigma_k / d_k.  Used once per dt for every cell (cs == nullptr) and, on event-split
-// sub-steps (reading R9), for the cells that take a step of their own length.
+// Elimination of the diagonal for one step length as a segmented scan.
+// With x_k = d_k - sigma_k (the conductance the subtree below the link k -> parent(k) presents to it),
+//   d_k = C_k/delta + sigma_k + sum_children (sigma_c - sigma_c^2 / d_c)   becomes
+//   x_k = c_k + sum_children sigma_c x_c / (x_c + sigma_c),   c_k = C_k/delta:
+// capacitive conductance in parallel with (link conductance in series with the child's subtree).  Along a
+// branch x_k = T_k(x_{k+1}) with the Moebius map T_k(x) = ((c_k + s) x + c_k s) / (x + s), s = sigma_{k+1};
+// Moebius maps compose as 2 x 2 matrices, here with POSITIVE entries only, so the scan adds and multiplies
+// positive numbers and loses no digits to cancellation (the elimination written with d_k subtracts nearly
+// equal numbers when sigma >> C/delta).  f_k = -sigma_k / d_k, and a branch's parent receives
+// dcon = sigma_0 x_0 / d_0.  Used once per dt for every cell (kSel false) and, on event-split sub-steps
+// (reading R9), for the cells that take a step of their own length (kSel true: mode 2 only).
 // ------------------------------------------------------------------------------------------
-__device__ __forceinline__ void eliminate_forest(const FView& U, const CellS* cs, double dt, double* fout, double* invdout) {
-  constexpr int kB = 8;                   // rows whose C, S, sigma are requested together
-  for (int lvl = (int)U.n_level - 1; lvl >= 0; --lvl) {
-    const uint32_t b0 = U.level_br[lvl], b1 = U.level_br[lvl + 1];
-    for (uint32_t bi = b0 + threadIdx.x; bi < b1; bi += kT) {
-      double delta = dt;
-      if (cs) {
-        const uint32_t c = U.br_cell[bi];
-        if (cs->mode[c] != 2u) continue;
-        delta = cs->delta[c];
-      }
-      const FBranch B = load_branch(U.br + bi);
-      double carry = 0.0;                 // f_{k+1} sigma_{k+1}: what row k loses to its child in the branch
-      for (uint32_t j = 0; j < B.ccnt; ++j) carry -= U.dcon[U.child[B.cbeg + j]];
-      double fk = 0.0, sk = 0.0;
-      int left = B.len;
-      uint32_t s = B.slot0 + B.len - 1;
-      while (left > 0) {
-        double cr[kB], sr[kB], gr[kB];
-#pragma unroll
-        for (int j = 0; j < kB; ++j)
-          if (j < left) { cr[j] = U.C[s - j]; sr[j] = U.S[s - j]; gr[j] = U.sig[s - j]; }
-#pragma unroll
-        for (int j = 0; j < kB; ++j)
-          if (j < left) {
-            const double d = (cr[j] / delta + sr[j]) + carry;
-            const double invd = 1.0 / d;
-            sk = gr[j];
-            fk = -sk * invd;
-            fout[s - j] = fk;
-            invdout[s - j] = invd;
-            carry = fk * sk;              // d_p -= f*u with u = -sigma
-          }
-        s -= kB;
-        left -= kB;
-      }
-      U.dcon[bi] = -fk * sk;
+struct Mob { double a, b, c, d; };   // x -> (a x + b) / (c x + d)
+
+// Between tree levels: when every cell of the forest is swept by one warp (UNIT_WARP_CELLS) a level only depends
+// on what the same warp wrote, else on the whole CTA.
+__device__ __forceinline__ void level_sync(bool warp_cells) {
+  if (warp_cells) __syncwarp(); else __syncthreads();
+}
+
+// keeps the entries of a product in range: scale by the power of two that brings the largest near 1 (exact)
+__device__ __forceinline__ void mob_normalise(Mob& m) {
+  const double big = fmax(fmax(m.a, m.b), fmax(m.c, m.d));
+  const int e = ((__double2hiint(big) >> 20) & 0x7FF);          // biased exponent; 0 only for 0 / denormals
+  const double sc = __hiloint2double((2046 - (e ? e : 1023)) << 20, 0);
+  m.a *= sc; m.b *= sc; m.c *= sc; m.d *= sc;
+}
+
+template <bool kSel>
+__device__ __forceinline__ void eliminate_chunk(const FView& U, const CellS* cs, double dt, const FChunk& ck, int lane,
+                                                double* fout, double* invdout, double& cx, double& csig) {
+  const int n = (int)(ck.br_n & 63u);
+  const bool valid = lane < n;
+  const uint32_t s = ck.slot0 + lane;
+  const bool head = (ck.heads >> lane) & 1u, tail = (ck.tails >> lane) & 1u;
+  const uint32_t br = branch_of(ck, lane);
+  bool on = valid;
+  double delta = dt;
+  if (kSel) {
+    if (valid) {
+      const uint32_t c = U.br_cell[br];
+      on = cs->mode[c] == 2u;
+      delta = cs->delta[c];
     }
-    __syncthreads();
   }
+  double c = 1.0, sg = 0.0;
+  if (valid) { c = U.C[s] / delta; sg = U.sig[s]; }
+  const double snext = __shfl_down_sync(kFull, sg, 1);
+  Mob m;
+  if (!valid || tail) {
+    double x = c;
+    if (valid) {
+      const FBranch B = load_branch(U.br + br);
+      for (uint32_t j = 0; j < B.ccnt; ++j) x += U.dcon[U.child[B.cbeg + j]];
+    }
+    m.a = 0.0; m.b = x; m.c = 0.0; m.d = 1.0;                     // constant map: the chain ends here
+  } else if (lane == n - 1) {
+    m.a = 0.0; m.b = c + csig * cx / (cx + csig); m.c = 0.0; m.d = 1.0;   // the branch continues in the chunk swept before
+  } else {
+    m.a = c + snext; m.b = c * snext; m.c = 1.0; m.d = snext;
+  }
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    Mob r;
+    r.a = __shfl_down_sync(kFull, m.a, d); r.b = __shfl_down_sync(kFull, m.b, d);
+    r.c = __shfl_down_sync(kFull, m.c, d); r.d = __shfl_down_sync(kFull, m.d, d);
+    if (lane + d < 32) {
+      Mob p;
+      p.a = fma(m.a, r.a, m.b * r.c); p.b = fma(m.a, r.b, m.b * r.d);
+      p.c = fma(m.c, r.a, m.d * r.c); p.d = fma(m.c, r.b, m.d * r.d);
+      m = p;
+      mob_normalise(m);
+    }
+  }
+  const double x = m.b / m.d;
+  const double dk = x + sg;
+  const double invd = 1.0 / dk;
+  if (on) {
+    fout[s] = -sg * invd;
+    invdout[s] = invd;
+    if (head) U.dcon[br] = sg * x * invd;
+  }
+  cx = __shfl_sync(kFull, x, 0);
+  csig = __shfl_sync(kFull, sg, 0);
+}
+
+template <bool kSel>
+__device__ __forceinline__ void eliminate_forest(const FView& U, const CellS* cs, double dt, double* fout, double* invdout) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int lvl = (int)U.n_level - 1; lvl >= 0; --lvl) {
+    const FRun R = U.runs[lvl * kW + warp];
+    double cx = 1.0, csig = 0.0;
+    const unsigned long long want = kSel ? U.masks[1] : ~0ull;
+    for (uint32_t ci = R.chunk_end; ci-- > R.chunk_beg;) {
+      if (kSel && !(U.chunk_cells[ci] & want)) continue;     // no cell of this chunk takes a step of its own length
+      eliminate_chunk<kSel>(U, cs, dt, load_chunk(U.chunks + ci), lane, fout, invdout, cx, csig);
+    }
+    level_sync((U.flags & UNIT_WARP_CELLS) != 0);
+  }
+  __syncthreads();
 }
 
 // ------------------------------------------------------------------------------------------
@@ -153,23 +209,26 @@ __device__ __forceinline__ void eliminate_forest(const FView& U, const CellS* cs
 // cf, cr: f and r of the slot that follows the chunk (the previous chunk of the run), for a branch that
 // continues there.
 // ------------------------------------------------------------------------------------------
-template <bool kGen>
-__device__ __forceinline__ void backward_chunk(const FView& U, const CellS& cs, const FChunk& ck, int lane, double& cf, double& cr) {
+// lookup (warp-uniform): some cell of the chunk is not on a plain step: each lane asks for its cell's mode
+// (0 inactive: left alone; 2: a step of its own length, factors from the forest's scratch record).
+__device__ __forceinline__ void backward_chunk(const FView& U, const CellS& cs, const FChunk& ck, double f, double invd, int lane,
+                                               bool lookup, double& cf, double& cr) {
   const int n = (int)(ck.br_n & 63u);
   const bool valid = lane < n;
   const uint32_t s = ck.slot0 + lane;
   const bool head = (ck.heads >> lane) & 1u, tail = (ck.tails >> lane) & 1u;
   const uint32_t br = branch_of(ck, lane);
   uint32_t md = 1u;
-  double r = 0.0, f = 0.0, invd = 0.0;
+  double r = 0.0;
   if (valid) {
-    if (kGen) md = cs.mode[U.br_cell[br]];
+    if (lookup) {
+      md = cs.mode[U.br_cell[br]];
+      if (md == 2u) { f = U.fgen[s]; invd = U.invdgen[s]; }
+    }
     r = U.V[s];
-    if (kGen && md == 2u) { f = U.fgen[s]; invd = U.invdgen[s]; }
-    else { f = __ldg(U.f + s); invd = __ldg(U.invd + s); }
     if (tail) {
       const FBranch B = load_branch(U.br + br);
-      for (uint32_t j = 0; j < B.ccnt; ++j) r -= U.con[__ldg(U.child + B.cbeg + j)];
+      for (uint32_t j = 0; j < B.ccnt; ++j) r -= U.con[U.child[B.cbeg + j]];
     }
   }
   const double fnext = __shfl_down_sync(kFull, f, 1);
@@ -178,11 +237,14 @@ __device__ __forceinline__ void backward_chunk(const FView& U, const CellS& cs, 
     if (lane == n - 1) r = fma(-cf, cr, r);    // the branch continues in the chunk swept before this one
     else a = -fnext;
   }
+  // (a lane whose partner lies beyond the warp receives its own values; its multiplier is already 0 there,
+  // because the window it has folded holds the chunk's last lane, whose multiplier is 0)
 #pragma unroll
   for (int d = 1; d < 32; d <<= 1) {
     const double a2 = __shfl_down_sync(kFull, a, d);
     const double r2 = __shfl_down_sync(kFull, r, d);
-    if (lane + d < 32) { r = fma(a, r2, r); a *= a2; }
+    r = fma(a, r2, r);
+    a *= a2;
   }
   if (valid && md) {
     U.V[s] = r * invd;
@@ -194,8 +256,7 @@ __device__ __forceinline__ void backward_chunk(const FView& U, const CellS& cs, 
 
 // Forward (root -> leaves) substitution of one chunk: V'_k = r_k/d_k - f_k V'_{k-1}; V <- V'.
 // cv: V' of the slot before the chunk (the chunk of the run swept before this one).
-template <bool kGen>
-__device__ __forceinline__ void forward_chunk(const FView& U, const CellS& cs, const FChunk& ck, int lane, double& cv) {
+__device__ __forceinline__ void forward_chunk(const FView& U, const CellS& cs, const FChunk& ck, double f, int lane, bool lookup, double& cv) {
   const int n = (int)(ck.br_n & 63u);
   const bool valid = lane < n;
   const uint32_t s = ck.slot0 + lane;
@@ -204,11 +265,13 @@ __device__ __forceinline__ void forward_chunk(const FView& U, const CellS& cs, c
   uint32_t md = 1u;
   double a = 0.0, b = 0.0;
   if (valid) {
-    if (kGen) md = cs.mode[U.br_cell[br]];
+    if (lookup) {
+      md = cs.mode[U.br_cell[br]];
+      if (md == 2u) f = U.fgen[s];
+    }
     const double q = U.V[s];
-    const double f = (kGen && md == 2u) ? U.fgen[s] : __ldg(U.f + s);
     if (head) {
-      const uint32_t ps = __ldg(&U.br[br].pslot);
+      const uint32_t ps = U.br[br].pslot;
       b = ps != kNoSlot ? fma(-f, U.V[ps], q) : q;
     } else if (lane == 0) {
       b = fma(-f, cv, q);
@@ -217,32 +280,44 @@ __device__ __forceinline__ void forward_chunk(const FView& U, const CellS& cs, c
     }
   }
 #pragma unroll
-  for (int d = 1; d < 32; d <<= 1) {
+  for (int d = 1; d < 32; d <<= 1) {            // (lanes below d receive their own values; their multiplier is 0 by then)
     const double a2 = __shfl_up_sync(kFull, a, d);
     const double b2 = __shfl_up_sync(kFull, b, d);
-    if (lane >= d) { b = fma(a, b2, b); a *= a2; }
+    b = fma(a, b2, b);
+    a *= a2;
   }
   if (valid && md) U.V[s] = b;
   cv = __shfl_sync(kFull, b, n - 1);
 }
 
+// HH gate update x <- x_inf(V') + (x - x_inf) exp(-delta (alpha + beta)) (reading R5).  Not inlined:
+// the exp / expm1 / divide chains are ~1,000 instructions and the kernel has two call sites.
+struct Gates { double m, h, n; };
+__device__ __noinline__ Gates hh_gates(double v, double delta, double m, double h, double n) {
+  const Rates r = hh_rates(v);
+  Gates g;
+  double inf = r.am / (r.am + r.bm);
+  g.m = inf + (m - inf) * exp(-delta * (r.am + r.bm));
+  inf = r.ah / (r.ah + r.bh);
+  g.h = inf + (h - inf) * exp(-delta * (r.ah + r.bh));
+  inf = r.an / (r.an + r.bn);
+  g.n = inf + (n - inf) * exp(-delta * (r.an + r.bn));
+  return g;
+}
+
 // ------------------------------------------------------------------------------------------
 // One (sub-)step of every active cell of the forest, phases B..F (phase A, event delivery and the choice
-// of the sub-step, is in run_forest).  kGen: cells may be inactive (mode 0) or on an event-split
-// sub-step of their own length (mode 2).
+// of the sub-step, is in run_forest).  kGen (a run-time flag: one copy of the code keeps the kernel inside
+// the instruction cache): cells may be inactive (mode 0) or on an event-split sub-step of their own length
+// (mode 2).
 // ------------------------------------------------------------------------------------------
-template <bool kGen>
-__device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U, const CellS& cs, double dt) {
+__device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U, const CellS& cs, double dt, const bool kGen) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const bool multi = U.n_cell > 1;
   const uint32_t n_hh = U.n_hh, n_syn = U.n_syn, n_cl = U.n_clamp;
 
   // event-split sub-steps: those cells' matrices are eliminated for their own step length (reading R9)
-  if (kGen) {
-    bool split = false;
-    if ((uint32_t)tid < U.n_cell) split = cs.mode[tid] == 2u;
-    if (__syncthreads_or(split)) eliminate_forest(U, &cs, dt, U.fgen, U.invdgen);
-  }
+  if (kGen && U.masks[1] != 0ull) eliminate_forest<true>(U, &cs, dt, U.fgen, U.invdgen);
 
   // ---- B: currents of HH, synapses and clamps from V(t); the passive current is
   // folded into a, b.  Items on one CV form a run; the first item of a run sums it in index order.
@@ -287,7 +362,9 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
 #pragma unroll 4
     for (uint32_t s = tid; s < n; s += kT) U.V[s] = fma(__ldg(U.a + s), U.V[s], __ldg(U.b + s));
   } else {
+    const unsigned long long actc = U.masks[0];
     for (uint32_t ci = warp; ci < U.n_chunk; ci += kW) {
+      if (!(U.chunk_cells[ci] & actc)) continue;
       const FChunk ck = load_chunk(U.chunks + ci);
       if (lane >= (int)(ck.br_n & 63u)) continue;
       const uint32_t c = U.br_cell[branch_of(ck, lane)], md = cs.mode[c];
@@ -328,31 +405,71 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
   if (disjoint && (n_hh | n_syn | n_cl)) __syncthreads();
 
   // ---- D: backward sweep, deepest level first; E: forward substitution, root first; V <- V'
+  // The chunk after the one being swept is fetched first (its record from shared memory, its factors from
+  // L2), so that only the scan itself is exposed.  On general passes chunks none of whose cells take part
+  // are skipped (a branch that spans two chunks belongs to one cell: both are swept or neither).
+  const unsigned long long act = kGen ? U.masks[0] : ~0ull;
+  const unsigned long long odd = kGen ? ~(U.masks[0] & ~U.masks[1]) : 0ull;     // cells that are not on a plain step
+  const bool warp_cells = (U.flags & UNIT_WARP_CELLS) != 0;
+  constexpr uint32_t kNone = 0xFFFFFFFFu;
   for (int lvl = (int)U.n_level - 1; lvl >= 0; --lvl) {
     const FRun R = U.runs[lvl * kW + warp];
-    double cf = 0.0, cr = 0.0;
-    for (uint32_t ci = R.chunk_end; ci-- > R.chunk_beg;) backward_chunk<kGen>(U, cs, load_chunk(U.chunks + ci), lane, cf, cr);
-    __syncthreads();
+    auto next = [&](uint32_t ci) -> uint32_t {
+      while (ci > R.chunk_beg) { --ci; if (!kGen || (U.chunk_cells[ci] & act)) return ci; }
+      return kNone;
+    };
+    auto fetch = [&](uint32_t ci, FChunk& k, double& f, double& invd) {
+      k = load_chunk(U.chunks + ci);
+      f = 0.0; invd = 0.0;
+      if (lane < (int)(k.br_n & 63u)) { f = __ldg(U.f + k.slot0 + lane); invd = __ldg(U.invd + k.slot0 + lane); }
+    };
+    double cf = 0.0, cr = 0.0, f = 0.0, invd = 0.0;
+    FChunk ck;
+    uint32_t cur = next(R.chunk_end);
+    if (cur != kNone) fetch(cur, ck, f, invd);
+    while (cur != kNone) {
+      const uint32_t nx = next(cur);
+      FChunk nck = ck;
+      double nf = 0.0, ni = 0.0;
+      if (nx != kNone) fetch(nx, nck, nf, ni);
+      backward_chunk(U, cs, ck, f, invd, lane, kGen && (U.chunk_cells[cur] & odd) != 0ull, cf, cr);
+      cur = nx; ck = nck; f = nf; invd = ni;
+    }
+    level_sync(warp_cells);
   }
   for (uint32_t lvl = 0; lvl < U.n_level; ++lvl) {
     const FRun R = U.runs[lvl * kW + warp];
-    double cv = 0.0;
-    for (uint32_t ci = R.chunk_beg; ci < R.chunk_end; ++ci) forward_chunk<kGen>(U, cs, load_chunk(U.chunks + ci), lane, cv);
-    __syncthreads();
+    auto next = [&](uint32_t ci) -> uint32_t {          // first chunk at or after ci that is swept
+      for (; ci < R.chunk_end; ++ci) if (!kGen || (U.chunk_cells[ci] & act)) return ci;
+      return kNone;
+    };
+    auto fetch = [&](uint32_t ci, FChunk& k, double& f) {
+      k = load_chunk(U.chunks + ci);
+      f = lane < (int)(k.br_n & 63u) ? __ldg(U.f + k.slot0 + lane) : 0.0;
+    };
+    double cv = 0.0, f = 0.0;
+    FChunk ck;
+    uint32_t cur = next(R.chunk_beg);
+    if (cur != kNone) fetch(cur, ck, f);
+    while (cur != kNone) {
+      const uint32_t nx = next(cur + 1);
+      FChunk nck = ck;
+      double nf = 0.0;
+      if (nx != kNone) fetch(nx, nck, nf);
+      forward_chunk(U, cs, ck, f, lane, kGen && (U.chunk_cells[cur] & odd) != 0ull, cv);
+      cur = nx; ck = nck; f = nf;
+    }
+    level_sync(warp_cells);
   }
+  if (warp_cells) __syncthreads();
 
   // ---- F: state update with V', threshold test
   for (uint32_t i = tid; i < n_hh; i += kT) {
     const uint32_t c = (kGen && multi) ? U.hh_cell[i] : 0;
     if (kGen && !cs.mode[c]) continue;
     const double delta = kGen ? cs.delta[c] : dt;
-    const Rates r = hh_rates(U.V[__ldg(U.hh_slot + i)]);
-    double inf = r.am / (r.am + r.bm);
-    U.m[i] = inf + (U.m[i] - inf) * exp(-delta * (r.am + r.bm));
-    inf = r.ah / (r.ah + r.bh);
-    U.h[i] = inf + (U.h[i] - inf) * exp(-delta * (r.ah + r.bh));
-    inf = r.an / (r.an + r.bn);
-    U.n[i] = inf + (U.n[i] - inf) * exp(-delta * (r.an + r.bn));
+    const Gates g = hh_gates(U.V[__ldg(U.hh_slot + i)], delta, U.m[i], U.h[i], U.n[i]);
+    U.m[i] = g.m; U.h[i] = g.h; U.n[i] = g.n;
   }
   for (uint32_t i = tid; i < n_syn; i += kT) {
     const uint32_t c = (kGen && multi) ? U.syn_cell[i] : 0;
@@ -385,6 +502,7 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ void run_forest(const DevModel& M, const StepArgs& A, const FView& U, const CellS& cs,
                                            unsigned& n_sub, unsigned& n_del) {
+  uint32_t* sMaskW = (uint32_t*)U.masks;     // the two 64-bit masks as four words (little endian)
   const int tid = threadIdx.x;
   const uint32_t n_cell = U.n_cell;
   if ((uint32_t)tid < n_cell) {
@@ -400,9 +518,9 @@ __device__ __forceinline__ void run_forest(const DevModel& M, const StepArgs& A,
     __syncthreads();
     for (;;) {
       bool active = false, plain = true;
+      uint32_t md = 0;
       if ((uint32_t)tid < n_cell) {
         const double t = cs.tcur[tid];
-        uint32_t md = 0;
         if (t < tb) {
           double tn = U.rt[kRtDoubles * tid];
           if (tn <= t) {
@@ -424,12 +542,14 @@ __device__ __forceinline__ void run_forest(const DevModel& M, const StepArgs& A,
         cs.mode[tid] = md;
         plain = md == 1u;
       }
-      // one barrier decides both questions: bit 0 = some cell is active, bit 1 = some cell is not on a plain step
+      if (tid < (int)kForestMaxCells) {       // warps 0 and 1: which cells take part, which take a step of their own length
+        const unsigned on = __ballot_sync(kFull, md != 0u), own = __ballot_sync(kFull, md == 2u);
+        if ((tid & 31) == 0) { sMaskW[tid >> 5] = on; sMaskW[2 + (tid >> 5)] = own; }
+      }
       const int any_active = __syncthreads_or(active);
       if (!any_active) break;
       const int general = __syncthreads_or(!plain);
-      if (general) forest_substep<true>(M, U, cs, A.dt);
-      else forest_substep<false>(M, U, cs, A.dt);
+      forest_substep(M, U, cs, A.dt, general != 0);
     }
   }
   if ((uint32_t)tid < n_cell) {
@@ -445,28 +565,35 @@ __device__ __forceinline__ void run_forest(const DevModel& M, const StepArgs& A,
 __global__ void __launch_bounds__(kForestThreads, 8) cable_forest_kernel(DevModel M, StepArgs A, int cls) {
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ UnitHeader H;
-  const ForestSmemPlan P = M.fcls[cls].plan;
+  __shared__ __align__(8) uint64_t mbar_mem;
+  __shared__ unsigned long long sMask[2];
   const UnitDesc d = M.units[M.fcls[cls].first + blockIdx.x];
   uint8_t* fast = M.fast + d.fast_off;
   double* Ss = (double*)smem;
-  uint64_t* mbar = (uint64_t*)(smem + P.off_mbar);
+  uint64_t* mbar = &mbar_mem;
   const int tid = threadIdx.x;
   if (tid == 0) {
     mbar_init(mbar, 1);
     fence_mbar_init();
     fence_proxy_async();
-    mbar_expect_tx(mbar, d.state_bytes);
+    mbar_expect_tx(mbar, d.state_bytes + d.topo_bytes);
     bulk_g2s(Ss, M.state + d.state_base, d.state_bytes, mbar);
+    bulk_g2s(smem + align_up(d.state_bytes, 128), M.topo + 16ull * d.topo_off16, d.topo_bytes, mbar);   // the tree record
     bulk_prefetch_l2(fast, d.fast_bytes);            // coefficients and instance tables -> L2
   }
   if (tid < (int)(sizeof(UnitHeader) / 4)) ((uint32_t*)&H)[tid] = __ldg((const uint32_t*)fast + tid);
   __syncthreads();
+  // every forest lays its own shared memory out; the launch reserves what the largest of its class needs
+  ForestCaps fc;
+  fc.state_bytes = d.state_bytes; fc.topo_bytes = d.topo_bytes; fc.n_branch = H.n_lane; fc.n_spec = H.n_hh + H.n_syn + H.n_clamp; fc.n_cell = H.n_cell;
+  const ForestSmemPlan P = forest_smem_plan(fc);
+  mbar_wait(mbar, 0);                        // state and tree records are in shared memory
   FView U;
-  make_fview(U, M, H, fast, Ss);
+  make_fview(U, M, H, fast, Ss, smem + P.off_topo);
+  U.masks = sMask;
   U.con = (double*)(smem + P.off_con);
   U.xI = (double*)(smem + P.off_xi);
   const CellS cs = carve_cells(smem + P.off_cell, U.n_cell);
-  mbar_wait(mbar, 0);
   unsigned n_sub = 0, n_del = 0;
   run_forest(M, A, U, cs, n_sub, n_del);
   // ---- state record -> HBM (one bulk store)
@@ -494,8 +621,8 @@ __global__ void __launch_bounds__(kForestThreads) forest_factor_kernel(DevModel 
   if (threadIdx.x < sizeof(UnitHeader) / 4) ((uint32_t*)&H)[threadIdx.x] = ((const uint32_t*)fast)[threadIdx.x];
   __syncthreads();
   FView U;
-  make_fview(U, M, H, fast, M.state + d.state_base);
-  eliminate_forest(U, nullptr, dt, const_cast<double*>(U.f), const_cast<double*>(U.invd));
+  make_fview(U, M, H, fast, M.state + d.state_base, M.topo + H.topo_off);
+  eliminate_forest<false>(U, nullptr, dt, const_cast<double*>(U.f), const_cast<double*>(U.invd));
   double* a = const_cast<double*>(U.a);
   double* b = const_cast<double*>(U.b);
   for (uint32_t s = threadIdx.x; s < U.n_slot; s += kT) {
@@ -516,7 +643,7 @@ __global__ void __launch_bounds__(kForestThreads) forest_init_kernel(DevModel M)
   if (threadIdx.x < sizeof(UnitHeader) / 4) ((uint32_t*)&H)[threadIdx.x] = ((const uint32_t*)fast)[threadIdx.x];
   __syncthreads();
   FView U;
-  make_fview(U, M, H, fast, M.state + d.state_base);
+  make_fview(U, M, H, fast, M.state + d.state_base, M.topo + H.topo_off);
   for (uint32_t i = threadIdx.x; i < U.n_hh; i += kT) {
     const Rates r = hh_rates(U.V[U.hh_slot[i]]);
     U.m[i] = r.am / (r.am + r.bm);

@@ -14,8 +14,10 @@
 //   branch   a maximal unbranched chain of control volumes; its slots are consecutive, proximal first
 //   level    branches at the same distance (in branches) from their cell's root; levels of all cells of
 //            the forest are aligned, __syncthreads separates levels
-//   run      the branches of one level that one warp of the CTA sweeps (whole branches, dealt longest
-//            first to the least loaded warp); its slots are consecutive
+//   run      the branches of one level that one warp of the CTA sweeps; its slots are consecutive.  A forest of
+//            few cells deals the branches of a level to the warps (whole branches, longest first to the least
+//            loaded warp); a forest of many cells deals whole CELLS to the warps (UNIT_WARP_CELLS), so that a
+//            warp never waits for another between levels
 //   chunk    32 consecutive slots of a run = one warp-wide segmented scan; a branch longer than a chunk
 //            carries its recurrence from one chunk of the run to the next in a register
 // Slot order: level (root first) -> warp -> branch -> control volume, so the forward sweep walks
@@ -38,7 +40,10 @@ constexpr uint32_t kForestMaxBranchLen = 32768;      // longer chains are cut (l
 constexpr int kForestClasses = 4;                    // launches by shared-memory need: 8, 4, 2, 1 CTAs per SM
 
 enum : uint32_t { UNIT_FOREST = 2u,                  // UnitHeader.flags
-                  UNIT_POINT_DISJOINT = 4u };        // no two kinds of point mechanism share a control volume
+                  UNIT_POINT_DISJOINT = 4u,          // no two kinds of point mechanism share a control volume
+                  UNIT_WARP_CELLS = 8u };            // every cell of the forest is swept by ONE warp (all its branches are
+                                                     // in that warp's runs): levels need __syncwarp only
+constexpr uint32_t kForestWarpCellsMin = 6;          // cells a forest needs before its cells are dealt to warps whole
 
 struct FRun { uint32_t chunk_beg, chunk_end; };      // chunks [beg, end) of (level, warp); backward runs them end -> beg
 
@@ -58,13 +63,26 @@ struct FBranch {         // 16 bytes, in slot order
 };
 
 // Byte offsets inside a forest's tree record (every section 16-byte aligned).
-struct FTopoOff { uint32_t runs, chunks, branches, br_cell, child, cell_det, level_br, total; };
+struct FTopoOff { uint32_t offs, runs, chunks, chunk_cells, branches, br_cell, child, cell_det, level_br, total; };
+// The record starts with a table of the offsets a CTA needs (FOffs), filled by the host, so that the kernel reads
+// them from shared memory instead of recomputing three dozen aligned sums per thread.
+struct FOffs {
+  uint32_t fast[18];     // bytes into the fast record, in the order of FastOff (f ... cl_cell)
+  uint32_t state[6];     // doubles into the state record: v, m, h, n, g, rt
+  uint32_t gen[6];       // doubles into the gen record: C, S, sig, G, b, syn_tau
+  uint32_t topo[8];      // bytes into this record: runs, chunks, chunk_cells, branches, br_cell, child, cell_det, level_br
+  uint32_t scratch[3];   // doubles into the scratch record: fgen, invdgen, dcon
+  uint32_t pad[23];
+};
+static_assert(sizeof(FOffs) == 256, "FOffs must be 256 bytes");
 ARBB_HD FTopoOff ftopo_offsets(uint32_t n_level, uint32_t n_chunk, uint32_t n_branch, uint32_t n_child, uint32_t n_cell) {
   FTopoOff o;
   uint32_t p = 0;
   auto sec = [&](uint32_t bytes) { uint32_t at = p; p = align_up(p + bytes, 16); return at; };
+  o.offs = sec((uint32_t)sizeof(FOffs));
   o.runs = sec(n_level * (uint32_t)kForestWarps * (uint32_t)sizeof(FRun));
   o.chunks = sec(n_chunk * (uint32_t)sizeof(FChunk));
+  o.chunk_cells = sec(n_chunk * 8);                  // uint64: bit c = the chunk holds control volumes of cell c
   o.branches = sec(n_branch * (uint32_t)sizeof(FBranch));
   o.br_cell = sec(n_branch * 2);                     // uint16: forest-local cell of every branch
   o.child = sec(n_child * 4);                        // uint32: child branches
@@ -74,20 +92,25 @@ ARBB_HD FTopoOff ftopo_offsets(uint32_t n_level, uint32_t n_chunk, uint32_t n_br
   return o;
 }
 
-// Shared memory of one CTA of the forest kernel: the state record (V | m | h | n | g | runtime), the
-// contributions of the branches to their parents, the point currents, per-cell scratch, one mbarrier.
-// Caps are maxima over the forests of one launch class.
-struct ForestCaps { uint32_t state_bytes, n_branch, n_spec, n_cell; };
-struct ForestSmemPlan { uint32_t off_con, off_xi, off_cell, off_mbar, bytes; };
+// Shared memory of one CTA of the forest kernel: the state record (V | m | h | n | g | runtime), the tree
+// record, the contributions of the branches to their parents, the point currents, per-cell scratch.
+// Every CTA lays out its own forest; a launch reserves what the largest forest of its class needs.
+struct ForestCaps { uint32_t state_bytes, topo_bytes, n_branch, n_spec, n_cell; };
+struct ForestSmemPlan { uint32_t off_topo, off_con, off_xi, off_cell, bytes; };
 ARBB_HD ForestSmemPlan forest_smem_plan(const ForestCaps& c) {
   ForestSmemPlan P;
   uint32_t p = align_up(c.state_bytes, 128);
+  P.off_topo = p; p = align_up(p + c.topo_bytes, 16);
   P.off_con = p;  p = align_up(p + 8 * c.n_branch, 16);
   P.off_xi = p;   p = align_up(p + 8 * c.n_spec, 16);
   P.off_cell = p; p = align_up(p + kCellScratchBytes * (c.n_cell ? c.n_cell : 1u), 16);
-  P.off_mbar = p; p += 16;
   P.bytes = align_up(p, 128);
   return P;
+}
+// upper bound of a tree record's size from counts known before the forest is built
+ARBB_HD uint32_t ftopo_bound(uint32_t n_cv, uint32_t n_branch, uint32_t n_cell) {
+  const uint32_t n_level = n_branch, n_chunk = n_cv / 32 + (uint32_t)kForestWarps * n_level + 1;
+  return ftopo_offsets(n_level, n_chunk, n_branch, n_branch, n_cell).total;
 }
 // shared-memory budget of launch class k (bytes per CTA so that 8 >> k CTAs share an SM's 227 KB)
 // (1 KB per CTA is reserved by the system; the kernel's static shared memory is below 1 KB)

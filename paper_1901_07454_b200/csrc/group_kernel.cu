@@ -338,7 +338,7 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
   const int rtid = kT - 1 - tid, rc = rtid % kG;      // reversed dealing of instances; cell of those
   const uint32_t nE_cv = gcv_elems(U.n_cv), nE_hh = U.n_hh * kG, nE_syn = U.n_syn * kG, nE_cl = U.n_cl * kG;
   const uint32_t md = kGen ? cs.mode[c] : 1u, rmd = kGen ? cs.mode[rc] : 1u;
-  const double delta = kGen ? cs.delta[c] : dt, rdelta = kGen ? cs.delta[rc] : dt;
+  const double rdelta = kGen ? cs.delta[rc] : dt;
   // ---- B: currents of HH, synapses and clamps from V(t); the passive current is
   // folded into a, b.  Items of one cell on one CV form a run; its first item sums it in index order.
   double* xI = buf;

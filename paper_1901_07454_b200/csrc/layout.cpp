@@ -147,10 +147,11 @@ struct UnitBuilder {
   std::vector<uint32_t> level_begin;
   bool bad = false;                        // a count does not fit its field
   // forests (forest_layout.h)
-  bool forest = false;
+  bool forest = false, warp_cells = false;
   std::vector<uint32_t> fslot0, flevel_br;
   std::vector<FRun> fruns;
   std::vector<FChunk> fchunks;
+  std::vector<uint64_t> fchunk_cells;
 
   bool has_hh(int64_t gi) const {
     return d.hh_gnabar && (d.hh_gnabar[gi] != 0.0 || d.hh_gkbar[gi] != 0.0 || d.hh_gl[gi] != 0.0);
@@ -255,7 +256,24 @@ struct UnitBuilder {
     for (const Lane& L : lanes) n_level = std::max(n_level, L.level + 1);
     std::vector<std::vector<uint32_t>> by_level(n_level);
     for (uint32_t i = 0; i < n_lane; ++i) by_level[lanes[i].level].push_back(i);
-    order.clear(); fslot0.clear(); flevel_br.clear(); fchunks.clear();
+    order.clear(); fslot0.clear(); flevel_br.clear(); fchunks.clear(); fchunk_cells.clear();
+    // many cells: whole cells are dealt to the warps (largest first to the least loaded warp)
+    warp_cells = cells.size() >= kForestWarpCellsMin;
+    std::vector<uint32_t> cell_warp(cells.size(), 0);
+    if (warp_cells) {
+      std::vector<uint64_t> ccv(cells.size(), 0);
+      for (const Lane& L : lanes) ccv[L.lc] += L.len;
+      std::vector<uint32_t> by_size(cells.size());
+      for (uint32_t c = 0; c < cells.size(); ++c) by_size[c] = c;
+      std::stable_sort(by_size.begin(), by_size.end(), [&](uint32_t x, uint32_t y) { return ccv[x] > ccv[y]; });
+      uint64_t wl[kForestWarps] = {0};
+      for (uint32_t c : by_size) {
+        int best = 0;
+        for (int w = 1; w < kForestWarps; ++w) if (wl[w] < wl[best]) best = w;
+        cell_warp[c] = (uint32_t)best;
+        wl[best] += ccv[c];
+      }
+    }
     fruns.assign((size_t)n_level * kForestWarps, FRun{0, 0});
     uint32_t slot = 0;
     for (uint32_t lvl = 0; lvl < n_level; ++lvl) {
@@ -264,13 +282,16 @@ struct UnitBuilder {
       std::stable_sort(v.begin(), v.end(), [&](uint32_t x, uint32_t y) { return lanes[x].len > lanes[y].len; });
       std::vector<uint32_t> dealt[kForestWarps];
       uint64_t load[kForestWarps] = {0};
-      for (uint32_t i : v) {               // longest first onto the least loaded warp
+      for (uint32_t i : v) {               // longest first onto the least loaded warp - or to the warp that owns the cell
         int best = 0;
-        for (int w = 1; w < kForestWarps; ++w) if (load[w] < load[best]) best = w;
+        if (warp_cells) best = (int)cell_warp[lanes[i].lc];
+        else for (int w = 1; w < kForestWarps; ++w) if (load[w] < load[best]) best = w;
         dealt[best].push_back(i);
         load[best] += lanes[i].len;
       }
       for (int w = 0; w < kForestWarps; ++w) {
+        // branches of one cell next to each other: a pass in which few cells are active skips whole chunks
+        std::stable_sort(dealt[w].begin(), dealt[w].end(), [&](uint32_t x, uint32_t y) { return lanes[x].lc < lanes[y].lc; });
         FRun& R = fruns[(size_t)lvl * kForestWarps + w];
         R.chunk_beg = (uint32_t)fchunks.size();
         const uint32_t pos0 = (uint32_t)order.size(), slot_beg = slot;
@@ -282,14 +303,17 @@ struct UnitBuilder {
           while (fslot0[pos] + lanes[order[pos]].len <= c0) ++pos;
           ck.slot0 = c0; ck.heads = 0; ck.tails = 0; ck.br_n = pos * 64u + n;
           uint32_t q = pos;
+          uint64_t cellmask = 0;
           for (uint32_t l = 0; l < 32; ++l) {
             if (l >= n) { ck.heads |= 1u << l; ck.tails |= 1u << l; continue; }
             const uint32_t sl = c0 + l;
             while (fslot0[q] + lanes[order[q]].len <= sl) ++q;
+            cellmask |= 1ull << lanes[order[q]].lc;
             if (sl == fslot0[q]) ck.heads |= 1u << l;
             if (sl == fslot0[q] + lanes[order[q]].len - 1) ck.tails |= 1u << l;
           }
           fchunks.push_back(ck);
+          fchunk_cells.push_back(cellmask);
         }
         R.chunk_end = (uint32_t)fchunks.size();
       }
@@ -354,14 +378,33 @@ struct UnitBuilder {
         for (int64_t q = clamp_off[orig]; q < clamp_off[orig + 1]; ++q) kind[d.clamp_cv[clamp_idx[q]]] |= 4;
         for (uint8_t k : kind) if (k & (k - 1)) disjoint = false;
       }
-      uc.flags |= UNIT_FOREST | (disjoint ? UNIT_POINT_DISJOINT : 0u);
+      uc.flags |= UNIT_FOREST | (disjoint ? UNIT_POINT_DISJOINT : 0u) | (warp_cells ? UNIT_WARP_CELLS : 0u);
     }
     if (topo_out && forest) {
       const FTopoOff to = ftopo_offsets(uc.n_level, uc.n_task, n_lane, n_child, n_cell);
       topo_out->assign(to.total, 0);
       uint8_t* tp = topo_out->data();
+      {
+        FOffs fo2;
+        std::memset(&fo2, 0, sizeof fo2);
+        const uint32_t fv[18] = {fo.f, fo.invd, fo.a, fo.b, fo.hh_gna, fo.hh_gk, fo.hh_gl, fo.syn_e, fo.syn_decay, fo.cl_t0, fo.cl_t1,
+                                 fo.cl_amp, fo.hh_slot, fo.syn_slot, fo.cl_slot, fo.hh_cell, fo.syn_cell, fo.cl_cell};
+        std::memcpy(fo2.fast, fv, sizeof fv);
+        const uint32_t sv[6] = {so.v, so.m, so.h, so.n, so.g, so.rt};
+        std::memcpy(fo2.state, sv, sizeof sv);
+        const GenOff go2 = gen_offsets(uc.n_slot, n_syn);
+        const uint32_t gv[6] = {go2.C, go2.S, go2.sig, go2.G, go2.b, go2.syn_tau};
+        std::memcpy(fo2.gen, gv, sizeof gv);
+        const uint32_t tv[8] = {to.runs, to.chunks, to.chunk_cells, to.branches, to.br_cell, to.child, to.cell_det, to.level_br};
+        std::memcpy(fo2.topo, tv, sizeof tv);
+        const FScratchOff sc2 = fscratch_offsets(uc.n_slot, n_lane);
+        const uint32_t cv2[3] = {sc2.fgen, sc2.invdgen, sc2.dcon};
+        std::memcpy(fo2.scratch, cv2, sizeof cv2);
+        std::memcpy(tp + to.offs, &fo2, sizeof fo2);
+      }
       std::memcpy(tp + to.runs, fruns.data(), fruns.size() * sizeof(FRun));
       std::memcpy(tp + to.chunks, fchunks.data(), fchunks.size() * sizeof(FChunk));
+      std::memcpy(tp + to.chunk_cells, fchunk_cells.data(), fchunk_cells.size() * 8);
       std::memcpy(tp + to.level_br, flevel_br.data(), flevel_br.size() * 4);
       FBranch* brec = (FBranch*)(tp + to.branches);
       uint16_t* br_cell = (uint16_t*)(tp + to.br_cell);
@@ -742,6 +785,7 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     ForestCaps fc;
     fc.state_bytes = 8 * state_offsets(align_up((uint32_t)n_cv, 2), (uint32_t)n_hh, (uint32_t)n_syn, (uint32_t)n_cell).total;
     fc.n_branch = (uint32_t)n_br; fc.n_spec = (uint32_t)(n_hh + n_syn + n_clamp); fc.n_cell = (uint32_t)n_cell;
+    fc.topo_bytes = ftopo_bound((uint32_t)n_cv, (uint32_t)n_br, (uint32_t)n_cell);
     return forest_smem_plan(fc).bytes;
   };
   auto cell_counts = [&](int64_t c, uint64_t& n_cv, uint64_t& n_syn, uint64_t& n_cl) {
@@ -865,6 +909,7 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     UnitBuilder B{d, P, H, clamp_off, clamp_idx, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, false};
     B.forest = u < H.n_forests;
     H.units[u] = B.run(unit_begin[u], unit_cells[u], &topo[u], nullptr, nullptr);
+    H.units[u].topo_bytes = (uint32_t)topo[u].size();
     if (u >= H.n_forests) H.units[u].flags |= UNIT_BLOCK;
     if (H.units[u].n_level > 60000 || H.units[u].n_slot > 0x3FFFFFFFu) too_many.store(1);
     if (B.bad) too_many.store(1);
@@ -875,7 +920,7 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
   {
     auto need_of = [&](const UnitCounts& uc) {
       ForestCaps fc;
-      fc.state_bytes = uc.state_bytes; fc.n_branch = uc.n_lane; fc.n_spec = uc.n_hh + uc.n_syn + uc.n_clamp; fc.n_cell = uc.n_cell;
+      fc.state_bytes = uc.state_bytes; fc.topo_bytes = uc.topo_bytes; fc.n_branch = uc.n_lane; fc.n_spec = uc.n_hh + uc.n_syn + uc.n_clamp; fc.n_cell = uc.n_cell;
       return forest_smem_plan(fc).bytes;
     };
     auto class_of = [&](const UnitCounts& uc) {
@@ -904,18 +949,16 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     for (int64_t i = 0; i < H.n_forests; ++i) topo[i].swap(topo2[i]);
     H.units.swap(units2); unit_begin.swap(begin2); unit_cells.swap(cells2);
     for (int k = 0; k < kForestClasses; ++k) { H.fcls[k].first = 0; H.fcls[k].count = 0; }
-    ForestCaps caps[kForestClasses];
-    for (int k = 0; k < kForestClasses; ++k) caps[k] = ForestCaps{0, 0, 0, 0};
+    for (int k = 0; k < kForestClasses; ++k) H.fcls[k].plan = forest_smem_plan(ForestCaps{0, 0, 0, 0, 0});
     for (int64_t i = 0; i < H.n_forests; ++i) {
       const UnitCounts& uc = H.units[i];
       const int k = class_of(uc);
       if (H.fcls[k].count++ == 0) H.fcls[k].first = i;
-      caps[k].state_bytes = std::max(caps[k].state_bytes, uc.state_bytes);
-      caps[k].n_branch = std::max(caps[k].n_branch, uc.n_lane);
-      caps[k].n_spec = std::max(caps[k].n_spec, uc.n_hh + uc.n_syn + uc.n_clamp);
-      caps[k].n_cell = std::max(caps[k].n_cell, uc.n_cell);
+      ForestCaps fc;
+      fc.state_bytes = uc.state_bytes; fc.topo_bytes = uc.topo_bytes; fc.n_branch = uc.n_lane; fc.n_spec = uc.n_hh + uc.n_syn + uc.n_clamp; fc.n_cell = uc.n_cell;
+      const ForestSmemPlan P = forest_smem_plan(fc);
+      if (P.bytes > H.fcls[k].plan.bytes) H.fcls[k].plan = P;   // the launch reserves the largest need of the class
     }
-    for (int k = 0; k < kForestClasses; ++k) H.fcls[k].plan = forest_smem_plan(caps[k]);
   }
   // groups: row counts, then placement (groups first in every pool)
   parallel_for(H.n_groups, [&](int64_t g) {
@@ -1035,8 +1078,8 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     uint8_t* cb = H.fast.data() + D.const_off;
     double* st = H.state.data() + D.state_base;
     double* gen = H.gen.data() + D.gen_base;
-    double* f = (double*)(cb + co.f); double* invd = (double*)(cb + co.invd);
-    double* a = (double*)(cb + co.a); double* b = (double*)(cb + co.b);
+    double* invd = (double*)(cb + co.invd);
+    double* a = (double*)(cb + co.a);
     double* hh_gna = (double*)(cb + co.hh_gna); double* hh_gk = (double*)(cb + co.hh_gk); double* hh_gl = (double*)(cb + co.hh_gl);
     double* syn_e = (double*)(cb + co.syn_e);
     double* cl_t0 = (double*)(cb + co.cl_t0); double* cl_t1 = (double*)(cb + co.cl_t1); double* cl_amp = (double*)(cb + co.cl_amp);
@@ -1126,7 +1169,9 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     UnitDesc& ud = H.descs[u];
     ud.fast_off = H.units[u].fast_off; ud.state_base = H.units[u].state_base;
     ud.fast_bytes = H.units[u].fast_bytes; ud.state_bytes = H.units[u].state_bytes;
-    ud.pad[0] = ud.pad[1] = 0;
+    const bool is_forest = (H.units[u].flags & UNIT_FOREST) != 0;
+    ud.topo_off16 = is_forest ? (uint32_t)(H.units[u].topo_off / 16) : 0u;
+    ud.topo_bytes = is_forest ? H.units[u].topo_bytes : 0u;
   }
   std::vector<std::vector<uint8_t>>().swap(topo);
   parallel_for(H.n_units, [&](int64_t u) {

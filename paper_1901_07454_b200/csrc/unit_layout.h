@@ -80,7 +80,8 @@ struct UnitDesc {        // what a loader needs before the header has arrived; 3
   int64_t fast_off;      // byte offset into the fast pool (128-byte aligned)
   int64_t state_base;    // double index into the state pool (16-double aligned)
   uint32_t fast_bytes, state_bytes;   // multiples of 16
-  uint32_t pad[2];
+  uint32_t topo_off16, topo_bytes;    // forests: the tree record (byte offset / 16 into the topo pool, bytes), which
+                                      // the kernel stages in shared memory; 0 for block units
 };
 
 ARBB_HD uint32_t align_up(uint32_t x, uint32_t a) { return (x + a - 1) / a * a; }
