@@ -131,6 +131,7 @@ struct orc_model {
   double *scr;                   /* 5*n_cv scratch: I, d, u, rhs, x */
   cell_t* cells;
   double t; int64_t seq, grid_steps;
+  int linearised;                /* 0: explicit membrane currents (R1); 1: conductance-linearised step (NEXT-2) */
   int64_t* sp_cell; double* sp_time; int64_t n_sp, sp_cap;
 };
 
@@ -197,13 +198,55 @@ static void cell_currents(const orc_model* M, const cell_t* c, double t, double*
   }
 }
 
+/* SURVEY.md 8(f) NEXT-2, the conductance-linearised variant of the implicit Euler equation at PAPER.md:152-156:
+ * every membrane current of the form g_k (V - E_k) is taken at the NEW voltage,
+ *   (c_i/delta + sum_j sigma_ij + sum_k g_k) V'_i - sum_j sigma_ij V'_j = (c_i/delta) V_i + sum_k g_k E_k + I_i^inj ,
+ * with the conductances g_k from the state at time t (HH: gnabar m^3 h, gkbar n^4, gl; passive g; synapses g_s),
+ * so the matrix is assembled and eliminated afresh every step.  gsum_i = sum_k g_k [uS], src_i = sum_k g_k E_k
+ * + clamp currents [nA]. */
+static void cell_conductances(const orc_model* M, const cell_t* c, double t, double* gsum, double* src) {
+  for (int64_t i = 0; i < c->n; ++i) {
+    int64_t gi = c->cv0 + i;
+    gsum[i] = 0.0; src[i] = 0.0;
+    if (has_hh(M, gi)) {
+      double m = M->m[gi], h = M->h[gi], n = M->nn[gi], sc = M->area[gi] * 1e-2;
+      double gna = M->gna[gi] * m * m * m * h * sc, gk = M->gk[gi] * n * n * n * n * sc, gl = M->gl[gi] * sc;
+      gsum[i] += gna + gk + gl;
+      src[i] += gna * M->ena + gk * M->ek + gl * M->el;
+    }
+    if (M->pg && M->pg[gi] != 0.0) {
+      double g = M->pg[gi] * M->area[gi] * 1e-2;
+      gsum[i] += g;
+      src[i] += g * M->pe[gi];
+    }
+  }
+  for (int64_t s = 0; s < c->ns; ++s) {                      /* ascending synapse index */
+    int64_t gs = c->syn0 + s; int32_t i = M->syn_cv[gs];
+    gsum[i] += M->g[gs];
+    src[i] += M->g[gs] * M->syn_e[gs];
+  }
+  for (int64_t k = 0; k < c->n_clamps; ++k) {                /* R8: a current source, not a conductance */
+    int64_t ck = c->clamps[k];
+    if (M->cl_t0[ck] <= t && t < M->cl_t1[ck]) src[M->cl_cv[ck]] += M->cl_amp[ck];
+  }
+}
+
 /* One (sub-)step of one cell from t to t+delta: steps 2-7 of SURVEY.md 8(c). */
 static void cell_step(orc_model* M, cell_t* c, double t, double delta) {
   double* I = M->scr + 5 * c->cv0;
   double *d = I + c->n, *u = d + c->n, *rhs = u + c->n, *x = rhs + c->n;
   double* v = M->v + c->cv0;
-  cell_currents(M, c, t, I);
-  orc_assemble(c->n, M->parent + c->cv0, M->area + c->cv0, M->cm + c->cv0, M->rax + c->cv0, v, I, delta, d, u, rhs);
+  if (!M->linearised) {
+    cell_currents(M, c, t, I);
+    orc_assemble(c->n, M->parent + c->cv0, M->area + c->cv0, M->cm + c->cv0, M->rax + c->cv0, v, I, delta, d, u, rhs);
+  } else {
+    /* assemble with no current (I = 0), then the conductances go on the diagonal and their sources on the rhs;
+     * x serves as scratch for src until the solve overwrites it */
+    for (int64_t i = 0; i < c->n; ++i) I[i] = 0.0;
+    orc_assemble(c->n, M->parent + c->cv0, M->area + c->cv0, M->cm + c->cv0, M->rax + c->cv0, v, I, delta, d, u, rhs);
+    cell_conductances(M, c, t, I, x);
+    for (int64_t i = 0; i < c->n; ++i) { d[i] += I[i]; rhs[i] += x[i]; }
+  }
   orc_hines_solve(c->n, M->parent + c->cv0, d, u, rhs, x);
   c->v_prev = v[c->det];
   for (int64_t i = 0; i < c->n; ++i) v[i] = x[i];            /* V <- V' */
@@ -506,6 +549,12 @@ int orc_set_state(orc_model* M, const double* v, const double* hm, const double*
   if (hn) memcpy(M->nn, hn, (size_t)M->n_cv * 8);
   if (syn_g) memcpy(M->g, syn_g, (size_t)M->n_syn * 8);
   for (int64_t c = 0; c < M->n_cells; ++c) { M->cells[c].v_prev = M->v[M->cells[c].cv0 + M->cells[c].det]; M->cells[c].armed = 1; }
+  return 0;
+}
+
+int orc_set_linearised(orc_model* M, int on) {
+  if (!M) FAIL(-1, "null model");
+  M->linearised = on != 0;
   return 0;
 }
 

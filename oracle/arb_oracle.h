@@ -77,6 +77,10 @@ int orc_cell_currents(orc_model* m, int64_t cell, double* i_out);
  * used by the parity tests to start both implementations from one state */
 int orc_set_state(orc_model* m, const double* v, const double* hm, const double* hh,
                   const double* hn, const double* syn_g);
+/* 0 (default): explicit membrane currents, the equation at PAPER.md:154 (reading R1).  1: the conductance-
+ * linearised variant: membrane conductances on the diagonal, matrix assembled and
+ * eliminated every step. */
+int orc_set_linearised(orc_model* m, int on);
 void orc_set_threads(int n);                                  /* OpenMP threads (timing only)  */
 int orc_get_threads(void);
 void orc_destroy(orc_model* m);

@@ -69,6 +69,7 @@ def lib():
         L.orc_probe.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int64]
         L.orc_cell_currents.argtypes = [C.c_void_p, C.c_int64, C.c_void_p]
         L.orc_set_state.argtypes = [C.c_void_p] * 6
+        L.orc_set_linearised.argtypes = [C.c_void_p, C.c_int]
         L.orc_set_threads.argtypes = [C.c_int]
         L.orc_get_threads.restype = C.c_int
         L.orc_destroy.argtypes = [C.c_void_p]
@@ -176,6 +177,9 @@ class Oracle:
     def set_state(self, v=None, m=None, h=None, n=None, syn_g=None):
         arrs = [None if a is None else np.ascontiguousarray(a, np.float64) for a in (v, m, h, n, syn_g)]
         self._check(lib().orc_set_state(self._h, *[_p(a) for a in arrs]))
+
+    def set_linearised(self, on=True):
+        self._check(lib().orc_set_linearised(self._h, 1 if on else 0))
 
     def close(self):
         if self._h:

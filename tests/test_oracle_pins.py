@@ -656,3 +656,124 @@ def test_ninth_spike_in_one_grid_step_is_an_error_not_a_drop(orc):
     o = orc.Oracle(W.finalize(m2))
     o.advance(3 * dt, dt)
     assert len(o.spikes()[1]) == 8
+
+
+# ---------------------------------------------------------------------------------------------
+# L1-L4 the conductance-linearised step (PAPER.md:152-156 with the membrane
+# conductances on the diagonal).  Pinned like the explicit step: dense LU, closed forms, an ODE solver.
+# ---------------------------------------------------------------------------------------------
+def _lin(orc, m):
+    o = orc.Oracle(m)
+    o.set_linearised(True)
+    return o
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3, 4])
+def test_l1_linearised_step_vs_dense_lu(orc, seed):
+    """One step of a random model (HH, passive, synapses with per-synapse e, clamps) against a dense solve of
+    (diag(C/dt + g) + Laplacian) V' = C/dt V + sum g E + I_inj written out here."""
+    m = W.random_model(seed, n_cells=4, n_conn=0, n_ext=0, t_end=5.0)
+    rng = np.random.default_rng(seed)
+    o = _lin(orc, m)
+    g0 = rng.uniform(0.0, 0.004, m["n_syn"])
+    o.set_state(syn_g=g0)
+    v0, (hm, hh, hn) = o.voltage(), o.gates()
+    o.advance(DT, DT)
+    v1 = o.voltage()
+    for c in range(m["n_cells"]):
+        a, b = m["cv_off"][c], m["cv_off"][c + 1]
+        n = b - a
+        area = m["cv_area"][a:b]
+        A, rhs = _dense_system(m["cv_parent"][a:b], area, m["cv_cm"][a:b], m["cv_raxial"][a:b], v0[a:b], np.zeros(n), DT)
+        sc = area * 1e-2
+        gna = m["hh_gnabar"][a:b] * hm[a:b] ** 3 * hh[a:b] * sc
+        gk = m["hh_gkbar"][a:b] * hn[a:b] ** 4 * sc
+        gl = m["hh_gl"][a:b] * sc
+        gp = m["pas_g"][a:b] * sc
+        g = gna + gk + gl + gp
+        src = gna * m["hh_ena"] + gk * m["hh_ek"] + gl * m["hh_el"] + gp * m["pas_e"][a:b]
+        for s in range(m["syn_off"][c], m["syn_off"][c + 1]):
+            g[m["syn_cv"][s]] += g0[s]
+            src[m["syn_cv"][s]] += g0[s] * m["syn_e"][s]
+        for k in np.flatnonzero(m["clamp_cell"] == c):
+            if m["clamp_t0"][k] <= 0.0 < m["clamp_t1"][k]:
+                src[m["clamp_cv"][k]] += m["clamp_amp"][k]
+        ref = np.linalg.solve(A + np.diag(g), rhs + src)
+        assert np.max(np.abs(v1[a:b] - ref)) <= 1e-12 * np.max(np.abs(ref)), c
+
+
+@pytest.mark.parametrize("k", [0, 1, 3, 11])
+def test_l2_linearised_eigenmode_decay_is_fully_implicit(orc, k):
+    """Passive chain: with the leak on the diagonal every mode decays by 1 / (1 + dt (G + lam_k) / C) per step
+    (the explicit step of P4 has (1 - dt G / C) / (1 + dt lam_k / C))."""
+    n, g_pas, area, rax, cm, e = 12, 2e-4, 150.0, 3.0, 1.3, -65.0
+    i = np.arange(n)
+    mode = np.cos(np.pi * k * (i + 0.5) / n)
+    o = _lin(orc, W.passive_cable(n, g_pas=g_pas, area=area, rax=rax, cm=cm, e_pas=e, vinit=e + mode))
+    nsteps = 50
+    o.advance(nsteps * DT, DT)
+    G, C, s = g_pas * area * 1e-2, cm * area * 1e-5, 1.0 / rax
+    lam_k = 2 * s * (1 - np.cos(np.pi * k / n))
+    rho = 1.0 / (1.0 + DT * (G + lam_k) / C)
+    assert np.max(np.abs(o.voltage() - (e + rho ** nsteps * mode))) <= 2e-12
+    rho_explicit = (1 - DT * G / C) / (1 + DT * lam_k / C)
+    assert abs(rho - rho_explicit) > 1e-7                      # the two schemes differ: the pin tells them apart
+
+
+def test_l3_linearised_steady_states(orc):
+    """Steady states do not depend on the scheme: the cable of P3 and the conductance-weighted mean of P13."""
+    n, g_pas, area, rax, e, i_inj = 7, 1e-4, 100.0, 5.0, -65.0, 0.02
+    o = _lin(orc, W.passive_cable(n, g_pas=g_pas, area=area, rax=rax, e_pas=e, i_inj=i_inj, t_end=600.0))
+    o.advance(600.0, DT)
+    G, s = g_pas * area * 1e-2, 1.0 / rax
+    kappa = np.arccosh(1 + G / (2 * s))
+    i = np.arange(n)
+    ref = e + i_inj * np.cosh(kappa * (n - 0.5 - i)) / (2 * s * np.sinh(kappa * n) * np.sinh(kappa / 2))
+    assert np.max(np.abs(o.voltage() - ref)) <= 1e-9
+    g, es, Gp = 0.0025, -30.0, 1e-4 * 400.0 * 1e-2
+    o = _lin(orc, _one_cv_syns([es], [1e15], vinit=-60.0))
+    o.set_state(syn_g=[g])
+    o.advance(40.0, DT)
+    assert o.voltage()[0] == pytest.approx((Gp * -65.0 + g * es) / (Gp + g), abs=1e-10)
+    # one step of that CV by hand: V' = (C/dt V + G E + g e) / (C/dt + G + g)
+    o = _lin(orc, _one_cv_syns([es], [2.0], vinit=-60.0))
+    o.set_state(syn_g=[g])
+    o.advance(DT, DT)
+    C = 1.0 * 400.0 * 1e-5
+    assert o.voltage()[0] == pytest.approx((C / DT * -60.0 + Gp * -65.0 + g * es) / (C / DT + Gp + g), rel=1e-14)
+
+
+def test_l4_linearised_converges_to_the_same_ode(orc):
+    """Single HH CV + current step against scipy: same spikes, first-order convergence (as P9), and it stays
+    finite at dt = 1 ms where the explicit step diverges (tests/test_gpu_parity.py::test_divergence_is_reported)."""
+    from scipy.integrate import solve_ivp
+    amp, t0, area = 0.08, 2.0, 500.0
+    C = 1.0 * area * 1e-5
+
+    def f(t, y):
+        v, m, h, n = y
+        am = 0.1 * (v + 40) / (1 - np.exp(-(v + 40) / 10)); bm = 4 * np.exp(-(v + 65) / 18)
+        ah = 0.07 * np.exp(-(v + 65) / 20); bh = 1 / (1 + np.exp(-(v + 35) / 10))
+        an = 0.01 * (v + 55) / (1 - np.exp(-(v + 55) / 10)); bn = 0.125 * np.exp(-(v + 65) / 80)
+        dens = W.GNABAR * m ** 3 * h * (v - W.ENA) + W.GKBAR * n ** 4 * (v - W.EK) + W.GL * (v - W.EL)
+        return [(-dens * area * 1e-2 + (amp if t >= t0 else 0.0)) / C, am * (1 - m) - bm * m, ah * (1 - h) - bh * h,
+                an * (1 - n) - bn * n]
+
+    r = orc.hh_rates(-65.0)
+    y0 = [-65.0, r[0] / (r[0] + r[1]), r[2] / (r[2] + r[3]), r[4] / (r[4] + r[5])]
+    up = lambda t, y: y[0] - W.THRESHOLD
+    up.direction = 1
+    s1 = solve_ivp(f, (0, t0), y0, rtol=1e-11, atol=1e-13, method="LSODA")
+    s2 = solve_ivp(f, (t0, 30.0), s1.y[:, -1], rtol=1e-11, atol=1e-13, method="LSODA", events=up)
+    ref = s2.t_events[0]
+    errs = []
+    for dt in (0.02, 0.01, 0.005):
+        o = _lin(orc, _single_hh(-65.0, amp, t0, 1e9, 30.0))
+        o.advance(30.0, dt)
+        ts = o.spikes()[1]
+        assert len(ts) == len(ref)
+        errs.append(abs(ts[0] - ref[0]))
+    assert errs[0] < 0.2 and 1.6 < errs[0] / errs[1] < 2.4 and 1.6 < errs[1] / errs[2] < 2.4
+    o = _lin(orc, W.config0())
+    o.advance(100.0, 1.0)
+    assert np.all(np.isfinite(o.voltage())) and np.all(np.abs(o.voltage()) < 200.0)
