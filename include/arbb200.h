@@ -65,6 +65,12 @@ enum {
                                 the coming step are integrated first (their event-split steps take longer and
                                 would otherwise end up at the tail of the launch); 0 = index order          */
   ARB_OPT_GROUP_CTAS = 6,    /* cell-group kernel: cap on the CTAs of a launch (0 = as many as are resident) */
+  ARB_OPT_LINEARISED = 8,    /* 1: the conductance-linearised variant of the implicit Euler step (PAPER.md:152-156
+                                with every membrane current g_k (V' - E_k) taken at the new voltage: conductances
+                                on the diagonal, sources g_k E_k on the right-hand side; the matrix is assembled
+                                and eliminated every step; unconditionally stable).  0 (default): explicit membrane
+                                currents, the equation as printed at PAPER.md:154 (reading R1), matrix
+                                factorised once per dt.  Not available for models with block units.         */
   ARB_OPT_TIMING = 3         /* 1: bracket the cable-step launches and the epoch-boundary kernels of
                                 every epoch with CUDA events on the model's stream (read them with
                                 ARB_PROBE_TIMING); setting the option clears the accumulated times  */

@@ -14,6 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libarbb200.so")
 ARB_OK, ARB_E_NULL, ARB_E_INVALID, ARB_E_WORKSPACE, ARB_E_CUDA, ARB_E_OVERFLOW, ARB_E_NOMEM, ARB_E_DIVERGED = 0, -1, -2, -3, -4, -5, -6, -7
 ARB_PROBE_M, ARB_PROBE_H, ARB_PROBE_N, ARB_PROBE_SYN_G, ARB_PROBE_TIME, ARB_PROBE_NSTEPS, ARB_PROBE_STATS, ARB_PROBE_TIMING = range(8)
 ARB_OPT_FUSED_STEPS, ARB_OPT_EPOCH_STEPS, ARB_OPT_TIMING, ARB_OPT_OVERLAP, ARB_OPT_L2_PREFETCH, ARB_OPT_GROUP_CTAS, ARB_OPT_HOT_FIRST = 1, 2, 3, 4, 5, 6, 7
+ARB_OPT_LINEARISED = 8
 
 EXPORTS = ("arb_plan", "arb_create", "arb_advance", "arb_spikes", "arb_clear_spikes", "arb_voltage", "arb_probe",
            "arb_set_state", "arb_set_option", "arb_fp64_peak", "arb_destroy", "arb_last_error")

@@ -640,6 +640,12 @@ int arb_set_option(arb_model* m, int key, int64_t value) {
     case ARB_OPT_FUSED_STEPS: m->opt_fused = value; return ARB_OK;
     case ARB_OPT_EPOCH_STEPS: m->opt_epoch = value; return ARB_OK;
     case ARB_OPT_OVERLAP: m->opt_overlap = value != 0; return ARB_OK;
+    case ARB_OPT_LINEARISED:
+      if (value != 0 && m->H.n_units > m->H.n_forests)
+        return fail(m, ARB_E_INVALID, "arb_set_option: the conductance-linearised step is not available for block units (cells with "
+                                      ">= 1,024 synapses or too large for shared memory)");
+      if ((value != 0) != (m->D.linearised != 0)) { m->D.linearised = value != 0; m->factored_dt = 0.0; }   // coefficients are rebuilt
+      return ARB_OK;
     case ARB_OPT_L2_PREFETCH: m->D.l2_prefetch = value != 0; return ARB_OK;
     case ARB_OPT_GROUP_CTAS: m->opt_group_ctas = value; return ARB_OK;
     case ARB_OPT_HOT_FIRST: m->opt_hot = value != 0; m->prev_marked_hot = false; return ARB_OK;

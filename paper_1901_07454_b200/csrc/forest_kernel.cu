@@ -127,7 +127,10 @@ __device__ __forceinline__ void mob_normalise(Mob& m) {
   m.a *= sc; m.b *= sc; m.c *= sc; m.d *= sc;
 }
 
-template <bool kSel>
+// kSel: 0 = once per dt, every cell, c_k = C_k/dt; 1 = event-split sub-steps: the cells in mode 2, c_k = C_k/delta;
+// 2 = conductance-linearised step (ARB_OPT_LINEARISED): every active cell, c_k read from invdout[], where
+// forest_substep has assembled C_k/delta + G_k + sum of the point mechanisms' conductances.
+template <int kSel>
 __device__ __forceinline__ void eliminate_chunk(const FView& U, const CellS* cs, double dt, const FChunk& ck, int lane,
                                                 double* fout, double* invdout, double& cx, double& csig) {
   const int n = (int)(ck.br_n & 63u);
@@ -140,12 +143,12 @@ __device__ __forceinline__ void eliminate_chunk(const FView& U, const CellS* cs,
   if (kSel) {
     if (valid) {
       const uint32_t c = U.br_cell[br];
-      on = cs->mode[c] == 2u;
+      on = kSel == 1 ? cs->mode[c] == 2u : cs->mode[c] != 0u;
       delta = cs->delta[c];
     }
   }
   double c = 1.0, sg = 0.0;
-  if (valid) { c = U.C[s] / delta; sg = U.sig[s]; }
+  if (valid) { c = kSel == 2 ? invdout[s] : U.C[s] / delta; sg = U.sig[s]; }
   const double snext = __shfl_down_sync(kFull, sg, 1);
   Mob m;
   if (!valid || tail) {
@@ -185,13 +188,13 @@ __device__ __forceinline__ void eliminate_chunk(const FView& U, const CellS* cs,
   csig = __shfl_sync(kFull, sg, 0);
 }
 
-template <bool kSel>
+template <int kSel>
 __device__ __forceinline__ void eliminate_forest(const FView& U, const CellS* cs, double dt, double* fout, double* invdout) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (int lvl = (int)U.n_level - 1; lvl >= 0; --lvl) {
     const FRun R = U.runs[lvl * kW + warp];
     double cx = 1.0, csig = 0.0;
-    const unsigned long long want = kSel ? U.masks[1] : ~0ull;
+    const unsigned long long want = kSel == 1 ? U.masks[1] : (kSel == 2 ? U.masks[0] : ~0ull);
     for (uint32_t ci = R.chunk_end; ci-- > R.chunk_beg;) {
       if (kSel && !(U.chunk_cells[ci] & want)) continue;     // no cell of this chunk takes a step of its own length
       eliminate_chunk<kSel>(U, cs, dt, load_chunk(U.chunks + ci), lane, fout, invdout, cx, csig);
@@ -212,7 +215,7 @@ __device__ __forceinline__ void eliminate_forest(const FView& U, const CellS* cs
 // lookup (warp-uniform): some cell of the chunk is not on a plain step: each lane asks for its cell's mode
 // (0 inactive: left alone; 2: a step of its own length, factors from the forest's scratch record).
 __device__ __forceinline__ void backward_chunk(const FView& U, const CellS& cs, const FChunk& ck, double f, double invd, int lane,
-                                               bool lookup, double& cf, double& cr) {
+                                               bool lookup, bool lin, double& cf, double& cr) {
   const int n = (int)(ck.br_n & 63u);
   const bool valid = lane < n;
   const uint32_t s = ck.slot0 + lane;
@@ -223,7 +226,7 @@ __device__ __forceinline__ void backward_chunk(const FView& U, const CellS& cs, 
   if (valid) {
     if (lookup) {
       md = cs.mode[U.br_cell[br]];
-      if (md == 2u) { f = U.fgen[s]; invd = U.invdgen[s]; }
+      if (md == 2u && !lin) { f = U.fgen[s]; invd = U.invdgen[s]; }
     }
     r = U.V[s];
     if (tail) {
@@ -256,7 +259,7 @@ __device__ __forceinline__ void backward_chunk(const FView& U, const CellS& cs, 
 
 // Forward (root -> leaves) substitution of one chunk: V'_k = r_k/d_k - f_k V'_{k-1}; V <- V'.
 // cv: V' of the slot before the chunk (the chunk of the run swept before this one).
-__device__ __forceinline__ void forward_chunk(const FView& U, const CellS& cs, const FChunk& ck, double f, int lane, bool lookup, double& cv) {
+__device__ __forceinline__ void forward_chunk(const FView& U, const CellS& cs, const FChunk& ck, double f, int lane, bool lookup, bool lin, double& cv) {
   const int n = (int)(ck.br_n & 63u);
   const bool valid = lane < n;
   const uint32_t s = ck.slot0 + lane;
@@ -267,7 +270,7 @@ __device__ __forceinline__ void forward_chunk(const FView& U, const CellS& cs, c
   if (valid) {
     if (lookup) {
       md = cs.mode[U.br_cell[br]];
-      if (md == 2u) f = U.fgen[s];
+      if (md == 2u && !lin) f = U.fgen[s];
     }
     const double q = U.V[s];
     if (head) {
@@ -317,7 +320,9 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
   const uint32_t n_hh = U.n_hh, n_syn = U.n_syn, n_cl = U.n_clamp;
 
   // event-split sub-steps: those cells' matrices are eliminated for their own step length (reading R9)
-  if (kGen && U.masks[1] != 0ull) eliminate_forest<true>(U, &cs, dt, U.fgen, U.invdgen);
+  const bool lin = M.linearised != 0;
+  double* xG = U.xI + (n_hh + n_syn + n_cl);                 // lin: conductances beside the sources
+  if (!lin && kGen && U.masks[1] != 0ull) eliminate_forest<1>(U, &cs, dt, U.fgen, U.invdgen);
 
   // ---- B: currents of HH, synapses and clamps from V(t); the passive current is
   // folded into a, b.  Items on one CV form a run; the first item of a run sums it in index order.
@@ -325,20 +330,29 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
     if (kGen && !cs.mode[multi ? U.hh_cell[i] : 0]) continue;
     const double v = U.V[__ldg(U.hh_slot + i)];
     const double m = U.m[i], h = U.h[i], n = U.n[i];
-    U.xI[i] = __ldg(U.hh_gna + i) * m * m * m * h * (v - M.ena) + __ldg(U.hh_gk + i) * n * n * n * n * (v - M.ek) + __ldg(U.hh_gl + i) * (v - M.el);
+    if (!lin) {
+      U.xI[i] = __ldg(U.hh_gna + i) * m * m * m * h * (v - M.ena) + __ldg(U.hh_gk + i) * n * n * n * n * (v - M.ek) + __ldg(U.hh_gl + i) * (v - M.el);
+    } else {
+      const double gna = __ldg(U.hh_gna + i) * m * m * m * h, gk = __ldg(U.hh_gk + i) * n * n * n * n, gl = __ldg(U.hh_gl + i);
+      xG[i] = gna + gk + gl;
+      U.xI[i] = gna * M.ena + gk * M.ek + gl * M.el;
+    }
   }
   for (uint32_t i = tid; i < n_syn; i += kT) {
     const uint32_t slot = __ldg(U.syn_slot + i);
     if (i > 0 && __ldg(U.syn_slot + i - 1) == slot) continue;
     if (kGen && !cs.mode[multi ? U.syn_cell[i] : 0]) continue;
     const double v = U.V[slot];
-    double I = 0.0;
+    double I = 0.0, G = 0.0;
     uint32_t j = i;
     do {
-      I += U.g[j] * (v - (M.syn_uniform ? M.syn_e_u : __ldg(U.syn_e + j)));
+      const double es = M.syn_uniform ? M.syn_e_u : __ldg(U.syn_e + j);
+      if (!lin) I += U.g[j] * (v - es);
+      else { G += U.g[j]; I += U.g[j] * es; }
       ++j;
     } while (j < n_syn && __ldg(U.syn_slot + j) == slot);
     U.xI[n_hh + i] = I;
+    if (lin) xG[n_hh + i] = G;
   }
   for (uint32_t i = tid; i < n_cl; i += kT) {
     const uint32_t slot = U.cl_slot[i];
@@ -352,7 +366,7 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
       if (U.cl_t0[j] <= t && t < U.cl_t1[j]) I -= U.cl_amp[j];
       ++j;
     } while (j < n_cl && U.cl_slot[j] == slot);
-    U.xI[n_hh + n_syn + i] = I;
+    U.xI[n_hh + n_syn + i] = lin ? -I : I;                   // lin: sources are ADDED to the rhs
   }
   __syncthreads();
 
@@ -370,8 +384,14 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
       const uint32_t c = U.br_cell[branch_of(ck, lane)], md = cs.mode[c];
       const uint32_t s = ck.slot0 + lane;
       if (md == 1u) U.V[s] = fma(__ldg(U.a + s), U.V[s], __ldg(U.b + s));
-      else if (md == 2u) U.V[s] = fma(U.C[s] / cs.delta[c] - U.G[s], U.V[s], U.bg[s]);
+      else if (md == 2u) U.V[s] = fma(lin ? U.C[s] / cs.delta[c] : U.C[s] / cs.delta[c] - U.G[s], U.V[s], U.bg[s]);
+      // lin: the diagonal without the point mechanisms, C/delta + G (the nominal one sits in the f slot)
+      if (lin && md) U.invdgen[s] = md == 1u ? __ldg(U.f + s) : U.C[s] / cs.delta[c] + U.G[s];
     }
+  }
+  if (lin && !kGen) {
+    const uint32_t n = U.n_slot;
+    for (uint32_t s = tid; s < n; s += kT) U.invdgen[s] = __ldg(U.f + s);
   }
   __syncthreads();
   // HH, synapse and clamp currents of a cell may meet on a control volume: barriers in between, unless the
@@ -380,7 +400,9 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
   if (n_hh) {
     for (uint32_t i = tid; i < n_hh; i += kT) {
       if (kGen && !cs.mode[multi ? U.hh_cell[i] : 0]) continue;
-      U.V[__ldg(U.hh_slot + i)] -= U.xI[i];
+      const uint32_t slot = __ldg(U.hh_slot + i);
+      if (!lin) U.V[slot] -= U.xI[i];
+      else { U.V[slot] += U.xI[i]; U.invdgen[slot] += xG[i]; }
     }
     if (!disjoint) __syncthreads();
   }
@@ -389,7 +411,8 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
       const uint32_t slot = __ldg(U.syn_slot + i);
       if (i > 0 && __ldg(U.syn_slot + i - 1) == slot) continue;
       if (kGen && !cs.mode[multi ? U.syn_cell[i] : 0]) continue;
-      U.V[slot] -= U.xI[n_hh + i];
+      if (!lin) U.V[slot] -= U.xI[n_hh + i];
+      else { U.V[slot] += U.xI[n_hh + i]; U.invdgen[slot] += xG[n_hh + i]; }
     }
     if (!disjoint) __syncthreads();
   }
@@ -398,11 +421,13 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
       const uint32_t slot = U.cl_slot[i];
       if (i > 0 && U.cl_slot[i - 1] == slot) continue;
       if (kGen && !cs.mode[multi ? U.cl_cell[i] : 0]) continue;
-      U.V[slot] -= U.xI[n_hh + n_syn + i];
+      if (!lin) U.V[slot] -= U.xI[n_hh + n_syn + i]; else U.V[slot] += U.xI[n_hh + n_syn + i];
     }
     if (!disjoint) __syncthreads();
   }
   if (disjoint && (n_hh | n_syn | n_cl)) __syncthreads();
+  // lin: every active cell's matrix is eliminated afresh (its factors go to the forest's scratch record)
+  if (lin) eliminate_forest<2>(U, &cs, dt, U.fgen, U.invdgen);
 
   // ---- D: backward sweep, deepest level first; E: forward substitution, root first; V <- V'
   // The chunk after the one being swept is fetched first (its record from shared memory, its factors from
@@ -421,7 +446,10 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
     auto fetch = [&](uint32_t ci, FChunk& k, double& f, double& invd) {
       k = load_chunk(U.chunks + ci);
       f = 0.0; invd = 0.0;
-      if (lane < (int)(k.br_n & 63u)) { f = __ldg(U.f + k.slot0 + lane); invd = __ldg(U.invd + k.slot0 + lane); }
+      if (lane < (int)(k.br_n & 63u)) {
+        if (!lin) { f = __ldg(U.f + k.slot0 + lane); invd = __ldg(U.invd + k.slot0 + lane); }
+        else { f = U.fgen[k.slot0 + lane]; invd = U.invdgen[k.slot0 + lane]; }
+      }
     };
     double cf = 0.0, cr = 0.0, f = 0.0, invd = 0.0;
     FChunk ck;
@@ -432,7 +460,7 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
       FChunk nck = ck;
       double nf = 0.0, ni = 0.0;
       if (nx != kNone) fetch(nx, nck, nf, ni);
-      backward_chunk(U, cs, ck, f, invd, lane, kGen && (U.chunk_cells[cur] & odd) != 0ull, cf, cr);
+      backward_chunk(U, cs, ck, f, invd, lane, kGen && (U.chunk_cells[cur] & odd) != 0ull, lin, cf, cr);
       cur = nx; ck = nck; f = nf; invd = ni;
     }
     level_sync(warp_cells);
@@ -445,7 +473,7 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
     };
     auto fetch = [&](uint32_t ci, FChunk& k, double& f) {
       k = load_chunk(U.chunks + ci);
-      f = lane < (int)(k.br_n & 63u) ? __ldg(U.f + k.slot0 + lane) : 0.0;
+      f = lane < (int)(k.br_n & 63u) ? (lin ? U.fgen[k.slot0 + lane] : __ldg(U.f + k.slot0 + lane)) : 0.0;
     };
     double cv = 0.0, f = 0.0;
     FChunk ck;
@@ -456,7 +484,7 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
       FChunk nck = ck;
       double nf = 0.0;
       if (nx != kNone) fetch(nx, nck, nf);
-      forward_chunk(U, cs, ck, f, lane, kGen && (U.chunk_cells[cur] & odd) != 0ull, cv);
+      forward_chunk(U, cs, ck, f, lane, kGen && (U.chunk_cells[cur] & odd) != 0ull, lin, cv);
       cur = nx; ck = nck; f = nf;
     }
     level_sync(warp_cells);
@@ -622,12 +650,26 @@ __global__ void __launch_bounds__(kForestThreads) forest_factor_kernel(DevModel 
   __syncthreads();
   FView U;
   make_fview(U, M, H, fast, M.state + d.state_base, M.topo + H.topo_off);
-  eliminate_forest<false>(U, nullptr, dt, const_cast<double*>(U.f), const_cast<double*>(U.invd));
   double* a = const_cast<double*>(U.a);
   double* b = const_cast<double*>(U.b);
-  for (uint32_t s = threadIdx.x; s < U.n_slot; s += kT) {
-    a[s] = U.C[s] / dt - U.G[s];
-    b[s] = U.bg[s];
+  if (!M.linearised) {
+    eliminate_forest<0>(U, nullptr, dt, const_cast<double*>(U.f), const_cast<double*>(U.invd));
+    for (uint32_t s = threadIdx.x; s < U.n_slot; s += kT) {
+      a[s] = U.C[s] / dt - U.G[s];
+      b[s] = U.bg[s];
+    }
+  } else {
+    // conductance-linearised step: rhs = (C/dt) V + G e + ..., and the part of the diagonal that does not change
+    // from step to step, C/dt + G, in the f slot (the elimination works with x_k = d_k - sigma_k and needs sigma)
+    double* f = const_cast<double*>(U.f);
+    double* invd = const_cast<double*>(U.invd);
+    for (uint32_t s = threadIdx.x; s < U.n_slot; s += kT) {
+      const double cdt = U.C[s] / dt;
+      a[s] = cdt;
+      b[s] = U.bg[s];
+      f[s] = cdt + U.G[s];
+      invd[s] = U.sig[s];
+    }
   }
   if (!M.syn_uniform) {
     double* decay = const_cast<double*>(U.syn_decay);

@@ -102,7 +102,7 @@ ARBB_HD ForestSmemPlan forest_smem_plan(const ForestCaps& c) {
   uint32_t p = align_up(c.state_bytes, 128);
   P.off_topo = p; p = align_up(p + c.topo_bytes, 16);
   P.off_con = p;  p = align_up(p + 8 * c.n_branch, 16);
-  P.off_xi = p;   p = align_up(p + 8 * c.n_spec, 16);
+  P.off_xi = p;   p = align_up(p + 16 * c.n_spec, 16);    // currents (sources | conductances when linearised)
   P.off_cell = p; p = align_up(p + kCellScratchBytes * (c.n_cell ? c.n_cell : 1u), 16);
   P.bytes = align_up(p, 128);
   return P;

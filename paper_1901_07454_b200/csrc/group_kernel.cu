@@ -168,6 +168,28 @@ __device__ __forceinline__ void eliminate_seg_smem(const GView& U, const SegRec&
   zcon[seg_idx * kG + c] = z;
 }
 
+// Elimination for the conductance-linearised step (PAPER.md:152-156 with the membrane
+// conductances on the diagonal): F holds the assembled diagonal C/delta + sum(sigma) + sum(g) of this cell, I its
+// link conductances sigma; both are replaced by f_k = -sigma_k / d_k and 1 / d_k.  The same recurrence as the
+// oracle's Hines elimination: d_parent -= sigma_c^2 / d_c.
+__device__ __forceinline__ void eliminate_seg_lin(const GView& U, const SegRec& sg, uint32_t seg_idx, int c, double* F, double* I, double* dcon) {
+  uint32_t lin = (sg.slot0 + sg.len - 1) * kG + c;
+  double carry = 0.0;                     // f_{k+1} sigma_{k+1}: what row k loses to its child in the segment
+  for (uint32_t j = 0; j < sg.ccnt; ++j) carry -= dcon[(uint32_t)U.child[sg.cbeg + j] * kG + c];
+  double fk = 0.0, sk = 0.0;
+#pragma unroll 2
+  for (int left = sg.len; left > 0; --left, lin -= kG) {
+    const uint32_t p = gswz(lin);
+    const double invd = 1.0 / (F[p] + carry);
+    sk = I[p];
+    fk = -sk * invd;
+    F[p] = fk;
+    I[p] = invd;
+    carry = fk * sk;
+  }
+  dcon[seg_idx * kG + c] = -fk * sk;
+}
+
 // ------------------------------------------------------------------------------------------
 // Backward (leaves -> root) sweep of one segment on the rhs held in Vs:
 //   rhs_{k-1} -= f_k rhs_k along the segment; the parent control volume loses con[segment] = f_0 rhs_0;
@@ -330,7 +352,11 @@ __device__ __forceinline__ void run_deferred(HHDefer& dh, double* dst0, double* 
 // from the END of the CTA (thread kT-1 first) so that they do not land on warp 0, which owns the
 // serial parts (phase A, the narrow stages).  The HH gate updates come back deferred in `dh`.
 // ------------------------------------------------------------------------------------------
-template <bool kGen>
+// kLin: the conductance-linearised step (ARB_OPT_LINEARISED).  The four coefficient arrays of the const record then
+// hold C/dt, G e, C/dt + sum(sigma) + G and sigma (group_factor_kernel): phase B computes every point mechanism's
+// conductance and source g E instead of its current, the sources are added to the rhs, the conductances to the
+// diagonal, and every cell's matrix is eliminated in shared memory before the sweeps.
+template <bool kGen, bool kLin>
 __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U, double* Vs, const double* Fs, const double* Is,
                                               double* buf, const CellS& cs, double dt, HHDefer& dh, double vprev, double tstart,
                                               const uint8_t* fg, uint32_t vbytes, uint64_t* mbarB, uint32_t& parB) {
@@ -342,14 +368,21 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
   // ---- B: currents of HH, synapses and clamps from V(t); the passive current is
   // folded into a, b.  Items of one cell on one CV form a run; its first item sums it in index order.
   double* xI = buf;
+  double* xG = buf + (nE_hh + nE_syn + nE_cl);       // kLin: conductances beside the sources
 #pragma unroll 1
   for (uint32_t e = rtid; e < nE_hh; e += kT) {
     const uint32_t slot = U.hh_slot[e];
     if (slot == kNoSlot16 || !rmd) continue;
     const double v = Vs[gpos(slot, rc)];
     const double m = U.sm[e], hh = U.sm[e + U.hh_ss], n = U.sm[e + 2 * U.hh_ss];
-    xI[e] = U.hh_gna[e] * m * m * m * hh * (v - M.ena) + U.hh_gna[e + U.hh_cs] * n * n * n * n * (v - M.ek) +
-            U.hh_gna[e + 2 * U.hh_cs] * (v - M.el);
+    if (!kLin) {
+      xI[e] = U.hh_gna[e] * m * m * m * hh * (v - M.ena) + U.hh_gna[e + U.hh_cs] * n * n * n * n * (v - M.ek) +
+              U.hh_gna[e + 2 * U.hh_cs] * (v - M.el);
+    } else {
+      const double gna = U.hh_gna[e] * m * m * m * hh, gk = U.hh_gna[e + U.hh_cs] * n * n * n * n, gl = U.hh_gna[e + 2 * U.hh_cs];
+      xG[e] = gna + gk + gl;
+      xI[e] = gna * M.ena + gk * M.ek + gl * M.el;
+    }
   }
 #pragma unroll 1
   for (uint32_t e = rtid; e < nE_syn; e += kT) {
@@ -357,13 +390,16 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
     if (slot == kNoSlot16 || !rmd) continue;
     if (e >= (uint32_t)kG && U.syn_slot[e - kG] == slot) continue;
     const double v = Vs[gpos(slot, rc)];
-    double I = 0.0;
+    double I = 0.0, G = 0.0;
     uint32_t j = e;
     do {
-      I += U.sg[j] * (v - (M.syn_uniform ? M.syn_e_u : U.syn_e()[j]));
+      const double es = M.syn_uniform ? M.syn_e_u : U.syn_e()[j];
+      if (!kLin) I += U.sg[j] * (v - es);
+      else { G += U.sg[j]; I += U.sg[j] * es; }
       j += kG;
     } while (j < nE_syn && U.syn_slot[j] == slot);
     xI[nE_hh + e] = I;
+    if (kLin) xG[nE_hh + e] = G;
   }
   if (nE_cl) {
     const double t = kGen ? cs.tcur[rc] : tstart;
@@ -379,7 +415,7 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
         if (cl_t0[j] <= t && t < cl_t1[j]) I -= cl_amp[j];
         j += kG;
       } while (j < nE_cl && cl_slot[j] == slot);
-      xI[nE_hh + nE_syn + e] = I;
+      xI[nE_hh + nE_syn + e] = kLin ? -I : I;          // kLin: sources are ADDED to the rhs
     }
   }
   __syncthreads();
@@ -401,7 +437,7 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
 #pragma unroll 4
       for (uint32_t p = tid; p < nE_cv; p += kT) Vr[p] = fma(ar[p], Vr[p], br[p]);
     } else if (pmd == 2u) {
-      // (C/delta - G) V + G e  with  C/delta - G = a + (r - 1) C/dt  and  G e = b
+      // (C/delta - G) V + G e  with  C/delta - G = a + (r - 1) C/dt  and  G e = b   (kLin: a = C/dt, C/delta = r a)
       const double* __restrict__ ar = Fs; const double* __restrict__ br = Is; const double* __restrict__ C = U.C();
       const double rm1 = dt / cs.delta[pcell] - 1.0;
 #pragma unroll 4
@@ -425,7 +461,7 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
   for (uint32_t e = rtid; e < nE_hh; e += kT) {
       const uint32_t slot = U.hh_slot[e];
       if (slot == kNoSlot16 || !rmd) continue;
-      Vs[gpos(slot, rc)] -= xI[e];
+      if (!kLin) Vs[gpos(slot, rc)] -= xI[e]; else Vs[gpos(slot, rc)] += xI[e];
     }
     if (!disjoint) __syncthreads();
   }
@@ -435,7 +471,7 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
       const uint32_t slot = U.syn_slot[e];
       if (slot == kNoSlot16 || !rmd) continue;
       if (e >= (uint32_t)kG && U.syn_slot[e - kG] == slot) continue;
-      Vs[gpos(slot, rc)] -= xI[nE_hh + e];
+      if (!kLin) Vs[gpos(slot, rc)] -= xI[nE_hh + e]; else Vs[gpos(slot, rc)] += xI[nE_hh + e];
     }
     if (!disjoint) __syncthreads();
   }
@@ -445,16 +481,56 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
       const uint32_t slot = cl_slot[e];
       if (slot == kNoSlot16 || !rmd) continue;
       if (e >= (uint32_t)kG && cl_slot[e - kG] == slot) continue;
-      Vs[gpos(slot, rc)] -= xI[nE_hh + nE_syn + e];
+      if (!kLin) Vs[gpos(slot, rc)] -= xI[nE_hh + nE_syn + e]; else Vs[gpos(slot, rc)] += xI[nE_hh + nE_syn + e];
     }
     if (!disjoint) __syncthreads();
   }
   if (disjoint && (nE_hh | nE_syn | nE_cl)) __syncthreads();
   mbar_wait(mbarB, parB);
   parB ^= 1u;
+  if (kLin) {
+    // the coefficient buffers now hold the assembled diagonal without the point mechanisms and sigma: add the
+    // conductances (different kinds may share a control volume: in turn), on event-split sub-steps the larger
+    // C/delta, then eliminate every cell's matrix, stage by stage
+    double* F = const_cast<double*>(Fs);
+    double* I = const_cast<double*>(Is);
+#pragma unroll 1
+    for (uint32_t e = rtid; e < nE_hh; e += kT) {
+      const uint32_t slot = U.hh_slot[e];
+      if (slot == kNoSlot16 || !rmd) continue;
+      F[gpos(slot, rc)] += xG[e];
+    }
+    __syncthreads();
+#pragma unroll 1
+    for (uint32_t e = rtid; e < nE_syn; e += kT) {
+      const uint32_t slot = U.syn_slot[e];
+      if (slot == kNoSlot16 || !rmd) continue;
+      if (e >= (uint32_t)kG && U.syn_slot[e - kG] == slot) continue;
+      F[gpos(slot, rc)] += xG[nE_hh + e];
+    }
+    if (kGen) {
+      __syncthreads();
+      const uint32_t pcell = gswz((uint32_t)tid) % kG;
+      if (cs.mode[pcell] == 2u) {
+        const double* __restrict__ C = U.C();
+        const double rm1 = dt / cs.delta[pcell] - 1.0;
+        for (uint32_t p = tid; p < nE_cv; p += kT) F[p] = fma(rm1, C[p] / dt, F[p]);
+      }
+    }
+    __syncthreads();
+    for (uint32_t st = 0; st < U.n_stage; ++st) {
+      const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
+      if (!kGen || md != 0u)
+        for (uint32_t q = beg; q < end; ++q) {
+          const uint32_t si = U.order[q];
+          eliminate_seg_lin(U, load_seg(U.segs + si), si, c, F, I, buf);
+        }
+      __syncthreads();
+    }
+  }
   // ---- event-split sub-steps: this cell's matrix is re-eliminated for its own delta (reading R9); its
   // column of the shared-memory factors is overwritten (every (sub-)step copies them afresh)
-  if (kGen) {
+  if (kGen && !kLin) {
     double* F = const_cast<double*>(Fs);
     double* I = const_cast<double*>(Is);
     for (uint32_t st = 0; st < U.n_stage; ++st) {
@@ -661,7 +737,8 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
         run_deferred(dh, U.sm, U.gm, U.hh_ss);
         if (!ab_ready) reload_ab();
         ab_ready = false;
-        group_substep<false>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, vprev, ta, M.fast + D.const_off + co.f, vbytes, mbar + 1, par2);
+        if (!M.linearised) group_substep<false, false>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, vprev, ta, M.fast + D.const_off + co.f, vbytes, mbar + 1, par2);
+        else group_substep<false, true>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, vprev, ta, M.fast + D.const_off + co.f, vbytes, mbar + 1, par2);
         __syncthreads();                  // flags are rewritten by the next grid step
         continue;
       }
@@ -706,7 +783,8 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
         if (!ab_ready) reload_ab();
         ab_ready = false;
         {                                 // (all cells nominal only after events delivered exactly at the step start)
-          group_substep<true>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, 0.0, 0.0, M.fast + D.const_off + co.f, vbytes, mbar + 1, par2);
+          if (!M.linearised) group_substep<true, false>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, 0.0, 0.0, M.fast + D.const_off + co.f, vbytes, mbar + 1, par2);
+          else group_substep<true, true>(M, U, Vs, Fs, Is, buf, cs, A.dt, dh, 0.0, 0.0, M.fast + D.const_off + co.f, vbytes, mbar + 1, par2);
         }
         __syncthreads();
       }
@@ -769,20 +847,32 @@ __global__ void __launch_bounds__(kGroupThreads) group_factor_kernel(DevModel M,
   const int tid = threadIdx.x, c = tid % kG, h = tid / kG;
   double* f = (double*)(cb + co.f);
   double* invd = (double*)(cb + co.invd);
-  for (uint32_t st = 0; st < U.n_stage; ++st) {
-    const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
-    for (uint32_t q = beg; q < end; ++q) {
-      const uint32_t si = U.order[q];
-      eliminate_seg(U, load_seg(U.segs + si), si, c, dt, f, invd, dcon);
-    }
-    __syncthreads();
-  }
   double* a = (double*)(cb + co.a);
   double* b = (double*)(cb + co.b);
   const double *C = U.C(), *G = U.G(), *bg = U.bg();
-  for (uint32_t e = tid; e < gcv_elems(U.n_cv); e += kT) {
-    a[e] = C[e] / dt - G[e];
-    b[e] = bg[e];
+  if (!M.linearised) {
+    for (uint32_t st = 0; st < U.n_stage; ++st) {
+      const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
+      for (uint32_t q = beg; q < end; ++q) {
+        const uint32_t si = U.order[q];
+        eliminate_seg(U, load_seg(U.segs + si), si, c, dt, f, invd, dcon);
+      }
+      __syncthreads();
+    }
+    for (uint32_t e = tid; e < gcv_elems(U.n_cv); e += kT) {
+      a[e] = C[e] / dt - G[e];
+      b[e] = bg[e];
+    }
+  } else {
+    // conductance-linearised step: rhs = (C/dt) V + G e + ..., diagonal C/dt + sum(sigma) + G + ..., sigma
+    const double *S = U.S(), *sig = U.sig();
+    for (uint32_t e = tid; e < gcv_elems(U.n_cv); e += kT) {
+      const double cdt = C[e] / dt;
+      a[e] = cdt;
+      b[e] = bg[e];
+      f[e] = (cdt + S[e]) + G[e];
+      invd[e] = sig[e];
+    }
   }
   if (!M.syn_uniform) {
     double* decay = (double*)(cb + co.syn_decay);

@@ -69,6 +69,7 @@ struct DevModel {
   GroupSmemPlan gplan;
   int l2_prefetch;            // group kernel: TMA-prefetch the next group's records into L2
   int sm_count;               // SMs of the device the model lives on (grid sizing)
+  int linearised;             // ARB_OPT_LINEARISED: conductance-linearised step
   uint32_t* ghot;             // group kernel: three lists of n_groups entries (see CNT_HOT0)
   uint32_t* ghotflag;         // [2][n_groups], half launch_id & 1: launch_id of the launch whose hot list holds the group
 };
