@@ -134,6 +134,12 @@ typedef struct {
    * afterwards (every later call returns the same error): create it again with a larger cap_*.
    * (reading R0 says why the state is not rolled back to the last epoch.) */
   int64_t layout_group_min_cells, layout_forest_cv, cap_spikes, cap_events;
+  /* Sharding (cells are distributed over ranks, spikes are exchanged once per epoch).
+   * shard_n_global == 0: the model is the whole network, conn_src are its own cells.
+   * shard_n_global > 0: the model holds cells [shard_gid_base, shard_gid_base + n_cells) of a network of
+   * shard_n_global cells; conn_dst stay local, conn_src are GLOBAL cell ids (the table holds every connection
+   * whose destination is local); spikes of remote sources arrive through arb_apply_spike_blocks.           */
+  int64_t shard_gid_base, shard_n_global;
 } arb_desc;
 
 typedef struct arb_model arb_model; /* opaque; lives in host memory, owned by the library */
@@ -168,6 +174,20 @@ int arb_advance(arb_model* m, double t_end, double dt);
  * count) entries sorted by (time, cell).  cell / time may be NULL when cap == 0.  Negative on
  * error.  The history lives in host memory (arb_advance drains the device buffer into it). */
 int64_t arb_spikes(arb_model* m, int64_t* cell, double* time, int64_t cap);
+
+/* Sharded networks (arb_desc.shard_*), one call pair per epoch between two arb_advance calls; the caller moves
+ * the blocks between ranks (an all-gather: ncclAllGather / torch.distributed.all_gather_into_tensor).
+ * arb_spike_block: writes the spikes this model has produced since the previous arb_spike_block call (or since
+ * creation) into `dev_block`, a DEVICE buffer of (1 + 2 cap) 8-byte words: int64 count | int64 gid[cap] |
+ * double time[cap], global cell ids.  Returns the count, ARB_E_OVERFLOW when it exceeds cap (nothing is lost:
+ * call again with a larger block).
+ * arb_apply_spike_blocks: `dev_blocks` holds n_blocks such blocks back to back (DEVICE memory); every spike of
+ * every block except block `own_block` (this model's own: arb_advance has turned those into events already; pass
+ * -1 to apply all) is pushed through the local connection table: events (spike time + delay, synapse, weight)
+ * on the targets' queues, delivered by the following arb_advance calls.  Every epoch advanced between two exchanges
+ * must be no longer than the shortest connection delay of the WHOLE network.                                  */
+int64_t arb_spike_block(arb_model* m, void* dev_block, int64_t cap);
+int arb_apply_spike_blocks(arb_model* m, const void* dev_blocks, int64_t n_blocks, int64_t cap, int64_t own_block);
 
 /* Forget the spikes recorded so far (a caller that reads spikes after every epoch keeps the
  * history short this way).  Does not touch events already generated from them. */

@@ -16,13 +16,14 @@ ARB_PROBE_M, ARB_PROBE_H, ARB_PROBE_N, ARB_PROBE_SYN_G, ARB_PROBE_TIME, ARB_PROB
 ARB_OPT_FUSED_STEPS, ARB_OPT_EPOCH_STEPS, ARB_OPT_TIMING, ARB_OPT_OVERLAP, ARB_OPT_L2_PREFETCH, ARB_OPT_GROUP_CTAS, ARB_OPT_HOT_FIRST = 1, 2, 3, 4, 5, 6, 7
 ARB_OPT_LINEARISED = 8
 
-EXPORTS = ("arb_plan", "arb_create", "arb_advance", "arb_spikes", "arb_clear_spikes", "arb_voltage", "arb_probe",
+EXPORTS = ("arb_plan", "arb_create", "arb_advance", "arb_spikes", "arb_clear_spikes", "arb_spike_block", "arb_apply_spike_blocks",
+           "arb_voltage", "arb_probe",
            "arb_set_state", "arb_set_option", "arb_fp64_peak", "arb_destroy", "arb_last_error")
 
 # arb_desc's layout / capacity options (0 = library default).  A workloads dict may carry them under the
 # same names; LAYOUT_DEFAULTS fills in the ones it does not (the parity tests run every case under
 # several layouts this way).
-OPTION_FIELDS = ("layout_group_min_cells", "layout_forest_cv", "cap_spikes", "cap_events")
+OPTION_FIELDS = ("layout_group_min_cells", "layout_forest_cv", "cap_spikes", "cap_events", "shard_gid_base", "shard_n_global")
 LAYOUT_DEFAULTS = {}
 
 
@@ -50,6 +51,7 @@ class arb_desc(C.Structure):
         ("ext_time", C.c_void_p), ("ext_weight", C.c_void_p),
         ("layout_group_min_cells", C.c_int64), ("layout_forest_cv", C.c_int64),
         ("cap_spikes", C.c_int64), ("cap_events", C.c_int64),
+        ("shard_gid_base", C.c_int64), ("shard_n_global", C.c_int64),
     ]
 
 
@@ -74,6 +76,9 @@ def lib():
         L.arb_set_state.argtypes = [C.c_void_p] * 6
         L.arb_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
         L.arb_clear_spikes.argtypes = [C.c_void_p]
+        L.arb_spike_block.restype = C.c_int64
+        L.arb_spike_block.argtypes = [C.c_void_p, C.c_void_p, C.c_int64]
+        L.arb_apply_spike_blocks.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64]
         L.arb_fp64_peak.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.arb_destroy.argtypes = [C.c_void_p]
         L.arb_destroy.restype = None
@@ -196,6 +201,13 @@ class Model:
         if n:
             self._check(lib().arb_spikes(self._h, _ptr(cell), _ptr(t), n))
         return cell, t
+
+    def spike_block(self, block, cap):
+        """Fill `block` (a CUDA int64 tensor of 1 + 2 cap words) with the spikes since the last call; returns their count."""
+        return self._check(lib().arb_spike_block(self._h, C.c_void_p(block.data_ptr()), int(cap)))
+
+    def apply_spike_blocks(self, blocks, n_blocks, cap, own_block):
+        self._check(lib().arb_apply_spike_blocks(self._h, C.c_void_p(blocks.data_ptr()), int(n_blocks), int(cap), int(own_block)))
 
     def clear_spikes(self):
         self._check(lib().arb_clear_spikes(self._h))

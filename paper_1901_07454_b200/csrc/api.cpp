@@ -83,7 +83,7 @@ Regions carve(const HostModel& H, const Caps& cap) {
   R.ext_gidx = C.take(4 * (size_t)H.n_ext);
   R.ext_w = C.take(8 * (size_t)H.n_ext);
   R.ext_cur = C.take(4 * nc);
-  R.conn_off = C.take(4 * (nc + 1));
+  R.conn_off = C.take(4 * ((size_t)H.n_src + 1));
   R.conn_dst = C.take(4 * (size_t)H.n_conn);
   R.conn_gidx = C.take(4 * (size_t)H.n_conn);
   R.conn_delay = C.take(8 * (size_t)H.n_conn);
@@ -142,6 +142,9 @@ struct arb_model {
   std::vector<uint32_t> sp_cell;
   std::vector<double> sp_time;
   bool sp_sorted = true;
+  // shards: spikes not yet handed to arb_spike_block (global ids)
+  std::vector<int64_t> pend_gid;
+  std::vector<double> pend_t;
 };
 
 namespace {
@@ -270,6 +273,7 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     D.ext_w = at<double>(m, R.ext_w); D.ext_cur = at<uint32_t>(m, R.ext_cur);
     D.conn_off = at<uint32_t>(m, R.conn_off); D.conn_dst = at<uint32_t>(m, R.conn_dst); D.conn_gidx = at<uint32_t>(m, R.conn_gidx);
     D.conn_delay = at<double>(m, R.conn_delay); D.conn_w = at<double>(m, R.conn_w);
+    D.gid_base = H.gid_base;
     for (int i = 0; i < 2; ++i) {
       D.pool[i].t = at<double>(m, R.pool_t[i]); D.pool[i].dst = at<uint32_t>(m, R.pool_dst[i]);
       D.pool[i].gidx = at<uint32_t>(m, R.pool_gidx[i]); D.pool[i].w = at<double>(m, R.pool_w[i]);
@@ -351,6 +355,8 @@ int drain(arb_model* m, unsigned long long* cnt) {
     CU(m, cudaMemsetAsync(D.counters + CNT_SPIKES, 0, 2 * sizeof(unsigned long long), m->stream));   // CNT_SPIKES, CNT_SPIKES_DONE
     CU(m, cudaStreamSynchronize(m->stream));
     m->sp_sorted = false;
+    if (m->H.n_src != m->H.n_cells || m->H.gid_base != 0)
+      for (size_t i = old; i < old + n; ++i) { m->pend_gid.push_back(m->H.gid_base + (int64_t)m->sp_cell[i]); m->pend_t.push_back(m->sp_time[i]); }
   }
   return ARB_OK;
 }
@@ -529,6 +535,41 @@ int64_t arb_spikes(arb_model* m, int64_t* cell, double* time, int64_t cap) {
     return fail(m, ARB_E_NOMEM, "arb_spikes: out of host memory");
   }
   return count;
+}
+
+int64_t arb_spike_block(arb_model* m, void* dev_block, int64_t cap) {
+  if (!m || !dev_block) return fail(m, ARB_E_NULL, "arb_spike_block: NULL argument");
+  if (cap < 0) return fail(m, ARB_E_INVALID, "arb_spike_block: negative capacity");
+  const int64_t n = (int64_t)m->pend_gid.size();
+  if (n > cap) return fail(m, ARB_E_OVERFLOW, "arb_spike_block: " + std::to_string(n) + " spikes do not fit a block of " + std::to_string(cap));
+  try {
+    std::vector<unsigned long long> blk(1 + 2 * (size_t)cap, 0ull);
+    blk[0] = (unsigned long long)n;
+    for (int64_t i = 0; i < n; ++i) {
+      blk[1 + i] = (unsigned long long)m->pend_gid[i];
+      std::memcpy(&blk[1 + cap + i], &m->pend_t[i], 8);
+    }
+    CU(m, cudaMemcpyAsync(dev_block, blk.data(), 8 * blk.size(), cudaMemcpyHostToDevice, m->stream));
+    CU(m, cudaStreamSynchronize(m->stream));
+  } catch (const std::bad_alloc&) {
+    return fail(m, ARB_E_NOMEM, "arb_spike_block: out of host memory");
+  }
+  m->pend_gid.clear(); m->pend_t.clear();
+  return n;
+}
+
+int arb_apply_spike_blocks(arb_model* m, const void* dev_blocks, int64_t n_blocks, int64_t cap, int64_t own_block) {
+  if (!m || !dev_blocks) return fail(m, ARB_E_NULL, "arb_apply_spike_blocks: NULL argument");
+  if (m->broken) return fail(m, m->broken_code, "model unusable after an earlier error: " + m->err);
+  if (n_blocks < 0 || cap < 0) return fail(m, ARB_E_INVALID, "arb_apply_spike_blocks: negative count");
+  if (m->H.n_conn == 0 || n_blocks == 0) return ARB_OK;
+  // the events join the pool the next arb_advance builds its epoch lists from
+  CU(m, launch_remote_spikes_to_events(m->D, m->cur_pool, static_cast<const unsigned long long*>(dev_blocks), n_blocks, cap, own_block, m->stream));
+  unsigned long long cnt[CNT_COUNT];
+  CU(m, cudaMemcpyAsync(cnt, m->D.counters, sizeof cnt, cudaMemcpyDeviceToHost, m->stream));
+  CU(m, cudaStreamSynchronize(m->stream));
+  m->launches += 2;
+  return check_error_bits(m, cnt);
 }
 
 int arb_clear_spikes(arb_model* m) {

@@ -630,7 +630,7 @@ __global__ void __launch_bounds__(256) spikes_to_events_kernel(DevModel M, int c
   const int64_t n_warps = (gridDim.x * (int64_t)blockDim.x) >> 5;
   const EventPool P = M.pool[cur];
   for (unsigned long long s = first + warp; s < n_sp; s += n_warps) {
-    const uint32_t src = M.spike_cell[s];
+    const int64_t src = M.gid_base + M.spike_cell[s];
     const double ts = M.spike_t[s];
     for (uint32_t e = M.conn_off[src] + lane; e < M.conn_off[src + 1]; e += 32) {
       const unsigned long long pos = atomicAdd(&M.counters[CNT_POOL], 1ull);
@@ -638,6 +638,33 @@ __global__ void __launch_bounds__(256) spikes_to_events_kernel(DevModel M, int c
         P.t[pos] = ts + M.conn_delay[e]; P.dst[pos] = M.conn_dst[e]; P.gidx[pos] = M.conn_gidx[e]; P.w[pos] = M.conn_w[e];
       } else {
         atomicOr(&M.counters[CNT_ERROR], 2ull);
+      }
+    }
+  }
+}
+
+// sharded networks: the spikes of the other ranks, gathered into blocks, walk the same table
+__global__ void __launch_bounds__(256) remote_spikes_to_events_kernel(DevModel M, int cur, const unsigned long long* blocks, int64_t n_blocks,
+                                                                      int64_t cap, int64_t own) {
+  const int lane = threadIdx.x & 31;
+  const int64_t warp = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+  const int64_t n_warps = (gridDim.x * (int64_t)blockDim.x) >> 5;
+  const EventPool P = M.pool[cur];
+  const int64_t stride = 1 + 2 * cap;
+  for (int64_t b = 0; b < n_blocks; ++b) {
+    if (b == own) continue;
+    const unsigned long long* blk = blocks + b * stride;
+    const int64_t n = (int64_t)blk[0] < cap ? (int64_t)blk[0] : cap;
+    for (int64_t s = warp; s < n; s += n_warps) {
+      const int64_t src = (int64_t)blk[1 + s];
+      const double ts = __longlong_as_double((long long)blk[1 + cap + s]);
+      for (uint32_t e = M.conn_off[src] + lane; e < M.conn_off[src + 1]; e += 32) {
+        const unsigned long long pos = atomicAdd(&M.counters[CNT_POOL], 1ull);
+        if ((int64_t)pos < M.pool_cap) {
+          P.t[pos] = ts + M.conn_delay[e]; P.dst[pos] = M.conn_dst[e]; P.gidx[pos] = M.conn_gidx[e]; P.w[pos] = M.conn_w[e];
+        } else {
+          atomicOr(&M.counters[CNT_ERROR], 2ull);
+        }
       }
     }
   }
@@ -845,6 +872,13 @@ cudaError_t launch_spikes_to_events(const DevModel& M, int cur, cudaStream_t s, 
   spikes_to_events_kernel<<<(unsigned)(2 * M.sm_count), 256, 0, s>>>(M, cur);
   spikes_done_kernel<<<1, 1, 0, s>>>(M);
   if (launches) *launches += 2;
+  return cudaGetLastError();
+}
+
+cudaError_t launch_remote_spikes_to_events(const DevModel& M, int cur, const unsigned long long* blocks, int64_t n_blocks, int64_t cap,
+                                           int64_t own, cudaStream_t s) {
+  remote_spikes_to_events_kernel<<<(unsigned)(2 * M.sm_count), 256, 0, s>>>(M, cur, blocks, n_blocks, cap, own);
+  spikes_done_kernel<<<1, 1, 0, s>>>(M);            // records the pool demand and clamps the counter
   return cudaGetLastError();
 }
 

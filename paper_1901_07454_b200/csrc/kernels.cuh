@@ -50,7 +50,8 @@ struct DevModel {
   // external events (CSR over internal cells, time sorted) and their cursors
   const uint32_t* ext_off; const double* ext_t; const uint32_t* ext_gidx; const double* ext_w;
   uint32_t* ext_cur;
-  // network grouped by caller's source cell
+  // network grouped by source cell (global ids when the model is a shard: local cell c is source gid_base + c)
+  int64_t gid_base;
   const uint32_t* conn_off; const uint32_t* conn_dst; const uint32_t* conn_gidx;
   const double* conn_delay; const double* conn_w;
   EventPool pool[2];
@@ -96,6 +97,10 @@ cudaError_t launch_forest_cable(const DevModel& M, const StepArgs& A, int cls, c
 cudaError_t configure_forest_kernel(int max_optin_bytes);
 cudaError_t launch_build_events(const DevModel& M, int cur_pool, double t_window_end, cudaStream_t s, int* launches);
 cudaError_t launch_spikes_to_events(const DevModel& M, int cur_pool, cudaStream_t s, int* launches);
+// sharded networks: push the spikes of `n_blocks` blocks (int64 count | int64 gid[cap] | double t[cap]) except block
+// `own` through the connection table into the event pool
+cudaError_t launch_remote_spikes_to_events(const DevModel& M, int cur_pool, const unsigned long long* blocks, int64_t n_blocks,
+                                           int64_t cap, int64_t own, cudaStream_t s);
 cudaError_t launch_gather(const double* state, const uint32_t* idx, int64_t n, double* out, cudaStream_t s);
 cudaError_t launch_scatter(double* state, const uint32_t* idx, int64_t n, const double* in, cudaStream_t s);
 cudaError_t launch_gather_hh(const double* state, const uint32_t* m_idx, const uint32_t* stride, const uint32_t* cv,

@@ -58,6 +58,9 @@ uint64_t fnv1a(const uint8_t* p, size_t n) {
 int validate(const arb_desc& d, std::string& err) {
   auto fail = [&](int code, const std::string& s) { err = s; return code; };
   if (d.n_cells < 0 || d.n_clamp < 0 || d.n_conn < 0 || d.n_ext < 0) return fail(ARB_E_INVALID, "negative count");
+  if (d.shard_n_global < 0 || d.shard_gid_base < 0 || (d.shard_n_global > 0 && d.shard_gid_base + d.n_cells > d.shard_n_global))
+    return fail(ARB_E_INVALID, "shard_gid_base / shard_n_global do not describe a range of the network");
+  if (d.shard_n_global >= (int64_t)0x7FFFFFFF) return fail(ARB_E_INVALID, "more than 2^31 cells are not supported");
   if (d.n_cells == 0) return fail(ARB_E_INVALID, "model has no cells");
   if (!d.cv_off || !d.cv_parent || !d.cv_area || !d.cv_cm || !d.cv_raxial) return fail(ARB_E_NULL, "compartment arrays must not be NULL");
   bool hh_any = d.hh_gnabar || d.hh_gkbar || d.hh_gl;
@@ -113,7 +116,8 @@ int validate(const arb_desc& d, std::string& err) {
   }
   for (int64_t k = 0; k < d.n_conn; ++k) {
     int64_t s = d.conn_src[k], t = d.conn_dst[k];
-    if (s < 0 || s >= d.n_cells || t < 0 || t >= d.n_cells) return fail(ARB_E_INVALID, "connection cell out of range");
+    const int64_t n_src = d.shard_n_global > 0 ? d.shard_n_global : d.n_cells;
+    if (s < 0 || s >= n_src || t < 0 || t >= d.n_cells) return fail(ARB_E_INVALID, "connection cell out of range");
     if (d.conn_syn[k] < 0 || d.conn_syn[k] >= d.syn_off[t + 1] - d.syn_off[t]) return fail(ARB_E_INVALID, "connection synapse out of range");
     if (!(d.conn_delay[k] > 0) || !finite(d.conn_delay[k])) return fail(ARB_E_INVALID, "connection delay must be > 0 and finite (PAPER.md:96)");
     if (!finite(d.conn_weight[k])) return fail(ARB_E_INVALID, "non-finite connection weight");
@@ -749,6 +753,8 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
   H.n_cv = d.cv_off[d.n_cells];
   H.n_syn = d.syn_off ? d.syn_off[d.n_cells] : 0;
   H.n_clamp = d.n_clamp; H.n_conn = d.n_conn; H.n_ext = d.n_ext;
+  H.gid_base = d.shard_n_global > 0 ? d.shard_gid_base : 0;
+  H.n_src = d.shard_n_global > 0 ? d.shard_n_global : d.n_cells;
   H.ena = d.hh_ena; H.ek = d.hh_ek; H.el = d.hh_el; H.threshold = d.threshold;
   const int64_t nc = d.n_cells;
   // uniform synapse parameters (true for every BASELINE config): no per-synapse e / decay arrays
@@ -1181,9 +1187,9 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     B.run(unit_begin[u], unit_cells[u], nullptr, &placed, &H);
   });
   // connections grouped by caller's source cell, ascending k inside a group
-  H.conn_off.assign(nc + 1, 0);
+  H.conn_off.assign(H.n_src + 1, 0);             // by GLOBAL source id when the model is a shard
   for (int64_t k = 0; k < d.n_conn; ++k) H.conn_off[d.conn_src[k] + 1]++;
-  for (int64_t c = 0; c < nc; ++c) H.conn_off[c + 1] += H.conn_off[c];
+  for (int64_t c = 0; c < H.n_src; ++c) H.conn_off[c + 1] += H.conn_off[c];
   H.conn_dst.resize(d.n_conn); H.conn_gidx.resize(d.n_conn); H.conn_delay.resize(d.n_conn); H.conn_w.resize(d.n_conn);
   {
     std::vector<uint32_t> cur(H.conn_off.begin(), H.conn_off.end() - 1);

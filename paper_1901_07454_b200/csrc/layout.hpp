@@ -38,6 +38,7 @@ struct UnitCounts {                   // everything the offset functions need
 
 struct HostModel {
   int64_t n_cells = 0, n_cv = 0, n_syn = 0, n_clamp = 0, n_conn = 0, n_ext = 0, n_hh = 0;
+  int64_t gid_base = 0, n_src = 0;    // sharding: global id of local cell 0, cells of the whole network (= n_cells when unsharded)
   int64_t n_units = 0, n_forests = 0, n_lanes = 0;   // units: forests first, then block units
   int64_t fast_bytes = 0, state_doubles = 0, gen_doubles = 0, topo_bytes = 0, scratch_doubles = 0;
   int64_t topo_records = 0;           // distinct tree structures

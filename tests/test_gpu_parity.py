@@ -546,6 +546,58 @@ def test_full_size_c2_100ms(B, orc, layout):
 
 
 # ---------------------------------------------------------------------------------------------
+# one network over several ranks: the ranks run one after the other on this GPU
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_ranks", [2, 3])
+def test_sharded_network_equals_single_model_bit_for_bit(B, orc, n_ranks):
+    """Cells split into contiguous ranges, connections by destination owner, spike blocks exchanged once per epoch
+    (arb_spike_block / arb_apply_spike_blocks): the same bits as one model advanced with the same calls, and the
+    oracle's spikes."""
+    from paper_1901_07454_b200 import sharded as S
+    m = W.config3(n_cells=90, t_end=40.0)
+    m["conn_weight"] = m["conn_weight"] * 4
+    m["ext_weight"] = m["ext_weight"] * 4
+    grp = S.LocalGroup(B, m, n_ranks)
+    single = B.Model(m)
+    es = S.epoch_steps(float(np.min(m["conn_delay"])), DT)
+    k = 0
+    while k * DT < 40.0:
+        k += es
+        t = min(40.0, k * DT)
+        grp.advance(t, DT)
+        single.advance(t, DT)
+    assert np.array_equal(grp.gather(lambda g: g.voltage()), single.voltage())
+    assert np.array_equal(grp.gather(lambda g: g.syn_g()), single.syn_g())
+    for a, b in zip(grp.gather(lambda g: np.stack(g.gates(), 1)).T, single.gates()):
+        assert np.array_equal(a, b)
+    gc, gt = grp.spikes()
+    sc, st = single.spikes()
+    assert np.array_equal(gc, sc) and np.array_equal(gt, st) and len(sc) > 20
+    assert sum(s.model.stats()["events_delivered"] for s in grp.ranks) == single.stats()["events_delivered"]
+    o = orc.Oracle(m, threads=4)
+    o.advance(40.0, DT)
+    check_spikes(single, o, 90)
+    grp.close(), single.close()
+
+
+def test_sharded_heterogeneous_network(B, orc):
+    """configs[4] cut over two ranks (forests and groups on both): spikes against the oracle."""
+    from paper_1901_07454_b200 import sharded as S
+    m = W.config4(n_cells=80, t_end=30.0)
+    grp = S.LocalGroup(B, m, 2)
+    grp.advance(30.0, DT)
+    o = orc.Oracle(m, threads=4)
+    o.advance(30.0, DT)
+    gc, gt = grp.spikes()
+    oc, ot = o.spikes()
+    assert np.array_equal(np.bincount(gc, minlength=80), np.bincount(oc, minlength=80)) and len(oc) > 10
+    gi, oi = np.lexsort((gt, gc)), np.lexsort((ot, oc))
+    assert np.max(np.abs(gt[gi] - ot[oi])) <= 1e-3
+    assert rel(grp.gather(lambda g: g.voltage()), o.voltage()) < 1e-6
+    grp.close()
+
+
+# ---------------------------------------------------------------------------------------------
 # capacities and error paths (include/arbb200.h "Capacities")
 # ---------------------------------------------------------------------------------------------
 def _firing_net(t_end=40.0):
