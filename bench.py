@@ -329,9 +329,24 @@ def run_ours(args):
     n_other = 0 if args.no_other else 1 + max(2, args.steps // 2)
     n_e2e = max(2, min(args.steps, 4))
     total_ms = (args.warmup + args.steps + n_other + n_e2e + 2) * step_ms
-    m = wl.make(cells, total_ms, rank * cells, True)
+    sm = None
+    if args.exchange:
+        if args.config != "3":
+            raise SystemExit("bench.py --exchange is implemented for --config 3")
+        from paper_1901_07454_b200 import sharded as S
+        m = W.config3(n_cells=cells, t_end=total_ms, first_cell=rank * cells, n_global=world * cells)
+        sm = S.ShardedModel(B, None, rank, world, S.DistGroup(torch, dev) if world > 1 else None, device="cuda:%d" % local, local=m)
+        g = sm.model
+    else:
+        m = wl.make(cells, total_ms, rank * cells, True)
+        g = B.Model(m, device="cuda:%d" % local)
     assert epoch_steps_of(m) == es
-    g = B.Model(m, device="cuda:%d" % local)
+    if sm is not None:           # every epoch: integrate, then exchange the epoch's spikes (inside the timed region)
+        _adv = g.advance
+        def _advance_and_exchange(t, dt):
+            _adv(t, dt)
+            sm.exchange()
+        g.advance = _advance_and_exchange
     fused_steps = {"stream": 1, "fused": 0}
     g.set_option(B.ARB_OPT_FUSED_STEPS, fused_steps[args.mode])
     if lin:
@@ -494,7 +509,8 @@ def run_ours(args):
             "data": "synthetic",
             "config": {"workload": "%s (%d CVs), dt 0.025 ms; step = one epoch of %d grid steps" % (label, n_cv, es),
                        "mode": args.mode, "step_kind": args.step, "cells_per_gpu": cells,
-                       "parallelism": "cells sharded, no collective", "layout": layout, "layout_options": dict(B.LAYOUT_DEFAULTS),
+                       "parallelism": ("one network, cells sharded by rank, spikes all-gathered once per epoch" if args.exchange
+                                       else "cells sharded, no collective (one closed network per rank)"), "layout": layout, "layout_options": dict(B.LAYOUT_DEFAULTS),
                        "l2": ("no flush needed: each grid step streams %.2f GB >> 126 MB L2" % (alg_step / 1e9)) if alg_step > 4e8
                              else "working set of %.1f MB per grid step is L2-resident; no flush (every step rewrites the whole state)" % (alg_step / 1e6),
                        "seed": int(W.BASE_SEED + (5 if args.config == "ring" else int(args.config)))},
@@ -544,6 +560,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other", action="store_true", help="skip the other launch granularity")
     ap.add_argument("--no-as-written", action="store_true", help="skip the undriven (as worded in BASELINE.json) variant of C3")
+    ap.add_argument("--exchange", action="store_true",
+                    help="config 3, N > 1: the ranks share ONE network of N x cells cells (cells sharded, connections by destination "
+                         "owner) and all-gather their spikes once per epoch (paper_1901_07454_b200/sharded.py, SURVEY.md 8(f) NEXT-3) "
+                         "instead of integrating one closed network each")
     ap.add_argument("--layout", action="append", default=[], metavar="KEY=VALUE",
                     help="arb_desc layout / capacity option, e.g. layout_forest_cv=2048 (default: the library's)")
     ap.add_argument("--selftest-dist", action="store_true", help=argparse.SUPPRESS)

@@ -97,12 +97,20 @@ class DistGroup:
 class ShardedModel:
     """One rank's part of a sharded network: arb_create on its shard, and the epoch loop with the exchange."""
 
-    def __init__(self, binding, m_global, rank, n_ranks, group, device="cuda:0", block_cap=None, ranges=None):
+    def __init__(self, binding, m_global, rank, n_ranks, group, device="cuda:0", block_cap=None, ranges=None, local=None):
+        """m_global: the whole network (every rank cuts its shard out of it), or None with `local` = this rank's shard
+        generated on its own (a workloads dict with shard_gid_base / shard_n_global set)."""
         import torch
         self.B, self.torch, self.rank, self.n_ranks, self.group = binding, torch, rank, n_ranks, group
-        self.ranges = ranges or partition(m_global["cv_off"], n_ranks)
-        lo, hi = self.ranges[rank]
-        self.local = shard(m_global, lo, hi)
+        if local is None:
+            self.ranges = ranges or partition(m_global["cv_off"], n_ranks)
+            lo, hi = self.ranges[rank]
+            self.local = shard(m_global, lo, hi)
+        else:
+            self.local = local
+            lo = int(local["shard_gid_base"])
+            hi = lo + int(local["n_cells"])
+            self.ranges = ranges
         self.model = binding.Model(self.local, device=device)
         self.cap = int(block_cap or max(1024, 4 * (hi - lo)))
         self.block = torch.zeros(block_words(self.cap), dtype=torch.int64, device=device)

@@ -213,24 +213,27 @@ def _homogeneous(cfg, n_cells, nb, n, n_syn, t_end, first_cell=0):
     return m, rngs
 
 
-def _random_network(m, rngs, n_in, weight, ext_rate_hz, ext_syn_lo, ext_syn_hi, ext_weight, t_end):
+def _random_network(m, rngs, n_in, weight, ext_rate_hz, ext_syn_lo, ext_syn_hi, ext_weight, t_end, first_cell=0, n_global=None):
     """n_in incoming connections per cell (sources uniform, no self connection),
-    connection j of a cell lands on its synapse j; delay U(5,10) ms; Poisson external events."""
+    connection j of a cell lands on its synapse j; delay U(5,10) ms; Poisson external events.
+    n_global: the cells of `m` are cells first_cell ... of a network of n_global cells (a shard, sharded.py):
+    sources are drawn over the whole network and stay global ids, exactly as when the network is generated whole."""
     n_cells = m["n_cells"]
+    n_net = n_cells if n_global is None else int(n_global)
     src = np.empty((n_cells, n_in), np.int64)
     dly = np.empty((n_cells, n_in))
     et, es, ec = [], [], []
     for c, rng in enumerate(rngs):
-        if n_cells > 1:
-            s = rng.integers(0, n_cells - 1, n_in)
-            src[c] = s + (s >= c)
+        if n_net > 1:
+            s = rng.integers(0, n_net - 1, n_in)
+            src[c] = s + (s >= c + (first_cell if n_global is not None else 0))
         else:
             src[c] = 0
         dly[c] = rng.uniform(5.0, 10.0, n_in)
         if ext_rate_hz > 0:
             t, s = _poisson_events(rng, ext_rate_hz, t_end, ext_syn_lo, ext_syn_hi)
             et.append(t), es.append(s), ec.append(np.full(len(t), c, np.int64))
-    if n_cells > 1:
+    if n_net > 1:
         m["conn_src"] = src.reshape(-1)
         m["conn_dst"] = np.repeat(np.arange(n_cells, dtype=np.int64), n_in)
         m["conn_syn"] = np.tile(np.arange(n_in, dtype=np.int32), n_cells)
@@ -291,13 +294,17 @@ def config2(n_cells=10000, t_end=1000.0):
     return finalize(m)
 
 
-def config3(n_cells=100000, t_end=200.0, driven=True, first_cell=0):
+def config3(n_cells=100000, t_end=200.0, driven=True, first_cell=0, n_global=None):
     """configs[3]: depth-6 trees (63 branches x 8 CVs), 50 expsyn, 50 incoming connections.
     BASELINE.json names no drive; `driven` adds 200 Hz/cell Poisson input.
-    `first_cell` selects another closed network of the same population (bench.py: one per rank)."""
+    `first_cell` selects another closed network of the same population (bench.py: one per rank); with
+    `n_global` the cells are instead cells first_cell ... first_cell + n_cells of ONE network of n_global cells
+    (a rank's shard, generated without the rest: conn_src are global ids, shard_* fields are set)."""
     m, rngs = _homogeneous(3, n_cells, 63, 8, 50, t_end, first_cell)
-    _random_network(m, rngs, 50, 0.002, 200.0 if driven else 0.0, 0, 50, 0.002, t_end)
+    _random_network(m, rngs, 50, 0.002, 200.0 if driven else 0.0, 0, 50, 0.002, t_end, first_cell, n_global)
     m["name"] = "C3 large %d%s" % (n_cells, "" if driven else " undriven")
+    if n_global is not None:
+        m["shard_gid_base"], m["shard_n_global"] = int(first_cell), int(n_global)
     return finalize(m)
 
 
