@@ -112,6 +112,9 @@ typedef struct {
   int64_t* clamps; int64_t n_clamps;
   int32_t det; double v_prev; int armed;
   double new_spikes[8]; int n_new;   /* spikes of the grid step in progress */
+  int kind;                          /* 0 cable, 1 LIF, 2 spike source (R20) */
+  double t_last, t_ref_end;          /* LIF: time V refers to; end of the refractory period */
+  int64_t src_cur;                   /* source: next scheduled spike */
   int spike_overflow;                /* a ninth spike in one grid step: orc_advance reports it, nothing is dropped silently */
   int64_t substeps;
 } cell_t;
@@ -121,6 +124,8 @@ struct orc_model {
   /* copies of the description */
   int32_t* parent; double *area, *cm, *rax, *gna, *gk, *gl, *pg, *pe;
   double ena, ek, el, theta;
+  double *lif_tau_m, *lif_v_th, *lif_c_m, *lif_e_l, *lif_e_r, *lif_t_ref;
+  int64_t* src_off; double* src_time;
   int32_t* syn_cv; double *syn_tau, *syn_e;
   double *cl_t0, *cl_t1, *cl_amp; int32_t* cl_cv;
   int64_t *out_off, *out_k;      /* connections grouped by source, ascending k inside a group */
@@ -296,6 +301,38 @@ static void cell_interval(orc_model* M, cell_t* c, double ta, double tb, double 
   }
 }
 
+/* Leaky integrate-and-fire cell (PAPER.md:170 names the kind only; reading R20): between events the membrane
+ * potential relaxes exactly, V(t) = E_L + (V(t_last) - E_L) exp(-(t - t_last)/tau_m); an event of weight w (a charge,
+ * pC = nA ms; C_m in nF) adds w / C_m [mV] to V; V >= V_th at an event emits a spike AT the event time,
+ * V <- E_R, and events are ignored for t_ref, after which relaxation resumes from E_R.  Event-driven and exact: the
+ * time grid plays no role.  Events with time < tb are processed in the grid interval that ends at tb. */
+static void lif_interval(orc_model* M, cell_t* c, int64_t ci, double tb) {
+  double* v = M->v + c->cv0;
+  while (c->qh < c->qn && c->q[c->qh].t < tb) {
+    const double te = c->q[c->qh].t, w = c->q[c->qh].w;
+    c->qh++;
+    if (te < c->t_ref_end) continue;                          /* refractory: the event is lost */
+    v[0] = M->lif_e_l[ci] + (v[0] - M->lif_e_l[ci]) * exp(-(te - c->t_last) / M->lif_tau_m[ci]);
+    c->t_last = te;
+    v[0] += w / M->lif_c_m[ci];
+    if (v[0] >= M->lif_v_th[ci]) {
+      if (c->n_new < 8) c->new_spikes[c->n_new++] = te; else c->spike_overflow = 1;
+      v[0] = M->lif_e_r[ci];
+      c->t_ref_end = te + M->lif_t_ref[ci];
+      c->t_last = c->t_ref_end;
+    }
+    c->substeps++;
+  }
+}
+
+/* Spike source ("artificial spike sources"; R20): emits its schedule, times in [ta, tb). */
+static void source_interval(orc_model* M, cell_t* c, int64_t ci, double tb) {
+  while (c->src_cur < M->src_off[ci + 1] && M->src_time[c->src_cur] < tb) {
+    if (c->n_new < 8) c->new_spikes[c->n_new++] = M->src_time[c->src_cur]; else c->spike_overflow = 1;
+    c->src_cur++;
+  }
+}
+
 /* ------------------------------------------------------------------------------------------ */
 static void* dup_arr(const void* p, size_t bytes) {
   if (!p) return NULL;
@@ -380,6 +417,15 @@ int orc_create(const orc_desc* D, orc_model** out) {
   M->conn_syn = (int32_t*)dup_arr(D->conn_syn, (size_t)D->n_conn * 4);
   M->conn_delay = (double*)dup_arr(D->conn_delay, (size_t)D->n_conn * 8);
   M->conn_w = (double*)dup_arr(D->conn_weight, (size_t)D->n_conn * 8);
+  if (D->cell_kind) {
+    M->lif_tau_m = (double*)dup_arr(D->lif_tau_m, (size_t)nc * 8); M->lif_v_th = (double*)dup_arr(D->lif_v_th, (size_t)nc * 8);
+    M->lif_c_m = (double*)dup_arr(D->lif_c_m, (size_t)nc * 8); M->lif_e_l = (double*)dup_arr(D->lif_e_l, (size_t)nc * 8);
+    M->lif_e_r = (double*)dup_arr(D->lif_e_r, (size_t)nc * 8); M->lif_t_ref = (double*)dup_arr(D->lif_t_ref, (size_t)nc * 8);
+    if (D->src_off) {
+      M->src_off = (int64_t*)dup_arr(D->src_off, (size_t)(nc + 1) * 8);
+      M->src_time = (double*)dup_arr(D->src_time, (size_t)D->src_off[nc] * 8);
+    }
+  }
   M->v = (double*)calloc((size_t)ncv + 1, 8); M->m = (double*)calloc((size_t)ncv + 1, 8);
   M->h = (double*)calloc((size_t)ncv + 1, 8); M->nn = (double*)calloc((size_t)ncv + 1, 8);
   M->g = (double*)calloc((size_t)nsyn + 1, 8);
@@ -410,6 +456,13 @@ int orc_create(const orc_desc* D, orc_model** out) {
     ce->syn0 = D->syn_off ? D->syn_off[c] : 0; ce->ns = D->syn_off ? D->syn_off[c + 1] - D->syn_off[c] : 0;
     ce->det = D->det_cv ? D->det_cv[c] : 0;
     ce->armed = 1; ce->v_prev = M->v[ce->cv0 + ce->det];
+    ce->kind = D->cell_kind ? D->cell_kind[c] : 0;
+    ce->t_last = 0.0; ce->t_ref_end = -INFINITY;
+    ce->src_cur = (ce->kind == 2 && M->src_off) ? M->src_off[c] : 0;
+    if (ce->kind == 1 && (!D->lif_tau_m || !(D->lif_tau_m[c] > 0) || !(D->lif_c_m[c] > 0) || !(D->lif_t_ref[c] >= 0))) {
+      orc_destroy(M); FAIL(-2, "bad LIF parameters"); }
+    if (ce->kind != 0 && ce->n != 1) { orc_destroy(M); FAIL(-2, "a LIF / source cell owns exactly one control volume"); }
+    if (ce->kind == 2 && !M->src_off) { orc_destroy(M); FAIL(-2, "spike sources need a schedule"); }
     ce->clamps = (int64_t*)calloc((size_t)ncl[c] + 1, 8);
   }
   for (int64_t k = 0; k < D->n_clamp; ++k) { cell_t* ce = &M->cells[D->clamp_cell[k]]; ce->clamps[ce->n_clamps++] = k; }
@@ -463,7 +516,9 @@ int orc_advance(orc_model* M, double t_end, double dt) {
 #endif
     for (int64_t c = 0; c < M->n_cells; ++c) {
       M->cells[c].n_new = 0;
-      cell_interval(M, &M->cells[c], ta, tb, dt, nominal);
+      if (M->cells[c].kind == 0) cell_interval(M, &M->cells[c], ta, tb, dt, nominal);
+      else if (M->cells[c].kind == 1) lif_interval(M, &M->cells[c], c, tb);
+      else source_interval(M, &M->cells[c], c, tb);
     }
     for (int64_t c = 0; c < M->n_cells; ++c)
       if (M->cells[c].spike_overflow) FAIL(-6, "cell %lld fired more than 8 spikes in one grid step", (long long)c);
@@ -509,6 +564,11 @@ int orc_voltage(orc_model* M, double* out, int64_t n_cv) {
   if (!M || !out) FAIL(-1, "null argument");
   if (n_cv != M->n_cv) FAIL(-2, "n_cv mismatch");
   memcpy(out, M->v, (size_t)n_cv * 8);
+  for (int64_t c = 0; c < M->n_cells; ++c) {                  /* LIF: the potential relaxed to the current time */
+    const cell_t* ce = &M->cells[c];
+    if (ce->kind == 1 && M->t > ce->t_last)
+      out[ce->cv0] = M->lif_e_l[c] + (M->v[ce->cv0] - M->lif_e_l[c]) * exp(-(M->t - ce->t_last) / M->lif_tau_m[c]);
+  }
   return 0;
 }
 
@@ -548,7 +608,10 @@ int orc_set_state(orc_model* M, const double* v, const double* hm, const double*
   if (hh) memcpy(M->h, hh, (size_t)M->n_cv * 8);
   if (hn) memcpy(M->nn, hn, (size_t)M->n_cv * 8);
   if (syn_g) memcpy(M->g, syn_g, (size_t)M->n_syn * 8);
-  for (int64_t c = 0; c < M->n_cells; ++c) { M->cells[c].v_prev = M->v[M->cells[c].cv0 + M->cells[c].det]; M->cells[c].armed = 1; }
+  for (int64_t c = 0; c < M->n_cells; ++c) {
+    M->cells[c].v_prev = M->v[M->cells[c].cv0 + M->cells[c].det]; M->cells[c].armed = 1;
+    if (v && M->cells[c].kind == 1) { M->cells[c].t_last = M->t; M->cells[c].t_ref_end = -INFINITY; }   /* V given at the current time */
+  }
   return 0;
 }
 
@@ -565,6 +628,8 @@ void orc_destroy(orc_model* M) {
   free(M->pg); free(M->pe); free(M->syn_cv); free(M->syn_tau); free(M->syn_e); free(M->cl_cv);
   free(M->cl_t0); free(M->cl_t1); free(M->cl_amp); free(M->conn_dst); free(M->conn_syn);
   free(M->conn_delay); free(M->conn_w); free(M->v); free(M->m); free(M->h); free(M->nn); free(M->g);
+  free(M->lif_tau_m); free(M->lif_v_th); free(M->lif_c_m); free(M->lif_e_l); free(M->lif_e_r); free(M->lif_t_ref);
+  free(M->src_off); free(M->src_time);
   free(M->scr); free(M->cells); free(M->out_off); free(M->out_k); free(M->sp_cell); free(M->sp_time);
   free(M);
 }

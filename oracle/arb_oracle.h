@@ -47,6 +47,14 @@ typedef struct {
   const int64_t* ext_cell;
   const int32_t* ext_syn;
   const double *ext_time, *ext_weight;
+  /* cell kinds other than the multi-compartment cell (reading R20):
+   * cell_kind[c] = 0 cable cell, 1 leaky integrate-and-fire cell, 2 spike source; NULL => all cable.
+   * A LIF / source cell still owns ONE control volume in the per-CV arrays (its area etc. are ignored; the CV's
+   * voltage is the LIF membrane potential, vinit its initial value) and its synapse range is its event targets. */
+  const int32_t* cell_kind;
+  const double *lif_tau_m, *lif_v_th, *lif_c_m, *lif_e_l, *lif_e_r, *lif_t_ref;   /* [n_cells]: ms, mV, nF, mV, mV, ms */
+  const int64_t* src_off;     /* [n_cells+1] spike schedule of every cell (empty unless it is a source) */
+  const double* src_time;     /* ascending inside a cell */
 } orc_desc;
 
 typedef struct orc_model orc_model;

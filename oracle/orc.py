@@ -46,6 +46,10 @@ class _Desc(C.Structure):
         ("conn_syn", C.c_void_p), ("conn_delay", C.c_void_p), ("conn_weight", C.c_void_p),
         ("n_ext", C.c_int64), ("ext_cell", C.c_void_p), ("ext_syn", C.c_void_p),
         ("ext_time", C.c_void_p), ("ext_weight", C.c_void_p),
+        ("cell_kind", C.c_void_p),
+        ("lif_tau_m", C.c_void_p), ("lif_v_th", C.c_void_p), ("lif_c_m", C.c_void_p), ("lif_e_l", C.c_void_p),
+        ("lif_e_r", C.c_void_p), ("lif_t_ref", C.c_void_p),
+        ("src_off", C.c_void_p), ("src_time", C.c_void_p),
     ]
 
 

@@ -126,6 +126,7 @@ _F64 = ("cv_area", "cv_cm", "cv_raxial", "cv_vinit", "hh_gnabar", "hh_gkbar", "h
         "conn_weight", "ext_time", "ext_weight")
 _I64 = ("cv_off", "syn_off", "clamp_cell", "conn_src", "conn_dst", "ext_cell")
 _I32 = ("cv_parent", "syn_cv", "clamp_cv", "det_cv", "conn_syn", "ext_syn")
+_LIF = ("lif_tau_m", "lif_v_th", "lif_c_m", "lif_e_l", "lif_e_r", "lif_t_ref")
 
 
 def finalize(m):
@@ -156,6 +157,17 @@ def finalize(m):
     for k in _I32:
         if m[k] is not None:
             m[k] = np.ascontiguousarray(m[k], dtype=np.int32)
+    # cell kinds: None = every cell is a multi-compartment cell
+    if m.get("cell_kind") is None:
+        m["cell_kind"] = None
+        for k in _LIF + ("src_off", "src_time"):
+            m[k] = None
+    else:
+        m["cell_kind"] = np.ascontiguousarray(m["cell_kind"], dtype=np.int32)
+        for k in _LIF:
+            m[k] = np.ascontiguousarray(m[k] if m.get(k) is not None else np.ones(n_cells), dtype=np.float64)
+        m["src_off"] = np.ascontiguousarray(m["src_off"] if m.get("src_off") is not None else np.zeros(n_cells + 1), dtype=np.int64)
+        m["src_time"] = np.ascontiguousarray(m["src_time"] if m.get("src_time") is not None else np.zeros(0), dtype=np.float64)
     m["n_cv"] = int(m["cv_off"][-1])
     m["n_syn"] = int(m["syn_off"][-1])
     m["n_clamp"] = len(m["clamp_cell"])
@@ -392,6 +404,64 @@ def paper_ring(n_cells=1024, n_syn=10000, t_end=200.0, weight=0.05, kick_weight=
 
 def config(k, **kw):
     return (config0, config1, config2, config3, config4)[k](**kw)
+
+
+# ----------------------------------------------------------------------------------------------
+# other cell kinds: LIF cells and spike sources beside cable cells
+# ----------------------------------------------------------------------------------------------
+LIF_DEFAULTS = dict(lif_tau_m=10.0, lif_v_th=-50.0, lif_c_m=0.25, lif_e_l=-65.0, lif_e_r=-70.0, lif_t_ref=2.0)
+
+
+def mixed_network(seed=0, n_cable=6, n_lif=8, n_src=4, t_end=60.0, rate_hz=60.0, n_in=4):
+    """A small network of all three cell kinds: Poisson spike sources drive LIF cells and cable cells (configs[1]
+    morphologies), LIF cells and cable cells project onto each other.  Cells are numbered sources, LIF, cable.
+    A LIF / source cell owns one (unused) control volume; a LIF cell's events target its synapse range (n_in
+    targets), an event's weight is a charge [pC] for LIF cells and a conductance [uS] for cable cells."""
+    rng = np.random.default_rng([BASE_SEED, 99, seed])
+    cab, _ = _homogeneous(1, n_cable, 15, 20, n_in, t_end)
+    n_cells = n_src + n_lif + n_cable
+    n_other = n_src + n_lif
+    ncv_c = int(cab["cv_off"][1])
+    off = np.concatenate([np.arange(n_other + 1), n_other + cab["cv_off"][1:]])
+    one = lambda v, arr: np.concatenate([np.full(n_other, v), arr])
+    m = dict(n_cells=n_cells, cv_off=off, cv_parent=np.concatenate([np.full(n_other, -1, np.int32), cab["cv_parent"]]),
+             cv_area=one(100.0, cab["cv_area"]), cv_cm=one(1.0, cab["cv_cm"]), cv_raxial=one(1.0, cab["cv_raxial"]),
+             cv_vinit=one(-65.0, np.full(n_cable * ncv_c, -65.0)),
+             hh_gnabar=one(0.0, cab["hh_gnabar"]), hh_gkbar=one(0.0, cab["hh_gkbar"]), hh_gl=one(0.0, cab["hh_gl"]),
+             pas_g=one(0.0, cab["pas_g"]), pas_e=one(-65.0, cab["pas_e"]),
+             syn_off=np.concatenate([np.zeros(n_src + 1, np.int64), np.arange(1, n_lif + n_cable + 1) * n_in]),
+             syn_cv=np.concatenate([np.zeros(n_lif * n_in, np.int32), np.zeros(n_cable * n_in, np.int32)]),
+             syn_tau=np.full((n_lif + n_cable) * n_in, SYN_TAU), syn_e=np.full((n_lif + n_cable) * n_in, SYN_E),
+             cell_kind=np.concatenate([np.full(n_src, 2), np.full(n_lif, 1), np.zeros(n_cable)]).astype(np.int32),
+             t_end=t_end, name="mixed network %d+%d+%d" % (n_src, n_lif, n_cable))
+    for k, v in LIF_DEFAULTS.items():
+        m[k] = np.full(n_cells, v) * (1.0 if k != "lif_tau_m" else 1.0) + (rng.uniform(-0.5, 0.5, n_cells) if k == "lif_tau_m" else 0.0)
+    # Poisson schedules of the sources
+    times, soff = [], [0]
+    for c in range(n_cells):
+        if c < n_src:
+            k = int(rng.poisson(rate_hz * t_end * 1e-3))
+            times.append(np.sort(rng.uniform(0.0, t_end, k)))
+        else:
+            times.append(np.zeros(0))
+        soff.append(soff[-1] + len(times[-1]))
+    m["src_off"], m["src_time"] = np.array(soff), np.concatenate(times)
+    # connections: target synapse j of every LIF / cable cell gets one source: sources and LIF cells drive everybody
+    src, dst, syn, dly, w = [], [], [], [], []
+    for c in range(n_src, n_cells):
+        for j in range(n_in):
+            s = int(rng.integers(0, n_other))
+            if s == c:
+                s = (s + 1) % n_other
+            src.append(s), dst.append(c), syn.append(j), dly.append(float(rng.uniform(1.0, 4.0)))
+            w.append(float(rng.uniform(1.5, 3.0)) if c < n_other else float(rng.uniform(0.005, 0.02)))
+    # cable cells project back onto the LIF cells
+    for c in range(n_other, n_cells):
+        for j in range(2):
+            src.append(c), dst.append(int(rng.integers(n_src, n_other))), syn.append(int(rng.integers(0, n_in)))
+            dly.append(float(rng.uniform(1.0, 4.0))), w.append(float(rng.uniform(2.0, 4.0)))
+    m.update(conn_src=src, conn_dst=dst, conn_syn=syn, conn_delay=dly, conn_weight=w)
+    return finalize(m)
 
 
 # ----------------------------------------------------------------------------------------------

@@ -777,3 +777,88 @@ def test_l4_linearised_converges_to_the_same_ode(orc):
     o = _lin(orc, W.config0())
     o.advance(100.0, 1.0)
     assert np.all(np.isfinite(o.voltage())) and np.all(np.abs(o.voltage()) < 200.0)
+
+
+# ---------------------------------------------------------------------------------------------
+# K1-K3 other cell kinds (reading R20): LIF cells and spike sources
+# ---------------------------------------------------------------------------------------------
+def _lif_net(ev_t, ev_w, t_end=50.0, **par):
+    p = dict(W.LIF_DEFAULTS)
+    p.update(par)
+    m = dict(n_cells=1, cv_off=[0, 1], cv_parent=[-1], cv_area=[100.0], cv_cm=[1.0], cv_raxial=[1.0], cv_vinit=[p["lif_e_l"]],
+             syn_off=[0, 1], syn_cv=[0], syn_tau=[2.0], syn_e=[0.0], cell_kind=[1],
+             ext_cell=np.zeros(len(ev_t), np.int64), ext_syn=np.zeros(len(ev_t), np.int32), ext_time=ev_t, ext_weight=ev_w, t_end=t_end)
+    for k, v in p.items():
+        m[k] = [v]
+    return W.finalize(m)
+
+
+def test_k1_lif_closed_form_charging_spike_and_refractory(orc):
+    tau, vth, cm, el, er, tref = 10.0, -50.0, 0.25, -65.0, -70.0, 2.0
+    w, gap = 1.0, 1.3                                  # every event lifts V by w / C_m = 4 mV
+    t = 0.7 + gap * np.arange(30)
+    o = orc.Oracle(_lif_net(t, np.full(30, w), lif_tau_m=tau, lif_v_th=vth, lif_c_m=cm, lif_e_l=el, lif_e_r=er, lif_t_ref=tref))
+    q = np.exp(-gap / tau)
+    # geometric series until the threshold is reached
+    k_spike = next(k for k in range(1, 31) if el + (w / cm) * (1 - q ** k) / (1 - q) >= vth)
+    o.advance(t[k_spike - 2] + 0.01, DT)               # just after event k_spike - 1
+    want = el + (w / cm) * (1 - q ** (k_spike - 1)) / (1 - q)
+    assert o.voltage()[0] == pytest.approx(el + (want - el) * np.exp(-0.01 / tau), rel=1e-13)
+    o.advance(50.0, DT)
+    sc, st = o.spikes()
+    assert st[0] == t[k_spike - 1]                     # the spike sits exactly on the event that crossed the threshold
+    # events inside the refractory period are lost; charging restarts from E_R at st + t_ref
+    nxt = [x for x in t if x >= st[0] + tref]
+    v, tl = er, st[0] + tref
+    second = None
+    for x in nxt:
+        v = el + (v - el) * np.exp(-(x - tl) / tau) + w / cm
+        tl = x
+        if v >= vth:
+            second = x
+            break
+    assert second is not None and st[1] == second and len(st) >= 2
+    assert np.all(np.diff(st) >= tref)
+
+
+def test_k2_spike_sources_emit_their_schedule_and_drive_a_cable_cell(orc):
+    """A source cell's spikes are its schedule; a connection source -> cable cell delivers g += w at t + delay."""
+    sched = np.array([0.4, 3.3, 3.31, 7.0, 19.5])
+    m = dict(n_cells=2, cv_off=[0, 1, 2], cv_parent=[-1, -1], cv_area=[100.0, 400.0], cv_cm=[1.0, 1.0], cv_raxial=[1.0, 1.0],
+             pas_g=[0.0, 1e-4], pas_e=[-65.0, -65.0], syn_off=[0, 0, 1], syn_cv=[0], syn_tau=[3.0], syn_e=[0.0],
+             cell_kind=[2, 0], src_off=[0, 5, 5], src_time=sched,
+             conn_src=[0], conn_dst=[1], conn_syn=[0], conn_delay=[1.25], conn_weight=[0.0002], t_end=12.0)
+    m = W.finalize(m)
+    o = orc.Oracle(m)
+    o.advance(12.0, DT)
+    sc, st = o.spikes()
+    assert list(sc) == [0, 0, 0, 0] and np.array_equal(st, sched[:4])
+    g = sum(0.0002 * np.exp(-(12.0 - (s + 1.25)) / 3.0) for s in sched[:4])
+    assert o.syn_g()[0] == pytest.approx(g, rel=1e-13)
+    assert o.voltage()[1] > -65.0
+
+
+def test_k3_mixed_network_invariants(orc):
+    """Sources, LIF and cable cells in one network: sources fire their schedule, LIF spikes coincide with event times
+    (spike time - delay is a spike of a presynaptic cell), refractory gaps hold, results do not depend on threads."""
+    m = W.mixed_network()
+    o = orc.Oracle(m)
+    o.advance(60.0, m["dt"])
+    sc, st = o.spikes()
+    kind = m["cell_kind"]
+    for c in np.flatnonzero(kind == 2):
+        a, b = m["src_off"][c], m["src_off"][c + 1]
+        assert np.array_equal(np.sort(st[sc == c]), m["src_time"][a:b][m["src_time"][a:b] < 60.0])
+    n_lif_spikes = 0
+    for c in np.flatnonzero(kind == 1):
+        mine = np.sort(st[sc == c])
+        n_lif_spikes += len(mine)
+        assert np.all(np.diff(mine) >= m["lif_t_ref"][c])
+        pre = np.flatnonzero(m["conn_dst"] == c)
+        arrivals = np.concatenate([st[sc == m["conn_src"][k]] + m["conn_delay"][k] for k in pre])
+        for x in mine:
+            assert np.min(np.abs(arrivals - x)) < 1e-12
+    assert n_lif_spikes > 20 and np.count_nonzero(kind[sc] == 0) > 3
+    o2 = orc.Oracle(m, threads=4)
+    o2.advance(60.0, m["dt"])
+    assert np.array_equal(o2.voltage(), o.voltage()) and np.array_equal(o2.spikes()[1], st)
