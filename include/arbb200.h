@@ -140,6 +140,19 @@ typedef struct {
    * shard_n_global cells; conn_dst stay local, conn_src are GLOBAL cell ids (the table holds every connection
    * whose destination is local); spikes of remote sources arrive through arb_apply_spike_blocks.           */
   int64_t shard_gid_base, shard_n_global;
+  /* Cell kinds other than the multi-compartment cell ("leaky integrate and fire cells and cells
+   * representing artificial spike sources"; the paper names them only, reading R20).
+   * cell_kind[c]: 0 = multi-compartment cell, 1 = LIF cell, 2 = spike source; NULL => all 0.
+   * A LIF / source cell owns exactly ONE control volume in the per-CV arrays (its geometry is ignored; the CV's
+   * voltage is the LIF membrane potential, cv_vinit its initial value) and its synapse range is its event targets.
+   * LIF (event-driven, exact): V relaxes to lif_e_l with lif_tau_m; an event of weight w (a charge, pC) adds
+   * w / lif_c_m; V >= lif_v_th at an event emits a spike AT the event time, V <- lif_e_r, events are ignored for
+   * lif_t_ref.  Spike source: emits the times src_time[src_off[c] .. src_off[c+1]) (ascending).
+   * The lif_* arrays are [n_cells] (read for LIF cells only); src_off is [n_cells+1]; all NULL when cell_kind is. */
+  const int32_t* cell_kind;
+  const double *lif_tau_m, *lif_v_th, *lif_c_m, *lif_e_l, *lif_e_r, *lif_t_ref; /* ms, mV, nF, mV, mV, ms */
+  const int64_t* src_off;
+  const double* src_time;
 } arb_desc;
 
 typedef struct arb_model arb_model; /* opaque; lives in host memory, owned by the library */
@@ -221,6 +234,18 @@ int arb_set_state(arb_model* m, const double* v, const double* hh_m, const doubl
                   const double* hh_n, const double* syn_g);
 
 int arb_set_option(arb_model* m, int key, int64_t value);
+
+/* The mechanism catalogue (mechanisms and cell kinds "are referenced by name").  The library's
+ * mechanisms are hand-written kernels; the catalogue is the table that names them, their kind and their parameters
+ * (the arb_desc fields that carry them), so that a front end can look a mechanism up instead of hard-coding fields.
+ * arb_catalogue_size: entries.  arb_catalogue_entry: name ("hh", "pas", "expsyn", "iclamp", "lif", "spike_source"),
+ * kind (0 density mechanism, 1 point mechanism, 2 cell kind), number of parameters; returns ARB_E_INVALID beyond the
+ * table.  arb_catalogue_param: name of the arb_desc field, unit and default value of one parameter.
+ * arb_catalogue_find: index of a name, or -1. */
+int arb_catalogue_size(void);
+int arb_catalogue_entry(int index, const char** name, int* kind, int* n_params);
+int arb_catalogue_param(int index, int param, const char** field, const char** unit, double* default_value);
+int arb_catalogue_find(const char* name);
 
 /* Measures the fp64 fused-multiply-add rate of the current device (independent DFMA chains in
  * registers, no memory traffic; kernel timed with CUDA events on `cuda_stream`, NULL = default

@@ -321,7 +321,6 @@ static void lif_interval(orc_model* M, cell_t* c, int64_t ci, double tb) {
       c->t_ref_end = te + M->lif_t_ref[ci];
       c->t_last = c->t_ref_end;
     }
-    c->substeps++;
   }
 }
 

@@ -17,7 +17,7 @@ ARB_OPT_FUSED_STEPS, ARB_OPT_EPOCH_STEPS, ARB_OPT_TIMING, ARB_OPT_OVERLAP, ARB_O
 ARB_OPT_LINEARISED = 8
 
 EXPORTS = ("arb_plan", "arb_create", "arb_advance", "arb_spikes", "arb_clear_spikes", "arb_spike_block", "arb_apply_spike_blocks",
-           "arb_voltage", "arb_probe",
+           "arb_voltage", "arb_probe", "arb_catalogue_size", "arb_catalogue_entry", "arb_catalogue_param", "arb_catalogue_find",
            "arb_set_state", "arb_set_option", "arb_fp64_peak", "arb_destroy", "arb_last_error")
 
 # arb_desc's layout / capacity options (0 = library default).  A workloads dict may carry them under the
@@ -52,6 +52,10 @@ class arb_desc(C.Structure):
         ("layout_group_min_cells", C.c_int64), ("layout_forest_cv", C.c_int64),
         ("cap_spikes", C.c_int64), ("cap_events", C.c_int64),
         ("shard_gid_base", C.c_int64), ("shard_n_global", C.c_int64),
+        ("cell_kind", C.c_void_p),
+        ("lif_tau_m", C.c_void_p), ("lif_v_th", C.c_void_p), ("lif_c_m", C.c_void_p), ("lif_e_l", C.c_void_p),
+        ("lif_e_r", C.c_void_p), ("lif_t_ref", C.c_void_p),
+        ("src_off", C.c_void_p), ("src_time", C.c_void_p),
     ]
 
 
@@ -76,6 +80,9 @@ def lib():
         L.arb_set_state.argtypes = [C.c_void_p] * 6
         L.arb_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
         L.arb_clear_spikes.argtypes = [C.c_void_p]
+        L.arb_catalogue_entry.argtypes = [C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_int), C.POINTER(C.c_int)]
+        L.arb_catalogue_param.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_char_p), C.POINTER(C.c_double)]
+        L.arb_catalogue_find.argtypes = [C.c_char_p]
         L.arb_spike_block.restype = C.c_int64
         L.arb_spike_block.argtypes = [C.c_void_p, C.c_void_p, C.c_int64]
         L.arb_apply_spike_blocks.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64]
@@ -115,6 +122,21 @@ def arb_fp64_peak(stream=None):
     if rc:
         raise ArbError(rc, "arb_fp64_peak failed")
     return r.value, ms.value
+
+
+def catalogue():
+    """The library's mechanism catalogue as {name: (kind, [(arb_desc field, unit, default), ...])}."""
+    L, out = lib(), {}
+    for i in range(L.arb_catalogue_size()):
+        name, kind, n = C.c_char_p(), C.c_int(), C.c_int()
+        L.arb_catalogue_entry(i, C.byref(name), C.byref(kind), C.byref(n))
+        ps = []
+        for j in range(n.value):
+            f, u, d = C.c_char_p(), C.c_char_p(), C.c_double()
+            L.arb_catalogue_param(i, j, C.byref(f), C.byref(u), C.byref(d))
+            ps.append((f.value.decode(), u.value.decode(), d.value))
+        out[name.value.decode()] = (kind.value, ps)
+    return out
 
 
 def arb_plan(m):

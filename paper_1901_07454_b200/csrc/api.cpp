@@ -35,7 +35,7 @@ struct Regions {
   Region units, gdescs, ghot, ghotflag, gen, fast, state, topo, scratch, factor_dcontrib, cell_rt_idx, cell_orig, ev_off, ev_t, ev_gidx, ev_w, ev_fill,
       ext_off, ext_t, ext_gidx, ext_w, ext_cur, conn_off, conn_dst, conn_gidx, conn_delay, conn_w,
       pool_t[2], pool_dst[2], pool_gidx[2], pool_w[2], spike_cell, spike_t, counters, scan_tmp,
-      cv_idx, syn_idx, hh_m_idx, hh_stride, hh_cv, io;
+      cv_idx, syn_idx, hh_m_idx, hh_stride, hh_cv, io, pc_kind, pc_par, pc_src_off, pc_src_time, pc_cv;
   size_t total = 0;
 };
 
@@ -104,6 +104,11 @@ Regions carve(const HostModel& H, const Caps& cap) {
   R.hh_stride = C.take(4 * (size_t)H.n_hh);
   R.hh_cv = C.take(4 * (size_t)H.n_hh);
   R.io = C.take(8 * (size_t)std::max<int64_t>(std::max(H.n_cv, H.n_syn), 16));
+  R.pc_kind = C.take(4 * (size_t)H.n_pcells);
+  R.pc_par = C.take(48 * (size_t)H.n_pcells);
+  R.pc_src_off = C.take(4 * ((size_t)H.n_pcells + 1));
+  R.pc_src_time = C.take(8 * (size_t)H.n_sched);
+  R.pc_cv = C.take(4 * (size_t)H.n_pcells);
   R.total = C.pos;
   return R;
 }
@@ -258,6 +263,9 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     if ((e = upload(m, R.hh_m_idx, H.hh_m_idx)) != cudaSuccess) return bail(e, "upload hh map");
     if ((e = upload(m, R.hh_stride, H.hh_stride)) != cudaSuccess) return bail(e, "upload hh map");
     if ((e = upload(m, R.hh_cv, H.hh_cv)) != cudaSuccess) return bail(e, "upload hh map");
+    if ((e = upload(m, R.pc_kind, H.pc_kind)) != cudaSuccess || (e = upload(m, R.pc_par, H.pc_par)) != cudaSuccess ||
+        (e = upload(m, R.pc_src_off, H.pc_src_off)) != cudaSuccess || (e = upload(m, R.pc_src_time, H.pc_src_time)) != cudaSuccess ||
+        (e = upload(m, R.pc_cv, H.pc_cv)) != cudaSuccess) return bail(e, "upload point cells");
     DevModel& D = m->D;
     std::memset(&D, 0, sizeof D);
     D.units = at<UnitDesc>(m, R.units);
@@ -274,6 +282,9 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     D.conn_off = at<uint32_t>(m, R.conn_off); D.conn_dst = at<uint32_t>(m, R.conn_dst); D.conn_gidx = at<uint32_t>(m, R.conn_gidx);
     D.conn_delay = at<double>(m, R.conn_delay); D.conn_w = at<double>(m, R.conn_w);
     D.gid_base = H.gid_base;
+    D.n_pcells = H.n_pcells; D.pc_first = H.pc_first; D.pc_state_base = H.pc_state_base;
+    D.pc_kind = at<int32_t>(m, R.pc_kind); D.pc_par = at<double>(m, R.pc_par); D.pc_src_off = at<uint32_t>(m, R.pc_src_off);
+    D.pc_src_time = at<double>(m, R.pc_src_time); D.pc_cv = at<uint32_t>(m, R.pc_cv);
     for (int i = 0; i < 2; ++i) {
       D.pool[i].t = at<double>(m, R.pool_t[i]); D.pool[i].dst = at<uint32_t>(m, R.pool_dst[i]);
       D.pool[i].gidx = at<uint32_t>(m, R.pool_gidx[i]); D.pool[i].w = at<double>(m, R.pool_w[i]);
@@ -458,6 +469,7 @@ int arb_advance(arb_model* m, double t_end, double dt) {
     int l0 = launches;
     CUB(stamp());
     CUB(launch_build_events(D, m->cur_pool, t_win, m->stream, &launches));
+    CUB(launch_point_cells(D, t_win, m->stream, &launches));
     m->cur_pool ^= 1;
     CUB(stamp());
     int l1 = launches;
@@ -583,6 +595,7 @@ int arb_voltage(arb_model* m, double* out, int64_t n_cv) {
   if (n_cv != m->H.n_cv) return fail(m, ARB_E_INVALID, "arb_voltage: n_cv mismatch");
   double* io = at<double>(m, m->R.io);
   CU(m, launch_gather(m->D.state, at<uint32_t>(m, m->R.cv_idx), n_cv, io, m->stream));
+  CU(m, launch_lif_relax(m->D, m->t, io, m->stream));
   CU(m, cudaMemcpyAsync(out, io, 8 * (size_t)n_cv, cudaMemcpyDeviceToHost, m->stream));
   CU(m, cudaStreamSynchronize(m->stream));
   return ARB_OK;
@@ -670,6 +683,7 @@ int arb_set_state(arb_model* m, const double* v, const double* hh_m, const doubl
     CU(m, cudaStreamSynchronize(m->stream));
   }
   CU(m, launch_reset_detectors(m->D, m->stream));
+  if (v) CU(m, launch_point_reset(m->D, m->t, m->stream));
   CU(m, cudaStreamSynchronize(m->stream));
   return ARB_OK;
 }
@@ -696,6 +710,47 @@ int arb_set_option(arb_model* m, int key, int64_t value) {
       return ARB_OK;
   }
   return fail(m, ARB_E_INVALID, "arb_set_option: unknown key");
+}
+
+// ---- the mechanism catalogue: a table that names the hand-written mechanisms and cell kinds ----
+namespace {
+struct CatParam { const char* field; const char* unit; double def; };
+struct CatEntry { const char* name; int kind; int n; CatParam par[6]; };
+const CatEntry kCatalogue[] = {
+    {"hh", 0, 6, {{"hh_gnabar", "S/cm2", 0.12}, {"hh_gkbar", "S/cm2", 0.036}, {"hh_gl", "S/cm2", 3e-4}, {"hh_ena", "mV", 50.0},
+                  {"hh_ek", "mV", -77.0}, {"hh_el", "mV", -54.3}}},
+    {"pas", 0, 2, {{"pas_g", "S/cm2", 1e-5}, {"pas_e", "mV", -65.0}}},
+    {"expsyn", 1, 2, {{"syn_tau", "ms", 2.0}, {"syn_e", "mV", 0.0}}},
+    {"iclamp", 1, 3, {{"clamp_t0", "ms", 0.0}, {"clamp_t1", "ms", 0.0}, {"clamp_amp", "nA", 0.0}}},
+    {"lif", 2, 6, {{"lif_tau_m", "ms", 10.0}, {"lif_v_th", "mV", -50.0}, {"lif_c_m", "nF", 0.25}, {"lif_e_l", "mV", -65.0},
+                   {"lif_e_r", "mV", -70.0}, {"lif_t_ref", "ms", 2.0}}},
+    {"spike_source", 2, 1, {{"src_time", "ms", 0.0}}},
+};
+constexpr int kCatalogueSize = (int)(sizeof kCatalogue / sizeof kCatalogue[0]);
+}  // namespace
+
+int arb_catalogue_size(void) { return kCatalogueSize; }
+
+int arb_catalogue_entry(int index, const char** name, int* kind, int* n_params) {
+  if (index < 0 || index >= kCatalogueSize) return ARB_E_INVALID;
+  if (name) *name = kCatalogue[index].name;
+  if (kind) *kind = kCatalogue[index].kind;
+  if (n_params) *n_params = kCatalogue[index].n;
+  return ARB_OK;
+}
+
+int arb_catalogue_param(int index, int param, const char** field, const char** unit, double* default_value) {
+  if (index < 0 || index >= kCatalogueSize || param < 0 || param >= kCatalogue[index].n) return ARB_E_INVALID;
+  if (field) *field = kCatalogue[index].par[param].field;
+  if (unit) *unit = kCatalogue[index].par[param].unit;
+  if (default_value) *default_value = kCatalogue[index].par[param].def;
+  return ARB_OK;
+}
+
+int arb_catalogue_find(const char* name) {
+  if (!name) return -1;
+  for (int i = 0; i < kCatalogueSize; ++i) if (std::strcmp(name, kCatalogue[i].name) == 0) return i;
+  return -1;
 }
 
 void arb_destroy(arb_model* m) {

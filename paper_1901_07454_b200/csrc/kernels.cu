@@ -20,6 +20,7 @@ namespace arbb {
 
 namespace {
 
+constexpr int kPcRecord = 8;         // doubles of a point cell's record (layout.hpp: kPcDoubles)
 constexpr int kBlockThreads = 128;              // cable_block_kernel, factor_kernel, init_kernel
 constexpr int kBlockWarps = kBlockThreads / 32;
 constexpr uint32_t kSynKeyReduceMin = 1024;     // block units with at least this many synapses reduce currents by key
@@ -789,6 +790,73 @@ __global__ void pool_swap_kernel(DevModel M) {
 }
 
 // ------------------------------------------------------------------------------------------
+// Point cells (reading R20), one thread per cell, once per epoch: a LIF cell walks its
+// epoch's events (time-sorted) - exact relaxation between events, V += w / C_m, spike AT the event that reaches
+// the threshold, reset, refractory period; a spike source emits its schedule.
+// Record in the state pool: V | runtime triple | t_last | t_ref_end | schedule cursor | pad.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void emit_spike(const DevModel& M, int64_t internal, double t) {
+  const unsigned long long pos = atomicAdd(&M.counters[CNT_SPIKES], 1ull);
+  if ((int64_t)pos < M.spike_cap) { M.spike_cell[pos] = M.cell_orig[internal]; M.spike_t[pos] = t; }
+  else atomicOr(&M.counters[CNT_ERROR], 1ull);
+}
+
+__global__ void __launch_bounds__(128) point_cells_kernel(DevModel M, double t_win) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= M.n_pcells) return;
+  double* st = M.state + M.pc_state_base + kPcRecord * i;
+  const unsigned long long pk = (unsigned long long)__double_as_longlong(st[2]);
+  uint32_t cur = (uint32_t)pk;
+  const uint32_t end = (uint32_t)(pk >> 32);
+  unsigned n_del = 0;
+  if (M.pc_kind[i] == 1) {
+    const double* par = M.pc_par + 6 * i;
+    const double tau = par[0], vth = par[1], cm = par[2], el = par[3], er = par[4], tref = par[5];
+    double v = st[0], tl = st[4], tre = st[5];
+    for (; cur < end; ++cur) {
+      const double te = M.ev_t[cur];
+      ++n_del;
+      if (te < tre) continue;                              // refractory: the event is lost
+      v = el + (v - el) * exp(-(te - tl) / tau);
+      tl = te;
+      v += M.ev_w[cur] / cm;
+      if (v >= vth) {
+        emit_spike(M, M.pc_first + i, te);
+        v = er; tre = te + tref; tl = tre;
+      }
+    }
+    st[0] = v; st[4] = tl; st[5] = tre;
+  } else {
+    uint32_t q = M.pc_src_off[i] + (uint32_t)st[6];
+    const uint32_t qe = M.pc_src_off[i + 1];
+    for (; q < qe && M.pc_src_time[q] < t_win; ++q) emit_spike(M, M.pc_first + i, M.pc_src_time[q]);
+    st[6] = (double)(q - M.pc_src_off[i]);
+    n_del = end - cur;                                     // events on a source have no effect
+    cur = end;
+  }
+  st[1] = CUDART_INF;
+  st[2] = __longlong_as_double((long long)(((unsigned long long)end << 32) | cur));
+  if (n_del) atomicAdd(&M.counters[CNT_DELIVERED], (unsigned long long)n_del);
+}
+
+// arb_voltage: a LIF cell's potential relaxed from the time of its last event to the current time
+__global__ void lif_relax_kernel(DevModel M, double t, double* io) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= M.n_pcells || M.pc_kind[i] != 1) return;
+  const double* st = M.state + M.pc_state_base + kPcRecord * i;
+  const double* par = M.pc_par + 6 * i;
+  if (t > st[4]) io[M.pc_cv[i]] = par[3] + (st[0] - par[3]) * exp(-(t - st[4]) / par[0]);
+}
+
+// arb_set_state: the injected V of a LIF cell is its potential at the current time, outside any refractory period
+__global__ void point_reset_kernel(DevModel M, double t) {
+  const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= M.n_pcells) return;
+  double* st = M.state + M.pc_state_base + kPcRecord * i;
+  st[4] = t; st[5] = -CUDART_INF;
+}
+
+// ------------------------------------------------------------------------------------------
 // read-back / state injection helpers
 // ------------------------------------------------------------------------------------------
 __global__ void gather_kernel(const double* state, const uint32_t* idx, int64_t n, double* out) {
@@ -879,6 +947,23 @@ cudaError_t launch_remote_spikes_to_events(const DevModel& M, int cur, const uns
                                            int64_t own, cudaStream_t s) {
   remote_spikes_to_events_kernel<<<(unsigned)(2 * M.sm_count), 256, 0, s>>>(M, cur, blocks, n_blocks, cap, own);
   spikes_done_kernel<<<1, 1, 0, s>>>(M);            // records the pool demand and clamps the counter
+  return cudaGetLastError();
+}
+
+cudaError_t launch_point_cells(const DevModel& M, double t_win, cudaStream_t s, int* launches) {
+  if (M.n_pcells == 0) return cudaSuccess;
+  point_cells_kernel<<<grid_for(M.n_pcells, 128), 128, 0, s>>>(M, t_win);
+  if (launches) ++*launches;
+  return cudaGetLastError();
+}
+cudaError_t launch_lif_relax(const DevModel& M, double t, double* io, cudaStream_t s) {
+  if (M.n_pcells == 0) return cudaSuccess;
+  lif_relax_kernel<<<grid_for(M.n_pcells, 128), 128, 0, s>>>(M, t, io);
+  return cudaGetLastError();
+}
+cudaError_t launch_point_reset(const DevModel& M, double t, cudaStream_t s) {
+  if (M.n_pcells == 0) return cudaSuccess;
+  point_reset_kernel<<<grid_for(M.n_pcells, 128), 128, 0, s>>>(M, t);
   return cudaGetLastError();
 }
 

@@ -69,6 +69,9 @@ struct DevModel {
   int64_t n_groups;
   GroupSmemPlan gplan;
   int l2_prefetch;            // group kernel: TMA-prefetch the next group's records into L2
+  // point cells (LIF cells, spike sources): the last n_pcells cells of the internal order
+  int64_t n_pcells, pc_first, pc_state_base;
+  const int32_t* pc_kind; const double* pc_par; const uint32_t* pc_src_off; const double* pc_src_time; const uint32_t* pc_cv;
   int sm_count;               // SMs of the device the model lives on (grid sizing)
   int linearised;             // ARB_OPT_LINEARISED: conductance-linearised step
   uint32_t* ghot;             // group kernel: three lists of n_groups entries (see CNT_HOT0)
@@ -108,6 +111,10 @@ cudaError_t launch_gather_hh(const double* state, const uint32_t* m_idx, const u
 cudaError_t launch_scatter_hh(double* state, const uint32_t* m_idx, const uint32_t* stride, const uint32_t* cv,
                               int which, int64_t n_hh, const double* in, cudaStream_t s);
 cudaError_t launch_reset_detectors(const DevModel& M, cudaStream_t s);
+// point cells: one epoch (events before t_win, scheduled spikes before t_win); read-back / state injection helpers
+cudaError_t launch_point_cells(const DevModel& M, double t_win, cudaStream_t s, int* launches);
+cudaError_t launch_lif_relax(const DevModel& M, double t, double* io, cudaStream_t s);
+cudaError_t launch_point_reset(const DevModel& M, double t, cudaStream_t s);
 // cell groups (group_kernel.cu)
 cudaError_t launch_group_factor(const DevModel& M, double dt, uint32_t seg_cap, cudaStream_t s);
 cudaError_t launch_group_init(const DevModel& M, cudaStream_t s);

@@ -109,6 +109,24 @@ int validate(const arb_desc& d, std::string& err) {
                                 "synapse CV out of range", "synapse tau must be > 0 and finite", "detector CV out of range"};
     return fail(ARB_E_INVALID, std::string(msg[bad.load()]) + " (cell " + std::to_string(bad_cell.load()) + ")");
   }
+  if (d.cell_kind) {
+    if (!d.lif_tau_m || !d.lif_v_th || !d.lif_c_m || !d.lif_e_l || !d.lif_e_r || !d.lif_t_ref || !d.src_off || (d.src_off[d.n_cells] > 0 && !d.src_time))
+      return fail(ARB_E_NULL, "cell_kind needs the lif_* arrays and src_off / src_time");
+    if (d.src_off[0] != 0) return fail(ARB_E_INVALID, "src_off[0] must be 0");
+    for (int64_t c = 0; c < d.n_cells; ++c) {
+      const int32_t kd = d.cell_kind[c];
+      if (kd < 0 || kd > 2) return fail(ARB_E_INVALID, "cell_kind must be 0, 1 or 2");
+      if (d.src_off[c + 1] < d.src_off[c]) return fail(ARB_E_INVALID, "src_off is not monotone");
+      if (kd != 0 && d.cv_off[c + 1] - d.cv_off[c] != 1) return fail(ARB_E_INVALID, "a LIF / source cell owns exactly one control volume");
+      if (kd == 1 && (!(d.lif_tau_m[c] > 0) || !finite(d.lif_tau_m[c]) || !(d.lif_c_m[c] > 0) || !finite(d.lif_c_m[c]) || !(d.lif_t_ref[c] >= 0) ||
+                      !finite(d.lif_t_ref[c]) || !finite(d.lif_v_th[c]) || !finite(d.lif_e_l[c]) || !finite(d.lif_e_r[c]) || !(d.lif_e_r[c] < d.lif_v_th[c])))
+        return fail(ARB_E_INVALID, "bad LIF parameters (cell " + std::to_string(c) + ")");
+      for (int64_t q = d.src_off[c]; q < d.src_off[c + 1]; ++q)
+        if (!(d.src_time[q] >= 0) || !finite(d.src_time[q]) || (q > d.src_off[c] && d.src_time[q] < d.src_time[q - 1]))
+          return fail(ARB_E_INVALID, "a spike schedule must be finite, >= 0 and ascending");
+    }
+    if (d.src_off[d.n_cells] >= (int64_t)0xFFFFFFF0u) return fail(ARB_E_INVALID, "more than 2^32 scheduled spikes are not supported");
+  }
   for (int64_t k = 0; k < d.n_clamp; ++k) {
     int64_t c = d.clamp_cell[k];
     if (c < 0 || c >= d.n_cells || d.clamp_cv[k] < 0 || d.clamp_cv[k] >= d.cv_off[c + 1] - d.cv_off[c]) return fail(ARB_E_INVALID, "clamp cell / CV out of range");
@@ -812,7 +830,7 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     std::unordered_map<uint64_t, std::vector<int32_t>> by_hash;
     for (int64_t c = 0; c < nc; ++c) {
       const uint32_t n = (uint32_t)(d.cv_off[c + 1] - d.cv_off[c]);
-      if (n > std::min(P.group_max_cv, kGroupMaxCv)) continue;
+      if (n > std::min(P.group_max_cv, kGroupMaxCv) || (d.cell_kind && d.cell_kind[c] != 0)) continue;
       auto& bucket = by_hash[hash[c]];
       int32_t cls = -1;
       for (int32_t k : bucket) {
@@ -867,9 +885,10 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
   H.n_groups = (int64_t)groups.size();
   H.n_group_cells = ngc;
   // internal cell order: group cells, forest cells (big first), block-unit cells
-  std::vector<uint32_t> forest_cells, block_cells;
+  std::vector<uint32_t> forest_cells, block_cells, point_cells;
   for (int64_t c = 0; c < nc; ++c) {
     if (cell_class[c] >= 0) continue;
+    if (d.cell_kind && d.cell_kind[c] != 0) { point_cells.push_back((uint32_t)c); continue; }
     uint64_t n_cv, n_syn, n_cl;
     cell_counts(c, n_cv, n_syn, n_cl);
     const bool fits = n_cv <= P.forest_max_cv && n_syn < P.forest_max_syn &&
@@ -882,6 +901,9 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
   H.cell_order = group_cells;
   H.cell_order.insert(H.cell_order.end(), forest_cells.begin(), forest_cells.end());
   H.cell_order.insert(H.cell_order.end(), block_cells.begin(), block_cells.end());
+  H.cell_order.insert(H.cell_order.end(), point_cells.begin(), point_cells.end());   // LIF cells and spike sources come last
+  H.n_pcells = (int64_t)point_cells.size();
+  H.pc_first = nc - H.n_pcells;
   H.cell_internal.resize(nc);
   for (int64_t i = 0; i < nc; ++i) H.cell_internal[H.cell_order[i]] = (uint32_t)i;
   // partition into units: forests (several small cells share one as long as it fits the smallest launch class),
@@ -901,7 +923,7 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     }
     H.n_forests = (int64_t)unit_begin.size();
     for (int64_t i = 0; i < (int64_t)block_cells.size(); ++i) unit_begin.push_back(ngc + (int64_t)forest_cells.size() + i);
-    unit_begin.push_back(nc);
+    unit_begin.push_back(nc - H.n_pcells);
   }
   H.n_units = (int64_t)unit_begin.size() - 1;
   H.units.resize(H.n_units);
@@ -1054,6 +1076,17 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
       H.block_lane_cap = std::max(H.block_lane_cap, uc.n_lane);
     }
   }
+  // point cells: a record each (V | runtime | t_last | t_ref_end | cursor), then one (unused) conductance slot per event
+  // target, so that events on them sort like everybody else's
+  H.pc_state_base = H.state_doubles;
+  {
+    int64_t targets = 0;
+    for (uint32_t c : point_cells) {
+      targets += d.syn_off ? d.syn_off[c + 1] - d.syn_off[c] : 0;
+      if (d.cell_kind[c] == 2) H.n_sched += d.src_off[c + 1] - d.src_off[c];
+    }
+    H.state_doubles += align_up((uint32_t)std::min<int64_t>(kPcDoubles * H.n_pcells + targets, 0x7FFFFFF0), 16);
+  }
   if (H.state_doubles >= (int64_t)0xFFFFFFF0u) { err = "state pool exceeds 2^32 doubles"; return ARB_E_INVALID; }
   // delays
   H.min_delay = std::numeric_limits<double>::infinity();
@@ -1186,6 +1219,31 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     UnitCounts placed = H.units[u];
     B.run(unit_begin[u], unit_cells[u], nullptr, &placed, &H);
   });
+  // point cells
+  H.pc_kind.resize(H.n_pcells); H.pc_par.assign(6 * (size_t)H.n_pcells, 0.0); H.pc_cv.resize(H.n_pcells);
+  H.pc_src_off.assign((size_t)H.n_pcells + 1, 0);
+  {
+    int64_t gpos = H.pc_state_base + kPcDoubles * H.n_pcells;
+    for (int64_t i = 0; i < H.n_pcells; ++i) {
+      const int64_t c = point_cells[i];
+      const int64_t cv = d.cv_off[c];
+      double* st = H.state.data() + H.pc_state_base + kPcDoubles * i;
+      st[0] = d.cv_vinit ? d.cv_vinit[cv] : -65.0;
+      st[1] = std::numeric_limits<double>::infinity(); st[2] = 0.0; st[3] = 1.0;
+      st[4] = 0.0; st[5] = -std::numeric_limits<double>::infinity(); st[6] = 0.0;
+      H.cv_state_idx[cv] = (uint32_t)(H.pc_state_base + kPcDoubles * i);
+      H.cell_rt_idx[H.pc_first + i] = (uint32_t)(H.pc_state_base + kPcDoubles * i + 1);
+      H.pc_kind[i] = d.cell_kind[c];
+      H.pc_cv[i] = (uint32_t)cv;
+      const double par[6] = {d.lif_tau_m[c], d.lif_v_th[c], d.lif_c_m[c], d.lif_e_l[c], d.lif_e_r[c], d.lif_t_ref[c]};
+      std::memcpy(H.pc_par.data() + 6 * i, par, sizeof par);
+      if (d.syn_off)
+        for (int64_t q = d.syn_off[c]; q < d.syn_off[c + 1]; ++q) H.syn_state_idx[q] = (uint32_t)gpos++;
+      const int64_t ns = d.cell_kind[c] == 2 ? d.src_off[c + 1] - d.src_off[c] : 0;
+      H.pc_src_off[i + 1] = H.pc_src_off[i] + (uint32_t)ns;
+      for (int64_t q = 0; q < ns; ++q) H.pc_src_time.push_back(d.src_time[d.src_off[c] + q]);
+    }
+  }
   // connections grouped by caller's source cell, ascending k inside a group
   H.conn_off.assign(H.n_src + 1, 0);             // by GLOBAL source id when the model is a shard
   for (int64_t k = 0; k < d.n_conn; ++k) H.conn_off[d.conn_src[k] + 1]++;

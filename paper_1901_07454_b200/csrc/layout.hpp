@@ -25,6 +25,8 @@ struct BuildParams {
                                   // group must fit in shared memory: 8 * kG bytes per control volume)
 };
 
+constexpr int kPcDoubles = 8;         // a point cell's record in the state pool: V | runtime triple | t_last | t_ref_end |
+                                      // schedule cursor | pad
 constexpr int64_t kMaxGroupCtas = 148 * 16;   // upper bound of resident CTAs of the group kernel (scratch sizing)
 
 struct UnitCounts {                   // everything the offset functions need
@@ -38,6 +40,13 @@ struct UnitCounts {                   // everything the offset functions need
 
 struct HostModel {
   int64_t n_cells = 0, n_cv = 0, n_syn = 0, n_clamp = 0, n_conn = 0, n_ext = 0, n_hh = 0;
+  // point cells (arb_desc.cell_kind != 0: LIF cells, spike sources): the last cells of the internal order
+  int64_t n_sched = 0;                  // scheduled spikes of all sources
+  int64_t n_pcells = 0, pc_first = 0, pc_state_base = 0;   // first internal index; double index of their records
+  std::vector<int32_t> pc_kind;
+  std::vector<double> pc_par;           // [n_pcells][6]: tau_m, v_th, c_m, e_l, e_r, t_ref
+  std::vector<uint32_t> pc_src_off, pc_cv;   // schedule offsets [n_pcells + 1]; caller's CV index of every point cell
+  std::vector<double> pc_src_time;
   int64_t gid_base = 0, n_src = 0;    // sharding: global id of local cell 0, cells of the whole network (= n_cells when unsharded)
   int64_t n_units = 0, n_forests = 0, n_lanes = 0;   // units: forests first, then block units
   int64_t fast_bytes = 0, state_doubles = 0, gen_doubles = 0, topo_bytes = 0, scratch_doubles = 0;

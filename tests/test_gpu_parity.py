@@ -546,6 +546,46 @@ def test_full_size_c2_100ms(B, orc, layout):
 
 
 # ---------------------------------------------------------------------------------------------
+# other cell kinds: LIF cells and spike sources beside cable cells
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_mixed_cell_kinds_network(B, orc, seed):
+    """Poisson spike sources drive LIF and cable cells which drive each other: identical spikes per cell (LIF and
+    source spikes sit exactly on event / schedule times: equal to 1e-12), LIF potentials and cable voltages."""
+    m = W.mixed_network(seed)
+    g, o = run_both(B, orc, m, 60.0)
+    n = check_spikes(g, o, m["n_cells"], tol=1e-9)
+    kind = m["cell_kind"]
+    gc, gt = g.spikes()
+    assert n > 60 and np.count_nonzero(kind[gc] == 1) > 20 and np.count_nonzero(kind[gc] == 0) > 3
+    src = np.flatnonzero(kind == 2)
+    assert np.array_equal(np.sort(gt[np.isin(gc, src)]), np.sort(m["src_time"][m["src_time"] < 60.0]))
+    gv, ov = g.voltage(), o.voltage()
+    lif_cv = m["cv_off"][:-1][kind == 1]
+    assert rel(gv[lif_cv], ov[lif_cv]) <= 1e-12
+    assert rel(gv, ov) < 1e-6
+    assert tuple(g.probe(B.ARB_PROBE_NSTEPS)) == tuple(o.probe(orc.PROBE_NSTEPS))
+    g.close()
+
+
+def test_mixed_cell_kinds_every_step(B, orc):
+    lockstep(B, orc, W.mixed_network(3, n_cable=5, n_lif=6, n_src=3, t_end=15.0), 600)
+
+
+def test_mixed_cell_kinds_launch_granularity_and_chunked_calls(B, orc):
+    m = W.mixed_network(4)
+    res = []
+    for fused, cuts in ((0, (60.0,)), (1, (7.3, 20.0, 33.125, 60.0))):
+        g = B.Model(m)
+        g.set_option(B.ARB_OPT_FUSED_STEPS, fused)
+        for t in cuts:
+            g.advance(t, DT)
+        res.append(g.spikes())
+        g.close()
+    assert np.array_equal(res[0][0], res[1][0]) and np.max(np.abs(res[0][1] - res[1][1])) < 1e-6
+
+
+# ---------------------------------------------------------------------------------------------
 # one network over several ranks (SURVEY.md 8(f) NEXT-3): the ranks run one after the other on this GPU
 # ---------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("n_ranks", [2, 3])

@@ -112,3 +112,38 @@ def test_product_does_not_touch_the_oracle():
                 src = open(os.path.join(dirpath, f)).read()
                 assert "arb_oracle" not in src and "liborc" not in src and "import orc" not in src, f
                 assert not re.search(r"^\s*(from|import)\s+oracle", src, flags=re.M), f
+
+
+def test_catalogue_names_the_mechanisms_and_cell_kinds(B):
+    """mechanisms are referenced by name from a catalogue; every parameter names an arb_desc field."""
+    cat = B.catalogue()
+    assert set(cat) == {"hh", "pas", "expsyn", "iclamp", "lif", "spike_source"}
+    assert cat["hh"][0] == 0 and cat["expsyn"][0] == 1 and cat["lif"][0] == 2
+    fields = {f for f, _ in B.arb_desc._fields_}
+    for name, (kind, params) in cat.items():
+        for field, unit, default in params:
+            assert field in fields, (name, field)
+    assert dict((f, d) for f, _, d in cat["hh"][1])["hh_gnabar"] == W.GNABAR
+    assert dict((f, d) for f, _, d in cat["lif"][1]) == W.LIF_DEFAULTS
+    L = B.lib()
+    assert L.arb_catalogue_find(b"pas") >= 0 and L.arb_catalogue_find(b"nope") == -1
+    assert L.arb_catalogue_entry(99, None, None, None) == B.ARB_E_INVALID
+
+
+def test_plan_accepts_and_validates_cell_kinds(B):
+    m = W.mixed_network()
+    assert B.arb_plan(m) > 0
+    bad = dict(m)
+    bad["cell_kind"] = m["cell_kind"].copy()
+    bad["cell_kind"][-1] = 1                          # a 301-CV cell cannot be a LIF cell
+    with pytest.raises(B.ArbError):
+        B.arb_plan(bad)
+    bad = dict(m)
+    bad["lif_tau_m"] = m["lif_tau_m"].copy()
+    bad["lif_tau_m"][np.flatnonzero(m["cell_kind"] == 1)[0]] = 0.0
+    with pytest.raises(B.ArbError):
+        B.arb_plan(bad)
+    bad = dict(m)
+    bad["src_time"] = m["src_time"][::-1].copy()      # schedules must ascend
+    with pytest.raises(B.ArbError):
+        B.arb_plan(bad)

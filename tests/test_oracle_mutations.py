@@ -16,6 +16,9 @@ The mutation list (what is changed, which pin is expected to catch it, the passa
   assemble_diag   parent loses the child's sigma     P1/P2 PAPER.md:154
   delay_half      event time = spike + delay/2       P11
   weight_drop     g = w instead of g += w            P8    PAPER.md:150, R7
+  lif_refractory  LIF: events are not ignored during t_ref             K1     R20
+  lif_reset       LIF: reset to E_L instead of E_R                     K1     R20
+  src_schedule    spike source: a spike at the interval's end emitted early (K2 compares exact times / counts)  K2  R20
   lin_syn_diag    linearised step: synaptic g missing on the diagonal   L1/L3  PAPER.md:152-156 (NEXT-2)
   lin_clamp_sign  linearised step: clamp current with the wrong sign   L1/L3  R8
   lin_hh_h        linearised step: g_Na without h                      L1/L4  R5
@@ -48,6 +51,9 @@ MUTATIONS = {
     "lin_syn_diag": ("    gsum[i] += M->g[gs];\n", "", "l1 or l3"),
     "lin_clamp_sign": ("src[M->cl_cv[ck]] += M->cl_amp[ck];", "src[M->cl_cv[ck]] -= M->cl_amp[ck];", "l1 or l3"),
     "lin_hh_h": ("double gna = M->gna[gi] * m * m * m * h * sc,", "double gna = M->gna[gi] * m * m * m * sc,", "l1 or l4"),
+    "lif_refractory": ("    if (te < c->t_ref_end) continue;", "", "k1"),
+    "lif_reset": ("      v[0] = M->lif_e_r[ci];\n", "      v[0] = M->lif_e_l[ci];\n", "k1"),
+    "src_schedule": ("M->src_time[c->src_cur] < tb) {", "M->src_time[c->src_cur] <= tb) {", "k2"),
     "weight_drop": ("M->g[c->syn0 + c->q[c->qh].syn] += c->q[c->qh].w;", "M->g[c->syn0 + c->q[c->qh].syn] = c->q[c->qh].w;", "p8"),
 }
 # gates_old_v needs a second edit: the rate call reads the saved copy
@@ -82,5 +88,5 @@ def test_mutation_is_caught(tmp_path, name):
 
 
 def test_unmutated_oracle_passes_the_same_pins():
-    r = _pins(None, "p1 or p2 or p8 or p9 or p11 or p13 or p14 or p15 or l1 or l3 or l4")
+    r = _pins(None, "p1 or p2 or p8 or p9 or p11 or p13 or p14 or p15 or l1 or l3 or l4 or k1 or k2")
     assert r.returncode == 0, r.stdout[-2000:]

@@ -794,7 +794,7 @@ def _lif_net(ev_t, ev_w, t_end=50.0, **par):
 
 
 def test_k1_lif_closed_form_charging_spike_and_refractory(orc):
-    tau, vth, cm, el, er, tref = 10.0, -50.0, 0.25, -65.0, -70.0, 2.0
+    tau, vth, cm, el, er, tref = 10.0, -50.0, 0.25, -65.0, -70.0, 6.0
     w, gap = 1.0, 1.3                                  # every event lifts V by w / C_m = 4 mV
     t = 0.7 + gap * np.arange(30)
     o = orc.Oracle(_lif_net(t, np.full(30, w), lif_tau_m=tau, lif_v_th=vth, lif_c_m=cm, lif_e_l=el, lif_e_r=er, lif_t_ref=tref))
@@ -807,8 +807,13 @@ def test_k1_lif_closed_form_charging_spike_and_refractory(orc):
     o.advance(50.0, DT)
     sc, st = o.spikes()
     assert st[0] == t[k_spike - 1]                     # the spike sits exactly on the event that crossed the threshold
-    # events inside the refractory period are lost; charging restarts from E_R at st + t_ref
+    # events inside the refractory period are lost (four of them here); charging restarts from E_R at st + t_ref
     nxt = [x for x in t if x >= st[0] + tref]
+    assert len([x for x in t if st[0] < x < st[0] + tref]) >= 4
+    o2 = orc.Oracle(_lif_net(t, np.full(30, w), lif_tau_m=tau, lif_v_th=vth, lif_c_m=cm, lif_e_l=el, lif_e_r=er, lif_t_ref=tref))
+    t_probe = 0.5 * (st[0] + tref + nxt[0])             # after the refractory period, before the next event
+    o2.advance(t_probe, DT)
+    assert o2.voltage()[0] == pytest.approx(el + (er - el) * np.exp(-(t_probe - (st[0] + tref)) / tau), rel=1e-13)
     v, tl = er, st[0] + tref
     second = None
     for x in nxt:
@@ -823,10 +828,10 @@ def test_k1_lif_closed_form_charging_spike_and_refractory(orc):
 
 def test_k2_spike_sources_emit_their_schedule_and_drive_a_cable_cell(orc):
     """A source cell's spikes are its schedule; a connection source -> cable cell delivers g += w at t + delay."""
-    sched = np.array([0.4, 3.3, 3.31, 7.0, 19.5])
+    sched = np.array([0.4, 3.3, 3.31, 7.0, 12.0, 19.5])   # 0.4 and 12.0 lie on grid points; 12.0 is the end of the run
     m = dict(n_cells=2, cv_off=[0, 1, 2], cv_parent=[-1, -1], cv_area=[100.0, 400.0], cv_cm=[1.0, 1.0], cv_raxial=[1.0, 1.0],
              pas_g=[0.0, 1e-4], pas_e=[-65.0, -65.0], syn_off=[0, 0, 1], syn_cv=[0], syn_tau=[3.0], syn_e=[0.0],
-             cell_kind=[2, 0], src_off=[0, 5, 5], src_time=sched,
+             cell_kind=[2, 0], src_off=[0, 6, 6], src_time=sched,
              conn_src=[0], conn_dst=[1], conn_syn=[0], conn_delay=[1.25], conn_weight=[0.0002], t_end=12.0)
     m = W.finalize(m)
     o = orc.Oracle(m)
