@@ -39,8 +39,8 @@ MUTATIONS = {
     "gates_old_v": ("  c->v_prev = v[c->det];\n  for (int64_t i = 0; i < c->n; ++i) v[i] = x[i];",
                     "  c->v_prev = v[c->det];\n  double* vold = (double*)malloc((size_t)c->n * 8); memcpy(vold, v, (size_t)c->n * 8);\n"
                     "  for (int64_t i = 0; i < c->n; ++i) v[i] = x[i];", "p14"),
-    "clamp_window": ("if (M->cl_t0[ck] <= t && t < M->cl_t1[ck])", "if (M->cl_t0[ck] < t && t <= M->cl_t1[ck])", "p15"),
-    "hh_m2": ("M->gna[gi] * m * m * m * h", "M->gna[gi] * m * m * h", "p9"),
+    "clamp_window": ("if (M->cl_t0[ck] <= t && t < M->cl_t1[ck]) I[", "if (M->cl_t0[ck] < t && t <= M->cl_t1[ck]) I[", "p15"),
+    "hh_m2": ("double dens = M->gna[gi] * m * m * m * h", "double dens = M->gna[gi] * m * m * h", "p9"),
     "area_scale": ("I[i] += dens * M->area[gi] * 1e-2;", "I[i] += dens * M->area[gi] * 1.1e-2;", "p9"),
     "syn_decay": ("M->g[gs] = M->g[gs] * exp(-delta / M->syn_tau[gs]);", "M->g[gs] = M->g[gs] * exp(-delta / (2.0 * M->syn_tau[gs]));", "p8"),
     "spike_interp": ("c->new_spikes[c->n_new++] = t + delta * (M->theta - c->v_prev) / (vd - c->v_prev);",
