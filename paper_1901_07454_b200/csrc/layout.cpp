@@ -864,7 +864,7 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
         caps.state_bytes = 8 * gstate_offsets(K.n_cv, mx_hh, mx_syn).total;
         caps.tail_bytes = co.total - co.hh_gna;
         caps.class_bytes = 64 + 40 * K.n_cv;               // upper bound: one segment per control volume
-        caps.buf_rows = std::max(K.n_cv, 2 * (mx_hh + mx_syn + mx_cl));
+        caps.buf_rows = std::max(K.n_cv, mx_hh + mx_syn + mx_cl);
         if (group_smem_plan(caps).bytes > P.group_max_smem) K.grouped = false;
       }
       if (!K.grouped) continue;
@@ -1037,7 +1037,7 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     G.hh_base = H.n_hh;
     for (uint32_t lc = 0; lc < G.n_cell; ++lc) H.n_hh += cell_hh[group_cells[G.cell_begin + lc]];
     H.gcaps.slot_cap = std::max(H.gcaps.slot_cap, K.n_cv);
-    H.gcaps.buf_rows = std::max(H.gcaps.buf_rows, std::max(K.n_seg, 2 * (G.n_hh_rows + G.n_syn_rows + G.n_cl_rows)));   // sources | conductances
+    H.gcaps.buf_rows = std::max(H.gcaps.buf_rows, std::max(K.n_seg, G.n_hh_rows + G.n_syn_rows + G.n_cl_rows));
   }
   // placement; tree structures are deduplicated by content
   std::unordered_map<uint64_t, std::vector<int64_t>> seen;   // hash -> units that own a stored record
