@@ -110,7 +110,24 @@ def algorithmic_bytes_per_grid_step(m, linearised=False):
     n_hh = 0
     if m["hh_gnabar"] is not None:
         n_hh = int(np.count_nonzero((m["hh_gnabar"] != 0) | (m["hh_gkbar"] != 0) | (m["hh_gl"] != 0)))
-    return 48 * m["n_cv"] + 4 * n_branch + 80 * n_hh + 20 * m["n_syn"]
+    return 48 * m["n_cv"] + 4 * n_branch + 80 * n_hh + 20 * synapse_instances(m)
+
+
+def synapse_instances(m):
+    """Synapse instances a step integrates: one per synapse, except in cells with >= 1,024 synapses, where the library
+    keeps ONE conductance per run of synapses on the same control volume with the same (tau, e) (DESIGN.md R22;
+    SURVEY.md 8(f) NEXT-1, second half) - the roofline is then quoted against that smaller count."""
+    so = np.asarray(m["syn_off"], np.int64)
+    per_cell = np.diff(so)
+    big = np.flatnonzero(per_cell >= 1024)
+    n = int(m["n_syn"])
+    for c in big:
+        a, b = int(so[c]), int(so[c + 1])
+        key = np.stack([m["syn_cv"][a:b].astype(np.float64), m["syn_tau"][a:b], m["syn_e"][a:b]], axis=1)
+        runs = len(np.unique(key, axis=0))
+        if 2 * runs <= b - a:
+            n -= (b - a) - runs
+    return n
 
 
 def committed_traffic(key):
@@ -468,7 +485,8 @@ def run_ours(args):
     roofline = {"kernel": "+".join(kernels), "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "frac_nominal_8tbs": achieved / NOMINAL_HBM_GBS,
                 "traffic": traffic, "traffic_source": traffic_src,
-                "peak_source": peak_src, "algorithmic_bytes_per_grid_step": alg_step,
+                "peak_source": peak_src, "algorithmic_bytes_per_grid_step": alg_step, "synapse_instances": synapse_instances(m), "synapses": int(m["n_syn"]),
+                "frac_if_every_synapse_were_integrated": (alg_step + 20 * (int(m["n_syn"]) - synapse_instances(m))) / (cable_ms_per_grid_step * 1e-3) / 1e9 / peak if cable_ms_per_grid_step > 0 else 0.0,
                 "cable_ms_per_grid_step": cable_ms_per_grid_step, "launches_per_grid_step": launches_per_grid_step,
                 "launches_timed": tim["cable_launches"],
                 "kernel_share_of_step": tim["cable_ms"] / ms if ms > 0 else None,

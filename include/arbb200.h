@@ -210,7 +210,12 @@ int arb_clear_spikes(arb_model* m);
 int arb_voltage(arb_model* m, double* out, int64_t n_cv);
 
 /* ARB_PROBE_M/H/N: gate state per CV (0 where the CV has no HH), n = n_cv.
- * ARB_PROBE_SYN_G: synaptic conductance per synapse in the caller's order, n = n_syn.
+ * ARB_PROBE_SYN_G: synaptic conductance per synapse in the caller's order, n = n_syn.  (In a cell with >= 1,024
+ *                  synapses the library integrates ONE conductance per run of synapses that sit on the same control
+ *                  volume with the same tau and e - I = (sum g_j)(V - e) and the exponential decay are exact for the
+ *                  sum - when that at least halves their number; every synapse keeps a record (g_j, time of last
+ *                  event) from which this probe returns its own conductance, and arb_set_state rebuilds the sums.
+ *                  DESIGN.md reading R22; 10,000 synapses on ~130 control volumes.)
  * ARB_PROBE_TIME:  out[0] = current time, n >= 1.
  * ARB_PROBE_NSTEPS: out[0] = grid steps so far, out[1] = cell sub-steps so far (>= cells*grid
  *                  steps; the excess comes from event-driven step splitting), n >= 2.

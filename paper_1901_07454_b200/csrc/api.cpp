@@ -35,7 +35,7 @@ struct Regions {
   Region units, gdescs, ghot, ghotflag, gen, fast, state, topo, scratch, factor_dcontrib, cell_rt_idx, cell_orig, ev_off, ev_t, ev_gidx, ev_w, ev_fill,
       ext_off, ext_t, ext_gidx, ext_w, ext_cur, conn_off, conn_dst, conn_gidx, conn_delay, conn_w,
       pool_t[2], pool_dst[2], pool_gidx[2], pool_w[2], spike_cell, spike_t, counters, scan_tmp,
-      cv_idx, syn_idx, hh_m_idx, hh_stride, hh_cv, io, pc_kind, pc_par, pc_src_off, pc_src_time, pc_cv;
+      cv_idx, syn_idx, hh_m_idx, hh_stride, hh_cv, io, pc_kind, pc_par, pc_src_off, pc_src_time, pc_cv, lazy_run, run_off, run_gidx;
   size_t total = 0;
 };
 
@@ -109,6 +109,9 @@ Regions carve(const HostModel& H, const Caps& cap) {
   R.pc_src_off = C.take(4 * ((size_t)H.n_pcells + 1));
   R.pc_src_time = C.take(8 * (size_t)H.n_sched);
   R.pc_cv = C.take(4 * (size_t)H.n_pcells);
+  R.lazy_run = C.take(4 * (size_t)H.n_lazy);
+  R.run_off = C.take(4 * ((size_t)H.n_runs + 1));
+  R.run_gidx = C.take(4 * (size_t)H.n_runs);
   R.total = C.pos;
   return R;
 }
@@ -266,6 +269,8 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     if ((e = upload(m, R.pc_kind, H.pc_kind)) != cudaSuccess || (e = upload(m, R.pc_par, H.pc_par)) != cudaSuccess ||
         (e = upload(m, R.pc_src_off, H.pc_src_off)) != cudaSuccess || (e = upload(m, R.pc_src_time, H.pc_src_time)) != cudaSuccess ||
         (e = upload(m, R.pc_cv, H.pc_cv)) != cudaSuccess) return bail(e, "upload point cells");
+    if ((e = upload(m, R.lazy_run, H.lazy_run)) != cudaSuccess || (e = upload(m, R.run_off, H.run_off)) != cudaSuccess ||
+        (e = upload(m, R.run_gidx, H.run_gidx)) != cudaSuccess) return bail(e, "upload synapse runs");
     DevModel& D = m->D;
     std::memset(&D, 0, sizeof D);
     D.units = at<UnitDesc>(m, R.units);
@@ -282,6 +287,8 @@ int arb_create(const arb_desc* desc, void* dev_workspace, size_t bytes, void* cu
     D.conn_off = at<uint32_t>(m, R.conn_off); D.conn_dst = at<uint32_t>(m, R.conn_dst); D.conn_gidx = at<uint32_t>(m, R.conn_gidx);
     D.conn_delay = at<double>(m, R.conn_delay); D.conn_w = at<double>(m, R.conn_w);
     D.gid_base = H.gid_base;
+    D.lazy_base = (uint32_t)H.lazy_base; D.lazy_n = (uint32_t)H.n_lazy; D.n_runs = H.n_runs;
+    D.lazy_run = at<uint32_t>(m, R.lazy_run); D.run_off = at<uint32_t>(m, R.run_off); D.run_gidx = at<uint32_t>(m, R.run_gidx);
     D.n_pcells = H.n_pcells; D.pc_first = H.pc_first; D.pc_state_base = H.pc_state_base;
     D.pc_kind = at<int32_t>(m, R.pc_kind); D.pc_par = at<double>(m, R.pc_par); D.pc_src_off = at<uint32_t>(m, R.pc_src_off);
     D.pc_src_time = at<double>(m, R.pc_src_time); D.pc_cv = at<uint32_t>(m, R.pc_cv);
@@ -617,7 +624,7 @@ int arb_probe(arb_model* m, int what, double* out, int64_t n) {
     case ARB_PROBE_SYN_G: {
       if (n != m->H.n_syn) return fail(m, ARB_E_INVALID, "arb_probe: size mismatch");
       if (n == 0) return ARB_OK;
-      CU(m, launch_gather(m->D.state, at<uint32_t>(m, m->R.syn_idx), n, io, m->stream));
+      CU(m, launch_gather_syn(m->D, at<uint32_t>(m, m->R.syn_idx), n, m->t, io, m->stream));
       CU(m, cudaMemcpyAsync(out, io, 8 * (size_t)n, cudaMemcpyDeviceToHost, m->stream));
       CU(m, cudaStreamSynchronize(m->stream));
       return ARB_OK;
@@ -680,6 +687,7 @@ int arb_set_state(arb_model* m, const double* v, const double* hh_m, const doubl
   if (syn_g && m->H.n_syn > 0) {
     CU(m, cudaMemcpyAsync(io, syn_g, 8 * (size_t)m->H.n_syn, cudaMemcpyHostToDevice, m->stream));
     CU(m, launch_scatter(m->D.state, at<uint32_t>(m, m->R.syn_idx), m->H.n_syn, io, m->stream));
+    CU(m, launch_lazy_rebuild(m->D, m->t, m->stream));      // cells that keep one conductance per run (R22)
     CU(m, cudaStreamSynchronize(m->stream));
   }
   CU(m, launch_reset_detectors(m->D, m->stream));

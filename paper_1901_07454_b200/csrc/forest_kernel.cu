@@ -554,7 +554,7 @@ __device__ __forceinline__ void run_forest(const DevModel& M, const StepArgs& A,
           if (tn <= t) {
             uint32_t cur = cs.evcur[tid];
             const uint32_t end = cs.evend[tid];
-            while (cur < end && M.ev_t[cur] <= t) { U.g[M.ev_gidx[cur] - U.g_gidx0] += M.ev_w[cur]; ++cur; ++n_del; }
+            while (cur < end && M.ev_t[cur] <= t) { U.g[event_target(M, M.ev_gidx[cur], t, M.ev_w[cur]) - U.g_gidx0] += M.ev_w[cur]; ++cur; ++n_del; }
             tn = cur < end ? M.ev_t[cur] : CUDART_INF;
             cs.evcur[tid] = cur; U.rt[kRtDoubles * tid] = tn;
           }

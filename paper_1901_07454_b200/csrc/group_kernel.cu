@@ -760,7 +760,7 @@ __global__ void __launch_bounds__(kGroupThreads, kGroupMinCtas) cable_group_kern
               if (tn <= t) {
                 uint32_t cur = cs.evcur[tid];
                 const uint32_t end = cs.evend[tid];
-                while (cur < end && M.ev_t[cur] <= t) { Ss[M.ev_gidx[cur] - (uint32_t)D.state_base] += M.ev_w[cur]; ++cur; ++n_del; }
+                while (cur < end && M.ev_t[cur] <= t) { Ss[event_target(M, M.ev_gidx[cur], t, M.ev_w[cur]) - (uint32_t)D.state_base] += M.ev_w[cur]; ++cur; ++n_del; }
                 tn = cur < end ? M.ev_t[cur] : CUDART_INF;
                 cs.evcur[tid] = cur; U.srt[kRtDoubles * tid] = tn;
               }

@@ -489,7 +489,7 @@ __device__ __forceinline__ void run_unit(const DevModel& M, const StepArgs& A, c
           if (tn <= t) {
             uint32_t cur = cs.evcur[tid];
             const uint32_t end = cs.evend[tid];
-            while (cur < end && M.ev_t[cur] <= t) { U.g[M.ev_gidx[cur] - U.g_gidx0] += M.ev_w[cur]; ++cur; ++n_del; }
+            while (cur < end && M.ev_t[cur] <= t) { U.g[event_target(M, M.ev_gidx[cur], t, M.ev_w[cur]) - U.g_gidx0] += M.ev_w[cur]; ++cur; ++n_del; }
             tn = cur < end ? M.ev_t[cur] : CUDART_INF;
             cs.evcur[tid] = cur; U.rt[kRtDoubles * tid] = tn; cs.dirty[tid] = 1;
           }
@@ -863,6 +863,21 @@ __global__ void gather_kernel(const double* state, const uint32_t* idx, int64_t 
   int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i < n) out[i] = state[idx[i]];
 }
+__global__ void gather_syn_kernel(DevModel M, const uint32_t* idx, int64_t n, double t, double* out) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t gx = idx[i];
+  double g = M.state[gx];
+  if (gx - M.lazy_base < M.lazy_n && g != 0.0) g *= exp(-(t - M.state[gx + M.lazy_n]) / M.state[gx + 2 * (size_t)M.lazy_n]);
+  out[i] = g;
+}
+__global__ void lazy_rebuild_kernel(DevModel M, double t) {
+  int64_t r = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (r >= M.n_runs) return;
+  double sum = 0.0;
+  for (uint32_t l = M.run_off[r]; l < M.run_off[r + 1]; ++l) { sum += M.state[M.lazy_base + l]; M.state[M.lazy_base + M.lazy_n + l] = t; }
+  M.state[M.run_gidx[r]] = sum;
+}
 __global__ void scatter_kernel(double* state, const uint32_t* idx, int64_t n, const double* in) {
   int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i < n) state[idx[i]] = in[i];
@@ -969,6 +984,14 @@ cudaError_t launch_point_reset(const DevModel& M, double t, cudaStream_t s) {
 
 cudaError_t launch_gather(const double* state, const uint32_t* idx, int64_t n, double* out, cudaStream_t s) {
   if (n > 0) gather_kernel<<<grid_for(n, 256), 256, 0, s>>>(state, idx, n, out);
+  return cudaGetLastError();
+}
+cudaError_t launch_gather_syn(const DevModel& M, const uint32_t* idx, int64_t n, double t, double* out, cudaStream_t s) {
+  if (n > 0) gather_syn_kernel<<<grid_for(n, 256), 256, 0, s>>>(M, idx, n, t, out);
+  return cudaGetLastError();
+}
+cudaError_t launch_lazy_rebuild(const DevModel& M, double t, cudaStream_t s) {
+  if (M.n_runs > 0) lazy_rebuild_kernel<<<grid_for(M.n_runs, 256), 256, 0, s>>>(M, t);
   return cudaGetLastError();
 }
 cudaError_t launch_scatter(double* state, const uint32_t* idx, int64_t n, const double* in, cudaStream_t s) {

@@ -74,6 +74,11 @@ struct DevModel {
   const int32_t* pc_kind; const double* pc_par; const uint32_t* pc_src_off; const double* pc_src_time; const uint32_t* pc_cv;
   int sm_count;               // SMs of the device the model lives on (grid sizing)
   int linearised;             // ARB_OPT_LINEARISED: conductance-linearised step
+  // synapse runs (reading R22): lazy records (g_j | time of last touch | tau, 3 x lazy_n doubles) at state[lazy_base];
+  // an event's target index inside that range names a record, lazy_run[record] the state index of the run it feeds
+  uint32_t lazy_base, lazy_n;
+  const uint32_t* lazy_run;
+  const uint32_t* run_off; const uint32_t* run_gidx; int64_t n_runs;
   uint32_t* ghot;             // group kernel: three lists of n_groups entries (see CNT_HOT0)
   uint32_t* ghotflag;         // [2][n_groups], half launch_id & 1: launch_id of the launch whose hot list holds the group
 };
@@ -87,6 +92,20 @@ struct StepArgs {
   int hot_valid;         // the hot list of this launch was written by the launch before it
   int mark_hot;          // write the hot list of the next launch
 };
+
+// Where an event with target index gx adds its weight.  A target inside the lazy range is a synapse of a
+// cell that keeps one conductance per run (R22): its own record is brought up to date at the delivery time t,
+// g_j <- g_j exp(-(t - t_j) / tau) + w, and the weight goes to the run.
+__device__ __forceinline__ uint32_t event_target(const DevModel& M, uint32_t gx, double t, double w) {
+  if (gx - M.lazy_base < M.lazy_n) {                 // (unsigned: false for everything below lazy_base, and when lazy_n == 0)
+    double* rec = M.state + gx;
+    const double tau = rec[2 * (size_t)M.lazy_n], tl = rec[M.lazy_n];
+    rec[0] = rec[0] * exp(-(t - tl) / tau) + w;
+    rec[M.lazy_n] = t;
+    return M.lazy_run[gx - M.lazy_base];
+  }
+  return gx;
+}
 
 // all launchers queue work on `s` and return the last CUDA error code
 cudaError_t launch_factor(const DevModel& M, double dt, cudaStream_t s);
@@ -105,6 +124,10 @@ cudaError_t launch_spikes_to_events(const DevModel& M, int cur_pool, cudaStream_
 cudaError_t launch_remote_spikes_to_events(const DevModel& M, int cur_pool, const unsigned long long* blocks, int64_t n_blocks,
                                            int64_t cap, int64_t own, cudaStream_t s);
 cudaError_t launch_gather(const double* state, const uint32_t* idx, int64_t n, double* out, cudaStream_t s);
+// synaptic conductances at time t: lazy records (R22) are decayed from their time of last touch on the way out
+cudaError_t launch_gather_syn(const DevModel& M, const uint32_t* idx, int64_t n, double t, double* out, cudaStream_t s);
+// after new g_j were scattered into the lazy records: stamp them with t and rebuild every run's sum (index order)
+cudaError_t launch_lazy_rebuild(const DevModel& M, double t, cudaStream_t s);
 cudaError_t launch_scatter(double* state, const uint32_t* idx, int64_t n, const double* in, cudaStream_t s);
 cudaError_t launch_gather_hh(const double* state, const uint32_t* m_idx, const uint32_t* stride, const uint32_t* cv,
                              int which, int64_t n_hh, double* out, cudaStream_t s);

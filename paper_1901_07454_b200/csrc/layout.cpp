@@ -763,9 +763,80 @@ struct GroupCounts { uint32_t cls = 0, n_cell = 0, n_hh_rows = 0, n_syn_rows = 0
 
 }  // namespace
 
-int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std::string& err) {
-  int rc = validate(d, err);
+// Synapse runs (second half; reading R22).  In a cell with many synapses, the synapses on one
+// control volume with the same (tau, e) only enter a step through their TOTAL conductance: I = (sum g_j)(V - e) and
+// sum g_j <- (sum g_j) exp(-delta / tau) are exact for the exponential integrator (R7).  Such cells are handed to the
+// builders with one synapse per run; every original synapse keeps a lazy record (g_j, time of last touch) that an
+// event brings up to date, so that read-back returns the individual g_j.
+struct SynRuns {
+  std::vector<int64_t> syn_off;           // derived description: per cell
+  std::vector<int32_t> syn_cv;
+  std::vector<double> syn_tau, syn_e;
+  std::vector<int64_t> map;               // original synapse -> derived synapse (global index)
+  std::vector<int64_t> lid;               // original synapse -> lazy record, or -1
+  std::vector<int64_t> run_of_lazy;       // lazy record -> derived synapse (its run)
+  int64_t n_lazy = 0, n_runs = 0;
+};
+
+static void build_runs(const arb_desc& d, const BuildParams& P, SynRuns& R) {
+  const int64_t nc = d.n_cells, ns = d.syn_off ? d.syn_off[nc] : 0;
+  R.syn_off.assign(nc + 1, 0);
+  R.map.assign(ns, 0); R.lid.assign(ns, -1);
+  R.syn_cv.reserve(ns); R.syn_tau.reserve(ns); R.syn_e.reserve(ns);
+  std::vector<int64_t> order;
+  for (int64_t c = 0; c < nc; ++c) {
+    const int64_t a = d.syn_off[c], n = d.syn_off[c + 1] - a;
+    bool merge = P.merge_min_syn > 0 && n >= (int64_t)P.merge_min_syn && !(d.cell_kind && d.cell_kind[c] != 0);
+    auto same = [&](int64_t x, int64_t y) { return d.syn_cv[x] == d.syn_cv[y] && d.syn_tau[x] == d.syn_tau[y] && d.syn_e[x] == d.syn_e[y]; };
+    if (merge) {
+      order.resize(n);
+      for (int64_t i = 0; i < n; ++i) order[i] = a + i;
+      std::sort(order.begin(), order.end(), [&](int64_t x, int64_t y) {
+        if (d.syn_cv[x] != d.syn_cv[y]) return d.syn_cv[x] < d.syn_cv[y];
+        if (d.syn_tau[x] != d.syn_tau[y]) return d.syn_tau[x] < d.syn_tau[y];
+        if (d.syn_e[x] != d.syn_e[y]) return d.syn_e[x] < d.syn_e[y];
+        return x < y;
+      });
+      int64_t nr = 1;
+      for (int64_t i = 1; i < n; ++i) nr += !same(order[i], order[i - 1]);
+      merge = 2 * nr <= n;                          // worth it only when runs are much fewer than synapses
+    }
+    if (!merge) {
+      for (int64_t s = a; s < a + n; ++s) {
+        R.map[s] = (int64_t)R.syn_cv.size();
+        R.syn_cv.push_back(d.syn_cv[s]); R.syn_tau.push_back(d.syn_tau[s]); R.syn_e.push_back(d.syn_e[s]);
+      }
+    } else {
+      for (int64_t i = 0; i < n; ++i) {
+        const int64_t s = order[i];
+        if (i == 0 || !same(s, order[i - 1])) { ++R.n_runs; R.syn_cv.push_back(d.syn_cv[s]); R.syn_tau.push_back(d.syn_tau[s]); R.syn_e.push_back(d.syn_e[s]); }
+        R.map[s] = (int64_t)R.syn_cv.size() - 1;
+        R.lid[s] = R.n_lazy++;                      // records of a run are contiguous, in ascending original index
+        R.run_of_lazy.push_back(R.map[s]);
+      }
+    }
+    R.syn_off[c + 1] = (int64_t)R.syn_cv.size();
+  }
+}
+
+int build(const arb_desc& d_in, const BuildParams& P, bool fill, HostModel& H, std::string& err) {
+  int rc = validate(d_in, err);
   if (rc) return rc;
+  // synapse runs: from here on `d` is the description the kernels integrate (one synapse per run in merged cells)
+  SynRuns runs;
+  arb_desc d_mod = d_in;
+  if (d_in.syn_off && P.merge_min_syn > 0) {
+    bool any = false;
+    for (int64_t c = 0; c < d_in.n_cells && !any; ++c)
+      any = d_in.syn_off[c + 1] - d_in.syn_off[c] >= (int64_t)P.merge_min_syn && !(d_in.cell_kind && d_in.cell_kind[c] != 0);
+    if (any) {
+      build_runs(d_in, P, runs);
+      d_mod.syn_off = runs.syn_off.data(); d_mod.syn_cv = runs.syn_cv.data();
+      d_mod.syn_tau = runs.syn_tau.data(); d_mod.syn_e = runs.syn_e.data();
+    }
+  }
+  const arb_desc& d = d_mod;
+  const int64_t n_syn_orig = d_in.syn_off ? d_in.syn_off[d_in.n_cells] : 0;
   H = HostModel();
   H.n_cells = d.n_cells;
   H.n_cv = d.cv_off[d.n_cells];
@@ -1087,12 +1158,16 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     }
     H.state_doubles += align_up((uint32_t)std::min<int64_t>(kPcDoubles * H.n_pcells + targets, 0x7FFFFFF0), 16);
   }
+  H.n_lazy = runs.n_lazy; H.n_runs = runs.n_runs;
+  H.lazy_base = H.state_doubles;
+  H.state_doubles += (3 * H.n_lazy + 15) / 16 * 16;
+  H.n_syn_inst = H.n_syn;
   if (H.state_doubles >= (int64_t)0xFFFFFFF0u) { err = "state pool exceeds 2^32 doubles"; return ARB_E_INVALID; }
   // delays
   H.min_delay = std::numeric_limits<double>::infinity();
   H.max_delay = 0;
   for (int64_t k = 0; k < d.n_conn; ++k) { H.min_delay = std::min(H.min_delay, d.conn_delay[k]); H.max_delay = std::max(H.max_delay, d.conn_delay[k]); }
-  if (!fill) return ARB_OK;
+  if (!fill) { H.n_syn = n_syn_orig; return ARB_OK; }
 
   // pass 2: fill
   H.fast.assign(H.fast_bytes, 0);
@@ -1244,6 +1319,26 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
       for (int64_t q = 0; q < ns; ++q) H.pc_src_time.push_back(d.src_time[d.src_off[c] + q]);
     }
   }
+  // state index of every ORIGINAL synapse: its instance, or its lazy record when its cell keeps run sums
+  if (H.n_lazy > 0) {
+    std::vector<uint32_t> final_idx((size_t)n_syn_orig);
+    H.lazy_run.resize(H.n_lazy);
+    double* lz = H.state.data() + H.lazy_base;
+    for (int64_t s = 0; s < n_syn_orig; ++s) {
+      const uint32_t inst = H.syn_state_idx[runs.map[s]];
+      if (runs.lid[s] < 0) { final_idx[s] = inst; continue; }
+      const int64_t l = runs.lid[s];
+      final_idx[s] = (uint32_t)(H.lazy_base + l);
+      H.lazy_run[l] = inst;
+      lz[l] = 0.0; lz[H.n_lazy + l] = 0.0; lz[2 * H.n_lazy + l] = d_in.syn_tau[s];   // g_j, time of last touch, tau
+    }
+    H.run_off.clear(); H.run_gidx.clear();
+    for (int64_t l = 0; l < H.n_lazy; ++l)
+      if (l == 0 || runs.run_of_lazy[l] != runs.run_of_lazy[l - 1]) { H.run_off.push_back((uint32_t)l); H.run_gidx.push_back(H.lazy_run[l]); }
+    H.run_off.push_back((uint32_t)H.n_lazy);
+    H.syn_state_idx.swap(final_idx);
+  }
+  H.n_syn = n_syn_orig;
   // connections grouped by caller's source cell, ascending k inside a group
   H.conn_off.assign(H.n_src + 1, 0);             // by GLOBAL source id when the model is a shard
   for (int64_t k = 0; k < d.n_conn; ++k) H.conn_off[d.conn_src[k] + 1]++;
@@ -1254,7 +1349,7 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     for (int64_t k = 0; k < d.n_conn; ++k) {
       uint32_t p = cur[d.conn_src[k]]++;
       H.conn_dst[p] = H.cell_internal[d.conn_dst[k]];
-      H.conn_gidx[p] = H.syn_state_idx[d.syn_off[d.conn_dst[k]] + d.conn_syn[k]];
+      H.conn_gidx[p] = H.syn_state_idx[d_in.syn_off[d.conn_dst[k]] + d.conn_syn[k]];
       H.conn_delay[p] = d.conn_delay[k];
       H.conn_w[p] = d.conn_weight[k];
     }
@@ -1279,7 +1374,7 @@ int build(const arb_desc& d, const BuildParams& P, bool fill, HostModel& H, std:
     for (int64_t p = 0; p < d.n_ext; ++p) {
       int64_t k = idx[p];
       H.ext_t[p] = d.ext_time[k];
-      H.ext_gidx[p] = H.syn_state_idx[d.syn_off[d.ext_cell[k]] + d.ext_syn[k]];
+      H.ext_gidx[p] = H.syn_state_idx[d_in.syn_off[d.ext_cell[k]] + d.ext_syn[k]];
       H.ext_w[p] = d.ext_weight[k];
     }
   }

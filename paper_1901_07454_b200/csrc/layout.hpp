@@ -18,6 +18,8 @@ struct BuildParams {
                                   // are a forest of their own)
   uint32_t forest_max_cv = 24000; // cells with more control volumes do not fit a CTA's shared memory: block units
   uint32_t forest_max_syn = 1024; // cells with at least this many synapses are block units (key reduction)
+  uint32_t merge_min_syn = 1024;  // cells with at least this many synapses keep ONE conductance per run of synapses on the same
+                                  // control volume with the same (tau, e) (second half); 0 = never
   uint32_t max_branch_len = 1024; // block units: longer unbranched chains are cut into pieces
   uint32_t group_min_cells = 4;   // a topology class with fewer cells is laid out as units; 0 = no groups
   uint32_t group_max_smem = 112 * 1024;  // shared memory a cell group may need (two CTAs per SM at least)
@@ -47,6 +49,12 @@ struct HostModel {
   std::vector<double> pc_par;           // [n_pcells][6]: tau_m, v_th, c_m, e_l, e_r, t_ref
   std::vector<uint32_t> pc_src_off, pc_cv;   // schedule offsets [n_pcells + 1]; caller's CV index of every point cell
   std::vector<double> pc_src_time;
+  // synapse runs (reading R22): synapses of merged cells keep a lazy record (g_j, time of last touch, tau) in the state pool
+  // at [lazy_base, lazy_base + 3 n_lazy); syn_state_idx of such a synapse is its record, lazy_run the state index of its run
+  int64_t n_lazy = 0, lazy_base = 0, n_runs = 0, n_syn_inst = 0;   // n_syn_inst: synapse instances the kernels integrate
+  std::vector<uint32_t> lazy_run;       // [n_lazy]
+  std::vector<uint32_t> run_off;        // [n_runs + 1]: lazy records of run r (contiguous)
+  std::vector<uint32_t> run_gidx;       // [n_runs]: state index of the run's conductance
   int64_t gid_base = 0, n_src = 0;    // sharding: global id of local cell 0, cells of the whole network (= n_cells when unsharded)
   int64_t n_units = 0, n_forests = 0, n_lanes = 0;   // units: forests first, then block units
   int64_t fast_bytes = 0, state_doubles = 0, gen_doubles = 0, topo_bytes = 0, scratch_doubles = 0;

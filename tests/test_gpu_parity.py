@@ -302,6 +302,47 @@ def test_many_synapses_key_reduction_every_step(B, orc):
     lockstep(B, orc, m, 200)
 
 
+def _many_synapse_runs(n_cells, n_syn, two_kinds):
+    """Ring cells whose synapses share (tau, e) per control volume: the library keeps one conductance per run."""
+    m = W.paper_ring(n_cells=n_cells, n_syn=n_syn, t_end=10.0)
+    rng = np.random.default_rng(11)
+    if two_kinds:                                  # two kinds of synapse on every control volume: two runs per CV
+        kind = rng.integers(0, 2, m["n_syn"])
+        m["syn_tau"] = np.where(kind == 0, 2.0, 3.5)
+        m["syn_e"] = np.where(kind == 0, 0.0, -70.0)
+    n_ev = 1500
+    m["ext_cell"] = np.concatenate([m["ext_cell"], rng.integers(0, n_cells, n_ev)])
+    m["ext_syn"] = np.concatenate([m["ext_syn"], rng.integers(0, n_syn, n_ev).astype(np.int32)])
+    t_ev = rng.uniform(0.0, 5.0, n_ev)
+    t_ev[::3] = np.round(t_ev[::3] / DT) * DT          # a third of them on grid points
+    m["ext_time"] = np.concatenate([m["ext_time"], t_ev])
+    m["ext_weight"] = np.concatenate([m["ext_weight"], rng.uniform(0.0001, 0.001, n_ev)])
+    return W.finalize(m)
+
+
+@pytest.mark.parametrize("two_kinds", [False, True])
+def test_synapse_runs_every_step(B, orc, two_kinds):
+    """SURVEY.md 8(f) NEXT-1, second half (R22): cells with >= 1,024 synapses keep one conductance per run of
+    synapses on one control volume with equal (tau, e); the individual g_j are lazy records.  Per-step parity of V, gates
+    and EVERY synapse's g against the oracle, the state re-injected every step (arb_set_state rebuilds the run sums)."""
+    lockstep(B, orc, _many_synapse_runs(3, 2500, two_kinds), 200)
+
+
+def test_synapse_runs_free_running_and_round_trip(B, orc):
+    """The same cells free-running for 400 steps (lazy records decay over many steps without being touched), then
+    read-back -> arb_set_state -> read-back returns the same conductances."""
+    m = _many_synapse_runs(4, 2000, True)
+    g, o = run_both(B, orc, m, 10.0)
+    assert g.stats()["block_units"] == 0           # merged, the cells fit a forest (or a group): no block units
+    g0 = g.syn_g()
+    assert np.count_nonzero(g0) > 500
+    assert rel_pure(g0, o.syn_g()) < 1e-9
+    assert rel(g.voltage(), o.voltage()) < 1e-6
+    g.set_state(syn_g=g0)
+    assert rel_pure(g.syn_g(), g0) < 1e-15
+    g.close()
+
+
 def test_heterogeneous_cut_spikes(B, orc):
     m = W.config4(n_cells=120, t_end=60.0)
     g, o = run_both(B, orc, m, 60.0)
