@@ -314,13 +314,14 @@ __device__ __noinline__ Gates hh_gates(double v, double delta, double m, double 
 // the instruction cache): cells may be inactive (mode 0) or on an event-split sub-step of their own length
 // (mode 2).
 // ------------------------------------------------------------------------------------------
+template <bool kLin>
 __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U, const CellS& cs, double dt, const bool kGen) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const bool multi = U.n_cell > 1;
   const uint32_t n_hh = U.n_hh, n_syn = U.n_syn, n_cl = U.n_clamp;
 
   // event-split sub-steps: those cells' matrices are eliminated for their own step length (reading R9)
-  const bool lin = M.linearised != 0;
+  constexpr bool lin = kLin;               // the linearised step is a kernel instantiation of its own (code size)
   double* xG = U.xI + (n_hh + n_syn + n_cl);                 // lin: conductances beside the sources
   if (!lin && kGen && U.masks[1] != 0ull) eliminate_forest<1>(U, &cs, dt, U.fgen, U.invdgen);
 
@@ -528,6 +529,7 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
 // A.nk grid steps of one forest.  Phase A: deliver the events due now and choose each cell's
 // sub-step (reading R9), then the step itself.
 // ------------------------------------------------------------------------------------------
+template <bool kLin>
 __device__ __forceinline__ void run_forest(const DevModel& M, const StepArgs& A, const FView& U, const CellS& cs,
                                            unsigned& n_sub, unsigned& n_del) {
   uint32_t* sMaskW = (uint32_t*)U.masks;     // the two 64-bit masks as four words (little endian)
@@ -577,7 +579,7 @@ __device__ __forceinline__ void run_forest(const DevModel& M, const StepArgs& A,
       const int any_active = __syncthreads_or(active);
       if (!any_active) break;
       const int general = __syncthreads_or(!plain);
-      forest_substep(M, U, cs, A.dt, general != 0);
+      forest_substep<kLin>(M, U, cs, A.dt, general != 0);
     }
   }
   if ((uint32_t)tid < n_cell) {
@@ -590,6 +592,7 @@ __device__ __forceinline__ void run_forest(const DevModel& M, const StepArgs& A,
 // ------------------------------------------------------------------------------------------
 // The cable step for forests: one CTA per forest of launch class `cls`.
 // ------------------------------------------------------------------------------------------
+template <bool kLin>
 __global__ void __launch_bounds__(kForestThreads, 8) cable_forest_kernel(DevModel M, StepArgs A, int cls) {
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ UnitHeader H;
@@ -623,7 +626,7 @@ __global__ void __launch_bounds__(kForestThreads, 8) cable_forest_kernel(DevMode
   U.xI = (double*)(smem + P.off_xi);
   const CellS cs = carve_cells(smem + P.off_cell, U.n_cell);
   unsigned n_sub = 0, n_del = 0;
-  run_forest(M, A, U, cs, n_sub, n_del);
+  run_forest<kLin>(M, A, U, cs, n_sub, n_del);
   // ---- state record -> HBM (one bulk store)
   fence_proxy_async();
   __syncthreads();
@@ -697,12 +700,16 @@ __global__ void __launch_bounds__(kForestThreads) forest_init_kernel(DevModel M)
 }  // namespace
 
 cudaError_t configure_forest_kernel(int max_optin_bytes) {
-  cudaFuncAttributes fa;
-  cudaError_t e = cudaFuncGetAttributes(&fa, cable_forest_kernel);
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(cable_forest_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_optin_bytes - (int)fa.sharedSizeBytes);
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(cable_forest_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  for (const void* k : {(const void*)cable_forest_kernel<false>, (const void*)cable_forest_kernel<true>}) {
+    cudaFuncAttributes fa;
+    cudaError_t e = cudaFuncGetAttributes(&fa, k);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, max_optin_bytes - (int)fa.sharedSizeBytes);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    if (e != cudaSuccess) return e;
+  }
+  return cudaSuccess;
 }
 
 cudaError_t launch_forest_factor(const DevModel& M, double dt, cudaStream_t s) {
@@ -720,7 +727,8 @@ cudaError_t launch_forest_init(const DevModel& M, cudaStream_t s) {
 cudaError_t launch_forest_cable(const DevModel& M, const StepArgs& A, int cls, cudaStream_t s, int* launches) {
   const ForestClass& K = M.fcls[cls];
   if (K.count == 0) return cudaSuccess;
-  cable_forest_kernel<<<(unsigned)K.count, kForestThreads, K.plan.bytes, s>>>(M, A, cls);
+  if (!M.linearised) cable_forest_kernel<false><<<(unsigned)K.count, kForestThreads, K.plan.bytes, s>>>(M, A, cls);
+  else cable_forest_kernel<true><<<(unsigned)K.count, kForestThreads, K.plan.bytes, s>>>(M, A, cls);
   if (launches) ++*launches;
   return cudaGetLastError();
 }

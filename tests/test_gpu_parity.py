@@ -343,6 +343,31 @@ def test_synapse_runs_free_running_and_round_trip(B, orc):
     g.close()
 
 
+@pytest.mark.parametrize("scale", [0.1, 0.01])
+def test_fine_discretisation_split_steps(B, orc, scale):
+    """Control volumes 10 x / 100 x shorter than the configs' (areas and axial resistances scaled): sigma dt / C rises from
+    ~50 to ~5e3 / ~5e5, where an elimination loses log10(sigma dt / C) digits to cancellation - the oracle's textbook
+    recurrence as much as the kernels' re-elimination of event-split sub-steps.  Per-step parity with
+    events on and off the grid, tolerance scaled with the conditioning: 1e-15 sigma dt / C (tolerance
+    derivation; measured 2e-16 and 7e-17 times the ratio)."""
+    m = W.config1(n_cells=8, t_end=5.0)
+    m["cv_area"] = m["cv_area"] * scale
+    m["cv_raxial"] = m["cv_raxial"] * scale
+    rng = np.random.default_rng(3)
+    n_ev = 400
+    m["ext_cell"] = np.concatenate([m["ext_cell"], rng.integers(0, 8, n_ev)])
+    m["ext_syn"] = np.concatenate([m["ext_syn"], rng.integers(0, 10, n_ev).astype(np.int32)])
+    t_ev = rng.uniform(0.0, 2.0, n_ev)
+    t_ev[::4] = np.round(t_ev[::4] / DT) * DT
+    m["ext_time"] = np.concatenate([m["ext_time"], t_ev])
+    m["ext_weight"] = np.concatenate([m["ext_weight"], rng.uniform(1e-5, 1e-4, n_ev) * scale])
+    m = W.finalize(m)
+    cap = m["cv_cm"] * m["cv_area"] * 1e-5
+    ratio = float(np.max(DT / (m["cv_raxial"][1:] * cap[1:])))
+    assert ratio > 1e3
+    lockstep(B, orc, m, 80, tol=max(STEP_TOL, 1e-15 * ratio))
+
+
 def test_heterogeneous_cut_spikes(B, orc):
     m = W.config4(n_cells=120, t_end=60.0)
     g, o = run_both(B, orc, m, 60.0)
