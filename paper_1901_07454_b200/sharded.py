@@ -8,6 +8,12 @@ the library's kernels (arb_advance, arb_spike_block, arb_apply_spike_blocks); th
 torch.distributed's (NCCL over NVLink on a multi-GPU box; the spike blocks are a few KB, so one fused gather per
 epoch is latency-bound by design).  `LocalGroup` runs the ranks of one process one after the other on a single
 GPU - the same calls in the same order - which is how the path is tested where only one GPU is available.
+
+overlap=True (the exchange is hidden behind the integration of the next interval): the exchange epoch
+is HALF the minimum delay, and the all-gather of the spikes of half-epoch h runs on NCCL's stream while half-epoch h + 1
+is integrated; its spikes are applied before half-epoch h + 2, which is early enough because a spike of half-epoch h
+cannot cause an event before its end plus half a minimum delay.  Results do not depend on the mode beyond rounding
+(events are applied in (time, synapse, weight) order whenever they were queued).
 """
 from __future__ import annotations
 
@@ -73,6 +79,24 @@ def epoch_steps(min_delay, dt):
     return max(1, min(1024, int(np.floor(min_delay / dt - 1e-6))))
 
 
+def exchange_steps(min_delay, dt, overlap):
+    """Grid steps between exchanges.  overlap: half an epoch, so that the spikes of one half-epoch may arrive while the
+    next is integrated (None when the epoch is a single grid step: nothing to hide the exchange behind)."""
+    if not np.isfinite(min_delay):
+        return 1024
+    es = epoch_steps(min_delay, dt)
+    if not overlap:
+        return es
+    return es // 2 if es >= 2 else None
+
+
+def exchange_point(t0, j, es, dt, t_end):
+    """The j-th exchange point of a call that started at t0 (by multiplication, like the library's grid), or t_end when
+    that is nearer than a rounding error (no sliver of a step at the end of a call)."""
+    t = t0 + (j * es) * dt
+    return t_end if t_end - t < 1e-9 * dt else t
+
+
 def block_words(cap):
     return 1 + 2 * int(cap)
 
@@ -90,14 +114,16 @@ class DistGroup:
         self.dist.all_reduce(t, op=self.dist.ReduceOp.MIN)
         return float(t.item())
 
-    def all_gather(self, block, out):
-        self.dist.all_gather_into_tensor(out, block)
+    def all_gather(self, block, out, async_op=False):
+        """Returns None, or (async_op) a handle whose wait() orders the gather before later work of the current stream."""
+        return self.dist.all_gather_into_tensor(out, block, async_op=async_op)
 
 
 class ShardedModel:
     """One rank's part of a sharded network: arb_create on its shard, and the epoch loop with the exchange."""
 
-    def __init__(self, binding, m_global, rank, n_ranks, group, device="cuda:0", block_cap=None, ranges=None, local=None):
+    def __init__(self, binding, m_global, rank, n_ranks, group, device="cuda:0", block_cap=None, ranges=None, local=None,
+                 overlap=False):
         """m_global: the whole network (every rank cuts its shard out of it), or None with `local` = this rank's shard
         generated on its own (a workloads dict with shard_gid_base / shard_n_global set)."""
         import torch
@@ -113,22 +139,49 @@ class ShardedModel:
             self.ranges = ranges
         self.model = binding.Model(self.local, device=device)
         self.cap = int(block_cap or max(1024, 4 * (hi - lo)))
-        self.block = torch.zeros(block_words(self.cap), dtype=torch.int64, device=device)
-        self.blocks = torch.zeros(n_ranks * block_words(self.cap), dtype=torch.int64, device=device)
+        self.overlap = bool(overlap)
+        # two of each: with overlap, the blocks of one half-epoch are in flight while the next one is written
+        self.block2 = [torch.zeros(block_words(self.cap), dtype=torch.int64, device=device) for _ in range(2)]
+        self.blocks2 = [torch.zeros(n_ranks * block_words(self.cap), dtype=torch.int64, device=device) for _ in range(2)]
+        self.block, self.blocks = self.block2[0], self.blocks2[0]
         local_min = float(np.min(self.local["conn_delay"])) if self.local["n_conn"] else float("inf")
         self.min_delay = group.min_delay(local_min) if group is not None else local_min
         self.t = 0.0
-        self.k = 0      # grid steps since t = 0 (exchange epochs start on the grid k * dt)
 
     def advance(self, t_end, dt):
-        """Integrate to t_end in exchange epochs of floor(min_delay / dt) grid steps; spikes are exchanged after each."""
-        es = epoch_steps(self.min_delay, dt) if np.isfinite(self.min_delay) else 1024
+        """Integrate to t_end in exchange epochs of floor(min_delay / dt) grid steps; spikes are exchanged after each.
+        overlap: epochs of half that length, the exchange of one hidden behind the integration of the next."""
+        es = exchange_steps(self.min_delay, dt, self.overlap)
+        t0 = self.t                        # exchange points of this call: t0 + j es dt (by multiplication, like the library's grid)
+        if not self.overlap or es is None:
+            es = es or epoch_steps(self.min_delay, dt)
+            j = 0
+            while self.t < t_end:
+                j += 1
+                self.t = exchange_point(t0, j, es, dt, t_end)
+                self.model.advance(self.t, dt)
+                self.exchange()
+            return
+        pending, h = None, 0               # (work handle, blocks buffer) of the half-epoch before the one being integrated
         while self.t < t_end:
-            nxt = min(t_end, (self.k + es) * dt)
-            self.model.advance(nxt, dt)
-            self.k += es
-            self.t = nxt
-            self.exchange()
+            self.t = exchange_point(t0, h + 1, es, dt, t_end)
+            self.model.advance(self.t, dt)
+            if pending is not None:
+                self._finish(pending)
+            block, blocks = self.block2[h & 1], self.blocks2[h & 1]
+            self.model.spike_block(block, self.cap)
+            pending = None
+            if self.group is not None and self.n_ranks > 1:
+                pending = (self.group.all_gather(block, blocks, async_op=True), blocks)
+            h += 1
+        if pending is not None:
+            self._finish(pending)          # a call ends with every exchange applied
+
+    def _finish(self, pending):
+        work, blocks = pending
+        if work is not None:
+            work.wait()
+        self.model.apply_spike_blocks(blocks, self.n_ranks, self.cap, self.rank)
 
     def exchange(self):
         self.model.spike_block(self.block, self.cap)
@@ -144,9 +197,9 @@ class LocalGroup:
     """All ranks in one process on one GPU, one after the other: the calls a multi-GPU run makes, in the same order,
     with the all-gather replaced by a copy.  For tests and for checking a partition on a single-GPU box."""
 
-    def __init__(self, binding, m_global, n_ranks, device="cuda:0", block_cap=None):
+    def __init__(self, binding, m_global, n_ranks, device="cuda:0", block_cap=None, overlap=False):
         import torch
-        self.torch, self.n_ranks = torch, n_ranks
+        self.torch, self.n_ranks, self.overlap = torch, n_ranks, bool(overlap)
         self.ranges = partition(m_global["cv_off"], n_ranks)
         self.ranks = [ShardedModel(binding, m_global, r, n_ranks, None, device, block_cap, self.ranges) for r in range(n_ranks)]
         self.min_delay = min(s.min_delay for s in self.ranks)
@@ -158,22 +211,38 @@ class LocalGroup:
                 s.cap = self.cap
                 s.block = torch.zeros(block_words(self.cap), dtype=torch.int64, device=device)
         self.blocks = torch.zeros(n_ranks * block_words(self.cap), dtype=torch.int64, device=device)
-        self.t, self.k = 0.0, 0
+        self.t = 0.0
 
     def advance(self, t_end, dt):
-        es = epoch_steps(self.min_delay, dt) if np.isfinite(self.min_delay) else 1024
+        es = exchange_steps(self.min_delay, dt, self.overlap)
+        late = self.overlap and es is not None      # apply the blocks of half-epoch h after half-epoch h + 1, as the overlap does
+        if es is None:
+            es = epoch_steps(self.min_delay, dt)
         w = block_words(self.cap)
+        pending, t0, j = None, self.t, 0
         while self.t < t_end:
-            nxt = min(t_end, (self.k + es) * dt)
-            for r, s in enumerate(self.ranks):
+            j += 1
+            nxt = exchange_point(t0, j, es, dt, t_end)
+            for s in self.ranks:
                 s.model.advance(nxt, dt)
-                s.model.spike_block(s.block, self.cap)
-                self.blocks[r * w:(r + 1) * w].copy_(s.block)
-            self.torch.cuda.synchronize()
+            if pending is not None:
+                self._apply(pending)
+            blocks = self.torch.zeros_like(self.blocks) if late else self.blocks
             for r, s in enumerate(self.ranks):
-                s.model.apply_spike_blocks(self.blocks, self.n_ranks, self.cap, r)
-            self.k += es
+                s.model.spike_block(s.block, self.cap)
+                blocks[r * w:(r + 1) * w].copy_(s.block)
+            self.torch.cuda.synchronize()
+            pending = blocks
+            if not late:
+                self._apply(pending)
+                pending = None
             self.t = nxt
+        if pending is not None:
+            self._apply(pending)
+
+    def _apply(self, blocks):
+        for r, s in enumerate(self.ranks):
+            s.model.apply_spike_blocks(blocks, self.n_ranks, self.cap, r)
 
     def gather(self, what):
         """Concatenate a per-CV / per-synapse read-back of all ranks in global order."""
@@ -223,7 +292,9 @@ def _selftest():
         block[1:1 + len(gids)] = torch.from_numpy(gids)
         block[1 + cap:1 + cap + len(gids)] = torch.from_numpy((epoch * 5.0 + gids * 1e-3).view(np.int64))
         blocks = torch.zeros(world * w, dtype=torch.int64)
-        group.all_gather(block, blocks)
+        work = group.all_gather(block, blocks, async_op=(epoch == 1))      # the overlapped exchange uses the asynchronous form
+        if work is not None:
+            work.wait()
         got = []
         for r in range(world):
             n = int(blocks[r * w])

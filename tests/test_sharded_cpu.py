@@ -59,3 +59,15 @@ def test_two_rank_exchange_over_gloo():
     line = [l for l in r.stdout.splitlines() if l.startswith("{")][-1]
     j = json.loads(line)
     assert j["ok"] and j["world"] == 2 and j["ranges"][0][1] == j["ranges"][1][0]
+
+
+def test_exchange_steps_with_and_without_overlap():
+    """Exchange epochs: the library's epoch rule on the global minimum delay; half of it when the exchange is hidden
+    behind the next half-epoch's integration; no overlap when the epoch is a single grid step."""
+    from paper_1901_07454_b200 import sharded as S
+    assert S.exchange_steps(5.0, 0.025, False) == S.epoch_steps(5.0, 0.025) == 199      # the 1e-6 guard (DESIGN.md R11/R12)
+    assert S.exchange_steps(5.0, 0.025, True) == 99
+    assert S.exchange_steps(7.3, 0.025, True) == 145 and 2 * 145 * 0.025 <= 7.3      # floor(291 / 2)
+    assert S.exchange_steps(0.03, 0.025, True) is None
+    assert S.exchange_steps(float("inf"), 0.025, True) == 1024
+    assert S.exchange_point(0.0, 2, 100, 0.025, 5.0) == 5.0 and S.exchange_point(0.0, 1, 100, 0.025, 5.0) == 2.5
