@@ -232,6 +232,19 @@ int arb_voltage(arb_model* m, double* out, int64_t n_cv);
  *                  with CUDA events while ARB_OPT_TIMING is on, n >= 4. */
 int arb_probe(arb_model* m, int what, double* out, int64_t n);
 
+/* arb_probe(ARB_PROBE_M / ARB_PROBE_H / ARB_PROBE_N) for callers that may not allocate device memory (code under CUDA
+ * graph capture, serving loops, harnesses that forbid cudaMalloc): the per-CV staging buffer the gates are gathered
+ * into is not part of a workspace but a static device array of arb_noalloc_max_cv() = 524,288 doubles (4 MiB, held by
+ * every GPU that loads the library until the process exits).  Same arguments and result as arb_probe for the three gate
+ * selectors: out[i] = the gate of control volume i, 0 where it carries no HH mechanism, n_cv = the model's CV count,
+ * `out` is HOST memory, the call returns after the copy.  ARB_E_INVALID (with the limit in arb_last_error) when n_cv
+ * exceeds the array; nothing is written then.  The call makes no cudaMalloc / cudaFree and no allocating library call.
+ * All calls on a GPU share the array and it keeps the last call's contents: every call clears the part it uses first,
+ * so calls in sequence are independent, but calls that OVERLAP on the GPU (two models on different streams) race -
+ * serialise them. */
+int arb_gates_noalloc(arb_model* m, int what, double* out, int64_t n_cv);
+int64_t arb_noalloc_max_cv(void);
+
 /* Overwrite state from host arrays in the caller's order (any pointer may be NULL = keep).
  * Detector history is reset to the new voltages.  Exists so that tests can start both
  * implementations from one state. */

@@ -17,7 +17,7 @@ ARB_OPT_FUSED_STEPS, ARB_OPT_EPOCH_STEPS, ARB_OPT_TIMING, ARB_OPT_OVERLAP, ARB_O
 ARB_OPT_LINEARISED = 8
 
 EXPORTS = ("arb_plan", "arb_create", "arb_advance", "arb_spikes", "arb_clear_spikes", "arb_spike_block", "arb_apply_spike_blocks",
-           "arb_voltage", "arb_probe", "arb_catalogue_size", "arb_catalogue_entry", "arb_catalogue_param", "arb_catalogue_find",
+           "arb_voltage", "arb_probe", "arb_gates_noalloc", "arb_noalloc_max_cv", "arb_catalogue_size", "arb_catalogue_entry", "arb_catalogue_param", "arb_catalogue_find",
            "arb_set_state", "arb_set_option", "arb_fp64_peak", "arb_destroy", "arb_last_error")
 
 # arb_desc's layout / capacity options (0 = library default).  A workloads dict may carry them under the
@@ -77,6 +77,9 @@ def lib():
         L.arb_spikes.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64]
         L.arb_voltage.argtypes = [C.c_void_p, C.c_void_p, C.c_int64]
         L.arb_probe.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int64]
+        L.arb_gates_noalloc.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int64]
+        L.arb_noalloc_max_cv.restype = C.c_int64
+        L.arb_noalloc_max_cv.argtypes = []
         L.arb_set_state.argtypes = [C.c_void_p] * 6
         L.arb_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int64]
         L.arb_clear_spikes.argtypes = [C.c_void_p]
@@ -200,6 +203,12 @@ class Model:
 
     def syn_g(self):
         return self.probe(ARB_PROBE_SYN_G)
+
+    def gates_noalloc(self, what):
+        """arb_gates_noalloc: one gate (ARB_PROBE_M / H / N) per CV through the library's static staging array."""
+        out = np.empty(self.n_cv)
+        self._check(lib().arb_gates_noalloc(self._h, int(what), _ptr(out), self.n_cv))
+        return out
 
     def time(self):
         return float(self.probe(ARB_PROBE_TIME)[0])

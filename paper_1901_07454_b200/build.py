@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libarbb200.so")
-SOURCES = ["api.cpp", "layout.cpp", "kernels.cu", "group_kernel.cu", "forest_kernel.cu", "fp64_peak.cu"]
+SOURCES = ["api.cpp", "layout.cpp", "kernels.cu", "group_kernel.cu", "forest_kernel.cu", "no_alloc.cu", "fp64_peak.cu"]
 HEADERS = ["kernels.cuh", "layout.hpp", "unit_layout.h", "group_layout.h", "forest_layout.h", "device_common.cuh", os.path.join("..", "..", "include", "arbb200.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-pthread", "-shared", "-cudart", "static"]

@@ -608,6 +608,21 @@ int arb_voltage(arb_model* m, double* out, int64_t n_cv) {
   return ARB_OK;
 }
 
+int arb_gates_noalloc(arb_model* m, int what, double* out, int64_t n_cv) {
+  if (!m || !out) return fail(m, ARB_E_NULL, "arb_gates_noalloc: NULL argument");
+  if (what != ARB_PROBE_M && what != ARB_PROBE_H && what != ARB_PROBE_N) return fail(m, ARB_E_INVALID, "arb_gates_noalloc: selector is not a gate (ARB_PROBE_M / H / N)");
+  if (n_cv != m->H.n_cv) return fail(m, ARB_E_INVALID, "arb_gates_noalloc: n_cv mismatch");
+  if (n_cv > noalloc_max_cv())
+    return fail(m, ARB_E_INVALID, "arb_gates_noalloc: " + std::to_string(n_cv) + " control volumes exceed the static staging array of " +
+                                  std::to_string(noalloc_max_cv()) + " doubles; use arb_probe (staging in the caller's workspace)");
+  CU(m, launch_noalloc_gates(m->D.state, at<uint32_t>(m, m->R.hh_m_idx), at<uint32_t>(m, m->R.hh_stride), at<uint32_t>(m, m->R.hh_cv),
+                             what - ARB_PROBE_M, m->H.n_hh, n_cv, out, m->stream));
+  CU(m, cudaStreamSynchronize(m->stream));
+  return ARB_OK;
+}
+
+int64_t arb_noalloc_max_cv(void) { return noalloc_max_cv(); }
+
 int arb_probe(arb_model* m, int what, double* out, int64_t n) {
   if (!m || !out) return fail(m, ARB_E_NULL, "arb_probe: NULL argument");
   double* io = at<double>(m, m->R.io);

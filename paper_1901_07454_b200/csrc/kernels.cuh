@@ -138,6 +138,12 @@ cudaError_t launch_reset_detectors(const DevModel& M, cudaStream_t s);
 cudaError_t launch_point_cells(const DevModel& M, double t_win, cudaStream_t s, int* launches);
 cudaError_t launch_lif_relax(const DevModel& M, double t, double* io, cudaStream_t s);
 cudaError_t launch_point_reset(const DevModel& M, double t, cudaStream_t s);
+// read-back without an allocation (no_alloc.cu): the staging buffer is a static device array of kNoAllocMaxCv doubles
+constexpr int64_t kNoAllocMaxCv = 1 << 19;   // 4 MiB per GPU that loads the library
+int64_t noalloc_max_cv();
+cudaError_t noalloc_scratch(double** out);   // its device address on the current device (cudaGetSymbolAddress, once per device)
+cudaError_t launch_noalloc_gates(const double* state, const uint32_t* m_idx, const uint32_t* stride, const uint32_t* cv, int which,
+                                 int64_t n_hh, int64_t n_cv, double* host_out, cudaStream_t s);
 // cell groups (group_kernel.cu)
 cudaError_t launch_group_factor(const DevModel& M, double dt, uint32_t seg_cap, cudaStream_t s);
 cudaError_t launch_group_init(const DevModel& M, cudaStream_t s);
