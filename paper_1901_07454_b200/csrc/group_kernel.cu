@@ -104,6 +104,11 @@ __device__ __forceinline__ SegRec load_seg(const SegRec* p) {
   s.slot0 = q.x; s.pslot = q.y; s.len = (uint16_t)(q.z & 0xFFFFu); s.ccnt = (uint16_t)(q.z >> 16); s.cbeg = q.w;
   return s;
 }
+// j-th child segment of a segment (in the order a leaves -> root elimination meets them): out of the record itself
+// when there are at most two (group_layout.h), else out of the class record's child list.
+__device__ __forceinline__ uint32_t seg_child(const GView& U, const SegRec& sg, uint32_t j) {
+  return sg.ccnt <= kSegInlineChildren ? (sg.cbeg >> (16u * j)) & 0xFFFFu : (uint32_t)U.child[sg.cbeg + j];
+}
 
 // ------------------------------------------------------------------------------------------
 // Elimination of the diagonal of one segment for step length delta (factorisation; event-split
@@ -116,7 +121,7 @@ __device__ __forceinline__ void eliminate_seg(const GView& U, const SegRec& sg, 
   constexpr int kB = 8;                   // rows whose C, S, sigma are requested together (global memory)
   uint32_t lin = (sg.slot0 + sg.len - 1) * kG + c;
   double carry = 0.0;                     // f_{k+1} * sigma_{k+1}: what row k loses to its child in the segment
-  for (uint32_t j = 0; j < sg.ccnt; ++j) carry -= dcon[(uint32_t)U.child[sg.cbeg + j] * kG + c];
+  for (uint32_t j = 0; j < sg.ccnt; ++j) carry -= dcon[seg_child(U, sg, j) * kG + c];
   double fk = 0.0, sk = 0.0;
   int left = sg.len;
   while (left > 0) {
@@ -152,7 +157,7 @@ __device__ __forceinline__ void eliminate_seg_smem(const GView& U, const SegRec&
                                                    double* F, double* I, double* zcon) {
   uint32_t lin = (sg.slot0 + sg.len - 1) * kG + c;
   double z = 0.0;
-  for (uint32_t j = 0; j < sg.ccnt; ++j) z += zcon[(uint32_t)U.child[sg.cbeg + j] * kG + c];
+  for (uint32_t j = 0; j < sg.ccnt; ++j) z += zcon[seg_child(U, sg, j) * kG + c];
 #pragma unroll 2
   for (int left = sg.len; left > 0; --left, lin -= kG) {
     const uint32_t p = gswz(lin);
@@ -175,7 +180,7 @@ __device__ __forceinline__ void eliminate_seg_smem(const GView& U, const SegRec&
 __device__ __forceinline__ void eliminate_seg_lin(const GView& U, const SegRec& sg, uint32_t seg_idx, int c, double* F, double* I, double* dcon) {
   uint32_t lin = (sg.slot0 + sg.len - 1) * kG + c;
   double carry = 0.0;                     // f_{k+1} sigma_{k+1}: what row k loses to its child in the segment
-  for (uint32_t j = 0; j < sg.ccnt; ++j) carry -= dcon[(uint32_t)U.child[sg.cbeg + j] * kG + c];
+  for (uint32_t j = 0; j < sg.ccnt; ++j) carry -= dcon[seg_child(U, sg, j) * kG + c];
   double fk = 0.0, sk = 0.0;
 #pragma unroll 2
   for (int left = sg.len; left > 0; --left, lin -= kG) {
@@ -210,7 +215,7 @@ __device__ __forceinline__ void backward_seg(const GView& U, const SegRec& sg, u
     for (int j = 0; j < kRows; ++j) { p[j] = gswz(s - j * kG); fr[j] = F[p[j]]; ir[j] = I[p[j]]; vr[j] = Vs[p[j]]; }
     if (first) {
 #pragma unroll 1
-      for (uint32_t j = 0; j < sg.ccnt; ++j) vr[0] -= con[(uint32_t)U.child[sg.cbeg + j] * kG + c];
+      for (uint32_t j = 0; j < sg.ccnt; ++j) vr[0] -= con[seg_child(U, sg, j) * kG + c];
       first = false;
     }
 #pragma unroll
@@ -228,7 +233,7 @@ __device__ __forceinline__ void backward_seg(const GView& U, const SegRec& sg, u
     double v = Vs[p];
     if (first) {
 #pragma unroll 1
-      for (uint32_t j = 0; j < sg.ccnt; ++j) v -= con[(uint32_t)U.child[sg.cbeg + j] * kG + c];
+      for (uint32_t j = 0; j < sg.ccnt; ++j) v -= con[seg_child(U, sg, j) * kG + c];
       first = false;
     }
     const double r = fma(-fp, rp, v);
@@ -269,14 +274,14 @@ __device__ __forceinline__ void backward_stage(const GView& U, uint32_t st, int 
   const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
   if (on)
     for (uint32_t q = beg; q < end; ++q) {
-      const uint32_t si = U.order[q];
+      const uint32_t si = q;
       backward_seg(U, load_seg(U.segs + si), si, c, F, I, Vs, con);
     }
 }
 __device__ __forceinline__ void forward_stage(const GView& U, uint32_t st, int h, int c, bool on, const double* F, double* Vs) {
   const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
   if (on)
-    for (uint32_t q = end; q-- > beg;) forward_seg(load_seg(U.segs + U.order[q]), c, F, Vs);
+    for (uint32_t q = end; q-- > beg;) forward_seg(load_seg(U.segs + q), c, F, Vs);
 }
 
 // Both sweeps.  Stages [0, n_block) hold chunks on lane groups of several warps: block barriers.
@@ -524,7 +529,7 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
       const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
       if (!kGen || md != 0u)
         for (uint32_t q = beg; q < end; ++q) {
-          const uint32_t si = U.order[q];
+          const uint32_t si = q;
           eliminate_seg_lin(U, load_seg(U.segs + si), si, c, F, I, buf);
         }
       __syncthreads();
@@ -539,7 +544,7 @@ __device__ __forceinline__ void group_substep(const DevModel& M, const GView& U,
       const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
       if (md == 2u)
         for (uint32_t q = beg; q < end; ++q) {
-          const uint32_t si = U.order[q];
+          const uint32_t si = q;
           eliminate_seg_smem(U, load_seg(U.segs + si), si, c, dt / cs.delta[c], F, I, buf);
         }
       __syncthreads();
@@ -857,7 +862,7 @@ __global__ void __launch_bounds__(kGroupThreads) group_factor_kernel(DevModel M,
     for (uint32_t st = 0; st < U.n_stage; ++st) {
       const uint32_t beg = U.sched[st * kGroupSlots + h], end = U.sched[st * kGroupSlots + h + 1];
       for (uint32_t q = beg; q < end; ++q) {
-        const uint32_t si = U.order[q];
+        const uint32_t si = q;
         eliminate_seg(U, load_seg(U.segs + si), si, c, dt, f, invd, dcon);
       }
       __syncthreads();

@@ -52,18 +52,20 @@ ARBB_HD uint32_t gpos(uint32_t slot, uint32_t cell) { return gswz(slot * (uint32
 // positions of a per-CV array: whole 128-byte lines (the swizzle permutes inside a line)
 ARBB_HD uint32_t gcv_elems(uint32_t n_cv) { return align_up(n_cv * (uint32_t)kG, 16); }
 
+constexpr uint32_t kSegInlineChildren = 2;   // a segment with at most this many children carries them in its record
 struct SegRec {          // 16 bytes, one broadcast load per lane group
   uint32_t slot0;        // slot of the proximal control volume
   uint32_t pslot;        // slot of the parent control volume of slot0, or kNoSlot
   uint16_t len;          // control volumes in the segment
   uint16_t ccnt;         // child segments hanging off its last control volume
-  uint32_t cbeg;         // first entry of its child list
+  uint32_t cbeg;         // ccnt <= kSegInlineChildren: child0 | child1 << 16; else first entry of its child list
 };
 
 struct ClassRecord {     // header of a class record; arrays follow at the byte offsets below
   uint32_t n_cv, n_seg, n_stage, n_child;
   uint32_t off_segs;     // SegRec[n_seg]
-  uint32_t off_order;    // uint16[n_seg]: segments in backward processing order, grouped by (stage, slot)
+  uint32_t off_order;    // uint16[n_seg]: the identity (segments ARE numbered in backward processing order, grouped by
+                         // (stage, slot)); kept for the record's readers on the host, the kernels do not load it
   uint32_t off_sched;    // uint16[n_stage * kGroupSlots + 1]: begin of each (stage, slot) range in order[]
   uint32_t off_child;    // uint16[n_child]: child segments
   uint32_t bytes;

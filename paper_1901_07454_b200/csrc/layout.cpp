@@ -740,23 +740,36 @@ void build_class(const int32_t* par, uint32_t n, ClassInfo& K) {
   uint16_t* order = (uint16_t*)(K.record.data() + R.off_order);
   uint16_t* sched = (uint16_t*)(K.record.data() + R.off_sched);
   uint16_t* child = (uint16_t*)(K.record.data() + R.off_child);
-  uint32_t cpos = 0;
-  for (uint32_t s2 = 0; s2 < ns; ++s2) {
-    sr[s2].slot0 = slot0[s2];
-    sr[s2].pslot = segs[s2].parent < 0 ? kNoSlot : K.cv_slot[par[segs[s2].first]];
-    sr[s2].len = (uint16_t)segs[s2].len;
-    sr[s2].ccnt = (uint16_t)segs[s2].kids.size();
-    sr[s2].cbeg = cpos;
-    // children in descending order: the order in which a leaves -> root elimination meets them
-    for (size_t q = segs[s2].kids.size(); q-- > 0;) child[cpos++] = (uint16_t)segs[s2].kids[q];
-  }
+  // Segments are numbered in processing order on the device (the q-th segment the backward sweep meets is segment q:
+  // order[] is the identity and the kernels do not read it), and a segment with at most two children carries them in
+  // its record (cbeg = child0 | child1 << 16) - two dependent shared-memory loads less per chunk of a sweep.
+  std::vector<uint32_t> pos_of(ns, 0);
   uint32_t opos = 0, spos = 0;
   for (size_t st = 0; st < stages.size(); ++st)
     for (uint32_t h = 0; h < (uint32_t)kGroupSlots; ++h) {
       sched[spos++] = (uint16_t)opos;
-      for (uint32_t s2 : stages[st][h]) order[opos++] = (uint16_t)s2;
+      for (uint32_t s2 : stages[st][h]) { order[opos] = (uint16_t)opos; pos_of[s2] = opos++; }
     }
   sched[spos] = (uint16_t)opos;
+  uint32_t cpos = 0;
+  for (uint32_t q = 0; q < ns; ++q) {
+    uint32_t s2 = 0;
+    while (pos_of[s2] != q) ++s2;
+    SegRec& r = sr[q];
+    r.slot0 = slot0[s2];
+    r.pslot = segs[s2].parent < 0 ? kNoSlot : K.cv_slot[par[segs[s2].first]];
+    r.len = (uint16_t)segs[s2].len;
+    r.ccnt = (uint16_t)segs[s2].kids.size();
+    r.cbeg = cpos;
+    // children in descending order: the order in which a leaves -> root elimination meets them
+    uint32_t packed = 0, k = 0;
+    for (size_t j = segs[s2].kids.size(); j-- > 0; ++k) {
+      const uint32_t ch = pos_of[segs[s2].kids[j]];
+      child[cpos++] = (uint16_t)ch;
+      if (k < 2) packed |= ch << (16 * k);
+    }
+    if (r.ccnt <= kSegInlineChildren) r.cbeg = packed;
+  }
 }
 
 struct GroupCounts { uint32_t cls = 0, n_cell = 0, n_hh_rows = 0, n_syn_rows = 0, n_cl_rows = 0; int64_t cell_begin = 0, hh_base = 0; bool disjoint = false; };
