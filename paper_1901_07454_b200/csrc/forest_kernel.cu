@@ -31,13 +31,13 @@ namespace arbb {
 
 namespace {
 
-constexpr int kT = kForestThreads;
-constexpr int kW = kForestWarps;
+constexpr int kT = kForestThreads;         // threads of the factor / init kernels (the cable kernel has 32 kW, a template parameter)
 
 // Pointers of one forest.  V, gates, g, runtime, con, xI address shared memory in the cable kernel
 // (global memory in the factor / init kernels); everything else is global.
 struct FView {
   uint32_t n_slot, n_branch, n_chunk, n_level, n_cell, n_hh, n_syn, n_clamp, flags;
+  int n_warp;                       // warps the forest's runs are dealt to (forest_layout.h): kForestWarps or kForestWarpsBig
   const double *f, *invd, *a, *b, *hh_gna, *hh_gk, *hh_gl, *syn_e, *syn_decay, *cl_t0, *cl_t1, *cl_amp;
   const uint32_t *hh_slot, *syn_slot, *cl_slot;
   const uint16_t *hh_cell, *syn_cell, *cl_cell;
@@ -57,6 +57,7 @@ struct FView {
 __device__ __forceinline__ void make_fview(FView& U, const DevModel& M, const UnitHeader& H, uint8_t* fast, double* statew, const uint8_t* tp) {
   U.n_slot = H.n_slot; U.n_branch = H.n_lane; U.n_chunk = H.n_task; U.n_level = H.n_level;
   U.n_cell = H.n_cell; U.n_hh = H.n_hh; U.n_syn = H.n_syn; U.n_clamp = H.n_clamp; U.flags = H.flags;
+  U.n_warp = (int)H.pad[2];
   const FOffs& o = *(const FOffs*)tp;
   U.f = (const double*)(fast + o.fast[0]); U.invd = (const double*)(fast + o.fast[1]);
   U.a = (const double*)(fast + o.fast[2]); U.b = (const double*)(fast + o.fast[3]);
@@ -190,14 +191,17 @@ __device__ __forceinline__ void eliminate_chunk(const FView& U, const CellS* cs,
 
 template <int kSel>
 __device__ __forceinline__ void eliminate_forest(const FView& U, const CellS* cs, double dt, double* fout, double* invdout) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  // the forest's runs of a level over the warps of the block: one each in the cable kernel, one or two in the factor kernel
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, n_warps = (int)(blockDim.x >> 5);
   for (int lvl = (int)U.n_level - 1; lvl >= 0; --lvl) {
-    const FRun R = U.runs[lvl * kW + warp];
-    double cx = 1.0, csig = 0.0;
-    const unsigned long long want = kSel == 1 ? U.masks[1] : (kSel == 2 ? U.masks[0] : ~0ull);
-    for (uint32_t ci = R.chunk_end; ci-- > R.chunk_beg;) {
-      if (kSel && !(U.chunk_cells[ci] & want)) continue;     // no cell of this chunk takes a step of its own length
-      eliminate_chunk<kSel>(U, cs, dt, load_chunk(U.chunks + ci), lane, fout, invdout, cx, csig);
+    for (int w = warp; w < U.n_warp; w += n_warps) {
+      const FRun R = U.runs[lvl * U.n_warp + w];
+      double cx = 1.0, csig = 0.0;
+      const unsigned long long want = kSel == 1 ? U.masks[1] : (kSel == 2 ? U.masks[0] : ~0ull);
+      for (uint32_t ci = R.chunk_end; ci-- > R.chunk_beg;) {
+        if (kSel && !(U.chunk_cells[ci] & want)) continue;     // no cell of this chunk takes a step of its own length
+        eliminate_chunk<kSel>(U, cs, dt, load_chunk(U.chunks + ci), lane, fout, invdout, cx, csig);
+      }
     }
     level_sync((U.flags & UNIT_WARP_CELLS) != 0);
   }
@@ -314,8 +318,9 @@ __device__ __noinline__ Gates hh_gates(double v, double delta, double m, double 
 // the instruction cache): cells may be inactive (mode 0) or on an event-split sub-step of their own length
 // (mode 2).
 // ------------------------------------------------------------------------------------------
-template <bool kLin>
+template <bool kLin, int kW>
 __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U, const CellS& cs, double dt, const bool kGen) {
+  constexpr int kT = 32 * kW;              // threads of the CTA (shadows the factor kernels' constant)
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const bool multi = U.n_cell > 1;
   const uint32_t n_hh = U.n_hh, n_syn = U.n_syn, n_cl = U.n_clamp;
@@ -529,7 +534,7 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
 // A.nk grid steps of one forest.  Phase A: deliver the events due now and choose each cell's
 // sub-step (reading R9), then the step itself.
 // ------------------------------------------------------------------------------------------
-template <bool kLin>
+template <bool kLin, int kW>
 __device__ __forceinline__ void run_forest(const DevModel& M, const StepArgs& A, const FView& U, const CellS& cs,
                                            unsigned& n_sub, unsigned& n_del) {
   uint32_t* sMaskW = (uint32_t*)U.masks;     // the two 64-bit masks as four words (little endian)
@@ -579,7 +584,7 @@ __device__ __forceinline__ void run_forest(const DevModel& M, const StepArgs& A,
       const int any_active = __syncthreads_or(active);
       if (!any_active) break;
       const int general = __syncthreads_or(!plain);
-      forest_substep<kLin>(M, U, cs, A.dt, general != 0);
+      forest_substep<kLin, kW>(M, U, cs, A.dt, general != 0);
     }
   }
   if ((uint32_t)tid < n_cell) {
@@ -592,8 +597,8 @@ __device__ __forceinline__ void run_forest(const DevModel& M, const StepArgs& A,
 // ------------------------------------------------------------------------------------------
 // The cable step for forests: one CTA per forest of launch class `cls`.
 // ------------------------------------------------------------------------------------------
-template <bool kLin>
-__global__ void __launch_bounds__(kForestThreads, 8) cable_forest_kernel(DevModel M, StepArgs A, int cls) {
+template <bool kLin, int kW>
+__global__ void __launch_bounds__(32 * kW, 32 / kW) cable_forest_kernel(DevModel M, StepArgs A, int cls) {
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ UnitHeader H;
   __shared__ __align__(8) uint64_t mbar_mem;
@@ -626,7 +631,7 @@ __global__ void __launch_bounds__(kForestThreads, 8) cable_forest_kernel(DevMode
   U.xI = (double*)(smem + P.off_xi);
   const CellS cs = carve_cells(smem + P.off_cell, U.n_cell);
   unsigned n_sub = 0, n_del = 0;
-  run_forest<kLin>(M, A, U, cs, n_sub, n_del);
+  run_forest<kLin, kW>(M, A, U, cs, n_sub, n_del);
   // ---- state record -> HBM (one bulk store)
   fence_proxy_async();
   __syncthreads();
@@ -700,7 +705,8 @@ __global__ void __launch_bounds__(kForestThreads) forest_init_kernel(DevModel M)
 }  // namespace
 
 cudaError_t configure_forest_kernel(int max_optin_bytes) {
-  for (const void* k : {(const void*)cable_forest_kernel<false>, (const void*)cable_forest_kernel<true>}) {
+  for (const void* k : {(const void*)cable_forest_kernel<false, kForestWarps>, (const void*)cable_forest_kernel<true, kForestWarps>,
+                        (const void*)cable_forest_kernel<false, kForestWarpsBig>, (const void*)cable_forest_kernel<true, kForestWarpsBig>}) {
     cudaFuncAttributes fa;
     cudaError_t e = cudaFuncGetAttributes(&fa, k);
     if (e != cudaSuccess) return e;
@@ -727,8 +733,14 @@ cudaError_t launch_forest_init(const DevModel& M, cudaStream_t s) {
 cudaError_t launch_forest_cable(const DevModel& M, const StepArgs& A, int cls, cudaStream_t s, int* launches) {
   const ForestClass& K = M.fcls[cls];
   if (K.count == 0) return cudaSuccess;
-  if (!M.linearised) cable_forest_kernel<false><<<(unsigned)K.count, kForestThreads, K.plan.bytes, s>>>(M, A, cls);
-  else cable_forest_kernel<true><<<(unsigned)K.count, kForestThreads, K.plan.bytes, s>>>(M, A, cls);
+  const unsigned n = (unsigned)K.count, b = K.plan.bytes;
+  if (K.n_warp == kForestWarps) {
+    if (!M.linearised) cable_forest_kernel<false, kForestWarps><<<n, 32 * kForestWarps, b, s>>>(M, A, cls);
+    else cable_forest_kernel<true, kForestWarps><<<n, 32 * kForestWarps, b, s>>>(M, A, cls);
+  } else {
+    if (!M.linearised) cable_forest_kernel<false, kForestWarpsBig><<<n, 32 * kForestWarpsBig, b, s>>>(M, A, cls);
+    else cable_forest_kernel<true, kForestWarpsBig><<<n, 32 * kForestWarpsBig, b, s>>>(M, A, cls);
+  }
   if (launches) ++*launches;
   return cudaGetLastError();
 }

@@ -25,7 +25,7 @@
 //
 // A forest reuses the unit records of unit_layout.h (UnitHeader, fast / state / gen records with the
 // same offset functions); only the tree record differs (FTopoOff below):
-//   n_lane = branches, n_task = chunks, n_level = levels of the deepest cell.
+//   n_lane = branches, n_task = chunks, n_level = levels of the deepest cell; pad[2] = warps that sweep the forest.
 #pragma once
 #include <stdint.h>
 
@@ -33,7 +33,10 @@
 
 namespace arbb {
 
-constexpr int kForestWarps = 4;                      // warps per CTA of the forest kernel
+constexpr int kForestWarps = 4;                      // warps per CTA of the forest kernel: forests of launch class 0 ...
+constexpr int kForestWarpsBig = 8;                   // ... and of the classes above it (one large cell each: twice the warps
+                                                     // halve the serial part of its step; measured on C4: 338 -> 251 us)
+constexpr int kForestMaxWarps = 8;
 constexpr int kForestThreads = kForestWarps * 32;
 constexpr uint32_t kForestMaxCells = 64;             // cells per forest (one thread per cell keeps its runtime)
 constexpr uint32_t kForestMaxBranchLen = 32768;      // longer chains are cut (len is stored in 16 bits)
@@ -75,12 +78,12 @@ struct FOffs {
   uint32_t pad[23];
 };
 static_assert(sizeof(FOffs) == 256, "FOffs must be 256 bytes");
-ARBB_HD FTopoOff ftopo_offsets(uint32_t n_level, uint32_t n_chunk, uint32_t n_branch, uint32_t n_child, uint32_t n_cell) {
+ARBB_HD FTopoOff ftopo_offsets(uint32_t n_level, uint32_t n_chunk, uint32_t n_branch, uint32_t n_child, uint32_t n_cell, uint32_t n_warp) {
   FTopoOff o;
   uint32_t p = 0;
   auto sec = [&](uint32_t bytes) { uint32_t at = p; p = align_up(p + bytes, 16); return at; };
   o.offs = sec((uint32_t)sizeof(FOffs));
-  o.runs = sec(n_level * (uint32_t)kForestWarps * (uint32_t)sizeof(FRun));
+  o.runs = sec(n_level * n_warp * (uint32_t)sizeof(FRun));
   o.chunks = sec(n_chunk * (uint32_t)sizeof(FChunk));
   o.chunk_cells = sec(n_chunk * 8);                  // uint64: bit c = the chunk holds control volumes of cell c
   o.branches = sec(n_branch * (uint32_t)sizeof(FBranch));
@@ -109,8 +112,8 @@ ARBB_HD ForestSmemPlan forest_smem_plan(const ForestCaps& c) {
 }
 // upper bound of a tree record's size from counts known before the forest is built
 ARBB_HD uint32_t ftopo_bound(uint32_t n_cv, uint32_t n_branch, uint32_t n_cell) {
-  const uint32_t n_level = n_branch, n_chunk = n_cv / 32 + (uint32_t)kForestWarps * n_level + 1;
-  return ftopo_offsets(n_level, n_chunk, n_branch, n_branch, n_cell).total;
+  const uint32_t n_level = n_branch, n_chunk = n_cv / 32 + (uint32_t)kForestMaxWarps * n_level + 1;
+  return ftopo_offsets(n_level, n_chunk, n_branch, n_branch, n_cell, (uint32_t)kForestMaxWarps).total;
 }
 // shared-memory budget of launch class k (bytes per CTA so that 8 >> k CTAs share an SM's 227 KB)
 // (1 KB per CTA is reserved by the system; the kernel's static shared memory is below 1 KB)
@@ -118,6 +121,7 @@ ARBB_HD uint32_t forest_class_budget(int k) { return ((227u * 1024u) >> (3 - k))
 
 struct ForestClass {     // one launch: forests [first, first + count) of the unit list
   int64_t first, count;
+  int n_warp;            // warps per CTA of the launch
   ForestSmemPlan plan;
 };
 

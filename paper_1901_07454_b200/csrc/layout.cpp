@@ -170,6 +170,7 @@ struct UnitBuilder {
   bool bad = false;                        // a count does not fit its field
   // forests (forest_layout.h)
   bool forest = false, warp_cells = false;
+  int n_warp = kForestWarps;               // warps that sweep the forest (kForestWarps or kForestWarpsBig)
   std::vector<uint32_t> fslot0, flevel_br;
   std::vector<FRun> fruns;
   std::vector<FChunk> fchunks;
@@ -288,33 +289,33 @@ struct UnitBuilder {
       std::vector<uint32_t> by_size(cells.size());
       for (uint32_t c = 0; c < cells.size(); ++c) by_size[c] = c;
       std::stable_sort(by_size.begin(), by_size.end(), [&](uint32_t x, uint32_t y) { return ccv[x] > ccv[y]; });
-      uint64_t wl[kForestWarps] = {0};
+      uint64_t wl[kForestMaxWarps] = {0};
       for (uint32_t c : by_size) {
         int best = 0;
-        for (int w = 1; w < kForestWarps; ++w) if (wl[w] < wl[best]) best = w;
+        for (int w = 1; w < n_warp; ++w) if (wl[w] < wl[best]) best = w;
         cell_warp[c] = (uint32_t)best;
         wl[best] += ccv[c];
       }
     }
-    fruns.assign((size_t)n_level * kForestWarps, FRun{0, 0});
+    fruns.assign((size_t)n_level * n_warp, FRun{0, 0});
     uint32_t slot = 0;
     for (uint32_t lvl = 0; lvl < n_level; ++lvl) {
       flevel_br.push_back((uint32_t)order.size());
       auto& v = by_level[lvl];
       std::stable_sort(v.begin(), v.end(), [&](uint32_t x, uint32_t y) { return lanes[x].len > lanes[y].len; });
-      std::vector<uint32_t> dealt[kForestWarps];
-      uint64_t load[kForestWarps] = {0};
+      std::vector<uint32_t> dealt[kForestMaxWarps];
+      uint64_t load[kForestMaxWarps] = {0};
       for (uint32_t i : v) {               // longest first onto the least loaded warp - or to the warp that owns the cell
         int best = 0;
         if (warp_cells) best = (int)cell_warp[lanes[i].lc];
-        else for (int w = 1; w < kForestWarps; ++w) if (load[w] < load[best]) best = w;
+        else for (int w = 1; w < n_warp; ++w) if (load[w] < load[best]) best = w;
         dealt[best].push_back(i);
         load[best] += lanes[i].len;
       }
-      for (int w = 0; w < kForestWarps; ++w) {
+      for (int w = 0; w < n_warp; ++w) {
         // branches of one cell next to each other: a pass in which few cells are active skips whole chunks
         std::stable_sort(dealt[w].begin(), dealt[w].end(), [&](uint32_t x, uint32_t y) { return lanes[x].lc < lanes[y].lc; });
-        FRun& R = fruns[(size_t)lvl * kForestWarps + w];
+        FRun& R = fruns[(size_t)lvl * n_warp + w];
         R.chunk_beg = (uint32_t)fchunks.size();
         const uint32_t pos0 = (uint32_t)order.size(), slot_beg = slot;
         for (uint32_t i : dealt[w]) { order.push_back(i); fslot0.push_back(slot); slot += lanes[i].len; }
@@ -403,7 +404,7 @@ struct UnitBuilder {
       uc.flags |= UNIT_FOREST | (disjoint ? UNIT_POINT_DISJOINT : 0u) | (warp_cells ? UNIT_WARP_CELLS : 0u);
     }
     if (topo_out && forest) {
-      const FTopoOff to = ftopo_offsets(uc.n_level, uc.n_task, n_lane, n_child, n_cell);
+      const FTopoOff to = ftopo_offsets(uc.n_level, uc.n_task, n_lane, n_child, n_cell, (uint32_t)n_warp);
       topo_out->assign(to.total, 0);
       uint8_t* tp = topo_out->data();
       {
@@ -525,6 +526,7 @@ struct UnitBuilder {
     hd.topo_off = uc.topo_off; hd.gen_base = uc.gen_base; hd.state_base = uc.state_base;
     hd.cell_base = uc.cell_base; hd.scratch_base = uc.scratch_base;
     hd.pad[0] = (uint32_t)(uc.lane_base & 0xFFFFFFFFu); hd.pad[1] = (uint32_t)((uint64_t)uc.lane_base >> 32);
+    hd.pad[2] = (uint32_t)n_warp;
     std::memcpy(fast, &hd, sizeof hd);
     double* hh_gna = (double*)(fast + fo.hh_gna);
     double* hh_gk = (double*)(fast + fo.hh_gk);
@@ -1022,6 +1024,22 @@ int build(const arb_desc& d_in, const BuildParams& P, bool fill, HostModel& H, s
     B.forest = u < H.n_forests;
     H.units[u] = B.run(unit_begin[u], unit_cells[u], &topo[u], nullptr, nullptr);
     H.units[u].topo_bytes = (uint32_t)topo[u].size();
+    if (B.forest) {
+      // a forest beyond launch class 0 (one large cell) is swept by twice the warps (forest_layout.h)
+      const UnitCounts& uc = H.units[u];
+      ForestCaps fc;
+      fc.state_bytes = uc.state_bytes; fc.topo_bytes = uc.topo_bytes; fc.n_branch = uc.n_lane; fc.n_spec = uc.n_hh + uc.n_syn + uc.n_clamp; fc.n_cell = uc.n_cell;
+      if (forest_smem_plan(fc).bytes > forest_class_budget(0)) {
+        UnitBuilder B2{d, P, H, clamp_off, clamp_idx, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, false};
+        B2.forest = true; B2.n_warp = kForestWarpsBig;
+        H.units[u] = B2.run(unit_begin[u], unit_cells[u], &topo[u], nullptr, nullptr);
+        H.units[u].topo_bytes = (uint32_t)topo[u].size();
+        H.units[u].n_warp = kForestWarpsBig;
+        if (B2.bad) too_many.store(1);
+      } else {
+        H.units[u].n_warp = kForestWarps;
+      }
+    }
     if (u >= H.n_forests) H.units[u].flags |= UNIT_BLOCK;
     if (H.units[u].n_level > 60000 || H.units[u].n_slot > 0x3FFFFFFFu) too_many.store(1);
     if (B.bad) too_many.store(1);
@@ -1060,7 +1078,7 @@ int build(const arb_desc& d_in, const BuildParams& P, bool fill, HostModel& H, s
     }
     for (int64_t i = 0; i < H.n_forests; ++i) topo[i].swap(topo2[i]);
     H.units.swap(units2); unit_begin.swap(begin2); unit_cells.swap(cells2);
-    for (int k = 0; k < kForestClasses; ++k) { H.fcls[k].first = 0; H.fcls[k].count = 0; }
+    for (int k = 0; k < kForestClasses; ++k) { H.fcls[k].first = 0; H.fcls[k].count = 0; H.fcls[k].n_warp = k == 0 ? kForestWarps : kForestWarpsBig; }
     for (int k = 0; k < kForestClasses; ++k) H.fcls[k].plan = forest_smem_plan(ForestCaps{0, 0, 0, 0, 0});
     for (int64_t i = 0; i < H.n_forests; ++i) {
       const UnitCounts& uc = H.units[i];
@@ -1305,6 +1323,7 @@ int build(const arb_desc& d_in, const BuildParams& P, bool fill, HostModel& H, s
     UnitBuilder B{d, P, H, clamp_off, clamp_idx, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, {}, false};
     B.forest = u < H.n_forests;
     UnitCounts placed = H.units[u];
+    if (B.forest) B.n_warp = placed.n_warp;
     B.run(unit_begin[u], unit_cells[u], nullptr, &placed, &H);
   });
   // point cells

@@ -38,6 +38,7 @@ struct UnitCounts {                   // everything the offset functions need
   int64_t cell_base = 0, lane_base = 0, hh_base = 0;
   int64_t fast_off = 0, state_base = 0, gen_base = 0, topo_off = 0, scratch_base = -1;
   uint32_t fast_bytes = 0, state_bytes = 0, topo_bytes = 0;
+  int n_warp = 0;                     // forests: warps that sweep the unit (forest_layout.h)
 };
 
 struct HostModel {
