@@ -461,6 +461,9 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
     FChunk ck;
     uint32_t cur = next(R.chunk_end);
     if (cur != kNone) fetch(cur, ck, f, invd);
+    // the barrier that ends the level below comes AFTER this level's first loads have been issued (they do not
+    // depend on what other warps wrote): their L2 latency overlaps the wait
+    if (lvl != (int)U.n_level - 1) level_sync(warp_cells);
     while (cur != kNone) {
       const uint32_t nx = next(cur);
       FChunk nck = ck;
@@ -469,7 +472,6 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
       backward_chunk(U, cs, ck, f, invd, lane, kGen && (U.chunk_cells[cur] & odd) != 0ull, lin, cf, cr);
       cur = nx; ck = nck; f = nf; invd = ni;
     }
-    level_sync(warp_cells);
   }
   for (uint32_t lvl = 0; lvl < U.n_level; ++lvl) {
     const FRun R = U.runs[lvl * kW + warp];
@@ -485,6 +487,7 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
     FChunk ck;
     uint32_t cur = next(R.chunk_beg);
     if (cur != kNone) fetch(cur, ck, f);
+    level_sync(warp_cells);                // ends the level above (for the root level: the backward sweep)
     while (cur != kNone) {
       const uint32_t nx = next(cur + 1);
       FChunk nck = ck;
@@ -493,9 +496,8 @@ __device__ __forceinline__ void forest_substep(const DevModel& M, const FView& U
       forward_chunk(U, cs, ck, f, lane, kGen && (U.chunk_cells[cur] & odd) != 0ull, lin, cv);
       cur = nx; ck = nck; f = nf;
     }
-    level_sync(warp_cells);
   }
-  if (warp_cells) __syncthreads();
+  __syncthreads();
 
   // ---- F: state update with V', threshold test
   for (uint32_t i = tid; i < n_hh; i += kT) {
@@ -540,6 +542,7 @@ __device__ __forceinline__ void run_forest(const DevModel& M, const StepArgs& A,
   uint32_t* sMaskW = (uint32_t*)U.masks;     // the two 64-bit masks as four words (little endian)
   const int tid = threadIdx.x;
   const uint32_t n_cell = U.n_cell;
+  bool gen_in_l2 = false;
   if ((uint32_t)tid < n_cell) {
     const unsigned long long pk = (unsigned long long)__double_as_longlong(U.rt[kRtDoubles * tid + 1]);
     cs.evcur[tid] = (uint32_t)pk; cs.evend[tid] = (uint32_t)(pk >> 32);
@@ -584,6 +587,10 @@ __device__ __forceinline__ void run_forest(const DevModel& M, const StepArgs& A,
       const int any_active = __syncthreads_or(active);
       if (!any_active) break;
       const int general = __syncthreads_or(!plain);
+      if (general && !gen_in_l2) {             // the dt-independent arrays (C, S, sigma, G, G e) of the re-elimination: cold in HBM until now
+        if (tid == 0) bulk_prefetch_l2(U.C, 8u * 5u * U.n_slot);
+        gen_in_l2 = true;
+      }
       forest_substep<kLin, kW>(M, U, cs, A.dt, general != 0);
     }
   }
