@@ -361,9 +361,18 @@ def run_ours(args):
     if sm is not None:           # every epoch: integrate, then exchange the epoch's spikes (inside the timed region)
         _adv = g.advance
         def _advance_and_exchange(t, dt):
+            if args.overlap:             # half-epoch exchange intervals, the all-gather hidden behind the next half-epoch
+                g.advance = _adv         # (the sharded loop calls the model's own advance)
+                try:
+                    sm.t = g.time()
+                    sm.advance(t, dt)
+                finally:
+                    g.advance = _advance_and_exchange
+                return
             _adv(t, dt)
             sm.exchange()
         g.advance = _advance_and_exchange
+        sm.overlap = bool(args.overlap)
     fused_steps = {"stream": 1, "fused": 0}
     g.set_option(B.ARB_OPT_FUSED_STEPS, fused_steps[args.mode])
     if lin:
@@ -529,7 +538,7 @@ def run_ours(args):
             "data": "synthetic",
             "config": {"workload": "%s (%d CVs), dt 0.025 ms; step = one epoch of %d grid steps" % (label, n_cv, es),
                        "mode": args.mode, "step_kind": args.step, "cells_per_gpu": cells,
-                       "parallelism": ("one network, cells sharded by rank, spikes all-gathered once per epoch" if args.exchange
+                       "parallelism": (("one network, cells sharded by rank, spikes all-gathered every half epoch behind the next half-epoch's integration" if args.overlap else "one network, cells sharded by rank, spikes all-gathered once per epoch") if args.exchange
                                        else "cells sharded, no collective (one closed network per rank)"), "layout": layout, "layout_options": dict(B.LAYOUT_DEFAULTS),
                        "l2": ("no flush needed: each grid step streams %.2f GB >> 126 MB L2" % (alg_step / 1e9)) if alg_step > 4e8
                              else "working set of %.1f MB per grid step is L2-resident; no flush (every step rewrites the whole state)" % (alg_step / 1e6),
@@ -584,6 +593,9 @@ def main():
                     help="config 3, N > 1: the ranks share ONE network of N x cells cells (cells sharded, connections by destination "
                          "owner) and all-gather their spikes once per epoch (paper_1901_07454_b200/sharded.py, SURVEY.md 8(f) NEXT-3) "
                          "instead of integrating one closed network each")
+    ap.add_argument("--overlap", action="store_true",
+                    help="with --exchange: exchange every half epoch and hide the all-gather behind the next half-epoch's "
+                         "integration (PAPER.md:96, 200)")
     ap.add_argument("--layout", action="append", default=[], metavar="KEY=VALUE",
                     help="arb_desc layout / capacity option, e.g. layout_forest_cv=2048 (default: the library's)")
     ap.add_argument("--selftest-dist", action="store_true", help=argparse.SUPPRESS)
