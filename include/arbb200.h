@@ -121,8 +121,10 @@ typedef struct {
    *                           (lane = cell) when their topology class has at least this many cells
    *                           (default 4; 1 = every cell in groups; >= 2^31 = no groups)
    *   layout_forest_cv        cells that do not share their tree are packed into forests of up to this
- *                           many control volumes, one CTA each (default 1024; a larger cell is a forest
- *                           of its own)
+   *                           many control volumes, one CTA each (default: 2048, less for models of fewer than 1.2e6 such
+   *                           control volumes so that they spread over the SMs, and never more than fits the
+   *                           27 KB of shared memory of the smallest launch class; a larger cell is a
+   *                           forest of its own)
    *   cap_spikes              entries of the device spike buffer.  arb_advance drains it into host
    *                           memory at least every 2,000 grid steps, so it bounds the spikes of
    *                           such a stretch, not of the run (default max(2^20, 64 n_cells))

@@ -180,7 +180,7 @@ cudaError_t upload(arb_model* m, const Region& r, const std::vector<T>& v) {
 // layout options travel in the description (no process-wide state)
 int params_of(const arb_desc& d, BuildParams& P, std::string& err) {
   if (d.layout_group_min_cells < 0 || d.layout_forest_cv < 0 || d.cap_spikes < 0 || d.cap_events < 0) { err = "negative layout / capacity option"; return ARB_E_INVALID; }
-  if (d.layout_forest_cv > 0) P.forest_cv = (uint32_t)std::min<int64_t>(d.layout_forest_cv, 1 << 20);
+  if (d.layout_forest_cv > 0) { P.forest_cv = (uint32_t)std::min<int64_t>(d.layout_forest_cv, 1 << 20); P.forest_cv_auto = false; }
   if (d.layout_group_min_cells > 0) P.group_min_cells = d.layout_group_min_cells >= 0x7FFFFFFF ? 0u : (uint32_t)d.layout_group_min_cells;
   return ARB_OK;
 }

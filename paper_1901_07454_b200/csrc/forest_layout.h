@@ -110,10 +110,11 @@ ARBB_HD ForestSmemPlan forest_smem_plan(const ForestCaps& c) {
   P.bytes = align_up(p, 128);
   return P;
 }
-// upper bound of a tree record's size from counts known before the forest is built
-ARBB_HD uint32_t ftopo_bound(uint32_t n_cv, uint32_t n_branch, uint32_t n_cell) {
-  const uint32_t n_level = n_branch, n_chunk = n_cv / 32 + (uint32_t)kForestMaxWarps * n_level + 1;
-  return ftopo_offsets(n_level, n_chunk, n_branch, n_branch, n_cell, (uint32_t)kForestMaxWarps).total;
+// upper bound of a tree record's size from counts known before the forest is built (n_level: levels of its deepest cell;
+// every (level, warp) run ends in at most one partly filled chunk)
+ARBB_HD uint32_t ftopo_bound(uint32_t n_cv, uint32_t n_branch, uint32_t n_cell, uint32_t n_warp, uint32_t n_level) {
+  const uint32_t n_chunk = n_cv / 32 + n_warp * n_level + 1;
+  return ftopo_offsets(n_level, n_chunk, n_branch, n_branch, n_cell, n_warp).total;
 }
 // shared-memory budget of launch class k (bytes per CTA so that 8 >> k CTAs share an SM's 227 KB)
 // (1 KB per CTA is reserved by the system; the kernel's static shared memory is below 1 KB)

@@ -876,7 +876,7 @@ int build(const arb_desc& d_in, const BuildParams& P, bool fill, HostModel& H, s
     for (int64_t k = 0; k < d.n_clamp; ++k) clamp_idx[cur[d.clamp_cell[k]]++] = k;
   }
   // HH instances and branches (maximal unbranched chains) of every cell
-  std::vector<uint32_t> cell_hh(nc, 0), cell_nbr(nc, 0);
+  std::vector<uint32_t> cell_hh(nc, 0), cell_nbr(nc, 0), cell_lvl(nc, 0);   // ..., branch levels of the cell's tree
   parallel_for(nc, [&](int64_t c) {
     const int64_t a = d.cv_off[c], n = d.cv_off[c + 1] - a;
     uint32_t nh = 0;
@@ -888,14 +888,22 @@ int build(const arb_desc& d_in, const BuildParams& P, bool fill, HostModel& H, s
     uint32_t nb = 1;
     for (int64_t i = 1; i < n; ++i) nb += nchild[d.cv_parent[a + i]] != 1;
     cell_nbr[c] = nb + (uint32_t)(n / kForestMaxBranchLen);     // chains longer than a branch may hold are cut
+    std::vector<uint32_t> lvl((size_t)n, 0);
+    uint32_t deepest = 0;
+    for (int64_t i = 1; i < n; ++i) {
+      const int64_t p = d.cv_parent[a + i];
+      lvl[i] = lvl[p] + (nchild[p] != 1 ? 1u : 0u);
+      deepest = std::max(deepest, lvl[i]);
+    }
+    cell_lvl[c] = deepest + 1 + (uint32_t)(n / kForestMaxBranchLen);
   });
   // shared memory a forest of these counts needs (forest_layout.h)
-  auto forest_need = [&](uint64_t n_cv, uint64_t n_br, uint64_t n_hh, uint64_t n_syn, uint64_t n_clamp, uint64_t n_cell) -> uint64_t {
+  auto forest_need = [&](uint64_t n_cv, uint64_t n_br, uint64_t n_hh, uint64_t n_syn, uint64_t n_clamp, uint64_t n_cell, int n_warp, uint32_t n_level) -> uint64_t {
     if (n_cv > 0x0FFFFFFFull || n_syn > 0x0FFFFFFFull || n_clamp > 0x0FFFFFFFull) return ~0ull;
     ForestCaps fc;
     fc.state_bytes = 8 * state_offsets(align_up((uint32_t)n_cv, 2), (uint32_t)n_hh, (uint32_t)n_syn, (uint32_t)n_cell).total;
     fc.n_branch = (uint32_t)n_br; fc.n_spec = (uint32_t)(n_hh + n_syn + n_clamp); fc.n_cell = (uint32_t)n_cell;
-    fc.topo_bytes = ftopo_bound((uint32_t)n_cv, (uint32_t)n_br, (uint32_t)n_cell);
+    fc.topo_bytes = ftopo_bound((uint32_t)n_cv, (uint32_t)n_br, (uint32_t)n_cell, (uint32_t)n_warp, n_level);
     return forest_smem_plan(fc).bytes;
   };
   auto cell_counts = [&](int64_t c, uint64_t& n_cv, uint64_t& n_syn, uint64_t& n_cl) {
@@ -978,7 +986,7 @@ int build(const arb_desc& d_in, const BuildParams& P, bool fill, HostModel& H, s
     uint64_t n_cv, n_syn, n_cl;
     cell_counts(c, n_cv, n_syn, n_cl);
     const bool fits = n_cv <= P.forest_max_cv && n_syn < P.forest_max_syn &&
-                      forest_need(n_cv, cell_nbr[c], cell_hh[c], n_syn, n_cl, 1) <= forest_class_budget(kForestClasses - 1);
+                      forest_need(n_cv, cell_nbr[c], cell_hh[c], n_syn, n_cl, 1, kForestMaxWarps, cell_lvl[c]) <= forest_class_budget(kForestClasses - 1);
     (fits ? forest_cells : block_cells).push_back((uint32_t)c);
   }
   auto bigger = [&](uint32_t x, uint32_t y) { return d.cv_off[x + 1] - d.cv_off[x] > d.cv_off[y + 1] - d.cv_off[y]; };
@@ -997,14 +1005,22 @@ int build(const arb_desc& d_in, const BuildParams& P, bool fill, HostModel& H, s
   std::vector<int64_t> unit_begin;
   {
     uint64_t cv = 0, br = 0, hh = 0, syn = 0, cl = 0, cells = 0;
+    uint32_t lv = 0;
+    uint64_t forest_cv = P.forest_cv;
+    if (P.forest_cv_auto) {                // few control volumes in all: more, smaller forests (measured on the paper's ring cell,
+      uint64_t total = 0;                  // 2.6e5 CVs: forests of 256 / 384 / 512 / 1,024 CVs 0.033 / 0.0225 / 0.0227 / 0.027 ms per step)
+      for (uint32_t c : forest_cells) total += (uint64_t)(d.cv_off[c + 1] - d.cv_off[c]);
+      forest_cv = std::min<uint64_t>(P.forest_cv, std::max<uint64_t>(384, total / (4 * 148)));
+    }
     for (int64_t i = 0; i < (int64_t)forest_cells.size(); ++i) {
       uint64_t n_cv, n_syn, n_cl;
       cell_counts(forest_cells[i], n_cv, n_syn, n_cl);
       const uint64_t n_hh = cell_hh[forest_cells[i]], n_br = cell_nbr[forest_cells[i]];
-      if (cells == 0 || cells >= kForestMaxCells || cv + n_cv > P.forest_cv ||
-          forest_need(cv + n_cv + 1, br + n_br, hh + n_hh, syn + n_syn, cl + n_cl, cells + 1) > forest_class_budget(0)) {
-        unit_begin.push_back(ngc + i); cv = br = hh = syn = cl = cells = 0;
+      if (cells == 0 || cells >= kForestMaxCells || cv + n_cv > forest_cv ||
+          forest_need(cv + n_cv + 1, br + n_br, hh + n_hh, syn + n_syn, cl + n_cl, cells + 1, kForestWarps, std::max(lv, cell_lvl[forest_cells[i]])) > forest_class_budget(0)) {
+        unit_begin.push_back(ngc + i); cv = br = hh = syn = cl = cells = 0; lv = 0;
       }
+      lv = std::max(lv, cell_lvl[forest_cells[i]]);
       cv += n_cv; br += n_br; hh += n_hh; syn += n_syn; cl += n_cl; ++cells;
     }
     H.n_forests = (int64_t)unit_begin.size();

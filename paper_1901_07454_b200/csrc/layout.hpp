@@ -14,7 +14,9 @@
 namespace arbb {
 
 struct BuildParams {
-  uint32_t forest_cv = 1024;      // cells are packed into forests of up to this many control volumes (larger cells
+  bool forest_cv_auto = true;     // a small model gets smaller forests, so that it still spreads over the SMs: forests of
+                                  // (control volumes in forests) / (4 x 148 SMs) control volumes, at least 384, at most forest_cv
+  uint32_t forest_cv = 2048;      // cells are packed into forests of up to this many control volumes (larger cells
                                   // are a forest of their own)
   uint32_t forest_max_cv = 24000; // cells with more control volumes do not fit a CTA's shared memory: block units
   uint32_t forest_max_syn = 1024; // cells with at least this many synapses are block units (key reduction)
