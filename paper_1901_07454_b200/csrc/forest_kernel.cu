@@ -154,8 +154,8 @@ __device__ __forceinline__ void eliminate_chunk(const FView& U, const CellS* cs,
   Mob m;
   if (!valid || tail) {
     double x = c;
-    if (valid) {
-      const FBranch B = load_branch(U.br + br);
+    if (valid && on) {                     // (a cell that sits this pass out has no fresh contributions: what the array holds
+      const FBranch B = load_branch(U.br + br);      //  for it may be anything, and 0 x NaN would reach its neighbours in the scan)
       for (uint32_t j = 0; j < B.ccnt; ++j) x += U.dcon[U.child[B.cbeg + j]];
     }
     m.a = 0.0; m.b = x; m.c = 0.0; m.d = 1.0;                     // constant map: the chain ends here
@@ -635,6 +635,8 @@ __global__ void __launch_bounds__(32 * kW, 32 / kW) cable_forest_kernel(DevModel
   make_fview(U, M, H, fast, Ss, smem + P.off_topo);
   U.masks = sMask;
   U.con = (double*)(smem + P.off_con);
+  U.dcon = U.con;                            // re-eliminations hand a branch's share to its parent through shared memory too (the
+                                             // sweeps, which use the same array, come after them)
   U.xI = (double*)(smem + P.off_xi);
   const CellS cs = carve_cells(smem + P.off_cell, U.n_cell);
   unsigned n_sub = 0, n_del = 0;
