@@ -133,7 +133,8 @@ __device__ __forceinline__ void mob_normalise(Mob& m) {
 // forest_substep has assembled C_k/delta + G_k + sum of the point mechanisms' conductances.
 template <int kSel>
 __device__ __forceinline__ void eliminate_chunk(const FView& U, const CellS* cs, double dt, const FChunk& ck, int lane,
-                                                double* fout, double* invdout, double& cx, double& csig) {
+                                                double* fout, double* invdout, double& cb, double& cd, double& csig) {
+  // cb / cd: x of the first control volume of the chunk swept before this one (where a branch may continue), csig its sigma
   const int n = (int)(ck.br_n & 63u);
   const bool valid = lane < n;
   const uint32_t s = ck.slot0 + lane;
@@ -160,7 +161,8 @@ __device__ __forceinline__ void eliminate_chunk(const FView& U, const CellS* cs,
     }
     m.a = 0.0; m.b = x; m.c = 0.0; m.d = 1.0;                     // constant map: the chain ends here
   } else if (lane == n - 1) {
-    m.a = 0.0; m.b = c + csig * cx / (cx + csig); m.c = 0.0; m.d = 1.0;   // the branch continues in the chunk swept before
+    // the branch continues in the chunk swept before: T(cb / cd) with T(x) = ((c + s) x + c s) / (x + s), s = csig - no division
+    m.a = 0.0; m.b = fma(c + csig, cb, c * csig * cd); m.c = 0.0; m.d = fma(csig, cd, cb);
   } else {
     m.a = c + snext; m.b = c * snext; m.c = 1.0; m.d = snext;
   }
@@ -174,18 +176,19 @@ __device__ __forceinline__ void eliminate_chunk(const FView& U, const CellS* cs,
       p.a = fma(m.a, r.a, m.b * r.c); p.b = fma(m.a, r.b, m.b * r.d);
       p.c = fma(m.c, r.a, m.d * r.c); p.d = fma(m.c, r.b, m.d * r.d);
       m = p;
-      mob_normalise(m);
+      if (d == 2 || d == 8) mob_normalise(m);     // (two doublings from entries <= 1 stay far from overflow)
     }
   }
-  const double x = m.b / m.d;
-  const double dk = x + sg;
-  const double invd = 1.0 / dk;
+  // x = b / d, d_k = x + sigma: one reciprocal gives 1/d_k = d / (b + sigma d) and what the parent loses, sigma x / d_k
+  const double r = 1.0 / fma(sg, m.d, m.b);
+  const double invd = m.d * r;
   if (on) {
     fout[s] = -sg * invd;
     invdout[s] = invd;
-    if (head) U.dcon[br] = sg * x * invd;
+    if (head) U.dcon[br] = sg * m.b * r;
   }
-  cx = __shfl_sync(kFull, x, 0);
+  cb = __shfl_sync(kFull, m.b, 0);
+  cd = __shfl_sync(kFull, m.d, 0);
   csig = __shfl_sync(kFull, sg, 0);
 }
 
@@ -196,11 +199,11 @@ __device__ __forceinline__ void eliminate_forest(const FView& U, const CellS* cs
   for (int lvl = (int)U.n_level - 1; lvl >= 0; --lvl) {
     for (int w = warp; w < U.n_warp; w += n_warps) {
       const FRun R = U.runs[lvl * U.n_warp + w];
-      double cx = 1.0, csig = 0.0;
+      double cb = 1.0, cd = 1.0, csig = 0.0;
       const unsigned long long want = kSel == 1 ? U.masks[1] : (kSel == 2 ? U.masks[0] : ~0ull);
       for (uint32_t ci = R.chunk_end; ci-- > R.chunk_beg;) {
         if (kSel && !(U.chunk_cells[ci] & want)) continue;     // no cell of this chunk takes a step of its own length
-        eliminate_chunk<kSel>(U, cs, dt, load_chunk(U.chunks + ci), lane, fout, invdout, cx, csig);
+        eliminate_chunk<kSel>(U, cs, dt, load_chunk(U.chunks + ci), lane, fout, invdout, cb, cd, csig);
       }
     }
     level_sync((U.flags & UNIT_WARP_CELLS) != 0);
