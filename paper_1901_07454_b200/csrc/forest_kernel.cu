@@ -301,17 +301,31 @@ __device__ __forceinline__ void forward_chunk(const FView& U, const CellS& cs, c
 }
 
 // HH gate update x <- x_inf(V') + (x - x_inf) exp(-delta (alpha + beta)) (reading R5).  Not inlined:
-// the exp / expm1 / divide chains are ~1,000 instructions and the kernel has two call sites.
+// the exp / expm1 chains are several hundred instructions and the kernel has two call sites.  The six quotients of
+// the rates and steady states (two x / expm1(x), 1 / (1 + exp), three alpha / (alpha + beta)) share ONE division: the
+// reciprocal of their denominators' product, multiplied back (the kernel is bound by instruction issue, and a double
+// division is ~40 instructions); results differ from the quotient-by-quotient form in the last bits only.
 struct Gates { double m, h, n; };
 __device__ __noinline__ Gates hh_gates(double v, double delta, double m, double h, double n) {
-  const Rates r = hh_rates(v);
+  const double xm = -(v + 40.0) / 10.0, xn = -(v + 55.0) / 10.0;
+  const double em = xm == 0.0 ? 1.0 : expm1(xm), en = xn == 0.0 ? 1.0 : expm1(xn);       // (x = 0: x / expm1(x) -> 1)
+  const double eh = 1.0 + exp(-(v + 35.0) / 10.0);
+  const double bm = 4.0 * exp(-(v + 65.0) / 18.0), ah = 0.07 * exp(-(v + 65.0) / 20.0), bn = 0.125 * exp(-(v + 65.0) / 80.0);
+  // 1 / em, 1 / en, 1 / eh from one reciprocal
+  const double p2 = em * en, inv3 = 1.0 / (p2 * eh);
+  const double ieh = p2 * inv3, i2 = eh * inv3, iem = en * i2, ien = em * i2;
+  const double am = xm == 0.0 ? 1.0 : xm * iem, an = 0.1 * (xn == 0.0 ? 1.0 : xn * ien), bh = ieh;
+  // 1 / (am + bm), 1 / (ah + bh), 1 / (an + bn) from one reciprocal
+  const double sm = am + bm, sh = ah + bh, sn = an + bn;
+  const double q2 = sm * sh, jnv3 = 1.0 / (q2 * sn);
+  const double isn = q2 * jnv3, j2 = sn * jnv3, ism = sh * j2, ish = sm * j2;
   Gates g;
-  double inf = r.am / (r.am + r.bm);
-  g.m = inf + (m - inf) * exp(-delta * (r.am + r.bm));
-  inf = r.ah / (r.ah + r.bh);
-  g.h = inf + (h - inf) * exp(-delta * (r.ah + r.bh));
-  inf = r.an / (r.an + r.bn);
-  g.n = inf + (n - inf) * exp(-delta * (r.an + r.bn));
+  double inf = am * ism;
+  g.m = inf + (m - inf) * exp(-delta * sm);
+  inf = ah * ish;
+  g.h = inf + (h - inf) * exp(-delta * sh);
+  inf = an * isn;
+  g.n = inf + (n - inf) * exp(-delta * sn);
   return g;
 }
 
