@@ -157,7 +157,9 @@ __device__ __forceinline__ void eliminate_chunk(const FView& U, const CellS* cs,
     double x = c;
     if (valid && on) {                     // (a cell that sits this pass out has no fresh contributions: what the array holds
       const FBranch B = load_branch(U.br + br);      //  for it may be anything, and 0 x NaN would reach its neighbours in the scan)
-      for (uint32_t j = 0; j < B.ccnt; ++j) x += U.dcon[U.child[B.cbeg + j]];
+      const uint32_t nc = B.ccnt & 0x7FFFu;
+      if (B.ccnt & kFBranchInlineFlag) { if (nc >= 1) x += U.dcon[B.cbeg & 0xFFFFu]; if (nc == 2) x += U.dcon[B.cbeg >> 16]; }
+      else for (uint32_t j = 0; j < nc; ++j) x += U.dcon[U.child[B.cbeg + j]];
     }
     m.a = 0.0; m.b = x; m.c = 0.0; m.d = 1.0;                     // constant map: the chain ends here
   } else if (lane == n - 1) {
@@ -238,7 +240,9 @@ __device__ __forceinline__ void backward_chunk(const FView& U, const CellS& cs, 
     r = U.V[s];
     if (tail) {
       const FBranch B = load_branch(U.br + br);
-      for (uint32_t j = 0; j < B.ccnt; ++j) r -= U.con[U.child[B.cbeg + j]];
+      const uint32_t nc = B.ccnt & 0x7FFFu;
+      if (B.ccnt & kFBranchInlineFlag) { if (nc >= 1) r -= U.con[B.cbeg & 0xFFFFu]; if (nc == 2) r -= U.con[B.cbeg >> 16]; }
+      else for (uint32_t j = 0; j < nc; ++j) r -= U.con[U.child[B.cbeg + j]];
     }
   }
   const double fnext = __shfl_down_sync(kFull, f, 1);

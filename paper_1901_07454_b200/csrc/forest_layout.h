@@ -60,10 +60,12 @@ struct FChunk {          // 16 bytes, one broadcast load
 struct FBranch {         // 16 bytes, in slot order
   uint32_t slot0;        // slot of its first control volume
   uint32_t pslot;        // slot of the parent control volume of slot0, or kNoSlot
-  uint32_t cbeg;         // first entry of its child list
+  uint32_t cbeg;         // first entry of its child list; with kFBranchInlineFlag: child0 | child1 << 16
   uint16_t len;          // control volumes
-  uint16_t ccnt;         // child branches hanging off its last control volume
+  uint16_t ccnt;         // child branches hanging off its last control volume (| kFBranchInlineFlag)
 };
+constexpr uint32_t kFBranchInlineChildren = 2;
+constexpr uint16_t kFBranchInlineFlag = 0x8000u;   // (a branch has fewer than 32,768 children)
 
 // Byte offsets inside a forest's tree record (every section 16-byte aligned).
 struct FTopoOff { uint32_t offs, runs, chunks, chunk_cells, branches, br_cell, child, cell_det, level_br, total; };

@@ -449,9 +449,16 @@ struct UnitBuilder {
         }
         std::sort(kids[i].begin(), kids[i].end(), [&](uint32_t x, uint32_t y) { return lanes[x].first_cv > lanes[y].first_cv; });
         R.cbeg = cpos;
-        if (kids[i].size() > 65535) bad = true;
-        R.ccnt = (uint16_t)std::min<size_t>(kids[i].size(), 65535);
+        if (kids[i].size() > 32767) bad = true;          // (bit 15 of ccnt is kFBranchInlineFlag)
+        R.ccnt = (uint16_t)std::min<size_t>(kids[i].size(), 32767);
         for (uint32_t k : kids[i]) child[cpos++] = tl_of[k];
+        // up to two children travel in the record itself (forest_layout.h): one dependent load less per branch end
+        if (kids[i].size() <= kFBranchInlineChildren && n_lane <= 0xFFFFu) {
+          uint32_t packed = 0;
+          for (size_t k = 0; k < kids[i].size(); ++k) packed |= tl_of[kids[i][k]] << (16 * k);
+          R.cbeg = packed;
+          R.ccnt |= kFBranchInlineFlag;
+        }
       }
       for (uint32_t lc = 0; lc < n_cell; ++lc) {
         const int64_t orig = H.cell_order[cell_begin + lc];
